@@ -1,0 +1,292 @@
+"""CPU ORACLE for the HDC hot path of arxiv/paper_2606_26547 (ApproxHDC) -- TEST INFRASTRUCTURE.
+
+Only `tests/`, `__graft_entry__.smoke()` and `bench.py`'s cpu_baseline / `--impl reference`
+legs may import this module.  It shares no code with `paper_2606_26547_b200/` (the CUDA path)
+and imports nothing from it.  It is a plain, slow restatement, in numpy float64 / exact
+integers, of what the paper defines; every function cites the PAPER.md passage (Lnn) it
+follows and, where the paper is silent, the DESIGN.md reading (A1..A15, S0..S10) it adopts.
+There is no blocking, fusion or reordering: each function is the definition written out, with
+a library routine (float64 matmul, sum, argmax, packbits) as a step.
+
+Pins (tests/test_oracle_*.py, `-m "not gpu"`): brute-force python loops on tiny inputs, the
+bipolar identity dot = D_eff - 2*Hamming, near-orthogonality |cos| <~ 3/sqrt(D), the
+angle/Hamming closed form for Gaussian projections, majority-bundling recovery probability
+1/2 + C(F-1,(F-1)/2)/2^F, D_eff slice-equivalence and Listing 1's "first 1024 of 2048",
+bf16 RNE against ml_dtypes, perceptron invariants (sum_k Delta = 0; B=1 == textbook online
+perceptron).  Unpinned: accuracy parity with the paper's ISOLET numbers (datasets absent) --
+"parity unpinned" for that one item only.
+
+Conventions (S0; paper silent, readings A1-A3): bipolar v in {+1,-1}; bit b = [v == -1], so
+XOR of bits == product of bipolars; sgn(a) = -1 iff a < 0 (0 -> +1, bit 0); packed element d
+sits in uint32 word d>>5 at bit d&31 (LSB first), tail bits zero; arg-extremum ties -> lowest
+index.
+"""
+from __future__ import annotations
+
+import numpy as np
+
+# precision / hv_bits / sim codes mirror include/hdc.h numerically but are typed here by hand
+F32, BF16, I8, B1 = 0, 1, 2, 3
+SIM_DOT, SIM_COS, SIM_HAMMING = 0, 1, 2
+
+
+# ------------------------------------------------------------------------------------- S0
+def unpack_bits(words: np.ndarray, D: int) -> np.ndarray:
+    """[R][>=ceil(D/32)] uint32 -> [R][D] uint8 bits, LSB-first (S0 / A2)."""
+    w = np.ascontiguousarray(words, dtype="<u4")
+    by = w.view(np.uint8).reshape(w.shape[0], -1)
+    return np.unpackbits(by, axis=1, bitorder="little")[:, :D].copy()
+
+
+def pack_bits(bits: np.ndarray) -> np.ndarray:
+    """[R][D] bits -> [R][ceil(D/32)] uint32, LSB-first, tail bits zero (S0 / A2)."""
+    bits = np.ascontiguousarray(bits, dtype=np.uint8)
+    R, D = bits.shape
+    W = (D + 31) // 32
+    pad = np.zeros((R, W * 32), dtype=np.uint8)
+    pad[:, :D] = bits
+    return np.packbits(pad, axis=1, bitorder="little").view("<u4").reshape(R, W).copy()
+
+
+def bipolar(bits: np.ndarray) -> np.ndarray:
+    """bit -> +1/-1 as float64 (bit 1 <=> -1, A2)."""
+    return 1.0 - 2.0 * bits.astype(np.float64)
+
+
+# ------------------------------------------------------------------------------------- S1
+def round_bf16(x: np.ndarray) -> np.ndarray:
+    """fp32 -> nearest bfloat16 (ties to even), returned as float32 holding that value.
+    PAPER.md L165 ("element type representation"); RNE is reading A7.  Finite inputs only."""
+    u = np.ascontiguousarray(x, dtype=np.float32).view(np.uint32).astype(np.uint64)
+    r = (u + 0x7FFF + ((u >> 16) & 1)) & 0xFFFF0000
+    return r.astype(np.uint32).view(np.float32).reshape(np.shape(x))
+
+
+def quantize_int8_rows(x: np.ndarray) -> np.ndarray:
+    """Per-row symmetric int8 (reading A7; "projecting ... onto lower-precision
+    integer types"): a = max_f |x|, s = fl32(127/a) (s = 1 if a == 0),
+    q = clamp(rint(fl32(x*s)), -127, 127).  Every step is one correctly rounded fp32 op."""
+    x = np.ascontiguousarray(x, dtype=np.float32)
+    a = np.max(np.abs(x), axis=1, keepdims=True).astype(np.float32)
+    s = np.where(a > 0, np.float32(127.0) / np.where(a > 0, a, np.float32(1)), np.float32(1.0))
+    s = s.astype(np.float32)
+    q = np.rint((x * s).astype(np.float32))
+    return np.clip(q, -127, 127).astype(np.int32)
+
+
+def quantize_int8_tensor(c: np.ndarray) -> np.ndarray:
+    """Per-tensor symmetric int8 over the given array (S5 / A7): s = fl32(127/max|c|)."""
+    c = np.ascontiguousarray(c, dtype=np.float32)
+    a = np.float32(np.max(np.abs(c))) if c.size else np.float32(0)
+    s = np.float32(127.0) / a if a > 0 else np.float32(1.0)
+    q = np.rint((c * np.float32(s)).astype(np.float32))
+    return np.clip(q, -127, 127).astype(np.int32)
+
+
+def rp_operands(X: np.ndarray, P: np.ndarray, precision: int):
+    """Operands of the random-projection contraction at `precision` (S1): FP32 identity;
+    BF16 RNE of both; INT8 per-row of X and per-row (per projection d) of P.  B1 means packed
+    hypervectors with the real-valued contraction done in bf16 (reading A6)."""
+    if precision == F32:
+        return X.astype(np.float64), P.astype(np.float64)
+    if precision in (BF16, B1):
+        return round_bf16(X).astype(np.float64), round_bf16(P).astype(np.float64)
+    if precision == I8:
+        return quantize_int8_rows(X).astype(np.float64), quantize_int8_rows(P).astype(np.float64)
+    raise ValueError("precision")
+
+
+def encode_rp(X: np.ndarray, P: np.ndarray, D_eff: int, precision: int = F32,
+              want_absum: bool = False):
+    """Random-projection encode + sign (Listing 1 L68-L70 `__hetero_hdc_matmul`,
+    L155 "matrix-vector dot-product", L161 "{+1,-1} representation"; always binarised: A5).
+
+        acc[n,d] = sum_{f<F} x~[n,f] * p~[d,f]      (P is [D][F]: `hypermatrix<2048,617>`, L65)
+        bit[n,d] = [acc[n,d] < 0]  for d < D_eff     (sgn(0) = +1, A1)
+
+    The F reduction is never perforated (L157, L187).  float64 accumulation; for INT8 the
+    operands are integers <= 127 so every product and sum is exact in float64.
+    Returns bits [N][D_eff] uint8, acc [N][D_eff] float64 and optionally
+    absum[n,d] = sum_f |x~ p~| (used by the sign-agreement band, S4)."""
+    Xo, Po = rp_operands(np.asarray(X), np.asarray(P)[:D_eff], precision)
+    acc = Xo @ Po.T
+    bits = (acc < 0).astype(np.uint8)
+    absum = (np.abs(Xo) @ np.abs(Po).T) if want_absum else None
+    return bits, acc, absum
+
+
+# ------------------------------------------------------------------------------------- S2
+def encode_levelid(levels: np.ndarray, ID: np.ndarray, LV: np.ndarray, D_eff: int) -> np.ndarray:
+    """Level-ID ("ID-based", record) encoding ("ID-based encoding [12]", L183
+    N_LEVELS, L239 "Level-ID encoding"; bind = XOR, bundle = majority: BASELINE north_star).
+
+        cnt[n,d] = sum_{f<F} ( ID[f,d] XOR LV[levels[n,f], d] )
+        bit[n,d] = [ 2*cnt[n,d] > F ]          (tie, F even -> bit 0 <=> bipolar sum 0 -> +1: A3)
+
+    levels [N][F] integer level indices < Q; ID [F][D], LV [Q][D] are 0/1 arrays."""
+    levels = np.asarray(levels)
+    ID = np.asarray(ID, dtype=np.uint8)[:, :D_eff]
+    LV = np.asarray(LV, dtype=np.uint8)[:, :D_eff]
+    N, F = levels.shape
+    out = np.empty((N, D_eff), dtype=np.uint8)
+    for n in range(N):
+        bound = ID ^ LV[levels[n].astype(np.int64)]           # [F][D_eff]
+        cnt = bound.sum(axis=0, dtype=np.int64)
+        out[n] = (2 * cnt > F)
+    return out
+
+
+# ------------------------------------------------------------------------------------- S5
+def class_operand(C_acc: np.ndarray, D_eff: int, hv_bits: int) -> np.ndarray:
+    """Class operand derived from the fp32 accumulators at the hypervector element width
+    (training in high precision, inference "projecting class ... hypervectors
+    onto lower-precision integer types"; S5): 32 -> C_acc; 16 -> bf16 RNE; 8 -> per-tensor
+    symmetric int8 over k<K, d<D_eff; 1 -> bit [C_acc < 0].  Returned as float64 values
+    (bits as uint8)."""
+    c = np.asarray(C_acc, dtype=np.float32)[:, :D_eff]
+    if hv_bits == 32:
+        return c.astype(np.float64)
+    if hv_bits == 16:
+        return round_bf16(c).astype(np.float64)
+    if hv_bits == 8:
+        return quantize_int8_tensor(c).astype(np.float64)
+    if hv_bits == 1:
+        return (c < 0).astype(np.uint8)
+    raise ValueError("hv_bits")
+
+
+# ------------------------------------------------------------------------------------- S6
+def hamming(hbits: np.ndarray, cbits: np.ndarray, D_eff: int) -> np.ndarray:
+    """dist[n,k] = sum_{d<D_eff} [h[n,d] != c[k,d]]  (Listing 1 L72-L74
+    `__hetero_hdc_hamming_distance`, L161 xor+popcount; prefix reduction-perforation L61,
+    L76-L77, result used as-is L155)."""
+    h = np.asarray(hbits, dtype=np.uint8)[:, :D_eff]
+    c = np.asarray(cbits, dtype=np.uint8)[:, :D_eff]
+    out = np.empty((h.shape[0], c.shape[0]), dtype=np.int64)
+    for k in range(c.shape[0]):
+        out[:, k] = (h ^ c[k][None, :]).sum(axis=1, dtype=np.int64)
+    return out
+
+
+def dot(hbits: np.ndarray, cop: np.ndarray, D_eff: int) -> np.ndarray:
+    """s[n,k] = sum_{d<D_eff} v[n,d]*c[k,d], v bipolar (PAPER.md L197/L229 dot-product
+    similarity; L155 perforated similarity "used as-is": no rescale, A11).  float64; exact
+    for integer operands."""
+    v = bipolar(np.asarray(hbits)[:, :D_eff])
+    return v @ np.asarray(cop, dtype=np.float64)[:, :D_eff].T
+
+
+def cosine(hbits: np.ndarray, cop: np.ndarray, D_eff: int) -> np.ndarray:
+    """s[n,k] = dot[n,k] / ( sqrt(D_eff) * sqrt(sum_{d<D_eff} c[k,d]^2) ), 0 where the class
+    norm is 0 ("cosine similarity", L110 `__hetero_hdc_cos_sim`; A8).  The query
+    norm of a bipolar vector restricted to D_eff dims is sqrt(D_eff)."""
+    c = np.asarray(cop, dtype=np.float64)[:, :D_eff]
+    s = dot(hbits, c, D_eff)
+    nrm = np.sqrt((c * c).sum(axis=1))
+    out = np.zeros_like(s)
+    nz = nrm > 0
+    out[:, nz] = s[:, nz] / (np.sqrt(float(D_eff)) * nrm[nz])[None, :]
+    return out
+
+
+def similarity(hbits: np.ndarray, C_acc: np.ndarray, D_eff: int, sim: int, hv_bits: int):
+    """Scores of every query against every class at the given knobs (S5 + S6)."""
+    cop = class_operand(C_acc, D_eff, hv_bits)
+    if sim == SIM_HAMMING:
+        if hv_bits != 1:
+            raise ValueError("Hamming needs hv_bits=1")
+        return hamming(hbits, cop, D_eff)
+    if hv_bits == 1:
+        cop = bipolar(cop)
+    if sim == SIM_DOT:
+        return dot(hbits, cop, D_eff)
+    if sim == SIM_COS:
+        return cosine(hbits, cop, D_eff)
+    raise ValueError("sim")
+
+
+# ------------------------------------------------------------------------------------- S7
+def classify(S: np.ndarray, sim: int):
+    """Label = arg-max of DOT/COS scores, arg-min of Hamming distances (Listing 1
+    L79-L80 `__hetero_hdc_arg_min` "select nearest cluster"); ties -> lowest index (A14).
+    Also returns best and runner-up values (runner-up = best of the rest; = best on a tie;
+    = best when K == 1)."""
+    S = np.asarray(S)
+    key = -S if sim == SIM_HAMMING else S
+    lab = np.argmax(key, axis=1).astype(np.int32)            # first occurrence = lowest index
+    n = np.arange(S.shape[0])
+    best = S[n, lab]
+    if S.shape[1] == 1:
+        return lab, best, best.copy()
+    rest = np.array(key, dtype=np.float64, copy=True)
+    rest[n, lab] = -np.inf
+    second = S[n, np.argmax(rest, axis=1)]
+    return lab, best, second
+
+
+# ------------------------------------------------------------------------------------- S8
+def bundle(hbits: np.ndarray, y: np.ndarray, K: int, D_eff: int, C_acc: np.ndarray | None = None):
+    """One-pass training: C_acc[k,d] += sum_{n: y_n = k} v[n,d]  ("hypervectors
+    corresponding to inputs from the same class are combined ... vector addition").  fp32
+    accumulators (A10) hold these integers exactly (|.| < 2^24)."""
+    v = bipolar(np.asarray(hbits)[:, :D_eff])
+    out = np.zeros((K, D_eff), dtype=np.float64) if C_acc is None else \
+        np.array(C_acc, dtype=np.float64)[:, :D_eff].copy()
+    for k in range(K):
+        out[k] += v[np.asarray(y) == k].sum(axis=0)
+    return out.astype(np.float32)
+
+
+# ------------------------------------------------------------------------------------- S9
+def train_epoch(hbits: np.ndarray, y: np.ndarray, C_acc: np.ndarray, D_eff: int, hv_bits: int,
+                sim: int, lr: float, batch: int = 0):
+    """One retraining epoch (PAPER.md L181 TRAIN_ITERATIONS "number of retraining epochs";
+    the per-sample rule is not in the paper -- reading A9 / S9, "perceptron-style" per
+    BASELINE north_star).  Samples in index order, no shuffle; per mini-batch of B samples:
+      (i)   class operands from the current C_acc (S5);
+      (ii)  yhat_n = classify(h_n) with the inference similarity;
+      (iii) Delta[k,d] = sum_{n in batch, yhat_n != y_n} ([k=y_n] - [k=yhat_n]) * v[n,d]  (integer);
+      (iv)  C_acc[k,d] = fl32( C_acc[k,d] + fl32( lr * (float)Delta[k,d] ) )   two rounded ops.
+    Returns (C_acc' fp32 [K][D_eff], number of mispredictions, predictions int32 [N])."""
+    hb = np.asarray(hbits, dtype=np.uint8)[:, :D_eff]
+    y = np.asarray(y)
+    C = np.array(C_acc, dtype=np.float32)[:, :D_eff].copy()
+    K = C.shape[0]
+    N = hb.shape[0]
+    B = N if batch in (0, None) or batch > N else int(batch)
+    lr32 = np.float32(lr)
+    pred = np.empty(N, dtype=np.int32)
+    wrong = 0
+    for b0 in range(0, N, B):
+        sl = slice(b0, min(N, b0 + B))
+        S = similarity(hb[sl], C, D_eff, sim, hv_bits)
+        yh, _, _ = classify(S, sim)
+        pred[sl] = yh
+        v = bipolar(hb[sl])
+        delta = np.zeros((K, D_eff), dtype=np.int64)
+        for i in np.nonzero(yh != y[sl])[0]:
+            vi = v[i].astype(np.int64)
+            delta[y[sl][i]] += vi
+            delta[yh[i]] -= vi
+            wrong += 1
+        step = (lr32 * delta.astype(np.float32)).astype(np.float32)
+        C = (C + step).astype(np.float32)
+    return C, wrong, pred
+
+
+# ------------------------------------------------------------------------------------- S10
+def train(hbits, y, K, D_eff, hv_bits, sim, epochs, lr, batch=0):
+    """Bundle then `epochs` retraining epochs (S10); "skipped retraining iterations" = fewer
+    epochs (10 -> 3)."""
+    C = bundle(hbits, y, K, D_eff)
+    hist = []
+    for _ in range(int(epochs)):
+        C, wrong, _ = train_epoch(hbits, y, C, D_eff, hv_bits, sim, lr, batch)
+        hist.append(wrong)
+    return C, hist
+
+
+def infer(hbits, C_acc, D_eff, sim, hv_bits):
+    """similarity + arg-extremum (Listing 1 L72-L80)."""
+    S = similarity(hbits, C_acc, D_eff, sim, hv_bits)
+    return classify(S, sim) + (S,)

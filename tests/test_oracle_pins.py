@@ -1,0 +1,446 @@
+"""Pins for the CPU oracle (`oracle/hdc_oracle.py`) against things other than itself:
+brute-force python loops on tiny inputs, closed forms, invariants, library routines
+(ml_dtypes bfloat16), and the one value the paper prints (tests/golden/).  CPU only."""
+import math
+import os
+
+import ml_dtypes
+import numpy as np
+import pytest
+
+import workloads as wl
+from oracle import hdc_oracle as o
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+rng = lambda s: np.random.default_rng(s)      # noqa: E731
+
+
+# ------------------------------------------------------------------ S0 layout
+def test_pack_layout_by_hand():
+    bits = np.zeros((1, 70), dtype=np.uint8)
+    bits[0, [0, 5, 31, 33, 69]] = 1
+    w = o.pack_bits(bits)
+    assert w.shape == (1, 3)
+    assert int(w[0, 0]) == (1 << 0) | (1 << 5) | (1 << 31)
+    assert int(w[0, 1]) == (1 << 1)
+    assert int(w[0, 2]) == (1 << 5)           # bit 69 = word 2, bit 5; bits 70..95 zero
+    assert np.array_equal(o.unpack_bits(w, 70), bits)
+    # the generator's packer (a separate implementation) uses the same layout
+    assert np.array_equal(wl.pack_bits_lsb(bits), w)
+
+
+@pytest.mark.parametrize("D", [1, 31, 32, 33, 64, 100, 313 * 32 - 16])
+def test_pack_roundtrip(D):
+    b = rng(D).integers(0, 2, size=(5, D), dtype=np.uint8)
+    w = o.pack_bits(b)
+    assert w.shape[1] == (D + 31) // 32
+    assert np.array_equal(o.unpack_bits(w, D), b)
+    if D % 32:
+        assert (w[:, -1] >> (D % 32) == 0).all()          # tail bits zero
+
+
+# ------------------------------------------------------------------ S1 precision conversions
+def test_bf16_rne_against_ml_dtypes():
+    r = rng(1)
+    x = np.concatenate([r.standard_normal(20000) * 10.0 ** r.integers(-20, 20, 20000),
+                        [0.0, -0.0, 1.0, 1.0 + 2.0 ** -8, 1.0 + 3 * 2.0 ** -8, 1.0 + 2.0 ** -7,
+                         -(1.0 + 2.0 ** -8), 3.3895314e38 * 0.5, 1e-40]]).astype(np.float32)
+    want = x.astype(ml_dtypes.bfloat16).astype(np.float32)
+    got = o.round_bf16(x)
+    assert np.array_equal(got.view(np.uint32), want.view(np.uint32))
+    # ties to even, by hand: 1+2^-8 is halfway between 1 and 1+2^-7 -> 1 (even mantissa)
+    assert o.round_bf16(np.float32(1.0 + 2.0 ** -8)) == np.float32(1.0)
+    assert o.round_bf16(np.float32(1.0 + 3 * 2.0 ** -8)) == np.float32(1.0 + 2.0 ** -6)
+
+
+def test_int8_rows_fixed_points():
+    q = np.array([[127, -127, 0, 5, -64], [0, 0, 0, 0, 0], [1, 2, 127, -3, 4]], dtype=np.float32)
+    assert np.array_equal(o.quantize_int8_rows(q), q.astype(np.int32))   # max 127 -> identity
+    x = np.array([[0.5, -1.0, 0.25, 1.0 / 127]], dtype=np.float32)
+    assert np.array_equal(o.quantize_int8_rows(x), [[64, -127, 32, 1]])  # 63.5 -> 64 (RNE), 31.75 -> 32
+    assert np.abs(o.quantize_int8_rows(rng(2).standard_normal((7, 33)).astype(np.float32))).max() == 127
+    # per-tensor variant: the single max maps to 127
+    c = rng(3).standard_normal((4, 9)).astype(np.float32)
+    qt = o.quantize_int8_tensor(c)
+    assert np.abs(qt).max() == 127 and (np.abs(qt) == 127).sum() == 1
+    assert np.array_equal(o.quantize_int8_tensor(np.zeros((2, 3), np.float32)), np.zeros((2, 3)))
+
+
+# ------------------------------------------------------------------ S1 random projection
+def _brute_encode(X, P, D_eff):
+    N, F = X.shape
+    out = np.zeros((N, D_eff), dtype=np.uint8)
+    for n in range(N):
+        for d in range(D_eff):
+            s = 0.0
+            for f in range(F):
+                s += float(X[n, f]) * float(P[d, f])
+            out[n, d] = 1 if s < 0 else 0
+    return out
+
+
+@pytest.mark.parametrize("N,F,D,D_eff", [(3, 5, 40, 40), (8, 16, 64, 33), (2, 1, 7, 7), (4, 17, 130, 31)])
+def test_encode_rp_brute_force(N, F, D, D_eff):
+    r = rng(N * 1000 + F)
+    X = r.standard_normal((N, F)).astype(np.float32)
+    P = r.standard_normal((D, F)).astype(np.float32)
+    bits, acc, absum = o.encode_rp(X, P, D_eff, o.F32, want_absum=True)
+    assert bits.shape == (N, D_eff)
+    assert np.array_equal(bits, _brute_encode(X, P, D_eff))
+    assert (absum >= np.abs(acc) - 1e-12).all()
+
+
+def test_encode_rp_transposed_operand_would_fail():
+    # P is [D][F] (Listing 1: hypermatrix<2048,617>): row d is projection d.
+    X = np.array([[1.0, 0.0]], dtype=np.float32)
+    P = np.array([[1.0, -5.0], [-1.0, 5.0], [-2.0, 1.0]], dtype=np.float32)     # D=3, F=2
+    bits, acc, _ = o.encode_rp(X, P, 3)
+    assert np.array_equal(acc, [[1.0, -1.0, -2.0]])
+    assert np.array_equal(bits, [[0, 1, 1]])
+
+
+def test_encode_rp_f1_scale_invariance_and_sign_zero():
+    r = rng(7)
+    X = r.standard_normal((6, 1)).astype(np.float32)
+    P = r.standard_normal((50, 1)).astype(np.float32)
+    bits, _, _ = o.encode_rp(X, P, 50)
+    assert np.array_equal(bits, ((X * P.T) < 0).astype(np.uint8))               # F=1: sgn(x*p)
+    X = r.standard_normal((5, 9)).astype(np.float32)
+    P = r.standard_normal((64, 9)).astype(np.float32)
+    b1, _, _ = o.encode_rp(X, P, 64)
+    b2, _, _ = o.encode_rp(np.float32(8.0) * X, P, 64)                          # alpha > 0 (exact *8)
+    assert np.array_equal(b1, b2)
+    # sgn(0) = +1 -> bit 0 (A1); sgn(-0.0) too
+    Xz = np.array([[1.0, 1.0], [0.0, -0.0]], dtype=np.float32)
+    Pz = np.array([[1.0, -1.0], [1.0, 1.0], [-1.0, -1.0]], dtype=np.float32)
+    bz, az, _ = o.encode_rp(Xz, Pz, 3)
+    assert np.array_equal(az[0], [0.0, 2.0, -2.0]) and np.array_equal(bz, [[0, 0, 1], [0, 0, 0]])
+
+
+def test_encode_rp_integer_inputs_exact_all_precisions():
+    r = rng(11)
+    X = r.integers(0, 128, size=(9, 23)).astype(np.float32)
+    X[:, 0] = 127                                           # row max 127 -> int8 quantisation is identity
+    P = (1 - 2 * r.integers(0, 2, size=(77, 23))).astype(np.float32) * 127
+    want = (X.astype(np.int64) @ P.astype(np.int64).T)
+    for prec in (o.F32, o.I8):
+        bits, acc, _ = o.encode_rp(X, P, 77, prec)
+        assert np.array_equal(acc, want) and np.array_equal(bits, (want < 0))
+    Xs = r.integers(0, 256, size=(9, 23)).astype(np.float32)        # 8-bit ints are exact in bf16
+    Ps = (1 - 2 * r.integers(0, 2, size=(77, 23))).astype(np.float32)
+    wants = Xs.astype(np.int64) @ Ps.astype(np.int64).T
+    for prec in (o.F32, o.BF16, o.B1):
+        bits, acc, _ = o.encode_rp(Xs, Ps, 77, prec)
+        assert np.array_equal(acc, wants) and np.array_equal(bits, (wants < 0))
+
+
+def test_encode_rp_angle_closed_form():
+    """Gaussian P: P(sign bit differs) = theta(x,y)/pi per dimension (random hyperplane)."""
+    D, F = 20000, 24
+    r = rng(13)
+    P = r.standard_normal((D, F)).astype(np.float32)
+    x = r.standard_normal(F)
+    for theta in (0.2, 1.0, math.pi / 2, 2.5):
+        u = r.standard_normal(F)
+        u -= (u @ x) / (x @ x) * x
+        yv = math.cos(theta) * x / np.linalg.norm(x) + math.sin(theta) * u / np.linalg.norm(u)
+        bits, _, _ = o.encode_rp(np.stack([x, 3.0 * yv]).astype(np.float32), P, D)
+        frac = (bits[0] != bits[1]).mean()
+        p = theta / math.pi
+        assert abs(frac - p) <= 4.0 * math.sqrt(p * (1 - p) / D), (theta, frac, p)
+
+
+def test_near_orthogonality_of_random_hypervectors():
+    D = 10000
+    bits = rng(17).integers(0, 2, size=(40, D), dtype=np.uint8)
+    S = o.cosine(bits, o.bipolar(bits), D)
+    off = S[~np.eye(40, dtype=bool)]
+    assert np.allclose(np.diag(S), 1.0) and np.abs(off).max() < 4.5 / math.sqrt(D)
+    assert np.sqrt((off ** 2).mean()) < 1.3 / math.sqrt(D)      # sd of cos is 1/sqrt(D)
+    # encoded independent inputs are near-orthogonal too (north_star: |cos| <~ 3/sqrt(D))
+    r = rng(18)
+    hb, _, _ = o.encode_rp(r.standard_normal((12, 300)).astype(np.float32),
+                           r.standard_normal((D, 300)).astype(np.float32), D)
+    Sx = o.cosine(hb, o.bipolar(hb), D)
+    assert np.abs(Sx[~np.eye(12, dtype=bool)]).max() < 0.25    # inputs in R^300 are ~1/sqrt(300) apart
+
+
+# ------------------------------------------------------------------ S6 similarity
+@pytest.mark.parametrize("D_eff", [1, 31, 32, 33, 64, 100, 257])
+def test_bipolar_identity_dot_equals_D_minus_2_hamming(D_eff):
+    r = rng(D_eff)
+    h = r.integers(0, 2, size=(6, 257), dtype=np.uint8)
+    c = r.integers(0, 2, size=(5, 257), dtype=np.uint8)
+    ham = o.hamming(h, c, D_eff)
+    dt = o.dot(h, o.bipolar(c), D_eff)
+    assert np.array_equal(dt, D_eff - 2 * ham)
+    # brute force Hamming
+    for n in range(6):
+        for k in range(5):
+            assert ham[n, k] == sum(int(h[n, d] != c[k, d]) for d in range(D_eff))
+
+
+def test_cosine_against_textbook_formula_and_zero_norm():
+    r = rng(23)
+    h = r.integers(0, 2, size=(7, 90), dtype=np.uint8)
+    C = r.standard_normal((4, 90)).astype(np.float32)
+    C[2] = 0.0
+    S = o.cosine(h, C, 64)
+    v = 1.0 - 2.0 * h[:, :64].astype(np.float64)
+    for n in range(7):
+        for k in range(4):
+            c = C[k, :64].astype(np.float64)
+            want = 0.0 if k == 2 else float(v[n] @ c) / (np.linalg.norm(v[n]) * np.linalg.norm(c))
+            assert abs(S[n, k] - want) < 1e-14
+    assert np.allclose(o.cosine(h, o.bipolar(h), 90).diagonal(), 1.0)
+    assert np.allclose(o.cosine(h, -o.bipolar(h), 90).diagonal(), -1.0)
+
+
+def test_similarity_precisions_of_class_operand():
+    r = rng(29)
+    h = r.integers(0, 2, size=(5, 70), dtype=np.uint8)
+    C = (r.standard_normal((3, 70)) * 7).astype(np.float32)
+    v = o.bipolar(h)
+    assert np.allclose(o.similarity(h, C, 70, o.SIM_DOT, 32), v @ C.astype(np.float64).T)
+    cb = C.astype(ml_dtypes.bfloat16).astype(np.float64)
+    assert np.array_equal(o.similarity(h, C, 70, o.SIM_DOT, 16), v @ cb.T)
+    q = o.similarity(h, C, 70, o.SIM_DOT, 8)
+    assert np.array_equal(q, np.rint(q)) and np.abs(q).max() <= 127 * 70
+    # per-tensor scale over the D_eff prefix only (S5): the max inside the prefix maps to 127
+    C2 = C.copy(); C2[0, 69] = 1e6
+    assert np.abs(o.class_operand(C2, 64, 8)).max() == 127
+    # hv_bits=1: sign bits; Hamming and bipolar dot agree through the identity
+    ham = o.similarity(h, C, 70, o.SIM_HAMMING, 1)
+    assert np.array_equal(o.similarity(h, C, 70, o.SIM_DOT, 1), 70 - 2 * ham)
+    Cz = C.copy(); Cz[1, 3] = 0.0
+    assert o.class_operand(Cz, 70, 1)[1, 3] == 0                 # sgn(0)=+1 -> bit 0
+
+
+# ------------------------------------------------------------------ S7 classify
+def test_classify_ties_and_runner_up():
+    S = np.array([[1.0, 3.0, 3.0, 2.0], [5.0, 1.0, 0.0, 5.0], [-1.0, -2.0, -3.0, -4.0]])
+    lab, best, second = o.classify(S, o.SIM_COS)
+    assert lab.tolist() == [1, 0, 0] and best.tolist() == [3.0, 5.0, -1.0]
+    assert second.tolist() == [3.0, 5.0, -2.0]
+    Hd = np.array([[7, 2, 2, 9], [4, 4, 4, 4]])
+    lab, best, second = o.classify(Hd, o.SIM_HAMMING)
+    assert lab.tolist() == [1, 0] and best.tolist() == [2, 4] and second.tolist() == [2, 4]
+    lab, best, second = o.classify(np.array([[0.25], [-3.0]]), o.SIM_DOT)          # K = 1
+    assert lab.tolist() == [0, 0] and second.tolist() == best.tolist()
+
+
+# ------------------------------------------------------------------ S2 level-ID
+def _brute_levelid(levels, ID, LV, D_eff):
+    N, F = levels.shape
+    out = np.zeros((N, D_eff), dtype=np.uint8)
+    for n in range(N):
+        for d in range(D_eff):
+            cnt = 0
+            for f in range(F):
+                cnt += int(ID[f, d]) ^ int(LV[levels[n, f], d])
+            out[n, d] = 1 if 2 * cnt > F else 0
+    return out
+
+
+@pytest.mark.parametrize("N,F,Q,D,D_eff", [(3, 7, 5, 40, 40), (4, 8, 4, 70, 33), (2, 1, 3, 35, 35), (5, 3, 2, 64, 64)])
+def test_levelid_brute_force(N, F, Q, D, D_eff):
+    r = rng(N + 10 * F + 100 * Q)
+    lv = r.integers(0, Q, size=(N, F)).astype(np.uint8)
+    ID = r.integers(0, 2, size=(F, D), dtype=np.uint8)
+    LV = r.integers(0, 2, size=(Q, D), dtype=np.uint8)
+    got = o.encode_levelid(lv, ID, LV, D_eff)
+    assert np.array_equal(got, _brute_levelid(lv, ID, LV, D_eff))
+    if F == 1:
+        assert np.array_equal(got, (ID[0] ^ LV[lv[:, 0]])[:, :D_eff])
+    if F == 3:
+        a, b, c = (ID[f] ^ LV[lv[:, f]] for f in range(3))
+        assert np.array_equal(got, ((a & b) | (a & c) | (b & c))[:, :D_eff])      # bitwise majority
+
+
+def test_levelid_even_F_tie_gives_bit0():
+    ID = np.array([[0, 1], [1, 1]], dtype=np.uint8)         # F=2, D=2
+    LV = np.array([[0, 0]], dtype=np.uint8)
+    got = o.encode_levelid(np.zeros((1, 2), np.uint8), ID, LV, 2)
+    assert got.tolist() == [[0, 1]]                          # d=0: cnt 1 of 2 -> tie -> 0; d=1: 2 of 2 -> 1
+
+
+@pytest.mark.parametrize("F", [9, 101])
+def test_majority_bundling_recovers_components_above_chance(F):
+    """For odd F and iid bound vectors, P(maj_d == component_f,d) = 1/2 + C(F-1,(F-1)/2)/2^F."""
+    D = 20000
+    r = rng(F)
+    ID = r.integers(0, 2, size=(F, D), dtype=np.uint8)
+    LV = r.integers(0, 2, size=(8, D), dtype=np.uint8)
+    lv = r.integers(0, 8, size=(6, F)).astype(np.uint8)
+    hb = o.encode_levelid(lv, ID, LV, D)
+    p = 0.5 + math.comb(F - 1, (F - 1) // 2) / 2.0 ** F
+    agree = np.mean([(hb[n] == (ID[f] ^ LV[lv[n, f]])).mean() for n in range(6) for f in range(F)])
+    sd = math.sqrt(p * (1 - p) / (D * 6 * F))
+    assert abs(agree - p) < 6 * sd + 1e-4, (agree, p)
+    assert {9: 0.6367, 101: 0.5398}[F] == round(p, 4)
+
+
+def test_level_table_hamming_closed_form():
+    Q, D = 17, 1000
+    LV = wl.level_table(99, Q, D)
+    m = [(q * (D // 2)) // (Q - 1) for q in range(Q)]
+    for a in range(Q):
+        for b in range(Q):
+            assert int((LV[a] != LV[b]).sum()) == abs(m[a] - m[b])
+    assert int((LV[0] != LV[Q - 1]).sum()) == D // 2
+
+
+# ------------------------------------------------------------------ S3 D_eff
+def test_listing1_first_1024_of_2048_golden():
+    rows = [l.split() for l in open(os.path.join(HERE, "golden", "listing1_redperf.txt"))
+            if l.strip() and not l.startswith("#")]
+    D, start, end, stride, D_eff, first, last = rows[0]
+    D, D_eff = int(D), int(D_eff)
+    assert int(math.floor(float(end) * D)) == D_eff and float(start) == 0.0 and int(stride) == 1
+    # Listing 1 shapes: F=617, D=2048, K=26
+    r = rng(2048)
+    h = r.integers(0, 2, size=(3, D), dtype=np.uint8)
+    c = r.integers(0, 2, size=(26, D), dtype=np.uint8)
+    want = (h[:, None, int(first):int(last) + 1] != c[None, :, int(first):int(last) + 1]).sum(axis=2)
+    assert np.array_equal(o.hamming(h, c, D_eff), want)
+
+
+@pytest.mark.parametrize("D_eff", [1, 31, 32, 33, 100, 200])
+def test_d_eff_slice_equivalence(D_eff):
+    r = rng(300 + D_eff)
+    D, F, K, N = 200, 11, 4, 24
+    X = r.standard_normal((N, F)).astype(np.float32)
+    P = r.standard_normal((D, F)).astype(np.float32)
+    y = r.integers(0, K, size=N)
+    for prec, hvb, sim in ((o.F32, 32, o.SIM_COS), (o.BF16, 16, o.SIM_DOT), (o.I8, 8, o.SIM_COS), (o.B1, 1, o.SIM_HAMMING)):
+        hb_full, _, _ = o.encode_rp(X, P, D, prec)
+        hb, _, _ = o.encode_rp(X, P, D_eff, prec)
+        hb_sl, _, _ = o.encode_rp(X, P[:D_eff], D_eff, prec)
+        assert np.array_equal(hb, hb_sl) and np.array_equal(hb, hb_full[:, :D_eff])
+        C_full = o.bundle(hb_full, y, K, D)
+        C = o.bundle(hb_full, y, K, D_eff)
+        assert np.array_equal(C, C_full[:, :D_eff])
+        S = o.similarity(hb_full, C_full, D_eff, sim, hvb)
+        S_sl = o.similarity(hb_full[:, :D_eff].copy(), C_full[:, :D_eff].copy(), D_eff, sim, hvb)
+        assert np.array_equal(S, S_sl)
+        C1, w1, p1 = o.train_epoch(hb_full, y, C_full, D_eff, hvb, sim, 0.25, 5)
+        C2, w2, p2 = o.train_epoch(hb_sl, y, C_full[:, :D_eff].copy(), D_eff, hvb, sim, 0.25, 5)
+        assert np.array_equal(C1, C2) and w1 == w2 and np.array_equal(p1, p2)
+
+
+# ------------------------------------------------------------------ S8 bundle
+def test_bundle_sums_and_counts():
+    r = rng(41)
+    hb = r.integers(0, 2, size=(50, 77), dtype=np.uint8)
+    y = r.integers(0, 5, size=50)
+    C = o.bundle(hb, y, 5, 77)
+    assert C.dtype == np.float32
+    v = 1 - 2 * hb.astype(np.int64)
+    assert np.array_equal(C.sum(axis=0), v.sum(axis=0))
+    for k in range(5):
+        want = np.zeros(77, dtype=np.int64)
+        for n in range(50):
+            if y[n] == k:
+                want += v[n]
+        assert np.array_equal(C[k], want)
+        assert np.abs(C[k]).max() <= (y == k).sum()
+    C2 = o.bundle(hb, y, 5, 77, C_acc=C)
+    assert np.array_equal(C2, 2 * C)
+
+
+# ------------------------------------------------------------------ S9 retraining
+def _textbook_online_perceptron(hb, y, C, lr):
+    """Separate 10-line statement of the B=1 rule: on a mistake add lr*h to the true class and
+    subtract it from the predicted one (dot similarity, fp32 class vectors)."""
+    C = C.astype(np.float32).copy()
+    wrong = 0
+    for n in range(hb.shape[0]):
+        h = (1.0 - 2.0 * hb[n]).astype(np.float32)
+        scores = [float(np.dot(h.astype(np.float64), C[k].astype(np.float64))) for k in range(C.shape[0])]
+        yh = int(np.argmax(scores))
+        if yh != y[n]:
+            wrong += 1
+            C[y[n]] = C[y[n]] + np.float32(lr) * h
+            C[yh] = C[yh] - np.float32(lr) * h
+    return C, wrong
+
+
+def test_train_epoch_b1_is_online_perceptron():
+    r = rng(43)
+    hb = r.integers(0, 2, size=(60, 96), dtype=np.uint8)
+    y = r.integers(0, 4, size=60)
+    C0 = o.bundle(hb[:8], y[:8], 4, 96)
+    for lr in (1.0, 0.05):
+        C1, w1, _ = o.train_epoch(hb, y, C0, 96, 32, o.SIM_DOT, lr, batch=1)
+        C2, w2 = _textbook_online_perceptron(hb, y, C0, lr)
+        assert w1 == w2 and w1 > 0 and np.array_equal(C1, C2)
+
+
+@pytest.mark.parametrize("B", [0, 1, 7, 64])
+def test_train_epoch_invariants(B):
+    r = rng(47 + B)
+    hb = r.integers(0, 2, size=(90, 130), dtype=np.uint8)
+    y = r.integers(0, 5, size=90)
+    C = o.bundle(hb, y, 5, 130)
+    col = C.astype(np.float64).sum(axis=0)
+    for _ in range(3):                                   # sum_k Delta[k,d] = 0: column sums conserved (lr = 2^-2 exact)
+        C, wrong, pred = o.train_epoch(hb, y, C, 130, 32, o.SIM_COS, 0.25, B)
+        assert np.array_equal(C.astype(np.float64).sum(axis=0), col)
+        assert 0 <= wrong <= 90 and pred.shape == (90,)
+    if B == 0:                                           # epoch-synchronous: mistakes counted against the epoch-start model
+        assert wrong == int((pred != y).sum())
+
+
+def test_train_separable_converges_and_fixed_point():
+    r = rng(53)
+    K, D, per = 3, 512, 20
+    protos = r.integers(0, 2, size=(K, D), dtype=np.uint8)
+    y = np.repeat(np.arange(K), per)
+    hb = protos[y] ^ (r.random((K * per, D)) < 0.15).astype(np.uint8)
+    C = o.bundle(hb[::7], y[::7], K, D)
+    hist = []
+    for _ in range(6):
+        C, wrong, _ = o.train_epoch(hb, y, C, D, 32, o.SIM_COS, 1.0, 0)
+        hist.append(wrong)
+    assert hist[-1] == 0 and hist[-2] == 0
+    C2, wrong, _ = o.train_epoch(hb, y, C, D, 32, o.SIM_COS, 1.0, 0)
+    assert wrong == 0 and np.array_equal(C2, C)           # zero mispredicts => unchanged
+
+
+def test_train_update_two_rounded_fp32_ops():
+    # one sample, one mistake: C_acc' = fl32(C + fl32(lr*delta)); check against python floats
+    hb = np.array([[0, 1, 0]], dtype=np.uint8)
+    C = np.array([[0.1, 0.2, 0.3], [5.0, -5.0, 5.0]], dtype=np.float32)   # class 1 wins: h=(+1,-1,+1)
+    Cn, wrong, pred = o.train_epoch(hb, np.array([0]), C, 3, 32, o.SIM_DOT, 0.05, 0)
+    assert wrong == 1 and pred.tolist() == [1]
+    lr = np.float32(0.05)
+    for d, v in enumerate([1.0, -1.0, 1.0]):
+        assert Cn[0, d] == np.float32(C[0, d] + np.float32(lr * np.float32(v)))
+        assert Cn[1, d] == np.float32(C[1, d] + np.float32(lr * np.float32(-v)))
+
+
+# ------------------------------------------------------------------ end-to-end sanity (not parity)
+def test_pipeline_sanity_c1():
+    c = wl.c1_tiny()
+    hb, _, _ = o.encode_rp(c["Xtr"], c["P"], c["D"], o.F32)
+    C = o.bundle(hb, c["ytr"], c["K"], c["D"])
+    ht, _, _ = o.encode_rp(c["Xte"], c["P"], c["D"], o.F32)
+    lab, best, second, S = o.infer(ht, C, c["D"], o.SIM_HAMMING, 1)
+    assert (lab == c["yte"]).mean() > 0.9                   # far above 1/K = 0.25
+    lab512, _, _, _ = o.infer(ht, C, 512, o.SIM_HAMMING, 1)
+    assert (lab512 == c["yte"]).mean() > 0.8
+
+
+def test_generators_are_seeded_and_shaped():
+    a, b = wl.c2_isolet_shaped(D=64, n_tr=50, n_te=20), wl.c2_isolet_shaped(D=64, n_tr=50, n_te=20)
+    assert a["Xtr"].shape == (50, 617) and a["P"].shape == (64, 617) and a["K"] == 26
+    assert np.array_equal(a["Xtr"], b["Xtr"]) and np.array_equal(a["P"], b["P"])
+    full = wl.c2_isolet_shaped(D=128, n_tr=50, n_te=20)
+    assert np.array_equal(full["P"][:64], a["P"])            # prefix-stable in D (S3)
+    c3 = wl.c3_mnist_shaped(D=256, n_tr=400, n_te=50)
+    assert c3["Ltr"].dtype == np.uint8 and c3["Ltr"].shape == (400, 784)
+    assert 0.70 < (c3["Ltr"] == 0).mean() < 0.90             # ~80 % zeros
+    c5 = wl.c5_large_batch(64, D=128, K=10, n_unstructured=16, per_class=2)
+    assert c5["X"].shape == (80, 1024) and c5["P"].shape == (128, 1024)
+    assert np.array_equal(o.round_bf16(c5["X"]), c5["X"])     # bf16-representable
+    assert abs(float(c5["X"][:64].std()) - 1.0) < 0.05
