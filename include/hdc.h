@@ -1,0 +1,191 @@
+/* hdc.h -- C ABI of libhdc.so: the data-parallel HDC hot path of arxiv/paper_2606_26547
+ * (ApproxHDC) as hand-written CUDA for NVIDIA B200 (sm_100a).
+ *
+ * The path (section 2.1, Listing 1 L63-L81): (1) encode feature vectors into D-dimensional
+ * hypervectors, (2) similarity search against K class hypervectors, (3) arg-extremum and the
+ * perceptron-style class update.  The paper's approximation knobs (section 4.2: reduction perforation
+ * L155, binarization L161, encoding dimensionality L163, element type L165, algorithmic choice
+ * L167, retraining epochs L181) are RUNTIME arguments (`hdc_knobs_t`, the `epochs` loop is the
+ * caller's).
+ *
+ * General contract
+ *  - Every data pointer is a DEVICE pointer owned by the caller, unless the parameter name ends in
+ *    `_host` (then it is a host pointer, pinned for full speed).  Nothing is allocated or freed
+ *    inside a compute call; scratch comes from the caller's workspace `ws` (size from
+ *    hdc_workspace_bytes()).  `stream` is a cudaStream_t (NULL = legacy default stream).  Calls
+ *    enqueue work and return; they do not synchronise (the `_host` entry point does, it says so).
+ *  - Return value: HDC_OK (0) or a negative hdc_status.  Argument errors are detected on the host
+ *    BEFORE anything is enqueued.  A failed launch maps to HDC_ERR_CUDA; hdc_last_error() gives
+ *    the text.  Device faults are sticky CUDA errors seen at the caller's next synchronisation.
+ *  - Layouts are row-major with the reduction axis contiguous: X[N][ldx], P[D][ldp] (row d =
+ *    projection d, Listing 1 `hypermatrix<2048,617>` L65), C[K][ldc] (`hypermatrix<26,2048>`
+ *    L66).  `ld*` are in ELEMENTS (uint32 words for bit matrices).  Base pointers must be 16-byte
+ *    aligned and fp32/bf16 leading dimensions a multiple of 4 / 8 elements where stated.
+ *  - Packed hypervectors: bipolar value v in {+1,-1} is stored as bit b = [v == -1]; element d is
+ *    bit (d & 31) of uint32 word (d >> 5), LSB first.  Exactly W = ceil(D_eff/32) words are
+ *    written per row; bits >= D_eff of the last word are written as 0.  sgn(0) = +1 (bit 0).
+ *  - D_eff (1 <= D_eff <= D): every reduction over d and every output row is restricted to
+ *    d < D_eff and nothing is rescaled (L61 "only the first 1024 elements", L155 "used as-is").
+ *    Results equal those obtained by slicing every [.][D] array to its first D_eff columns.
+ *  - arg-max / arg-min ties go to the lowest class index.  Inputs must be finite.
+ *  - Outputs must not alias inputs (except C_acc, which is in/out).  A handle is not thread-safe;
+ *    distinct handles are independent.  There is no CPU fallback and no other architecture:
+ *    hdc_create() fails with HDC_ERR_ARCH unless the device is compute capability 10.x.
+ */
+#ifndef HDC_H_
+#define HDC_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct hdc_ctx* hdc_handle_t;
+
+typedef enum {
+  HDC_OK = 0,
+  HDC_ERR_INVALID_ARG = -1, /* null pointer, size <= 0, D_eff out of range, bad enum        */
+  HDC_ERR_UNSUPPORTED = -2, /* a valid combination this build does not implement             */
+  HDC_ERR_ALIGNMENT = -3,   /* base pointer / leading dimension alignment                    */
+  HDC_ERR_WORKSPACE = -4,   /* ws == NULL or ws_bytes < hdc_workspace_bytes(...)             */
+  HDC_ERR_CUDA = -5,        /* CUDA runtime / launch error (text in hdc_last_error)          */
+  HDC_ERR_ARCH = -6         /* device is not sm_100                                          */
+} hdc_status;
+
+/* element types of buffers */
+enum { HDC_F32 = 0, HDC_BF16 = 1, HDC_I8 = 2, HDC_B1 = 3, HDC_U8 = 4, HDC_I32 = 5 };
+/* similarity kinds (L167 algorithmic choice) */
+enum { HDC_SIM_DOT = 0, HDC_SIM_COS = 1, HDC_SIM_HAMMING = 2 };
+/* hdc_train_epoch modes */
+enum { HDC_TRAIN_BUNDLE = 0, HDC_TRAIN_PERCEPTRON = 1 };
+/* hdc_encode_rp outputs (bit-or) */
+enum { HDC_OUT_BITS = 1, HDC_OUT_RAW = 4 };
+/* hdc_workspace_bytes ops */
+enum { HDC_OP_ENCODE_RP = 0, HDC_OP_ENCODE_LEVELID = 1, HDC_OP_SIMILARITY = 2, HDC_OP_CLASSIFY = 3,
+       HDC_OP_TRAIN_EPOCH = 4, HDC_OP_INFER_RP_HOST = 5 };
+/* knobs.flags */
+enum {
+  HDC_FLAG_NONE = 0,
+  HDC_FLAG_SIMT = 1 /* force the CUDA-core (FFMA / popcount) kernels where a tensor-core kernel
+                       exists for the same operation (debugging, A/B measurement)              */
+};
+
+/* Approximation knobs (section 4.2).
+ *  D_eff      effective dimensionality, 1..D (L61, L155, L163).
+ *  precision  operand type of the encode contraction (L165): HDC_F32 | HDC_BF16 | HDC_I8 | HDC_B1.
+ *             HDC_BF16: operands rounded to nearest-even bf16, fp32 accumulate.  HDC_I8: per-row
+ *             symmetric int8 of X and of P (a = max|row|, s = 127/a, q = clamp(rint(x*s),+-127)),
+ *             int32 accumulate.  HDC_B1: packed hypervectors with the real-valued contraction in
+ *             bf16 (same contraction as HDC_BF16).
+ *  hv_bits    element width of the CLASS hypervectors in similarity / classify / train (L165):
+ *             32 fp32 | 16 bf16 (RNE of C_acc) | 8 int8 (per-tensor symmetric over k<K, d<D_eff)
+ *             | 1 sign bit [C_acc < 0].  Query hypervectors are always bipolar (packed bits).
+ *  sim        HDC_SIM_*; HDC_SIM_HAMMING requires hv_bits == 1.
+ *  flags      HDC_FLAG_*.                                                                        */
+typedef struct {
+  int32_t D_eff;
+  int32_t precision;
+  int32_t hv_bits;
+  int32_t sim;
+  int32_t flags;
+} hdc_knobs_t;
+
+/* ---- handle ------------------------------------------------------------------------------ */
+/* Creates a context on CUDA device `device` (sets nothing globally except cudaSetDevice during
+ * the call).  HDC_ERR_ARCH unless compute capability 10.x; HDC_ERR_CUDA if no device. */
+int32_t hdc_create(hdc_handle_t* out, int32_t device);
+int32_t hdc_destroy(hdc_handle_t h);
+/* Host string describing the last error on this handle; valid until the next call on it. */
+const char* hdc_last_error(hdc_handle_t h);
+/* ABI version of this header (major*100 + minor). */
+int32_t hdc_version(void);
+/* Number of kernel launches this handle has enqueued since creation (bench `gpu_launches`). */
+int64_t hdc_launch_count(hdc_handle_t h);
+
+/* Bytes of device workspace the given op needs for these sizes and knobs (0 is possible).
+ * F_or_Q: F for encode_rp / infer_rp_host, Q for encode_levelid, ignored otherwise.
+ * For HDC_OP_TRAIN_EPOCH, N is the mini-batch size actually used (batch, or N when batch = 0). */
+size_t hdc_workspace_bytes(hdc_handle_t h, int32_t op, int64_t N, int32_t F_or_Q, int32_t D,
+                           int32_t K, const hdc_knobs_t* knobs);
+
+/* ---- (1a) random-projection encode + sign + pack ------------------------------------------
+ * PAPER.md Listing 1 L68-L70 `__hetero_hdc_matmul`, L155, L161 (automatic binarization).
+ *   acc[n,d] = sum_{f<F} x~[n,f] * p~[d,f],   bit[n,d] = [acc[n,d] < 0],   d < D_eff
+ * (x~, p~ = operands at knobs->precision).  The F reduction is never perforated (L157, L187).
+ * X [N][ldx] of x_dtype (HDC_F32 or HDC_BF16); P [D][ldp] of p_dtype (HDC_F32 or HDC_BF16).
+ * A bf16 input under precision HDC_F32 is widened exactly.  out_kinds: HDC_OUT_BITS writes
+ * Hbits [N][ldh_words]; HDC_OUT_RAW additionally writes the accumulators to Hraw [N][ldraw]
+ * (float for F32/BF16/B1, int32 for I8).  Unused outputs may be NULL. */
+int32_t hdc_encode_rp(hdc_handle_t h, const void* X, int32_t x_dtype, int64_t N, int32_t F,
+                      int64_t ldx, const void* P, int32_t p_dtype, int32_t D, int64_t ldp,
+                      const hdc_knobs_t* knobs, int32_t out_kinds, uint32_t* Hbits,
+                      int64_t ldh_words, void* Hraw, int64_t ldraw, void* ws, size_t ws_bytes,
+                      void* stream);
+
+/* ---- (1b) level-ID record encode ----------------------------------------------------------
+ * PAPER.md L167 ("ID-based encoding"), L183 (N_LEVELS), L239 (Level-ID); bind = XOR, bundle =
+ * majority (BASELINE.json north_star).
+ *   cnt[n,d] = sum_{f<F} ( ID[f,d] XOR LV[levels[n,f], d] ),   bit[n,d] = [2*cnt > F]
+ * levels [N][ldl] uint8 level indices, each < Q <= 256 (unchecked on device);
+ * IDbits [F][ldid_words], LVbits [Q][ldlv_words] packed tables covering D bits. */
+int32_t hdc_encode_levelid(hdc_handle_t h, const uint8_t* levels, int64_t N, int32_t F, int64_t ldl,
+                           const uint32_t* IDbits, int64_t ldid_words, const uint32_t* LVbits,
+                           int32_t Q, int64_t ldlv_words, int32_t D, const hdc_knobs_t* knobs,
+                           uint32_t* Hbits, int64_t ldh_words, void* ws, size_t ws_bytes,
+                           void* stream);
+
+/* ---- (2) similarity -----------------------------------------------------------------------
+ * PAPER.md L72-L74 `__hetero_hdc_hamming_distance`, L110 `__hetero_hdc_cos_sim`, L197 dot.
+ * Hbits [N][ldh_words] packed queries; C_acc [K][ldc] fp32 class accumulators, from which the
+ * class operand is derived at knobs->hv_bits.  Over d < D_eff:
+ *   HAMMING  dist[n,k] = popcount(h[n] xor cbit[k])                       -> S int32 [N][lds]
+ *   DOT      s[n,k]   = sum_d v[n,d]*c[k,d]                               -> S fp32 (int32 if hv_bits 8 or 1)
+ *   COS      s[n,k]   = DOT / (sqrt(D_eff) * sqrt(sum_d c[k,d]^2)), 0 if the norm is 0   -> S fp32
+ * s_dtype must be HDC_I32 for HAMMING, HDC_F32 for COS, HDC_F32 or HDC_I32 for DOT (HDC_I32 only
+ * for hv_bits 8 or 1). */
+int32_t hdc_similarity(hdc_handle_t h, const uint32_t* Hbits, int64_t N, int64_t ldh_words,
+                       const float* C_acc, int32_t K, int64_t ldc, int32_t D,
+                       const hdc_knobs_t* knobs, void* S, int32_t s_dtype, int64_t lds, void* ws,
+                       size_t ws_bytes, void* stream);
+
+/* ---- (2+3a) classify = similarity + arg-extremum, fused (no S matrix) ----------------------
+ * PAPER.md Listing 1 L72-L80.  labels[n] = arg-max (DOT, COS) or arg-min (HAMMING) over k, ties
+ * to the lowest k.  best / second (nullable, fp32 [N]) receive the winning and runner-up score
+ * (distances as floats for HAMMING; second = best when K == 1 or on a tie). */
+int32_t hdc_classify(hdc_handle_t h, const uint32_t* Hbits, int64_t N, int64_t ldh_words,
+                     const float* C_acc, int32_t K, int64_t ldc, int32_t D,
+                     const hdc_knobs_t* knobs, int32_t* labels, float* best, float* second,
+                     void* ws, size_t ws_bytes, void* stream);
+
+/* ---- (3b,3c) one-pass bundling and one retraining epoch ------------------------------------
+ * PAPER.md L53 (class hypervectors by vector addition), L181 (TRAIN_ITERATIONS); the update
+ * rule is the perceptron-style reading S9 of DESIGN.md.
+ *  mode HDC_TRAIN_BUNDLE:      C_acc[k,d] += sum_{n: y_n = k} v[n,d]             (knobs: D_eff only)
+ *  mode HDC_TRAIN_PERCEPTRON:  samples in index order; per mini-batch of `batch` samples
+ *      (0 => N): yhat = classify(h) with the current C_acc at knobs->{hv_bits,sim};
+ *      Delta[k,d] = sum_{yhat_n != y_n} ([k = y_n] - [k = yhat_n]) * v[n,d]   (integer);
+ *      C_acc[k,d] = fl32(C_acc[k,d] + fl32(lr * (float)Delta[k,d])).
+ * y [N] int32 labels in [0,K) (unchecked on device).  pred (nullable, int32 [N]) receives yhat;
+ * n_wrong (nullable, device uint64) is INCREMENTED by the number of mispredictions.
+ * Deterministic: integer Delta, no floating-point atomics. */
+int32_t hdc_train_epoch(hdc_handle_t h, int32_t mode, const uint32_t* Hbits, int64_t N,
+                        int64_t ldh_words, const int32_t* y, float* C_acc, int32_t K, int64_t ldc,
+                        int32_t D, const hdc_knobs_t* knobs, float lr, int64_t batch, int32_t* pred,
+                        unsigned long long* n_wrong, void* ws, size_t ws_bytes, void* stream);
+
+/* ---- end-to-end inference from host buffers ------------------------------------------------
+ * encode_rp + classify for N queries whose features live in HOST memory (pinned for full speed):
+ * copies X_host in chunks to the device (inside the call), runs (1a)+(2)+(3a) and copies the
+ * labels back to labels_host; synchronises `stream` before returning.  P and C_acc are device
+ * pointers as above.  Used for the end-to-end (`e2e`) measurement. */
+int32_t hdc_infer_rp_host(hdc_handle_t h, const void* X_host, int32_t x_dtype, int64_t N, int32_t F,
+                          int64_t ldx, const void* P, int32_t p_dtype, int32_t D, int64_t ldp,
+                          const float* C_acc, int32_t K, int64_t ldc, const hdc_knobs_t* knobs,
+                          int32_t* labels_host, void* ws, size_t ws_bytes, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HDC_H_ */
