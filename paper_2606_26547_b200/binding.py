@@ -1,0 +1,249 @@
+"""ctypes binding of libhdc.so (include/hdc.h).  Argument marshalling only: every step of the HDC
+hot path runs in the CUDA kernels behind the C ABI.  PyTorch is used for device memory
+(`torch.empty`, `data_ptr()`) and streams, nothing else.  There is no CPU fallback: a missing
+library or a failing call raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import torch
+
+_LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "lib", "libhdc.so")
+
+# enums of include/hdc.h
+HDC_OK = 0
+HDC_ERR_INVALID_ARG, HDC_ERR_UNSUPPORTED, HDC_ERR_ALIGNMENT = -1, -2, -3
+HDC_ERR_WORKSPACE, HDC_ERR_CUDA, HDC_ERR_ARCH = -4, -5, -6
+HDC_F32, HDC_BF16, HDC_I8, HDC_B1, HDC_U8, HDC_I32 = 0, 1, 2, 3, 4, 5
+HDC_SIM_DOT, HDC_SIM_COS, HDC_SIM_HAMMING = 0, 1, 2
+HDC_TRAIN_BUNDLE, HDC_TRAIN_PERCEPTRON = 0, 1
+HDC_OUT_BITS, HDC_OUT_RAW = 1, 4
+HDC_OP_ENCODE_RP, HDC_OP_ENCODE_LEVELID, HDC_OP_SIMILARITY = 0, 1, 2
+HDC_OP_CLASSIFY, HDC_OP_TRAIN_EPOCH, HDC_OP_INFER_RP_HOST = 3, 4, 5
+HDC_FLAG_NONE, HDC_FLAG_SIMT = 0, 1
+
+EXPORTS = ("hdc_create", "hdc_destroy", "hdc_last_error", "hdc_version", "hdc_launch_count",
+           "hdc_workspace_bytes", "hdc_encode_rp", "hdc_encode_levelid", "hdc_similarity",
+           "hdc_classify", "hdc_train_epoch", "hdc_infer_rp_host")
+
+
+class hdc_knobs_t(C.Structure):
+    _fields_ = [("D_eff", C.c_int32), ("precision", C.c_int32), ("hv_bits", C.c_int32),
+                ("sim", C.c_int32), ("flags", C.c_int32)]
+
+
+class HdcError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"libhdc error {code}: {msg}")
+        self.code = code
+
+
+_lib = None
+
+
+def lib() -> C.CDLL:
+    """Loads libhdc.so (built in-tree by paper_2606_26547_b200.build); raises if it is missing."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_LIB_PATH):
+        raise RuntimeError(f"{_LIB_PATH} is missing: run `python -m paper_2606_26547_b200.build` "
+                           "(there is no fallback path)")
+    L = C.CDLL(_LIB_PATH)
+    vp, i32, i64, sz = C.c_void_p, C.c_int32, C.c_int64, C.c_size_t
+    kp = C.POINTER(hdc_knobs_t)
+    L.hdc_create.argtypes = [C.POINTER(vp), i32]
+    L.hdc_create.restype = i32
+    L.hdc_destroy.argtypes = [vp]
+    L.hdc_destroy.restype = i32
+    L.hdc_last_error.argtypes = [vp]
+    L.hdc_last_error.restype = C.c_char_p
+    L.hdc_version.argtypes = []
+    L.hdc_version.restype = i32
+    L.hdc_launch_count.argtypes = [vp]
+    L.hdc_launch_count.restype = i64
+    L.hdc_workspace_bytes.argtypes = [vp, i32, i64, i32, i32, i32, kp]
+    L.hdc_workspace_bytes.restype = sz
+    L.hdc_encode_rp.argtypes = [vp, vp, i32, i64, i32, i64, vp, i32, i32, i64, kp, i32, vp, i64, vp, i64,
+                                vp, sz, vp]
+    L.hdc_encode_rp.restype = i32
+    L.hdc_encode_levelid.argtypes = [vp, vp, i64, i32, i64, vp, i64, vp, i32, i64, i32, kp, vp, i64, vp, sz,
+                                     vp]
+    L.hdc_encode_levelid.restype = i32
+    L.hdc_similarity.argtypes = [vp, vp, i64, i64, vp, i32, i64, i32, kp, vp, i32, i64, vp, sz, vp]
+    L.hdc_similarity.restype = i32
+    L.hdc_classify.argtypes = [vp, vp, i64, i64, vp, i32, i64, i32, kp, vp, vp, vp, vp, sz, vp]
+    L.hdc_classify.restype = i32
+    L.hdc_train_epoch.argtypes = [vp, i32, vp, i64, i64, vp, vp, i32, i64, i32, kp, C.c_float, i64, vp, vp,
+                                  vp, sz, vp]
+    L.hdc_train_epoch.restype = i32
+    L.hdc_infer_rp_host.argtypes = [vp, vp, i32, i64, i32, i64, vp, i32, i32, i64, vp, i32, i64, kp, vp, vp,
+                                    sz, vp]
+    L.hdc_infer_rp_host.restype = i32
+    _lib = L
+    return L
+
+
+def knobs(D_eff: int, precision: int = HDC_F32, hv_bits: int = 32, sim: int = HDC_SIM_COS,
+          flags: int = 0) -> hdc_knobs_t:
+    return hdc_knobs_t(int(D_eff), int(precision), int(hv_bits), int(sim), int(flags))
+
+
+_DT = {torch.float32: HDC_F32, torch.bfloat16: HDC_BF16, torch.int8: HDC_I8, torch.uint8: HDC_U8,
+       torch.int32: HDC_I32}
+
+
+def _ptr(t):
+    return None if t is None else C.c_void_p(t.data_ptr())
+
+
+def _rowmajor(t: torch.Tensor, name: str):
+    if t.dim() != 2 or t.stride(1) != 1:
+        raise ValueError(f"{name} must be 2-D with a contiguous last axis")
+    return t.stride(0) if t.shape[0] > 1 else max(t.stride(0), t.shape[1])
+
+
+class Handle:
+    """hdc_handle_t with a grow-only device workspace.  Methods mirror the C entry points."""
+
+    def __init__(self, device: int = 0):
+        self._L = lib()
+        self._h = C.c_void_p()
+        rc = self._L.hdc_create(C.byref(self._h), int(device))
+        if rc != HDC_OK:
+            raise HdcError(rc, "hdc_create failed (needs a compute-capability 10.x device)")
+        self.device = torch.device("cuda", device)
+        self._ws = None
+
+    def close(self):
+        if self._h:
+            self._L.hdc_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):  # pragma: no cover
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -------------------------------------------------------------------------------- helpers
+    def _check(self, rc: int):
+        if rc != HDC_OK:
+            raise HdcError(rc, self._L.hdc_last_error(self._h).decode())
+
+    def last_error(self) -> str:
+        return self._L.hdc_last_error(self._h).decode()
+
+    def launch_count(self) -> int:
+        return int(self._L.hdc_launch_count(self._h))
+
+    def workspace_bytes(self, op: int, N: int, F_or_Q: int, D: int, K: int, kn: hdc_knobs_t) -> int:
+        return int(self._L.hdc_workspace_bytes(self._h, op, N, F_or_Q, D, K, C.byref(kn)))
+
+    def _workspace(self, nbytes: int):
+        if nbytes <= 0:
+            return None, 0
+        if self._ws is None or self._ws.numel() < nbytes:
+            self._ws = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+        return C.c_void_p(self._ws.data_ptr()), self._ws.numel()
+
+    @staticmethod
+    def _stream():
+        return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+    # -------------------------------------------------------------------------------- (1a)
+    def hdc_encode_rp(self, X, P, kn: hdc_knobs_t, Hbits=None, want_raw: bool = False):
+        N, F = X.shape
+        D = P.shape[0]
+        W = (kn.D_eff + 31) // 32
+        if Hbits is None:
+            Hbits = torch.empty((N, W), dtype=torch.int32, device=self.device)
+        Hraw = None
+        if want_raw:
+            Hraw = torch.empty((N, kn.D_eff), device=self.device,
+                               dtype=torch.int32 if kn.precision == HDC_I8 else torch.float32)
+        ws, wsb = self._workspace(self.workspace_bytes(HDC_OP_ENCODE_RP, N, F, D, 0, kn))
+        rc = self._L.hdc_encode_rp(self._h, _ptr(X), _DT[X.dtype], N, F, _rowmajor(X, "X"), _ptr(P),
+                                   _DT[P.dtype], D, _rowmajor(P, "P"), C.byref(kn),
+                                   HDC_OUT_BITS | (HDC_OUT_RAW if want_raw else 0), _ptr(Hbits),
+                                   _rowmajor(Hbits, "Hbits"), _ptr(Hraw),
+                                   0 if Hraw is None else Hraw.stride(0), ws, wsb, self._stream())
+        self._check(rc)
+        return (Hbits, Hraw) if want_raw else Hbits
+
+    # -------------------------------------------------------------------------------- (1b)
+    def hdc_encode_levelid(self, levels, IDbits, LVbits, D: int, kn: hdc_knobs_t, Hbits=None):
+        N, F = levels.shape
+        Q = LVbits.shape[0]
+        W = (kn.D_eff + 31) // 32
+        if Hbits is None:
+            Hbits = torch.empty((N, W), dtype=torch.int32, device=self.device)
+        rc = self._L.hdc_encode_levelid(self._h, _ptr(levels), N, F, _rowmajor(levels, "levels"),
+                                        _ptr(IDbits), _rowmajor(IDbits, "IDbits"), _ptr(LVbits), Q,
+                                        _rowmajor(LVbits, "LVbits"), D, C.byref(kn), _ptr(Hbits),
+                                        _rowmajor(Hbits, "Hbits"), None, 0, self._stream())
+        self._check(rc)
+        return Hbits
+
+    # -------------------------------------------------------------------------------- (2)
+    def hdc_similarity(self, Hbits, C_acc, kn: hdc_knobs_t, s_dtype=None):
+        N = Hbits.shape[0]
+        K, D = C_acc.shape
+        if s_dtype is None:
+            s_dtype = torch.int32 if kn.sim == HDC_SIM_HAMMING else torch.float32
+        S = torch.empty((N, K), dtype=s_dtype, device=self.device)
+        ws, wsb = self._workspace(self.workspace_bytes(HDC_OP_SIMILARITY, N, 0, D, K, kn))
+        rc = self._L.hdc_similarity(self._h, _ptr(Hbits), N, _rowmajor(Hbits, "Hbits"), _ptr(C_acc), K,
+                                    _rowmajor(C_acc, "C_acc"), D, C.byref(kn), _ptr(S), _DT[s_dtype],
+                                    S.stride(0) if N > 1 else K, ws, wsb, self._stream())
+        self._check(rc)
+        return S
+
+    # -------------------------------------------------------------------------------- (2+3a)
+    def hdc_classify(self, Hbits, C_acc, kn: hdc_knobs_t, want_scores: bool = False, labels=None):
+        N = Hbits.shape[0]
+        K, D = C_acc.shape
+        if labels is None:
+            labels = torch.empty(N, dtype=torch.int32, device=self.device)
+        best = second = None
+        if want_scores:
+            best = torch.empty(N, dtype=torch.float32, device=self.device)
+            second = torch.empty(N, dtype=torch.float32, device=self.device)
+        ws, wsb = self._workspace(self.workspace_bytes(HDC_OP_CLASSIFY, N, 0, D, K, kn))
+        rc = self._L.hdc_classify(self._h, _ptr(Hbits), N, _rowmajor(Hbits, "Hbits"), _ptr(C_acc), K,
+                                  _rowmajor(C_acc, "C_acc"), D, C.byref(kn), _ptr(labels), _ptr(best),
+                                  _ptr(second), ws, wsb, self._stream())
+        self._check(rc)
+        return (labels, best, second) if want_scores else labels
+
+    # -------------------------------------------------------------------------------- (3b, 3c)
+    def hdc_train_epoch(self, mode: int, Hbits, y, C_acc, kn: hdc_knobs_t, lr: float = 1.0,
+                        batch: int = 0, pred=None, n_wrong=None):
+        N = Hbits.shape[0]
+        K, D = C_acc.shape
+        B = N if batch in (0, None) or batch > N else batch
+        ws, wsb = self._workspace(self.workspace_bytes(HDC_OP_TRAIN_EPOCH, B, 0, D, K, kn))
+        rc = self._L.hdc_train_epoch(self._h, mode, _ptr(Hbits), N, _rowmajor(Hbits, "Hbits"), _ptr(y),
+                                     _ptr(C_acc), K, _rowmajor(C_acc, "C_acc"), D, C.byref(kn),
+                                     C.c_float(lr), int(batch or 0), _ptr(pred), _ptr(n_wrong), ws, wsb,
+                                     self._stream())
+        self._check(rc)
+        return C_acc
+
+    # -------------------------------------------------------------------------------- host e2e
+    def hdc_infer_rp_host(self, X_host, P, C_acc, kn: hdc_knobs_t, labels_host=None):
+        """X_host: CPU tensor (pinned for full speed); returns CPU int32 labels.  Synchronises."""
+        N, F = X_host.shape
+        D = P.shape[0]
+        K = C_acc.shape[0]
+        if labels_host is None:
+            labels_host = torch.empty(N, dtype=torch.int32).pin_memory()
+        ws, wsb = self._workspace(self.workspace_bytes(HDC_OP_INFER_RP_HOST, N, F, D, K, kn))
+        rc = self._L.hdc_infer_rp_host(self._h, _ptr(X_host), _DT[X_host.dtype], N, F,
+                                       _rowmajor(X_host, "X_host"), _ptr(P), _DT[P.dtype], D,
+                                       _rowmajor(P, "P"), _ptr(C_acc), K, _rowmajor(C_acc, "C_acc"),
+                                       C.byref(kn), _ptr(labels_host), ws, wsb, self._stream())
+        self._check(rc)
+        return labels_host

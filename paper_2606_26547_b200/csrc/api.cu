@@ -1,0 +1,576 @@
+// api.cu -- the C ABI of libhdc.so (include/hdc.h): argument validation on the host before anything
+// is enqueued, workspace carving, and the sequencing of the kernels of each entry point.  No
+// arithmetic of the method lives here.
+#include <stdio.h>
+
+#include <string>
+
+#include "common.cuh"
+
+struct hdc_ctx {
+  int device = 0;
+  int sm_count = 0;
+  int smem_optin = 0;
+  int64_t launches = 0;
+  std::string err;
+  hdc::TcContext* tc = nullptr;
+  cudaStream_t copy_stream = nullptr;
+  cudaEvent_t ev_copied[2] = {nullptr, nullptr};
+  cudaEvent_t ev_done[2] = {nullptr, nullptr};
+  cudaEvent_t ev_entry = nullptr;
+};
+
+namespace hdc {
+namespace {
+
+// Bump allocator over the caller's workspace; with base == nullptr it only measures.
+struct Bump {
+  char* base;
+  size_t off = 0;
+  explicit Bump(void* b) : base((char*)b) {}
+  template <typename T>
+  T* take(size_t count) {
+    off = (size_t)round_up((int64_t)off, 256);
+    T* p = base ? reinterpret_cast<T*>(base + off) : nullptr;
+    off += count * sizeof(T);
+    return p;
+  }
+};
+
+int fail(hdc_ctx* h, int code, const char* msg) {
+  if (h) h->err = msg;
+  return code;
+}
+int cuda_fail(hdc_ctx* h, cudaError_t e, const char* where) {
+  if (h) h->err = std::string(where) + ": " + cudaGetErrorString(e);
+  return HDC_ERR_CUDA;
+}
+bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15) == 0; }
+
+int check_knobs(hdc_ctx* h, const hdc_knobs_t* k, int D) {
+  if (!k) return fail(h, HDC_ERR_INVALID_ARG, "knobs is NULL");
+  if (k->D_eff < 1 || k->D_eff > D) return fail(h, HDC_ERR_INVALID_ARG, "D_eff outside 1..D");
+  return HDC_OK;
+}
+int check_sim_knobs(hdc_ctx* h, const hdc_knobs_t* k) {
+  if (k->hv_bits != 32 && k->hv_bits != 16 && k->hv_bits != 8 && k->hv_bits != 1)
+    return fail(h, HDC_ERR_INVALID_ARG, "hv_bits must be 32, 16, 8 or 1");
+  if (k->sim != HDC_SIM_DOT && k->sim != HDC_SIM_COS && k->sim != HDC_SIM_HAMMING)
+    return fail(h, HDC_ERR_INVALID_ARG, "bad sim");
+  if (k->sim == HDC_SIM_HAMMING && k->hv_bits != 1)
+    return fail(h, HDC_ERR_INVALID_ARG, "HDC_SIM_HAMMING requires hv_bits == 1");
+  return HDC_OK;
+}
+
+// ------------------------------------------------------------------------------------- encode
+struct EncodePlan {
+  bool tc = false;         // tensor-core kernel
+  void* Xs = nullptr;      // staged X (bf16 or int8), null = use input in place
+  void* Ps = nullptr;      // staged P
+  int64_t ldxs = 0, ldps = 0;
+  int Fp = 0;
+};
+
+bool use_tc(const hdc_ctx* h, const hdc_knobs_t* k) {
+  return h->tc != nullptr && !(k->flags & HDC_FLAG_SIMT);
+}
+
+// Carves the staging buffers of hdc_encode_rp.  x_inplace / p_inplace: operand usable as given.
+void plan_encode(const hdc_ctx* h, int64_t N, int F, int D_eff, const hdc_knobs_t* k, bool x_inplace,
+                 bool p_inplace, Bump& b, EncodePlan& pl) {
+  const int prec = k->precision;
+  if (prec == HDC_F32) return;
+  if (prec == HDC_I8) {
+    pl.Fp = (int)round_up(F, 64);
+    pl.ldxs = pl.ldps = pl.Fp;
+    pl.tc = use_tc(h, k);
+    if (!x_inplace) pl.Xs = b.take<int8_t>((size_t)N * pl.Fp);
+    if (!p_inplace) pl.Ps = b.take<int8_t>((size_t)D_eff * pl.Fp);
+    return;
+  }
+  // BF16 / B1
+  pl.tc = use_tc(h, k);
+  if (!pl.tc) return;  // CUDA-core kernel rounds on load, no staging
+  pl.Fp = (int)round_up(F, 64);
+  pl.ldxs = pl.ldps = pl.Fp;
+  if (!x_inplace) pl.Xs = b.take<__nv_bfloat16>((size_t)N * pl.Fp);
+  if (!p_inplace) pl.Ps = b.take<__nv_bfloat16>((size_t)D_eff * pl.Fp);
+}
+
+int do_encode_rp(hdc_ctx* h, const void* X, int x_dtype, int64_t N, int F, int64_t ldx, const void* P,
+                 int p_dtype, int D, int64_t ldp, const hdc_knobs_t* k, int out_kinds, uint32_t* Hbits,
+                 int64_t ldh, void* Hraw, int64_t ldraw, Bump& b, size_t ws_bytes, cudaStream_t st) {
+  (void)D;
+  const int D_eff = k->D_eff;
+  const int prec = k->precision;
+  const bool want_raw = (out_kinds & HDC_OUT_RAW) != 0;
+  Epilogue e{};
+  e.kind = EPI_SIGN;
+  e.bits = Hbits;
+  e.ldbits = ldh;
+  e.raw = want_raw ? Hraw : nullptr;
+  e.ldraw = ldraw;
+  const int xk = x_dtype == HDC_BF16 ? OPK_BF16 : OPK_F32;
+  const int pk = p_dtype == HDC_BF16 ? OPK_BF16 : (p_dtype == HDC_I8 ? OPK_I8 : OPK_F32);
+  cudaError_t ce;
+
+  if (prec == HDC_F32) {
+    ce = launch_gemm_simt(Operand{X, ldx, xk}, Operand{P, ldp, pk}, N, D_eff, F, false, e, st, &h->launches);
+    return ce == cudaSuccess ? HDC_OK : cuda_fail(h, ce, "encode_rp fp32");
+  }
+
+  EncodePlan pl;
+  const bool tc_ok_x = x_dtype == HDC_BF16 && (ldx % 8) == 0 && aligned16(X);
+  const bool tc_ok_p = p_dtype == HDC_BF16 && (ldp % 8) == 0 && aligned16(P);
+  if (prec == HDC_I8) {
+    const bool p_in = p_dtype == HDC_I8 && (ldp % 16) == 0 && aligned16(P);
+    plan_encode(h, N, F, D_eff, k, false, p_in, b, pl);
+    if (b.off > ws_bytes) return fail(h, HDC_ERR_WORKSPACE, "encode_rp: workspace too small");
+    ce = launch_quantize_rows_i8(X, xk, N, F, ldx, (int8_t*)pl.Xs, pl.ldxs, st, &h->launches);
+    if (ce != cudaSuccess) return cuda_fail(h, ce, "quantize X");
+    const void* Pq = P;
+    int64_t ldpq = ldp;
+    if (!p_in) {
+      ce = launch_quantize_rows_i8(P, pk, D_eff, F, ldp, (int8_t*)pl.Ps, pl.ldps, st, &h->launches);
+      if (ce != cudaSuccess) return cuda_fail(h, ce, "quantize P");
+      Pq = pl.Ps;
+      ldpq = pl.ldps;
+    }
+    if (pl.tc) {
+      ce = launch_gemm_tc(h->tc, pl.Xs, Pq, OPK_I8, N, D_eff, pl.Fp, pl.ldxs, ldpq, e, h->sm_count, st,
+                          &h->launches);
+      if (ce == cudaSuccess) return HDC_OK;
+      if (ce != cudaErrorNotSupported) return cuda_fail(h, ce, "encode_rp int8 tcgen05");
+    }
+    ce = launch_gemm_simt(Operand{pl.Xs, pl.ldxs, OPK_I8}, Operand{Pq, ldpq, OPK_I8}, N, D_eff, F, true, e,
+                          st, &h->launches);
+    return ce == cudaSuccess ? HDC_OK : cuda_fail(h, ce, "encode_rp int8");
+  }
+
+  // BF16 / B1
+  plan_encode(h, N, F, D_eff, k, tc_ok_x, tc_ok_p, b, pl);
+  if (b.off > ws_bytes) return fail(h, HDC_ERR_WORKSPACE, "encode_rp: workspace too small");
+  if (pl.tc) {
+    const void* Xb = X;
+    const void* Pb = P;
+    int64_t ldxb = ldx, ldpb = ldp;
+    if (!tc_ok_x) {
+      ce = launch_convert_bf16(X, xk, N, F, ldx, (__nv_bfloat16*)pl.Xs, pl.ldxs, st, &h->launches);
+      if (ce != cudaSuccess) return cuda_fail(h, ce, "convert X");
+      Xb = pl.Xs;
+      ldxb = pl.ldxs;
+    }
+    if (!tc_ok_p) {
+      ce = launch_convert_bf16(P, pk, D_eff, F, ldp, (__nv_bfloat16*)pl.Ps, pl.ldps, st, &h->launches);
+      if (ce != cudaSuccess) return cuda_fail(h, ce, "convert P");
+      Pb = pl.Ps;
+      ldpb = pl.ldps;
+    }
+    ce = launch_gemm_tc(h->tc, Xb, Pb, OPK_BF16, N, D_eff, F, ldxb, ldpb, e, h->sm_count, st, &h->launches);
+    if (ce == cudaSuccess) return HDC_OK;
+    if (ce != cudaErrorNotSupported) return cuda_fail(h, ce, "encode_rp bf16 tcgen05");
+  }
+  const int xr = x_dtype == HDC_BF16 ? OPK_BF16 : OPK_F32_RBF16;
+  const int pr = p_dtype == HDC_BF16 ? OPK_BF16 : OPK_F32_RBF16;
+  ce = launch_gemm_simt(Operand{X, ldx, xr}, Operand{P, ldp, pr}, N, D_eff, F, false, e, st, &h->launches);
+  return ce == cudaSuccess ? HDC_OK : cuda_fail(h, ce, "encode_rp bf16");
+}
+
+// ------------------------------------------------------------------------------------- similarity
+// Shared by hdc_similarity (S != null), hdc_classify (labels != null) and hdc_train_epoch.
+int do_similarity(hdc_ctx* h, const uint32_t* Hbits, int64_t N, int64_t ldh, const float* C_acc, int K,
+                  int64_t ldc, const hdc_knobs_t* k, void* S, int s_i32, int64_t lds, int32_t* labels,
+                  float* best, float* second, Bump& b, size_t ws_bytes, cudaStream_t st) {
+  const int D_eff = k->D_eff;
+  const int W = words_of(D_eff);
+  cudaError_t ce;
+  if (k->sim == HDC_SIM_HAMMING) {
+    uint32_t* cbits = b.take<uint32_t>((size_t)K * W);
+    if (b.off > ws_bytes) return fail(h, HDC_ERR_WORKSPACE, "similarity: workspace too small");
+    ce = launch_sign_bits(C_acc, K, D_eff, ldc, cbits, W, st, &h->launches);
+    if (ce != cudaSuccess) return cuda_fail(h, ce, "sign_bits");
+    ce = launch_hamming(Hbits, N, ldh, cbits, K, W, D_eff, (int32_t*)S, lds, labels, best, second,
+                        h->sm_count, h->smem_optin, st, &h->launches);
+    return ce == cudaSuccess ? HDC_OK : cuda_fail(h, ce, "hamming");
+  }
+  // DOT / COS: contraction of +-1 queries with the class operand at hv_bits
+  Operand B{};
+  bool int_acc = false;
+  double* colscale = nullptr;
+  if (k->sim == HDC_SIM_COS) colscale = b.take<double>((size_t)K);
+  if (k->hv_bits == 32) {
+    B = Operand{C_acc, ldc, OPK_F32};
+  } else if (k->hv_bits == 16) {
+    B = Operand{C_acc, ldc, OPK_F32_RBF16};
+  } else if (k->hv_bits == 8) {
+    const int64_t ldq = round_up(D_eff, 16);
+    int8_t* Cq = b.take<int8_t>((size_t)K * ldq);
+    float* amax = b.take<float>(1);
+    if (b.off > ws_bytes) return fail(h, HDC_ERR_WORKSPACE, "similarity: workspace too small");
+    ce = launch_quantize_tensor_i8(C_acc, K, D_eff, ldc, Cq, ldq, amax, st, &h->launches);
+    if (ce != cudaSuccess) return cuda_fail(h, ce, "quantize C");
+    B = Operand{Cq, ldq, OPK_I8};
+    int_acc = true;
+  } else {
+    uint32_t* cbits = b.take<uint32_t>((size_t)K * W);
+    if (b.off > ws_bytes) return fail(h, HDC_ERR_WORKSPACE, "similarity: workspace too small");
+    ce = launch_sign_bits(C_acc, K, D_eff, ldc, cbits, W, st, &h->launches);
+    if (ce != cudaSuccess) return cuda_fail(h, ce, "sign_bits");
+    B = Operand{cbits, W, OPK_BITS};
+    int_acc = true;
+  }
+  if (b.off > ws_bytes) return fail(h, HDC_ERR_WORKSPACE, "similarity: workspace too small");
+  if (colscale) {
+    ce = launch_col_scale(B, K, D_eff, 1, colscale, st, &h->launches);
+    if (ce != cudaSuccess) return cuda_fail(h, ce, "col_scale");
+  }
+  Epilogue e{};
+  e.colscale = colscale;
+  if (labels) {
+    e.kind = EPI_ARGMAX;
+    e.labels = labels;
+    e.best = best;
+    e.second = second;
+  } else {
+    e.kind = EPI_SCORE;
+    e.S = S;
+    e.lds = lds;
+    e.s_i32 = s_i32;
+  }
+  ce = launch_gemm_simt(Operand{Hbits, ldh, OPK_BITS}, B, N, K, D_eff, int_acc, e, st, &h->launches);
+  return ce == cudaSuccess ? HDC_OK : cuda_fail(h, ce, "similarity contraction");
+}
+
+size_t similarity_ws(int K, const hdc_knobs_t* k) {
+  Bump b(nullptr);
+  const int W = words_of(k->D_eff);
+  b.take<double>((size_t)K);
+  b.take<int8_t>((size_t)K * round_up(k->D_eff, 16));
+  b.take<float>(1);
+  b.take<uint32_t>((size_t)K * W);
+  return b.off + 256;
+}
+
+constexpr int64_t HOST_CHUNK = 16384;
+
+}  // namespace
+}  // namespace hdc
+
+using namespace hdc;
+
+// =================================================================================== handle
+extern "C" int32_t hdc_version(void) { return 100; }
+
+extern "C" int32_t hdc_create(hdc_handle_t* out, int32_t device) {
+  if (!out) return HDC_ERR_INVALID_ARG;
+  *out = nullptr;
+  int count = 0;
+  if (cudaGetDeviceCount(&count) != cudaSuccess || device < 0 || device >= count) {
+    (void)cudaGetLastError();
+    return HDC_ERR_CUDA;
+  }
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return HDC_ERR_CUDA;
+  if (prop.major != 10) return HDC_ERR_ARCH;
+  if (cudaSetDevice(device) != cudaSuccess) return HDC_ERR_CUDA;
+  hdc_ctx* h = new hdc_ctx();
+  h->device = device;
+  h->sm_count = prop.multiProcessorCount;
+  h->smem_optin = (int)prop.sharedMemPerBlockOptin;
+  h->tc = tc_context_create();
+  if (cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking) != cudaSuccess) {
+    delete h;
+    return HDC_ERR_CUDA;
+  }
+  for (int i = 0; i < 2; ++i) {
+    cudaEventCreateWithFlags(&h->ev_copied[i], cudaEventDisableTiming);
+    cudaEventCreateWithFlags(&h->ev_done[i], cudaEventDisableTiming);
+  }
+  cudaEventCreateWithFlags(&h->ev_entry, cudaEventDisableTiming);
+  *out = h;
+  return HDC_OK;
+}
+
+extern "C" int32_t hdc_destroy(hdc_handle_t h) {
+  if (!h) return HDC_ERR_INVALID_ARG;
+  for (int i = 0; i < 2; ++i) {
+    if (h->ev_copied[i]) cudaEventDestroy(h->ev_copied[i]);
+    if (h->ev_done[i]) cudaEventDestroy(h->ev_done[i]);
+  }
+  if (h->ev_entry) cudaEventDestroy(h->ev_entry);
+  if (h->copy_stream) cudaStreamDestroy(h->copy_stream);
+  tc_context_destroy(h->tc);
+  delete h;
+  return HDC_OK;
+}
+
+extern "C" const char* hdc_last_error(hdc_handle_t h) { return h ? h->err.c_str() : "null handle"; }
+
+extern "C" int64_t hdc_launch_count(hdc_handle_t h) { return h ? h->launches : -1; }
+
+// =================================================================================== workspace
+extern "C" size_t hdc_workspace_bytes(hdc_handle_t h, int32_t op, int64_t N, int32_t F_or_Q, int32_t D,
+                                      int32_t K, const hdc_knobs_t* knobs) {
+  if (!h || !knobs || N < 0) return 0;
+  hdc_knobs_t k = *knobs;
+  if (k.D_eff < 1 || k.D_eff > D) k.D_eff = D;
+  Bump b(nullptr);
+  switch (op) {
+    case HDC_OP_ENCODE_RP: {
+      EncodePlan pl;
+      plan_encode(h, N, F_or_Q, k.D_eff, &k, false, false, b, pl);
+      return b.off + 256;
+    }
+    case HDC_OP_ENCODE_LEVELID:
+      return 0;
+    case HDC_OP_SIMILARITY:
+    case HDC_OP_CLASSIFY:
+      return similarity_ws(K, &k);
+    case HDC_OP_TRAIN_EPOCH: {
+      b.take<int32_t>((size_t)K * words_of(k.D_eff) * 32);  // Delta
+      b.take<int32_t>((size_t)N);                           // predictions of one mini-batch
+      return b.off + 256 + similarity_ws(K, &k);
+    }
+    case HDC_OP_INFER_RP_HOST: {
+      const int64_t chunk = N < HOST_CHUNK ? N : HOST_CHUNK;
+      b.take<float>((size_t)chunk * F_or_Q);  // two staging buffers for X (fp32 upper bound)
+      b.take<float>((size_t)chunk * F_or_Q);
+      b.take<uint32_t>((size_t)chunk * words_of(k.D_eff));
+      b.take<int32_t>((size_t)N);
+      EncodePlan pl;
+      plan_encode(h, chunk, F_or_Q, k.D_eff, &k, false, false, b, pl);
+      return b.off + 512 + similarity_ws(K, &k);
+    }
+    default:
+      return 0;
+  }
+}
+
+// =================================================================================== (1a)
+static int check_encode_rp_args(hdc_ctx* h, const void* X, int x_dtype, int64_t N, int F, int64_t ldx,
+                                const void* P, int p_dtype, int D, int64_t ldp, const hdc_knobs_t* k) {
+  if (!X || !P) return fail(h, HDC_ERR_INVALID_ARG, "encode_rp: NULL operand");
+  if (N < 0 || F < 1 || D < 1 || ldx < F || ldp < F) return fail(h, HDC_ERR_INVALID_ARG, "encode_rp: bad sizes");
+  if (x_dtype != HDC_F32 && x_dtype != HDC_BF16) return fail(h, HDC_ERR_INVALID_ARG, "encode_rp: x_dtype");
+  if (p_dtype != HDC_F32 && p_dtype != HDC_BF16 && p_dtype != HDC_I8)
+    return fail(h, HDC_ERR_INVALID_ARG, "encode_rp: p_dtype");
+  int rc = check_knobs(h, k, D);
+  if (rc) return rc;
+  if (k->precision != HDC_F32 && k->precision != HDC_BF16 && k->precision != HDC_I8 && k->precision != HDC_B1)
+    return fail(h, HDC_ERR_INVALID_ARG, "encode_rp: precision");
+  if (p_dtype == HDC_I8 && k->precision != HDC_I8)
+    return fail(h, HDC_ERR_INVALID_ARG, "encode_rp: int8 P needs precision HDC_I8");
+  const size_t xa = x_dtype == HDC_BF16 ? 2 : 4, pa = p_dtype == HDC_BF16 ? 2 : (p_dtype == HDC_I8 ? 1 : 4);
+  if ((reinterpret_cast<uintptr_t>(X) % xa) || (reinterpret_cast<uintptr_t>(P) % pa))
+    return fail(h, HDC_ERR_ALIGNMENT, "encode_rp: operand not element aligned");
+  return HDC_OK;
+}
+
+extern "C" int32_t hdc_encode_rp(hdc_handle_t h, const void* X, int32_t x_dtype, int64_t N, int32_t F,
+                                 int64_t ldx, const void* P, int32_t p_dtype, int32_t D, int64_t ldp,
+                                 const hdc_knobs_t* knobs, int32_t out_kinds, uint32_t* Hbits,
+                                 int64_t ldh_words, void* Hraw, int64_t ldraw, void* ws, size_t ws_bytes,
+                                 void* stream) {
+  if (!h) return HDC_ERR_INVALID_ARG;
+  int rc = check_encode_rp_args(h, X, x_dtype, N, F, ldx, P, p_dtype, D, ldp, knobs);
+  if (rc) return rc;
+  if (!(out_kinds & HDC_OUT_BITS) || !Hbits) return fail(h, HDC_ERR_INVALID_ARG, "encode_rp: Hbits required");
+  if (ldh_words < words_of(knobs->D_eff)) return fail(h, HDC_ERR_INVALID_ARG, "encode_rp: ldh_words < W");
+  if ((out_kinds & HDC_OUT_RAW) && (!Hraw || ldraw < knobs->D_eff))
+    return fail(h, HDC_ERR_INVALID_ARG, "encode_rp: Hraw / ldraw");
+  if (reinterpret_cast<uintptr_t>(Hbits) & 3) return fail(h, HDC_ERR_ALIGNMENT, "encode_rp: Hbits alignment");
+  if (N == 0) return HDC_OK;
+  Bump b(ws);
+  if (!ws) ws_bytes = 0;
+  return do_encode_rp(h, X, x_dtype, N, F, ldx, P, p_dtype, D, ldp, knobs, out_kinds, Hbits, ldh_words, Hraw,
+                      ldraw, b, ws_bytes, (cudaStream_t)stream);
+}
+
+// =================================================================================== (1b)
+extern "C" int32_t hdc_encode_levelid(hdc_handle_t h, const uint8_t* levels, int64_t N, int32_t F,
+                                      int64_t ldl, const uint32_t* IDbits, int64_t ldid_words,
+                                      const uint32_t* LVbits, int32_t Q, int64_t ldlv_words, int32_t D,
+                                      const hdc_knobs_t* knobs, uint32_t* Hbits, int64_t ldh_words, void* ws,
+                                      size_t ws_bytes, void* stream) {
+  (void)ws;
+  (void)ws_bytes;
+  if (!h) return HDC_ERR_INVALID_ARG;
+  if (!levels || !IDbits || !LVbits || !Hbits) return fail(h, HDC_ERR_INVALID_ARG, "encode_levelid: NULL pointer");
+  if (N < 0 || F < 1 || F > 65535 || Q < 1 || Q > 256 || D < 1 || ldl < F)
+    return fail(h, HDC_ERR_INVALID_ARG, "encode_levelid: bad sizes");
+  int rc = check_knobs(h, knobs, D);
+  if (rc) return rc;
+  const int W = words_of(knobs->D_eff);
+  if (ldid_words < W || ldlv_words < W || ldh_words < W)
+    return fail(h, HDC_ERR_INVALID_ARG, "encode_levelid: leading dimension < W");
+  if ((reinterpret_cast<uintptr_t>(IDbits) | reinterpret_cast<uintptr_t>(LVbits) |
+       reinterpret_cast<uintptr_t>(Hbits)) & 3)
+    return fail(h, HDC_ERR_ALIGNMENT, "encode_levelid: bit matrices must be 4-byte aligned");
+  if (N == 0) return HDC_OK;
+  cudaError_t ce = launch_levelid(levels, N, F, ldl, IDbits, ldid_words, LVbits, Q, ldlv_words, knobs->D_eff,
+                                  Hbits, ldh_words, h->sm_count, h->smem_optin, (cudaStream_t)stream,
+                                  &h->launches);
+  return ce == cudaSuccess ? HDC_OK : cuda_fail(h, ce, "encode_levelid");
+}
+
+// =================================================================================== (2), (2+3a)
+static int check_sim_args(hdc_ctx* h, const uint32_t* Hbits, int64_t N, int64_t ldh, const float* C_acc,
+                          int K, int64_t ldc, int D, const hdc_knobs_t* k) {
+  if (!Hbits || !C_acc) return fail(h, HDC_ERR_INVALID_ARG, "similarity: NULL operand");
+  if (N < 0 || K < 1 || K > 65535 || D < 1 || ldc < D) return fail(h, HDC_ERR_INVALID_ARG, "similarity: bad sizes");
+  int rc = check_knobs(h, k, D);
+  if (rc) return rc;
+  rc = check_sim_knobs(h, k);
+  if (rc) return rc;
+  if (ldh < words_of(k->D_eff)) return fail(h, HDC_ERR_INVALID_ARG, "similarity: ldh_words < W");
+  if ((reinterpret_cast<uintptr_t>(Hbits) | reinterpret_cast<uintptr_t>(C_acc)) & 3)
+    return fail(h, HDC_ERR_ALIGNMENT, "similarity: operands must be 4-byte aligned");
+  return HDC_OK;
+}
+
+extern "C" int32_t hdc_similarity(hdc_handle_t h, const uint32_t* Hbits, int64_t N, int64_t ldh_words,
+                                  const float* C_acc, int32_t K, int64_t ldc, int32_t D,
+                                  const hdc_knobs_t* knobs, void* S, int32_t s_dtype, int64_t lds, void* ws,
+                                  size_t ws_bytes, void* stream) {
+  if (!h) return HDC_ERR_INVALID_ARG;
+  int rc = check_sim_args(h, Hbits, N, ldh_words, C_acc, K, ldc, D, knobs);
+  if (rc) return rc;
+  if (!S || lds < K) return fail(h, HDC_ERR_INVALID_ARG, "similarity: S / lds");
+  if (knobs->sim == HDC_SIM_HAMMING && s_dtype != HDC_I32)
+    return fail(h, HDC_ERR_INVALID_ARG, "similarity: HAMMING writes int32");
+  if (knobs->sim == HDC_SIM_COS && s_dtype != HDC_F32) return fail(h, HDC_ERR_INVALID_ARG, "similarity: COS writes fp32");
+  if (knobs->sim == HDC_SIM_DOT) {
+    if (s_dtype != HDC_F32 && s_dtype != HDC_I32) return fail(h, HDC_ERR_INVALID_ARG, "similarity: s_dtype");
+    if (s_dtype == HDC_I32 && knobs->hv_bits != 8 && knobs->hv_bits != 1)
+      return fail(h, HDC_ERR_INVALID_ARG, "similarity: int32 DOT needs hv_bits 8 or 1");
+  }
+  if (N == 0) return HDC_OK;
+  Bump b(ws);
+  if (!ws) ws_bytes = 0;
+  return do_similarity(h, Hbits, N, ldh_words, C_acc, K, ldc, knobs, S, s_dtype == HDC_I32, lds, nullptr,
+                       nullptr, nullptr, b, ws_bytes, (cudaStream_t)stream);
+}
+
+extern "C" int32_t hdc_classify(hdc_handle_t h, const uint32_t* Hbits, int64_t N, int64_t ldh_words,
+                                const float* C_acc, int32_t K, int64_t ldc, int32_t D,
+                                const hdc_knobs_t* knobs, int32_t* labels, float* best, float* second,
+                                void* ws, size_t ws_bytes, void* stream) {
+  if (!h) return HDC_ERR_INVALID_ARG;
+  int rc = check_sim_args(h, Hbits, N, ldh_words, C_acc, K, ldc, D, knobs);
+  if (rc) return rc;
+  if (!labels) return fail(h, HDC_ERR_INVALID_ARG, "classify: labels is NULL");
+  if (N == 0) return HDC_OK;
+  Bump b(ws);
+  if (!ws) ws_bytes = 0;
+  return do_similarity(h, Hbits, N, ldh_words, C_acc, K, ldc, knobs, nullptr, 0, 0, labels, best, second, b,
+                       ws_bytes, (cudaStream_t)stream);
+}
+
+// =================================================================================== (3b, 3c)
+extern "C" int32_t hdc_train_epoch(hdc_handle_t h, int32_t mode, const uint32_t* Hbits, int64_t N,
+                                   int64_t ldh_words, const int32_t* y, float* C_acc, int32_t K, int64_t ldc,
+                                   int32_t D, const hdc_knobs_t* knobs, float lr, int64_t batch, int32_t* pred,
+                                   unsigned long long* n_wrong, void* ws, size_t ws_bytes, void* stream) {
+  if (!h) return HDC_ERR_INVALID_ARG;
+  if (mode != HDC_TRAIN_BUNDLE && mode != HDC_TRAIN_PERCEPTRON) return fail(h, HDC_ERR_INVALID_ARG, "train: mode");
+  if (!y) return fail(h, HDC_ERR_INVALID_ARG, "train: y is NULL");
+  if (batch < 0) return fail(h, HDC_ERR_INVALID_ARG, "train: batch < 0");
+  hdc_knobs_t k;
+  if (!knobs) return fail(h, HDC_ERR_INVALID_ARG, "knobs is NULL");
+  k = *knobs;
+  if (mode == HDC_TRAIN_BUNDLE) {  // only D_eff matters
+    k.hv_bits = 32;
+    k.sim = HDC_SIM_DOT;
+  }
+  int rc = check_sim_args(h, Hbits, N, ldh_words, C_acc, K, ldc, D, &k);
+  if (rc) return rc;
+  if (N == 0) return HDC_OK;
+  cudaStream_t st = (cudaStream_t)stream;
+  Bump b(ws);
+  if (!ws) ws_bytes = 0;
+  int32_t* delta = b.take<int32_t>((size_t)K * words_of(k.D_eff) * 32);
+  if (b.off > ws_bytes) return fail(h, HDC_ERR_WORKSPACE, "train: workspace too small");
+  cudaError_t ce;
+  if (mode == HDC_TRAIN_BUNDLE) {
+    ce = launch_class_update(Hbits, 0, N, ldh_words, y, nullptr, C_acc, K, ldc, k.D_eff, 1.0f, delta, nullptr,
+                             h->sm_count, st, &h->launches);
+    return ce == cudaSuccess ? HDC_OK : cuda_fail(h, ce, "bundle");
+  }
+  const int64_t B = (batch == 0 || batch > N) ? N : batch;
+  int32_t* pbuf = pred;
+  if (!pbuf) pbuf = b.take<int32_t>((size_t)B);
+  if (b.off > ws_bytes) return fail(h, HDC_ERR_WORKSPACE, "train: workspace too small");
+  const size_t base_off = b.off;
+  for (int64_t n0 = 0; n0 < N; n0 += B) {
+    const int64_t nb = (N - n0 < B) ? (N - n0) : B;
+    int32_t* pb = pred ? pred + n0 : pbuf;
+    Bump bs(ws);
+    bs.off = base_off;
+    rc = do_similarity(h, Hbits + n0 * ldh_words, nb, ldh_words, C_acc, K, ldc, &k, nullptr, 0, 0, pb, nullptr,
+                       nullptr, bs, ws_bytes, st);
+    if (rc) return rc;
+    // class_update indexes y and pred with absolute sample numbers
+    ce = launch_class_update(Hbits, n0, nb, ldh_words, y, pb - n0, C_acc, K, ldc, k.D_eff, lr, delta, n_wrong,
+                             h->sm_count, st, &h->launches);
+    if (ce != cudaSuccess) return cuda_fail(h, ce, "class update");
+  }
+  return HDC_OK;
+}
+
+// =================================================================================== host end-to-end
+extern "C" int32_t hdc_infer_rp_host(hdc_handle_t h, const void* X_host, int32_t x_dtype, int64_t N, int32_t F,
+                                     int64_t ldx, const void* P, int32_t p_dtype, int32_t D, int64_t ldp,
+                                     const float* C_acc, int32_t K, int64_t ldc, const hdc_knobs_t* knobs,
+                                     int32_t* labels_host, void* ws, size_t ws_bytes, void* stream) {
+  if (!h) return HDC_ERR_INVALID_ARG;
+  int rc = check_encode_rp_args(h, X_host, x_dtype, N, F, ldx, P, p_dtype, D, ldp, knobs);
+  if (rc) return rc;
+  if (!C_acc || !labels_host) return fail(h, HDC_ERR_INVALID_ARG, "infer_rp_host: NULL pointer");
+  if (K < 1 || K > 65535 || ldc < D) return fail(h, HDC_ERR_INVALID_ARG, "infer_rp_host: bad sizes");
+  rc = check_sim_knobs(h, knobs);
+  if (rc) return rc;
+  if (N == 0) return HDC_OK;
+  cudaStream_t st = (cudaStream_t)stream;
+  const size_t es = x_dtype == HDC_BF16 ? 2 : 4;
+  const int64_t chunk = N < HOST_CHUNK ? N : HOST_CHUNK;
+  const int W = words_of(knobs->D_eff);
+  Bump b(ws);
+  if (!ws) ws_bytes = 0;
+  char* Xd[2];
+  Xd[0] = (char*)b.take<float>((size_t)chunk * F);
+  Xd[1] = (char*)b.take<float>((size_t)chunk * F);
+  uint32_t* Hd = b.take<uint32_t>((size_t)chunk * W);
+  int32_t* Ld = b.take<int32_t>((size_t)N);
+  if (b.off > ws_bytes) return fail(h, HDC_ERR_WORKSPACE, "infer_rp_host: workspace too small");
+  const size_t base_off = b.off;
+  cudaError_t ce = cudaEventRecord(h->ev_entry, st);
+  if (ce == cudaSuccess) ce = cudaStreamWaitEvent(h->copy_stream, h->ev_entry, 0);
+  if (ce != cudaSuccess) return cuda_fail(h, ce, "infer_rp_host: entry");
+  int64_t c = 0;
+  for (int64_t n0 = 0; n0 < N; n0 += chunk, ++c) {
+    const int64_t nb = (N - n0 < chunk) ? (N - n0) : chunk;
+    const int buf = (int)(c & 1);
+    if (c >= 2) cudaStreamWaitEvent(h->copy_stream, h->ev_done[buf], 0);
+    // rows are copied densely: device leading dimension is F
+    ce = cudaMemcpy2DAsync(Xd[buf], (size_t)F * es, (const char*)X_host + (size_t)n0 * ldx * es,
+                           (size_t)ldx * es, (size_t)F * es, (size_t)nb, cudaMemcpyHostToDevice,
+                           h->copy_stream);
+    if (ce != cudaSuccess) return cuda_fail(h, ce, "infer_rp_host: H2D");
+    cudaEventRecord(h->ev_copied[buf], h->copy_stream);
+    cudaStreamWaitEvent(st, h->ev_copied[buf], 0);
+    Bump be(ws);
+    be.off = base_off;
+    rc = do_encode_rp(h, Xd[buf], x_dtype, nb, F, F, P, p_dtype, D, ldp, knobs, HDC_OUT_BITS, Hd, W, nullptr, 0,
+                      be, ws_bytes, st);
+    if (rc) return rc;
+    rc = do_similarity(h, Hd, nb, W, C_acc, K, ldc, knobs, nullptr, 0, 0, Ld + n0, nullptr, nullptr, be,
+                       ws_bytes, st);
+    if (rc) return rc;
+    cudaEventRecord(h->ev_done[buf], st);
+  }
+  ce = cudaMemcpyAsync(labels_host, Ld, sizeof(int32_t) * (size_t)N, cudaMemcpyDeviceToHost, st);
+  if (ce != cudaSuccess) return cuda_fail(h, ce, "infer_rp_host: D2H");
+  ce = cudaStreamSynchronize(st);
+  if (ce != cudaSuccess) return cuda_fail(h, ce, "infer_rp_host: sync");
+  return HDC_OK;
+}

@@ -1,0 +1,103 @@
+// common.cuh -- internal declarations shared by the translation units of libhdc.so (sm_100a only).
+// Nothing here is part of the public ABI (include/hdc.h is).  No code is shared with oracle/.
+#pragma once
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "hdc.h"
+
+namespace hdc {
+
+// ---- operand kinds of the contraction loaders (device-side view of a matrix element) ----------
+enum OperandKind : int {
+  OPK_F32 = 0,        // float
+  OPK_BF16 = 1,       // __nv_bfloat16, widened exactly
+  OPK_F32_RBF16 = 2,  // float rounded to nearest-even bf16 on load (precision BF16 / hv_bits 16)
+  OPK_BITS = 3,       // packed hypervector bits: element k -> bit k&31 of word k>>5, value 1-2*bit
+  OPK_I8 = 4          // int8
+};
+
+struct Operand {
+  const void* p;
+  int64_t ld;  // in elements (words for OPK_BITS)
+  int kind;
+};
+
+enum EpilogueKind : int { EPI_SIGN = 0, EPI_SCORE = 1, EPI_ARGMAX = 2 };
+
+// Epilogue of C[m,n] = sum_k A[m,k] * B[n,k]
+struct Epilogue {
+  int kind;
+  // EPI_SIGN: bit[m,n] = [acc < 0] packed into bits[m][n>>5]; optional raw accumulators
+  uint32_t* bits;
+  int64_t ldbits;
+  void* raw;  // float* (float accumulate) or int32_t* (integer accumulate), nullable
+  int64_t ldraw;
+  // EPI_SCORE: S[m,n] = acc * colscale[n] (colscale nullable => 1); s_i32 => store as int32
+  void* S;
+  int64_t lds;
+  int s_i32;
+  const double* colscale;
+  // EPI_ARGMAX: label = argmax_n acc*colscale[n], ties to lowest n; best/second nullable.
+  // ham_D > 0: report best/second as Hamming distances (ham_D - dot)/2 (bits x bits).
+  int32_t* labels;
+  float* best;
+  float* second;
+  int ham_D;
+};
+
+// ---- launchers (each returns the CUDA error of its launches and adds to *nlaunch) -------------
+cudaError_t launch_gemm_simt(const Operand& A, const Operand& B, int64_t M, int Nc, int Kr,
+                             bool int_acc, const Epilogue& e, cudaStream_t st, int64_t* nlaunch);
+
+// tcgen05 path (gemm_tc.cu).  A and B must be K-contiguous bf16 (or int8) with Kr padded to a
+// multiple of 64 bytes*... see gemm_tc.cu.  Returns cudaErrorNotSupported when shapes do not fit.
+struct TcContext;  // opaque: holds the cuTensorMapEncodeTiled entry point
+TcContext* tc_context_create();
+void tc_context_destroy(TcContext*);
+cudaError_t launch_gemm_tc(TcContext* tc, const void* A, const void* B, int elem_kind /*OPK_BF16|OPK_I8*/,
+                           int64_t M, int Nc, int Kr_padded, int64_t lda, int64_t ldb,
+                           const Epilogue& e, int sm_count, cudaStream_t st, int64_t* nlaunch);
+
+// fp32/bf16 -> bf16 staging with zero padding of the reduction axis: dst [rows][ld_dst]
+cudaError_t launch_convert_bf16(const void* src, int src_kind, int64_t rows, int cols, int64_t ld_src,
+                                __nv_bfloat16* dst, int64_t ld_dst, cudaStream_t st, int64_t* nlaunch);
+// per-row symmetric int8 quantisation (S1/A7): dst [rows][ld_dst] int8, zero padded
+cudaError_t launch_quantize_rows_i8(const void* src, int src_kind, int64_t rows, int cols, int64_t ld_src,
+                                    int8_t* dst, int64_t ld_dst, cudaStream_t st, int64_t* nlaunch);
+// per-tensor symmetric int8 of C_acc[k<K][d<D_eff] (S5): amax_scratch is one float in ws
+cudaError_t launch_quantize_tensor_i8(const float* C, int K, int D_eff, int64_t ldc, int8_t* dst,
+                                      int64_t ld_dst, float* amax_scratch, cudaStream_t st,
+                                      int64_t* nlaunch);
+// sign bits of C_acc: cbits [K][W] (tail bits zero)
+cudaError_t launch_sign_bits(const float* C, int K, int D_eff, int64_t ldc, uint32_t* cbits, int W,
+                             cudaStream_t st, int64_t* nlaunch);
+// colscale[k] = cos ? (nrm_k > 0 ? 1/(sqrt(D_eff)*nrm_k) : 0) : 1, nrm over the operand as loaded
+cudaError_t launch_col_scale(const Operand& C, int K, int D_eff, int cos, double* colscale,
+                             cudaStream_t st, int64_t* nlaunch);
+
+// packed XOR+popcount similarity with class bits in shared memory (hamming.cu)
+bool hamming_smem_fits(int K, int W, int smem_optin);
+cudaError_t launch_hamming(const uint32_t* Hbits, int64_t N, int64_t ldh, const uint32_t* Cbits, int K,
+                           int W, int D_eff, int32_t* dist, int64_t lds, int32_t* labels, float* best,
+                           float* second, int sm_count, int smem_optin, cudaStream_t st,
+                           int64_t* nlaunch);
+
+// level-ID encode (levelid.cu)
+cudaError_t launch_levelid(const uint8_t* levels, int64_t N, int F, int64_t ldl, const uint32_t* ID,
+                           int64_t ldid, const uint32_t* LV, int Q, int64_t ldlv, int D_eff,
+                           uint32_t* Hbits, int64_t ldh, int sm_count, int smem_optin, cudaStream_t st,
+                           int64_t* nlaunch);
+
+// class update (train.cu): delta int32 [K][W*32] workspace
+cudaError_t launch_class_update(const uint32_t* Hbits, int64_t n0, int64_t nb, int64_t ldh,
+                                const int32_t* y, const int32_t* pred /*null => bundle*/, float* C_acc,
+                                int K, int64_t ldc, int D_eff, float lr, int32_t* delta,
+                                unsigned long long* n_wrong, int sm_count, cudaStream_t st,
+                                int64_t* nlaunch);
+
+static inline int64_t round_up(int64_t x, int64_t m) { return (x + m - 1) / m * m; }
+static inline int words_of(int D_eff) { return (D_eff + 31) >> 5; }
+
+}  // namespace hdc

@@ -1,0 +1,224 @@
+// convert.cu -- operand preparation kernels ("element type representation"; DESIGN.md
+// readings S1, S5, A7): fp32 -> bf16 staging, per-row / per-tensor symmetric int8 quantisation,
+// sign bits of the class accumulators, cosine column scales.  All HBM-bound elementwise / row
+// reductions; every rounding step is a single correctly rounded fp32 operation (__fdiv_rn,
+// __fmul_rn, rintf) so that the integers produced are the ones the definition fixes.
+#include "common.cuh"
+
+namespace hdc {
+namespace {
+
+__device__ __forceinline__ float load_as_f32(const void* p, int kind, int64_t idx) {
+  if (kind == OPK_BF16) return __bfloat162float(((const __nv_bfloat16*)p)[idx]);
+  return __ldg((const float*)p + idx);
+}
+
+// ---------------------------------------------------------------------------------- bf16 staging
+// One thread produces 8 consecutive bf16 (one 16-byte store); columns >= cols are zero.
+__global__ void convert_bf16_kernel(const void* __restrict__ src, int src_kind, int64_t rows, int cols,
+                                    int64_t ld_src, __nv_bfloat16* __restrict__ dst, int64_t ld_dst) {
+  const int chunks = (int)(ld_dst >> 3);
+  const int64_t total = rows * chunks;
+  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < total;
+       i += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t r = i / chunks;
+    const int c0 = (int)(i - r * chunks) << 3;
+    __align__(16) __nv_bfloat16 v[8];
+    const int64_t base = r * ld_src + c0;
+    if (src_kind == OPK_F32 && c0 + 8 <= cols && ((ld_src & 3) == 0) &&
+        ((reinterpret_cast<uintptr_t>(src) & 15) == 0)) {
+      const float4 a = __ldg(reinterpret_cast<const float4*>((const float*)src + base));
+      const float4 b = __ldg(reinterpret_cast<const float4*>((const float*)src + base) + 1);
+      v[0] = __float2bfloat16_rn(a.x); v[1] = __float2bfloat16_rn(a.y);
+      v[2] = __float2bfloat16_rn(a.z); v[3] = __float2bfloat16_rn(a.w);
+      v[4] = __float2bfloat16_rn(b.x); v[5] = __float2bfloat16_rn(b.y);
+      v[6] = __float2bfloat16_rn(b.z); v[7] = __float2bfloat16_rn(b.w);
+    } else {
+#pragma unroll
+      for (int j = 0; j < 8; ++j)
+        v[j] = (c0 + j < cols) ? __float2bfloat16_rn(load_as_f32(src, src_kind, base + j))
+                               : __float2bfloat16_rn(0.0f);
+    }
+    *reinterpret_cast<uint4*>(dst + r * ld_dst + c0) = *reinterpret_cast<const uint4*>(v);
+  }
+}
+
+// ---------------------------------------------------------------------------------- int8 per row
+__device__ __forceinline__ int quant_i8(float x, float s) {
+  float q = rintf(__fmul_rn(x, s));  // round-half-even, one rounded multiply (no FMA contraction)
+  q = fminf(fmaxf(q, -127.0f), 127.0f);
+  return (int)q;
+}
+
+// One warp per row: a = max|x|, s = fl32(127/a) (1 if a == 0), q = clamp(rint(fl32(x*s)), +-127).
+__global__ void quantize_rows_i8_kernel(const void* __restrict__ src, int src_kind, int64_t rows, int cols,
+                                        int64_t ld_src, int8_t* __restrict__ dst, int64_t ld_dst) {
+  const int lane = threadIdx.x & 31;
+  const int64_t warp = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
+  const int64_t nwarps = ((int64_t)gridDim.x * blockDim.x) >> 5;
+  for (int64_t r = warp; r < rows; r += nwarps) {
+    float a = 0.0f;
+    for (int c = lane; c < cols; c += 32) a = fmaxf(a, fabsf(load_as_f32(src, src_kind, r * ld_src + c)));
+#pragma unroll
+    for (int off = 16; off; off >>= 1) a = fmaxf(a, __shfl_xor_sync(0xffffffffu, a, off));
+    const float s = a > 0.0f ? __fdiv_rn(127.0f, a) : 1.0f;
+    for (int c = lane; c < (int)ld_dst; c += 32) {
+      int q = 0;
+      if (c < cols) q = quant_i8(load_as_f32(src, src_kind, r * ld_src + c), s);
+      dst[r * ld_dst + c] = (int8_t)q;
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------- int8 per tensor
+// max |C[k][d]| over k < K, d < D_eff; non-negative floats order as unsigned ints.
+__global__ void tensor_amax_kernel(const float* __restrict__ C, int K, int D_eff, int64_t ldc,
+                                   float* __restrict__ amax) {
+  float a = 0.0f;
+  const int64_t total = (int64_t)K * D_eff;
+  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < total;
+       i += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t k = i / D_eff;
+    const int d = (int)(i - k * D_eff);
+    a = fmaxf(a, fabsf(__ldg(C + k * ldc + d)));
+  }
+#pragma unroll
+  for (int off = 16; off; off >>= 1) a = fmaxf(a, __shfl_xor_sync(0xffffffffu, a, off));
+  if ((threadIdx.x & 31) == 0) atomicMax(reinterpret_cast<unsigned int*>(amax), __float_as_uint(a));
+}
+
+__global__ void quantize_tensor_i8_kernel(const float* __restrict__ C, int K, int D_eff, int64_t ldc,
+                                          int8_t* __restrict__ dst, int64_t ld_dst,
+                                          const float* __restrict__ amax) {
+  const float a = *amax;
+  const float s = a > 0.0f ? __fdiv_rn(127.0f, a) : 1.0f;
+  const int64_t total = (int64_t)K * ld_dst;
+  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < total;
+       i += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t k = i / ld_dst;
+    const int d = (int)(i - k * ld_dst);
+    dst[i] = (int8_t)(d < D_eff ? quant_i8(__ldg(C + k * ldc + d), s) : 0);
+  }
+}
+
+// ---------------------------------------------------------------------------------- sign bits
+// One warp produces 32 words (1024 dims) of one class row: coalesced loads, one ballot per word.
+__global__ void sign_bits_kernel(const float* __restrict__ C, int K, int D_eff, int64_t ldc,
+                                 uint32_t* __restrict__ cbits, int W) {
+  const int lane = threadIdx.x & 31;
+  const int groups = (W + 31) >> 5;
+  const int64_t warp = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
+  if (warp >= (int64_t)K * groups) return;
+  const int k = (int)(warp / groups);
+  const int g = (int)(warp - (int64_t)k * groups);
+  uint32_t mine = 0;
+#pragma unroll 4
+  for (int i = 0; i < 32; ++i) {
+    const int d = (g * 32 + i) * 32 + lane;
+    const float v = d < D_eff ? __ldg(C + (int64_t)k * ldc + d) : 0.0f;
+    const uint32_t b = __ballot_sync(0xffffffffu, v < 0.0f);
+    if (i == lane) mine = b;
+  }
+  const int w = g * 32 + lane;
+  if (w < W) cbits[(int64_t)k * W + w] = mine;
+}
+
+// ---------------------------------------------------------------------------------- cosine scales
+// colscale[k] = cos ? (nrm > 0 ? 1 / (sqrt(D_eff) * nrm) : 0) : 1, nrm^2 = sum_d c[k,d]^2 in double
+// over the operand as the contraction loads it.  One block per class, fixed reduction order.
+__global__ void col_scale_kernel(Operand C, int K, int D_eff, int cos, double* __restrict__ colscale) {
+  const int k = blockIdx.x;
+  __shared__ double part[8];
+  double s = 0.0;
+  if (cos) {
+    for (int d = threadIdx.x; d < D_eff; d += blockDim.x) {
+      double v;
+      const int64_t idx = (int64_t)k * C.ld + d;
+      switch (C.kind) {
+        case OPK_F32: v = (double)__ldg((const float*)C.p + idx); break;
+        case OPK_BF16: v = (double)__bfloat162float(((const __nv_bfloat16*)C.p)[idx]); break;
+        case OPK_F32_RBF16:
+          v = (double)__bfloat162float(__float2bfloat16_rn(__ldg((const float*)C.p + idx)));
+          break;
+        case OPK_BITS: v = 1.0; break;
+        default: v = (double)((const int8_t*)C.p)[idx]; break;
+      }
+      s += v * v;
+    }
+#pragma unroll
+    for (int off = 16; off; off >>= 1) s += __shfl_xor_sync(0xffffffffu, s, off);
+    if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = s;
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) {
+    if (!cos) {
+      colscale[k] = 1.0;
+    } else {
+      double t = 0.0;
+      for (int i = 0; i < (int)(blockDim.x >> 5); ++i) t += part[i];
+      const double nrm = sqrt(t);
+      colscale[k] = nrm > 0.0 ? 1.0 / (sqrt((double)D_eff) * nrm) : 0.0;
+    }
+  }
+}
+
+inline int grid_for(int64_t work_items, int threads, int cap) {
+  int64_t g = (work_items + threads - 1) / threads;
+  if (g < 1) g = 1;
+  if (g > cap) g = cap;
+  return (int)g;
+}
+
+}  // namespace
+
+cudaError_t launch_convert_bf16(const void* src, int src_kind, int64_t rows, int cols, int64_t ld_src,
+                                __nv_bfloat16* dst, int64_t ld_dst, cudaStream_t st, int64_t* nlaunch) {
+  if (rows <= 0) return cudaSuccess;
+  const int64_t total = rows * (ld_dst >> 3);
+  convert_bf16_kernel<<<grid_for(total, 256, 148 * 16), 256, 0, st>>>(src, src_kind, rows, cols, ld_src,
+                                                                     dst, ld_dst);
+  ++*nlaunch;
+  return cudaGetLastError();
+}
+
+cudaError_t launch_quantize_rows_i8(const void* src, int src_kind, int64_t rows, int cols, int64_t ld_src,
+                                    int8_t* dst, int64_t ld_dst, cudaStream_t st, int64_t* nlaunch) {
+  if (rows <= 0) return cudaSuccess;
+  quantize_rows_i8_kernel<<<grid_for(rows * 32, 256, 148 * 16), 256, 0, st>>>(src, src_kind, rows, cols,
+                                                                             ld_src, dst, ld_dst);
+  ++*nlaunch;
+  return cudaGetLastError();
+}
+
+cudaError_t launch_quantize_tensor_i8(const float* C, int K, int D_eff, int64_t ldc, int8_t* dst,
+                                      int64_t ld_dst, float* amax_scratch, cudaStream_t st,
+                                      int64_t* nlaunch) {
+  cudaError_t e = cudaMemsetAsync(amax_scratch, 0, sizeof(float), st);
+  if (e != cudaSuccess) return e;
+  tensor_amax_kernel<<<grid_for((int64_t)K * D_eff, 256, 148 * 4), 256, 0, st>>>(C, K, D_eff, ldc,
+                                                                                amax_scratch);
+  ++*nlaunch;
+  e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  quantize_tensor_i8_kernel<<<grid_for((int64_t)K * ld_dst, 256, 148 * 8), 256, 0, st>>>(
+      C, K, D_eff, ldc, dst, ld_dst, amax_scratch);
+  ++*nlaunch;
+  return cudaGetLastError();
+}
+
+cudaError_t launch_sign_bits(const float* C, int K, int D_eff, int64_t ldc, uint32_t* cbits, int W,
+                             cudaStream_t st, int64_t* nlaunch) {
+  const int64_t warps = (int64_t)K * ((W + 31) >> 5);
+  sign_bits_kernel<<<(unsigned)((warps * 32 + 255) / 256), 256, 0, st>>>(C, K, D_eff, ldc, cbits, W);
+  ++*nlaunch;
+  return cudaGetLastError();
+}
+
+cudaError_t launch_col_scale(const Operand& C, int K, int D_eff, int cos, double* colscale,
+                             cudaStream_t st, int64_t* nlaunch) {
+  col_scale_kernel<<<K, 256, 0, st>>>(C, K, D_eff, cos, colscale);
+  ++*nlaunch;
+  return cudaGetLastError();
+}
+
+}  // namespace hdc

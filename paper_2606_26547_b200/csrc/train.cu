@@ -1,0 +1,129 @@
+// train.cu -- class-hypervector update ("vector addition" of same-class hypervectors;
+// L181 TRAIN_ITERATIONS; perceptron-style rule = DESIGN.md reading S9/A9):
+//
+//   bundle      Delta[k,d] = sum_{n: y_n = k} v[n,d]
+//   perceptron  Delta[k,d] = sum_{n: yhat_n != y_n} ([k = y_n] - [k = yhat_n]) * v[n,d]
+//   then        C_acc[k,d] = fl32( C_acc[k,d] + fl32( lr * (float)Delta[k,d] ) )      (two rounded ops)
+//
+// with v = 1 - 2*bit.  Delta is an exact int32 segmented reduction per class: a CTA owns (class k,
+// 128 word-columns, a segment of the samples); a thread owns one word-column and 32 signed counters
+// in registers, walks its sample segment (label reads are warp-uniform broadcasts, word reads are
+// coalesced) and finally adds its 32 partial sums into Delta with integer atomics -- integer
+// addition commutes, so the result is deterministic; there are no floating-point atomics.
+#include "common.cuh"
+
+namespace hdc {
+namespace {
+
+constexpr int WT = 128;  // word-columns per CTA
+
+__global__ void __launch_bounds__(WT)
+class_delta_kernel(const uint32_t* __restrict__ Hbits, int64_t n0, int64_t nb, int64_t ldh,
+                   const int32_t* __restrict__ y, const int32_t* __restrict__ pred, int W,
+                   int32_t* __restrict__ delta, int64_t ldd, int64_t seg_len) {
+  const int k = blockIdx.y;
+  const int w = blockIdx.x * WT + threadIdx.x;
+  const int64_t s0 = n0 + (int64_t)blockIdx.z * seg_len;
+  int64_t s1 = s0 + seg_len;
+  if (s1 > n0 + nb) s1 = n0 + nb;
+  int cnt[32];
+#pragma unroll
+  for (int b = 0; b < 32; ++b) cnt[b] = 0;
+  int m = 0;  // signed number of contributing samples
+  for (int64_t n = s0; n < s1; ++n) {
+    const int yn = __ldg(y + n);
+    int s;
+    if (pred) {
+      const int pn = __ldg(pred + n);
+      s = (pn != yn) ? ((yn == k) - (pn == k)) : 0;
+    } else {
+      s = (yn == k);
+    }
+    if (s == 0) continue;  // uniform across the CTA
+    const uint32_t word = (w < W) ? __ldg(Hbits + n * ldh + w) : 0u;
+    m += s;
+#pragma unroll
+    for (int b = 0; b < 32; ++b) cnt[b] += s * (int)((word >> b) & 1u);
+  }
+  if (w < W) {
+    int32_t* out = delta + (int64_t)k * ldd + (int64_t)w * 32;
+#pragma unroll
+    for (int b = 0; b < 32; ++b) {
+      const int v = m - 2 * cnt[b];
+      if (v != 0) atomicAdd(out + b, v);
+    }
+  }
+}
+
+__global__ void apply_update_kernel(float* __restrict__ C, int K, int D_eff, int64_t ldc,
+                                    const int32_t* __restrict__ delta, int64_t ldd, float lr) {
+  const int64_t total = (int64_t)K * D_eff;
+  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < total;
+       i += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t k = i / D_eff;
+    const int d = (int)(i - k * D_eff);
+    const int dv = delta[k * ldd + d];
+    if (dv != 0) {
+      float* c = C + k * ldc + d;
+      *c = __fadd_rn(*c, __fmul_rn(lr, (float)dv));
+    }
+  }
+}
+
+__global__ void count_wrong_kernel(const int32_t* __restrict__ y, const int32_t* __restrict__ pred,
+                                   int64_t n0, int64_t nb, unsigned long long* __restrict__ n_wrong) {
+  unsigned int c = 0;
+  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < nb;
+       i += (int64_t)gridDim.x * blockDim.x)
+    c += (y[n0 + i] != pred[n0 + i]);
+#pragma unroll
+  for (int off = 16; off; off >>= 1) c += __shfl_xor_sync(0xffffffffu, c, off);
+  if ((threadIdx.x & 31) == 0 && c) atomicAdd(n_wrong, (unsigned long long)c);
+}
+
+}  // namespace
+
+// delta: int32 [K][W*32] workspace (zeroed here).
+cudaError_t launch_class_update(const uint32_t* Hbits, int64_t n0, int64_t nb, int64_t ldh,
+                                const int32_t* y, const int32_t* pred, float* C_acc, int K,
+                                int64_t ldc, int D_eff, float lr, int32_t* delta,
+                                unsigned long long* n_wrong, int sm_count, cudaStream_t st,
+                                int64_t* nlaunch) {
+  if (nb <= 0) return cudaSuccess;
+  const int W = words_of(D_eff);
+  const int64_t ldd = (int64_t)W * 32;
+  cudaError_t e = cudaMemsetAsync(delta, 0, sizeof(int32_t) * (size_t)K * ldd, st);
+  if (e != cudaSuccess) return e;
+  const int gx = (W + WT - 1) / WT;
+  // split the samples into segments so that about 4 CTAs per SM exist; each segment >= 64 samples
+  int64_t segs = ((int64_t)sm_count * 4 + (int64_t)gx * K - 1) / ((int64_t)gx * K);
+  const int64_t max_segs = (nb + 63) / 64;
+  if (segs > max_segs) segs = max_segs;
+  if (segs < 1) segs = 1;
+  if (segs > 65535) segs = 65535;
+  const int64_t seg_len = (nb + segs - 1) / segs;
+  segs = (nb + seg_len - 1) / seg_len;
+  if (K > 65535) return cudaErrorNotSupported;  // class index is blockIdx.y (checked by the API too)
+  dim3 grid(gx, K, (unsigned)segs);
+  class_delta_kernel<<<grid, WT, 0, st>>>(Hbits, n0, nb, ldh, y, pred, W, delta, ldd, seg_len);
+  ++*nlaunch;
+  e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  const int64_t total = (int64_t)K * D_eff;
+  int64_t g = (total + 255) / 256;
+  if (g > sm_count * 8) g = sm_count * 8;
+  apply_update_kernel<<<(unsigned)g, 256, 0, st>>>(C_acc, K, D_eff, ldc, delta, ldd, lr);
+  ++*nlaunch;
+  e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  if (n_wrong && pred) {
+    int64_t gw = (nb + 255) / 256;
+    if (gw > sm_count * 4) gw = sm_count * 4;
+    count_wrong_kernel<<<(unsigned)gw, 256, 0, st>>>(y, pred, n0, nb, n_wrong);
+    ++*nlaunch;
+    e = cudaGetLastError();
+  }
+  return e;
+}
+
+}  // namespace hdc

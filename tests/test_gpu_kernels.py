@@ -1,0 +1,299 @@
+"""Per-function parity of the CUDA path (through the C ABI) against the CPU oracle -- `-m gpu`.
+Integer / bit paths: bit-exact.  Float paths: the agreement rules of DESIGN.md."""
+from __future__ import annotations
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import hdc_oracle as O
+from workloads import gen
+
+from gpu_util import (check_labels_float, check_scores, check_sign_band, dev, dev_bits, host_bits,
+                      host_words)
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def hd():
+    import paper_2606_26547_b200 as pkg
+    return pkg
+
+
+@pytest.fixture(scope="module")
+def h(hd):
+    hh = hd.Handle(0)
+    yield hh
+    hh.close()
+
+
+def rng(*key):
+    return np.random.default_rng([26547, *key])
+
+
+# ------------------------------------------------------------------------------------ Hamming
+@pytest.mark.parametrize("N,K,D,D_eff", [(1, 1, 32, 32), (300, 4, 2048, 2048), (300, 4, 2048, 1024),
+                                         (257, 26, 10000, 10000), (129, 10, 10000, 4099),
+                                         (77, 40, 4500, 33), (64, 3, 100, 1), (50, 70, 2100, 2047),
+                                         (40, 5, 64, 31)])
+def test_hamming_similarity_and_classify(hd, h, N, K, D, D_eff):
+    r = rng(1, N, K, D_eff)
+    hb = r.integers(0, 2, size=(N, D), dtype=np.uint8)
+    C = r.standard_normal((K, D)).astype(np.float32)
+    C[r.random((K, D)) < 0.05] = 0.0                      # sgn(0) = +1 cases
+    if K > 2:
+        C[2] = C[1]                                        # exact tie between classes 1 and 2
+    kn = hd.knobs(D_eff, hv_bits=1, sim=hd.HDC_SIM_HAMMING)
+    S_or = O.similarity(hb, C, D_eff, O.SIM_HAMMING, 1)
+    lab_or, best_or, sec_or = O.classify(S_or, O.SIM_HAMMING)
+    Hd = dev_bits(hb)                                      # bits beyond D_eff are NOT zero: must be ignored
+    S = h.hdc_similarity(Hd, dev(C), kn).cpu().numpy()
+    assert np.array_equal(S, S_or)
+    lab, best, sec = h.hdc_classify(Hd, dev(C), kn, want_scores=True)
+    assert np.array_equal(lab.cpu().numpy(), lab_or)
+    assert np.array_equal(best.cpu().numpy(), best_or.astype(np.float32))
+    assert np.array_equal(sec.cpu().numpy(), sec_or.astype(np.float32))
+
+
+def test_hamming_padded_leading_dimensions(hd, h):
+    r = rng(2)
+    N, K, D = 100, 7, 1000
+    hb = r.integers(0, 2, size=(N, D), dtype=np.uint8)
+    C = r.standard_normal((K, D + 24)).astype(np.float32)
+    Hd = dev_bits(hb, ld_words=40)
+    kn = hd.knobs(D, hv_bits=1, sim=hd.HDC_SIM_HAMMING)
+    Cd = dev(C)[:, :D]                                     # ldc = D + 24
+    S = h.hdc_similarity(Hd, Cd, kn).cpu().numpy()
+    assert np.array_equal(S, O.similarity(hb, C[:, :D], D, O.SIM_HAMMING, 1))
+
+
+# ------------------------------------------------------------------------------------ level-ID
+@pytest.mark.parametrize("N,F,Q,D,D_eff", [(5, 1, 2, 64, 64), (33, 3, 4, 100, 100), (70, 16, 16, 2048, 2048),
+                                           (70, 17, 256, 1100, 1000), (129, 100, 7, 3000, 2049),
+                                           (40, 784, 256, 10000, 10000), (35, 1030, 256, 200, 33),
+                                           (64, 31, 5, 40, 1)])
+def test_levelid_bit_exact(hd, h, N, F, Q, D, D_eff):
+    r = rng(3, N, F, Q, D_eff)
+    lv = r.integers(0, Q, size=(N, F), dtype=np.uint8)
+    lv[r.random((N, F)) < 0.5] = 0
+    ID = r.integers(0, 2, size=(F, D), dtype=np.uint8)
+    LV = gen.level_table(9, Q, D)
+    bits_or = O.encode_levelid(lv, ID, LV, D_eff)
+    kn = hd.knobs(D_eff)
+    H = h.hdc_encode_levelid(dev(lv), dev_bits(ID), dev_bits(LV), D, kn)
+    assert np.array_equal(host_bits(H, D_eff), bits_or)
+    W = (D_eff + 31) // 32
+    if D_eff % 32:                                          # tail bits of the last word are zero
+        assert (host_words(H)[:, W - 1] >> (D_eff % 32) == 0).all()
+
+
+# ------------------------------------------------------------------------------------ RP encode
+def _encode(hd, h, X, P, D_eff, prec, flags=0, bf16_inputs=False):
+    kn = hd.knobs(D_eff, precision=prec, flags=flags)
+    Xd, Pd = dev(X), dev(P)
+    if bf16_inputs:
+        Xd, Pd = Xd.to(torch.bfloat16), Pd.to(torch.bfloat16)
+    H, raw = h.hdc_encode_rp(Xd, Pd, kn, want_raw=True)
+    torch.cuda.synchronize()
+    return host_bits(H, D_eff), raw.cpu().numpy(), host_words(H)
+
+
+@pytest.mark.parametrize("prec", ["F32", "BF16", "I8", "B1"])
+@pytest.mark.parametrize("flags", [0, 1])
+@pytest.mark.parametrize("N,F,D,D_eff", [(200, 64, 2048, 2048), (131, 617, 1000, 999), (300, 100, 700, 33),
+                                         (3, 7, 40, 40), (520, 784, 520, 515)])
+def test_encode_rp_exact_arithmetic(hd, h, prec, flags, N, F, D, D_eff):
+    """Integer features (0..255) and +-1 projections: every product and partial sum is an integer
+    < 2^24, exact in bf16 operands and fp32 accumulation in any order, so fp32 / bf16 kernels
+    (CUDA-core and tensor-core) must match the oracle bit for bit, sgn(0) cases included."""
+    r = rng(4, N, F, D_eff)
+    X = r.integers(0, 256, size=(N, F)).astype(np.float32)
+    X[r.random((N, F)) < 0.3] = 0
+    X[0] = 0                                                # all-zero row: every acc is 0 -> bit 0
+    P = (1.0 - 2.0 * r.integers(0, 2, size=(D, F))).astype(np.float32)
+    if F % 2 == 0:
+        P[1, ::2], P[1, 1::2] = 1.0, -1.0
+        X[1] = 7.0                                          # acc[1,1] == 0 exactly
+    p = getattr(O, prec)
+    if prec == "I8":
+        X[:, 0] = np.where(X.max(axis=1) > 0, 254.0, 0.0)   # row max 254 -> scale 0.5, ties to even
+    bits_or, acc_or, _ = O.encode_rp(X, P, D_eff, p)
+    bits, raw, words = _encode(hd, h, X, P, D_eff, getattr(hd, "HDC_" + prec), flags)
+    assert np.array_equal(raw.astype(np.float64), acc_or)
+    assert np.array_equal(bits, bits_or)
+    W = (D_eff + 31) // 32
+    if D_eff % 32:
+        assert (words[:, W - 1] >> (D_eff % 32) == 0).all()
+
+
+@pytest.mark.parametrize("prec", ["F32", "BF16", "I8"])
+@pytest.mark.parametrize("flags", [0, 1])
+def test_encode_rp_float_c2_shape(hd, h, prec, flags):
+    """Gaussian features / projection at the C2 shape (F=617, D=10000 sliced): raw accumulators
+    within 1e-3 relative of the float64 oracle; sign mismatches only inside the rounding band."""
+    w = gen.c2_isolet_shaped(D=1500, n_tr=8, n_te=300)
+    X, P, D_eff = w["Xte"], w["P"], 1500
+    p = getattr(O, prec)
+    bits_or, acc_or, absum = O.encode_rp(X, P, D_eff, p, want_absum=True)
+    bits, raw, _ = _encode(hd, h, X, P, D_eff, getattr(hd, "HDC_" + prec), flags)
+    if prec == "I8":
+        assert np.array_equal(raw.astype(np.float64), acc_or)
+        assert np.array_equal(bits, bits_or)
+    else:
+        assert (np.abs(raw - acc_or) <= 1e-3 * np.abs(acc_or) + 1e-6 * absum).all()
+        n = check_sign_band(bits, bits_or, acc_or, absum, X.shape[1])
+        assert n <= 1e-4 * bits.size
+
+
+def test_encode_rp_bf16_inputs_in_place(hd, h):
+    """bf16 X and P handed over as bf16 (C5 style): used in place, identical to rounding fp32."""
+    w = gen.c5_large_batch(n=200, D=768, K=10, F=1024, per_class=1)
+    X, P = w["X"], w["P"]
+    bits_or, acc_or, absum = O.encode_rp(X, P, 768, O.BF16, want_absum=True)
+    bits, raw, _ = _encode(hd, h, X, P, 768, hd.HDC_BF16, 0, bf16_inputs=True)
+    assert (np.abs(raw - acc_or) <= 1e-3 * np.abs(acc_or) + 1e-6 * absum).all()
+    check_sign_band(bits, bits_or, acc_or, absum, 1024)
+
+
+# ------------------------------------------------------------------------------------ dot / cos
+@pytest.mark.parametrize("sim", ["DOT", "COS"])
+@pytest.mark.parametrize("hv_bits", [32, 16, 8, 1])
+@pytest.mark.parametrize("N,K,D,D_eff", [(150, 26, 2100, 2100), (64, 6, 10000, 4099), (33, 1, 500, 500),
+                                         (140, 70, 1300, 1000)])
+def test_dot_cos_similarity_and_classify(hd, h, sim, hv_bits, N, K, D, D_eff):
+    r = rng(5, N, K, D_eff, hv_bits)
+    hb = r.integers(0, 2, size=(N, D), dtype=np.uint8)
+    C = (r.standard_normal((K, D)) * 30).astype(np.float32)
+    C[r.random((K, D)) < 0.03] = 0.0
+    if K > 3:
+        C[3] = 0.0                                          # zero-norm class: cosine 0
+    simc = getattr(O, "SIM_" + sim)
+    S_or = O.similarity(hb, C, D_eff, simc, hv_bits)
+    kn = hd.knobs(D_eff, hv_bits=hv_bits, sim=getattr(hd, "HDC_SIM_" + sim))
+    Hd, Cd = dev_bits(hb), dev(C)
+    S = h.hdc_similarity(Hd, Cd, kn).cpu().numpy()
+    lab, best, sec = h.hdc_classify(Hd, Cd, kn, want_scores=True)
+    lab = lab.cpu().numpy()
+    lab_or, best_or, sec_or = O.classify(S_or, simc)
+    if hv_bits in (8, 1):                                   # integer contraction: exact
+        if sim == "DOT":
+            assert np.array_equal(S.astype(np.float64), S_or)
+            Si = h.hdc_similarity(Hd, Cd, kn, s_dtype=torch.int32).cpu().numpy()
+            assert np.array_equal(Si.astype(np.float64), S_or)
+        else:
+            assert np.allclose(S, S_or, rtol=1e-6, atol=1e-9)
+        assert np.array_equal(lab, lab_or)
+    else:
+        cop = O.class_operand(C, D_eff, hv_bits)
+        floor = 1e-6 * np.sqrt(D_eff) * np.sqrt((cop * cop).sum(axis=1))[None, :] if sim == "DOT" else 1e-6
+        check_scores(S, S_or, floor)
+        check_labels_float(lab, S_or, simc)
+    same = lab == lab_or
+    assert np.allclose(best.cpu().numpy()[same], best_or[same], rtol=1e-3, atol=1e-5)
+    assert np.allclose(sec.cpu().numpy()[same], sec_or[same], rtol=1e-3, atol=1e-5)
+
+
+def test_classify_ties_go_to_lowest_index(hd, h):
+    r = rng(6)
+    N, K, D = 90, 9, 640
+    hb = r.integers(0, 2, size=(N, D), dtype=np.uint8)
+    C = r.integers(-5, 6, size=(K, D)).astype(np.float32)
+    C[5] = C[2]
+    C[7] = C[2]
+    for hv_bits, sim in [(32, "DOT"), (32, "COS"), (8, "COS"), (1, "HAMMING"), (1, "DOT")]:
+        simc = getattr(O, "SIM_" + sim)
+        lab_or, _, _ = O.classify(O.similarity(hb, C, D, simc, hv_bits), simc)
+        kn = hd.knobs(D, hv_bits=hv_bits, sim=getattr(hd, "HDC_SIM_" + sim))
+        lab = h.hdc_classify(dev_bits(hb), dev(C), kn).cpu().numpy()
+        assert np.array_equal(lab, lab_or), (hv_bits, sim)
+        assert not np.isin(lab, [5, 7]).any()
+
+
+# ------------------------------------------------------------------------------------ training
+@pytest.mark.parametrize("N,K,D,D_eff", [(256, 4, 2048, 2048), (1000, 26, 1100, 1000), (70, 3, 64, 33)])
+def test_bundle_exact(hd, h, N, K, D, D_eff):
+    r = rng(7, N, K, D_eff)
+    hb = r.integers(0, 2, size=(N, D), dtype=np.uint8)
+    y = r.integers(0, K, size=N).astype(np.int32)
+    C0 = r.integers(-3, 4, size=(K, D)).astype(np.float32)
+    C_or = O.bundle(hb, y, K, D_eff, C0)
+    Cd = dev(C0.copy())
+    h.hdc_train_epoch(hd.HDC_TRAIN_BUNDLE, dev_bits(hb), dev(y), Cd, hd.knobs(D_eff))
+    out = Cd.cpu().numpy()
+    assert np.array_equal(out[:, :D_eff], C_or)
+    assert np.array_equal(out[:, D_eff:], C0[:, D_eff:])    # columns >= D_eff untouched
+
+
+@pytest.mark.parametrize("B", [0, 1, 7, 64])
+@pytest.mark.parametrize("hv_bits,sim", [(1, "HAMMING"), (8, "COS")])
+def test_perceptron_epoch_integer_paths_exact(hd, h, B, hv_bits, sim):
+    """Integer similarity => identical predictions => identical Delta => identical fp32 update."""
+    w = gen.c1_tiny(D=512)
+    hb, _, _ = O.encode_rp(w["Xtr"], w["P"], 512, O.F32)
+    y = w["ytr"].copy()
+    y[::5] = (y[::5] + 1) % w["K"]                          # label noise so mispredictions persist
+    D_eff = 500
+    simc = getattr(O, "SIM_" + sim)
+    C = O.bundle(hb, y, w["K"], 512)
+    kn = hd.knobs(D_eff, hv_bits=hv_bits, sim=getattr(hd, "HDC_SIM_" + sim))
+    Cd = dev(C.copy())
+    Hd, yd = dev_bits(hb), dev(y)
+    C_or = C[:, :D_eff].copy()
+    for _ in range(3):
+        C_or, wrong_or, pred_or = O.train_epoch(hb, y, C_or, D_eff, hv_bits, simc, 0.05, B)
+        pred = torch.empty(len(y), dtype=torch.int32, device="cuda")
+        nw = torch.zeros(1, dtype=torch.int64, device="cuda")
+        h.hdc_train_epoch(hd.HDC_TRAIN_PERCEPTRON, Hd, yd, Cd, kn, lr=0.05, batch=B, pred=pred, n_wrong=nw)
+        assert np.array_equal(pred.cpu().numpy(), pred_or)
+        assert int(nw.item()) == wrong_or
+        assert np.array_equal(Cd.cpu().numpy()[:, :D_eff], C_or)
+    assert np.array_equal(Cd.cpu().numpy()[:, D_eff:], C[:, D_eff:])
+
+
+@pytest.mark.parametrize("hv_bits", [32, 16])
+def test_perceptron_epoch_float_teacher_forced(hd, h, hv_bits):
+    """fp32 / bf16 cosine: each epoch starts from the oracle's accumulators; predictions equal
+    except near-ties; C_acc equal on every class row not touched by a near-tie sample."""
+    w = gen.c2_isolet_shaped(D=2000, n_tr=1200, n_te=8)
+    hb, _, _ = O.encode_rp(w["Xtr"], w["P"], 2000, O.F32)
+    y, K, D_eff = w["ytr"], w["K"], 2000
+    C_or = O.bundle(hb, y, K, D_eff)
+    kn = hd.knobs(D_eff, hv_bits=hv_bits, sim=hd.HDC_SIM_COS)
+    Hd, yd = dev_bits(hb), dev(y)
+    for _ in range(3):
+        S_or = O.similarity(hb, C_or, D_eff, O.SIM_COS, hv_bits)
+        C_next, wrong_or, pred_or = O.train_epoch(hb, y, C_or, D_eff, hv_bits, O.SIM_COS, 0.05, 0)
+        Cd = dev(C_or.copy())
+        pred = torch.empty(len(y), dtype=torch.int32, device="cuda")
+        h.hdc_train_epoch(hd.HDC_TRAIN_PERCEPTRON, Hd, yd, Cd, kn, lr=0.05, batch=0, pred=pred)
+        pred = pred.cpu().numpy()
+        check_labels_float(pred, S_or, O.SIM_COS)
+        near = np.nonzero(pred != pred_or)[0]
+        touched = set(y[near]) | set(pred[near]) | set(pred_or[near])
+        rows = [k for k in range(K) if k not in touched]
+        assert np.array_equal(Cd.cpu().numpy()[rows], C_next[rows])
+        assert wrong_or > 0
+        C_or = C_next
+
+
+# ------------------------------------------------------------------------------------ D_eff
+@pytest.mark.parametrize("D_eff", [10000, 8192, 4096, 2048, 1024, 1000])
+def test_d_eff_equals_physical_slice_on_gpu(hd, h, D_eff):
+    """S3: results at D_eff equal those on arrays physically sliced to D_eff columns (bit-exact,
+    GPU vs GPU and GPU vs oracle on the integer paths)."""
+    w = gen.c4_har_shaped(D=10000, n_tr=8, n_te=96)
+    X, P = w["Xte"], w["P"]
+    kn_full = hd.knobs(D_eff, precision=hd.HDC_I8)
+    H1 = h.hdc_encode_rp(dev(X), dev(P), kn_full)
+    H2 = h.hdc_encode_rp(dev(X), dev(P[:D_eff].copy()), kn_full)
+    assert torch.equal(H1, H2)
+    bits_or, _, _ = O.encode_rp(X, P, D_eff, O.I8)
+    assert np.array_equal(host_bits(H1, D_eff), bits_or)
+    r = rng(8, D_eff)
+    C = r.standard_normal((6, 10000)).astype(np.float32)
+    kn = hd.knobs(D_eff, hv_bits=1, sim=hd.HDC_SIM_HAMMING)
+    Hfull = h.hdc_encode_rp(dev(X), dev(P), hd.knobs(10000, precision=hd.HDC_I8))
+    S1 = h.hdc_similarity(Hfull, dev(C), kn)
+    S2 = h.hdc_similarity(H1, dev(C[:, :D_eff].copy()), kn)
+    assert torch.equal(S1, S2)
