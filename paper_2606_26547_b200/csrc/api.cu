@@ -63,9 +63,14 @@ int check_sim_knobs(hdc_ctx* h, const hdc_knobs_t* k) {
 }
 
 // ------------------------------------------------------------------------------------- encode
+// Reduction-segment schedule of the fp32-precision contraction over 3-way bf16 splits: segment s
+// multiplies A part a(s) with B part b(s); smallest terms first (x3p1, x2p2, x1p3, x2p1, x1p2, x1p1).
+constexpr uint32_t SPLIT_A_SEGS = 0x001012u;  // nibble s = a(s): 2,1,0,1,0,0
+constexpr uint32_t SPLIT_B_SEGS = 0x010210u;  // nibble s = b(s): 0,1,2,0,1,0
+
 struct EncodePlan {
   bool tc = false;         // tensor-core kernel
-  void* Xs = nullptr;      // staged X (bf16 or int8), null = use input in place
+  void* Xs = nullptr;      // staged X (bf16, 3 x bf16 or int8), null = use input in place
   void* Ps = nullptr;      // staged P
   int64_t ldxs = 0, ldps = 0;
   int Fp = 0;
@@ -79,19 +84,23 @@ bool use_tc(const hdc_ctx* h, const hdc_knobs_t* k) {
 void plan_encode(const hdc_ctx* h, int64_t N, int F, int D_eff, const hdc_knobs_t* k, bool x_inplace,
                  bool p_inplace, Bump& b, EncodePlan& pl) {
   const int prec = k->precision;
-  if (prec == HDC_F32) return;
+  pl.tc = use_tc(h, k);
+  pl.Fp = (int)round_up(F, 64);
+  if (prec == HDC_F32) {
+    if (!pl.tc) return;  // FFMA kernel reads the operands in place
+    pl.ldxs = pl.ldps = 3 * (int64_t)pl.Fp;
+    pl.Xs = b.take<__nv_bfloat16>((size_t)N * pl.ldxs);
+    pl.Ps = b.take<__nv_bfloat16>((size_t)D_eff * pl.ldps);
+    return;
+  }
   if (prec == HDC_I8) {
-    pl.Fp = (int)round_up(F, 64);
     pl.ldxs = pl.ldps = pl.Fp;
-    pl.tc = use_tc(h, k);
     if (!x_inplace) pl.Xs = b.take<int8_t>((size_t)N * pl.Fp);
     if (!p_inplace) pl.Ps = b.take<int8_t>((size_t)D_eff * pl.Fp);
     return;
   }
   // BF16 / B1
-  pl.tc = use_tc(h, k);
   if (!pl.tc) return;  // CUDA-core kernel rounds on load, no staging
-  pl.Fp = (int)round_up(F, 64);
   pl.ldxs = pl.ldps = pl.Fp;
   if (!x_inplace) pl.Xs = b.take<__nv_bfloat16>((size_t)N * pl.Fp);
   if (!p_inplace) pl.Ps = b.take<__nv_bfloat16>((size_t)D_eff * pl.Fp);
@@ -113,13 +122,26 @@ int do_encode_rp(hdc_ctx* h, const void* X, int x_dtype, int64_t N, int F, int64
   const int xk = x_dtype == HDC_BF16 ? OPK_BF16 : OPK_F32;
   const int pk = p_dtype == HDC_BF16 ? OPK_BF16 : (p_dtype == HDC_I8 ? OPK_I8 : OPK_F32);
   cudaError_t ce;
+  EncodePlan pl;
 
   if (prec == HDC_F32) {
+    plan_encode(h, N, F, D_eff, k, false, false, b, pl);
+    if (b.off > ws_bytes) return fail(h, HDC_ERR_WORKSPACE, "encode_rp: workspace too small");
+    if (pl.tc) {
+      ce = launch_split3_bf16(X, xk, N, F, ldx, (__nv_bfloat16*)pl.Xs, pl.Fp, st, &h->launches);
+      if (ce != cudaSuccess) return cuda_fail(h, ce, "split X");
+      ce = launch_split3_bf16(P, pk, D_eff, F, ldp, (__nv_bfloat16*)pl.Ps, pl.Fp, st, &h->launches);
+      if (ce != cudaSuccess) return cuda_fail(h, ce, "split P");
+      TcOperands o{pl.Xs, pl.Ps, OPK_BF16, pl.ldxs, pl.ldps, pl.ldxs, pl.ldps, pl.Fp, 6,
+                   SPLIT_A_SEGS, SPLIT_B_SEGS, pl.Fp};
+      ce = launch_gemm_tc(h->tc, o, N, D_eff, e, h->sm_count, st, &h->launches);
+      if (ce == cudaSuccess) return HDC_OK;
+      if (ce != cudaErrorNotSupported) return cuda_fail(h, ce, "encode_rp fp32 tcgen05");
+    }
     ce = launch_gemm_simt(Operand{X, ldx, xk}, Operand{P, ldp, pk}, N, D_eff, F, false, e, st, &h->launches);
     return ce == cudaSuccess ? HDC_OK : cuda_fail(h, ce, "encode_rp fp32");
   }
 
-  EncodePlan pl;
   const bool tc_ok_x = x_dtype == HDC_BF16 && (ldx % 8) == 0 && aligned16(X);
   const bool tc_ok_p = p_dtype == HDC_BF16 && (ldp % 8) == 0 && aligned16(P);
   if (prec == HDC_I8) {
@@ -137,8 +159,8 @@ int do_encode_rp(hdc_ctx* h, const void* X, int x_dtype, int64_t N, int F, int64
       ldpq = pl.ldps;
     }
     if (pl.tc) {
-      ce = launch_gemm_tc(h->tc, pl.Xs, Pq, OPK_I8, N, D_eff, pl.Fp, pl.ldxs, ldpq, e, h->sm_count, st,
-                          &h->launches);
+      TcOperands o{pl.Xs, Pq, OPK_I8, pl.ldxs, ldpq, F, F, F, 1, 0u, 0u, 0};
+      ce = launch_gemm_tc(h->tc, o, N, D_eff, e, h->sm_count, st, &h->launches);
       if (ce == cudaSuccess) return HDC_OK;
       if (ce != cudaErrorNotSupported) return cuda_fail(h, ce, "encode_rp int8 tcgen05");
     }
@@ -166,7 +188,8 @@ int do_encode_rp(hdc_ctx* h, const void* X, int x_dtype, int64_t N, int F, int64
       Pb = pl.Ps;
       ldpb = pl.ldps;
     }
-    ce = launch_gemm_tc(h->tc, Xb, Pb, OPK_BF16, N, D_eff, F, ldxb, ldpb, e, h->sm_count, st, &h->launches);
+    TcOperands o{Xb, Pb, OPK_BF16, ldxb, ldpb, F, F, F, 1, 0u, 0u, 0};
+    ce = launch_gemm_tc(h->tc, o, N, D_eff, e, h->sm_count, st, &h->launches);
     if (ce == cudaSuccess) return HDC_OK;
     if (ce != cudaErrorNotSupported) return cuda_fail(h, ce, "encode_rp bf16 tcgen05");
   }

@@ -51,18 +51,36 @@ struct Epilogue {
 cudaError_t launch_gemm_simt(const Operand& A, const Operand& B, int64_t M, int Nc, int Kr,
                              bool int_acc, const Epilogue& e, cudaStream_t st, int64_t* nlaunch);
 
-// tcgen05 path (gemm_tc.cu).  A and B must be K-contiguous bf16 (or int8) with Kr padded to a
-// multiple of 64 bytes*... see gemm_tc.cu.  Returns cudaErrorNotSupported when shapes do not fit.
+// tcgen05 path (gemm_tc.cu): both operands K-contiguous bf16 or int8, 16-byte aligned bases and row
+// strides.  The reduction axis is a list of `nseg` segments of Kr elements: segment s reads A
+// columns [a_seg(s)*seg_stride, +Kr) and B columns [b_seg(s)*seg_stride, +Kr), a_seg(s) = 4-bit
+// field s of a_segs (nseg = 1, a_segs = b_segs = 0: a plain GEMM).  Columns >= cols_a / cols_b read
+// as zero (TMA out-of-bounds fill), so Kr need not be a multiple of the k-block.
+// Returns cudaErrorNotSupported when the operands do not meet the alignment rules.
 struct TcContext;  // opaque: holds the cuTensorMapEncodeTiled entry point
 TcContext* tc_context_create();
 void tc_context_destroy(TcContext*);
-cudaError_t launch_gemm_tc(TcContext* tc, const void* A, const void* B, int elem_kind /*OPK_BF16|OPK_I8*/,
-                           int64_t M, int Nc, int Kr_padded, int64_t lda, int64_t ldb,
-                           const Epilogue& e, int sm_count, cudaStream_t st, int64_t* nlaunch);
+struct TcOperands {
+  const void* A;
+  const void* B;
+  int elem_kind;  // OPK_BF16 | OPK_I8
+  int64_t lda, ldb;
+  int64_t cols_a, cols_b;
+  int Kr;
+  int nseg;
+  uint32_t a_segs, b_segs;
+  int seg_stride;
+};
+cudaError_t launch_gemm_tc(TcContext* tc, const TcOperands& o, int64_t M, int Nc, const Epilogue& e,
+                           int sm_count, cudaStream_t st, int64_t* nlaunch);
 
 // fp32/bf16 -> bf16 staging with zero padding of the reduction axis: dst [rows][ld_dst]
 cudaError_t launch_convert_bf16(const void* src, int src_kind, int64_t rows, int cols, int64_t ld_src,
                                 __nv_bfloat16* dst, int64_t ld_dst, cudaStream_t st, int64_t* nlaunch);
+// fp32/bf16 -> three bf16 segments [x1 | x2 | x3] with x1 = bf16(x), x2 = bf16(x - x1),
+// x3 = bf16(x - x1 - x2) (each subtraction exact in fp32): dst [rows][3*seg] , zero padded
+cudaError_t launch_split3_bf16(const void* src, int src_kind, int64_t rows, int cols, int64_t ld_src,
+                               __nv_bfloat16* dst, int seg, cudaStream_t st, int64_t* nlaunch);
 // per-row symmetric int8 quantisation (S1/A7): dst [rows][ld_dst] int8, zero padded
 cudaError_t launch_quantize_rows_i8(const void* src, int src_kind, int64_t rows, int cols, int64_t ld_src,
                                     int8_t* dst, int64_t ld_dst, cudaStream_t st, int64_t* nlaunch);

@@ -43,6 +43,46 @@ __global__ void convert_bf16_kernel(const void* __restrict__ src, int src_kind, 
   }
 }
 
+// ---------------------------------------------------------------------------------- bf16 x3 split
+// x = x1 + x2 + x3 (+ O(2^-25 |x|)): x1 = bf16(x), x2 = bf16(x - x1), x3 = bf16(x - x1 - x2); both
+// residuals are exact fp32 subtractions.  dst [rows][3*seg]: segment s holds x_{s+1}; columns >=
+// cols of every segment are zero.  One thread = 8 consecutive columns of all three segments.
+__global__ void split3_bf16_kernel(const void* __restrict__ src, int src_kind, int64_t rows, int cols,
+                                   int64_t ld_src, __nv_bfloat16* __restrict__ dst, int seg) {
+  const int chunks = seg >> 3;
+  const int64_t total = rows * chunks;
+  const bool vec = src_kind == OPK_F32 && ((ld_src & 3) == 0) && ((reinterpret_cast<uintptr_t>(src) & 15) == 0);
+  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < total;
+       i += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t r = i / chunks;
+    const int c0 = (int)(i - r * chunks) << 3;
+    float x[8];
+    const int64_t base = r * ld_src + c0;
+    if (vec && c0 + 8 <= cols) {
+      const float4 a = __ldg(reinterpret_cast<const float4*>((const float*)src + base));
+      const float4 b = __ldg(reinterpret_cast<const float4*>((const float*)src + base) + 1);
+      x[0] = a.x; x[1] = a.y; x[2] = a.z; x[3] = a.w;
+      x[4] = b.x; x[5] = b.y; x[6] = b.z; x[7] = b.w;
+    } else {
+#pragma unroll
+      for (int j = 0; j < 8; ++j) x[j] = (c0 + j < cols) ? load_as_f32(src, src_kind, base + j) : 0.0f;
+    }
+    __align__(16) __nv_bfloat16 v1[8], v2[8], v3[8];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+      v1[j] = __float2bfloat16_rn(x[j]);
+      const float r1 = __fsub_rn(x[j], __bfloat162float(v1[j]));
+      v2[j] = __float2bfloat16_rn(r1);
+      const float r2 = __fsub_rn(r1, __bfloat162float(v2[j]));
+      v3[j] = __float2bfloat16_rn(r2);
+    }
+    __nv_bfloat16* o = dst + r * (int64_t)(3 * seg) + c0;
+    *reinterpret_cast<uint4*>(o) = *reinterpret_cast<const uint4*>(v1);
+    *reinterpret_cast<uint4*>(o + seg) = *reinterpret_cast<const uint4*>(v2);
+    *reinterpret_cast<uint4*>(o + 2 * seg) = *reinterpret_cast<const uint4*>(v3);
+  }
+}
+
 // ---------------------------------------------------------------------------------- int8 per row
 __device__ __forceinline__ int quant_i8(float x, float s) {
   float q = rintf(__fmul_rn(x, s));  // round-half-even, one rounded multiply (no FMA contraction)
@@ -177,6 +217,15 @@ cudaError_t launch_convert_bf16(const void* src, int src_kind, int64_t rows, int
   const int64_t total = rows * (ld_dst >> 3);
   convert_bf16_kernel<<<grid_for(total, 256, 148 * 16), 256, 0, st>>>(src, src_kind, rows, cols, ld_src,
                                                                      dst, ld_dst);
+  ++*nlaunch;
+  return cudaGetLastError();
+}
+
+cudaError_t launch_split3_bf16(const void* src, int src_kind, int64_t rows, int cols, int64_t ld_src,
+                               __nv_bfloat16* dst, int seg, cudaStream_t st, int64_t* nlaunch) {
+  if (rows <= 0) return cudaSuccess;
+  const int64_t total = rows * (seg >> 3);
+  split3_bf16_kernel<<<grid_for(total, 256, 148 * 16), 256, 0, st>>>(src, src_kind, rows, cols, ld_src, dst, seg);
   ++*nlaunch;
   return cudaGetLastError();
 }

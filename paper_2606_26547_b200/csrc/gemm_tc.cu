@@ -1,12 +1,497 @@
-// gemm_tc.cu -- placeholder until the tcgen05 kernel lands: reports "not supported" so callers use
-// the CUDA-core contraction.
+// gemm_tc.cu -- tensor-core contraction C[m,n] = sum_k A[m,k] * B[n,k] for sm_100a: TMA ->
+// shared memory (128-byte swizzle) -> tcgen05.mma -> TMEM -> tcgen05.ld epilogue, with the HDC
+// epilogues fused: sign + pack (random-projection encode, Listing 1 L68-L70 + L161),
+// scores (L110 cos_sim / L197 dot) and row arg-max (L79-L80).
+//
+// One persistent CTA per SM, 6 warps: warp 0 = TMA producer, warp 1 = MMA issuer (+ TMEM
+// allocation), warps 2-5 = epilogue (warp w reads TMEM lanes 32*(w%4).., thread = accumulator
+// row).  CTA tile 128 x 256, k-blocks of 128 bytes (64 bf16 / 128 int8), 4-stage mbarrier ring
+// between producer and issuer, two 256-column TMEM accumulators so that the epilogue of tile i
+// overlaps the MMAs of tile i+1.  Operands are K-contiguous ("K-major") for both A and B, which is
+// the layout of X[N][F], P[D][F] and C[K][D] (include/hdc.h).
+//
+// The reduction axis is a list of SEGMENTS: k-block kb reads A columns a_seg[kb / nkb_seg] *
+// seg_stride + (kb % nkb_seg) * BK and B columns b_seg[..] likewise.  One segment = a plain GEMM.
+// Six segments over 3-way bf16-split operands [x1|x2|x3], [p1|p2|p3] give the fp32-precision
+// contraction  x*p ~= x3p1 + x2p2 + x1p3 + x2p1 + x1p2 + x1p1  (smallest terms first, fp32
+// accumulation in TMEM) without materialising the repeated operands (DESIGN.md "fp32 on tensor
+// cores").
+#include <cuda.h>
+#include <cudaTypedefs.h>
+#include <limits.h>
+
+#include <type_traits>
+
 #include "common.cuh"
+
 namespace hdc {
-struct TcContext { int dummy; };
-TcContext* tc_context_create() { return nullptr; }
-void tc_context_destroy(TcContext*) {}
-cudaError_t launch_gemm_tc(TcContext*, const void*, const void*, int, int64_t, int, int, int64_t, int64_t,
-                           const Epilogue&, int, cudaStream_t, int64_t*) {
-  return cudaErrorNotSupported;
+
+struct TcContext {
+  PFN_cuTensorMapEncodeTiled_v12000 encode;
+};
+
+TcContext* tc_context_create() {
+  void* fn = nullptr;
+  cudaDriverEntryPointQueryResult q;
+  if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q) != cudaSuccess ||
+      q != cudaDriverEntryPointSuccess || fn == nullptr) {
+    (void)cudaGetLastError();
+    return nullptr;
+  }
+  TcContext* tc = new TcContext();
+  tc->encode = reinterpret_cast<PFN_cuTensorMapEncodeTiled_v12000>(fn);
+  return tc;
 }
+void tc_context_destroy(TcContext* tc) { delete tc; }
+
+namespace {
+
+constexpr int BM = 128;            // rows of A per tile == TMEM lanes
+constexpr int BN = 256;            // rows of B per tile == TMEM columns of one accumulator
+constexpr int KB_BYTES = 128;      // bytes of the reduction axis per k-block (one swizzle row)
+constexpr int STAGES = 4;
+constexpr int A_BYTES = BM * KB_BYTES;   // 16 KB
+constexpr int B_BYTES = BN * KB_BYTES;   // 32 KB
+constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
+constexpr int NTHREADS = 192;
+constexpr int TMEM_COLS = 512;
+constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*alignment slack*/ + 256 /*barriers*/;
+
+struct TcParams {
+  int64_t M;
+  int Nc;
+  int m_tiles, n_tiles;
+  int nseg, nkb_seg;            // number of reduction segments, k-blocks per segment
+  uint32_t a_segs, b_segs;      // 4 bits per segment: which operand segment it reads
+  int seg_stride;               // elements between operand segments
+  int group_m;                  // m-tiles per rasterisation group (EPI_SIGN / EPI_SCORE)
+  Epilogue e;
+};
+
+// ------------------------------------------------------------------------------------ PTX
+__device__ __forceinline__ uint32_t smem_u32(const void* p) {
+  return static_cast<uint32_t>(__cvta_generic_to_shared(p));
+}
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+// Spins on the phase parity.  A wait that lasts ~2 s of SM clocks is a protocol bug: trap instead
+// of hanging the device.
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  uint32_t done = 0;
+  long long t0 = 0;
+  for (uint32_t it = 0;; ++it) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(done)
+        : "r"(bar), "r"(parity)
+        : "memory");
+    if (done) return;
+    if ((it & 1023u) == 1023u) {
+      const long long t = clock64();
+      if (t0 == 0) t0 = t;
+      else if (t - t0 > 4000000000LL) __trap();
+    }
+  }
+}
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* tm, uint32_t bar, int c0, int c1) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
+      ::"r"(dst), "l"(reinterpret_cast<uint64_t>(tm)), "r"(bar), "r"(c0), "r"(c1)
+      : "memory");
+}
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_commit(uint32_t bar) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+template <bool INT8>
+__device__ __forceinline__ void tc_mma(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc,
+                                       uint32_t accumulate) {
+  if (INT8) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, p;\n\t}"
+        ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
+        : "memory");
+  } else {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
+        ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
+        : "memory");
+  }
+}
+// 32 lanes x 32 consecutive 32-bit columns: thread t of the warp gets lane (base + t), v[j] = column j
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+      "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+      "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+      : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+        "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]),
+        "=r"(v[16]), "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]),
+        "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+      : "r"(taddr)
+      : "memory");
+}
+__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+
+// Shared-memory matrix descriptor of a K-major tile stored as rows of 128 bytes with the 128-byte
+// swizzle (what TMA writes for SWIZZLE_128B): 8-row groups are 1024 bytes apart (SBO), the
+// leading-dimension offset is unused for swizzled K-major layouts, descriptor version 1 (sm_100),
+// layout type 2 = SWIZZLE_128B.  Advancing by one MMA along K (32 bytes) adds 2 to the address field.
+__device__ __forceinline__ uint64_t smem_desc(uint32_t saddr) {
+  uint64_t d = 0;
+  d |= (uint64_t)((saddr & 0x3FFFFu) >> 4);
+  d |= (uint64_t)1 << 16;                 // LBO (ignored)
+  d |= (uint64_t)(1024 >> 4) << 32;       // SBO
+  d |= (uint64_t)1 << 46;                 // version
+  d |= (uint64_t)2 << 61;                 // SWIZZLE_128B
+  return d;
+}
+// Instruction descriptor: D format (1 = f32, 2 = s32) bits 4-5, A/B format bits 7-9 / 10-12
+// (kind::f16: 1 = bf16; kind::i8: 1 = signed), both operands K-major (bits 15, 16 = 0),
+// N >> 3 at bit 17, M >> 4 at bit 24.
+template <bool INT8>
+__device__ __forceinline__ uint32_t instr_desc(int n) {
+  uint32_t d = 0;
+  d |= (INT8 ? 2u : 1u) << 4;
+  d |= 1u << 7;
+  d |= 1u << 10;
+  d |= (uint32_t)(n >> 3) << 17;
+  d |= (uint32_t)(BM >> 4) << 24;
+  return d;
+}
+
+struct Top2 {
+  double b1;
+  int i1;
+  double b2;
+};
+constexpr double NEG_BIG = -1.0e300;
+
+// i-th tile of this CTA: EPI_ARGMAX owns whole m-tiles (n inner, so a thread sees every class of
+// its row); the others walk groups of group_m m-tiles, m fastest, so that CTAs running at the same
+// time share B tiles and reuse A tiles from L2.
+template <int EPI>
+__device__ __forceinline__ bool tile_at(const TcParams& p, int64_t i, int& mt, int& nt) {
+  if (EPI == EPI_ARGMAX) {
+    const int64_t u = blockIdx.x + (i / p.n_tiles) * (int64_t)gridDim.x;
+    if (u >= p.m_tiles) return false;
+    mt = (int)u;
+    nt = (int)(i % p.n_tiles);
+    return true;
+  }
+  const int64_t t = blockIdx.x + i * (int64_t)gridDim.x;
+  if (t >= (int64_t)p.m_tiles * p.n_tiles) return false;
+  const int64_t gsz = (int64_t)p.group_m * p.n_tiles;
+  const int64_t g = t / gsz;
+  const int r = (int)(t - g * gsz);
+  int gm = p.m_tiles - (int)g * p.group_m;
+  if (gm > p.group_m) gm = p.group_m;
+  mt = (int)g * p.group_m + r % gm;
+  nt = r / gm;
+  return true;
+}
+
+template <bool INT8, int EPI>
+__global__ void __launch_bounds__(NTHREADS, 1)
+gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
+               const TcParams p) {
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  // barriers live after the stage ring
+  const uint32_t bar0 = base + STAGES * STAGE_BYTES;
+  auto full_bar = [&](int s) { return bar0 + 8u * s; };
+  auto empty_bar = [&](int s) { return bar0 + 8u * (STAGES + s); };
+  auto tfull_bar = [&](int s) { return bar0 + 8u * (2 * STAGES + s); };
+  auto tempty_bar = [&](int s) { return bar0 + 8u * (2 * STAGES + 2 + s); };
+  const uint32_t tmem_slot = bar0 + 8u * (2 * STAGES + 4);
+  uint32_t* tmem_slot_ptr = reinterpret_cast<uint32_t*>(smem_raw + (tmem_slot - smem_u32(smem_raw)));
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  constexpr int BK = INT8 ? 128 : 64;  // elements per k-block
+  const int num_kb = p.nseg * p.nkb_seg;
+
+  if (warp == 0 && lane == 0) {
+    asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&tmA)) : "memory");
+    asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&tmB)) : "memory");
+    for (int s = 0; s < STAGES; ++s) {
+      mbar_init(full_bar(s), 1);
+      mbar_init(empty_bar(s), 1);
+    }
+    for (int s = 0; s < 2; ++s) {
+      mbar_init(tfull_bar(s), 1);
+      mbar_init(tempty_bar(s), 4);
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  if (warp == 1) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tmem_slot),
+                 "r"((uint32_t)TMEM_COLS)
+                 : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = *tmem_slot_ptr;
+
+  if (warp == 0) {
+    // ================================================================= TMA producer
+    int stage = 0;
+    uint32_t phase = 0;
+    int mt, nt;
+    for (int64_t i = 0; tile_at<EPI>(p, i, mt, nt); ++i) {
+      const int m0 = mt * BM, n0 = nt * BN;
+      for (int kb = 0; kb < num_kb; ++kb) {
+        const int seg = kb / p.nkb_seg;
+        const int j = kb - seg * p.nkb_seg;
+        const int acol = (int)((p.a_segs >> (4 * seg)) & 15u) * p.seg_stride + j * BK;
+        const int bcol = (int)((p.b_segs >> (4 * seg)) & 15u) * p.seg_stride + j * BK;
+        mbar_wait(empty_bar(stage), phase ^ 1u);
+        if (lane == 0) {
+          const uint32_t sa = base + stage * STAGE_BYTES;
+          mbar_arrive_expect_tx(full_bar(stage), STAGE_BYTES);
+          tma_load_2d(sa, &tmA, full_bar(stage), acol, m0);
+          tma_load_2d(sa + A_BYTES, &tmB, full_bar(stage), bcol, n0);
+        }
+        __syncwarp();
+        if (++stage == STAGES) {
+          stage = 0;
+          phase ^= 1u;
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ================================================================= MMA issuer
+    int stage = 0;
+    uint32_t phase = 0;
+    int acc = 0;
+    uint32_t acc_phase = 0;
+    int mt, nt;
+    for (int64_t i = 0; tile_at<EPI>(p, i, mt, nt); ++i) {
+      int n_valid = p.Nc - nt * BN;
+      if (n_valid > BN) n_valid = BN;
+      const uint32_t idesc = instr_desc<INT8>((n_valid + 15) & ~15);
+      mbar_wait(tempty_bar(acc), acc_phase ^ 1u);
+      tc_fence_after();
+      const uint32_t d_tmem = tmem_base + (uint32_t)(acc * BN);
+      for (int kb = 0; kb < num_kb; ++kb) {
+        mbar_wait(full_bar(stage), phase);
+        tc_fence_after();
+        if (lane == 0) {
+          const uint32_t sa = base + stage * STAGE_BYTES;
+          const uint64_t da = smem_desc(sa), db = smem_desc(sa + A_BYTES);
+#pragma unroll
+          for (int k = 0; k < KB_BYTES / 32; ++k)
+            tc_mma<INT8>(d_tmem, da + 2u * k, db + 2u * k, idesc, (kb | k) != 0 ? 1u : 0u);
+          tc_commit(empty_bar(stage));            // frees the smem slot when these MMAs retire
+          if (kb == num_kb - 1) tc_commit(tfull_bar(acc));  // accumulator complete
+        }
+        __syncwarp();
+        if (++stage == STAGES) {
+          stage = 0;
+          phase ^= 1u;
+        }
+      }
+      if (++acc == 2) {
+        acc = 0;
+        acc_phase ^= 1u;
+      }
+    }
+  } else {
+    // ================================================================= epilogue (warps 2..5)
+    using AccT = typename std::conditional<INT8, int, float>::type;
+    const int q = warp & 3;  // TMEM lane quadrant this warp may read
+    int acc = 0;
+    uint32_t acc_phase = 0;
+    Top2 run = Top2{NEG_BIG, INT_MAX, NEG_BIG};
+    int mt, nt;
+    for (int64_t i = 0; tile_at<EPI>(p, i, mt, nt); ++i) {
+      const int n0 = nt * BN;
+      int n_valid = p.Nc - n0;
+      if (n_valid > BN) n_valid = BN;
+      const int64_t row = (int64_t)mt * BM + q * 32 + lane;
+      const bool row_ok = row < p.M;
+      mbar_wait(tfull_bar(acc), acc_phase);
+      tc_fence_after();
+      const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(acc * BN);
+      const int nchunks = (n_valid + 31) >> 5;
+      for (int c = 0; c < nchunks; ++c) {
+        uint32_t v[32];
+        tmem_ld32(taddr + (uint32_t)(c * 32), v);
+        tmem_ld_wait();
+        const int valid = n_valid - c * 32;  // >= 1
+        if (EPI == EPI_SIGN) {
+          uint32_t word = 0;
+#pragma unroll
+          for (int j = 0; j < 32; ++j) {
+            const bool neg = INT8 ? ((int)v[j] < 0) : (__uint_as_float(v[j]) < 0.0f);
+            word |= (neg ? 1u : 0u) << j;
+          }
+          if (valid < 32) word &= (1u << valid) - 1u;
+          if (row_ok) {
+            p.e.bits[row * p.e.ldbits + (n0 >> 5) + c] = word;
+            if (p.e.raw) {
+              uint32_t* out = reinterpret_cast<uint32_t*>(p.e.raw) + row * p.e.ldraw + n0 + c * 32;
+#pragma unroll
+              for (int j = 0; j < 32; ++j)
+                if (j < valid) out[j] = v[j];
+            }
+          }
+        } else if (EPI == EPI_SCORE) {
+          if (row_ok) {
+#pragma unroll
+            for (int j = 0; j < 32; ++j) {
+              if (j < valid) {
+                const int col = n0 + c * 32 + j;
+                const AccT a = INT8 ? (AccT)(int)v[j] : (AccT)__uint_as_float(v[j]);
+                if (p.e.s_i32) {
+                  reinterpret_cast<int32_t*>(p.e.S)[row * p.e.lds + col] = (int32_t)a;
+                } else {
+                  const float s = p.e.colscale ? (float)((double)a * p.e.colscale[col]) : (float)a;
+                  reinterpret_cast<float*>(p.e.S)[row * p.e.lds + col] = s;
+                }
+              }
+            }
+          }
+        } else {
+#pragma unroll
+          for (int j = 0; j < 32; ++j) {
+            if (j < valid) {
+              const int col = n0 + c * 32 + j;
+              const AccT a = INT8 ? (AccT)(int)v[j] : (AccT)__uint_as_float(v[j]);
+              const double s = p.e.colscale ? (double)a * p.e.colscale[col] : (double)a;
+              if (s > run.b1) {  // columns arrive in increasing order: strict > keeps the lowest index
+                run.b2 = run.b1;
+                run.b1 = s;
+                run.i1 = col;
+              } else if (s > run.b2) {
+                run.b2 = s;
+              }
+            }
+          }
+        }
+      }
+      // accumulator drained: hand it back to the MMA issuer
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(tempty_bar(acc));
+      if (++acc == 2) {
+        acc = 0;
+        acc_phase ^= 1u;
+      }
+      if (EPI == EPI_ARGMAX && nt == p.n_tiles - 1) {
+        if (row_ok) {
+          double b1 = run.b1, b2 = run.b2;
+          if (b2 == NEG_BIG) b2 = b1;  // K == 1
+          if (p.e.ham_D > 0) {
+            b1 = 0.5 * ((double)p.e.ham_D - b1);
+            b2 = 0.5 * ((double)p.e.ham_D - b2);
+          }
+          p.e.labels[row] = run.i1;
+          if (p.e.best) p.e.best[row] = (float)b1;
+          if (p.e.second) p.e.second[row] = (float)b2;
+        }
+        run = Top2{NEG_BIG, INT_MAX, NEG_BIG};
+      }
+    }
+  }
+
+  // ------------------------------------------------------------------- teardown
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) {
+    tc_fence_after();
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"((uint32_t)TMEM_COLS)
+                 : "memory");
+  }
+}
+
+// [rows][cols] matrix of `es`-byte elements, row stride ld elements, boxes of (128 bytes) x box_rows
+// with the 128-byte swizzle; out-of-range elements read as zero.
+CUresult make_map(TcContext* tc, CUtensorMap* out, const void* ptr, bool int8, int64_t rows, int64_t cols,
+                  int64_t ld, int box_rows) {
+  const cuuint64_t es = int8 ? 1 : 2;
+  cuuint64_t dims[2] = {(cuuint64_t)cols, (cuuint64_t)rows};
+  cuuint64_t strides[1] = {(cuuint64_t)ld * es};
+  cuuint32_t box[2] = {(cuuint32_t)(KB_BYTES / es), (cuuint32_t)box_rows};
+  cuuint32_t estr[2] = {1, 1};
+  return tc->encode(out, int8 ? CU_TENSOR_MAP_DATA_TYPE_UINT8 : CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2,
+                    const_cast<void*>(ptr), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                    CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+}
+
+template <bool INT8, int EPI>
+cudaError_t launch_one(const CUtensorMap& tmA, const CUtensorMap& tmB, const TcParams& p, int grid,
+                       cudaStream_t st) {
+  static bool attr_set = false;  // per instantiation; the attribute is sticky for the function
+  if (!attr_set) {
+    cudaError_t e = cudaFuncSetAttribute(gemm_tc_kernel<INT8, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         SMEM_BYTES);
+    if (e != cudaSuccess) return e;
+    attr_set = true;
+  }
+  gemm_tc_kernel<INT8, EPI><<<grid, NTHREADS, SMEM_BYTES, st>>>(tmA, tmB, p);
+  return cudaGetLastError();
+}
+
+}  // namespace
+
+cudaError_t launch_gemm_tc(TcContext* tc, const TcOperands& o, int64_t M, int Nc, const Epilogue& e,
+                           int sm_count, cudaStream_t st, int64_t* nlaunch) {
+  if (!tc) return cudaErrorNotSupported;
+  if (M <= 0 || Nc <= 0) return cudaSuccess;
+  const bool int8 = o.elem_kind == OPK_I8;
+  const int es = int8 ? 1 : 2;
+  const int BK = KB_BYTES / es;
+  // TMA needs 16-byte aligned bases and row strides; segments must start on k-block boundaries
+  if ((reinterpret_cast<uintptr_t>(o.A) & 15) || (reinterpret_cast<uintptr_t>(o.B) & 15) ||
+      ((o.lda * es) & 15) || ((o.ldb * es) & 15) || o.nseg < 1 || o.nseg > 8 ||
+      (o.nseg > 1 && (o.seg_stride % BK) != 0))
+    return cudaErrorNotSupported;
+  if (M > (int64_t)INT_MAX - BM || o.cols_a > INT_MAX || o.cols_b > INT_MAX) return cudaErrorNotSupported;
+  TcParams p;
+  p.M = M;
+  p.Nc = Nc;
+  p.m_tiles = (int)((M + BM - 1) / BM);
+  p.n_tiles = (Nc + BN - 1) / BN;
+  p.nseg = o.nseg;
+  p.nkb_seg = (o.Kr + BK - 1) / BK;
+  p.a_segs = o.a_segs;
+  p.b_segs = o.b_segs;
+  p.seg_stride = o.seg_stride;
+  p.group_m = 16;
+  p.e = e;
+  CUtensorMap tmA, tmB;
+  if (make_map(tc, &tmA, o.A, int8, M, o.cols_a, o.lda, BM) != CUDA_SUCCESS) return cudaErrorInvalidValue;
+  if (make_map(tc, &tmB, o.B, int8, Nc, o.cols_b, o.ldb, BN) != CUDA_SUCCESS) return cudaErrorInvalidValue;
+  const int64_t units = e.kind == EPI_ARGMAX ? p.m_tiles : (int64_t)p.m_tiles * p.n_tiles;
+  const int grid = (int)(units < sm_count ? units : sm_count);
+  ++*nlaunch;
+  if (int8) {
+    switch (e.kind) {
+      case EPI_SIGN: return launch_one<true, EPI_SIGN>(tmA, tmB, p, grid, st);
+      case EPI_SCORE: return launch_one<true, EPI_SCORE>(tmA, tmB, p, grid, st);
+      default: return launch_one<true, EPI_ARGMAX>(tmA, tmB, p, grid, st);
+    }
+  }
+  switch (e.kind) {
+    case EPI_SIGN: return launch_one<false, EPI_SIGN>(tmA, tmB, p, grid, st);
+    case EPI_SCORE: return launch_one<false, EPI_SCORE>(tmA, tmB, p, grid, st);
+    default: return launch_one<false, EPI_ARGMAX>(tmA, tmB, p, grid, st);
+  }
+}
+
 }  // namespace hdc
