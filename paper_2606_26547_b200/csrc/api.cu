@@ -207,6 +207,48 @@ int do_similarity(hdc_ctx* h, const uint32_t* Hbits, int64_t N, int64_t ldh, con
   const int D_eff = k->D_eff;
   const int W = words_of(D_eff);
   cudaError_t ce;
+  // tensor-core path from packed queries: DOT / COS at any K; Hamming once K is large enough that
+  // the popcount pipe would bound it (dist = (D_eff - dot)/2 is exact in int32)
+  if (use_tc(h, k) && (k->sim != HDC_SIM_HAMMING || K >= 64)) {
+    double* colscale = nullptr;
+    if (k->sim == HDC_SIM_COS) colscale = b.take<double>((size_t)K);
+    float* amax = b.take<float>(1);
+    void* cop = b.take<uint8_t>(sim_tc_operand_bytes(K, k->hv_bits, D_eff));
+    if (b.off > ws_bytes) return fail(h, HDC_ERR_WORKSPACE, "similarity: workspace too small");
+    if (colscale) {
+      // norms over the operand as the contraction sees it (permutation-invariant)
+      if (k->hv_bits == 8) {
+        const int64_t ldq = round_up(D_eff, 16);
+        int8_t* Cq = b.take<int8_t>((size_t)K * ldq);
+        if (b.off > ws_bytes) return fail(h, HDC_ERR_WORKSPACE, "similarity: workspace too small");
+        ce = launch_quantize_tensor_i8(C_acc, K, D_eff, ldc, Cq, ldq, amax, st, &h->launches);
+        if (ce != cudaSuccess) return cuda_fail(h, ce, "quantize C");
+        ce = launch_col_scale(Operand{Cq, ldq, OPK_I8}, K, D_eff, 1, colscale, st, &h->launches);
+      } else {
+        const int ck = k->hv_bits == 32 ? OPK_F32 : (k->hv_bits == 16 ? OPK_F32_RBF16 : OPK_BITS);
+        ce = launch_col_scale(Operand{C_acc, ldc, ck}, K, D_eff, 1, colscale, st, &h->launches);
+      }
+      if (ce != cudaSuccess) return cuda_fail(h, ce, "col_scale");
+    }
+    Epilogue e{};
+    e.colscale = colscale;
+    e.ham_D = k->sim == HDC_SIM_HAMMING ? D_eff : 0;
+    if (labels) {
+      e.kind = EPI_ARGMAX;
+      e.labels = labels;
+      e.best = best;
+      e.second = second;
+    } else {
+      e.kind = EPI_SCORE;
+      e.S = S;
+      e.lds = lds;
+      e.s_i32 = s_i32;
+    }
+    ce = launch_sim_tc(h->tc, Hbits, N, ldh, C_acc, K, ldc, D_eff, k->hv_bits, cop, amax, e, h->sm_count, st,
+                       &h->launches);
+    if (ce == cudaSuccess) return HDC_OK;
+    if (ce != cudaErrorNotSupported) return cuda_fail(h, ce, "similarity tcgen05");
+  }
   if (k->sim == HDC_SIM_HAMMING) {
     uint32_t* cbits = b.take<uint32_t>((size_t)K * W);
     if (b.off > ws_bytes) return fail(h, HDC_ERR_WORKSPACE, "similarity: workspace too small");
@@ -271,7 +313,9 @@ size_t similarity_ws(int K, const hdc_knobs_t* k) {
   b.take<int8_t>((size_t)K * round_up(k->D_eff, 16));
   b.take<float>(1);
   b.take<uint32_t>((size_t)K * W);
-  return b.off + 256;
+  b.take<uint8_t>(sim_tc_operand_bytes(K, k->hv_bits == 32 || k->hv_bits == 16 || k->hv_bits == 8 ? k->hv_bits : 1,
+                                       k->D_eff));
+  return b.off + 1024;
 }
 
 constexpr int64_t HOST_CHUNK = 16384;

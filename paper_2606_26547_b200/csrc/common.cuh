@@ -74,6 +74,17 @@ struct TcOperands {
 cudaError_t launch_gemm_tc(TcContext* tc, const TcOperands& o, int64_t M, int Nc, const Epilogue& e,
                            int sm_count, cudaStream_t st, int64_t* nlaunch);
 
+// similarity on the tensor cores from packed queries (simtc.cu).  cop: workspace of
+// sim_tc_operand_bytes() for the staged class operand; amax_scratch: one float (hv_bits 8).
+// e.kind is EPI_SCORE or EPI_ARGMAX; e.ham_D > 0 reports Hamming distances (hv_bits 1).
+size_t sim_tc_operand_bytes(int K, int hv_bits, int D_eff);
+cudaError_t launch_sim_tc(TcContext* tc, const uint32_t* Hbits, int64_t N, int64_t ldh, const float* C_acc,
+                          int K, int64_t ldc, int D_eff, int hv_bits, void* cop, float* amax_scratch,
+                          const Epilogue& e, int sm_count, cudaStream_t st, int64_t* nlaunch);
+// amax = max |C[k][d]| over k < K, d < D_eff (amax zeroed here)
+cudaError_t launch_tensor_amax(const float* C, int K, int D_eff, int64_t ldc, float* amax, cudaStream_t st,
+                               int64_t* nlaunch);
+
 // fp32/bf16 -> bf16 staging with zero padding of the reduction axis: dst [rows][ld_dst]
 cudaError_t launch_convert_bf16(const void* src, int src_kind, int64_t rows, int cols, int64_t ld_src,
                                 __nv_bfloat16* dst, int64_t ld_dst, cudaStream_t st, int64_t* nlaunch);

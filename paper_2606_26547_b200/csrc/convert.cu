@@ -239,15 +239,19 @@ cudaError_t launch_quantize_rows_i8(const void* src, int src_kind, int64_t rows,
   return cudaGetLastError();
 }
 
+cudaError_t launch_tensor_amax(const float* C, int K, int D_eff, int64_t ldc, float* amax, cudaStream_t st,
+                               int64_t* nlaunch) {
+  cudaError_t e = cudaMemsetAsync(amax, 0, sizeof(float), st);
+  if (e != cudaSuccess) return e;
+  tensor_amax_kernel<<<grid_for((int64_t)K * D_eff, 256, 148 * 4), 256, 0, st>>>(C, K, D_eff, ldc, amax);
+  ++*nlaunch;
+  return cudaGetLastError();
+}
+
 cudaError_t launch_quantize_tensor_i8(const float* C, int K, int D_eff, int64_t ldc, int8_t* dst,
                                       int64_t ld_dst, float* amax_scratch, cudaStream_t st,
                                       int64_t* nlaunch) {
-  cudaError_t e = cudaMemsetAsync(amax_scratch, 0, sizeof(float), st);
-  if (e != cudaSuccess) return e;
-  tensor_amax_kernel<<<grid_for((int64_t)K * D_eff, 256, 148 * 4), 256, 0, st>>>(C, K, D_eff, ldc,
-                                                                                amax_scratch);
-  ++*nlaunch;
-  e = cudaGetLastError();
+  cudaError_t e = launch_tensor_amax(C, K, D_eff, ldc, amax_scratch, st, nlaunch);
   if (e != cudaSuccess) return e;
   quantize_tensor_i8_kernel<<<grid_for((int64_t)K * ld_dst, 256, 148 * 8), 256, 0, st>>>(
       C, K, D_eff, ldc, dst, ld_dst, amax_scratch);

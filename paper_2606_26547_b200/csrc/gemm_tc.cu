@@ -23,6 +23,7 @@
 #include <type_traits>
 
 #include "common.cuh"
+#include "tc_ptx.cuh"
 
 namespace hdc {
 
@@ -44,11 +45,28 @@ TcContext* tc_context_create() {
 }
 void tc_context_destroy(TcContext* tc) { delete tc; }
 
+// [rows][cols] matrix of `es`-byte elements, row stride ld elements, boxes of (128 bytes) x box_rows
+// with the 128-byte swizzle; out-of-range elements read as zero.
+bool tc_make_map(TcContext* tc, CUtensorMap* out, const void* ptr, bool int8, int64_t rows, int64_t cols,
+                  int64_t ld, int box_rows) {
+  const cuuint64_t es = int8 ? 1 : 2;
+  cuuint64_t dims[2] = {(cuuint64_t)cols, (cuuint64_t)rows};
+  cuuint64_t strides[1] = {(cuuint64_t)ld * es};
+  cuuint32_t box[2] = {(cuuint32_t)(tcp::KB_BYTES / es), (cuuint32_t)box_rows};
+  cuuint32_t estr[2] = {1, 1};
+  return CUDA_SUCCESS == tc->encode(out, int8 ? CU_TENSOR_MAP_DATA_TYPE_UINT8 : CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2,
+                    const_cast<void*>(ptr), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                    CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+}
+
+
 namespace {
+
+using namespace tcp;
 
 constexpr int BM = 128;            // rows of A per tile == TMEM lanes
 constexpr int BN = 256;            // rows of B per tile == TMEM columns of one accumulator
-constexpr int KB_BYTES = 128;      // bytes of the reduction axis per k-block (one swizzle row)
 constexpr int STAGES = 4;
 constexpr int A_BYTES = BM * KB_BYTES;   // 16 KB
 constexpr int B_BYTES = BN * KB_BYTES;   // 32 KB
@@ -67,110 +85,6 @@ struct TcParams {
   int group_m;                  // m-tiles per rasterisation group (EPI_SIGN / EPI_SCORE)
   Epilogue e;
 };
-
-// ------------------------------------------------------------------------------------ PTX
-__device__ __forceinline__ uint32_t smem_u32(const void* p) {
-  return static_cast<uint32_t>(__cvta_generic_to_shared(p));
-}
-__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
-  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-}
-// Spins on the phase parity.  A wait that lasts ~2 s of SM clocks is a protocol bug: trap instead
-// of hanging the device.
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-  uint32_t done = 0;
-  long long t0 = 0;
-  for (uint32_t it = 0;; ++it) {
-    asm volatile(
-        "{\n\t.reg .pred p;\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
-        "selp.u32 %0, 1, 0, p;\n\t}"
-        : "=r"(done)
-        : "r"(bar), "r"(parity)
-        : "memory");
-    if (done) return;
-    if ((it & 1023u) == 1023u) {
-      const long long t = clock64();
-      if (t0 == 0) t0 = t;
-      else if (t - t0 > 4000000000LL) __trap();
-    }
-  }
-}
-__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* tm, uint32_t bar, int c0, int c1) {
-  asm volatile(
-      "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
-      ::"r"(dst), "l"(reinterpret_cast<uint64_t>(tm)), "r"(bar), "r"(c0), "r"(c1)
-      : "memory");
-}
-__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
-__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
-__device__ __forceinline__ void tc_commit(uint32_t bar) {
-  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
-}
-template <bool INT8>
-__device__ __forceinline__ void tc_mma(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc,
-                                       uint32_t accumulate) {
-  if (INT8) {
-    asm volatile(
-        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
-        "tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, p;\n\t}"
-        ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
-        : "memory");
-  } else {
-    asm volatile(
-        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
-        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
-        ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
-        : "memory");
-  }
-}
-// 32 lanes x 32 consecutive 32-bit columns: thread t of the warp gets lane (base + t), v[j] = column j
-__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
-  asm volatile(
-      "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
-      "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
-      "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
-      : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
-        "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]),
-        "=r"(v[16]), "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]),
-        "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
-      : "r"(taddr)
-      : "memory");
-}
-__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
-
-// Shared-memory matrix descriptor of a K-major tile stored as rows of 128 bytes with the 128-byte
-// swizzle (what TMA writes for SWIZZLE_128B): 8-row groups are 1024 bytes apart (SBO), the
-// leading-dimension offset is unused for swizzled K-major layouts, descriptor version 1 (sm_100),
-// layout type 2 = SWIZZLE_128B.  Advancing by one MMA along K (32 bytes) adds 2 to the address field.
-__device__ __forceinline__ uint64_t smem_desc(uint32_t saddr) {
-  uint64_t d = 0;
-  d |= (uint64_t)((saddr & 0x3FFFFu) >> 4);
-  d |= (uint64_t)1 << 16;                 // LBO (ignored)
-  d |= (uint64_t)(1024 >> 4) << 32;       // SBO
-  d |= (uint64_t)1 << 46;                 // version
-  d |= (uint64_t)2 << 61;                 // SWIZZLE_128B
-  return d;
-}
-// Instruction descriptor: D format (1 = f32, 2 = s32) bits 4-5, A/B format bits 7-9 / 10-12
-// (kind::f16: 1 = bf16; kind::i8: 1 = signed), both operands K-major (bits 15, 16 = 0),
-// N >> 3 at bit 17, M >> 4 at bit 24.
-template <bool INT8>
-__device__ __forceinline__ uint32_t instr_desc(int n) {
-  uint32_t d = 0;
-  d |= (INT8 ? 2u : 1u) << 4;
-  d |= 1u << 7;
-  d |= 1u << 10;
-  d |= (uint32_t)(n >> 3) << 17;
-  d |= (uint32_t)(BM >> 4) << 24;
-  return d;
-}
 
 struct Top2 {
   double b1;
@@ -236,10 +150,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == 1) {
-    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tmem_slot),
-                 "r"((uint32_t)TMEM_COLS)
-                 : "memory");
-    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    tmem_alloc(tmem_slot, TMEM_COLS);
   }
   tc_fence_before();
   __syncthreads();
@@ -282,7 +193,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     for (int64_t i = 0; tile_at<EPI>(p, i, mt, nt); ++i) {
       int n_valid = p.Nc - nt * BN;
       if (n_valid > BN) n_valid = BN;
-      const uint32_t idesc = instr_desc<INT8>((n_valid + 15) & ~15);
+      const uint32_t idesc = instr_desc<INT8>(BM, (n_valid + 15) & ~15);
       mbar_wait(tempty_bar(acc), acc_phase ^ 1u);
       tc_fence_after();
       const uint32_t d_tmem = tmem_base + (uint32_t)(acc * BN);
@@ -413,24 +324,8 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
   __syncthreads();
   if (warp == 1) {
     tc_fence_after();
-    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"((uint32_t)TMEM_COLS)
-                 : "memory");
+    tmem_dealloc(tmem_base, TMEM_COLS);
   }
-}
-
-// [rows][cols] matrix of `es`-byte elements, row stride ld elements, boxes of (128 bytes) x box_rows
-// with the 128-byte swizzle; out-of-range elements read as zero.
-CUresult make_map(TcContext* tc, CUtensorMap* out, const void* ptr, bool int8, int64_t rows, int64_t cols,
-                  int64_t ld, int box_rows) {
-  const cuuint64_t es = int8 ? 1 : 2;
-  cuuint64_t dims[2] = {(cuuint64_t)cols, (cuuint64_t)rows};
-  cuuint64_t strides[1] = {(cuuint64_t)ld * es};
-  cuuint32_t box[2] = {(cuuint32_t)(KB_BYTES / es), (cuuint32_t)box_rows};
-  cuuint32_t estr[2] = {1, 1};
-  return tc->encode(out, int8 ? CU_TENSOR_MAP_DATA_TYPE_UINT8 : CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2,
-                    const_cast<void*>(ptr), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                    CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
 }
 
 template <bool INT8, int EPI>
@@ -475,8 +370,8 @@ cudaError_t launch_gemm_tc(TcContext* tc, const TcOperands& o, int64_t M, int Nc
   p.group_m = 16;
   p.e = e;
   CUtensorMap tmA, tmB;
-  if (make_map(tc, &tmA, o.A, int8, M, o.cols_a, o.lda, BM) != CUDA_SUCCESS) return cudaErrorInvalidValue;
-  if (make_map(tc, &tmB, o.B, int8, Nc, o.cols_b, o.ldb, BN) != CUDA_SUCCESS) return cudaErrorInvalidValue;
+  if (!tc_make_map(tc, &tmA, o.A, int8, M, o.cols_a, o.lda, BM)) return cudaErrorInvalidValue;
+  if (!tc_make_map(tc, &tmB, o.B, int8, Nc, o.cols_b, o.ldb, BN)) return cudaErrorInvalidValue;
   const int64_t units = e.kind == EPI_ARGMAX ? p.m_tiles : (int64_t)p.m_tiles * p.n_tiles;
   const int grid = (int)(units < sm_count ? units : sm_count);
   ++*nlaunch;

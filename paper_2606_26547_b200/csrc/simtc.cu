@@ -1,0 +1,476 @@
+// simtc.cu -- similarity search on the tensor cores straight from PACKED query hypervectors
+// (PAPER.md L110 cos_sim, L197 dot, L72-L74 Hamming via dist = (D_eff - dot)/2, L79-L80 arg-extremum):
+//
+//   S[n,k] = sum_{d<D_eff} v[n,d] * c[k,d],   v = 1 - 2*bit
+//
+// The +-1 query operand never exists in HBM: four "expander" warps turn the packed words of a
+// 128-query tile into the K-major, 128-byte-swizzled shared-memory tile that tcgen05.mma reads (the
+// layout TMA would have written), while the class operand arrives by TMA.  Roles (10 warps, one
+// persistent CTA per SM): warp 0 = TMA producer (class tiles), warp 1 = MMA issuer + TMEM
+// allocation, warps 2-5 = epilogue (thread = query row), warps 6-9 = expanders (thread = query row).
+//
+// Reduction-axis permutation.  A sum over d is invariant under any permutation of d applied to both
+// operands, so the k-block position kappa <-> dimension map is chosen to make the expansion two or
+// three ALU ops per 32-bit shared-memory word (perm_bf16 / perm_i8 below); the class operand is
+// staged once per call in the same order by class_operand_kernel (it is tiny: K x D_eff).
+//
+// Class operand precisions (S5): bf16 (hv_bits 16); fp32 (hv_bits 32) as three bf16 parts
+// c1+c2+c3 stacked along the class axis of one tile -- the three partial accumulators are summed in
+// the epilogue, so the queries are expanded once; int8 (hv_bits 8) and +-1 int8 (hv_bits 1) with
+// int32 accumulation (exact).
+#include <limits.h>
+
+#include <type_traits>
+
+#include "common.cuh"
+#include "tc_ptx.cuh"
+
+namespace hdc {
+namespace {
+
+using namespace tcp;
+
+constexpr int BM = 128;
+constexpr int BN_MAX = 256;
+constexpr int STAGES = 4;
+constexpr int A_BYTES = BM * KB_BYTES;
+constexpr int B_BYTES = BN_MAX * KB_BYTES;
+constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
+constexpr int NTHREADS = 320;
+constexpr int TMEM_COLS = 512;
+constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 + 256;
+constexpr int CH = 16;  // packed words a thread keeps in flight per register chunk
+
+// dimension offset (within a k-block) of shared-memory K position kappa
+__host__ __device__ __forceinline__ int perm_bf16(int kappa) {  // k-block = 64 dims = 2 words
+  const int i = kappa >> 1;
+  return 32 * (i >> 4) + (i & 15) + 16 * (kappa & 1);
+}
+__host__ __device__ __forceinline__ int perm_i8(int kappa) {  // k-block = 128 dims = 4 words
+  const int i = kappa >> 2;
+  return 32 * (i >> 3) + 8 * (kappa & 3) + (i & 7);
+}
+
+struct SimParams {
+  const uint32_t* Hbits;
+  int64_t N;
+  int64_t ldh;
+  int W;        // words holding d < D_eff
+  int K;        // classes
+  int kc;       // classes per n-tile (multiple of 16)
+  int nparts;   // 1, or 3 for the fp32 class operand
+  int m_tiles, n_tiles;
+  int num_kb;
+  Epilogue e;
+};
+
+struct Top2 {
+  double b1;
+  int i1;
+  double b2;
+};
+constexpr double NEG_BIG = -1.0e300;
+
+__device__ __forceinline__ uint32_t prmt_sign_bytes(uint32_t v) {
+  uint32_t d;
+  asm("prmt.b32 %0, %1, %1, 0xBA98;" : "=r"(d) : "r"(v));  // byte b <- 0xFF if msb of byte b of v else 0
+  return d;
+}
+
+template <bool INT8, int EPI>
+__global__ void __launch_bounds__(NTHREADS, 1)
+sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  const uint32_t bar0 = base + STAGES * STAGE_BYTES;
+  auto full_bar = [&](int s) { return bar0 + 8u * s; };
+  auto empty_bar = [&](int s) { return bar0 + 8u * (STAGES + s); };
+  auto tfull_bar = [&](int s) { return bar0 + 8u * (2 * STAGES + s); };
+  auto tempty_bar = [&](int s) { return bar0 + 8u * (2 * STAGES + 2 + s); };
+  const uint32_t tmem_slot = bar0 + 8u * (2 * STAGES + 4);
+  uint32_t* tmem_slot_ptr = reinterpret_cast<uint32_t*>(smem_raw + (tmem_slot - smem_u32(smem_raw)));
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  constexpr int BK = INT8 ? 128 : 64;
+  const int nb_rows = p.nparts * p.kc;
+
+  if (warp == 0 && lane == 0) {
+    asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&tmB)) : "memory");
+    for (int s = 0; s < STAGES; ++s) {
+      mbar_init(full_bar(s), 5);  // producer (with the TMA byte count) + one arrival per expander warp
+      mbar_init(empty_bar(s), 1);
+    }
+    for (int s = 0; s < 2; ++s) {
+      mbar_init(tfull_bar(s), 1);
+      mbar_init(tempty_bar(s), 4);
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  if (warp == 1) tmem_alloc(tmem_slot, TMEM_COLS);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = *tmem_slot_ptr;
+
+  const int64_t tiles_per_cta =
+      (p.m_tiles > (int)blockIdx.x) ? ((int64_t)(p.m_tiles - 1 - (int)blockIdx.x) / gridDim.x + 1) * p.n_tiles : 0;
+
+  if (warp == 0) {
+    // ================================================================= TMA producer (class tiles)
+    int stage = 0;
+    uint32_t phase = 0;
+    for (int64_t i = 0; i < tiles_per_cta; ++i) {
+      const int nt = (int)(i % p.n_tiles);
+      for (int kb = 0; kb < p.num_kb; ++kb) {
+        mbar_wait(empty_bar(stage), phase ^ 1u);
+        if (lane == 0) {
+          mbar_arrive_expect_tx(full_bar(stage), (uint32_t)nb_rows * KB_BYTES);
+          tma_load_2d(base + stage * STAGE_BYTES + A_BYTES, &tmB, full_bar(stage), kb * BK, nt * nb_rows);
+        }
+        __syncwarp();
+        if (++stage == STAGES) {
+          stage = 0;
+          phase ^= 1u;
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ================================================================= MMA issuer
+    int stage = 0;
+    uint32_t phase = 0;
+    int acc = 0;
+    uint32_t acc_phase = 0;
+    const uint32_t idesc = instr_desc<INT8>(BM, nb_rows);
+    for (int64_t i = 0; i < tiles_per_cta; ++i) {
+      mbar_wait(tempty_bar(acc), acc_phase ^ 1u);
+      tc_fence_after();
+      const uint32_t d_tmem = tmem_base + (uint32_t)(acc * BN_MAX);
+      for (int kb = 0; kb < p.num_kb; ++kb) {
+        mbar_wait(full_bar(stage), phase);
+        tc_fence_after();
+        if (lane == 0) {
+          const uint32_t sa = base + stage * STAGE_BYTES;
+          const uint64_t da = smem_desc(sa), db = smem_desc(sa + A_BYTES);
+#pragma unroll
+          for (int k = 0; k < KB_BYTES / 32; ++k)
+            tc_mma<INT8>(d_tmem, da + 2u * k, db + 2u * k, idesc, (kb | k) != 0 ? 1u : 0u);
+          tc_commit(empty_bar(stage));
+          if (kb == p.num_kb - 1) tc_commit(tfull_bar(acc));
+        }
+        __syncwarp();
+        if (++stage == STAGES) {
+          stage = 0;
+          phase ^= 1u;
+        }
+      }
+      if (++acc == 2) {
+        acc = 0;
+        acc_phase ^= 1u;
+      }
+    }
+  } else if (warp < 6) {
+    // ================================================================= epilogue (warps 2..5)
+    const int q = warp & 3;
+    int acc = 0;
+    uint32_t acc_phase = 0;
+    Top2 run = Top2{NEG_BIG, INT_MAX, NEG_BIG};
+    for (int64_t i = 0; i < tiles_per_cta; ++i) {
+      const int mt = (int)blockIdx.x + (int)(i / p.n_tiles) * (int)gridDim.x;
+      const int nt = (int)(i % p.n_tiles);
+      const int64_t row = (int64_t)mt * BM + q * 32 + lane;
+      const bool row_ok = row < p.N;
+      mbar_wait(tfull_bar(acc), acc_phase);
+      tc_fence_after();
+      const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(acc * BN_MAX);
+      const int k_base = nt * p.kc;
+      int k_valid = p.K - k_base;
+      if (k_valid > p.kc) k_valid = p.kc;
+      for (int c0 = 0; c0 < k_valid; c0 += 16) {
+        uint32_t v0[16], v1[16], v2[16];
+        tmem_ld16(taddr + (uint32_t)c0, v0);
+        if (!INT8 && p.nparts == 3) {
+          tmem_ld16(taddr + (uint32_t)(p.kc + c0), v1);
+          tmem_ld16(taddr + (uint32_t)(2 * p.kc + c0), v2);
+        }
+        tmem_ld_wait();
+#pragma unroll
+        for (int j = 0; j < 16; ++j) {
+          if (c0 + j < k_valid) {
+            const int k = k_base + c0 + j;
+            double a;
+            if (INT8) {
+              a = (double)(int)v0[j];
+            } else if (p.nparts == 3) {
+              a = ((double)__uint_as_float(v2[j]) + (double)__uint_as_float(v1[j])) + (double)__uint_as_float(v0[j]);
+            } else {
+              a = (double)__uint_as_float(v0[j]);
+            }
+            if (EPI == EPI_SCORE) {
+              if (row_ok) {
+                if (p.e.s_i32) {
+                  int iv = (int)v0[j];
+                  if (p.e.ham_D > 0) iv = (p.e.ham_D - iv) >> 1;
+                  reinterpret_cast<int32_t*>(p.e.S)[row * p.e.lds + k] = iv;
+                } else {
+                  const float s = p.e.colscale ? (float)(a * p.e.colscale[k]) : (float)a;
+                  reinterpret_cast<float*>(p.e.S)[row * p.e.lds + k] = s;
+                }
+              }
+            } else {
+              const double s = p.e.colscale ? a * p.e.colscale[k] : a;
+              if (s > run.b1) {  // classes arrive in increasing order: strict > keeps the lowest index
+                run.b2 = run.b1;
+                run.b1 = s;
+                run.i1 = k;
+              } else if (s > run.b2) {
+                run.b2 = s;
+              }
+            }
+          }
+        }
+      }
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(tempty_bar(acc));
+      if (++acc == 2) {
+        acc = 0;
+        acc_phase ^= 1u;
+      }
+      if (EPI == EPI_ARGMAX && nt == p.n_tiles - 1) {
+        if (row_ok) {
+          double b1 = run.b1, b2 = run.b2;
+          if (b2 == NEG_BIG) b2 = b1;  // K == 1
+          if (p.e.ham_D > 0) {
+            b1 = 0.5 * ((double)p.e.ham_D - b1);
+            b2 = 0.5 * ((double)p.e.ham_D - b2);
+          }
+          p.e.labels[row] = run.i1;
+          if (p.e.best) p.e.best[row] = (float)b1;
+          if (p.e.second) p.e.second[row] = (float)b2;
+        }
+        run = Top2{NEG_BIG, INT_MAX, NEG_BIG};
+      }
+    }
+  } else {
+    // ================================================================= expanders (warps 6..9)
+    const int t = (int)threadIdx.x - 192;  // row of the tile
+    constexpr int WPK = INT8 ? 4 : 2;      // packed words per k-block
+    constexpr int KPC = CH / WPK;          // k-blocks per register chunk
+    const uint32_t sw = (uint32_t)(t & 7);
+    const bool vec_ok = ((p.ldh & 3) == 0) && ((reinterpret_cast<uintptr_t>(p.Hbits) & 15) == 0);
+    int stage = 0;
+    uint32_t phase = 0;
+    for (int64_t i = 0; i < tiles_per_cta; ++i) {
+      const int mt = (int)blockIdx.x + (int)(i / p.n_tiles) * (int)gridDim.x;
+      const int64_t row = (int64_t)mt * BM + t;
+      const bool row_ok = row < p.N;
+      const uint32_t* hrow = p.Hbits + (row_ok ? row : 0) * p.ldh;
+      uint32_t cur[CH], nxt[CH];
+      auto load_chunk = [&](uint32_t (&dst)[CH], int w0) {
+        if (row_ok && vec_ok && w0 + CH <= p.W) {
+#pragma unroll
+          for (int u = 0; u < CH / 4; ++u) {
+            const uint4 x = __ldg(reinterpret_cast<const uint4*>(hrow + w0) + u);
+            dst[4 * u] = x.x;
+            dst[4 * u + 1] = x.y;
+            dst[4 * u + 2] = x.z;
+            dst[4 * u + 3] = x.w;
+          }
+        } else {
+#pragma unroll
+          for (int u = 0; u < CH; ++u) dst[u] = (row_ok && w0 + u < p.W) ? __ldg(hrow + w0 + u) : 0u;
+        }
+      };
+      load_chunk(nxt, 0);
+      for (int kb0 = 0; kb0 < p.num_kb; kb0 += KPC) {
+#pragma unroll
+        for (int u = 0; u < CH; ++u) cur[u] = nxt[u];
+        if (kb0 + KPC < p.num_kb) load_chunk(nxt, (kb0 + KPC) * WPK);
+#pragma unroll
+        for (int j = 0; j < KPC; ++j) {
+          if (kb0 + j < p.num_kb) {
+            mbar_wait(empty_bar(stage), phase ^ 1u);
+            const uint32_t a_row = base + stage * STAGE_BYTES + (uint32_t)t * KB_BYTES;
+#pragma unroll
+            for (int c = 0; c < 8; ++c) {  // 16-byte chunk c of the row = 4 shared-memory words
+              uint32_t o[4];
+#pragma unroll
+              for (int e = 0; e < 4; ++e) {
+                const int iw = 4 * c + e;  // word index within the k-block's 32 output words
+                if (INT8) {
+                  const uint32_t w = cur[j * WPK + (iw >> 3)];
+                  o[e] = prmt_sign_bytes(w << (7 - (iw & 7))) | 0x01010101u;
+                } else {
+                  const uint32_t w = cur[j * WPK + (iw >> 4)];
+                  o[e] = ((w << (15 - (iw & 15))) & 0x80008000u) | 0x3F803F80u;
+                }
+              }
+              const uint32_t dst = a_row + ((((uint32_t)c) ^ sw) << 4);
+              asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(dst), "r"(o[0]), "r"(o[1]), "r"(o[2]),
+                           "r"(o[3])
+                           : "memory");
+            }
+            fence_proxy_async_smem();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(full_bar(stage));
+            if (++stage == STAGES) {
+              stage = 0;
+              phase ^= 1u;
+            }
+          }
+        }
+      }
+    }
+  }
+
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) {
+    tc_fence_after();
+    tmem_dealloc(tmem_base, TMEM_COLS);
+  }
+}
+
+// ---------------------------------------------------------------------------------- class operand
+// Stages the class operand of sim_tc_kernel from the fp32 accumulators: staged row r holds class
+// k = tile*kc + (r % (nparts*kc)) % kc, part (r % (nparts*kc)) / kc of tile r / (nparts*kc); staged
+// column kb*BK + kappa holds dimension kb*BK + perm(kappa), zero for d >= D_eff or k >= K.
+// mode: 32 -> bf16 part j of the 3-way split; 16 -> bf16 RNE; 8 -> int8 with scale 127/amax;
+// 1 -> +-1 int8 from the sign.
+__device__ __forceinline__ int quant_i8_c(float x, float s) {
+  float q = rintf(__fmul_rn(x, s));
+  q = fminf(fmaxf(q, -127.0f), 127.0f);
+  return (int)q;
+}
+
+template <bool INT8>
+__global__ void class_operand_kernel(const float* __restrict__ C, int K, int D_eff, int64_t ldc, int mode,
+                                     int kc, int nparts, int rows_total, int num_kb,
+                                     const float* __restrict__ amax, void* __restrict__ dst) {
+  constexpr int BK = INT8 ? 128 : 64;
+  const int64_t ld = (int64_t)num_kb * BK;
+  const int64_t total = (int64_t)rows_total * ld;
+  float s = 1.0f;
+  if (mode == 8) {
+    const float a = *amax;
+    s = a > 0.0f ? __fdiv_rn(127.0f, a) : 1.0f;
+  }
+  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < total;
+       i += (int64_t)gridDim.x * blockDim.x) {
+    const int r = (int)(i / ld);
+    const int col = (int)(i - (int64_t)r * ld);
+    const int rem = r % (nparts * kc);
+    const int part = rem / kc;
+    const int k = (r / (nparts * kc)) * kc + rem % kc;
+    const int kb = col / BK, kappa = col % BK;
+    const int d = kb * BK + (INT8 ? perm_i8(kappa) : perm_bf16(kappa));
+    float x = 0.0f;
+    const bool live = k < K && d < D_eff;
+    if (live) x = __ldg(C + (int64_t)k * ldc + d);
+    if (INT8) {
+      int qv = 0;
+      if (live) qv = (mode == 8) ? quant_i8_c(x, s) : (x < 0.0f ? -1 : 1);
+      reinterpret_cast<int8_t*>(dst)[i] = (int8_t)qv;
+    } else {
+      __nv_bfloat16 b1 = __float2bfloat16_rn(x);
+      if (mode == 32 && part > 0) {
+        const float r1 = __fsub_rn(x, __bfloat162float(b1));
+        b1 = __float2bfloat16_rn(r1);
+        if (part > 1) {
+          const float r2 = __fsub_rn(r1, __bfloat162float(b1));
+          b1 = __float2bfloat16_rn(r2);
+        }
+      }
+      reinterpret_cast<__nv_bfloat16*>(dst)[i] = b1;
+    }
+  }
+}
+
+template <bool INT8, int EPI>
+cudaError_t launch_one(const CUtensorMap& tmB, const SimParams& p, int grid, cudaStream_t st) {
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaError_t e = cudaFuncSetAttribute(sim_tc_kernel<INT8, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         SMEM_BYTES);
+    if (e != cudaSuccess) return e;
+    attr_set = true;
+  }
+  sim_tc_kernel<INT8, EPI><<<grid, NTHREADS, SMEM_BYTES, st>>>(tmB, p);
+  return cudaGetLastError();
+}
+
+void sim_tc_shape(int K, int hv_bits, int D_eff, int& kc, int& nparts, int& n_tiles, int& num_kb, bool& int8) {
+  int8 = hv_bits == 8 || hv_bits == 1;
+  nparts = hv_bits == 32 ? 3 : 1;
+  const int kc_max = nparts == 3 ? 80 : 256;
+  kc = (K + 15) & ~15;
+  if (kc > kc_max) kc = kc_max;
+  n_tiles = (K + kc - 1) / kc;
+  const int BK = int8 ? 128 : 64;
+  num_kb = (D_eff + BK - 1) / BK;
+}
+
+}  // namespace
+
+size_t sim_tc_operand_bytes(int K, int hv_bits, int D_eff) {
+  int kc, nparts, n_tiles, num_kb;
+  bool int8;
+  sim_tc_shape(K, hv_bits, D_eff, kc, nparts, n_tiles, num_kb, int8);
+  return (size_t)n_tiles * nparts * kc * num_kb * KB_BYTES;
+}
+
+cudaError_t launch_sim_tc(TcContext* tc, const uint32_t* Hbits, int64_t N, int64_t ldh, const float* C_acc,
+                          int K, int64_t ldc, int D_eff, int hv_bits, void* cop, float* amax_scratch,
+                          const Epilogue& e, int sm_count, cudaStream_t st, int64_t* nlaunch) {
+  if (!tc) return cudaErrorNotSupported;
+  if (N <= 0) return cudaSuccess;
+  if ((reinterpret_cast<uintptr_t>(cop) & 15) != 0) return cudaErrorNotSupported;
+  int kc, nparts, n_tiles, num_kb;
+  bool int8;
+  sim_tc_shape(K, hv_bits, D_eff, kc, nparts, n_tiles, num_kb, int8);
+  const int rows_total = n_tiles * nparts * kc;
+  const int BK = int8 ? 128 : 64;
+  const int64_t ld = (int64_t)num_kb * BK;
+  cudaError_t ce;
+  if (hv_bits == 8) {
+    ce = launch_tensor_amax(C_acc, K, D_eff, ldc, amax_scratch, st, nlaunch);
+    if (ce != cudaSuccess) return ce;
+  }
+  {
+    const int64_t total = (int64_t)rows_total * ld;
+    int64_t g = (total + 255) / 256;
+    if (g > (int64_t)sm_count * 16) g = (int64_t)sm_count * 16;
+    if (int8)
+      class_operand_kernel<true><<<(unsigned)g, 256, 0, st>>>(C_acc, K, D_eff, ldc, hv_bits, kc, nparts, rows_total,
+                                                             num_kb, amax_scratch, cop);
+    else
+      class_operand_kernel<false><<<(unsigned)g, 256, 0, st>>>(C_acc, K, D_eff, ldc, hv_bits, kc, nparts,
+                                                              rows_total, num_kb, amax_scratch, cop);
+    ++*nlaunch;
+    ce = cudaGetLastError();
+    if (ce != cudaSuccess) return ce;
+  }
+  CUtensorMap tmB;
+  if (!tc_make_map(tc, &tmB, cop, int8, rows_total, ld, ld, nparts * kc)) return cudaErrorInvalidValue;
+  SimParams p;
+  p.Hbits = Hbits;
+  p.N = N;
+  p.ldh = ldh;
+  p.W = words_of(D_eff);
+  p.K = K;
+  p.kc = kc;
+  p.nparts = nparts;
+  p.m_tiles = (int)((N + BM - 1) / BM);
+  p.n_tiles = n_tiles;
+  p.num_kb = num_kb;
+  p.e = e;
+  const int grid = p.m_tiles < sm_count ? p.m_tiles : sm_count;
+  ++*nlaunch;
+  if (int8)
+    return e.kind == EPI_SCORE ? launch_one<true, EPI_SCORE>(tmB, p, grid, st)
+                               : launch_one<true, EPI_ARGMAX>(tmB, p, grid, st);
+  return e.kind == EPI_SCORE ? launch_one<false, EPI_SCORE>(tmB, p, grid, st)
+                             : launch_one<false, EPI_ARGMAX>(tmB, p, grid, st);
+}
+
+}  // namespace hdc
