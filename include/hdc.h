@@ -104,6 +104,16 @@ int32_t hdc_version(void);
 /* Number of kernel launches this handle has enqueued since creation (bench `gpu_launches`). */
 int64_t hdc_launch_count(hdc_handle_t h);
 
+/* Per-kernel device timing (for roofline reporting).  While enabled, the dominant kernel of each
+ * entry point is bracketed by CUDA events on the caller's stream: HDC_K_ENCODE_GEMM (contraction of
+ * hdc_encode_rp, staging excluded), HDC_K_SIM (similarity / classify kernel, operand staging
+ * excluded), HDC_K_LEVELID, HDC_K_CLASS_UPDATE.  hdc_kernel_time() synchronises the recorded events,
+ * returns the summed milliseconds and the number of launches of that kernel since the last call (or
+ * since enabling) and resets them.  At most 1024 launches per kernel id are kept between reads. */
+enum { HDC_K_ENCODE_GEMM = 0, HDC_K_SIM = 1, HDC_K_LEVELID = 2, HDC_K_CLASS_UPDATE = 3, HDC_K_COUNT = 4 };
+int32_t hdc_kernel_timing(hdc_handle_t h, int32_t enable);
+int32_t hdc_kernel_time(hdc_handle_t h, int32_t kernel_id, float* ms_total, int64_t* launches);
+
 /* Bytes of device workspace the given op needs for these sizes and knobs (0 is possible).
  * F_or_Q: F for encode_rp / infer_rp_host, Q for encode_levelid, ignored otherwise.
  * For HDC_OP_TRAIN_EPOCH, N is the mini-batch size actually used (batch, or N when batch = 0). */

@@ -23,10 +23,12 @@ HDC_OUT_BITS, HDC_OUT_RAW = 1, 4
 HDC_OP_ENCODE_RP, HDC_OP_ENCODE_LEVELID, HDC_OP_SIMILARITY = 0, 1, 2
 HDC_OP_CLASSIFY, HDC_OP_TRAIN_EPOCH, HDC_OP_INFER_RP_HOST = 3, 4, 5
 HDC_FLAG_NONE, HDC_FLAG_SIMT = 0, 1
+HDC_K_ENCODE_GEMM, HDC_K_SIM, HDC_K_LEVELID, HDC_K_CLASS_UPDATE = 0, 1, 2, 3
 
 EXPORTS = ("hdc_create", "hdc_destroy", "hdc_last_error", "hdc_version", "hdc_launch_count",
            "hdc_workspace_bytes", "hdc_encode_rp", "hdc_encode_levelid", "hdc_similarity",
-           "hdc_classify", "hdc_train_epoch", "hdc_infer_rp_host")
+           "hdc_classify", "hdc_train_epoch", "hdc_infer_rp_host", "hdc_kernel_timing",
+           "hdc_kernel_time")
 
 
 class hdc_knobs_t(C.Structure):
@@ -82,6 +84,10 @@ def lib() -> C.CDLL:
     L.hdc_infer_rp_host.argtypes = [vp, vp, i32, i64, i32, i64, vp, i32, i32, i64, vp, i32, i64, kp, vp, vp,
                                     sz, vp]
     L.hdc_infer_rp_host.restype = i32
+    L.hdc_kernel_timing.argtypes = [vp, i32]
+    L.hdc_kernel_timing.restype = i32
+    L.hdc_kernel_time.argtypes = [vp, i32, C.POINTER(C.c_float), C.POINTER(i64)]
+    L.hdc_kernel_time.restype = i32
     _lib = L
     return L
 
@@ -138,6 +144,15 @@ class Handle:
 
     def launch_count(self) -> int:
         return int(self._L.hdc_launch_count(self._h))
+
+    def kernel_timing(self, enable: bool):
+        self._check(self._L.hdc_kernel_timing(self._h, 1 if enable else 0))
+
+    def kernel_time(self, kernel_id: int):
+        """(summed ms, launches) of one kernel id since the last read; synchronises its events."""
+        ms, n = C.c_float(0.0), C.c_int64(0)
+        self._check(self._L.hdc_kernel_time(self._h, kernel_id, C.byref(ms), C.byref(n)))
+        return float(ms.value), int(n.value)
 
     def workspace_bytes(self, op: int, N: int, F_or_Q: int, D: int, K: int, kn: hdc_knobs_t) -> int:
         return int(self._L.hdc_workspace_bytes(self._h, op, N, F_or_Q, D, K, C.byref(kn)))

@@ -4,6 +4,8 @@
 #include <stdio.h>
 
 #include <string>
+#include <utility>
+#include <vector>
 
 #include "common.cuh"
 
@@ -18,6 +20,9 @@ struct hdc_ctx {
   cudaEvent_t ev_copied[2] = {nullptr, nullptr};
   cudaEvent_t ev_done[2] = {nullptr, nullptr};
   cudaEvent_t ev_entry = nullptr;
+  bool timing = false;
+  std::vector<std::pair<cudaEvent_t, cudaEvent_t>> tev[HDC_K_COUNT];  // event pool per kernel id
+  size_t tused[HDC_K_COUNT] = {0, 0, 0, 0};
 };
 
 namespace hdc {
@@ -45,6 +50,27 @@ int cuda_fail(hdc_ctx* h, cudaError_t e, const char* where) {
   if (h) h->err = std::string(where) + ": " + cudaGetErrorString(e);
   return HDC_ERR_CUDA;
 }
+// Brackets one kernel launch with CUDA events on `st` while hdc_kernel_timing is enabled.
+struct Timed {
+  hdc_ctx* h;
+  cudaStream_t st;
+  cudaEvent_t stop = nullptr;
+  Timed(hdc_ctx* h_, int id, cudaStream_t st_) : h(h_), st(st_) {
+    if (!h->timing || h->tused[id] >= 1024) return;
+    if (h->tused[id] == h->tev[id].size()) {
+      cudaEvent_t a, b;
+      if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) return;
+      h->tev[id].push_back({a, b});
+    }
+    auto& pr = h->tev[id][h->tused[id]++];
+    cudaEventRecord(pr.first, st);
+    stop = pr.second;
+  }
+  ~Timed() {
+    if (stop) cudaEventRecord(stop, st);
+  }
+};
+
 bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15) == 0; }
 
 int check_knobs(hdc_ctx* h, const hdc_knobs_t* k, int D) {
@@ -134,11 +160,17 @@ int do_encode_rp(hdc_ctx* h, const void* X, int x_dtype, int64_t N, int F, int64
       if (ce != cudaSuccess) return cuda_fail(h, ce, "split P");
       TcOperands o{pl.Xs, pl.Ps, OPK_BF16, pl.ldxs, pl.ldps, pl.ldxs, pl.ldps, pl.Fp, 6,
                    SPLIT_A_SEGS, SPLIT_B_SEGS, pl.Fp};
-      ce = launch_gemm_tc(h->tc, o, N, D_eff, e, h->sm_count, st, &h->launches);
+      {
+        Timed tm(h, HDC_K_ENCODE_GEMM, st);
+        ce = launch_gemm_tc(h->tc, o, N, D_eff, e, h->sm_count, st, &h->launches);
+      }
       if (ce == cudaSuccess) return HDC_OK;
       if (ce != cudaErrorNotSupported) return cuda_fail(h, ce, "encode_rp fp32 tcgen05");
     }
-    ce = launch_gemm_simt(Operand{X, ldx, xk}, Operand{P, ldp, pk}, N, D_eff, F, false, e, st, &h->launches);
+    {
+      Timed tm(h, HDC_K_ENCODE_GEMM, st);
+      ce = launch_gemm_simt(Operand{X, ldx, xk}, Operand{P, ldp, pk}, N, D_eff, F, false, e, st, &h->launches);
+    }
     return ce == cudaSuccess ? HDC_OK : cuda_fail(h, ce, "encode_rp fp32");
   }
 
@@ -160,7 +192,10 @@ int do_encode_rp(hdc_ctx* h, const void* X, int x_dtype, int64_t N, int F, int64
     }
     if (pl.tc) {
       TcOperands o{pl.Xs, Pq, OPK_I8, pl.ldxs, ldpq, F, F, F, 1, 0u, 0u, 0};
-      ce = launch_gemm_tc(h->tc, o, N, D_eff, e, h->sm_count, st, &h->launches);
+      {
+        Timed tm(h, HDC_K_ENCODE_GEMM, st);
+        ce = launch_gemm_tc(h->tc, o, N, D_eff, e, h->sm_count, st, &h->launches);
+      }
       if (ce == cudaSuccess) return HDC_OK;
       if (ce != cudaErrorNotSupported) return cuda_fail(h, ce, "encode_rp int8 tcgen05");
     }
@@ -189,7 +224,10 @@ int do_encode_rp(hdc_ctx* h, const void* X, int x_dtype, int64_t N, int F, int64
       ldpb = pl.ldps;
     }
     TcOperands o{Xb, Pb, OPK_BF16, ldxb, ldpb, F, F, F, 1, 0u, 0u, 0};
-    ce = launch_gemm_tc(h->tc, o, N, D_eff, e, h->sm_count, st, &h->launches);
+    {
+      Timed tm(h, HDC_K_ENCODE_GEMM, st);
+      ce = launch_gemm_tc(h->tc, o, N, D_eff, e, h->sm_count, st, &h->launches);
+    }
     if (ce == cudaSuccess) return HDC_OK;
     if (ce != cudaErrorNotSupported) return cuda_fail(h, ce, "encode_rp bf16 tcgen05");
   }
@@ -244,8 +282,11 @@ int do_similarity(hdc_ctx* h, const uint32_t* Hbits, int64_t N, int64_t ldh, con
       e.lds = lds;
       e.s_i32 = s_i32;
     }
-    ce = launch_sim_tc(h->tc, Hbits, N, ldh, C_acc, K, ldc, D_eff, k->hv_bits, cop, amax, e, h->sm_count, st,
-                       &h->launches);
+    {
+      Timed tm(h, HDC_K_SIM, st);
+      ce = launch_sim_tc(h->tc, Hbits, N, ldh, C_acc, K, ldc, D_eff, k->hv_bits, cop, amax, e, h->sm_count, st,
+                         &h->launches);
+    }
     if (ce == cudaSuccess) return HDC_OK;
     if (ce != cudaErrorNotSupported) return cuda_fail(h, ce, "similarity tcgen05");
   }
@@ -254,8 +295,11 @@ int do_similarity(hdc_ctx* h, const uint32_t* Hbits, int64_t N, int64_t ldh, con
     if (b.off > ws_bytes) return fail(h, HDC_ERR_WORKSPACE, "similarity: workspace too small");
     ce = launch_sign_bits(C_acc, K, D_eff, ldc, cbits, W, st, &h->launches);
     if (ce != cudaSuccess) return cuda_fail(h, ce, "sign_bits");
-    ce = launch_hamming(Hbits, N, ldh, cbits, K, W, D_eff, (int32_t*)S, lds, labels, best, second,
-                        h->sm_count, h->smem_optin, st, &h->launches);
+    {
+      Timed tm(h, HDC_K_SIM, st);
+      ce = launch_hamming(Hbits, N, ldh, cbits, K, W, D_eff, (int32_t*)S, lds, labels, best, second,
+                          h->sm_count, h->smem_optin, st, &h->launches);
+    }
     return ce == cudaSuccess ? HDC_OK : cuda_fail(h, ce, "hamming");
   }
   // DOT / COS: contraction of +-1 queries with the class operand at hv_bits
@@ -366,6 +410,11 @@ extern "C" int32_t hdc_destroy(hdc_handle_t h) {
   }
   if (h->ev_entry) cudaEventDestroy(h->ev_entry);
   if (h->copy_stream) cudaStreamDestroy(h->copy_stream);
+  for (auto& v : h->tev)
+    for (auto& pr : v) {
+      cudaEventDestroy(pr.first);
+      cudaEventDestroy(pr.second);
+    }
   tc_context_destroy(h->tc);
   delete h;
   return HDC_OK;
@@ -374,6 +423,31 @@ extern "C" int32_t hdc_destroy(hdc_handle_t h) {
 extern "C" const char* hdc_last_error(hdc_handle_t h) { return h ? h->err.c_str() : "null handle"; }
 
 extern "C" int64_t hdc_launch_count(hdc_handle_t h) { return h ? h->launches : -1; }
+
+extern "C" int32_t hdc_kernel_timing(hdc_handle_t h, int32_t enable) {
+  if (!h) return HDC_ERR_INVALID_ARG;
+  h->timing = enable != 0;
+  for (auto& u : h->tused) u = 0;
+  return HDC_OK;
+}
+
+extern "C" int32_t hdc_kernel_time(hdc_handle_t h, int32_t kernel_id, float* ms_total, int64_t* launches) {
+  if (!h || kernel_id < 0 || kernel_id >= HDC_K_COUNT || !ms_total || !launches)
+    return h ? fail(h, HDC_ERR_INVALID_ARG, "kernel_time: bad argument") : HDC_ERR_INVALID_ARG;
+  float total = 0.0f;
+  for (size_t i = 0; i < h->tused[kernel_id]; ++i) {
+    auto& pr = h->tev[kernel_id][i];
+    cudaError_t ce = cudaEventSynchronize(pr.second);
+    float ms = 0.0f;
+    if (ce == cudaSuccess) ce = cudaEventElapsedTime(&ms, pr.first, pr.second);
+    if (ce != cudaSuccess) return cuda_fail(h, ce, "kernel_time");
+    total += ms;
+  }
+  *ms_total = total;
+  *launches = (int64_t)h->tused[kernel_id];
+  h->tused[kernel_id] = 0;
+  return HDC_OK;
+}
 
 // =================================================================================== workspace
 extern "C" size_t hdc_workspace_bytes(hdc_handle_t h, int32_t op, int64_t N, int32_t F_or_Q, int32_t D,
@@ -474,9 +548,12 @@ extern "C" int32_t hdc_encode_levelid(hdc_handle_t h, const uint8_t* levels, int
        reinterpret_cast<uintptr_t>(Hbits)) & 3)
     return fail(h, HDC_ERR_ALIGNMENT, "encode_levelid: bit matrices must be 4-byte aligned");
   if (N == 0) return HDC_OK;
-  cudaError_t ce = launch_levelid(levels, N, F, ldl, IDbits, ldid_words, LVbits, Q, ldlv_words, knobs->D_eff,
-                                  Hbits, ldh_words, h->sm_count, h->smem_optin, (cudaStream_t)stream,
-                                  &h->launches);
+  cudaError_t ce;
+  {
+    Timed tm(h, HDC_K_LEVELID, (cudaStream_t)stream);
+    ce = launch_levelid(levels, N, F, ldl, IDbits, ldid_words, LVbits, Q, ldlv_words, knobs->D_eff, Hbits,
+                        ldh_words, h->sm_count, h->smem_optin, (cudaStream_t)stream, &h->launches);
+  }
   return ce == cudaSuccess ? HDC_OK : cuda_fail(h, ce, "encode_levelid");
 }
 
@@ -577,8 +654,11 @@ extern "C" int32_t hdc_train_epoch(hdc_handle_t h, int32_t mode, const uint32_t*
                        nullptr, bs, ws_bytes, st);
     if (rc) return rc;
     // class_update indexes y and pred with absolute sample numbers
-    ce = launch_class_update(Hbits, n0, nb, ldh_words, y, pb - n0, C_acc, K, ldc, k.D_eff, lr, delta, n_wrong,
-                             h->sm_count, st, &h->launches);
+    {
+      Timed tm(h, HDC_K_CLASS_UPDATE, st);
+      ce = launch_class_update(Hbits, n0, nb, ldh_words, y, pb - n0, C_acc, K, ldc, k.D_eff, lr, delta, n_wrong,
+                               h->sm_count, st, &h->launches);
+    }
     if (ce != cudaSuccess) return cuda_fail(h, ce, "class update");
   }
   return HDC_OK;
@@ -619,9 +699,13 @@ extern "C" int32_t hdc_infer_rp_host(hdc_handle_t h, const void* X_host, int32_t
     const int buf = (int)(c & 1);
     if (c >= 2) cudaStreamWaitEvent(h->copy_stream, h->ev_done[buf], 0);
     // rows are copied densely: device leading dimension is F
-    ce = cudaMemcpy2DAsync(Xd[buf], (size_t)F * es, (const char*)X_host + (size_t)n0 * ldx * es,
-                           (size_t)ldx * es, (size_t)F * es, (size_t)nb, cudaMemcpyHostToDevice,
-                           h->copy_stream);
+    if (ldx == F)
+      ce = cudaMemcpyAsync(Xd[buf], (const char*)X_host + (size_t)n0 * ldx * es, (size_t)nb * F * es,
+                           cudaMemcpyHostToDevice, h->copy_stream);
+    else
+      ce = cudaMemcpy2DAsync(Xd[buf], (size_t)F * es, (const char*)X_host + (size_t)n0 * ldx * es,
+                             (size_t)ldx * es, (size_t)F * es, (size_t)nb, cudaMemcpyHostToDevice,
+                             h->copy_stream);
     if (ce != cudaSuccess) return cuda_fail(h, ce, "infer_rp_host: H2D");
     cudaEventRecord(h->ev_copied[buf], h->copy_stream);
     cudaStreamWaitEvent(st, h->ev_copied[buf], 0);
