@@ -1,0 +1,213 @@
+"""Per-row measurements of the hot path beyond bench.py's headline step:
+each row times one entry point of the C ABI on device-resident, seeded synthetic inputs of the
+shapes of BASELINE.json's configs, with CUDA events around the calls and the library's own per-kernel
+events (hdc_kernel_time) for the dominant kernel, and states the roofline it is held against.
+
+    python -m paper_2606_26547_b200.bench_rows [--row NAME] [--reps R]
+
+Used by `bench.py --rows` and as the (committed) command of the ncu captures under profiles/.
+No arithmetic of the method lives here.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+
+import torch
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import paper_2606_26547_b200 as hd  # noqa: E402
+
+SEED = 26547
+
+
+def _gen(seed):
+    g = torch.Generator(device="cuda")
+    g.manual_seed(SEED + seed)
+    return g
+
+
+def _time(fn, reps, warm=3):
+    for _ in range(warm):
+        fn()
+    torch.cuda.synchronize()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record()
+    for _ in range(reps):
+        fn()
+    b.record()
+    torch.cuda.synchronize()
+    return a.elapsed_time(b) / reps
+
+
+def _kernel(h, kid, fn, reps):
+    h.kernel_timing(True)
+    for _ in range(reps):
+        fn()
+    torch.cuda.synchronize()
+    ms, n = h.kernel_time(kid)
+    h.kernel_timing(False)
+    return ms / max(1, n), n // max(1, reps)
+
+
+def _rand_bits(n, w, seed):
+    return torch.randint(-2 ** 31, 2 ** 31 - 1, (n, w), dtype=torch.int32, device="cuda", generator=_gen(seed))
+
+
+def _class_acc(K, D, seed, per_class=32):
+    """Accumulators shaped like a bundle of `per_class` bipolar hypervectors per class (exact ints)."""
+    u = torch.randint(0, 2, (per_class, K, D), dtype=torch.int8, device="cuda", generator=_gen(seed))
+    return (per_class - 2 * u.sum(0, dtype=torch.int32)).to(torch.float32).contiguous()
+
+
+# ------------------------------------------------------------------------------------ encode rows
+def row_encode(h, peaks, reps, N, F, D, prec_name, x_bf16=False):
+    prec = {"f32": hd.HDC_F32, "bf16": hd.HDC_BF16, "i8": hd.HDC_I8}[prec_name]
+    X = torch.randn((N, F), device="cuda", generator=_gen(1))
+    P = torch.randn((D, F), device="cuda", generator=_gen(2))
+    if x_bf16:
+        X, P = X.to(torch.bfloat16), P.to(torch.bfloat16)
+    kn = hd.knobs(D, precision=prec)
+    H = torch.empty((N, (D + 31) // 32), dtype=torch.int32, device="cuda")
+    fn = lambda: h.hdc_encode_rp(X, P, kn, Hbits=H)  # noqa: E731
+    call_ms = _time(fn, reps)
+    k_ms, _ = _kernel(h, hd.HDC_K_ENCODE_GEMM, fn, reps)
+    flops = 2.0 * N * F * D
+    mult = {"f32": 1.0 / 6.0, "bf16": 1.0, "i8": 2.0}[prec_name]
+    peak = peaks["bf16_tflops"] * mult
+    ach = flops / (k_ms * 1e-3) / 1e12
+    return {"what": f"hdc_encode_rp N={N} F={F} D={D} precision={prec_name}" + (" (bf16 inputs in place)" if x_bf16 else ""),
+            "call_ms": call_ms, "kernel_ms": k_ms, "queries_per_s": N / (call_ms * 1e-3),
+            "roofline": {"bound": "tensor", "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
+                         "peak_source": f"bf16_tflops (burst, measured) x {mult:.4g}"}}
+
+
+# ------------------------------------------------------------------------------------ similarity rows
+def row_classify(h, peaks, reps, N, K, D, hv_bits, sim_name):
+    sim = {"cos": hd.HDC_SIM_COS, "dot": hd.HDC_SIM_DOT, "hamming": hd.HDC_SIM_HAMMING}[sim_name]
+    W = (D + 31) // 32
+    H = _rand_bits(N, W, 3)
+    C = _class_acc(K, D, 4)
+    kn = hd.knobs(D, hv_bits=hv_bits, sim=sim)
+    lab = torch.empty(N, dtype=torch.int32, device="cuda")
+    fn = lambda: h.hdc_classify(H, C, kn, labels=lab)  # noqa: E731
+    call_ms = _time(fn, reps)
+    k_ms, _ = _kernel(h, hd.HDC_K_SIM, fn, reps)
+    out = {"what": f"hdc_classify N={N} K={K} D={D} hv_bits={hv_bits} sim={sim_name}", "call_ms": call_ms,
+           "kernel_ms": k_ms, "queries_per_s": N / (call_ms * 1e-3)}
+    hbm = N * W * 4 / (k_ms * 1e-3) / 1e9
+    out["hbm_GBps_query_bits"] = hbm
+    if sim_name == "hamming" and K < 64:
+        popc = float(N) * K * W / (k_ms * 1e-3) / 1e12
+        peak = 148 * 16 * peaks["sm_max_mhz"] * 1e6 / 1e12
+        out["roofline"] = {"bound": "alu", "achieved": popc, "peak": peak, "unit": "Tpopc/s", "frac": popc / peak,
+                           "peak_source": "148 SM x 16 POPC lanes x sm_max_mhz"}
+    else:
+        parts = 3 if hv_bits == 32 else 1
+        mult = 2.0 if hv_bits in (8, 1) else 1.0
+        kp = ((K + 15) // 16) * 16
+        flops = 2.0 * N * D * kp * parts
+        ach = flops / (k_ms * 1e-3) / 1e12
+        peak = peaks["bf16_tflops"] * mult
+        out["roofline"] = {"bound": "tensor" if K >= 128 else "hbm",
+                           "achieved": ach if K >= 128 else hbm,
+                           "peak": peak if K >= 128 else peaks["hbm_gbs"],
+                           "unit": "TFLOP/s" if K >= 128 else "GB/s",
+                           "frac": (ach / peak) if K >= 128 else hbm / peaks["hbm_gbs"],
+                           "executed_tflops": ach}
+    return out
+
+
+# ------------------------------------------------------------------------------------ level-ID row
+def row_levelid(h, peaks, reps, N=65536, F=784, Q=256, D=10000):
+    from workloads import gen
+    import numpy as np
+    w = gen.c3_mnist_shaped(D=D, n_tr=16, n_te=4096, Q=Q)
+    lv = torch.from_numpy(gen.tile_rows(w["Lte"], N)).cuda()
+    ID = torch.from_numpy(gen.pack_bits_lsb(w["ID"]).view(np.int32)).cuda()
+    LV = torch.from_numpy(gen.pack_bits_lsb(w["LV"]).view(np.int32)).cuda()
+    Wd = (D + 31) // 32
+    H = torch.empty((N, Wd), dtype=torch.int32, device="cuda")
+    kn = hd.knobs(D)
+    fn = lambda: h.hdc_encode_levelid(lv, ID, LV, D, kn, Hbits=H)  # noqa: E731
+    call_ms = _time(fn, reps)
+    k_ms, _ = _kernel(h, hd.HDC_K_LEVELID, fn, reps)
+    # algorithmic logic ops per sample: F*W binds + 30 LOP3 per 16 features per word for the CSA tree
+    # + ripple into the upper planes: ~ (1 + 30/16 + 14/16) * F * W
+    ops = (1.0 + 30.0 / 16.0 + 14.0 / 16.0) * F * Wd * N
+    ach = ops / (k_ms * 1e-3) / 1e12
+    peak = 148 * 64 * peaks["sm_max_mhz"] * 1e6 / 1e12
+    return {"what": f"hdc_encode_levelid N={N} F={F} Q={Q} D={D} (C3-shaped, ~80% zero pixels)", "call_ms": call_ms,
+            "kernel_ms": k_ms, "samples_per_s": N / (call_ms * 1e-3),
+            "hbm_GBps": N * (F + 4 * Wd) / (k_ms * 1e-3) / 1e9,
+            "roofline": {"bound": "alu", "achieved": ach, "peak": peak, "unit": "Tlop/s (32-bit logic ops)",
+                         "frac": ach / peak, "peak_source": "148 SM x 64 INT lanes x sm_max_mhz"}}
+
+
+# ------------------------------------------------------------------------------------ training row
+def row_train(h, peaks, reps, N=6238, K=26, D=10000, hv_bits=32, sim_name="cos"):
+    sim = {"cos": hd.HDC_SIM_COS, "hamming": hd.HDC_SIM_HAMMING}[sim_name]
+    W = (D + 31) // 32
+    H = _rand_bits(N, W, 5)
+    y = torch.randint(0, K, (N,), dtype=torch.int32, device="cuda", generator=_gen(6))
+    C = torch.zeros((K, D), dtype=torch.float32, device="cuda")
+    kn = hd.knobs(D, hv_bits=hv_bits, sim=sim)
+    h.hdc_train_epoch(hd.HDC_TRAIN_BUNDLE, H, y, C, kn)
+    fn = lambda: h.hdc_train_epoch(hd.HDC_TRAIN_PERCEPTRON, H, y, C, kn, lr=0.05, batch=0)  # noqa: E731
+    call_ms = _time(fn, reps)
+    return {"what": f"hdc_train_epoch (perceptron, B=N) N={N} K={K} D={D} hv_bits={hv_bits} sim={sim_name} "
+                    "on random hypervectors (every sample mispredicted: worst case for the class update)",
+            "call_ms": call_ms, "samples_per_s": N / (call_ms * 1e-3)}
+
+
+ROWS = {
+    "c2_encode_f32": lambda h, p, r: row_encode(h, p, r, 131072, 617, 10000, "f32"),
+    "c2_encode_bf16": lambda h, p, r: row_encode(h, p, r, 131072, 617, 10000, "bf16"),
+    "c2_encode_i8": lambda h, p, r: row_encode(h, p, r, 131072, 617, 10000, "i8"),
+    "c2_classify_cos32": lambda h, p, r: row_classify(h, p, r, 131072, 26, 10000, 32, "cos"),
+    "c4_classify_cos8": lambda h, p, r: row_classify(h, p, r, 131072, 6, 10000, 8, "cos"),
+    "c3_levelid": lambda h, p, r: row_levelid(h, p, r),
+    "c3_hamming_k10": lambda h, p, r: row_classify(h, p, r, 131072, 10, 10000, 1, "hamming"),
+    "c5_encode_bf16": lambda h, p, r: row_encode(h, p, r, 65536, 1024, 16384, "bf16", x_bf16=True),
+    "c5_classify_bf16": lambda h, p, r: row_classify(h, p, r, 65536, 1000, 16384, 16, "cos"),
+    "c5_classify_1bit": lambda h, p, r: row_classify(h, p, r, 65536, 1000, 16384, 1, "hamming"),
+    "c2_train_epoch": lambda h, p, r: row_train(h, p, r),
+}
+
+
+def run(h, peaks, reps=5, only=None):
+    out = {}
+    for name, fn in ROWS.items():
+        if only and name != only:
+            continue
+        out[name] = fn(h, peaks, reps)
+        torch.cuda.empty_cache()
+    return out
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--row", default=None, choices=sorted(ROWS))
+    ap.add_argument("--reps", type=int, default=5)
+    a = ap.parse_args()
+    pk = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(pk):
+        with open(pk) as f:
+            peaks = json.load(f)
+    else:  # the profiling guide's fallback figures
+        peaks = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "sm_max_mhz": 1965.0}
+    torch.cuda.set_device(0)
+    h = hd.Handle(0)
+    res = run(h, peaks, a.reps, a.row)
+    for k, v in res.items():
+        print(json.dumps({k: v}), flush=True)
+    h.close()
+
+
+if __name__ == "__main__":
+    main()

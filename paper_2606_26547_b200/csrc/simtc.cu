@@ -32,13 +32,12 @@ using namespace tcp;
 
 constexpr int BM = 128;
 constexpr int BN_MAX = 256;
-constexpr int STAGES = 4;
+constexpr int MAX_STAGES = 10;  // ring depth is a runtime value: as many stages as fit in shared memory
 constexpr int A_BYTES = BM * KB_BYTES;
-constexpr int B_BYTES = BN_MAX * KB_BYTES;
-constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
 constexpr int NTHREADS = 320;
 constexpr int TMEM_COLS = 512;
-constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 + 256;
+constexpr int SMEM_LIMIT = 227 * 1024;
+constexpr int SMEM_EXTRA = 1024 /*alignment slack*/ + 256 /*barriers*/;
 constexpr int CH = 16;  // packed words a thread keeps in flight per register chunk
 
 // dimension offset (within a k-block) of shared-memory K position kappa
@@ -61,6 +60,8 @@ struct SimParams {
   int nparts;   // 1, or 3 for the fp32 class operand
   int m_tiles, n_tiles;
   int num_kb;
+  int stages;       // ring depth
+  int stage_bytes;  // A_BYTES + nparts*kc*KB_BYTES
   Epilogue e;
 };
 
@@ -82,12 +83,14 @@ __global__ void __launch_bounds__(NTHREADS, 1)
 sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
   extern __shared__ uint8_t smem_raw[];
   const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  const int STAGES = p.stages;
+  const uint32_t STAGE_BYTES = (uint32_t)p.stage_bytes;
   const uint32_t bar0 = base + STAGES * STAGE_BYTES;
   auto full_bar = [&](int s) { return bar0 + 8u * s; };
-  auto empty_bar = [&](int s) { return bar0 + 8u * (STAGES + s); };
-  auto tfull_bar = [&](int s) { return bar0 + 8u * (2 * STAGES + s); };
-  auto tempty_bar = [&](int s) { return bar0 + 8u * (2 * STAGES + 2 + s); };
-  const uint32_t tmem_slot = bar0 + 8u * (2 * STAGES + 4);
+  auto empty_bar = [&](int s) { return bar0 + 8u * (MAX_STAGES + s); };
+  auto tfull_bar = [&](int s) { return bar0 + 8u * (2 * MAX_STAGES + s); };
+  auto tempty_bar = [&](int s) { return bar0 + 8u * (2 * MAX_STAGES + 2 + s); };
+  const uint32_t tmem_slot = bar0 + 8u * (2 * MAX_STAGES + 4);
   uint32_t* tmem_slot_ptr = reinterpret_cast<uint32_t*>(smem_raw + (tmem_slot - smem_u32(smem_raw)));
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -391,11 +394,12 @@ cudaError_t launch_one(const CUtensorMap& tmB, const SimParams& p, int grid, cud
   static bool attr_set = false;
   if (!attr_set) {
     cudaError_t e = cudaFuncSetAttribute(sim_tc_kernel<INT8, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         SMEM_BYTES);
+                                         SMEM_LIMIT);
     if (e != cudaSuccess) return e;
     attr_set = true;
   }
-  sim_tc_kernel<INT8, EPI><<<grid, NTHREADS, SMEM_BYTES, st>>>(tmB, p);
+  const int smem = p.stages * p.stage_bytes + SMEM_EXTRA;
+  sim_tc_kernel<INT8, EPI><<<grid, NTHREADS, smem, st>>>(tmB, p);
   return cudaGetLastError();
 }
 
@@ -463,6 +467,9 @@ cudaError_t launch_sim_tc(TcContext* tc, const uint32_t* Hbits, int64_t N, int64
   p.m_tiles = (int)((N + BM - 1) / BM);
   p.n_tiles = n_tiles;
   p.num_kb = num_kb;
+  p.stage_bytes = A_BYTES + nparts * kc * KB_BYTES;
+  p.stages = (SMEM_LIMIT - SMEM_EXTRA) / p.stage_bytes;
+  if (p.stages > MAX_STAGES) p.stages = MAX_STAGES;
   p.e = e;
   const int grid = p.m_tiles < sm_count ? p.m_tiles : sm_count;
   ++*nlaunch;
