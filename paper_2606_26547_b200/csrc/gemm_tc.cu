@@ -238,18 +238,20 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
       tc_fence_after();
       const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(acc * BN);
       const int nchunks = (n_valid + 31) >> 5;
-      for (int c = 0; c < nchunks; ++c) {
-        uint32_t v[32];
-        tmem_ld32(taddr + (uint32_t)(c * 32), v);
-        tmem_ld_wait();
-        const int valid = n_valid - c * 32;  // >= 1
-        if (EPI == EPI_SIGN) {
+      if (EPI == EPI_SIGN) {
+        // Two register buffers: the tcgen05.ld of chunk c+1 is in flight while chunk c is packed.
+        // Sign + pack: one funnel shift per accumulator moves its sign bit into the word (last
+        // column first, so column j lands in bit j); for floats x + (+0.0) first turns -0.0 into
+        // +0.0 (reading A1: sgn(-0.0) = +1) on the FMA pipe, leaving the ALU pipe one op per value.
+        uint32_t va[32], vb[32];
+        auto pack_store = [&](const uint32_t (&v)[32], int c) {
           uint32_t word = 0;
 #pragma unroll
-          for (int j = 0; j < 32; ++j) {
-            const bool neg = INT8 ? ((int)v[j] < 0) : (__uint_as_float(v[j]) < 0.0f);
-            word |= (neg ? 1u : 0u) << j;
+          for (int j = 31; j >= 0; --j) {
+            const uint32_t u = INT8 ? v[j] : __float_as_uint(__fadd_rn(__uint_as_float(v[j]), 0.0f));
+            word = __funnelshift_l(u, word, 1);
           }
+          const int valid = n_valid - c * 32;  // >= 1
           if (valid < 32) word &= (1u << valid) - 1u;
           if (row_ok) {
             p.e.bits[row * p.e.ldbits + (n0 >> 5) + c] = word;
@@ -260,7 +262,25 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
                 if (j < valid) out[j] = v[j];
             }
           }
-        } else if (EPI == EPI_SCORE) {
+        };
+        tmem_ld32(taddr, va);
+        for (int c = 0; c < nchunks; c += 2) {
+          tmem_ld_wait();
+          if (c + 1 < nchunks) tmem_ld32(taddr + (uint32_t)((c + 1) * 32), vb);
+          pack_store(va, c);
+          if (c + 1 < nchunks) {
+            tmem_ld_wait();
+            if (c + 2 < nchunks) tmem_ld32(taddr + (uint32_t)((c + 2) * 32), va);
+            pack_store(vb, c + 1);
+          }
+        }
+      }
+      for (int c = 0; EPI != EPI_SIGN && c < nchunks; ++c) {
+        uint32_t v[32];
+        tmem_ld32(taddr + (uint32_t)(c * 32), v);
+        tmem_ld_wait();
+        const int valid = n_valid - c * 32;  // >= 1
+        if (EPI == EPI_SCORE) {
           if (row_ok) {
 #pragma unroll
             for (int j = 0; j < 32; ++j) {

@@ -4,12 +4,19 @@
 //   dist[n,k] = popcount( (h[n] xor c[k]) restricted to bits d < D_eff )
 //
 // Mapping: one thread owns one query and keeps the distances to a group of KC classes in
-// registers, so no cross-lane reduction is needed.  A CTA of QT threads stages a [WC words][QT
+// registers (KC is a template parameter chosen from K, so no popcount is spent on classes that do
+// not exist), so no cross-lane reduction is needed.  A CTA of QT threads stages a [WC words][QT
 // queries] tile of query bits in shared memory (transposed, stride QT+1: conflict-free both ways)
 // and the matching [KC][WC] tile of class bits, which every thread then reads as a broadcast
-// (one 16-byte LDS feeds four XOR+POPC).  For K > KC the query tile is re-staged per class group
-// (it comes from L2; 32 popcounts are done per word staged).  The bound at K >= 3 is the POPC
-// pipe, not HBM (kernel table).
+// (one 16-byte LDS feeds four words).  For K > KC the query tile is re-staged per class group (it
+// comes from L2).
+//
+// Pipe balance (DESIGN.md kernel table): POPC issues on the XU pipe at 16 lanes/clk/SM, LOP3 on the
+// ALU pipe at 64 lanes/clk/SM, so a plain XOR+POPC loop is XU-bound at 8 clk per word per warp.  A
+// block of 8 words is therefore reduced Harley-Seal style: seven XORed words go through four
+// carry-save adders (8 LOP3) into a ones / twos / fours word and the eighth is counted directly:
+//   sum_{i<8} popc(x_i) = popc(ones) + 2 popc(twos) + 4 popc(fours) + popc(x_7)
+// = 16 LOP3 (32 ALU clk) + 4 POPC (32 XU clk) per 8 words: both pipes level at 4 clk per word.
 #include <limits.h>
 
 #include "common.cuh"
@@ -19,8 +26,15 @@ namespace {
 
 constexpr int QT = 128;  // queries per CTA == threads per CTA
 constexpr int WC = 32;   // words per staged chunk
-constexpr int KC = 32;   // classes per register group
+constexpr int KC_MAX = 32;
 
+// carry-save adder: (hi, lo) = a + b + c per bit
+__device__ __forceinline__ void csa(uint32_t& hi, uint32_t& lo, uint32_t a, uint32_t b, uint32_t c) {
+  lo = a ^ b ^ c;
+  hi = (a & b) | ((a ^ b) & c);
+}
+
+template <int KC>
 __global__ void __launch_bounds__(QT)
 hamming_kernel(const uint32_t* __restrict__ Hbits, int64_t N, int64_t ldh,
                const uint32_t* __restrict__ Cbits, int K, int W, int D_eff,
@@ -44,15 +58,17 @@ hamming_kernel(const uint32_t* __restrict__ Hbits, int64_t N, int64_t ldh,
         const int w0 = ch * WC;
         __syncthreads();  // previous chunk fully consumed
         // queries: each warp stages QT/4 rows, one coalesced 128-byte read per row
-        for (int r = warp; r < QT; r += QT / 32) {
-          const int64_t row = q0 + r;
+        {
           const int w = w0 + lane;
-          uint32_t v = 0;
-          if (row < N && w < W) {
-            v = __ldg(Hbits + row * ldh + w);
-            if (w == W - 1) v &= tail_mask;
+          const bool w_ok = w < W;
+          const uint32_t m = (w == W - 1) ? tail_mask : 0xffffffffu;
+#pragma unroll 8
+          for (int r = warp; r < QT; r += QT / 32) {
+            const int64_t row = q0 + r;
+            uint32_t v = 0;
+            if (row < N && w_ok) v = __ldg(Hbits + row * ldh + w) & m;
+            hq[lane][r] = v;
           }
-          hq[lane][r] = v;
         }
         // classes: KC rows of WC words
         for (int i = tid; i < KC * WC; i += QT) {
@@ -66,13 +82,21 @@ hamming_kernel(const uint32_t* __restrict__ Hbits, int64_t N, int64_t ldh,
           cs[k][wl] = v;
         }
         __syncthreads();
-#pragma unroll 2
-        for (int w = 0; w < WC; w += 4) {
-          const uint32_t h0 = hq[w][tid], h1 = hq[w + 1][tid], h2 = hq[w + 2][tid], h3 = hq[w + 3][tid];
+#pragma unroll 1
+        for (int w = 0; w < WC; w += 8) {
+          uint32_t h[8];
+#pragma unroll
+          for (int i = 0; i < 8; ++i) h[i] = hq[w + i][tid];
 #pragma unroll
           for (int k = 0; k < KC; ++k) {
-            const uint4 c = *reinterpret_cast<const uint4*>(&cs[k][w]);
-            acc[k] += (__popc(h0 ^ c.x) + __popc(h1 ^ c.y)) + (__popc(h2 ^ c.z) + __popc(h3 ^ c.w));
+            const uint4 ca = *reinterpret_cast<const uint4*>(&cs[k][w]);
+            const uint4 cb = *reinterpret_cast<const uint4*>(&cs[k][w + 4]);
+            uint32_t a1, s1, a2, s2, a3, ones, fours, twos;
+            csa(a1, s1, h[0] ^ ca.x, h[1] ^ ca.y, h[2] ^ ca.z);
+            csa(a2, s2, h[3] ^ ca.w, h[4] ^ cb.x, h[5] ^ cb.y);
+            csa(a3, ones, s1, s2, h[6] ^ cb.z);
+            csa(fours, twos, a1, a2, a3);
+            acc[k] += (__popc(ones) + __popc(h[7] ^ cb.w)) + 2 * __popc(twos) + 4 * __popc(fours);
           }
         }
       }
@@ -117,7 +141,21 @@ cudaError_t launch_hamming(const uint32_t* Hbits, int64_t N, int64_t ldh, const 
   int64_t tiles = (N + QT - 1) / QT;
   const int64_t cap = (int64_t)sm_count * 8;
   const int grid = (int)(tiles < cap ? tiles : cap);
-  hamming_kernel<<<grid, QT, 0, st>>>(Hbits, N, ldh, Cbits, K, W, D_eff, dist, lds, labels, best, second);
+#define HDC_HAM(KC_)                                                                                         \
+  hamming_kernel<KC_><<<grid, QT, 0, st>>>(Hbits, N, ldh, Cbits, K, W, D_eff, dist, lds, labels, best, second)
+  // smallest register group that covers K in one pass; K > 32 walks groups of 32
+  if (K <= 2) HDC_HAM(2);
+  else if (K <= 4) HDC_HAM(4);
+  else if (K <= 6) HDC_HAM(6);
+  else if (K <= 8) HDC_HAM(8);
+  else if (K <= 10) HDC_HAM(10);
+  else if (K <= 12) HDC_HAM(12);
+  else if (K <= 16) HDC_HAM(16);
+  else if (K <= 20) HDC_HAM(20);
+  else if (K <= 24) HDC_HAM(24);
+  else if (K <= 28) HDC_HAM(28);
+  else HDC_HAM(KC_MAX);
+#undef HDC_HAM
   ++*nlaunch;
   return cudaGetLastError();
 }
