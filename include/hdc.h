@@ -68,8 +68,11 @@ enum { HDC_OP_ENCODE_RP = 0, HDC_OP_ENCODE_LEVELID = 1, HDC_OP_SIMILARITY = 2, H
 /* knobs.flags */
 enum {
   HDC_FLAG_NONE = 0,
-  HDC_FLAG_SIMT = 1 /* force the CUDA-core (FFMA / popcount) kernels where a tensor-core kernel
-                       exists for the same operation (debugging, A/B measurement)              */
+  HDC_FLAG_SIMT = 1, /* force the CUDA-core (FFMA / popcount) kernels where a tensor-core kernel
+                        exists for the same operation (debugging, A/B measurement)              */
+  HDC_FLAG_TC_1CTA = 2, /* encode contraction: force the one-CTA-per-tile tcgen05 kernel        */
+  HDC_FLAG_TC_2CTA = 4  /* encode contraction: force the CTA-pair (cta_group::2) tcgen05 kernel;
+                           without either flag the library chooses by problem size              */
 };
 
 /* Approximation knobs (section 4.2).

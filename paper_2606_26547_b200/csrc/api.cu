@@ -102,6 +102,11 @@ struct EncodePlan {
   int Fp = 0;
 };
 
+// 1 / 2 when the knobs force the 1-CTA / CTA-pair contraction kernel, 0 = by problem size
+int tc_cta_group(const hdc_knobs_t* k) {
+  return (k->flags & HDC_FLAG_TC_1CTA) ? 1 : (k->flags & HDC_FLAG_TC_2CTA) ? 2 : 0;
+}
+
 bool use_tc(const hdc_ctx* h, const hdc_knobs_t* k) {
   return h->tc != nullptr && !(k->flags & HDC_FLAG_SIMT);
 }
@@ -162,7 +167,7 @@ int do_encode_rp(hdc_ctx* h, const void* X, int x_dtype, int64_t N, int F, int64
                    SPLIT_A_SEGS, SPLIT_B_SEGS, pl.Fp};
       {
         Timed tm(h, HDC_K_ENCODE_GEMM, st);
-        ce = launch_gemm_tc(h->tc, o, N, D_eff, e, h->sm_count, st, &h->launches);
+        ce = launch_gemm_tc(h->tc, o, N, D_eff, e, h->sm_count, tc_cta_group(k), st, &h->launches);
       }
       if (ce == cudaSuccess) return HDC_OK;
       if (ce != cudaErrorNotSupported) return cuda_fail(h, ce, "encode_rp fp32 tcgen05");
@@ -194,7 +199,7 @@ int do_encode_rp(hdc_ctx* h, const void* X, int x_dtype, int64_t N, int F, int64
       TcOperands o{pl.Xs, Pq, OPK_I8, pl.ldxs, ldpq, F, F, F, 1, 0u, 0u, 0};
       {
         Timed tm(h, HDC_K_ENCODE_GEMM, st);
-        ce = launch_gemm_tc(h->tc, o, N, D_eff, e, h->sm_count, st, &h->launches);
+        ce = launch_gemm_tc(h->tc, o, N, D_eff, e, h->sm_count, tc_cta_group(k), st, &h->launches);
       }
       if (ce == cudaSuccess) return HDC_OK;
       if (ce != cudaErrorNotSupported) return cuda_fail(h, ce, "encode_rp int8 tcgen05");
@@ -226,7 +231,7 @@ int do_encode_rp(hdc_ctx* h, const void* X, int x_dtype, int64_t N, int F, int64
     TcOperands o{Xb, Pb, OPK_BF16, ldxb, ldpb, F, F, F, 1, 0u, 0u, 0};
     {
       Timed tm(h, HDC_K_ENCODE_GEMM, st);
-      ce = launch_gemm_tc(h->tc, o, N, D_eff, e, h->sm_count, st, &h->launches);
+      ce = launch_gemm_tc(h->tc, o, N, D_eff, e, h->sm_count, tc_cta_group(k), st, &h->launches);
     }
     if (ce == cudaSuccess) return HDC_OK;
     if (ce != cudaErrorNotSupported) return cuda_fail(h, ce, "encode_rp bf16 tcgen05");

@@ -71,8 +71,9 @@ struct TcOperands {
   uint32_t a_segs, b_segs;
   int seg_stride;
 };
+// cta_group: 1 / 2 force the 1-CTA / CTA-pair kernel, anything else chooses by problem size
 cudaError_t launch_gemm_tc(TcContext* tc, const TcOperands& o, int64_t M, int Nc, const Epilogue& e,
-                           int sm_count, cudaStream_t st, int64_t* nlaunch);
+                           int sm_count, int cta_group, cudaStream_t st, int64_t* nlaunch);
 
 // similarity on the tensor cores from packed queries (simtc.cu).  cop: workspace of
 // sim_tc_operand_bytes() for the staged class operand; amax_scratch: one float (hv_bits 8).

@@ -5,10 +5,19 @@
 //
 // One persistent CTA per SM, 6 warps: warp 0 = TMA producer, warp 1 = MMA issuer (+ TMEM
 // allocation), warps 2-5 = epilogue (warp w reads TMEM lanes 32*(w%4).., thread = accumulator
-// row).  CTA tile 128 x 256, k-blocks of 128 bytes (64 bf16 / 128 int8), 4-stage mbarrier ring
-// between producer and issuer, two 256-column TMEM accumulators so that the epilogue of tile i
-// overlaps the MMAs of tile i+1.  Operands are K-contiguous ("K-major") for both A and B, which is
-// the layout of X[N][F], P[D][F] and C[K][D] (include/hdc.h).
+// row).  k-blocks of 128 bytes (64 bf16 / 128 int8), mbarrier ring between producer and issuer, two
+// 256-column TMEM accumulators so that the epilogue of tile i overlaps the MMAs of tile i+1.
+// Operands are K-contiguous ("K-major") for both A and B, which is the layout of X[N][F], P[D][F]
+// and C[K][D] (include/hdc.h).
+//
+// CG = 2 (default for large problems): the two CTAs of a cluster (one TPC) share a 256 x 256 tile
+// with tcgen05.mma.cta_group::2.  Each CTA loads its own 128 rows of A and HALF of the B tile, so a
+// k-block costs 32 KB of shared-memory fill per SM instead of 48 KB (the 1-CTA kernel is bound by
+// the L2 -> SM fill rate, profiles/r1_tcgen05_path.md) and the ring is 6 deep.  The even CTA issues
+// the MMAs for both; barriers: `full` lives in the leader and counts the TMA bytes of both CTAs,
+// `empty` and `tmem full` are signalled in both CTAs by a multicast tcgen05.commit, `tmem empty`
+// lives in the leader and collects the epilogue warps of both CTAs.
+// CG = 1: one CTA per 128 x 256 tile, 4-deep ring (small problems, HDC_FLAG_TC_1CTA).
 //
 // The reduction axis is a list of SEGMENTS: k-block kb reads A columns a_seg[kb / nkb_seg] *
 // seg_stride + (kb % nkb_seg) * BK and B columns b_seg[..] likewise.  One segment = a plain GEMM.
@@ -67,13 +76,18 @@ using namespace tcp;
 
 constexpr int BM = 128;            // rows of A per tile == TMEM lanes
 constexpr int BN = 256;            // rows of B per tile == TMEM columns of one accumulator
-constexpr int STAGES = 4;
 constexpr int A_BYTES = BM * KB_BYTES;   // 16 KB
-constexpr int B_BYTES = BN * KB_BYTES;   // 32 KB
-constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
 constexpr int NTHREADS = 192;
 constexpr int TMEM_COLS = 512;
-constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*alignment slack*/ + 256 /*barriers*/;
+constexpr int MAX_STAGES = 6;
+template <int CG>
+struct Cfg {
+  static constexpr int STAGES = CG == 2 ? 6 : 4;
+  static constexpr int B_ROWS = BN / CG;               // rows of B this CTA stages
+  static constexpr int B_BYTES = B_ROWS * KB_BYTES;    // 32 KB / 16 KB
+  static constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
+  static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*alignment slack*/ + 256 /*barriers*/;
+};
 
 struct TcParams {
   int64_t M;
@@ -96,16 +110,18 @@ constexpr double NEG_BIG = -1.0e300;
 // i-th tile of this CTA: EPI_ARGMAX owns whole m-tiles (n inner, so a thread sees every class of
 // its row); the others walk groups of group_m m-tiles, m fastest, so that CTAs running at the same
 // time share B tiles and reuse A tiles from L2.
-template <int EPI>
+// (CG = 2: the unit that walks the tiles is the cluster, and an m-tile is 256 rows.)
+template <int EPI, int CG>
 __device__ __forceinline__ bool tile_at(const TcParams& p, int64_t i, int& mt, int& nt) {
+  const int64_t unit = blockIdx.x / CG, nunits = gridDim.x / CG;
   if (EPI == EPI_ARGMAX) {
-    const int64_t u = blockIdx.x + (i / p.n_tiles) * (int64_t)gridDim.x;
+    const int64_t u = unit + (i / p.n_tiles) * nunits;
     if (u >= p.m_tiles) return false;
     mt = (int)u;
     nt = (int)(i % p.n_tiles);
     return true;
   }
-  const int64_t t = blockIdx.x + i * (int64_t)gridDim.x;
+  const int64_t t = unit + i * nunits;
   if (t >= (int64_t)p.m_tiles * p.n_tiles) return false;
   const int64_t gsz = (int64_t)p.group_m * p.n_tiles;
   const int64_t g = t / gsz;
@@ -117,22 +133,25 @@ __device__ __forceinline__ bool tile_at(const TcParams& p, int64_t i, int& mt, i
   return true;
 }
 
-template <bool INT8, int EPI>
+template <bool INT8, int EPI, int CG>
 __global__ void __launch_bounds__(NTHREADS, 1)
 gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
                const TcParams p) {
+  constexpr int STAGES = Cfg<CG>::STAGES;
+  constexpr int STAGE_BYTES = Cfg<CG>::STAGE_BYTES;
   extern __shared__ uint8_t smem_raw[];
   const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
-  // barriers live after the stage ring
+  // barriers live after the stage ring (same offsets in both CTAs of a pair)
   const uint32_t bar0 = base + STAGES * STAGE_BYTES;
   auto full_bar = [&](int s) { return bar0 + 8u * s; };
-  auto empty_bar = [&](int s) { return bar0 + 8u * (STAGES + s); };
-  auto tfull_bar = [&](int s) { return bar0 + 8u * (2 * STAGES + s); };
-  auto tempty_bar = [&](int s) { return bar0 + 8u * (2 * STAGES + 2 + s); };
-  const uint32_t tmem_slot = bar0 + 8u * (2 * STAGES + 4);
+  auto empty_bar = [&](int s) { return bar0 + 8u * (MAX_STAGES + s); };
+  auto tfull_bar = [&](int s) { return bar0 + 8u * (2 * MAX_STAGES + s); };
+  auto tempty_bar = [&](int s) { return bar0 + 8u * (2 * MAX_STAGES + 2 + s); };
+  const uint32_t tmem_slot = bar0 + 8u * (2 * MAX_STAGES + 4);
   uint32_t* tmem_slot_ptr = reinterpret_cast<uint32_t*>(smem_raw + (tmem_slot - smem_u32(smem_raw)));
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int rank = CG == 2 ? (int)cluster_ctarank() : 0;  // 0 = leader (issues the MMAs)
   constexpr int BK = INT8 ? 128 : 64;  // elements per k-block
   const int num_kb = p.nseg * p.nkb_seg;
 
@@ -145,15 +164,15 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     }
     for (int s = 0; s < 2; ++s) {
       mbar_init(tfull_bar(s), 1);
-      mbar_init(tempty_bar(s), 4);
+      mbar_init(tempty_bar(s), 4 * CG);
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == 1) {
-    tmem_alloc(tmem_slot, TMEM_COLS);
+    tmem_alloc<CG>(tmem_slot, TMEM_COLS);
   }
   tc_fence_before();
-  __syncthreads();
+  if (CG == 2) cluster_sync_all(); else __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot_ptr;
 
@@ -162,8 +181,15 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     int stage = 0;
     uint32_t phase = 0;
     int mt, nt;
-    for (int64_t i = 0; tile_at<EPI>(p, i, mt, nt); ++i) {
-      const int m0 = mt * BM, n0 = nt * BN;
+    for (int64_t i = 0; tile_at<EPI, CG>(p, i, mt, nt); ++i) {
+      const int n0 = nt * BN;
+      int nb = 0;
+      if (CG == 2) {  // this CTA stages rows [rank * N/2, +N/2) of the tile's N (rounded to 16) columns
+        int n_valid = p.Nc - n0;
+        if (n_valid > BN) n_valid = BN;
+        nb = rank * (((n_valid + 15) & ~15) >> 1);
+      }
+      const int m0 = (mt * CG + rank) * BM;
       for (int kb = 0; kb < num_kb; ++kb) {
         const int seg = kb / p.nkb_seg;
         const int j = kb - seg * p.nkb_seg;
@@ -172,9 +198,16 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
         mbar_wait(empty_bar(stage), phase ^ 1u);
         if (lane == 0) {
           const uint32_t sa = base + stage * STAGE_BYTES;
-          mbar_arrive_expect_tx(full_bar(stage), STAGE_BYTES);
-          tma_load_2d(sa, &tmA, full_bar(stage), acol, m0);
-          tma_load_2d(sa + A_BYTES, &tmB, full_bar(stage), bcol, n0);
+          if (CG == 2) {
+            // both CTAs' bytes complete on the leader's barrier; only the leader arms it
+            if (rank == 0) mbar_arrive_expect_tx(full_bar(stage), 2 * STAGE_BYTES);
+            tma_load_2d_2sm(sa, &tmA, full_bar(stage) & PEER_MASK, acol, m0);
+            tma_load_2d_2sm(sa + A_BYTES, &tmB, full_bar(stage) & PEER_MASK, bcol, n0 + nb);
+          } else {
+            mbar_arrive_expect_tx(full_bar(stage), STAGE_BYTES);
+            tma_load_2d(sa, &tmA, full_bar(stage), acol, m0);
+            tma_load_2d(sa + A_BYTES, &tmB, full_bar(stage), bcol, n0);
+          }
         }
         __syncwarp();
         if (++stage == STAGES) {
@@ -184,16 +217,16 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
       }
     }
   } else if (warp == 1) {
-    // ================================================================= MMA issuer
+    // ================================================================= MMA issuer (leader CTA)
     int stage = 0;
     uint32_t phase = 0;
     int acc = 0;
     uint32_t acc_phase = 0;
     int mt, nt;
-    for (int64_t i = 0; tile_at<EPI>(p, i, mt, nt); ++i) {
+    for (int64_t i = 0; rank == 0 && tile_at<EPI, CG>(p, i, mt, nt); ++i) {
       int n_valid = p.Nc - nt * BN;
       if (n_valid > BN) n_valid = BN;
-      const uint32_t idesc = instr_desc<INT8>(BM, (n_valid + 15) & ~15);
+      const uint32_t idesc = instr_desc<INT8>(BM * CG, (n_valid + 15) & ~15);
       mbar_wait(tempty_bar(acc), acc_phase ^ 1u);
       tc_fence_after();
       const uint32_t d_tmem = tmem_base + (uint32_t)(acc * BN);
@@ -205,9 +238,9 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
           const uint64_t da = smem_desc(sa), db = smem_desc(sa + A_BYTES);
 #pragma unroll
           for (int k = 0; k < KB_BYTES / 32; ++k)
-            tc_mma<INT8>(d_tmem, da + 2u * k, db + 2u * k, idesc, (kb | k) != 0 ? 1u : 0u);
-          tc_commit(empty_bar(stage));            // frees the smem slot when these MMAs retire
-          if (kb == num_kb - 1) tc_commit(tfull_bar(acc));  // accumulator complete
+            tc_mma<INT8, CG>(d_tmem, da + 2u * k, db + 2u * k, idesc, (kb | k) != 0 ? 1u : 0u);
+          tc_commit<CG>(empty_bar(stage));            // frees the smem slot when these MMAs retire
+          if (kb == num_kb - 1) tc_commit<CG>(tfull_bar(acc));  // accumulator complete
         }
         __syncwarp();
         if (++stage == STAGES) {
@@ -228,11 +261,11 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     uint32_t acc_phase = 0;
     Top2 run = Top2{NEG_BIG, INT_MAX, NEG_BIG};
     int mt, nt;
-    for (int64_t i = 0; tile_at<EPI>(p, i, mt, nt); ++i) {
+    for (int64_t i = 0; tile_at<EPI, CG>(p, i, mt, nt); ++i) {
       const int n0 = nt * BN;
       int n_valid = p.Nc - n0;
       if (n_valid > BN) n_valid = BN;
-      const int64_t row = (int64_t)mt * BM + q * 32 + lane;
+      const int64_t row = (int64_t)(mt * CG + rank) * BM + q * 32 + lane;
       const bool row_ok = row < p.M;
       mbar_wait(tfull_bar(acc), acc_phase);
       tc_fence_after();
@@ -317,7 +350,10 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
       // accumulator drained: hand it back to the MMA issuer
       tc_fence_before();
       __syncwarp();
-      if (lane == 0) mbar_arrive(tempty_bar(acc));
+      if (lane == 0) {
+        if (CG == 2) mbar_arrive_cluster(tempty_bar(acc) & PEER_MASK);  // the leader's barrier
+        else mbar_arrive(tempty_bar(acc));
+      }
       if (++acc == 2) {
         acc = 0;
         acc_phase ^= 1u;
@@ -341,31 +377,60 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
 
   // ------------------------------------------------------------------- teardown
   tc_fence_before();
-  __syncthreads();
+  if (CG == 2) cluster_sync_all(); else __syncthreads();
   if (warp == 1) {
     tc_fence_after();
-    tmem_dealloc(tmem_base, TMEM_COLS);
+    tmem_dealloc<CG>(tmem_base, TMEM_COLS);
   }
 }
 
-template <bool INT8, int EPI>
+template <bool INT8, int EPI, int CG>
 cudaError_t launch_one(const CUtensorMap& tmA, const CUtensorMap& tmB, const TcParams& p, int grid,
                        cudaStream_t st) {
   static bool attr_set = false;  // per instantiation; the attribute is sticky for the function
+  constexpr int SMEM_BYTES = Cfg<CG>::SMEM_BYTES;
   if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(gemm_tc_kernel<INT8, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         SMEM_BYTES);
+    cudaError_t e = cudaFuncSetAttribute(gemm_tc_kernel<INT8, EPI, CG>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
     if (e != cudaSuccess) return e;
     attr_set = true;
   }
-  gemm_tc_kernel<INT8, EPI><<<grid, NTHREADS, SMEM_BYTES, st>>>(tmA, tmB, p);
-  return cudaGetLastError();
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)grid);
+  cfg.blockDim = dim3(NTHREADS);
+  cfg.dynamicSmemBytes = SMEM_BYTES;
+  cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeClusterDimension;
+  at[0].val.clusterDim.x = CG;
+  at[0].val.clusterDim.y = 1;
+  at[0].val.clusterDim.z = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, gemm_tc_kernel<INT8, EPI, CG>, tmA, tmB, p);
+}
+
+template <int CG>
+cudaError_t launch_cg(bool int8, int kind, const CUtensorMap& tmA, const CUtensorMap& tmB, const TcParams& p,
+                      int grid, cudaStream_t st) {
+  if (int8) {
+    switch (kind) {
+      case EPI_SIGN: return launch_one<true, EPI_SIGN, CG>(tmA, tmB, p, grid, st);
+      case EPI_SCORE: return launch_one<true, EPI_SCORE, CG>(tmA, tmB, p, grid, st);
+      default: return launch_one<true, EPI_ARGMAX, CG>(tmA, tmB, p, grid, st);
+    }
+  }
+  switch (kind) {
+    case EPI_SIGN: return launch_one<false, EPI_SIGN, CG>(tmA, tmB, p, grid, st);
+    case EPI_SCORE: return launch_one<false, EPI_SCORE, CG>(tmA, tmB, p, grid, st);
+    default: return launch_one<false, EPI_ARGMAX, CG>(tmA, tmB, p, grid, st);
+  }
 }
 
 }  // namespace
 
 cudaError_t launch_gemm_tc(TcContext* tc, const TcOperands& o, int64_t M, int Nc, const Epilogue& e,
-                           int sm_count, cudaStream_t st, int64_t* nlaunch) {
+                           int sm_count, int cta_group, cudaStream_t st, int64_t* nlaunch) {
   if (!tc) return cudaErrorNotSupported;
   if (M <= 0 || Nc <= 0) return cudaSuccess;
   const bool int8 = o.elem_kind == OPK_I8;
@@ -376,37 +441,35 @@ cudaError_t launch_gemm_tc(TcContext* tc, const TcOperands& o, int64_t M, int Nc
       ((o.lda * es) & 15) || ((o.ldb * es) & 15) || o.nseg < 1 || o.nseg > 8 ||
       (o.nseg > 1 && (o.seg_stride % BK) != 0))
     return cudaErrorNotSupported;
-  if (M > (int64_t)INT_MAX - BM || o.cols_a > INT_MAX || o.cols_b > INT_MAX) return cudaErrorNotSupported;
+  if (M > (int64_t)INT_MAX - 2 * BM || o.cols_a > INT_MAX || o.cols_b > INT_MAX) return cudaErrorNotSupported;
+  const int n_tiles = (Nc + BN - 1) / BN;
+  const int64_t units1 = e.kind == EPI_ARGMAX ? (M + BM - 1) / BM : (M + BM - 1) / BM * n_tiles;
+  // CTA pairs once every SM has a tile of its own either way; small problems keep the 1-CTA kernel
+  // (twice as many independent tiles)
+  int cg = cta_group;
+  if (cg != 1 && cg != 2) cg = units1 >= 2 * (int64_t)sm_count ? 2 : 1;
+  if (sm_count < 2) cg = 1;
   TcParams p;
   p.M = M;
   p.Nc = Nc;
-  p.m_tiles = (int)((M + BM - 1) / BM);
-  p.n_tiles = (Nc + BN - 1) / BN;
+  p.m_tiles = (int)((M + BM * cg - 1) / (BM * cg));
+  p.n_tiles = n_tiles;
   p.nseg = o.nseg;
   p.nkb_seg = (o.Kr + BK - 1) / BK;
   p.a_segs = o.a_segs;
   p.b_segs = o.b_segs;
   p.seg_stride = o.seg_stride;
-  p.group_m = 16;
+  p.group_m = 16 / cg;
   p.e = e;
   CUtensorMap tmA, tmB;
   if (!tc_make_map(tc, &tmA, o.A, int8, M, o.cols_a, o.lda, BM)) return cudaErrorInvalidValue;
-  if (!tc_make_map(tc, &tmB, o.B, int8, Nc, o.cols_b, o.ldb, BN)) return cudaErrorInvalidValue;
+  if (!tc_make_map(tc, &tmB, o.B, int8, Nc, o.cols_b, o.ldb, BN / cg)) return cudaErrorInvalidValue;
   const int64_t units = e.kind == EPI_ARGMAX ? p.m_tiles : (int64_t)p.m_tiles * p.n_tiles;
-  const int grid = (int)(units < sm_count ? units : sm_count);
+  const int max_units = sm_count / cg;
+  const int grid = (int)(units < max_units ? units : max_units) * cg;
   ++*nlaunch;
-  if (int8) {
-    switch (e.kind) {
-      case EPI_SIGN: return launch_one<true, EPI_SIGN>(tmA, tmB, p, grid, st);
-      case EPI_SCORE: return launch_one<true, EPI_SCORE>(tmA, tmB, p, grid, st);
-      default: return launch_one<true, EPI_ARGMAX>(tmA, tmB, p, grid, st);
-    }
-  }
-  switch (e.kind) {
-    case EPI_SIGN: return launch_one<false, EPI_SIGN>(tmA, tmB, p, grid, st);
-    case EPI_SCORE: return launch_one<false, EPI_SCORE>(tmA, tmB, p, grid, st);
-    default: return launch_one<false, EPI_ARGMAX>(tmA, tmB, p, grid, st);
-  }
+  if (cg == 2) return launch_cg<2>(int8, e.kind, tmA, tmB, p, grid, st);
+  return launch_cg<1>(int8, e.kind, tmA, tmB, p, grid, st);
 }
 
 }  // namespace hdc

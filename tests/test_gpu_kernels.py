@@ -100,7 +100,7 @@ def _encode(hd, h, X, P, D_eff, prec, flags=0, bf16_inputs=False):
 
 
 @pytest.mark.parametrize("prec", ["F32", "BF16", "I8", "B1"])
-@pytest.mark.parametrize("flags", [0, 1])
+@pytest.mark.parametrize("flags", [0, 1, 2, 4])
 @pytest.mark.parametrize("N,F,D,D_eff", [(200, 64, 2048, 2048), (131, 617, 1000, 999), (300, 100, 700, 33),
                                          (3, 7, 40, 40), (520, 784, 520, 515)])
 def test_encode_rp_exact_arithmetic(hd, h, prec, flags, N, F, D, D_eff):
@@ -128,7 +128,7 @@ def test_encode_rp_exact_arithmetic(hd, h, prec, flags, N, F, D, D_eff):
 
 
 @pytest.mark.parametrize("prec", ["F32", "BF16", "I8"])
-@pytest.mark.parametrize("flags", [0, 1])
+@pytest.mark.parametrize("flags", [0, 1, 2, 4])
 def test_encode_rp_float_c2_shape(hd, h, prec, flags):
     """Gaussian features / projection at the C2 shape (F=617, D=10000 sliced): raw accumulators
     within 1e-3 relative of the float64 oracle; sign mismatches only inside the rounding band."""
