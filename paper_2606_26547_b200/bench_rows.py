@@ -137,9 +137,9 @@ def row_levelid(h, peaks, reps, N=65536, F=784, Q=256, D=10000):
     fn = lambda: h.hdc_encode_levelid(lv, ID, LV, D, kn, Hbits=H)  # noqa: E731
     call_ms = _time(fn, reps)
     k_ms, _ = _kernel(h, hd.HDC_K_LEVELID, fn, reps)
-    # algorithmic logic ops per sample: F*W binds + 30 LOP3 per 16 features per word for the CSA tree
-    # + ripple into the upper planes: ~ (1 + 30/16 + 14/16) * F * W
-    ops = (1.0 + 30.0 / 16.0 + 14.0 / 16.0) * F * Wd * N
+    # algorithmic logic ops per sample: one bind XOR plus one full
+    # adder (2 LOP3) per (feature, word) = 3*F*W; the kernel executes 3.69 (address + ripple extra)
+    ops = 3.0 * F * Wd * N
     ach = ops / (k_ms * 1e-3) / 1e12
     peak = 148 * 64 * peaks["sm_max_mhz"] * 1e6 / 1e12
     return {"what": f"hdc_encode_levelid N={N} F={F} Q={Q} D={D} (C3-shaped, ~80% zero pixels)", "call_ms": call_ms,

@@ -46,6 +46,7 @@ struct LevelIdParams {
   int64_t n_batches;
   int Fpad;     // staged level row stride (bytes), multiple of 16
   int tables_in_smem;
+  uint32_t mul_hi16;  // 65536 (passed at run time so that mad.hi is not strength-reduced to a shift)
 };
 
 // NP = number of counter planes (p + 1 with 2^p > F); S = samples per warp iteration
@@ -164,6 +165,214 @@ __global__ void __launch_bounds__(NTHREADS, 1) levelid_kernel(const LevelIdParam
   }
 }
 
+// ---------------------------------------------------------------------------------------------
+// Fast path (F % 4 == 0, F < 1024, tables + one batch fit in shared memory, 4-byte aligned level
+// rows): same mapping (CTA = 1024-bit slice, lane = word, warp = FS samples at a time) with the
+// instruction stream cut to what the counter needs:
+//   * levels are staged as 16-bit table byte-offsets (level << 7), two per word, read by the warp
+//     as broadcast 16-byte loads; the LV address is one LOP3 (low half) or one IMAD.HI (high half,
+//     FMA pipe) -- no 64-bit address arithmetic, no predication in the loop;
+//   * features go in blocks of 32: two 16-input CSA trees (30 LOP3 each) whose weight-16 carries
+//     meet in one more CSA, so the ripple into the upper planes runs once per 32 features;
+//   * the next batch's level bytes are prefetched into registers before the block loop, so the
+//     only exposed staging cost is the conversion between two barriers.
+// ALU ops per (feature, sample, word): 1 bind XOR + 0.5 address + 1.875 + 0.44 counter = 3.8.
+constexpr int FS = 4;                   // samples per warp
+constexpr int FWARPS = 12;              // warps per CTA (3 per scheduler; 166 registers x 384 threads fit)
+constexpr int FTHREADS = FWARPS * 32;
+constexpr int FSB = FWARPS * FS;        // samples per batch (48)
+constexpr int PF_ROW = 8;               // prefetched level words per lane per sample row (F <= 1024)
+constexpr int PF_MAX = FS * PF_ROW;
+
+template <int NP>
+__global__ void __launch_bounds__(FTHREADS, 1) levelid_fast_kernel(const LevelIdParams p) {
+  extern __shared__ __align__(16) uint8_t smem[];
+  uint32_t* sID = reinterpret_cast<uint32_t*>(smem);          // [F][SW]
+  uint32_t* sLV = sID + (size_t)p.F * SW;                      // [Q][SW]
+  uint32_t* sOff = sLV + (size_t)p.Q * SW;                     // [FSB][Fp2] packed 16-bit offsets
+  const int Fp2 = p.Fpad;                                      // words per staged row (multiple of 8)
+
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  constexpr int P = NP - 1;
+  const uint32_t init = (1u << P) - (uint32_t)(p.F / 2 + 1);
+  const uint32_t lane4 = (uint32_t)lane * 4u;
+  const uint32_t k65536 = p.mul_hi16;                           // 65536, opaque to the compiler
+  const int F4 = p.F >> 2;                                     // level words per sample row
+
+  const int64_t units = (int64_t)p.n_slices * p.n_batches;
+  const int64_t u_begin = units * blockIdx.x / gridDim.x;
+  const int64_t u_end = units * (blockIdx.x + 1) / gridDim.x;
+  int cur_slice = -1;
+
+  // Each warp stages the level rows of its own FS samples (lanes stride over the row's words), so
+  // a unit needs no block-wide barrier unless the slice -- and with it the tables -- changes.
+  uint32_t pf[PF_MAX];
+  auto prefetch = [&](int64_t u) {
+    const int64_t n0 = (u % p.n_batches) * FSB + warp * FS;
+#pragma unroll
+    for (int j = 0; j < FS; ++j) {
+      const int64_t n = n0 + j;
+      const uint32_t* row = reinterpret_cast<const uint32_t*>(p.levels + (n < p.N ? n : 0) * p.ldl);
+#pragma unroll
+      for (int i = 0; i < PF_ROW; ++i) {
+        const int g = lane + 32 * i;
+        pf[j * PF_ROW + i] = (g < F4 && n < p.N) ? __ldg(row + g) : 0u;
+      }
+    }
+  };
+  if (u_begin < u_end) prefetch(u_begin);
+
+  for (int64_t u = u_begin; u < u_end; ++u) {
+    const int slice = (int)(u / p.n_batches);
+    const int64_t batch = u - (int64_t)slice * p.n_batches;
+    const int w_glob = slice * SW + lane;
+    if (slice != cur_slice) {
+      __syncthreads();  // everyone is done with the previous slice's tables
+      for (int f = warp; f < p.F; f += FWARPS)
+        sID[f * SW + lane] = w_glob < p.W ? __ldg(p.ID + (int64_t)f * p.ldid + w_glob) : 0u;
+      for (int q = warp; q < p.Q; q += FWARPS)
+        sLV[q * SW + lane] = w_glob < p.W ? __ldg(p.LV + (int64_t)q * p.ldlv + w_glob) : 0u;
+      cur_slice = slice;
+      __syncthreads();
+    }
+    __syncwarp();  // this warp is done reading its rows of the previous unit
+    // four level bytes -> two words of 16-bit offsets (level * 128)
+#pragma unroll
+    for (int j = 0; j < FS; ++j) {
+#pragma unroll
+      for (int i = 0; i < PF_ROW; ++i) {
+        const int g = lane + 32 * i;
+        if (g < F4) {
+          const uint32_t v = pf[j * PF_ROW + i];
+          uint2 o;
+          o.x = ((v & 0xffu) << 7) | ((v & 0xff00u) << 15);
+          o.y = ((v >> 9) & 0x7f80u) | ((v >> 1) & 0x7f800000u);
+          *reinterpret_cast<uint2*>(sOff + (size_t)(warp * FS + j) * Fp2 + 2 * g) = o;
+        }
+      }
+    }
+    __syncwarp();
+    if (u + 1 < u_end) prefetch(u + 1);
+
+    uint32_t pl[FS][NP];
+#pragma unroll
+    for (int j = 0; j < FS; ++j)
+#pragma unroll
+      for (int i = 0; i < NP; ++i) pl[j][i] = ((init >> i) & 1u) ? 0xffffffffu : 0u;
+
+    const uint32_t* idp = sID + lane;
+    const char* lvb = reinterpret_cast<const char*>(sLV);
+    const uint32_t* myo = sOff + (size_t)(warp * FS) * Fp2;
+
+    // bound words of 16 features of sample j starting at feature f (f % 16 == 0)
+    auto bind16 = [&](int f, int j, const uint32_t (&idw)[16], uint32_t (&x)[16]) {
+      const uint4* op = reinterpret_cast<const uint4*>(myo + (size_t)j * Fp2 + (f >> 1));
+      const uint4 oa = op[0], ob = op[1];
+      const uint32_t o[8] = {oa.x, oa.y, oa.z, oa.w, ob.x, ob.y, ob.z, ob.w};
+#pragma unroll
+      for (int i = 0; i < 8; ++i) {
+        const uint32_t a_lo = (o[i] & 0xffffu) | lane4;
+        uint32_t a_hi;  // (o >> 16) + lane4 as a multiply-add: FMA pipe, leaves the ALU pipe to the LOP3s
+        asm("mad.hi.u32 %0, %1, %2, %3;" : "=r"(a_hi) : "r"(o[i]), "r"(k65536), "r"(lane4));
+        x[2 * i] = idw[2 * i] ^ *reinterpret_cast<const uint32_t*>(lvb + a_lo);
+        x[2 * i + 1] = idw[2 * i + 1] ^ *reinterpret_cast<const uint32_t*>(lvb + a_hi);
+      }
+    };
+    // 16 inputs into planes 0..3; returns the weight-16 carry
+    auto tree16 = [&](uint32_t (&q)[NP], const uint32_t (&x)[16]) -> uint32_t {
+      uint32_t tA, tB, fA, fB, eA, eB, sx;
+      HDC_CSA(tA, q[0], q[0], x[0], x[1]);
+      HDC_CSA(tB, q[0], q[0], x[2], x[3]);
+      HDC_CSA(fA, q[1], q[1], tA, tB);
+      HDC_CSA(tA, q[0], q[0], x[4], x[5]);
+      HDC_CSA(tB, q[0], q[0], x[6], x[7]);
+      HDC_CSA(fB, q[1], q[1], tA, tB);
+      HDC_CSA(eA, q[2], q[2], fA, fB);
+      HDC_CSA(tA, q[0], q[0], x[8], x[9]);
+      HDC_CSA(tB, q[0], q[0], x[10], x[11]);
+      HDC_CSA(fA, q[1], q[1], tA, tB);
+      HDC_CSA(tA, q[0], q[0], x[12], x[13]);
+      HDC_CSA(tB, q[0], q[0], x[14], x[15]);
+      HDC_CSA(fB, q[1], q[1], tA, tB);
+      HDC_CSA(eB, q[2], q[2], fA, fB);
+      HDC_CSA(sx, q[3], q[3], eA, eB);
+      return sx;
+    };
+    auto ripple = [&](uint32_t (&q)[NP], uint32_t c, int from) {
+#pragma unroll
+      for (int i = 0; i < NP; ++i) {
+        if (i >= from) {
+          const uint32_t t = q[i] & c;
+          q[i] ^= c;
+          c = t;
+        }
+      }
+    };
+
+    int f = 0;
+#pragma unroll 1
+    for (; f + 32 <= p.F; f += 32) {
+      uint32_t sxa[FS];
+      {
+        uint32_t idw[16];
+#pragma unroll
+        for (int i = 0; i < 16; ++i) idw[i] = idp[(f + i) * SW];
+#pragma unroll
+        for (int j = 0; j < FS; ++j) {
+          uint32_t x[16];
+          bind16(f, j, idw, x);
+          sxa[j] = tree16(pl[j], x);
+        }
+      }
+      {
+        uint32_t idw[16];
+#pragma unroll
+        for (int i = 0; i < 16; ++i) idw[i] = idp[(f + 16 + i) * SW];
+#pragma unroll
+        for (int j = 0; j < FS; ++j) {
+          uint32_t x[16];
+          bind16(f + 16, j, idw, x);
+          const uint32_t sxb = tree16(pl[j], x);
+          uint32_t c32;
+          HDC_CSA(c32, pl[j][4], pl[j][4], sxa[j], sxb);
+          ripple(pl[j], c32, 5);
+        }
+      }
+    }
+    if (f + 16 <= p.F) {
+      uint32_t idw[16];
+#pragma unroll
+      for (int i = 0; i < 16; ++i) idw[i] = idp[(f + i) * SW];
+#pragma unroll
+      for (int j = 0; j < FS; ++j) {
+        uint32_t x[16];
+        bind16(f, j, idw, x);
+        ripple(pl[j], tree16(pl[j], x), 4);
+      }
+      f += 16;
+    }
+    for (; f < p.F; ++f) {  // remainder features: plain ripple add
+      const uint32_t idw = idp[f * SW];
+#pragma unroll
+      for (int j = 0; j < FS; ++j) {
+        const uint32_t o = myo[(size_t)j * Fp2 + (f >> 1)];
+        const uint32_t a = (((f & 1) ? (o >> 16) : o) & 0xffffu) | lane4;
+        ripple(pl[j], idw ^ *reinterpret_cast<const uint32_t*>(lvb + a), 0);
+      }
+    }
+
+    if (w_glob < p.W) {
+      const uint32_t mask = (w_glob == p.W - 1 && (p.D_eff & 31)) ? ((1u << (p.D_eff & 31)) - 1u) : 0xffffffffu;
+      const int64_t n0 = batch * FSB;
+#pragma unroll
+      for (int j = 0; j < FS; ++j) {
+        const int64_t n = n0 + warp * FS + j;
+        if (n < p.N) p.Hbits[n * p.ldh + w_glob] = pl[j][P] & mask;
+      }
+    }
+  }
+}
+
 template <int NP, int S>
 cudaError_t launch_t(const LevelIdParams& p, int grid, size_t smem, cudaStream_t st) {
   cudaError_t e = cudaFuncSetAttribute(levelid_kernel<NP, S>, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -181,6 +390,31 @@ cudaError_t launch_levelid(const uint8_t* levels, int64_t N, int F, int64_t ldl,
                            int64_t* nlaunch) {
   if (N <= 0) return cudaSuccess;
   constexpr int S = 4;
+  {  // fast path
+    const size_t fp2 = (size_t)round_up((F + 1) / 2, 8);
+    const size_t smem_fast = ((size_t)F + Q) * SW * 4 + (size_t)FSB * fp2 * 4;
+    if (F % 4 == 0 && F < 1024 && (ldl & 3) == 0 && (reinterpret_cast<uintptr_t>(levels) & 3) == 0 &&
+        smem_fast <= (size_t)smem_optin) {
+      LevelIdParams p;
+      p.levels = levels; p.N = N; p.F = F; p.ldl = ldl;
+      p.ID = ID; p.ldid = ldid; p.LV = LV; p.Q = Q; p.ldlv = ldlv;
+      p.D_eff = D_eff; p.W = words_of(D_eff);
+      p.Hbits = Hbits; p.ldh = ldh;
+      p.n_slices = (p.W + SW - 1) / SW;
+      p.n_batches = (N + FSB - 1) / FSB;
+      p.Fpad = (int)fp2;
+      p.tables_in_smem = 1;
+      p.mul_hi16 = 65536u;
+      const int64_t units = (int64_t)p.n_slices * p.n_batches;
+      const int grid = (int)(units < sm_count ? units : sm_count);
+      cudaError_t e = cudaFuncSetAttribute(levelid_fast_kernel<11>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                           (int)smem_fast);
+      if (e != cudaSuccess) return e;
+      ++*nlaunch;
+      levelid_fast_kernel<11><<<grid, FTHREADS, smem_fast, st>>>(p);
+      return cudaGetLastError();
+    }
+  }
   LevelIdParams p;
   p.levels = levels; p.N = N; p.F = F; p.ldl = ldl;
   p.ID = ID; p.ldid = ldid; p.LV = LV; p.Q = Q; p.ldlv = ldlv;
