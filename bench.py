@@ -30,6 +30,8 @@ if ROOT not in sys.path:
 METRIC = "hdc_inference_queries_per_sec_D10000"
 UNIT = "queries/s"
 NQ = 131072            # queries per step (test set tiled)
+NCU_TRAFFIC_BYTES = 1084.9e6
+NCU_TRAFFIC_SOURCE = "profiles/r1_tcgen05_path.md (gemm_tc_kernel, fp32-precision encode, 131072 x 617 x 10000)"
 SM_COUNT = 148
 FP32_LANES = 128       # FFMA lanes per SM per clock
 
@@ -78,7 +80,7 @@ class ClockSampler:
                         self.reasons.add(nm)
             except Exception:
                 pass
-            self._stop.wait(0.02)
+            self._stop.wait(0.004)
 
     def __enter__(self):
         if self.ok:
@@ -98,10 +100,16 @@ class ClockSampler:
                 "reasons": sorted(self.reasons), "samples": len(self.samples)}
 
 
-def c2_workload():
+def c2_workload(world: int = 1, rank: int = 0):
+    """C2 model inputs + this rank's shard of the query stream: the test set tiled to world*NQ rows,
+    split by shard.shard_bounds (contiguous blocks, NQ rows per rank: weak scaling)."""
     from workloads import gen
+    from paper_2606_26547_b200 import shard
     w = gen.c2_isolet_shaped()
-    Xq = gen.tile_rows(w["Xte"], NQ)
+    lo, hi = shard.shard_bounds(world * NQ, world, rank)
+    n_te = w["Xte"].shape[0]
+    idx = np.arange(lo, hi) % n_te
+    Xq = np.ascontiguousarray(w["Xte"][idx])
     return w, Xq
 
 
@@ -155,6 +163,7 @@ def run_gpu(args):
     import torch.distributed as dist
 
     import paper_2606_26547_b200 as hd
+    from paper_2606_26547_b200 import shard
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -168,7 +177,7 @@ def run_gpu(args):
     h = hd.Handle(local)
     dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()  # noqa: E731
 
-    w, Xq = c2_workload()
+    w, Xq = c2_workload(world, rank)
     D, K, F = w["D"], w["K"], w["F"]
     Pd = dev(w["P"])
     kn_e = hd.knobs(D, precision=hd.HDC_F32)
@@ -214,13 +223,12 @@ def run_gpu(args):
         torch.cuda.synchronize()
     launches = h.launch_count() - l0
     ms = ev[0].elapsed_time(ev[1])
-    tmax = torch.tensor([ms], dtype=torch.float64, device="cuda")
     if world > 1:
         dist.barrier()
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-    ms = float(tmax.item())
+    ms = shard.max_over_ranks(ms, torch.device("cuda", local))
     value = world * NQ * args.steps / (ms * 1e-3)
-    acc = float((labels[: w["Xte"].shape[0]].cpu().numpy() == w["yte"]).mean())
+    n_te = w["Xte"].shape[0]
+    acc = float((labels[:n_te].cpu().numpy() == w["yte"][np.arange(rank * NQ, rank * NQ + n_te) % n_te]).mean())
 
     # ---- dominant kernel: the encode contraction.  Its launches are bracketed by CUDA events
     # inside the library (hdc_kernel_timing) on the stream they are launched on; measured (a) over a
@@ -251,8 +259,8 @@ def run_gpu(args):
     peak = peaks["bf16_tflops_sustained"] / 6.0
     clocks = cs.summary()
     roofline = {"bound": "tensor",
-                "kernel": "gemm_tc_kernel<bf16,EPI_SIGN> (tcgen05 fp32-precision encode: 6 bf16 segment "
-                          "products per MAC over 3-way split operands, sign+pack epilogue)",
+                "kernel": "gemm_tc_kernel<bf16,EPI_SIGN,cta_group::2> (tcgen05 fp32-precision encode on CTA pairs: 6 "
+                          "bf16 segment products per MAC over 3-way split operands, sign+pack epilogue)",
                 "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
                 "peak_source": f"bf16_tflops_sustained / 6 ({peaks['_source']} MEASURED_PEAKS.json; kernel timed "
                                "inside the step loop)",
@@ -265,7 +273,10 @@ def run_gpu(args):
                 "encode_call_ms": enc_call_ms, "classify_kernel_ms": cls_ms,
                 "share_of_step": enc_ms / (ms / args.steps),
                 "fp32_alu_peak_tflops": SM_COUNT * FP32_LANES * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12,
-                "traffic": None}
+                # dram__bytes_read.sum + dram__bytes_write.sum of this kernel at this shape, one launch, from
+                # the ncu --set full capture summarised in profiles/ (bytes)
+                "traffic": NCU_TRAFFIC_BYTES, "traffic_source": NCU_TRAFFIC_SOURCE,
+                "algorithmic_bytes_per_launch": float(NQ) * 3 * 640 * 2 + float(D) * 3 * 640 * 2 + float(NQ) * W * 4}
 
     # ---- end to end through the host entry point (pinned host buffers, H2D + D2H inside)
     e2e = None
@@ -280,10 +291,7 @@ def run_gpu(args):
         for _ in range(args.steps):
             h.hdc_infer_rp_host(Xh, Pd, C, kn, labels_host=Lh)      # synchronises before returning
         dt = time.perf_counter() - t0
-        tt = torch.tensor([dt], dtype=torch.float64, device="cuda")
-        if world > 1:
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        dt = float(tt.item())
+        dt = shard.max_over_ranks(dt, torch.device("cuda", local))
         assert np.array_equal(Lh.numpy(), labels.cpu().numpy()), "e2e labels differ from the device path"
         e2e = {"value": world * NQ * args.steps / dt, "unit": UNIT, "h2d_bytes_per_step": int(Xh.numel() * 4),
                "d2h_bytes_per_step": int(NQ * 4), "api": "hdc_infer_rp_host"}
@@ -329,7 +337,7 @@ def cpu_baseline(w, Xq):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="own", choices=["own", "reference"])
     ap.add_argument("--rows", action="store_true", help="also measure the other hot-path rows")
