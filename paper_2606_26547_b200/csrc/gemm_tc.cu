@@ -196,17 +196,17 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
         const int acol = (int)((p.a_segs >> (4 * seg)) & 15u) * p.seg_stride + j * BK;
         const int bcol = (int)((p.b_segs >> (4 * seg)) & 15u) * p.seg_stride + j * BK;
         mbar_wait(empty_bar(stage), phase ^ 1u);
-        if (lane == 0) {
+        {
           const uint32_t sa = base + stage * STAGE_BYTES;
           if (CG == 2) {
             // both CTAs' bytes complete on the leader's barrier; only the leader arms it
-            if (rank == 0) mbar_arrive_expect_tx(full_bar(stage), 2 * STAGE_BYTES);
-            tma_load_2d_2sm(sa, &tmA, full_bar(stage) & PEER_MASK, acol, m0);
-            tma_load_2d_2sm(sa + A_BYTES, &tmB, full_bar(stage) & PEER_MASK, bcol, n0 + nb);
+            if (rank == 0) mbar_arrive_expect_tx_elect(full_bar(stage), 2 * STAGE_BYTES);
+            tma_load_2d_2sm_elect(sa, &tmA, full_bar(stage) & PEER_MASK, acol, m0);
+            tma_load_2d_2sm_elect(sa + A_BYTES, &tmB, full_bar(stage) & PEER_MASK, bcol, n0 + nb);
           } else {
-            mbar_arrive_expect_tx(full_bar(stage), STAGE_BYTES);
-            tma_load_2d(sa, &tmA, full_bar(stage), acol, m0);
-            tma_load_2d(sa + A_BYTES, &tmB, full_bar(stage), bcol, n0);
+            mbar_arrive_expect_tx_elect(full_bar(stage), STAGE_BYTES);
+            tma_load_2d_elect(sa, &tmA, full_bar(stage), acol, m0);
+            tma_load_2d_elect(sa + A_BYTES, &tmB, full_bar(stage), bcol, n0);
           }
         }
         __syncwarp();
@@ -233,14 +233,14 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
       for (int kb = 0; kb < num_kb; ++kb) {
         mbar_wait(full_bar(stage), phase);
         tc_fence_after();
-        if (lane == 0) {
+        {  // whole warp, converged: each call issues once (tc_ptx.cuh, *_elect)
           const uint32_t sa = base + stage * STAGE_BYTES;
           const uint64_t da = smem_desc(sa), db = smem_desc(sa + A_BYTES);
 #pragma unroll
           for (int k = 0; k < KB_BYTES / 32; ++k)
-            tc_mma<INT8, CG>(d_tmem, da + 2u * k, db + 2u * k, idesc, (kb | k) != 0 ? 1u : 0u);
-          tc_commit<CG>(empty_bar(stage));            // frees the smem slot when these MMAs retire
-          if (kb == num_kb - 1) tc_commit<CG>(tfull_bar(acc));  // accumulator complete
+            tc_mma_elect<INT8, CG>(d_tmem, da + 2u * k, db + 2u * k, idesc, (kb | k) != 0 ? 1u : 0u);
+          tc_commit_elect<CG>(empty_bar(stage));            // frees the smem slot when these MMAs retire
+          if (kb == num_kb - 1) tc_commit_elect<CG>(tfull_bar(acc));  // accumulator complete
         }
         __syncwarp();
         if (++stage == STAGES) {

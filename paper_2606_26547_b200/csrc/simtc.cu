@@ -5,9 +5,9 @@
 //
 // The +-1 query operand never exists in HBM: four "expander" warps turn the packed words of a
 // 128-query tile into the K-major, 128-byte-swizzled shared-memory tile that tcgen05.mma reads (the
-// layout TMA would have written), while the class operand arrives by TMA.  Roles (10 warps, one
+// layout TMA would have written), while the class operand arrives by TMA.  Roles (14 warps, one
 // persistent CTA per SM): warp 0 = TMA producer (class tiles), warp 1 = MMA issuer + TMEM
-// allocation, warps 2-5 = epilogue (thread = query row), warps 6-9 = expanders (thread = query row).
+// allocation, warps 2-5 = epilogue (thread = query row), warps 6-13 = expanders (thread = query row x half of a k-block).
 //
 // Reduction-axis permutation.  A sum over d is invariant under any permutation of d applied to both
 // operands, so the k-block position kappa <-> dimension map is chosen to make the expansion two or
@@ -34,11 +34,16 @@ constexpr int BM = 128;
 constexpr int BN_MAX = 256;
 constexpr int MAX_STAGES = 10;  // ring depth is a runtime value: as many stages as fit in shared memory
 constexpr int A_BYTES = BM * KB_BYTES;
-constexpr int NTHREADS = 320;
+constexpr int EXW = 8;                 // expander warps: two per 128-row tile half (4 of a k-block's 8 chunks each)
+constexpr int NTHREADS = 192 + 32 * EXW;
 constexpr int TMEM_COLS = 512;
 constexpr int SMEM_LIMIT = 227 * 1024;
 constexpr int SMEM_EXTRA = 1024 /*alignment slack*/ + 256 /*barriers*/;
-constexpr int CH = 16;  // packed words a thread keeps in flight per register chunk
+constexpr int QW = 32;                       // packed words per row in one tile of the query ring
+constexpr int Q_LD = BM + 1;                 // words between consecutive word-rows of a ring tile
+constexpr int Q_SLOT_WORDS = QW * Q_LD;
+constexpr int Q_SLOTS = 3;
+constexpr int QRING_BYTES = Q_SLOTS * Q_SLOT_WORDS * 4;
 
 // dimension offset (within a k-block) of shared-memory K position kappa
 __host__ __device__ __forceinline__ int perm_bf16(int kappa) {  // k-block = 64 dims = 2 words
@@ -100,7 +105,7 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
   if (warp == 0 && lane == 0) {
     asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&tmB)) : "memory");
     for (int s = 0; s < STAGES; ++s) {
-      mbar_init(full_bar(s), 5);  // producer (with the TMA byte count) + one arrival per expander warp
+      mbar_init(full_bar(s), 1 + EXW);  // producer (with the TMA byte count) + one arrival per expander warp
       mbar_init(empty_bar(s), 1);
     }
     for (int s = 0; s < 2; ++s) {
@@ -126,11 +131,8 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
       const int nt = (int)(i % p.n_tiles);
       for (int kb = 0; kb < p.num_kb; ++kb) {
         mbar_wait(empty_bar(stage), phase ^ 1u);
-        if (lane == 0) {
-          mbar_arrive_expect_tx(full_bar(stage), (uint32_t)nb_rows * KB_BYTES);
-          tma_load_2d(base + stage * STAGE_BYTES + A_BYTES, &tmB, full_bar(stage), kb * BK, nt * nb_rows);
-        }
-        __syncwarp();
+        mbar_arrive_expect_tx_elect(full_bar(stage), (uint32_t)nb_rows * KB_BYTES);
+        tma_load_2d_elect(base + stage * STAGE_BYTES + A_BYTES, &tmB, full_bar(stage), kb * BK, nt * nb_rows);
         if (++stage == STAGES) {
           stage = 0;
           phase ^= 1u;
@@ -151,16 +153,15 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
       for (int kb = 0; kb < p.num_kb; ++kb) {
         mbar_wait(full_bar(stage), phase);
         tc_fence_after();
-        if (lane == 0) {
+        {  // whole warp, converged: each call issues once (tc_ptx.cuh, *_elect)
           const uint32_t sa = base + stage * STAGE_BYTES;
           const uint64_t da = smem_desc(sa), db = smem_desc(sa + A_BYTES);
 #pragma unroll
           for (int k = 0; k < KB_BYTES / 32; ++k)
-            tc_mma<INT8>(d_tmem, da + 2u * k, db + 2u * k, idesc, (kb | k) != 0 ? 1u : 0u);
-          tc_commit(empty_bar(stage));
-          if (kb == p.num_kb - 1) tc_commit(tfull_bar(acc));
+            tc_mma_elect<INT8>(d_tmem, da + 2u * k, db + 2u * k, idesc, (kb | k) != 0 ? 1u : 0u);
+          tc_commit_elect(empty_bar(stage));
+          if (kb == p.num_kb - 1) tc_commit_elect(tfull_bar(acc));
         }
-        __syncwarp();
         if (++stage == STAGES) {
           stage = 0;
           phase ^= 1u;
@@ -255,75 +256,131 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
       }
     }
   } else {
-    // ================================================================= expanders (warps 6..9)
-    const int t = (int)threadIdx.x - 192;  // row of the tile
-    constexpr int WPK = INT8 ? 4 : 2;      // packed words per k-block
-    constexpr int KPC = CH / WPK;          // k-blocks per register chunk
+    // ================================================================= expanders (warps 6..13)
+    // Query words reach the expanders through a 3-deep cp.async ring of [32 words][128 rows] tiles
+    // (transposed, row stride 129 words: conflict-free both ways): every copy instruction of a
+    // warp reads 128 contiguous bytes of one row whatever ldh is, and nothing is staged in registers.
+    const int et = (int)threadIdx.x - 192;    // 0..255
+    const int t = et & (BM - 1);              // row of the tile
+    const int part_id = et / BM;              // which half of a row's eight 16-byte chunks (warp-uniform)
+    const int ew = et >> 5;                   // expander warp 0..7
+    constexpr int C_PER = 8 / (EXW / 4);
+    static_assert(EXW == 8, "two expander threads per row");
+    constexpr int WPK = INT8 ? 4 : 2;         // packed words per k-block
+    constexpr int KPC = QW / WPK;             // k-blocks per ring tile
+    constexpr int WPP = WPK / 2;              // words of a k-block this thread's half needs
+    const int FB = STAGES >= 8 ? 4 : (STAGES >= 4 ? 2 : 1);  // k-blocks published per proxy fence (<= half the ring)
     const uint32_t sw = (uint32_t)(t & 7);
-    const bool vec_ok = ((p.ldh & 3) == 0) && ((reinterpret_cast<uintptr_t>(p.Hbits) & 15) == 0);
+    const uint32_t q_smem = bar0 + 256u;      // ring base (after the barriers)
+    const uint32_t* q_ptr = reinterpret_cast<const uint32_t*>(smem_raw + (q_smem - smem_u32(smem_raw)));
+    const int nch = (p.num_kb + KPC - 1) / KPC;
+    const int64_t steps = tiles_per_cta * nch;
+
+    int64_t is_i = 0;   // producer cursor: tile, chunk, ring slot
+    int is_c = 0, is_slot = 0;
+    auto issue = [&]() {
+      const int mt = (int)blockIdx.x + (int)(is_i / p.n_tiles) * (int)gridDim.x;
+      const int64_t m0 = (int64_t)mt * BM;
+      const int w = is_c * QW + lane;
+      const int64_t rows_left = p.N - m0;
+      const int nrow = w < p.W ? (rows_left < BM ? (int)rows_left : BM) : 0;
+      const uint32_t* src = p.Hbits + (m0 + ew) * p.ldh + w;
+      uint32_t dst = q_smem + (uint32_t)(is_slot * Q_SLOT_WORDS + lane * Q_LD + ew) * 4u;
+#pragma unroll 4
+      for (int rr = ew; rr < BM; rr += EXW) {
+        const bool ok = rr < nrow;
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 4, %2;" ::"r"(dst), "l"(ok ? src : p.Hbits),
+                     "r"(ok ? 4 : 0)
+                     : "memory");
+        src += EXW * p.ldh;
+        dst += EXW * 4u;
+      }
+      if (++is_slot == Q_SLOTS) is_slot = 0;
+      if (++is_c == nch) {
+        is_c = 0;
+        ++is_i;
+      }
+    };
+    for (int s0 = 0; s0 < Q_SLOTS - 1; ++s0) {
+      if (s0 < steps) issue();
+      asm volatile("cp.async.commit_group;" ::: "memory");
+    }
+
     int stage = 0;
     uint32_t phase = 0;
+    int slot = 0;
+    int64_t step = 0;
     for (int64_t i = 0; i < tiles_per_cta; ++i) {
-      const int mt = (int)blockIdx.x + (int)(i / p.n_tiles) * (int)gridDim.x;
-      const int64_t row = (int64_t)mt * BM + t;
-      const bool row_ok = row < p.N;
-      const uint32_t* hrow = p.Hbits + (row_ok ? row : 0) * p.ldh;
-      uint32_t cur[CH], nxt[CH];
-      auto load_chunk = [&](uint32_t (&dst)[CH], int w0) {
-        if (row_ok && vec_ok && w0 + CH <= p.W) {
-#pragma unroll
-          for (int u = 0; u < CH / 4; ++u) {
-            const uint4 x = __ldg(reinterpret_cast<const uint4*>(hrow + w0) + u);
-            dst[4 * u] = x.x;
-            dst[4 * u + 1] = x.y;
-            dst[4 * u + 2] = x.z;
-            dst[4 * u + 3] = x.w;
-          }
-        } else {
-#pragma unroll
-          for (int u = 0; u < CH; ++u) dst[u] = (row_ok && w0 + u < p.W) ? __ldg(hrow + w0 + u) : 0u;
-        }
-      };
-      load_chunk(nxt, 0);
-      for (int kb0 = 0; kb0 < p.num_kb; kb0 += KPC) {
-#pragma unroll
-        for (int u = 0; u < CH; ++u) cur[u] = nxt[u];
-        if (kb0 + KPC < p.num_kb) load_chunk(nxt, (kb0 + KPC) * WPK);
+      int first_stage = stage, pending = 0;
+      for (int c = 0; c < nch; ++c, ++step) {
+        asm volatile("cp.async.wait_group %0;" ::"n"(Q_SLOTS - 2) : "memory");
+        asm volatile("bar.sync 1, %0;" ::"n"(32 * EXW) : "memory");  // tile visible; previous slot free
+        if (step + Q_SLOTS - 1 < steps) issue();
+        asm volatile("cp.async.commit_group;" ::: "memory");
+        const uint32_t* qs = q_ptr + slot * Q_SLOT_WORDS + t;
+        const int kb0 = c * KPC;
 #pragma unroll
         for (int j = 0; j < KPC; ++j) {
           if (kb0 + j < p.num_kb) {
             mbar_wait(empty_bar(stage), phase ^ 1u);
             const uint32_t a_row = base + stage * STAGE_BYTES + (uint32_t)t * KB_BYTES;
+            // the chunk range is a compile-time constant per branch
+            auto expand = [&](auto part) {
+              constexpr int PART = decltype(part)::value;
+              constexpr int C0 = PART * C_PER;
+              uint32_t wq[WPP];
 #pragma unroll
-            for (int c = 0; c < 8; ++c) {  // 16-byte chunk c of the row = 4 shared-memory words
-              uint32_t o[4];
+              for (int u = 0; u < WPP; ++u) wq[u] = qs[(j * WPK + PART * WPP + u) * Q_LD];
 #pragma unroll
-              for (int e = 0; e < 4; ++e) {
-                const int iw = 4 * c + e;  // word index within the k-block's 32 output words
-                if (INT8) {
-                  const uint32_t w = cur[j * WPK + (iw >> 3)];
-                  o[e] = prmt_sign_bytes(w << (7 - (iw & 7))) | 0x01010101u;
-                } else {
-                  const uint32_t w = cur[j * WPK + (iw >> 4)];
-                  o[e] = ((w << (15 - (iw & 15))) & 0x80008000u) | 0x3F803F80u;
+              for (int cc = 0; cc < C_PER; ++cc) {  // 16-byte chunk cidx of the row = 4 shared-memory words
+                const int cidx = C0 + cc;
+                uint32_t o[4];
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                  const int iw = 4 * cidx + e;  // word index within the k-block's 32 output words
+                  if (INT8) {
+                    const uint32_t w = wq[(iw >> 3) - PART * WPP];
+                    o[e] = prmt_sign_bytes(w << (7 - (iw & 7))) | 0x01010101u;
+                  } else {
+                    const uint32_t w = wq[(iw >> 4) - PART * WPP];
+                    o[e] = ((w << (15 - (iw & 15))) & 0x80008000u) | 0x3F803F80u;
+                  }
                 }
+                const uint32_t dst = a_row + ((((uint32_t)cidx) ^ sw) << 4);
+                asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(dst), "r"(o[0]), "r"(o[1]),
+                             "r"(o[2]), "r"(o[3])
+                             : "memory");
               }
-              const uint32_t dst = a_row + ((((uint32_t)c) ^ sw) << 4);
-              asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(dst), "r"(o[0]), "r"(o[1]), "r"(o[2]),
-                           "r"(o[3])
-                           : "memory");
-            }
-            fence_proxy_async_smem();
-            __syncwarp();
-            if (lane == 0) mbar_arrive(full_bar(stage));
+            };
+            if (part_id == 0) expand(std::integral_constant<int, 0>{});
+            else expand(std::integral_constant<int, 1>{});
             if (++stage == STAGES) {
               stage = 0;
               phase ^= 1u;
             }
+            ++pending;
+          }
+          // One proxy fence publishes a batch of FB k-blocks, then their full barriers are signalled.
+          if ((j % FB) == FB - 1 || j == KPC - 1) {
+            if (pending) {
+              fence_proxy_async_smem();
+              __syncwarp();
+              if (lane == 0) {
+                int st = first_stage;
+                for (int q = 0; q < pending; ++q) {
+                  mbar_arrive(full_bar(st));
+                  if (++st == STAGES) st = 0;
+                }
+              }
+              first_stage = stage;
+              pending = 0;
+            }
           }
         }
+        if (++slot == Q_SLOTS) slot = 0;
       }
     }
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
   }
 
   tc_fence_before();
@@ -398,7 +455,7 @@ cudaError_t launch_one(const CUtensorMap& tmB, const SimParams& p, int grid, cud
     if (e != cudaSuccess) return e;
     attr_set = true;
   }
-  const int smem = p.stages * p.stage_bytes + SMEM_EXTRA;
+  const int smem = p.stages * p.stage_bytes + SMEM_EXTRA + QRING_BYTES;
   sim_tc_kernel<INT8, EPI><<<grid, NTHREADS, smem, st>>>(tmB, p);
   return cudaGetLastError();
 }
@@ -468,7 +525,7 @@ cudaError_t launch_sim_tc(TcContext* tc, const uint32_t* Hbits, int64_t N, int64
   p.n_tiles = n_tiles;
   p.num_kb = num_kb;
   p.stage_bytes = A_BYTES + nparts * kc * KB_BYTES;
-  p.stages = (SMEM_LIMIT - SMEM_EXTRA) / p.stage_bytes;
+  p.stages = (SMEM_LIMIT - SMEM_EXTRA - QRING_BYTES) / p.stage_bytes;
   if (p.stages > MAX_STAGES) p.stages = MAX_STAGES;
   p.e = e;
   const int grid = p.m_tiles < sm_count ? p.m_tiles : sm_count;

@@ -120,6 +120,68 @@ __device__ __forceinline__ void tc_mma(uint32_t d_tmem, uint64_t adesc, uint64_t
         : "memory");
   }
 }
+// ---- warp-converged single-issue forms -------------------------------------------------------
+// tcgen05.mma / tcgen05.commit / cp.async.bulk.tensor execute once per warp (uniform datapath).
+// Written under `if (lane == 0)` ptxas wraps each one in an ELECT / R2UR.BROADCAST / BRA.U.ANY
+// loop (~100 issue cycles apiece, measured: profiles/r1_tcgen05_path.md); predicated by the result
+// of elect.sync inside the same asm block, in a fully converged warp, it emits the bare
+// instruction.  All *_elect functions must be called by all 32 lanes of a converged warp with
+// warp-uniform arguments.
+__device__ __forceinline__ void mbar_arrive_expect_tx_elect(uint32_t bar, uint32_t bytes) {
+  asm volatile(
+      "{\n\t.reg .pred q;\n\telect.sync _|q, 0xffffffff;\n\t"
+      "@q mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n\t}" ::"r"(bar), "r"(bytes)
+      : "memory");
+}
+__device__ __forceinline__ void tma_load_2d_elect(uint32_t dst, const CUtensorMap* tm, uint32_t bar, int c0, int c1) {
+  asm volatile(
+      "{\n\t.reg .pred q;\n\telect.sync _|q, 0xffffffff;\n\t"
+      "@q cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];\n\t}"
+      ::"r"(dst), "l"(reinterpret_cast<uint64_t>(tm)), "r"(bar), "r"(c0), "r"(c1)
+      : "memory");
+}
+__device__ __forceinline__ void tma_load_2d_2sm_elect(uint32_t dst, const CUtensorMap* tm, uint32_t bar, int c0,
+                                                      int c1) {
+  asm volatile(
+      "{\n\t.reg .pred q;\n\telect.sync _|q, 0xffffffff;\n\t"
+      "@q cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];\n\t}"
+      ::"r"(dst), "l"(reinterpret_cast<uint64_t>(tm)), "r"(bar), "r"(c0), "r"(c1)
+      : "memory");
+}
+template <int CG = 1>
+__device__ __forceinline__ void tc_commit_elect(uint32_t bar) {
+  if (CG == 2) {
+    asm volatile(
+        "{\n\t.reg .pred q;\n\telect.sync _|q, 0xffffffff;\n\t"
+        "@q tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;\n\t}"
+        ::"r"(bar), "h"((uint16_t)3)
+        : "memory");
+  } else {
+    asm volatile(
+        "{\n\t.reg .pred q;\n\telect.sync _|q, 0xffffffff;\n\t"
+        "@q tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];\n\t}" ::"r"(bar)
+        : "memory");
+  }
+}
+#define HDC_MMA_ELECT(CGS, KIND)                                                                     \
+  asm volatile(                                                                                      \
+      "{\n\t.reg .pred p, q;\n\telect.sync _|q, 0xffffffff;\n\tsetp.ne.b32 p, %4, 0;\n\t"            \
+      "@q tcgen05.mma.cta_group::" CGS ".kind::" KIND " [%0], %1, %2, %3, p;\n\t}" ::"r"(d_tmem),    \
+      "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)                                            \
+      : "memory")
+template <bool INT8, int CG = 1>
+__device__ __forceinline__ void tc_mma_elect(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc,
+                                             uint32_t accumulate) {
+  if (CG == 2) {
+    if (INT8) HDC_MMA_ELECT("2", "i8");
+    else HDC_MMA_ELECT("2", "f16");
+  } else {
+    if (INT8) HDC_MMA_ELECT("1", "i8");
+    else HDC_MMA_ELECT("1", "f16");
+  }
+}
+#undef HDC_MMA_ELECT
+
 // 32 lanes x 32 consecutive 32-bit columns: thread t of the warp gets lane (base + t), v[j] = column j
 __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
   asm volatile(
