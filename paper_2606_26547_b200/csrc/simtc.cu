@@ -65,6 +65,7 @@ struct SimParams {
   int nparts;   // 1, or 3 for the fp32 class operand
   int m_tiles, n_tiles;
   int num_kb;
+  int kps;          // k-blocks per pipeline group
   int stages;       // ring depth
   int stage_bytes;  // A_BYTES + nparts*kc*KB_BYTES
   Epilogue e;
@@ -88,7 +89,9 @@ __global__ void __launch_bounds__(NTHREADS, 1)
 sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
   extern __shared__ uint8_t smem_raw[];
   const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
-  const int STAGES = p.stages;
+  const int STAGES = p.stages;  // k-block slots in the ring
+  const int G = p.kps;          // k-blocks per pipeline group (one full / empty barrier pair per group)
+  const int NG = STAGES / G;
   const uint32_t STAGE_BYTES = (uint32_t)p.stage_bytes;
   const uint32_t bar0 = base + STAGES * STAGE_BYTES;
   auto full_bar = [&](int s) { return bar0 + 8u * s; };
@@ -104,7 +107,7 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
 
   if (warp == 0 && lane == 0) {
     asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&tmB)) : "memory");
-    for (int s = 0; s < STAGES; ++s) {
+    for (int s = 0; s < NG; ++s) {
       mbar_init(full_bar(s), 1 + EXW);  // producer (with the TMA byte count) + one arrival per expander warp
       mbar_init(empty_bar(s), 1);
     }
@@ -125,23 +128,26 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
 
   if (warp == 0) {
     // ================================================================= TMA producer (class tiles)
-    int stage = 0;
+    int grp = 0;
     uint32_t phase = 0;
     for (int64_t i = 0; i < tiles_per_cta; ++i) {
       const int nt = (int)(i % p.n_tiles);
-      for (int kb = 0; kb < p.num_kb; ++kb) {
-        mbar_wait(empty_bar(stage), phase ^ 1u);
-        mbar_arrive_expect_tx_elect(full_bar(stage), (uint32_t)nb_rows * KB_BYTES);
-        tma_load_2d_elect(base + stage * STAGE_BYTES + A_BYTES, &tmB, full_bar(stage), kb * BK, nt * nb_rows);
-        if (++stage == STAGES) {
-          stage = 0;
+      for (int kb0 = 0; kb0 < p.num_kb; kb0 += G) {
+        const int n = p.num_kb - kb0 < G ? p.num_kb - kb0 : G;
+        mbar_wait(empty_bar(grp), phase ^ 1u);
+        mbar_arrive_expect_tx_elect(full_bar(grp), (uint32_t)(n * nb_rows) * KB_BYTES);
+        for (int u = 0; u < n; ++u)
+          tma_load_2d_elect(base + (grp * G + u) * STAGE_BYTES + A_BYTES, &tmB, full_bar(grp), (kb0 + u) * BK,
+                            nt * nb_rows);
+        if (++grp == NG) {
+          grp = 0;
           phase ^= 1u;
         }
       }
     }
   } else if (warp == 1) {
     // ================================================================= MMA issuer
-    int stage = 0;
+    int grp = 0;
     uint32_t phase = 0;
     int acc = 0;
     uint32_t acc_phase = 0;
@@ -150,20 +156,22 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
       mbar_wait(tempty_bar(acc), acc_phase ^ 1u);
       tc_fence_after();
       const uint32_t d_tmem = tmem_base + (uint32_t)(acc * BN_MAX);
-      for (int kb = 0; kb < p.num_kb; ++kb) {
-        mbar_wait(full_bar(stage), phase);
+      for (int kb0 = 0; kb0 < p.num_kb; kb0 += G) {
+        const int n = p.num_kb - kb0 < G ? p.num_kb - kb0 : G;
+        mbar_wait(full_bar(grp), phase);
         tc_fence_after();
-        {  // whole warp, converged: each call issues once (tc_ptx.cuh, *_elect)
-          const uint32_t sa = base + stage * STAGE_BYTES;
+        // whole warp, converged: each call issues once (tc_ptx.cuh, *_elect)
+        for (int u = 0; u < n; ++u) {
+          const uint32_t sa = base + (grp * G + u) * STAGE_BYTES;
           const uint64_t da = smem_desc(sa), db = smem_desc(sa + A_BYTES);
 #pragma unroll
           for (int k = 0; k < KB_BYTES / 32; ++k)
-            tc_mma_elect<INT8>(d_tmem, da + 2u * k, db + 2u * k, idesc, (kb | k) != 0 ? 1u : 0u);
-          tc_commit_elect(empty_bar(stage));
-          if (kb == p.num_kb - 1) tc_commit_elect(tfull_bar(acc));
+            tc_mma_elect<INT8>(d_tmem, da + 2u * k, db + 2u * k, idesc, ((kb0 + u) | k) != 0 ? 1u : 0u);
         }
-        if (++stage == STAGES) {
-          stage = 0;
+        tc_commit_elect(empty_bar(grp));  // frees the group's slots when these MMAs retire
+        if (kb0 + n == p.num_kb) tc_commit_elect(tfull_bar(acc));
+        if (++grp == NG) {
+          grp = 0;
           phase ^= 1u;
         }
       }
@@ -269,7 +277,6 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
     constexpr int WPK = INT8 ? 4 : 2;         // packed words per k-block
     constexpr int KPC = QW / WPK;             // k-blocks per ring tile
     constexpr int WPP = WPK / 2;              // words of a k-block this thread's half needs
-    const int FB = STAGES >= 8 ? 4 : (STAGES >= 4 ? 2 : 1);  // k-blocks published per proxy fence (<= half the ring)
     const uint32_t sw = (uint32_t)(t & 7);
     const uint32_t q_smem = bar0 + 256u;      // ring base (after the barriers)
     const uint32_t* q_ptr = reinterpret_cast<const uint32_t*>(smem_raw + (q_smem - smem_u32(smem_raw)));
@@ -306,12 +313,12 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
       asm volatile("cp.async.commit_group;" ::: "memory");
     }
 
-    int stage = 0;
+    int grp = 0;
     uint32_t phase = 0;
     int slot = 0;
     int64_t step = 0;
     for (int64_t i = 0; i < tiles_per_cta; ++i) {
-      int first_stage = stage, pending = 0;
+      int u = 0;  // position inside the current group
       for (int c = 0; c < nch; ++c, ++step) {
         asm volatile("cp.async.wait_group %0;" ::"n"(Q_SLOTS - 2) : "memory");
         asm volatile("bar.sync 1, %0;" ::"n"(32 * EXW) : "memory");  // tile visible; previous slot free
@@ -322,15 +329,15 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
 #pragma unroll
         for (int j = 0; j < KPC; ++j) {
           if (kb0 + j < p.num_kb) {
-            mbar_wait(empty_bar(stage), phase ^ 1u);
-            const uint32_t a_row = base + stage * STAGE_BYTES + (uint32_t)t * KB_BYTES;
+            if (u == 0) mbar_wait(empty_bar(grp), phase ^ 1u);
+            const uint32_t a_row = base + (grp * G + u) * STAGE_BYTES + (uint32_t)t * KB_BYTES;
             // the chunk range is a compile-time constant per branch
             auto expand = [&](auto part) {
               constexpr int PART = decltype(part)::value;
               constexpr int C0 = PART * C_PER;
               uint32_t wq[WPP];
 #pragma unroll
-              for (int u = 0; u < WPP; ++u) wq[u] = qs[(j * WPK + PART * WPP + u) * Q_LD];
+              for (int v = 0; v < WPP; ++v) wq[v] = qs[(j * WPK + PART * WPP + v) * Q_LD];
 #pragma unroll
               for (int cc = 0; cc < C_PER; ++cc) {  // 16-byte chunk cidx of the row = 4 shared-memory words
                 const int cidx = C0 + cc;
@@ -354,26 +361,16 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
             };
             if (part_id == 0) expand(std::integral_constant<int, 0>{});
             else expand(std::integral_constant<int, 1>{});
-            if (++stage == STAGES) {
-              stage = 0;
-              phase ^= 1u;
-            }
-            ++pending;
-          }
-          // One proxy fence publishes a batch of FB k-blocks, then their full barriers are signalled.
-          if ((j % FB) == FB - 1 || j == KPC - 1) {
-            if (pending) {
+            // the group is published (one proxy fence, one arrival per warp) when its last k-block is written
+            if (++u == G || kb0 + j == p.num_kb - 1) {
               fence_proxy_async_smem();
               __syncwarp();
-              if (lane == 0) {
-                int st = first_stage;
-                for (int q = 0; q < pending; ++q) {
-                  mbar_arrive(full_bar(st));
-                  if (++st == STAGES) st = 0;
-                }
+              if (lane == 0) mbar_arrive(full_bar(grp));
+              u = 0;
+              if (++grp == NG) {
+                grp = 0;
+                phase ^= 1u;
               }
-              first_stage = stage;
-              pending = 0;
             }
           }
         }
@@ -527,6 +524,10 @@ cudaError_t launch_sim_tc(TcContext* tc, const uint32_t* Hbits, int64_t N, int64
   p.stage_bytes = A_BYTES + nparts * kc * KB_BYTES;
   p.stages = (SMEM_LIMIT - SMEM_EXTRA - QRING_BYTES) / p.stage_bytes;
   if (p.stages > MAX_STAGES) p.stages = MAX_STAGES;
+  // k-blocks per pipeline group: every hand-off through the full / empty barriers costs several hundred
+  // cycles whatever the k-block holds, so short k-blocks (few class rows) travel in groups
+  p.kps = p.stages >= 8 ? 4 : (p.stages >= 4 ? 2 : 1);
+  p.stages -= p.stages % p.kps;
   p.e = e;
   const int grid = p.m_tiles < sm_count ? p.m_tiles : sm_count;
   ++*nlaunch;
