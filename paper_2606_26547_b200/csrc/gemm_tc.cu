@@ -3,9 +3,9 @@
 // epilogues fused: sign + pack (random-projection encode, Listing 1 L68-L70 + L161),
 // scores (L110 cos_sim / L197 dot) and row arg-max (L79-L80).
 //
-// One persistent CTA per SM, 6 warps: warp 0 = TMA producer, warp 1 = MMA issuer (+ TMEM
-// allocation), warps 2-5 = epilogue (warp w reads TMEM lanes 32*(w%4).., thread = accumulator
-// row).  k-blocks of 128 bytes (64 bf16 / 128 int8), mbarrier ring between producer and issuer, two
+// One persistent CTA per SM, 10 warps: warp 0 = TMA producer, warp 1 = MMA issuer (+ TMEM
+// allocation), warps 2-9 = epilogue (warp w reads TMEM lanes 32*(w%4).., thread = accumulator
+// row; two warps per lane quadrant split a tile's columns).  k-blocks of 128 bytes (64 bf16 / 128 int8), mbarrier ring between producer and issuer, two
 // 256-column TMEM accumulators so that the epilogue of tile i overlaps the MMAs of tile i+1.
 // Operands are K-contiguous ("K-major") for both A and B, which is the layout of X[N][F], P[D][F]
 // and C[K][D] (include/hdc.h).
@@ -77,7 +77,8 @@ using namespace tcp;
 constexpr int BM = 128;            // rows of A per tile == TMEM lanes
 constexpr int BN = 256;            // rows of B per tile == TMEM columns of one accumulator
 constexpr int A_BYTES = BM * KB_BYTES;   // 16 KB
-constexpr int NTHREADS = 192;
+constexpr int EPI_WARPS = 8;            // two per TMEM lane quadrant: columns 0-127 and 128-255 of a tile
+constexpr int NTHREADS = 64 + 32 * EPI_WARPS;
 constexpr int TMEM_COLS = 512;
 constexpr int MAX_STAGES = 6;
 template <int CG>
@@ -164,7 +165,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     }
     for (int s = 0; s < 2; ++s) {
       mbar_init(tfull_bar(s), 1);
-      mbar_init(tempty_bar(s), 4 * CG);
+      mbar_init(tempty_bar(s), EPI_WARPS * CG);
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
@@ -254,9 +255,14 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
       }
     }
   } else {
-    // ================================================================= epilogue (warps 2..5)
+    // ================================================================= epilogue (warps 2..9)
     using AccT = typename std::conditional<INT8, int, float>::type;
     const int q = warp & 3;  // TMEM lane quadrant this warp may read
+    // EPI_SIGN: warps 2-5 drain chunks 0-3 of a tile, warps 6-9 chunks 4-7 (with few k-blocks per
+    // tile the sign epilogue, not the MMAs, set the pace: profiles/r1_tcgen05_path.md, int8).  The
+    // score / arg-max epilogues need every column of a row in one thread: warps 6-9 only hand the
+    // accumulator back.
+    const int ehalf = (warp - 2) >> 2;
     int acc = 0;
     uint32_t acc_phase = 0;
     Top2 run = Top2{NEG_BIG, INT_MAX, NEG_BIG};
@@ -296,19 +302,21 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
             }
           }
         };
-        tmem_ld32(taddr, va);
-        for (int c = 0; c < nchunks; c += 2) {
+        const int c_begin = ehalf * 4;
+        const int c_end = nchunks < c_begin + 4 ? nchunks : c_begin + 4;
+        if (c_begin < c_end) tmem_ld32(taddr + (uint32_t)(c_begin * 32), va);
+        for (int c = c_begin; c < c_end; c += 2) {
           tmem_ld_wait();
-          if (c + 1 < nchunks) tmem_ld32(taddr + (uint32_t)((c + 1) * 32), vb);
+          if (c + 1 < c_end) tmem_ld32(taddr + (uint32_t)((c + 1) * 32), vb);
           pack_store(va, c);
-          if (c + 1 < nchunks) {
+          if (c + 1 < c_end) {
             tmem_ld_wait();
-            if (c + 2 < nchunks) tmem_ld32(taddr + (uint32_t)((c + 2) * 32), va);
+            if (c + 2 < c_end) tmem_ld32(taddr + (uint32_t)((c + 2) * 32), va);
             pack_store(vb, c + 1);
           }
         }
       }
-      for (int c = 0; EPI != EPI_SIGN && c < nchunks; ++c) {
+      for (int c = 0; EPI != EPI_SIGN && ehalf == 0 && c < nchunks; ++c) {
         uint32_t v[32];
         tmem_ld32(taddr + (uint32_t)(c * 32), v);
         tmem_ld_wait();
@@ -359,7 +367,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
         acc_phase ^= 1u;
       }
       if (EPI == EPI_ARGMAX && nt == p.n_tiles - 1) {
-        if (row_ok) {
+        if (row_ok && ehalf == 0) {
           double b1 = run.b1, b2 = run.b2;
           if (b2 == NEG_BIG) b2 = b1;  // K == 1
           if (p.e.ham_D > 0) {
