@@ -286,6 +286,33 @@ def train(hbits, y, K, D_eff, hv_bits, sim, epochs, lr, batch=0):
     return C, hist
 
 
+# ------------------------------------------------------------------------------------- S11
+def kmeans_epoch(hbits: np.ndarray, C_acc: np.ndarray, D_eff: int, hv_bits: int, sim: int, prev=None):
+    """One iteration of HD-Clustering ("HD-Clustering implements K-Means clustering
+    using HDC", L221: cosine or Hamming similarity, TRAIN_ITERATIONS epochs).  The paper gives no
+    pseudo-code; reading A16 is Lloyd's iteration with the path's own primitives:
+      (i)   a_n = classify(h_n) against the current cluster accumulators (S5-S7: the similarity and
+            element precision of the knobs, ties to the lowest cluster index);
+      (ii)  every cluster that received at least one sample is re-bundled from its members,
+            C_acc[k,d] = sum_{n: a_n = k} v[n,d]   (S8);  a cluster with no member keeps its
+            accumulator unchanged.
+    Returns (C_acc' fp32 [K][D_eff], assignments int32 [N], number of n with a_n != prev[n]
+    (0 if prev is None))."""
+    hb = np.asarray(hbits, dtype=np.uint8)[:, :D_eff]
+    C = np.array(C_acc, dtype=np.float32)[:, :D_eff].copy()
+    K = C.shape[0]
+    S = similarity(hb, C, D_eff, sim, hv_bits)
+    a, _, _ = classify(S, sim)
+    a = a.astype(np.int32)
+    v = bipolar(hb).astype(np.int64)
+    for k in range(K):
+        members = np.nonzero(a == k)[0]
+        if members.size:
+            C[k] = v[members].sum(axis=0).astype(np.float32)
+    changed = 0 if prev is None else int((a != np.asarray(prev)).sum())
+    return C, a, changed
+
+
 def infer(hbits, C_acc, D_eff, sim, hv_bits):
     """similarity + arg-extremum (Listing 1 L72-L80)."""
     S = similarity(hbits, C_acc, D_eff, sim, hv_bits)

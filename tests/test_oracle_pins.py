@@ -444,3 +444,101 @@ def test_generators_are_seeded_and_shaped():
     assert c5["X"].shape == (80, 1024) and c5["P"].shape == (128, 1024)
     assert np.array_equal(o.round_bf16(c5["X"]), c5["X"])     # bf16-representable
     assert abs(float(c5["X"][:64].std()) - 1.0) < 0.05
+
+
+# ------------------------------------------------------------------------------------- S11 k-means
+def _kmeans_brute(hb, C, D_eff, sim):
+    """Plain python loops: assign by cosine (double) or Hamming to sign bits, re-bundle members."""
+    N, K = hb.shape[0], C.shape[0]
+    a = []
+    for n in range(N):
+        best, bi = None, 0
+        for k in range(K):
+            if sim == o.SIM_HAMMING:
+                s = -sum(int(hb[n, d]) != int(C[k, d] < 0) for d in range(D_eff))
+            else:
+                dotv = sum((1 - 2 * int(hb[n, d])) * float(C[k, d]) for d in range(D_eff))
+                nrm = sum(float(C[k, d]) ** 2 for d in range(D_eff)) ** 0.5
+                s = dotv / (D_eff ** 0.5 * nrm) if nrm > 0 else 0.0
+            if best is None or s > best:
+                best, bi = s, k
+        a.append(bi)
+    Cn = np.array(C[:, :D_eff], dtype=np.float32)
+    for k in range(K):
+        mem = [n for n in range(N) if a[n] == k]
+        if mem:
+            Cn[k] = [sum(1 - 2 * int(hb[n, d]) for n in mem) for d in range(D_eff)]
+    return Cn, np.array(a, dtype=np.int32)
+
+
+@pytest.mark.parametrize("sim,hv_bits", [(o.SIM_COS, 32), (o.SIM_HAMMING, 1)])
+@pytest.mark.parametrize("N,K,D,D_eff", [(9, 3, 40, 40), (12, 4, 70, 33), (5, 1, 16, 16)])
+def test_kmeans_epoch_brute_force(sim, hv_bits, N, K, D, D_eff):
+    r = np.random.default_rng(N * 100 + K)
+    hb = r.integers(0, 2, size=(N, D), dtype=np.uint8)
+    C = r.integers(-5, 6, size=(K, D)).astype(np.float32)
+    C[C == 0] = 1.0
+    Cn, a, ch = o.kmeans_epoch(hb, C, D_eff, hv_bits, sim, prev=np.zeros(N, dtype=np.int32))
+    Cb, ab = _kmeans_brute(hb, C, D_eff, sim)
+    assert np.array_equal(a, ab)
+    assert np.array_equal(Cn, Cb)
+    assert ch == int((ab != 0).sum())
+
+
+def test_kmeans_empty_cluster_keeps_its_accumulator_and_k1_is_the_bundle():
+    r = np.random.default_rng(7)
+    hb = r.integers(0, 2, size=(20, 64), dtype=np.uint8)
+    c0 = 1.0 - 2.0 * hb[0].astype(np.float32)
+    C = np.stack([c0, -c0])               # cluster 1 = the antipode of sample 0
+    far = (hb ^ hb[0]).sum(axis=1) > 32  # samples closer to the antipode
+    hb = hb[~far]
+    Cn, a, _ = o.kmeans_epoch(hb, C, 64, 32, o.SIM_COS)
+    assert (a == 0).all()
+    assert np.array_equal(Cn[1], C[1])                                   # empty: unchanged
+    assert np.array_equal(Cn[0], o.bundle(hb, np.zeros(len(hb), dtype=np.int64), 1, 64)[0])
+    C1, a1, _ = o.kmeans_epoch(hb, C[:1], 64, 32, o.SIM_COS)           # K = 1 -> the bundle of everything
+    assert (a1 == 0).all() and np.array_equal(C1[0], Cn[0])
+
+
+def test_kmeans_spherical_objective_never_decreases_and_reaches_a_fixed_point():
+    """With cosine similarity, (assign to the most similar centre, centre = sum of members) is
+    spherical k-means: J = sum_n <v_n, c_hat_a(n)> is non-decreasing from one epoch to the next and
+    the iteration stops at a fixed point (textbook property, independent of the oracle's code)."""
+    r = np.random.default_rng(11)
+    D, K, N = 512, 5, 300
+    proto = r.integers(0, 2, size=(K, D), dtype=np.uint8)
+    yt = r.integers(0, K, size=N)
+    hb = proto[yt] ^ (r.random((N, D)) < 0.3).astype(np.uint8)
+    C = (1.0 - 2.0 * hb[r.choice(N, K, replace=False)]).astype(np.float32)   # random samples as seeds
+    v = 1.0 - 2.0 * hb.astype(np.float64)
+
+    def J(Cc, a):
+        ch = Cc.astype(np.float64)
+        ch = ch / np.maximum(np.linalg.norm(ch, axis=1, keepdims=True), 1e-300)
+        return float((v * ch[a]).sum())
+
+    prev, hist = None, []
+    for _ in range(30):
+        C2, a, ch = o.kmeans_epoch(hb, C, D, 32, o.SIM_COS, prev)
+        hist.append(J(C2, a))
+        if prev is not None and ch == 0:
+            assert np.array_equal(C2, C)                                 # fixed point
+            break
+        C, prev = C2, a
+    else:
+        raise AssertionError("k-means did not converge in 30 epochs")
+    assert all(b >= a_ - 1e-9 for a_, b in zip(hist, hist[1:]))
+
+
+def test_kmeans_recovers_well_separated_clusters():
+    r = np.random.default_rng(12)
+    D, K, N = 2048, 4, 200
+    proto = r.integers(0, 2, size=(K, D), dtype=np.uint8)
+    yt = np.arange(N) % K
+    hb = proto[yt] ^ (r.random((N, D)) < 0.1).astype(np.uint8)
+    for sim, bits in ((o.SIM_COS, 32), (o.SIM_HAMMING, 1)):
+        C = (1.0 - 2.0 * hb[:K]).astype(np.float32)                      # one seed per true cluster
+        C, a, _ = o.kmeans_epoch(hb, C, D, bits, sim)
+        assert np.array_equal(a, yt)
+        C2, a2, ch = o.kmeans_epoch(hb, C, D, bits, sim, prev=a)
+        assert ch == 0 and np.array_equal(C2, C)
