@@ -59,7 +59,7 @@ enum { HDC_F32 = 0, HDC_BF16 = 1, HDC_I8 = 2, HDC_B1 = 3, HDC_U8 = 4, HDC_I32 = 
 /* similarity kinds (L167 algorithmic choice) */
 enum { HDC_SIM_DOT = 0, HDC_SIM_COS = 1, HDC_SIM_HAMMING = 2 };
 /* hdc_train_epoch modes */
-enum { HDC_TRAIN_BUNDLE = 0, HDC_TRAIN_PERCEPTRON = 1 };
+enum { HDC_TRAIN_BUNDLE = 0, HDC_TRAIN_PERCEPTRON = 1, HDC_TRAIN_KMEANS = 2 };
 /* hdc_encode_rp outputs (bit-or) */
 enum { HDC_OUT_BITS = 1, HDC_OUT_RAW = 4 };
 /* hdc_workspace_bytes ops */
@@ -180,6 +180,12 @@ int32_t hdc_classify(hdc_handle_t h, const uint32_t* Hbits, int64_t N, int64_t l
  *      (0 => N): yhat = classify(h) with the current C_acc at knobs->{hv_bits,sim};
  *      Delta[k,d] = sum_{yhat_n != y_n} ([k = y_n] - [k = yhat_n]) * v[n,d]   (integer);
  *      C_acc[k,d] = fl32(C_acc[k,d] + fl32(lr * (float)Delta[k,d])).
+ *  mode HDC_TRAIN_KMEANS (HD-Clustering; reading A16): one Lloyd
+ *      iteration over all N samples: a = classify(h) with the current C_acc at knobs->{hv_bits,sim};
+ *      every cluster with at least one member is re-bundled, C_acc[k,d] = sum_{n: a_n = k} v[n,d];
+ *      a cluster without members keeps its accumulator.  y is the PREVIOUS assignment (nullable),
+ *      pred receives a, n_wrong is incremented by #{n : a_n != y_n} (0 moved = converged);
+ *      lr and batch are ignored.
  * y [N] int32 labels in [0,K) (unchecked on device).  pred (nullable, int32 [N]) receives yhat;
  * n_wrong (nullable, device uint64) is INCREMENTED by the number of mispredictions.
  * Deterministic: integer Delta, no floating-point atomics. */

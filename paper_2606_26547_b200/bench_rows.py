@@ -165,6 +165,23 @@ def row_train(h, peaks, reps, N=6238, K=26, D=10000, hv_bits=32, sim_name="cos")
             "call_ms": call_ms, "samples_per_s": N / (call_ms * 1e-3)}
 
 
+def row_kmeans(h, peaks, reps, N=7797, K=26, D=10000, hv_bits=32, sim_name="cos"):
+    """HD-Clustering epoch (assign + re-bundle) on noisy copies of K prototypes, ISOLET-sized."""
+    sim = {"cos": hd.HDC_SIM_COS, "hamming": hd.HDC_SIM_HAMMING}[sim_name]
+    W = (D + 31) // 32
+    proto = _rand_bits(K, W, 7)
+    yt = torch.randint(0, K, (N,), device="cuda", generator=_gen(8))
+    noise = _rand_bits(N, W, 9) & _rand_bits(N, W, 10) & _rand_bits(N, W, 11)      # ~12.5 % flipped bits
+    H = (proto[yt] ^ noise).contiguous()
+    C = _class_acc(K, D, 12, per_class=1)
+    kn = hd.knobs(D, hv_bits=hv_bits, sim=sim)
+    a = torch.empty(N, dtype=torch.int32, device="cuda")
+    fn = lambda: h.hdc_train_epoch(hd.HDC_TRAIN_KMEANS, H, None, C, kn, pred=a)  # noqa: E731
+    call_ms = _time(fn, reps)
+    return {"what": f"hdc_train_epoch (k-means epoch) N={N} K={K} D={D} hv_bits={hv_bits} sim={sim_name}",
+            "call_ms": call_ms, "samples_per_s": N / (call_ms * 1e-3)}
+
+
 ROWS = {
     "c2_encode_f32": lambda h, p, r: row_encode(h, p, r, 131072, 617, 10000, "f32"),
     "c2_encode_bf16": lambda h, p, r: row_encode(h, p, r, 131072, 617, 10000, "bf16"),
@@ -177,6 +194,7 @@ ROWS = {
     "c5_classify_bf16": lambda h, p, r: row_classify(h, p, r, 65536, 1000, 16384, 16, "cos"),
     "c5_classify_1bit": lambda h, p, r: row_classify(h, p, r, 65536, 1000, 16384, 1, "hamming"),
     "c2_train_epoch": lambda h, p, r: row_train(h, p, r),
+    "c2_kmeans_epoch": lambda h, p, r: row_kmeans(h, p, r),
 }
 
 

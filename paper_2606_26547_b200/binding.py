@@ -18,7 +18,7 @@ HDC_ERR_INVALID_ARG, HDC_ERR_UNSUPPORTED, HDC_ERR_ALIGNMENT = -1, -2, -3
 HDC_ERR_WORKSPACE, HDC_ERR_CUDA, HDC_ERR_ARCH = -4, -5, -6
 HDC_F32, HDC_BF16, HDC_I8, HDC_B1, HDC_U8, HDC_I32 = 0, 1, 2, 3, 4, 5
 HDC_SIM_DOT, HDC_SIM_COS, HDC_SIM_HAMMING = 0, 1, 2
-HDC_TRAIN_BUNDLE, HDC_TRAIN_PERCEPTRON = 0, 1
+HDC_TRAIN_BUNDLE, HDC_TRAIN_PERCEPTRON, HDC_TRAIN_KMEANS = 0, 1, 2
 HDC_OUT_BITS, HDC_OUT_RAW = 1, 4
 HDC_OP_ENCODE_RP, HDC_OP_ENCODE_LEVELID, HDC_OP_SIMILARITY = 0, 1, 2
 HDC_OP_CLASSIFY, HDC_OP_TRAIN_EPOCH, HDC_OP_INFER_RP_HOST = 3, 4, 5
@@ -239,7 +239,7 @@ class Handle:
         N = Hbits.shape[0]
         K, D = C_acc.shape
         B = N if batch in (0, None) or batch > N else batch
-        ws, wsb = self._workspace(self.workspace_bytes(HDC_OP_TRAIN_EPOCH, B, 0, D, K, kn))
+        ws, wsb = self._workspace(self.workspace_bytes(HDC_OP_TRAIN_EPOCH, N if mode == HDC_TRAIN_KMEANS else B, 0, D, K, kn))
         rc = self._L.hdc_train_epoch(self._h, mode, _ptr(Hbits), N, _rowmajor(Hbits, "Hbits"), _ptr(y),
                                      _ptr(C_acc), K, _rowmajor(C_acc, "C_acc"), D, C.byref(kn),
                                      C.c_float(lr), int(batch or 0), _ptr(pred), _ptr(n_wrong), ws, wsb,

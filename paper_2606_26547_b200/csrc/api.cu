@@ -475,6 +475,7 @@ extern "C" size_t hdc_workspace_bytes(hdc_handle_t h, int32_t op, int64_t N, int
     case HDC_OP_TRAIN_EPOCH: {
       b.take<int32_t>((size_t)K * words_of(k.D_eff) * 32);  // Delta
       b.take<int32_t>((size_t)N);                           // predictions of one mini-batch
+      b.take<int32_t>((size_t)K);                           // members per cluster (HDC_TRAIN_KMEANS)
       return b.off + 256 + similarity_ws(K, &k);
     }
     case HDC_OP_INFER_RP_HOST: {
@@ -621,8 +622,9 @@ extern "C" int32_t hdc_train_epoch(hdc_handle_t h, int32_t mode, const uint32_t*
                                    int32_t D, const hdc_knobs_t* knobs, float lr, int64_t batch, int32_t* pred,
                                    unsigned long long* n_wrong, void* ws, size_t ws_bytes, void* stream) {
   if (!h) return HDC_ERR_INVALID_ARG;
-  if (mode != HDC_TRAIN_BUNDLE && mode != HDC_TRAIN_PERCEPTRON) return fail(h, HDC_ERR_INVALID_ARG, "train: mode");
-  if (!y) return fail(h, HDC_ERR_INVALID_ARG, "train: y is NULL");
+  if (mode != HDC_TRAIN_BUNDLE && mode != HDC_TRAIN_PERCEPTRON && mode != HDC_TRAIN_KMEANS)
+    return fail(h, HDC_ERR_INVALID_ARG, "train: mode");
+  if (!y && mode != HDC_TRAIN_KMEANS) return fail(h, HDC_ERR_INVALID_ARG, "train: y is NULL");
   if (batch < 0) return fail(h, HDC_ERR_INVALID_ARG, "train: batch < 0");
   hdc_knobs_t k;
   if (!knobs) return fail(h, HDC_ERR_INVALID_ARG, "knobs is NULL");
@@ -644,6 +646,22 @@ extern "C" int32_t hdc_train_epoch(hdc_handle_t h, int32_t mode, const uint32_t*
     ce = launch_class_update(Hbits, 0, N, ldh_words, y, nullptr, C_acc, K, ldc, k.D_eff, 1.0f, delta, nullptr,
                              h->sm_count, st, &h->launches);
     return ce == cudaSuccess ? HDC_OK : cuda_fail(h, ce, "bundle");
+  }
+  if (mode == HDC_TRAIN_KMEANS) {
+    // assign every sample with the current accumulators, then re-bundle the clusters that have members
+    int32_t* assign = pred ? pred : b.take<int32_t>((size_t)N);
+    int32_t* members = b.take<int32_t>((size_t)K);
+    if (b.off > ws_bytes) return fail(h, HDC_ERR_WORKSPACE, "train: workspace too small");
+    rc = do_similarity(h, Hbits, N, ldh_words, C_acc, K, ldc, &k, nullptr, 0, 0, assign, nullptr, nullptr, b,
+                       ws_bytes, st);
+    if (rc) return rc;
+    Timed tm(h, HDC_K_CLASS_UPDATE, st);
+    ce = launch_kmeans_reset(assign, y, N, C_acc, K, ldc, k.D_eff, members, n_wrong, h->sm_count, st,
+                             &h->launches);
+    if (ce != cudaSuccess) return cuda_fail(h, ce, "kmeans reset");
+    ce = launch_class_update(Hbits, 0, N, ldh_words, assign, nullptr, C_acc, K, ldc, k.D_eff, 1.0f, delta, nullptr,
+                             h->sm_count, st, &h->launches);
+    return ce == cudaSuccess ? HDC_OK : cuda_fail(h, ce, "kmeans bundle");
   }
   const int64_t B = (batch == 0 || batch > N) ? N : batch;
   int32_t* pbuf = pred;

@@ -127,6 +127,13 @@ cudaError_t launch_class_update(const uint32_t* Hbits, int64_t n0, int64_t nb, i
                                 unsigned long long* n_wrong, int sm_count, cudaStream_t st,
                                 int64_t* nlaunch);
 
+// HD-Clustering re-bundle step (train.cu): counts members per cluster (members: int32 [K] workspace),
+// adds the number of samples with assign != prev to *n_changed (both nullable) and zeroes the
+// accumulator rows of the clusters that have members
+cudaError_t launch_kmeans_reset(const int32_t* assign, const int32_t* prev, int64_t N, float* C_acc, int K,
+                                int64_t ldc, int D_eff, int32_t* members, unsigned long long* n_changed,
+                                int sm_count, cudaStream_t st, int64_t* nlaunch);
+
 static inline int64_t round_up(int64_t x, int64_t m) { return (x + m - 1) / m * m; }
 static inline int words_of(int D_eff) { return (D_eff + 31) >> 5; }
 

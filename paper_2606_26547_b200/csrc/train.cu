@@ -81,7 +81,56 @@ __global__ void count_wrong_kernel(const int32_t* __restrict__ y, const int32_t*
   if ((threadIdx.x & 31) == 0 && c) atomicAdd(n_wrong, (unsigned long long)c);
 }
 
+// HD-Clustering (reading A16): members per cluster and, when the
+// previous assignment is given, the number of samples that moved.
+__global__ void assign_stats_kernel(const int32_t* __restrict__ assign, const int32_t* __restrict__ prev,
+                                    int64_t N, int32_t* __restrict__ members,
+                                    unsigned long long* __restrict__ n_changed) {
+  unsigned int c = 0;
+  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < N;
+       i += (int64_t)gridDim.x * blockDim.x) {
+    const int a = assign[i];
+    atomicAdd(members + a, 1);
+    if (prev) c += (prev[i] != a);
+  }
+#pragma unroll
+  for (int off = 16; off; off >>= 1) c += __shfl_xor_sync(0xffffffffu, c, off);
+  if (n_changed && (threadIdx.x & 31) == 0 && c) atomicAdd(n_changed, (unsigned long long)c);
+}
+
+// clusters that received members are rebuilt from scratch; empty ones keep their accumulator
+__global__ void zero_member_rows_kernel(float* __restrict__ C, int K, int D_eff, int64_t ldc,
+                                        const int32_t* __restrict__ members) {
+  const int64_t total = (int64_t)K * D_eff;
+  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < total;
+       i += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t k = i / D_eff;
+    if (members[k] > 0) C[k * ldc + (i - k * D_eff)] = 0.0f;
+  }
+}
+
 }  // namespace
+
+// members: int32 [K] workspace (zeroed here)
+cudaError_t launch_kmeans_reset(const int32_t* assign, const int32_t* prev, int64_t N, float* C_acc, int K,
+                                int64_t ldc, int D_eff, int32_t* members, unsigned long long* n_changed,
+                                int sm_count, cudaStream_t st, int64_t* nlaunch) {
+  cudaError_t e = cudaMemsetAsync(members, 0, sizeof(int32_t) * (size_t)K, st);
+  if (e != cudaSuccess) return e;
+  int64_t g = (N + 255) / 256;
+  if (g > sm_count * 4) g = sm_count * 4;
+  if (g < 1) g = 1;
+  assign_stats_kernel<<<(unsigned)g, 256, 0, st>>>(assign, prev, N, members, n_changed);
+  ++*nlaunch;
+  e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  const int64_t total = (int64_t)K * D_eff;
+  g = (total + 255) / 256;
+  if (g > sm_count * 8) g = sm_count * 8;
+  zero_member_rows_kernel<<<(unsigned)g, 256, 0, st>>>(C_acc, K, D_eff, ldc, members);
+  ++*nlaunch;
+  return cudaGetLastError();
+}
 
 // delta: int32 [K][W*32] workspace (zeroed here).
 cudaError_t launch_class_update(const uint32_t* Hbits, int64_t n0, int64_t nb, int64_t ldh,

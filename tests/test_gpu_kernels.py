@@ -297,3 +297,53 @@ def test_d_eff_equals_physical_slice_on_gpu(hd, h, D_eff):
     S1 = h.hdc_similarity(Hfull, dev(C), kn)
     S2 = h.hdc_similarity(H1, dev(C[:, :D_eff].copy()), kn)
     assert torch.equal(S1, S2)
+
+
+# ------------------------------------------------------------------------------------ HD-Clustering
+@pytest.mark.parametrize("hv_bits,sim", [(1, "HAMMING"), (8, "COS"), (32, "COS"), (16, "COS")])
+@pytest.mark.parametrize("N,K,D,D_eff", [(300, 5, 2048, 2048), (1000, 26, 3000, 2500), (40, 1, 96, 96)])
+def test_kmeans_epochs_match_oracle(hd, h, hv_bits, sim, N, K, D, D_eff):
+    """HD-Clustering epochs (PAPER.md L197 / L221, reading A16) from seeds taken among the samples,
+    on noisy copies of K prototypes (clusters separated well enough that no cosine is a near-tie):
+    assignments, moved-sample counts and re-bundled accumulators equal the oracle's exactly (the
+    accumulators are small integers; empty clusters keep theirs)."""
+    r = rng(9, N, K, D_eff, hv_bits)
+    proto = r.integers(0, 2, size=(K, D), dtype=np.uint8)
+    yt = r.integers(0, K, size=N)
+    hb = proto[yt] ^ (r.random((N, D)) < 0.2).astype(np.uint8)
+    seeds = r.choice(N, K, replace=False)
+    C = np.zeros((K, D), dtype=np.float32)
+    C[:, :] = 1.0 - 2.0 * hb[seeds]
+    simc = getattr(O, "SIM_" + sim)
+    kn = hd.knobs(D_eff, hv_bits=hv_bits, sim=getattr(hd, "HDC_SIM_" + sim))
+    Cd, Hd = dev(C.copy()), dev_bits(hb)
+    C_or, prev_or = C[:, :D_eff].copy(), None
+    prev_d = None
+    for _ in range(4):
+        C_or, a_or, ch_or = O.kmeans_epoch(hb, C_or, D_eff, hv_bits, simc, prev_or)
+        a_d = torch.empty(N, dtype=torch.int32, device="cuda")
+        nch = torch.zeros(1, dtype=torch.int64, device="cuda")
+        h.hdc_train_epoch(hd.HDC_TRAIN_KMEANS, Hd, prev_d, Cd, kn, pred=a_d, n_wrong=nch)
+        assert np.array_equal(a_d.cpu().numpy(), a_or)
+        assert int(nch.item()) == ch_or
+        assert np.array_equal(Cd.cpu().numpy()[:, :D_eff], C_or)
+        prev_or, prev_d = a_or, a_d
+    assert np.array_equal(Cd.cpu().numpy()[:, D_eff:], C[:, D_eff:])      # columns >= D_eff untouched
+
+
+def test_kmeans_empty_cluster_keeps_accumulator(hd, h):
+    r = rng(10)
+    D = 512
+    hb = r.integers(0, 2, size=(64, D), dtype=np.uint8)
+    hb[:, :256] = hb[0, :256]                                # all samples close to sample 0
+    c0 = 1.0 - 2.0 * hb[0].astype(np.float32)
+    C = np.stack([c0, -c0, c0 * 0.5])                         # cluster 1 = antipode: never chosen; 2 ties with 0
+    kn = hd.knobs(D, hv_bits=1, sim=hd.HDC_SIM_HAMMING)
+    Cd = dev(C.copy())
+    a_d = torch.empty(64, dtype=torch.int32, device="cuda")
+    h.hdc_train_epoch(hd.HDC_TRAIN_KMEANS, dev_bits(hb), None, Cd, kn, pred=a_d)
+    C_or, a_or, _ = O.kmeans_epoch(hb, C, D, 1, O.SIM_HAMMING)
+    assert np.array_equal(a_d.cpu().numpy(), a_or) and (a_or == 0).all()   # ties -> lowest index
+    got = Cd.cpu().numpy()
+    assert np.array_equal(got, C_or)
+    assert np.array_equal(got[1], C[1]) and np.array_equal(got[2], C[2])
