@@ -317,62 +317,64 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
     uint32_t phase = 0;
     int slot = 0;
     int64_t step = 0;
+    // one k-block of this thread's row half: WPP packed words -> C_PER 16-byte chunks of the A tile
+    auto expand = [&](auto part, const uint32_t* qk, uint32_t a_row) {
+      constexpr int PART = decltype(part)::value;
+      constexpr int C0 = PART * C_PER;
+      uint32_t wq[WPP];
+#pragma unroll
+      for (int v = 0; v < WPP; ++v) wq[v] = qk[v * Q_LD];
+#pragma unroll
+      for (int cc = 0; cc < C_PER; ++cc) {  // 16-byte chunk cidx of the row = 4 shared-memory words
+        const int cidx = C0 + cc;
+        uint32_t o[4];
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+          const int iw = 4 * cidx + e;  // word index within the k-block's 32 output words
+          if (INT8) {
+            const uint32_t w = wq[(iw >> 3) - PART * WPP];
+            o[e] = prmt_sign_bytes(w << (7 - (iw & 7))) | 0x01010101u;
+          } else {
+            const uint32_t w = wq[(iw >> 4) - PART * WPP];
+            o[e] = ((w << (15 - (iw & 15))) & 0x80008000u) | 0x3F803F80u;
+          }
+        }
+        const uint32_t dst = a_row + ((((uint32_t)cidx) ^ sw) << 4);
+        asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(dst), "r"(o[0]), "r"(o[1]), "r"(o[2]),
+                     "r"(o[3])
+                     : "memory");
+      }
+    };
     for (int64_t i = 0; i < tiles_per_cta; ++i) {
-      int u = 0;  // position inside the current group
       for (int c = 0; c < nch; ++c, ++step) {
         asm volatile("cp.async.wait_group %0;" ::"n"(Q_SLOTS - 2) : "memory");
         asm volatile("bar.sync 1, %0;" ::"n"(32 * EXW) : "memory");  // tile visible; previous slot free
         if (step + Q_SLOTS - 1 < steps) issue();
         asm volatile("cp.async.commit_group;" ::: "memory");
-        const uint32_t* qs = q_ptr + slot * Q_SLOT_WORDS + t;
-        const int kb0 = c * KPC;
-#pragma unroll
-        for (int j = 0; j < KPC; ++j) {
-          if (kb0 + j < p.num_kb) {
-            if (u == 0) mbar_wait(empty_bar(grp), phase ^ 1u);
-            const uint32_t a_row = base + (grp * G + u) * STAGE_BYTES + (uint32_t)t * KB_BYTES;
-            // the chunk range is a compile-time constant per branch
-            auto expand = [&](auto part) {
-              constexpr int PART = decltype(part)::value;
-              constexpr int C0 = PART * C_PER;
-              uint32_t wq[WPP];
-#pragma unroll
-              for (int v = 0; v < WPP; ++v) wq[v] = qs[(j * WPK + PART * WPP + v) * Q_LD];
-#pragma unroll
-              for (int cc = 0; cc < C_PER; ++cc) {  // 16-byte chunk cidx of the row = 4 shared-memory words
-                const int cidx = C0 + cc;
-                uint32_t o[4];
-#pragma unroll
-                for (int e = 0; e < 4; ++e) {
-                  const int iw = 4 * cidx + e;  // word index within the k-block's 32 output words
-                  if (INT8) {
-                    const uint32_t w = wq[(iw >> 3) - PART * WPP];
-                    o[e] = prmt_sign_bytes(w << (7 - (iw & 7))) | 0x01010101u;
-                  } else {
-                    const uint32_t w = wq[(iw >> 4) - PART * WPP];
-                    o[e] = ((w << (15 - (iw & 15))) & 0x80008000u) | 0x3F803F80u;
-                  }
-                }
-                const uint32_t dst = a_row + ((((uint32_t)cidx) ^ sw) << 4);
-                asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(dst), "r"(o[0]), "r"(o[1]),
-                             "r"(o[2]), "r"(o[3])
-                             : "memory");
-              }
-            };
-            if (part_id == 0) expand(std::integral_constant<int, 0>{});
-            else expand(std::integral_constant<int, 1>{});
-            // the group is published (one proxy fence, one arrival per warp) when its last k-block is written
-            if (++u == G || kb0 + j == p.num_kb - 1) {
-              fence_proxy_async_smem();
-              __syncwarp();
-              if (lane == 0) mbar_arrive(full_bar(grp));
-              u = 0;
-              if (++grp == NG) {
-                grp = 0;
-                phase ^= 1u;
-              }
-            }
+        // this thread's words of the chunk's first k-block (groups never straddle a chunk: G | KPC)
+        const uint32_t* qk = q_ptr + slot * Q_SLOT_WORDS + t + part_id * (WPP * Q_LD);
+        int left = p.num_kb - c * KPC;
+        if (left > KPC) left = KPC;
+        while (left > 0) {
+          const int n = left < G ? left : G;
+          mbar_wait(empty_bar(grp), phase ^ 1u);
+          uint32_t a_row = base + (uint32_t)(grp * G) * STAGE_BYTES + (uint32_t)t * KB_BYTES;
+#pragma unroll 1
+          for (int u = 0; u < n; ++u) {
+            if (part_id == 0) expand(std::integral_constant<int, 0>{}, qk, a_row);
+            else expand(std::integral_constant<int, 1>{}, qk, a_row);
+            qk += WPK * Q_LD;
+            a_row += STAGE_BYTES;
           }
+          // the group is published with one proxy fence and one arrival per warp
+          fence_proxy_async_smem();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(full_bar(grp));
+          if (++grp == NG) {
+            grp = 0;
+            phase ^= 1u;
+          }
+          left -= n;
         }
         if (++slot == Q_SLOTS) slot = 0;
       }
