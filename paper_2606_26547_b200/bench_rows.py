@@ -14,6 +14,7 @@ import argparse
 import json
 import os
 import sys
+import time
 
 import torch
 
@@ -165,6 +166,44 @@ def row_train(h, peaks, reps, N=6238, K=26, D=10000, hv_bits=32, sim_name="cos")
             "call_ms": call_ms, "samples_per_s": N / (call_ms * 1e-3)}
 
 
+def row_c5_stream(h, peaks, reps, hv_bits, sim_name, N=1 << 20, B=65536, F=1024, D=16384, K=1000):
+    """BASELINE.json configs[4]: N = 2^20 bf16 queries streamed in 64K-query device-resident batches
+    through hdc_encode_rp (bf16) + hdc_classify against K = 1000 classes (bf16 cosine or packed 1-bit
+    Hamming).  Four distinct input batches (537 MB > L2) are cycled."""
+    sim = {"cos": hd.HDC_SIM_COS, "hamming": hd.HDC_SIM_HAMMING}[sim_name]
+    nb = N // B
+    Xs = [torch.randn((B, F), device="cuda", generator=_gen(20 + i)).to(torch.bfloat16) for i in range(4)]
+    P = torch.randn((D, F), device="cuda", generator=_gen(2)).to(torch.bfloat16)
+    C = _class_acc(K, D, 4)
+    kn_e = hd.knobs(D, precision=hd.HDC_BF16)
+    kn = hd.knobs(D, hv_bits=hv_bits, sim=sim)
+    H = torch.empty((B, (D + 31) // 32), dtype=torch.int32, device="cuda")
+    lab = torch.empty(N, dtype=torch.int32, device="cuda")
+
+    def fn():
+        for i in range(nb):
+            h.hdc_encode_rp(Xs[i & 3], P, kn_e, Hbits=H)
+            h.hdc_classify(H, C, kn, labels=lab[i * B:(i + 1) * B])
+
+    call_ms = _time(fn, max(1, reps // 5), warm=1)
+    flops = 2.0 * N * D * (F + (K if hv_bits != 1 else 0))
+    out = {"what": f"C5 stream: N={N} in {nb} batches of {B}, F={F} bf16, D={D}, K={K}, classes hv_bits={hv_bits} "
+                   f"sim={sim_name}: hdc_encode_rp + hdc_classify per batch",
+           "call_ms": call_ms, "queries_per_s": N / (call_ms * 1e-3)}
+    if hv_bits != 1:
+        ach = flops / (call_ms * 1e-3) / 1e12
+        out["roofline"] = {"bound": "tensor", "achieved": ach, "peak": peaks["bf16_tflops_sustained"],
+                           "unit": "TFLOP/s", "frac": ach / peaks["bf16_tflops_sustained"],
+                           "peak_source": "bf16_tflops_sustained (measured); 2*D*(F+K) flop per query"}
+    else:
+        t_ideal = (2.0 * N * D * F / (peaks["bf16_tflops_sustained"] * 1e12)
+                   + 2.0 * N * D * 1008 / (2.0 * peaks["bf16_tflops_sustained"] * 1e12))
+        out["roofline"] = {"bound": "tensor", "achieved": N / (call_ms * 1e-3), "peak": N / t_ideal,
+                           "unit": "queries/s", "frac": t_ideal / (call_ms * 1e-3),
+                           "peak_source": "bf16 encode at bf16_tflops_sustained + +-1 int8 similarity at 2x that"}
+    return out
+
+
 def row_kmeans(h, peaks, reps, N=7797, K=26, D=10000, hv_bits=32, sim_name="cos"):
     """HD-Clustering epoch (assign + re-bundle) on noisy copies of K prototypes, ISOLET-sized."""
     sim = {"cos": hd.HDC_SIM_COS, "hamming": hd.HDC_SIM_HAMMING}[sim_name]
@@ -193,6 +232,8 @@ ROWS = {
     "c5_encode_bf16": lambda h, p, r: row_encode(h, p, r, 65536, 1024, 16384, "bf16", x_bf16=True),
     "c5_classify_bf16": lambda h, p, r: row_classify(h, p, r, 65536, 1000, 16384, 16, "cos"),
     "c5_classify_1bit": lambda h, p, r: row_classify(h, p, r, 65536, 1000, 16384, 1, "hamming"),
+    "c5_stream_bf16": lambda h, p, r: row_c5_stream(h, p, r, 16, "cos"),
+    "c5_stream_1bit": lambda h, p, r: row_c5_stream(h, p, r, 1, "hamming"),
     "c2_train_epoch": lambda h, p, r: row_train(h, p, r),
     "c2_kmeans_epoch": lambda h, p, r: row_kmeans(h, p, r),
 }
@@ -203,6 +244,7 @@ def run(h, peaks, reps=5, only=None):
     for name, fn in ROWS.items():
         if only and name != only:
             continue
+        time.sleep(1.0)   # let the part cool between rows: each row is a burst measurement of its own
         out[name] = fn(h, peaks, reps)
         torch.cuda.empty_cache()
     return out
