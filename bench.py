@@ -30,8 +30,8 @@ if ROOT not in sys.path:
 METRIC = "hdc_inference_queries_per_sec_D10000"
 UNIT = "queries/s"
 NQ = 131072            # queries per step (test set tiled)
-NCU_TRAFFIC_BYTES = 1084.9e6
-NCU_TRAFFIC_SOURCE = "profiles/r1_tcgen05_path.md (gemm_tc_kernel, fp32-precision encode, 131072 x 617 x 10000)"
+NCU_TRAFFIC_BYTES = 804.4e6
+NCU_TRAFFIC_SOURCE = "profiles/r1_final_kernels.md (gemm_tc_kernel, fp32-precision encode, 131072 x 617 x 10000)"
 SM_COUNT = 148
 FP32_LANES = 128       # FFMA lanes per SM per clock
 
