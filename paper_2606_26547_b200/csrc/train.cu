@@ -7,8 +7,8 @@
 //
 // with v = 1 - 2*bit.  Delta is an exact int32 segmented reduction per class: a CTA owns (class k,
 // 128 word-columns, a segment of the samples); a thread owns one word-column and 32 signed counters
-// in registers, walks its sample segment (label reads are warp-uniform broadcasts, word reads are
-// coalesced) and finally adds its 32 partial sums into Delta with integer atomics -- integer
+// in registers, walks the samples of its segment that touch class k (compacted through shared memory;
+// word reads are coalesced) and finally adds its 32 partial sums into Delta with integer atomics -- integer
 // addition commutes, so the result is deterministic; there are no floating-point atomics.
 #include "common.cuh"
 
@@ -17,10 +17,18 @@ namespace {
 
 constexpr int WT = 128;  // word-columns per CTA
 
+constexpr int LCH = 1024;  // samples scanned per compaction round
+
 __global__ void __launch_bounds__(WT)
 class_delta_kernel(const uint32_t* __restrict__ Hbits, int64_t n0, int64_t nb, int64_t ldh,
                    const int32_t* __restrict__ y, const int32_t* __restrict__ pred, int W,
                    int32_t* __restrict__ delta, int64_t ldd, int64_t seg_len) {
+  // Samples that touch class k are first compacted into shared memory (coalesced label reads, one
+  // atomic per hit), then only those are walked: a CTA no longer pays two dependent label loads
+  // for each of the (K-2)/K samples that do not concern its class.  The list order is arbitrary;
+  // the sums are integers, so the result does not depend on it.
+  __shared__ int s_list[LCH];  // (sample offset from c0) * 2 + (sign < 0)
+  __shared__ int s_cnt;
   const int k = blockIdx.y;
   const int w = blockIdx.x * WT + threadIdx.x;
   const int64_t s0 = n0 + (int64_t)blockIdx.z * seg_len;
@@ -30,20 +38,34 @@ class_delta_kernel(const uint32_t* __restrict__ Hbits, int64_t n0, int64_t nb, i
 #pragma unroll
   for (int b = 0; b < 32; ++b) cnt[b] = 0;
   int m = 0;  // signed number of contributing samples
-  for (int64_t n = s0; n < s1; ++n) {
-    const int yn = __ldg(y + n);
-    int s;
-    if (pred) {
-      const int pn = __ldg(pred + n);
-      s = (pn != yn) ? ((yn == k) - (pn == k)) : 0;
-    } else {
-      s = (yn == k);
+  for (int64_t c0 = s0; c0 < s1; c0 += LCH) {
+    const int len = (int)(s1 - c0 < LCH ? s1 - c0 : LCH);
+    if (threadIdx.x == 0) s_cnt = 0;
+    __syncthreads();
+    for (int i = threadIdx.x; i < len; i += WT) {
+      const int yn = __ldg(y + c0 + i);
+      int sg;
+      if (pred) {
+        const int pn = __ldg(pred + c0 + i);
+        sg = (pn != yn) ? ((yn == k) - (pn == k)) : 0;
+      } else {
+        sg = (yn == k);
+      }
+      if (sg != 0) s_list[atomicAdd(&s_cnt, 1)] = i * 2 + (sg < 0);
     }
-    if (s == 0) continue;  // uniform across the CTA
-    const uint32_t word = (w < W) ? __ldg(Hbits + n * ldh + w) : 0u;
-    m += s;
+    __syncthreads();
+    const int n_hit = s_cnt;
+    const uint32_t* hcol = Hbits + c0 * ldh + (w < W ? w : 0);
+#pragma unroll 4
+    for (int j = 0; j < n_hit; ++j) {
+      const int e = s_list[j];
+      const int sg = 1 - 2 * (e & 1);
+      const uint32_t word = (w < W) ? __ldg(hcol + (int64_t)(e >> 1) * ldh) : 0u;
+      m += sg;
 #pragma unroll
-    for (int b = 0; b < 32; ++b) cnt[b] += s * (int)((word >> b) & 1u);
+      for (int b = 0; b < 32; ++b) cnt[b] += sg * (int)((word >> b) & 1u);
+    }
+    __syncthreads();  // the list is rewritten in the next round
   }
   if (w < W) {
     int32_t* out = delta + (int64_t)k * ldd + (int64_t)w * 32;
