@@ -168,9 +168,10 @@ __global__ void sign_bits_kernel(const float* __restrict__ C, int K, int D_eff, 
 // over the operand as the contraction loads it.  One block per class, fixed reduction order.
 __global__ void col_scale_kernel(Operand C, int K, int D_eff, int cos, double* __restrict__ colscale) {
   const int k = blockIdx.x;
-  __shared__ double part[8];
+  __shared__ double part[32];
   double s = 0.0;
   if (cos) {
+#pragma unroll 4
     for (int d = threadIdx.x; d < D_eff; d += blockDim.x) {
       double v;
       const int64_t idx = (int64_t)k * C.ld + d;
@@ -269,7 +270,7 @@ cudaError_t launch_sign_bits(const float* C, int K, int D_eff, int64_t ldc, uint
 
 cudaError_t launch_col_scale(const Operand& C, int K, int D_eff, int cos, double* colscale,
                              cudaStream_t st, int64_t* nlaunch) {
-  col_scale_kernel<<<K, 256, 0, st>>>(C, K, D_eff, cos, colscale);
+  col_scale_kernel<<<K, 1024, 0, st>>>(C, K, D_eff, cos, colscale);
   ++*nlaunch;
   return cudaGetLastError();
 }
