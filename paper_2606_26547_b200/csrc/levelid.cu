@@ -46,7 +46,7 @@ struct LevelIdParams {
   int64_t n_batches;
   int Fpad;     // staged level row stride (bytes), multiple of 16
   int tables_in_smem;
-  uint32_t mul_hi16;  // 65536 (passed at run time so that mad.hi is not strength-reduced to a shift)
+  uint32_t mul_hi16;  // 0x0101: the dp2a selectors, passed at run time so that they are not strength-reduced
 };
 
 // NP = number of counter planes (p + 1 with 2^p > F); S = samples per warp iteration
@@ -172,11 +172,12 @@ __global__ void __launch_bounds__(NTHREADS, 1) levelid_kernel(const LevelIdParam
 //   * levels are staged as 16-bit table byte-offsets (level << 7), two per word, read by the warp
 //     as broadcast 16-byte loads; the LV address is one LOP3 (low half) or one IMAD.HI (high half,
 //     FMA pipe) -- no 64-bit address arithmetic, no predication in the loop;
-//   * features go in blocks of 32: two 16-input CSA trees (30 LOP3 each) whose weight-16 carries
-//     meet in one more CSA, so the ripple into the upper planes runs once per 32 features;
+//   * features go in blocks of 64 (then 32, 16, 1): four 16-input CSA trees (30 LOP3 each) whose
+//     weight-16 carries meet in three more CSAs, so the ripple into the upper planes runs once per
+//     64 features;
 //   * the next batch's level bytes are prefetched into registers before the block loop, so the
 //     only exposed staging cost is the conversion between two barriers.
-// ALU ops per (feature, sample, word): 1 bind XOR + 0.5 address + 1.875 + 0.44 counter = 3.8.
+// ALU ops per (feature, sample, word): 1 bind XOR + 1.875 + 0.25 counter = 3.1 (addresses are dp2a).
 constexpr int FS = 4;                   // samples per warp
 constexpr int FWARPS = 12;              // warps per CTA (3 per scheduler; 166 registers x 384 threads fit)
 constexpr int FTHREADS = FWARPS * 32;
@@ -196,7 +197,7 @@ __global__ void __launch_bounds__(FTHREADS, 1) levelid_fast_kernel(const LevelId
   constexpr int P = NP - 1;
   const uint32_t init = (1u << P) - (uint32_t)(p.F / 2 + 1);
   const uint32_t lane4 = (uint32_t)lane * 4u;
-  const uint32_t k65536 = p.mul_hi16;                           // 65536, opaque to the compiler
+  const uint32_t sel_lo = p.mul_hi16 & 0x0001u, sel_hi = p.mul_hi16 & 0x0100u;  // dp2a byte selectors (run-time: not folded)
   const int F4 = p.F >> 2;                                     // level words per sample row
 
   const int64_t units = (int64_t)p.n_slices * p.n_batches;
@@ -271,9 +272,10 @@ __global__ void __launch_bounds__(FTHREADS, 1) levelid_fast_kernel(const LevelId
       const uint32_t o[8] = {oa.x, oa.y, oa.z, oa.w, ob.x, ob.y, ob.z, ob.w};
 #pragma unroll
       for (int i = 0; i < 8; ++i) {
-        const uint32_t a_lo = (o[i] & 0xffffu) | lane4;
-        uint32_t a_hi;  // (o >> 16) + lane4 as a multiply-add: FMA pipe, leaves the ALU pipe to the LOP3s
-        asm("mad.hi.u32 %0, %1, %2, %3;" : "=r"(a_hi) : "r"(o[i]), "r"(k65536), "r"(lane4));
+        // byte offset of the level row + lane word: 16-bit half of o times 1 plus lane4 as one dp2a
+        // (integer dot-product pipe, not the ALU pipe that the LOP3s saturate)
+        const uint32_t a_lo = __dp2a_lo(o[i], sel_lo, lane4);
+        const uint32_t a_hi = __dp2a_lo(o[i], sel_hi, lane4);
         x[2 * i] = idw[2 * i] ^ *reinterpret_cast<const uint32_t*>(lvb + a_lo);
         x[2 * i + 1] = idw[2 * i + 1] ^ *reinterpret_cast<const uint32_t*>(lvb + a_hi);
       }
@@ -310,6 +312,33 @@ __global__ void __launch_bounds__(FTHREADS, 1) levelid_fast_kernel(const LevelId
     };
 
     int f = 0;
+    // 64 features: four 16-input trees, their weight-16 carries folded by three more CSAs, so the
+    // ripple into the upper planes runs once per 64 features
+#pragma unroll 1
+    for (; f + 64 <= p.F; f += 64) {
+      uint32_t sxs[FS][3];
+#pragma unroll
+      for (int q4 = 0; q4 < 4; ++q4) {
+        uint32_t idw[16];
+#pragma unroll
+        for (int i = 0; i < 16; ++i) idw[i] = idp[(f + 16 * q4 + i) * SW];
+#pragma unroll
+        for (int j = 0; j < FS; ++j) {
+          uint32_t x[16];
+          bind16(f + 16 * q4, j, idw, x);
+          const uint32_t sx = tree16(pl[j], x);
+          if (q4 < 3) {
+            sxs[j][q4] = sx;
+          } else {
+            uint32_t ca, cb, c64;
+            HDC_CSA(ca, pl[j][4], pl[j][4], sxs[j][0], sxs[j][1]);
+            HDC_CSA(cb, pl[j][4], pl[j][4], sxs[j][2], sx);
+            HDC_CSA(c64, pl[j][5], pl[j][5], ca, cb);
+            ripple(pl[j], c64, 6);
+          }
+        }
+      }
+    }
 #pragma unroll 1
     for (; f + 32 <= p.F; f += 32) {
       uint32_t sxa[FS];
@@ -404,7 +433,7 @@ cudaError_t launch_levelid(const uint8_t* levels, int64_t N, int F, int64_t ldl,
       p.n_batches = (N + FSB - 1) / FSB;
       p.Fpad = (int)fp2;
       p.tables_in_smem = 1;
-      p.mul_hi16 = 65536u;
+      p.mul_hi16 = 0x0101u;
       const int64_t units = (int64_t)p.n_slices * p.n_batches;
       const int grid = (int)(units < sm_count ? units : sm_count);
       cudaError_t e = cudaFuncSetAttribute(levelid_fast_kernel<11>, cudaFuncAttributeMaxDynamicSharedMemorySize,
