@@ -189,8 +189,28 @@ def cosine(hbits: np.ndarray, cop: np.ndarray, D_eff: int) -> np.ndarray:
     return out
 
 
-def similarity(hbits: np.ndarray, C_acc: np.ndarray, D_eff: int, sim: int, hv_bits: int):
-    """Scores of every query against every class at the given knobs (S5 + S6)."""
+def perforated_index(D_eff: int, begin: int = 0, stride: int = 1) -> np.ndarray:
+    """Reduction perforation (the reduction-axis loop "skip[s] iterations at regular
+    intervals, defined by a specified stride", annotation parameters "starting offset, ending offset,
+    and stride"; L76-L77 red_perf(v, 0, 0.5, 1); L130 {"stride": 8, "extent": 0.84}): the dimensions
+    a similarity reduction visits are d = begin, begin + stride, ... < D_eff (end offset = D_eff)."""
+    if stride < 1 or not 0 <= begin < D_eff:
+        raise ValueError("bad perforation")
+    return np.arange(begin, D_eff, stride)
+
+
+def similarity(hbits: np.ndarray, C_acc: np.ndarray, D_eff: int, sim: int, hv_bits: int,
+               begin: int = 0, stride: int = 1):
+    """Scores of every query against every class at the given knobs (S5 + S6).
+    Perforation (reading A17): the result equals that of physically gathering the visited
+    dimensions of both operands and running with D = their number -- nothing is rescaled
+    (L155: "for similarity and dissimilarity computations, the resultant values are used as-is"),
+    the cosine is the cosine of the sub-vectors, the per-tensor int8 scale is taken over them."""
+    if begin != 0 or stride != 1:
+        idx = perforated_index(D_eff, begin, stride)
+        hb = np.asarray(hbits, dtype=np.uint8)[:, idx]
+        Cg = np.asarray(C_acc, dtype=np.float32)[:, idx]
+        return similarity(hb, Cg, len(idx), sim, hv_bits)
     cop = class_operand(C_acc, D_eff, hv_bits)
     if sim == SIM_HAMMING:
         if hv_bits != 1:
@@ -239,7 +259,7 @@ def bundle(hbits: np.ndarray, y: np.ndarray, K: int, D_eff: int, C_acc: np.ndarr
 
 # ------------------------------------------------------------------------------------- S9
 def train_epoch(hbits: np.ndarray, y: np.ndarray, C_acc: np.ndarray, D_eff: int, hv_bits: int,
-                sim: int, lr: float, batch: int = 0):
+                sim: int, lr: float, batch: int = 0, begin: int = 0, stride: int = 1):
     """One retraining epoch (PAPER.md L181 TRAIN_ITERATIONS "number of retraining epochs";
     the per-sample rule is not in the paper -- reading A9 / S9, "perceptron-style" per
     BASELINE north_star).  Samples in index order, no shuffle; per mini-batch of B samples:
@@ -259,7 +279,7 @@ def train_epoch(hbits: np.ndarray, y: np.ndarray, C_acc: np.ndarray, D_eff: int,
     wrong = 0
     for b0 in range(0, N, B):
         sl = slice(b0, min(N, b0 + B))
-        S = similarity(hb[sl], C, D_eff, sim, hv_bits)
+        S = similarity(hb[sl], C, D_eff, sim, hv_bits, begin, stride)   # only the similarity is perforated
         yh, _, _ = classify(S, sim)
         pred[sl] = yh
         v = bipolar(hb[sl])
@@ -287,7 +307,8 @@ def train(hbits, y, K, D_eff, hv_bits, sim, epochs, lr, batch=0):
 
 
 # ------------------------------------------------------------------------------------- S11
-def kmeans_epoch(hbits: np.ndarray, C_acc: np.ndarray, D_eff: int, hv_bits: int, sim: int, prev=None):
+def kmeans_epoch(hbits: np.ndarray, C_acc: np.ndarray, D_eff: int, hv_bits: int, sim: int, prev=None,
+                 begin: int = 0, stride: int = 1):
     """One iteration of HD-Clustering ("HD-Clustering implements K-Means clustering
     using HDC", L221: cosine or Hamming similarity, TRAIN_ITERATIONS epochs).  The paper gives no
     pseudo-code; reading A16 is Lloyd's iteration with the path's own primitives:
@@ -301,7 +322,7 @@ def kmeans_epoch(hbits: np.ndarray, C_acc: np.ndarray, D_eff: int, hv_bits: int,
     hb = np.asarray(hbits, dtype=np.uint8)[:, :D_eff]
     C = np.array(C_acc, dtype=np.float32)[:, :D_eff].copy()
     K = C.shape[0]
-    S = similarity(hb, C, D_eff, sim, hv_bits)
+    S = similarity(hb, C, D_eff, sim, hv_bits, begin, stride)
     a, _, _ = classify(S, sim)
     a = a.astype(np.int32)
     v = bipolar(hb).astype(np.int64)

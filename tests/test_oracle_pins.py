@@ -542,3 +542,56 @@ def test_kmeans_recovers_well_separated_clusters():
         assert np.array_equal(a, yt)
         C2, a2, ch = o.kmeans_epoch(hb, C, D, bits, sim, prev=a)
         assert ch == 0 and np.array_equal(C2, C)
+
+
+# ------------------------------------------------------------------------------------- A17 perforation
+@pytest.mark.parametrize("begin,stride,D_eff", [(0, 1, 40), (0, 8, 40), (3, 8, 37), (5, 2, 33), (39, 7, 40), (1, 3, 32)])
+def test_perforated_similarity_brute_force(begin, stride, D_eff):
+    """Reduction perforation (PAPER.md L155, L130): loops over the visited dimensions written out by hand;
+    dot = n_visited - 2 * Hamming on them; (0, 1) is the unperforated similarity."""
+    r = np.random.default_rng(begin * 100 + stride)
+    N, K, D = 6, 4, 40
+    hb = r.integers(0, 2, size=(N, D), dtype=np.uint8)
+    C = r.integers(-9, 10, size=(K, D)).astype(np.float32)
+    C[C == 0] = 2.0
+    vis = [d for d in range(D_eff) if d >= begin and (d - begin) % stride == 0]
+    assert list(o.perforated_index(D_eff, begin, stride)) == vis
+    H = o.similarity(hb, C, D_eff, o.SIM_HAMMING, 1, begin, stride)
+    Dt = o.similarity(hb, C, D_eff, o.SIM_DOT, 1, begin, stride)
+    Dd = o.similarity(hb, C, D_eff, o.SIM_DOT, 32, begin, stride)
+    Cs = o.similarity(hb, C, D_eff, o.SIM_COS, 32, begin, stride)
+    for n in range(N):
+        for k in range(K):
+            ham = sum(int(hb[n, d]) != int(C[k, d] < 0) for d in vis)
+            dt = sum((1 - 2 * int(hb[n, d])) * float(C[k, d]) for d in vis)
+            nrm = math.sqrt(sum(float(C[k, d]) ** 2 for d in vis))
+            assert H[n, k] == ham
+            assert Dt[n, k] == len(vis) - 2 * ham
+            assert Dd[n, k] == dt
+            assert abs(Cs[n, k] - dt / (math.sqrt(len(vis)) * nrm)) < 1e-12
+    if (begin, stride) == (0, 1):
+        assert np.array_equal(H, o.similarity(hb, C, D_eff, o.SIM_HAMMING, 1))
+
+
+def test_perforated_int8_scale_is_taken_over_the_visited_dimensions():
+    hb = np.zeros((1, 8), dtype=np.uint8)
+    C = np.array([[1000.0, 2.0, 3.0, 127.0, 5.0, 6.0, 7.0, 8.0]], dtype=np.float32)
+    # visiting 1, 3, 5, 7: max |c| = 127 -> scale 1 -> the integers themselves
+    S = o.similarity(hb, C, 8, o.SIM_DOT, 8, begin=1, stride=2)
+    assert S[0, 0] == 2 + 127 + 6 + 8
+    # unperforated: 1000 sets the scale and the small entries collapse
+    assert o.similarity(hb, C, 8, o.SIM_DOT, 8)[0, 0] != S[0, 0]
+
+
+def test_perforated_training_updates_every_dimension():
+    """Only the similarity reduction is perforated (L155); the class update still touches d < D_eff."""
+    w = wl.c1_tiny(D=256)
+    hb, _, _ = o.encode_rp(w["Xtr"], w["P"], 256, o.F32)
+    y = w["ytr"].copy()
+    y[::3] = (y[::3] + 1) % w["K"]
+    C0 = o.bundle(hb, y, w["K"], 256)
+    C1, wrong, pred = o.train_epoch(hb, y, C0, 256, 1, o.SIM_HAMMING, 1.0, 0, begin=2, stride=4)
+    lab, _, _ = o.classify(o.similarity(hb, C0, 256, o.SIM_HAMMING, 1, 2, 4), o.SIM_HAMMING)
+    assert np.array_equal(pred, lab) and wrong == int((lab != y).sum()) and wrong > 0
+    touched = np.nonzero((C1 != C0).any(axis=0))[0]
+    assert (touched % 4 != 2).any()                      # columns outside the visited set changed too
