@@ -86,13 +86,25 @@ enum {
  *             32 fp32 | 16 bf16 (RNE of C_acc) | 8 int8 (per-tensor symmetric over k<K, d<D_eff)
  *             | 1 sign bit [C_acc < 0].  Query hypervectors are always bipolar (packed bits).
  *  sim        HDC_SIM_*; HDC_SIM_HAMMING requires hv_bits == 1.
- *  flags      HDC_FLAG_*.                                                                        */
+ *  flags      HDC_FLAG_*.
+ *  perf_begin, perf_stride   reduction perforation of the SIMILARITY (L155 "skip iterations at
+ *             regular intervals, defined by a specified stride"; parameters starting offset, ending
+ *             offset, stride: L76-L77, L130): the reductions over d in hdc_similarity / hdc_classify
+ *             and in the prediction step of hdc_train_epoch visit d = perf_begin + j*perf_stride
+ *             < D_eff only (D_eff is the ending offset).  Results equal those obtained by gathering
+ *             the visited dimensions of both operands; nothing is rescaled (L155); the int8 class
+ *             scale and the cosine norms are taken over the visited dimensions.  0 <= perf_begin
+ *             < D_eff; perf_stride 0 or 1 = every dimension.  Encoders and class updates are not
+ *             perforated (L157, L187).  Not available with HDC_FLAG_SIMT for DOT / COS
+ *             (HDC_ERR_UNSUPPORTED).                                                             */
 typedef struct {
   int32_t D_eff;
   int32_t precision;
   int32_t hv_bits;
   int32_t sim;
   int32_t flags;
+  int32_t perf_begin;
+  int32_t perf_stride;
 } hdc_knobs_t;
 
 /* ---- handle ------------------------------------------------------------------------------ */

@@ -33,7 +33,8 @@ EXPORTS = ("hdc_create", "hdc_destroy", "hdc_last_error", "hdc_version", "hdc_la
 
 class hdc_knobs_t(C.Structure):
     _fields_ = [("D_eff", C.c_int32), ("precision", C.c_int32), ("hv_bits", C.c_int32),
-                ("sim", C.c_int32), ("flags", C.c_int32)]
+                ("sim", C.c_int32), ("flags", C.c_int32), ("perf_begin", C.c_int32),
+                ("perf_stride", C.c_int32)]
 
 
 class HdcError(RuntimeError):
@@ -93,8 +94,9 @@ def lib() -> C.CDLL:
 
 
 def knobs(D_eff: int, precision: int = HDC_F32, hv_bits: int = 32, sim: int = HDC_SIM_COS,
-          flags: int = 0) -> hdc_knobs_t:
-    return hdc_knobs_t(int(D_eff), int(precision), int(hv_bits), int(sim), int(flags))
+          flags: int = 0, perf_begin: int = 0, perf_stride: int = 1) -> hdc_knobs_t:
+    return hdc_knobs_t(int(D_eff), int(precision), int(hv_bits), int(sim), int(flags), int(perf_begin),
+                       int(perf_stride))
 
 
 _DT = {torch.float32: HDC_F32, torch.bfloat16: HDC_BF16, torch.int8: HDC_I8, torch.uint8: HDC_U8,

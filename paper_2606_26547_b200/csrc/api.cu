@@ -85,8 +85,11 @@ int check_sim_knobs(hdc_ctx* h, const hdc_knobs_t* k) {
     return fail(h, HDC_ERR_INVALID_ARG, "bad sim");
   if (k->sim == HDC_SIM_HAMMING && k->hv_bits != 1)
     return fail(h, HDC_ERR_INVALID_ARG, "HDC_SIM_HAMMING requires hv_bits == 1");
+  if (k->perf_stride < 0 || k->perf_begin < 0 || k->perf_begin >= k->D_eff)
+    return fail(h, HDC_ERR_INVALID_ARG, "perforation: need perf_stride >= 0 and 0 <= perf_begin < D_eff");
   return HDC_OK;
 }
+Perf perf_of(const hdc_knobs_t* k) { return Perf{k->perf_begin, k->perf_stride <= 1 ? 1 : k->perf_stride}; }
 
 // ------------------------------------------------------------------------------------- encode
 // Reduction-segment schedule of the fp32-precision contraction over 3-way bf16 splits: segment s
@@ -249,6 +252,8 @@ int do_similarity(hdc_ctx* h, const uint32_t* Hbits, int64_t N, int64_t ldh, con
                   float* best, float* second, Bump& b, size_t ws_bytes, cudaStream_t st) {
   const int D_eff = k->D_eff;
   const int W = words_of(D_eff);
+  const Perf pf = perf_of(k);
+  const int n_vis = perf_count(pf, D_eff);  // dimensions the reduction visits (= D_eff unless perforated)
   cudaError_t ce;
   // tensor-core path from packed queries: DOT / COS at any K; Hamming once K is large enough that
   // the popcount pipe would bound it (dist = (D_eff - dot)/2 is exact in int32)
@@ -264,18 +269,18 @@ int do_similarity(hdc_ctx* h, const uint32_t* Hbits, int64_t N, int64_t ldh, con
         const int64_t ldq = round_up(D_eff, 16);
         int8_t* Cq = b.take<int8_t>((size_t)K * ldq);
         if (b.off > ws_bytes) return fail(h, HDC_ERR_WORKSPACE, "similarity: workspace too small");
-        ce = launch_quantize_tensor_i8(C_acc, K, D_eff, ldc, Cq, ldq, amax, st, &h->launches);
+        ce = launch_quantize_tensor_i8(C_acc, K, D_eff, ldc, pf, Cq, ldq, amax, st, &h->launches);
         if (ce != cudaSuccess) return cuda_fail(h, ce, "quantize C");
-        ce = launch_col_scale(Operand{Cq, ldq, OPK_I8}, K, D_eff, 1, colscale, st, &h->launches);
+        ce = launch_col_scale(Operand{Cq, ldq, OPK_I8}, K, D_eff, 1, pf, colscale, st, &h->launches);
       } else {
         const int ck = k->hv_bits == 32 ? OPK_F32 : (k->hv_bits == 16 ? OPK_F32_RBF16 : OPK_BITS);
-        ce = launch_col_scale(Operand{C_acc, ldc, ck}, K, D_eff, 1, colscale, st, &h->launches);
+        ce = launch_col_scale(Operand{C_acc, ldc, ck}, K, D_eff, 1, pf, colscale, st, &h->launches);
       }
       if (ce != cudaSuccess) return cuda_fail(h, ce, "col_scale");
     }
     Epilogue e{};
     e.colscale = colscale;
-    e.ham_D = k->sim == HDC_SIM_HAMMING ? D_eff : 0;
+    e.ham_D = k->sim == HDC_SIM_HAMMING ? n_vis : 0;
     if (labels) {
       e.kind = EPI_ARGMAX;
       e.labels = labels;
@@ -289,7 +294,7 @@ int do_similarity(hdc_ctx* h, const uint32_t* Hbits, int64_t N, int64_t ldh, con
     }
     {
       Timed tm(h, HDC_K_SIM, st);
-      ce = launch_sim_tc(h->tc, Hbits, N, ldh, C_acc, K, ldc, D_eff, k->hv_bits, cop, amax, e, h->sm_count, st,
+      ce = launch_sim_tc(h->tc, Hbits, N, ldh, C_acc, K, ldc, D_eff, k->hv_bits, cop, amax, e, pf, h->sm_count, st,
                          &h->launches);
     }
     if (ce == cudaSuccess) return HDC_OK;
@@ -300,14 +305,22 @@ int do_similarity(hdc_ctx* h, const uint32_t* Hbits, int64_t N, int64_t ldh, con
     if (b.off > ws_bytes) return fail(h, HDC_ERR_WORKSPACE, "similarity: workspace too small");
     ce = launch_sign_bits(C_acc, K, D_eff, ldc, cbits, W, st, &h->launches);
     if (ce != cudaSuccess) return cuda_fail(h, ce, "sign_bits");
+    uint32_t* pmask = nullptr;
+    if (perf_on(pf)) {
+      pmask = b.take<uint32_t>((size_t)W);
+      if (b.off > ws_bytes) return fail(h, HDC_ERR_WORKSPACE, "similarity: workspace too small");
+      ce = launch_perf_mask(pmask, W, D_eff, pf, st, &h->launches);
+      if (ce != cudaSuccess) return cuda_fail(h, ce, "perforation mask");
+    }
     {
       Timed tm(h, HDC_K_SIM, st);
-      ce = launch_hamming(Hbits, N, ldh, cbits, K, W, D_eff, (int32_t*)S, lds, labels, best, second,
+      ce = launch_hamming(Hbits, N, ldh, cbits, K, W, D_eff, pmask, (int32_t*)S, lds, labels, best, second,
                           h->sm_count, h->smem_optin, st, &h->launches);
     }
     return ce == cudaSuccess ? HDC_OK : cuda_fail(h, ce, "hamming");
   }
-  // DOT / COS: contraction of +-1 queries with the class operand at hv_bits
+  // DOT / COS: contraction of +-1 queries with the class operand at hv_bits (CUDA-core kernels)
+  if (perf_on(pf)) return fail(h, HDC_ERR_UNSUPPORTED, "perforated DOT / COS needs the tensor-core path");
   Operand B{};
   bool int_acc = false;
   double* colscale = nullptr;
@@ -321,7 +334,7 @@ int do_similarity(hdc_ctx* h, const uint32_t* Hbits, int64_t N, int64_t ldh, con
     int8_t* Cq = b.take<int8_t>((size_t)K * ldq);
     float* amax = b.take<float>(1);
     if (b.off > ws_bytes) return fail(h, HDC_ERR_WORKSPACE, "similarity: workspace too small");
-    ce = launch_quantize_tensor_i8(C_acc, K, D_eff, ldc, Cq, ldq, amax, st, &h->launches);
+    ce = launch_quantize_tensor_i8(C_acc, K, D_eff, ldc, pf, Cq, ldq, amax, st, &h->launches);
     if (ce != cudaSuccess) return cuda_fail(h, ce, "quantize C");
     B = Operand{Cq, ldq, OPK_I8};
     int_acc = true;
@@ -335,7 +348,7 @@ int do_similarity(hdc_ctx* h, const uint32_t* Hbits, int64_t N, int64_t ldh, con
   }
   if (b.off > ws_bytes) return fail(h, HDC_ERR_WORKSPACE, "similarity: workspace too small");
   if (colscale) {
-    ce = launch_col_scale(B, K, D_eff, 1, colscale, st, &h->launches);
+    ce = launch_col_scale(B, K, D_eff, 1, pf, colscale, st, &h->launches);
     if (ce != cudaSuccess) return cuda_fail(h, ce, "col_scale");
   }
   Epilogue e{};
@@ -362,6 +375,7 @@ size_t similarity_ws(int K, const hdc_knobs_t* k) {
   b.take<int8_t>((size_t)K * round_up(k->D_eff, 16));
   b.take<float>(1);
   b.take<uint32_t>((size_t)K * W);
+  b.take<uint32_t>((size_t)W);  // perforation mask
   b.take<uint8_t>(sim_tc_operand_bytes(K, k->hv_bits == 32 || k->hv_bits == 16 || k->hv_bits == 8 ? k->hv_bits : 1,
                                        k->D_eff));
   return b.off + 1024;

@@ -24,6 +24,21 @@ struct Operand {
   int kind;
 };
 
+// Reduction perforation of the similarity (include/hdc.h knobs perf_begin /
+// perf_stride): the visited dimensions are d = begin + j*stride < D_eff.
+struct Perf {
+  int begin;
+  int stride;
+};
+__host__ __device__ __forceinline__ bool perf_visits(const Perf& pf, int d) {
+  return d >= pf.begin && (pf.stride <= 1 || (d - pf.begin) % pf.stride == 0);
+}
+static inline int perf_count(const Perf& pf, int D_eff) {
+  const int st = pf.stride <= 1 ? 1 : pf.stride;
+  return D_eff > pf.begin ? (D_eff - pf.begin + st - 1) / st : 0;
+}
+static inline bool perf_on(const Perf& pf) { return pf.begin > 0 || pf.stride > 1; }
+
 enum EpilogueKind : int { EPI_SIGN = 0, EPI_SCORE = 1, EPI_ARGMAX = 2 };
 
 // Epilogue of C[m,n] = sum_k A[m,k] * B[n,k]
@@ -81,10 +96,12 @@ cudaError_t launch_gemm_tc(TcContext* tc, const TcOperands& o, int64_t M, int Nc
 size_t sim_tc_operand_bytes(int K, int hv_bits, int D_eff);
 cudaError_t launch_sim_tc(TcContext* tc, const uint32_t* Hbits, int64_t N, int64_t ldh, const float* C_acc,
                           int K, int64_t ldc, int D_eff, int hv_bits, void* cop, float* amax_scratch,
-                          const Epilogue& e, int sm_count, cudaStream_t st, int64_t* nlaunch);
-// amax = max |C[k][d]| over k < K, d < D_eff (amax zeroed here)
-cudaError_t launch_tensor_amax(const float* C, int K, int D_eff, int64_t ldc, float* amax, cudaStream_t st,
-                               int64_t* nlaunch);
+                          const Epilogue& e, Perf pf, int sm_count, cudaStream_t st, int64_t* nlaunch);
+// amax = max |C[k][d]| over k < K and the visited d < D_eff (amax zeroed here)
+cudaError_t launch_tensor_amax(const float* C, int K, int D_eff, int64_t ldc, Perf pf, float* amax,
+                               cudaStream_t st, int64_t* nlaunch);
+// mask[w] = bits of word w whose dimension is visited and < D_eff (W words)
+cudaError_t launch_perf_mask(uint32_t* mask, int W, int D_eff, Perf pf, cudaStream_t st, int64_t* nlaunch);
 
 // fp32/bf16 -> bf16 staging with zero padding of the reduction axis: dst [rows][ld_dst]
 cudaError_t launch_convert_bf16(const void* src, int src_kind, int64_t rows, int cols, int64_t ld_src,
@@ -97,21 +114,23 @@ cudaError_t launch_split3_bf16(const void* src, int src_kind, int64_t rows, int 
 cudaError_t launch_quantize_rows_i8(const void* src, int src_kind, int64_t rows, int cols, int64_t ld_src,
                                     int8_t* dst, int64_t ld_dst, cudaStream_t st, int64_t* nlaunch);
 // per-tensor symmetric int8 of C_acc[k<K][d<D_eff] (S5): amax_scratch is one float in ws
-cudaError_t launch_quantize_tensor_i8(const float* C, int K, int D_eff, int64_t ldc, int8_t* dst,
+cudaError_t launch_quantize_tensor_i8(const float* C, int K, int D_eff, int64_t ldc, Perf pf, int8_t* dst,
                                       int64_t ld_dst, float* amax_scratch, cudaStream_t st,
                                       int64_t* nlaunch);
 // sign bits of C_acc: cbits [K][W] (tail bits zero)
 cudaError_t launch_sign_bits(const float* C, int K, int D_eff, int64_t ldc, uint32_t* cbits, int W,
                              cudaStream_t st, int64_t* nlaunch);
-// colscale[k] = cos ? (nrm_k > 0 ? 1/(sqrt(D_eff)*nrm_k) : 0) : 1, nrm over the operand as loaded
-cudaError_t launch_col_scale(const Operand& C, int K, int D_eff, int cos, double* colscale,
+// colscale[k] = cos ? (nrm_k > 0 ? 1/(sqrt(n_visited)*nrm_k) : 0) : 1, nrm over the visited
+// dimensions of the operand as loaded
+cudaError_t launch_col_scale(const Operand& C, int K, int D_eff, int cos, Perf pf, double* colscale,
                              cudaStream_t st, int64_t* nlaunch);
 
 // packed XOR+popcount similarity with class bits in shared memory (hamming.cu)
 bool hamming_smem_fits(int K, int W, int smem_optin);
+// mask (nullable): W words; distances count only the bits set in it (reduction perforation)
 cudaError_t launch_hamming(const uint32_t* Hbits, int64_t N, int64_t ldh, const uint32_t* Cbits, int K,
-                           int W, int D_eff, int32_t* dist, int64_t lds, int32_t* labels, float* best,
-                           float* second, int sm_count, int smem_optin, cudaStream_t st,
+                           int W, int D_eff, const uint32_t* mask, int32_t* dist, int64_t lds, int32_t* labels,
+                           float* best, float* second, int sm_count, int smem_optin, cudaStream_t st,
                            int64_t* nlaunch);
 
 // level-ID encode (levelid.cu)

@@ -112,7 +112,7 @@ __global__ void quantize_rows_i8_kernel(const void* __restrict__ src, int src_ki
 
 // ---------------------------------------------------------------------------------- int8 per tensor
 // max |C[k][d]| over k < K, d < D_eff; non-negative floats order as unsigned ints.
-__global__ void tensor_amax_kernel(const float* __restrict__ C, int K, int D_eff, int64_t ldc,
+__global__ void tensor_amax_kernel(const float* __restrict__ C, int K, int D_eff, int64_t ldc, Perf pf,
                                    float* __restrict__ amax) {
   float a = 0.0f;
   const int64_t total = (int64_t)K * D_eff;
@@ -120,7 +120,7 @@ __global__ void tensor_amax_kernel(const float* __restrict__ C, int K, int D_eff
        i += (int64_t)gridDim.x * blockDim.x) {
     const int64_t k = i / D_eff;
     const int d = (int)(i - k * D_eff);
-    a = fmaxf(a, fabsf(__ldg(C + k * ldc + d)));
+    if (perf_visits(pf, d)) a = fmaxf(a, fabsf(__ldg(C + k * ldc + d)));
   }
 #pragma unroll
   for (int off = 16; off; off >>= 1) a = fmaxf(a, __shfl_xor_sync(0xffffffffu, a, off));
@@ -166,13 +166,15 @@ __global__ void sign_bits_kernel(const float* __restrict__ C, int K, int D_eff, 
 // ---------------------------------------------------------------------------------- cosine scales
 // colscale[k] = cos ? (nrm > 0 ? 1 / (sqrt(D_eff) * nrm) : 0) : 1, nrm^2 = sum_d c[k,d]^2 in double
 // over the operand as the contraction loads it.  One block per class, fixed reduction order.
-__global__ void col_scale_kernel(Operand C, int K, int D_eff, int cos, double* __restrict__ colscale) {
+__global__ void col_scale_kernel(Operand C, int K, int D_eff, int cos, Perf pf, int n_vis,
+                                 double* __restrict__ colscale) {
   const int k = blockIdx.x;
   __shared__ double part[32];
   double s = 0.0;
   if (cos) {
 #pragma unroll 4
     for (int d = threadIdx.x; d < D_eff; d += blockDim.x) {
+      if (!perf_visits(pf, d)) continue;
       double v;
       const int64_t idx = (int64_t)k * C.ld + d;
       switch (C.kind) {
@@ -198,7 +200,7 @@ __global__ void col_scale_kernel(Operand C, int K, int D_eff, int cos, double* _
       double t = 0.0;
       for (int i = 0; i < (int)(blockDim.x >> 5); ++i) t += part[i];
       const double nrm = sqrt(t);
-      colscale[k] = nrm > 0.0 ? 1.0 / (sqrt((double)D_eff) * nrm) : 0.0;
+      colscale[k] = nrm > 0.0 ? 1.0 / (sqrt((double)n_vis) * nrm) : 0.0;
     }
   }
 }
@@ -240,19 +242,39 @@ cudaError_t launch_quantize_rows_i8(const void* src, int src_kind, int64_t rows,
   return cudaGetLastError();
 }
 
-cudaError_t launch_tensor_amax(const float* C, int K, int D_eff, int64_t ldc, float* amax, cudaStream_t st,
-                               int64_t* nlaunch) {
-  cudaError_t e = cudaMemsetAsync(amax, 0, sizeof(float), st);
-  if (e != cudaSuccess) return e;
-  tensor_amax_kernel<<<grid_for((int64_t)K * D_eff, 256, 148 * 4), 256, 0, st>>>(C, K, D_eff, ldc, amax);
+namespace {
+__global__ void perf_mask_kernel(uint32_t* __restrict__ mask, int W, int D_eff, Perf pf) {
+  const int w = blockIdx.x * blockDim.x + threadIdx.x;
+  if (w >= W) return;
+  uint32_t m = 0;
+  for (int b = 0; b < 32; ++b) {
+    const int d = w * 32 + b;
+    if (d < D_eff && perf_visits(pf, d)) m |= 1u << b;
+  }
+  mask[w] = m;
+}
+
+}  // namespace
+
+cudaError_t launch_perf_mask(uint32_t* mask, int W, int D_eff, Perf pf, cudaStream_t st, int64_t* nlaunch) {
+  perf_mask_kernel<<<(W + 255) / 256, 256, 0, st>>>(mask, W, D_eff, pf);
   ++*nlaunch;
   return cudaGetLastError();
 }
 
-cudaError_t launch_quantize_tensor_i8(const float* C, int K, int D_eff, int64_t ldc, int8_t* dst,
+cudaError_t launch_tensor_amax(const float* C, int K, int D_eff, int64_t ldc, Perf pf, float* amax,
+                               cudaStream_t st, int64_t* nlaunch) {
+  cudaError_t e = cudaMemsetAsync(amax, 0, sizeof(float), st);
+  if (e != cudaSuccess) return e;
+  tensor_amax_kernel<<<grid_for((int64_t)K * D_eff, 256, 148 * 4), 256, 0, st>>>(C, K, D_eff, ldc, pf, amax);
+  ++*nlaunch;
+  return cudaGetLastError();
+}
+
+cudaError_t launch_quantize_tensor_i8(const float* C, int K, int D_eff, int64_t ldc, Perf pf, int8_t* dst,
                                       int64_t ld_dst, float* amax_scratch, cudaStream_t st,
                                       int64_t* nlaunch) {
-  cudaError_t e = launch_tensor_amax(C, K, D_eff, ldc, amax_scratch, st, nlaunch);
+  cudaError_t e = launch_tensor_amax(C, K, D_eff, ldc, pf, amax_scratch, st, nlaunch);
   if (e != cudaSuccess) return e;
   quantize_tensor_i8_kernel<<<grid_for((int64_t)K * ld_dst, 256, 148 * 8), 256, 0, st>>>(
       C, K, D_eff, ldc, dst, ld_dst, amax_scratch);
@@ -268,9 +290,9 @@ cudaError_t launch_sign_bits(const float* C, int K, int D_eff, int64_t ldc, uint
   return cudaGetLastError();
 }
 
-cudaError_t launch_col_scale(const Operand& C, int K, int D_eff, int cos, double* colscale,
+cudaError_t launch_col_scale(const Operand& C, int K, int D_eff, int cos, Perf pf, double* colscale,
                              cudaStream_t st, int64_t* nlaunch) {
-  col_scale_kernel<<<K, 1024, 0, st>>>(C, K, D_eff, cos, colscale);
+  col_scale_kernel<<<K, 1024, 0, st>>>(C, K, D_eff, cos, pf, perf_count(pf, D_eff), colscale);
   ++*nlaunch;
   return cudaGetLastError();
 }

@@ -36,7 +36,7 @@ __device__ __forceinline__ void csa(uint32_t& hi, uint32_t& lo, uint32_t a, uint
 
 constexpr int NST = 3;                      // cp.async ring depth
 constexpr int HQ_WORDS = WC * (QT + 1);     // transposed query tile, stride QT+1: conflict-free
-__host__ __device__ constexpr int stage_words(int KC) { return HQ_WORDS + KC * WC; }
+__host__ __device__ constexpr int stage_words(int KC) { return HQ_WORDS + (KC + 1) * WC; }  // + mask row
 
 __device__ __forceinline__ void cp_async4(uint32_t dst_smem, const void* src, bool ok) {
   // 4-byte asynchronous copy global -> shared; src-size 0 writes zeros (rows >= N, words >= W)
@@ -46,11 +46,13 @@ __device__ __forceinline__ void cp_async4(uint32_t dst_smem, const void* src, bo
 
 // Work of a CTA = its query tiles (grid-stride) x class groups x chunks, flattened into steps; the
 // query / class words of step s+2 are in flight (cp.async, no registers) while step s is counted.
-template <int KC>
+// PERF: a mask row (the visited dimensions of a perforated reduction) travels with the
+// class tile and is ANDed into every XORed word -- the AND folds into the same LOP3 as the XOR.
+template <int KC, bool PERF>
 __global__ void __launch_bounds__(QT)
 hamming_kernel(const uint32_t* __restrict__ Hbits, int64_t N, int64_t ldh,
                const uint32_t* __restrict__ Cbits, int K, int W, int D_eff,
-               int32_t* __restrict__ dist, int64_t lds, int32_t* __restrict__ labels,
+               const uint32_t* __restrict__ mask, int32_t* __restrict__ dist, int64_t lds, int32_t* __restrict__ labels,
                float* __restrict__ best, float* __restrict__ second) {
   extern __shared__ __align__(16) uint32_t sm[];
   constexpr int STW = stage_words(KC);
@@ -88,6 +90,10 @@ hamming_kernel(const uint32_t* __restrict__ Hbits, int64_t N, int64_t ldh,
       const bool ok = k0 + k < K && w0 + wl < W;
       cp_async4(st + (uint32_t)(HQ_WORDS + idx) * 4u, ok ? Cbits + (int64_t)(k0 + k) * W + w0 + wl : Cbits, ok);
     }
+    if (PERF && tid < WC) {
+      const bool ok = w0 + tid < W;
+      cp_async4(st + (uint32_t)(HQ_WORDS + KC * WC + tid) * 4u, ok ? mask + w0 + tid : mask, ok);
+    }
     if (++is_st == NST) is_st = 0;
     if (++is_ch == nchunks) {
       is_ch = 0;
@@ -119,22 +125,28 @@ hamming_kernel(const uint32_t* __restrict__ Hbits, int64_t N, int64_t ldh,
 #pragma unroll
       for (int k = 0; k < KC; ++k) acc[k] = 0;
     }
-    if (w0 + WC >= W && tail_mask != 0xffffffffu) hq[(W - 1 - w0) * (QT + 1) + tid] &= tail_mask;  // own column
+    if (!PERF && w0 + WC >= W && tail_mask != 0xffffffffu)
+      hq[(W - 1 - w0) * (QT + 1) + tid] &= tail_mask;  // own column (the perforation mask covers the tail)
 #pragma unroll 1
     for (int w = 0; w < WC; w += 8) {
       uint32_t h[8];
 #pragma unroll
       for (int j = 0; j < 8; ++j) h[j] = hq[(w + j) * (QT + 1) + tid];
+      uint4 ma = make_uint4(~0u, ~0u, ~0u, ~0u), mb = ma;
+      if (PERF) {
+        ma = *reinterpret_cast<const uint4*>(&cs[KC * WC + w]);
+        mb = *reinterpret_cast<const uint4*>(&cs[KC * WC + w + 4]);
+      }
 #pragma unroll
       for (int k = 0; k < KC; ++k) {
         const uint4 ca = *reinterpret_cast<const uint4*>(&cs[k * WC + w]);
         const uint4 cb = *reinterpret_cast<const uint4*>(&cs[k * WC + w + 4]);
         uint32_t a1, s1, a2, s2, a3, ones, fours, twos;
-        csa(a1, s1, h[0] ^ ca.x, h[1] ^ ca.y, h[2] ^ ca.z);
-        csa(a2, s2, h[3] ^ ca.w, h[4] ^ cb.x, h[5] ^ cb.y);
-        csa(a3, ones, s1, s2, h[6] ^ cb.z);
+        csa(a1, s1, (h[0] ^ ca.x) & ma.x, (h[1] ^ ca.y) & ma.y, (h[2] ^ ca.z) & ma.z);
+        csa(a2, s2, (h[3] ^ ca.w) & ma.w, (h[4] ^ cb.x) & mb.x, (h[5] ^ cb.y) & mb.y);
+        csa(a3, ones, s1, s2, (h[6] ^ cb.z) & mb.z);
         csa(fours, twos, a1, a2, a3);
-        acc[k] += (__popc(ones) + __popc(h[7] ^ cb.w)) + 2 * __popc(twos) + 4 * __popc(fours);
+        acc[k] += (__popc(ones) + __popc((h[7] ^ cb.w) & mb.w)) + 2 * __popc(twos) + 4 * __popc(fours);
       }
     }
     if (ch == nchunks - 1) {
@@ -183,19 +195,29 @@ hamming_kernel(const uint32_t* __restrict__ Hbits, int64_t N, int64_t ldh,
   asm volatile("cp.async.wait_group 0;" ::: "memory");
 }
 
-template <int KC>
-cudaError_t launch_ham(int grid, cudaStream_t st, const uint32_t* Hbits, int64_t N, int64_t ldh,
-                       const uint32_t* Cbits, int K, int W, int D_eff, int32_t* dist, int64_t lds,
-                       int32_t* labels, float* best, float* second) {
+template <int KC, bool PERF>
+cudaError_t launch_ham2(int grid, cudaStream_t st, const uint32_t* Hbits, int64_t N, int64_t ldh,
+                        const uint32_t* Cbits, int K, int W, int D_eff, const uint32_t* mask, int32_t* dist,
+                        int64_t lds, int32_t* labels, float* best, float* second) {
   constexpr int SMEM = NST * stage_words(KC) * 4;
   static bool attr_set = false;
   if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(hamming_kernel<KC>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM);
+    cudaError_t e =
+        cudaFuncSetAttribute(hamming_kernel<KC, PERF>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM);
     if (e != cudaSuccess) return e;
     attr_set = true;
   }
-  hamming_kernel<KC><<<grid, QT, SMEM, st>>>(Hbits, N, ldh, Cbits, K, W, D_eff, dist, lds, labels, best, second);
+  hamming_kernel<KC, PERF><<<grid, QT, SMEM, st>>>(Hbits, N, ldh, Cbits, K, W, D_eff, mask, dist, lds, labels,
+                                                   best, second);
   return cudaGetLastError();
+}
+template <int KC>
+cudaError_t launch_ham(int grid, cudaStream_t st, const uint32_t* Hbits, int64_t N, int64_t ldh,
+                       const uint32_t* Cbits, int K, int W, int D_eff, const uint32_t* mask, int32_t* dist,
+                       int64_t lds, int32_t* labels, float* best, float* second) {
+  if (mask)
+    return launch_ham2<KC, true>(grid, st, Hbits, N, ldh, Cbits, K, W, D_eff, mask, dist, lds, labels, best, second);
+  return launch_ham2<KC, false>(grid, st, Hbits, N, ldh, Cbits, K, W, D_eff, mask, dist, lds, labels, best, second);
 }
 
 }  // namespace
@@ -203,15 +225,15 @@ cudaError_t launch_ham(int grid, cudaStream_t st, const uint32_t* Hbits, int64_t
 bool hamming_smem_fits(int, int, int) { return true; }
 
 cudaError_t launch_hamming(const uint32_t* Hbits, int64_t N, int64_t ldh, const uint32_t* Cbits, int K,
-                           int W, int D_eff, int32_t* dist, int64_t lds, int32_t* labels, float* best,
-                           float* second, int sm_count, int, cudaStream_t st, int64_t* nlaunch) {
+                           int W, int D_eff, const uint32_t* mask, int32_t* dist, int64_t lds, int32_t* labels,
+                           float* best, float* second, int sm_count, int, cudaStream_t st, int64_t* nlaunch) {
   if (N <= 0) return cudaSuccess;
   int64_t tiles = (N + QT - 1) / QT;
   const int64_t cap = (int64_t)sm_count * 64;  // one tile per CTA up to here: the block scheduler balances the SMs
   const int grid = (int)(tiles < cap ? tiles : cap);
   cudaError_t ce;
 #define HDC_HAM(KC_) \
-  ce = launch_ham<KC_>(grid, st, Hbits, N, ldh, Cbits, K, W, D_eff, dist, lds, labels, best, second)
+  ce = launch_ham<KC_>(grid, st, Hbits, N, ldh, Cbits, K, W, D_eff, mask, dist, lds, labels, best, second)
   // smallest register group that covers K in one pass; K > 32 walks groups of 32
   if (K <= 2) HDC_HAM(2);
   else if (K <= 4) HDC_HAM(4);

@@ -405,7 +405,7 @@ __device__ __forceinline__ int quant_i8_c(float x, float s) {
 template <bool INT8>
 __global__ void class_operand_kernel(const float* __restrict__ C, int K, int D_eff, int64_t ldc, int mode,
                                      int kc, int nparts, int rows_total, int num_kb,
-                                     const float* __restrict__ amax, void* __restrict__ dst) {
+                                     const float* __restrict__ amax, Perf pf, void* __restrict__ dst) {
   constexpr int BK = INT8 ? 128 : 64;
   const int64_t ld = (int64_t)num_kb * BK;
   const int64_t total = (int64_t)rows_total * ld;
@@ -424,7 +424,7 @@ __global__ void class_operand_kernel(const float* __restrict__ C, int K, int D_e
     const int kb = col / BK, kappa = col % BK;
     const int d = kb * BK + (INT8 ? perm_i8(kappa) : perm_bf16(kappa));
     float x = 0.0f;
-    const bool live = k < K && d < D_eff;
+    const bool live = k < K && d < D_eff && perf_visits(pf, d);  // unvisited dimensions contribute 0
     if (live) x = __ldg(C + (int64_t)k * ldc + d);
     if (INT8) {
       int qv = 0;
@@ -481,7 +481,7 @@ size_t sim_tc_operand_bytes(int K, int hv_bits, int D_eff) {
 
 cudaError_t launch_sim_tc(TcContext* tc, const uint32_t* Hbits, int64_t N, int64_t ldh, const float* C_acc,
                           int K, int64_t ldc, int D_eff, int hv_bits, void* cop, float* amax_scratch,
-                          const Epilogue& e, int sm_count, cudaStream_t st, int64_t* nlaunch) {
+                          const Epilogue& e, Perf pf, int sm_count, cudaStream_t st, int64_t* nlaunch) {
   if (!tc) return cudaErrorNotSupported;
   if (N <= 0) return cudaSuccess;
   if ((reinterpret_cast<uintptr_t>(cop) & 15) != 0) return cudaErrorNotSupported;
@@ -493,7 +493,7 @@ cudaError_t launch_sim_tc(TcContext* tc, const uint32_t* Hbits, int64_t N, int64
   const int64_t ld = (int64_t)num_kb * BK;
   cudaError_t ce;
   if (hv_bits == 8) {
-    ce = launch_tensor_amax(C_acc, K, D_eff, ldc, amax_scratch, st, nlaunch);
+    ce = launch_tensor_amax(C_acc, K, D_eff, ldc, pf, amax_scratch, st, nlaunch);
     if (ce != cudaSuccess) return ce;
   }
   {
@@ -502,10 +502,10 @@ cudaError_t launch_sim_tc(TcContext* tc, const uint32_t* Hbits, int64_t N, int64
     if (g > (int64_t)sm_count * 16) g = (int64_t)sm_count * 16;
     if (int8)
       class_operand_kernel<true><<<(unsigned)g, 256, 0, st>>>(C_acc, K, D_eff, ldc, hv_bits, kc, nparts, rows_total,
-                                                             num_kb, amax_scratch, cop);
+                                                             num_kb, amax_scratch, pf, cop);
     else
       class_operand_kernel<false><<<(unsigned)g, 256, 0, st>>>(C_acc, K, D_eff, ldc, hv_bits, kc, nparts,
-                                                              rows_total, num_kb, amax_scratch, cop);
+                                                              rows_total, num_kb, amax_scratch, pf, cop);
     ++*nlaunch;
     ce = cudaGetLastError();
     if (ce != cudaSuccess) return ce;

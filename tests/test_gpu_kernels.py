@@ -347,3 +347,72 @@ def test_kmeans_empty_cluster_keeps_accumulator(hd, h):
     got = Cd.cpu().numpy()
     assert np.array_equal(got, C_or)
     assert np.array_equal(got[1], C[1]) and np.array_equal(got[2], C[2])
+
+
+# ------------------------------------------------------------------------------------ perforation
+@pytest.mark.parametrize("begin,stride", [(0, 8), (3, 8), (5, 2), (1, 3), (17, 1), (0, 64)])
+@pytest.mark.parametrize("sim,hv_bits", [("HAMMING", 1), ("DOT", 1), ("DOT", 8), ("COS", 8), ("COS", 32), ("COS", 16),
+                                         ("DOT", 32)])
+@pytest.mark.parametrize("N,K,D,D_eff", [(150, 10, 2100, 2100), (70, 70, 1300, 1000), (33, 3, 10000, 8400)])
+def test_perforated_similarity_and_classify(hd, h, begin, stride, sim, hv_bits, N, K, D, D_eff):
+    """General reduction perforation of the similarity (reading A17): the kernels
+    visit d = begin + j*stride < D_eff only and agree with the oracle's gather of those dimensions --
+    exactly on the integer paths (popcount kernel for K < 64, +-1 / int8 tensor path), within the
+    float rules otherwise."""
+    r = rng(12, N, K, D_eff, hv_bits, begin, stride)
+    hb = r.integers(0, 2, size=(N, D), dtype=np.uint8)
+    C = (r.standard_normal((K, D)) * 30).astype(np.float32)
+    C[r.random((K, D)) < 0.03] = 0.0
+    simc = getattr(O, "SIM_" + sim)
+    S_or = O.similarity(hb, C, D_eff, simc, hv_bits, begin, stride)
+    kn = hd.knobs(D_eff, hv_bits=hv_bits, sim=getattr(hd, "HDC_SIM_" + sim), perf_begin=begin, perf_stride=stride)
+    Hd, Cd = dev_bits(hb), dev(C)
+    S = h.hdc_similarity(Hd, Cd, kn).cpu().numpy()
+    lab = h.hdc_classify(Hd, Cd, kn).cpu().numpy()
+    lab_or, _, _ = O.classify(S_or, simc)
+    if hv_bits in (8, 1):
+        if sim == "COS":
+            assert np.allclose(S, S_or, rtol=1e-6, atol=1e-9)
+        else:
+            assert np.array_equal(S.astype(np.float64), S_or.astype(np.float64))
+        assert np.array_equal(lab, lab_or)
+    else:
+        idx = O.perforated_index(D_eff, begin, stride)
+        cop = O.class_operand(C[:, idx], len(idx), hv_bits)
+        floor = 1e-6 * np.sqrt(len(idx)) * np.sqrt((cop * cop).sum(axis=1))[None, :] if sim == "DOT" else 1e-6
+        check_scores(S, S_or, floor)
+        check_labels_float(lab, S_or, simc)
+
+
+@pytest.mark.parametrize("hv_bits,sim", [(1, "HAMMING"), (8, "COS")])
+def test_perforated_training_epoch_exact(hd, h, hv_bits, sim):
+    """Predictions use the perforated similarity, the update still touches every d < D_eff."""
+    w = gen.c1_tiny(D=512)
+    hb, _, _ = O.encode_rp(w["Xtr"], w["P"], 512, O.F32)
+    y = w["ytr"].copy()
+    y[::5] = (y[::5] + 1) % w["K"]
+    simc = getattr(O, "SIM_" + sim)
+    C = O.bundle(hb, y, w["K"], 512)
+    kn = hd.knobs(500, hv_bits=hv_bits, sim=getattr(hd, "HDC_SIM_" + sim), perf_begin=2, perf_stride=4)
+    Cd, Hd, yd = dev(C.copy()), dev_bits(hb), dev(y)
+    C_or = C[:, :500].copy()
+    for _ in range(2):
+        C_or, wrong_or, pred_or = O.train_epoch(hb, y, C_or, 500, hv_bits, simc, 0.05, 64, begin=2, stride=4)
+        pred = torch.empty(len(y), dtype=torch.int32, device="cuda")
+        nw = torch.zeros(1, dtype=torch.int64, device="cuda")
+        h.hdc_train_epoch(hd.HDC_TRAIN_PERCEPTRON, Hd, yd, Cd, kn, lr=0.05, batch=64, pred=pred, n_wrong=nw)
+        assert np.array_equal(pred.cpu().numpy(), pred_or)
+        assert int(nw.item()) == wrong_or
+        assert np.array_equal(Cd.cpu().numpy()[:, :500], C_or)
+
+
+def test_perforation_argument_errors(hd, h):
+    Hd = torch.zeros((4, 4), dtype=torch.int32, device="cuda")
+    Cd = torch.ones((2, 128), dtype=torch.float32, device="cuda")
+    for bad in (dict(perf_begin=128), dict(perf_begin=-1), dict(perf_stride=-2)):
+        with pytest.raises(hd.HdcError) as ei:
+            h.hdc_classify(Hd, Cd, hd.knobs(128, hv_bits=1, sim=hd.HDC_SIM_HAMMING, **bad))
+        assert ei.value.code == hd.HDC_ERR_INVALID_ARG
+    with pytest.raises(hd.HdcError) as ei:                  # CUDA-core DOT / COS kernels are not perforated
+        h.hdc_classify(Hd, Cd, hd.knobs(128, hv_bits=32, sim=hd.HDC_SIM_COS, flags=hd.HDC_FLAG_SIMT, perf_stride=2))
+    assert ei.value.code == hd.HDC_ERR_UNSUPPORTED
