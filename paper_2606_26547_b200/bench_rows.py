@@ -222,6 +222,84 @@ def row_c5_stream(h, peaks, reps, hv_bits, sim_name, N=1 << 20, B=65536, F=1024,
     return out
 
 
+def row_c3_pipeline(h, peaks, reps, N=65536, F=784, Q=256, D=10000, K=10):
+    """configs[2] inference: level-ID encode + packed Hamming classify against K = 10 classes."""
+    from workloads import gen
+    import numpy as np
+    w = gen.c3_mnist_shaped(D=D, n_tr=16, n_te=4096, Q=Q)
+    lv = torch.from_numpy(gen.tile_rows(w["Lte"], N)).cuda()
+    ID = torch.from_numpy(gen.pack_bits_lsb(w["ID"]).view(np.int32)).cuda()
+    LV = torch.from_numpy(gen.pack_bits_lsb(w["LV"]).view(np.int32)).cuda()
+    H = torch.empty((N, (D + 31) // 32), dtype=torch.int32, device="cuda")
+    C = _class_acc(K, D, 4)
+    lab = torch.empty(N, dtype=torch.int32, device="cuda")
+    kn_e, kn = hd.knobs(D), hd.knobs(D, hv_bits=1, sim=hd.HDC_SIM_HAMMING)
+
+    def fn():
+        h.hdc_encode_levelid(lv, ID, LV, D, kn_e, Hbits=H)
+        h.hdc_classify(H, C, kn, labels=lab)
+
+    call_ms = _time(fn, reps)
+    ops = 3.0 * F * ((D + 31) // 32) * N
+    ach = ops / (call_ms * 1e-3) / 1e12
+    peak = 148 * 64 * peaks["sm_max_mhz"] * 1e6 / 1e12
+    return {"what": f"C3 inference: hdc_encode_levelid + hdc_classify (Hamming) N={N} F={F} Q={Q} D={D} K={K}",
+            "call_ms": call_ms, "queries_per_s": N / (call_ms * 1e-3),
+            "roofline": {"bound": "alu", "achieved": ach, "peak": peak, "unit": "Tlop/s (32-bit logic ops)",
+                         "frac": ach / peak, "peak_source": "148 SM x 64 INT lanes x sm_max_mhz; 3*F*W ops per query"}}
+
+
+def c4_sweep(h, peaks, reps=5, NQ=131072):
+    """configs[3]: D_eff x precision x retraining epochs on the HAR-shaped Gaussian mixture.  Per
+    point: inference queries/s (encode at D_eff + classify, test set tiled to NQ), training
+    samples/s of one retraining epoch, and the test accuracy after E = 0 / 5 / 20 epochs (accuracy
+    parity with the oracle is the job of tests/test_gpu_configs.py)."""
+    from workloads import gen
+    import numpy as np
+    w = gen.c4_har_shaped()
+    D, K = w["D"], w["K"]
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()  # noqa: E731
+    Xtr, Xte, ytr, P = dev(w["Xtr"]), dev(w["Xte"]), dev(w["ytr"]), dev(w["P"])
+    Xq = dev(gen.tile_rows(w["Xte"], NQ))
+    yte = w["yte"]
+    points = []
+    precs = [("fp32", hd.HDC_F32, 32, hd.HDC_SIM_COS), ("bf16", hd.HDC_BF16, 16, hd.HDC_SIM_COS),
+             ("int8", hd.HDC_I8, 8, hd.HDC_SIM_COS), ("1bit", hd.HDC_B1, 1, hd.HDC_SIM_HAMMING)]
+    for name, prec, hv_bits, sim in precs:
+        for D_eff in w["d_eff"]:
+            kn_e = hd.knobs(D_eff, precision=prec)
+            kn = hd.knobs(D_eff, precision=prec, hv_bits=hv_bits, sim=sim)
+            Htr = h.hdc_encode_rp(Xtr, P, kn_e)
+            Hte = h.hdc_encode_rp(Xte, P, kn_e)
+            C = torch.zeros((K, D), dtype=torch.float32, device="cuda")
+            h.hdc_train_epoch(hd.HDC_TRAIN_BUNDLE, Htr, ytr, C, kn)
+            acc = {}
+            done = 0
+            for E in w["epochs"]:
+                for _ in range(E - done):
+                    h.hdc_train_epoch(hd.HDC_TRAIN_PERCEPTRON, Htr, ytr, C, kn, lr=w["lr"], batch=0)
+                done = E
+                lab = h.hdc_classify(Hte, C, kn).cpu().numpy()
+                acc[f"E{E}"] = float((lab == yte).mean())
+            Ct = C.clone()
+            ep_ms = _time(lambda: h.hdc_train_epoch(hd.HDC_TRAIN_PERCEPTRON, Htr, ytr, Ct, kn, lr=w["lr"], batch=0),
+                          reps)
+            Hq = torch.empty((NQ, (D_eff + 31) // 32), dtype=torch.int32, device="cuda")
+            lab_q = torch.empty(NQ, dtype=torch.int32, device="cuda")
+
+            def infer():
+                h.hdc_encode_rp(Xq, P, kn_e, Hbits=Hq)
+                h.hdc_classify(Hq, C, kn, labels=lab_q)
+
+            time.sleep(0.3)
+            inf_ms = _time(infer, reps)
+            points.append({"precision": name, "D_eff": D_eff, "queries_per_s": NQ / (inf_ms * 1e-3),
+                           "train_samples_per_s": Xtr.shape[0] / (ep_ms * 1e-3), "accuracy": acc})
+            del Hq, lab_q
+            torch.cuda.empty_cache()
+    return points
+
+
 def row_kmeans(h, peaks, reps, N=7797, K=26, D=10000, hv_bits=32, sim_name="cos"):
     """HD-Clustering epoch (assign + re-bundle) on noisy copies of K prototypes, ISOLET-sized."""
     sim = {"cos": hd.HDC_SIM_COS, "hamming": hd.HDC_SIM_HAMMING}[sim_name]
@@ -250,6 +328,7 @@ ROWS = {
     "c5_encode_bf16": lambda h, p, r: row_encode(h, p, r, 65536, 1024, 16384, "bf16", x_bf16=True),
     "c5_classify_bf16": lambda h, p, r: row_classify(h, p, r, 65536, 1000, 16384, 16, "cos"),
     "c5_classify_1bit": lambda h, p, r: row_classify(h, p, r, 65536, 1000, 16384, 1, "hamming"),
+    "c3_pipeline": lambda h, p, r: row_c3_pipeline(h, p, r),
     "c5_stream_bf16": lambda h, p, r: row_c5_stream(h, p, r, 16, "cos"),
     "c5_stream_1bit": lambda h, p, r: row_c5_stream(h, p, r, 1, "hamming"),
     "c2_train_epoch": lambda h, p, r: row_train(h, p, r),
@@ -272,6 +351,7 @@ def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--row", default=None, choices=sorted(ROWS))
     ap.add_argument("--reps", type=int, default=5)
+    ap.add_argument("--c4-sweep", action="store_true", help="configs[3]: D_eff x precision x epochs table")
     a = ap.parse_args()
     pk = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(pk):
@@ -281,6 +361,11 @@ def main():
         peaks = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "sm_max_mhz": 1965.0}
     torch.cuda.set_device(0)
     h = hd.Handle(0)
+    if a.c4_sweep:
+        for pt in c4_sweep(h, peaks, a.reps):
+            print(json.dumps({"c4_sweep": pt}), flush=True)
+        h.close()
+        return
     res = run(h, peaks, a.reps, a.row)
     for k, v in res.items():
         print(json.dumps({k: v}), flush=True)
