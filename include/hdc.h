@@ -28,6 +28,8 @@
  *    d < D_eff and nothing is rescaled (L61 "only the first 1024 elements", L155 "used as-is").
  *    Results equal those obtained by slicing every [.][D] array to its first D_eff columns.
  *  - arg-max / arg-min ties go to the lowest class index.  Inputs must be finite.
+ *  - Empty inputs: a call with N == 0 validates its other arguments, enqueues nothing and returns
+ *    HDC_OK; the per-sample pointers (X, levels, Hbits, S, labels, y, pred) may then be NULL.
  *  - Outputs must not alias inputs (except C_acc, which is in/out).  A handle is not thread-safe;
  *    distinct handles are independent.  There is no CPU fallback and no other architecture:
  *    hdc_create() fails with HDC_ERR_ARCH unless the device is compute capability 10.x.

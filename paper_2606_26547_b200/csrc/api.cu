@@ -510,7 +510,7 @@ extern "C" size_t hdc_workspace_bytes(hdc_handle_t h, int32_t op, int64_t N, int
 // =================================================================================== (1a)
 static int check_encode_rp_args(hdc_ctx* h, const void* X, int x_dtype, int64_t N, int F, int64_t ldx,
                                 const void* P, int p_dtype, int D, int64_t ldp, const hdc_knobs_t* k) {
-  if (!X || !P) return fail(h, HDC_ERR_INVALID_ARG, "encode_rp: NULL operand");
+  if ((!X && N > 0) || !P) return fail(h, HDC_ERR_INVALID_ARG, "encode_rp: NULL operand");
   if (N < 0 || F < 1 || D < 1 || ldx < F || ldp < F) return fail(h, HDC_ERR_INVALID_ARG, "encode_rp: bad sizes");
   if (x_dtype != HDC_F32 && x_dtype != HDC_BF16) return fail(h, HDC_ERR_INVALID_ARG, "encode_rp: x_dtype");
   if (p_dtype != HDC_F32 && p_dtype != HDC_BF16 && p_dtype != HDC_I8)
@@ -535,9 +535,10 @@ extern "C" int32_t hdc_encode_rp(hdc_handle_t h, const void* X, int32_t x_dtype,
   if (!h) return HDC_ERR_INVALID_ARG;
   int rc = check_encode_rp_args(h, X, x_dtype, N, F, ldx, P, p_dtype, D, ldp, knobs);
   if (rc) return rc;
-  if (!(out_kinds & HDC_OUT_BITS) || !Hbits) return fail(h, HDC_ERR_INVALID_ARG, "encode_rp: Hbits required");
+  if (!(out_kinds & HDC_OUT_BITS) || (!Hbits && N > 0))
+    return fail(h, HDC_ERR_INVALID_ARG, "encode_rp: Hbits required");
   if (ldh_words < words_of(knobs->D_eff)) return fail(h, HDC_ERR_INVALID_ARG, "encode_rp: ldh_words < W");
-  if ((out_kinds & HDC_OUT_RAW) && (!Hraw || ldraw < knobs->D_eff))
+  if ((out_kinds & HDC_OUT_RAW) && ((!Hraw && N > 0) || ldraw < knobs->D_eff))
     return fail(h, HDC_ERR_INVALID_ARG, "encode_rp: Hraw / ldraw");
   if (reinterpret_cast<uintptr_t>(Hbits) & 3) return fail(h, HDC_ERR_ALIGNMENT, "encode_rp: Hbits alignment");
   if (N == 0) return HDC_OK;
@@ -556,7 +557,8 @@ extern "C" int32_t hdc_encode_levelid(hdc_handle_t h, const uint8_t* levels, int
   (void)ws;
   (void)ws_bytes;
   if (!h) return HDC_ERR_INVALID_ARG;
-  if (!levels || !IDbits || !LVbits || !Hbits) return fail(h, HDC_ERR_INVALID_ARG, "encode_levelid: NULL pointer");
+  if (((!levels || !Hbits) && N > 0) || !IDbits || !LVbits)
+    return fail(h, HDC_ERR_INVALID_ARG, "encode_levelid: NULL pointer");
   if (N < 0 || F < 1 || F > 65535 || Q < 1 || Q > 256 || D < 1 || ldl < F)
     return fail(h, HDC_ERR_INVALID_ARG, "encode_levelid: bad sizes");
   int rc = check_knobs(h, knobs, D);
@@ -580,7 +582,7 @@ extern "C" int32_t hdc_encode_levelid(hdc_handle_t h, const uint8_t* levels, int
 // =================================================================================== (2), (2+3a)
 static int check_sim_args(hdc_ctx* h, const uint32_t* Hbits, int64_t N, int64_t ldh, const float* C_acc,
                           int K, int64_t ldc, int D, const hdc_knobs_t* k) {
-  if (!Hbits || !C_acc) return fail(h, HDC_ERR_INVALID_ARG, "similarity: NULL operand");
+  if ((!Hbits && N > 0) || !C_acc) return fail(h, HDC_ERR_INVALID_ARG, "similarity: NULL operand");
   if (N < 0 || K < 1 || K > 65535 || D < 1 || ldc < D) return fail(h, HDC_ERR_INVALID_ARG, "similarity: bad sizes");
   int rc = check_knobs(h, k, D);
   if (rc) return rc;
@@ -599,7 +601,7 @@ extern "C" int32_t hdc_similarity(hdc_handle_t h, const uint32_t* Hbits, int64_t
   if (!h) return HDC_ERR_INVALID_ARG;
   int rc = check_sim_args(h, Hbits, N, ldh_words, C_acc, K, ldc, D, knobs);
   if (rc) return rc;
-  if (!S || lds < K) return fail(h, HDC_ERR_INVALID_ARG, "similarity: S / lds");
+  if ((!S && N > 0) || lds < K) return fail(h, HDC_ERR_INVALID_ARG, "similarity: S / lds");
   if (knobs->sim == HDC_SIM_HAMMING && s_dtype != HDC_I32)
     return fail(h, HDC_ERR_INVALID_ARG, "similarity: HAMMING writes int32");
   if (knobs->sim == HDC_SIM_COS && s_dtype != HDC_F32) return fail(h, HDC_ERR_INVALID_ARG, "similarity: COS writes fp32");
@@ -622,7 +624,7 @@ extern "C" int32_t hdc_classify(hdc_handle_t h, const uint32_t* Hbits, int64_t N
   if (!h) return HDC_ERR_INVALID_ARG;
   int rc = check_sim_args(h, Hbits, N, ldh_words, C_acc, K, ldc, D, knobs);
   if (rc) return rc;
-  if (!labels) return fail(h, HDC_ERR_INVALID_ARG, "classify: labels is NULL");
+  if (!labels && N > 0) return fail(h, HDC_ERR_INVALID_ARG, "classify: labels is NULL");
   if (N == 0) return HDC_OK;
   Bump b(ws);
   if (!ws) ws_bytes = 0;
@@ -638,7 +640,7 @@ extern "C" int32_t hdc_train_epoch(hdc_handle_t h, int32_t mode, const uint32_t*
   if (!h) return HDC_ERR_INVALID_ARG;
   if (mode != HDC_TRAIN_BUNDLE && mode != HDC_TRAIN_PERCEPTRON && mode != HDC_TRAIN_KMEANS)
     return fail(h, HDC_ERR_INVALID_ARG, "train: mode");
-  if (!y && mode != HDC_TRAIN_KMEANS) return fail(h, HDC_ERR_INVALID_ARG, "train: y is NULL");
+  if (!y && N > 0 && mode != HDC_TRAIN_KMEANS) return fail(h, HDC_ERR_INVALID_ARG, "train: y is NULL");
   if (batch < 0) return fail(h, HDC_ERR_INVALID_ARG, "train: batch < 0");
   hdc_knobs_t k;
   if (!knobs) return fail(h, HDC_ERR_INVALID_ARG, "knobs is NULL");
