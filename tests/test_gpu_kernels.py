@@ -88,6 +88,29 @@ def test_levelid_bit_exact(hd, h, N, F, Q, D, D_eff):
         assert (host_words(H)[:, W - 1] >> (D_eff % 32) == 0).all()
 
 
+@pytest.mark.parametrize("zeros", [0.8, 0.97, 1.0])
+@pytest.mark.parametrize("N,F,Q,D,D_eff", [(200, 784, 256, 10000, 10000), (97, 100, 16, 3000, 2049), (50, 36, 256, 1100, 1000),
+                                           (130, 1020, 256, 200, 33), (49, 4, 3, 64, 64)])
+def test_levelid_sparse_path_bit_exact(hd, h, zeros, N, F, Q, D, D_eff):
+    """Mostly-zero level rows take the sparse path of the fast kernel (per-warp decision, base counter +
+    listed features); a few fully dense rows mixed in exercise the per-warp fallback and the list
+    capacity guard.  Bit-exact against the oracle either way."""
+    r = rng(13, N, F, Q, D_eff, int(zeros * 100))
+    lv = r.integers(1, Q, size=(N, F), dtype=np.uint8)
+    lv[r.random((N, F)) < zeros] = 0
+    lv[5 % N] = r.integers(1, Q, size=F, dtype=np.uint8)      # one fully dense sample
+    if N > 60:
+        lv[48:52] = r.integers(0, Q, size=(4, F), dtype=np.uint8)   # a dense group of four
+    ID = r.integers(0, 2, size=(F, D), dtype=np.uint8)
+    LV = gen.level_table(9, Q, D)
+    bits_or = O.encode_levelid(lv, ID, LV, D_eff)
+    H = h.hdc_encode_levelid(dev(lv), dev_bits(ID), dev_bits(LV), D, hd.knobs(D_eff))
+    assert np.array_equal(host_bits(H, D_eff), bits_or)
+    W = (D_eff + 31) // 32
+    if D_eff % 32:
+        assert (host_words(H)[:, W - 1] >> (D_eff % 32) == 0).all()
+
+
 # ------------------------------------------------------------------------------------ RP encode
 def _encode(hd, h, X, P, D_eff, prec, flags=0, bf16_inputs=False):
     kn = hd.knobs(D_eff, precision=prec, flags=flags)
