@@ -183,7 +183,8 @@ def test_encode_rp_bf16_inputs_in_place(hd, h):
 @pytest.mark.parametrize("sim", ["DOT", "COS"])
 @pytest.mark.parametrize("hv_bits", [32, 16, 8, 1])
 @pytest.mark.parametrize("N,K,D,D_eff", [(150, 26, 2100, 2100), (64, 6, 10000, 4099), (33, 1, 500, 500),
-                                         (140, 70, 1300, 1000)])
+                                         (140, 70, 1300, 1000), (140, 600, 1300, 1000), (300, 200, 700, 640),
+                                         (130, 1000, 520, 520)])
 def test_dot_cos_similarity_and_classify(hd, h, sim, hv_bits, N, K, D, D_eff):
     r = rng(5, N, K, D_eff, hv_bits)
     hb = r.integers(0, 2, size=(N, D), dtype=np.uint8)
