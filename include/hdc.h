@@ -208,6 +208,24 @@ int32_t hdc_train_epoch(hdc_handle_t h, int32_t mode, const uint32_t* Hbits, int
                         int32_t D, const hdc_knobs_t* knobs, float lr, int64_t batch, int32_t* pred,
                         unsigned long long* n_wrong, void* ws, size_t ws_bytes, void* stream);
 
+/* ---- (3c) the two halves of a retraining mini-batch, for data-parallel training ------------------
+ * hdc_train_epoch(PERCEPTRON) is, per mini-batch, hdc_train_delta followed by hdc_train_apply.
+ * With the mini-batch split over several GPUs every rank calls hdc_train_delta
+ * on its shard, the int32 deltas are summed across ranks (one all-reduce of K*W*32 integers: integer
+ * addition, so the result does not depend on the order), and every rank calls hdc_train_apply with
+ * the summed delta: the replicas of C_acc stay bit-identical.
+ *  hdc_train_delta: yhat = classify(h) with C_acc at knobs->{hv_bits, sim, perforation};
+ *      delta[k][d] = sum_{n < N, yhat_n != y_n} ([k = y_n] - [k = yhat_n]) * v[n,d], written (not
+ *      accumulated) as int32 [K][W*32], W = ceil(D_eff/32); pred (nullable) receives yhat; n_wrong
+ *      (nullable) is incremented.  N == 0 writes zeros.  Workspace: HDC_OP_TRAIN_EPOCH for N.
+ *  hdc_train_apply: C_acc[k,d] = fl32(C_acc[k,d] + fl32(lr * (float)delta[k][d])) for d < D_eff. */
+int32_t hdc_train_delta(hdc_handle_t h, const uint32_t* Hbits, int64_t N, int64_t ldh_words,
+                        const int32_t* y, const float* C_acc, int32_t K, int64_t ldc, int32_t D,
+                        const hdc_knobs_t* knobs, int32_t* delta, int32_t* pred,
+                        unsigned long long* n_wrong, void* ws, size_t ws_bytes, void* stream);
+int32_t hdc_train_apply(hdc_handle_t h, float* C_acc, int32_t K, int64_t ldc, int32_t D,
+                        const hdc_knobs_t* knobs, const int32_t* delta, float lr, void* stream);
+
 /* ---- end-to-end inference from host buffers ------------------------------------------------
  * encode_rp + classify for N queries whose features live in HOST memory (pinned for full speed):
  * copies X_host in chunks to the device (inside the call), runs (1a)+(2)+(3a) and copies the

@@ -27,8 +27,8 @@ HDC_K_ENCODE_GEMM, HDC_K_SIM, HDC_K_LEVELID, HDC_K_CLASS_UPDATE = 0, 1, 2, 3
 
 EXPORTS = ("hdc_create", "hdc_destroy", "hdc_last_error", "hdc_version", "hdc_launch_count",
            "hdc_workspace_bytes", "hdc_encode_rp", "hdc_encode_levelid", "hdc_similarity",
-           "hdc_classify", "hdc_train_epoch", "hdc_infer_rp_host", "hdc_kernel_timing",
-           "hdc_kernel_time")
+           "hdc_classify", "hdc_train_epoch", "hdc_train_delta", "hdc_train_apply", "hdc_infer_rp_host",
+           "hdc_kernel_timing", "hdc_kernel_time")
 
 
 class hdc_knobs_t(C.Structure):
@@ -82,6 +82,10 @@ def lib() -> C.CDLL:
     L.hdc_train_epoch.argtypes = [vp, i32, vp, i64, i64, vp, vp, i32, i64, i32, kp, C.c_float, i64, vp, vp,
                                   vp, sz, vp]
     L.hdc_train_epoch.restype = i32
+    L.hdc_train_delta.argtypes = [vp, vp, i64, i64, vp, vp, i32, i64, i32, kp, vp, vp, vp, vp, sz, vp]
+    L.hdc_train_delta.restype = i32
+    L.hdc_train_apply.argtypes = [vp, vp, i32, i64, i32, kp, vp, C.c_float, vp]
+    L.hdc_train_apply.restype = i32
     L.hdc_infer_rp_host.argtypes = [vp, vp, i32, i64, i32, i64, vp, i32, i32, i64, vp, i32, i64, kp, vp, vp,
                                     sz, vp]
     L.hdc_infer_rp_host.restype = i32
@@ -246,6 +250,27 @@ class Handle:
                                      _ptr(C_acc), K, _rowmajor(C_acc, "C_acc"), D, C.byref(kn),
                                      C.c_float(lr), int(batch or 0), _ptr(pred), _ptr(n_wrong), ws, wsb,
                                      self._stream())
+        self._check(rc)
+        return C_acc
+
+    def hdc_train_delta(self, Hbits, y, C_acc, kn: hdc_knobs_t, delta=None, pred=None, n_wrong=None):
+        """int32 [K][W*32] class update of these samples against the current C_acc (not applied)."""
+        N = Hbits.shape[0]
+        K, D = C_acc.shape
+        W = (kn.D_eff + 31) // 32
+        if delta is None:
+            delta = torch.empty((K, W * 32), dtype=torch.int32, device=self.device)
+        ws, wsb = self._workspace(self.workspace_bytes(HDC_OP_TRAIN_EPOCH, max(N, 1), 0, D, K, kn))
+        rc = self._L.hdc_train_delta(self._h, _ptr(Hbits), N, _rowmajor(Hbits, "Hbits") if N else W, _ptr(y),
+                                     _ptr(C_acc), K, _rowmajor(C_acc, "C_acc"), D, C.byref(kn), _ptr(delta),
+                                     _ptr(pred), _ptr(n_wrong), ws, wsb, self._stream())
+        self._check(rc)
+        return delta
+
+    def hdc_train_apply(self, C_acc, kn: hdc_knobs_t, delta, lr: float):
+        K, D = C_acc.shape
+        rc = self._L.hdc_train_apply(self._h, _ptr(C_acc), K, _rowmajor(C_acc, "C_acc"), D, C.byref(kn),
+                                     _ptr(delta), C.c_float(lr), self._stream())
         self._check(rc)
         return C_acc
 

@@ -703,6 +703,45 @@ extern "C" int32_t hdc_train_epoch(hdc_handle_t h, int32_t mode, const uint32_t*
   return HDC_OK;
 }
 
+// =================================================================================== (3c) split for data-parallel training
+extern "C" int32_t hdc_train_delta(hdc_handle_t h, const uint32_t* Hbits, int64_t N, int64_t ldh_words,
+                                   const int32_t* y, const float* C_acc, int32_t K, int64_t ldc, int32_t D,
+                                   const hdc_knobs_t* knobs, int32_t* delta, int32_t* pred,
+                                   unsigned long long* n_wrong, void* ws, size_t ws_bytes, void* stream) {
+  if (!h) return HDC_ERR_INVALID_ARG;
+  if (!delta) return fail(h, HDC_ERR_INVALID_ARG, "train_delta: delta is NULL");
+  if (!y && N > 0) return fail(h, HDC_ERR_INVALID_ARG, "train_delta: y is NULL");
+  int rc = check_sim_args(h, Hbits, N, ldh_words, C_acc, K, ldc, D, knobs);
+  if (rc) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  Bump b(ws);
+  if (!ws) ws_bytes = 0;
+  int32_t* pb = pred;
+  if (!pb && N > 0) pb = b.take<int32_t>((size_t)N);
+  if (b.off > ws_bytes) return fail(h, HDC_ERR_WORKSPACE, "train_delta: workspace too small");
+  if (N > 0) {
+    rc = do_similarity(h, Hbits, N, ldh_words, C_acc, K, ldc, knobs, nullptr, 0, 0, pb, nullptr, nullptr, b, ws_bytes,
+                       st);
+    if (rc) return rc;
+  }
+  Timed tm(h, HDC_K_CLASS_UPDATE, st);
+  cudaError_t ce = launch_class_delta(Hbits, 0, N, ldh_words, y, pb, K, knobs->D_eff, delta, n_wrong, h->sm_count, st,
+                                      &h->launches);
+  return ce == cudaSuccess ? HDC_OK : cuda_fail(h, ce, "train_delta");
+}
+
+extern "C" int32_t hdc_train_apply(hdc_handle_t h, float* C_acc, int32_t K, int64_t ldc, int32_t D,
+                                   const hdc_knobs_t* knobs, const int32_t* delta, float lr, void* stream) {
+  if (!h) return HDC_ERR_INVALID_ARG;
+  if (!C_acc || !delta) return fail(h, HDC_ERR_INVALID_ARG, "train_apply: NULL pointer");
+  if (K < 1 || K > 65535 || D < 1 || ldc < D) return fail(h, HDC_ERR_INVALID_ARG, "train_apply: bad sizes");
+  int rc = check_knobs(h, knobs, D);
+  if (rc) return rc;
+  cudaError_t ce = launch_apply_update(C_acc, K, ldc, knobs->D_eff, delta, lr, h->sm_count, (cudaStream_t)stream,
+                                       &h->launches);
+  return ce == cudaSuccess ? HDC_OK : cuda_fail(h, ce, "train_apply");
+}
+
 // =================================================================================== host end-to-end
 extern "C" int32_t hdc_infer_rp_host(hdc_handle_t h, const void* X_host, int32_t x_dtype, int64_t N, int32_t F,
                                      int64_t ldx, const void* P, int32_t p_dtype, int32_t D, int64_t ldp,

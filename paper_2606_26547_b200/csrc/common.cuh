@@ -146,6 +146,13 @@ cudaError_t launch_class_update(const uint32_t* Hbits, int64_t n0, int64_t nb, i
                                 unsigned long long* n_wrong, int sm_count, cudaStream_t st,
                                 int64_t* nlaunch);
 
+// the two halves of launch_class_update (multi-GPU training exchanges delta between them)
+cudaError_t launch_class_delta(const uint32_t* Hbits, int64_t n0, int64_t nb, int64_t ldh, const int32_t* y,
+                               const int32_t* pred, int K, int D_eff, int32_t* delta,
+                               unsigned long long* n_wrong, int sm_count, cudaStream_t st, int64_t* nlaunch);
+cudaError_t launch_apply_update(float* C_acc, int K, int64_t ldc, int D_eff, const int32_t* delta, float lr,
+                                int sm_count, cudaStream_t st, int64_t* nlaunch);
+
 // HD-Clustering re-bundle step (train.cu): counts members per cluster (members: int32 [K] workspace),
 // adds the number of samples with assign != prev to *n_changed (both nullable) and zeroes the
 // accumulator rows of the clusters that have members

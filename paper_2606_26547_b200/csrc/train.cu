@@ -154,17 +154,15 @@ cudaError_t launch_kmeans_reset(const int32_t* assign, const int32_t* prev, int6
   return cudaGetLastError();
 }
 
-// delta: int32 [K][W*32] workspace (zeroed here).
-cudaError_t launch_class_update(const uint32_t* Hbits, int64_t n0, int64_t nb, int64_t ldh,
-                                const int32_t* y, const int32_t* pred, float* C_acc, int K,
-                                int64_t ldc, int D_eff, float lr, int32_t* delta,
-                                unsigned long long* n_wrong, int sm_count, cudaStream_t st,
-                                int64_t* nlaunch) {
-  if (nb <= 0) return cudaSuccess;
+// delta: int32 [K][W*32] (zeroed here, then filled): the exact integer class update of samples
+// [n0, n0+nb); n_wrong (nullable) is incremented by the mispredictions among them.
+cudaError_t launch_class_delta(const uint32_t* Hbits, int64_t n0, int64_t nb, int64_t ldh, const int32_t* y,
+                               const int32_t* pred, int K, int D_eff, int32_t* delta,
+                               unsigned long long* n_wrong, int sm_count, cudaStream_t st, int64_t* nlaunch) {
   const int W = words_of(D_eff);
   const int64_t ldd = (int64_t)W * 32;
   cudaError_t e = cudaMemsetAsync(delta, 0, sizeof(int32_t) * (size_t)K * ldd, st);
-  if (e != cudaSuccess) return e;
+  if (e != cudaSuccess || nb <= 0) return e;
   const int gx = (W + WT - 1) / WT;
   // split the samples into segments so that about 4 CTAs per SM exist; each segment >= 64 samples
   int64_t segs = ((int64_t)sm_count * 4 + (int64_t)gx * K - 1) / ((int64_t)gx * K);
@@ -180,13 +178,6 @@ cudaError_t launch_class_update(const uint32_t* Hbits, int64_t n0, int64_t nb, i
   ++*nlaunch;
   e = cudaGetLastError();
   if (e != cudaSuccess) return e;
-  const int64_t total = (int64_t)K * D_eff;
-  int64_t g = (total + 255) / 256;
-  if (g > sm_count * 8) g = sm_count * 8;
-  apply_update_kernel<<<(unsigned)g, 256, 0, st>>>(C_acc, K, D_eff, ldc, delta, ldd, lr);
-  ++*nlaunch;
-  e = cudaGetLastError();
-  if (e != cudaSuccess) return e;
   if (n_wrong && pred) {
     int64_t gw = (nb + 255) / 256;
     if (gw > sm_count * 4) gw = sm_count * 4;
@@ -195,6 +186,29 @@ cudaError_t launch_class_update(const uint32_t* Hbits, int64_t n0, int64_t nb, i
     e = cudaGetLastError();
   }
   return e;
+}
+
+// C_acc[k,d] = fl32(C_acc[k,d] + fl32(lr * (float)delta[k,d])) for d < D_eff
+cudaError_t launch_apply_update(float* C_acc, int K, int64_t ldc, int D_eff, const int32_t* delta, float lr,
+                                int sm_count, cudaStream_t st, int64_t* nlaunch) {
+  const int64_t ldd = (int64_t)words_of(D_eff) * 32;
+  const int64_t total = (int64_t)K * D_eff;
+  int64_t g = (total + 255) / 256;
+  if (g > sm_count * 8) g = sm_count * 8;
+  apply_update_kernel<<<(unsigned)g, 256, 0, st>>>(C_acc, K, D_eff, ldc, delta, ldd, lr);
+  ++*nlaunch;
+  return cudaGetLastError();
+}
+
+cudaError_t launch_class_update(const uint32_t* Hbits, int64_t n0, int64_t nb, int64_t ldh,
+                                const int32_t* y, const int32_t* pred, float* C_acc, int K,
+                                int64_t ldc, int D_eff, float lr, int32_t* delta,
+                                unsigned long long* n_wrong, int sm_count, cudaStream_t st,
+                                int64_t* nlaunch) {
+  if (nb <= 0) return cudaSuccess;
+  cudaError_t e = launch_class_delta(Hbits, n0, nb, ldh, y, pred, K, D_eff, delta, n_wrong, sm_count, st, nlaunch);
+  if (e != cudaSuccess) return e;
+  return launch_apply_update(C_acc, K, ldc, D_eff, delta, lr, sm_count, st, nlaunch);
 }
 
 }  // namespace hdc

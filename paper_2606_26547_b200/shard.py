@@ -64,3 +64,23 @@ def classify_sharded(classify_rows: Callable[[int, int], torch.Tensor], n_total:
     local = classify_rows(lo, hi)
     assert local.numel() == hi - lo
     return gather_labels(local, n_total)
+
+
+def train_epoch_sharded(delta_fn: Callable[[int, int], torch.Tensor], apply_fn: Callable[[torch.Tensor], None],
+                        n_total: int, batch: int = 0) -> None:
+    """One data-parallel retraining epoch: the samples of every mini-batch are
+    split over the ranks (shard_bounds inside the mini-batch), `delta_fn(lo, hi)` returns this rank's
+    int32 class update of global samples [lo, hi) against the current accumulators (hdc_train_delta),
+    the deltas are summed over the ranks with ONE all-reduce per mini-batch, and `apply_fn(delta)`
+    applies the sum (hdc_train_apply).  Integer addition commutes, so every rank applies the same
+    delta and the replicas of the class accumulators stay bit-identical to a single-GPU epoch."""
+    world = dist.get_world_size() if dist.is_initialized() else 1
+    rank = dist.get_rank() if dist.is_initialized() else 0
+    B = n_total if batch in (0, None) or batch > n_total else int(batch)
+    for b0 in range(0, n_total, B):
+        nb = min(B, n_total - b0)
+        lo, hi = shard_bounds(nb, world, rank)
+        delta = delta_fn(b0 + lo, b0 + hi)
+        if world > 1:
+            dist.all_reduce(delta, op=dist.ReduceOp.SUM)
+        apply_fn(delta)

@@ -440,3 +440,54 @@ def test_perforation_argument_errors(hd, h):
     with pytest.raises(hd.HdcError) as ei:                  # CUDA-core DOT / COS kernels are not perforated
         h.hdc_classify(Hd, Cd, hd.knobs(128, hv_bits=32, sim=hd.HDC_SIM_COS, flags=hd.HDC_FLAG_SIMT, perf_stride=2))
     assert ei.value.code == hd.HDC_ERR_UNSUPPORTED
+
+
+# ------------------------------------------------------------------------------------ data-parallel training
+@pytest.mark.parametrize("hv_bits,sim", [(1, "HAMMING"), (8, "COS"), (32, "COS"), (16, "COS")])
+@pytest.mark.parametrize("B", [0, 100])
+def test_train_delta_plus_apply_equals_train_epoch(hd, h, hv_bits, sim, B):
+    """hdc_train_epoch(PERCEPTRON) = per mini-batch hdc_train_delta + hdc_train_apply; and the delta of
+    a mini-batch is the integer sum of the deltas of its shards (two "ranks" emulated one after the
+    other on this GPU -- predictions depend only on the current C_acc), so data-parallel replicas
+    that all-reduce the int32 delta stay bit-identical to the single-GPU epoch."""
+    w = gen.c1_tiny(D=512)
+    hb, _, _ = O.encode_rp(w["Xtr"], w["P"], 512, O.F32)
+    y = w["ytr"].copy()
+    y[::4] = (y[::4] + 1) % w["K"]
+    N, K, D_eff = len(y), w["K"], 500
+    kn = hd.knobs(D_eff, hv_bits=hv_bits, sim=getattr(hd, "HDC_SIM_" + sim))
+    C0 = O.bundle(hb, y, K, 512)
+    Hd, yd = dev_bits(hb), dev(y)
+    C_ref, C_split, C_shard = dev(C0.copy()), dev(C0.copy()), dev(C0.copy())
+    nw_ref = torch.zeros(1, dtype=torch.int64, device="cuda")
+    nw_shard = torch.zeros(1, dtype=torch.int64, device="cuda")
+    for _ in range(2):
+        h.hdc_train_epoch(hd.HDC_TRAIN_PERCEPTRON, Hd, yd, C_ref, kn, lr=0.05, batch=B, n_wrong=nw_ref)
+        Bb = N if B == 0 else B
+        for b0 in range(0, N, Bb):
+            b1 = min(N, b0 + Bb)
+            d = h.hdc_train_delta(Hd[b0:b1], yd[b0:b1], C_split, kn)
+            h.hdc_train_apply(C_split, kn, d, 0.05)
+            mid = b0 + (b1 - b0 + 1) // 2                          # shard_bounds of two ranks
+            d0 = h.hdc_train_delta(Hd[b0:mid], yd[b0:mid], C_shard, kn, n_wrong=nw_shard).clone()
+            d1 = h.hdc_train_delta(Hd[mid:b1], yd[mid:b1], C_shard, kn, n_wrong=nw_shard)
+            h.hdc_train_apply(C_shard, kn, d0 + d1, 0.05)          # what the all-reduce hands every rank
+        assert torch.equal(C_split, C_ref)
+        assert torch.equal(C_shard, C_ref)
+    assert int(nw_shard.item()) == int(nw_ref.item())
+    # and the oracle agrees on the integer paths
+    if hv_bits in (1, 8):
+        C_or = C0[:, :D_eff].copy()
+        for _ in range(2):
+            C_or, _, _ = O.train_epoch(hb, y, C_or, D_eff, hv_bits, getattr(O, "SIM_" + sim), 0.05, B)
+        assert np.array_equal(C_ref.cpu().numpy()[:, :D_eff], C_or)
+
+
+def test_train_delta_of_an_empty_shard_is_zero(hd, h):
+    kn = hd.knobs(128, hv_bits=1, sim=hd.HDC_SIM_HAMMING)
+    Cc = torch.ones((3, 128), dtype=torch.float32, device="cuda")
+    H0 = torch.zeros((0, 4), dtype=torch.int32, device="cuda")
+    y0 = torch.zeros(0, dtype=torch.int32, device="cuda")
+    d = torch.full((3, 128), 7, dtype=torch.int32, device="cuda")
+    h.hdc_train_delta(H0, y0, Cc, kn, delta=d)
+    assert int(d.abs().sum().item()) == 0

@@ -82,3 +82,52 @@ def test_single_process_paths_need_no_group():
     lab = shard.classify_sharded(lambda lo, hi: torch.arange(lo, hi, dtype=torch.int32), 5)
     assert lab.tolist() == [0, 1, 2, 3, 4]
     assert shard.max_over_ranks(2.5) == 2.5
+
+
+def _train_worker(rank: int, world: int, port: int, out_dir: str):
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        n_total, batch = 103, 40
+        state = {"C": torch.zeros(4, dtype=torch.int64), "calls": []}
+
+        def delta_fn(lo, hi):                      # stand-in for hdc_train_delta: depends on the rows and on C
+            state["calls"].append((lo, hi))
+            idx = torch.arange(lo, hi, dtype=torch.int64)
+            d = torch.zeros(4, dtype=torch.int64)
+            d.index_add_(0, idx % 4, idx + state["C"].sum())
+            return d
+
+        def apply_fn(d):                           # stand-in for hdc_train_apply
+            state["C"] = state["C"] + d
+
+        shard.train_epoch_sharded(delta_fn, apply_fn, n_total, batch)
+        torch.save((state["C"], state["calls"]), os.path.join(out_dir, f"train_{rank}.pt"))
+        dist.barrier()
+    finally:
+        dist.destroy_process_group()
+
+
+def test_two_gloo_ranks_train_epoch_all_reduces_one_delta_per_mini_batch(tmp_path):
+    world = 2
+    mp.spawn(_train_worker, args=(world, _free_port(), str(tmp_path)), nprocs=world, join=True)
+    C0, calls0 = torch.load(os.path.join(str(tmp_path), "train_0.pt"))
+    C1, calls1 = torch.load(os.path.join(str(tmp_path), "train_1.pt"))
+    assert torch.equal(C0, C1)                                         # identical replicas
+    # single-process run of the same stand-ins
+    state = {"C": torch.zeros(4, dtype=torch.int64)}
+
+    def delta_fn(lo, hi):
+        idx = torch.arange(lo, hi, dtype=torch.int64)
+        d = torch.zeros(4, dtype=torch.int64)
+        d.index_add_(0, idx % 4, idx + state["C"].sum())
+        return d
+
+    def apply_fn(d):
+        state["C"] = state["C"] + d
+
+    shard.train_epoch_sharded(delta_fn, apply_fn, 103, 40)
+    assert torch.equal(state["C"], C0)
+    # each mini-batch was split in two contiguous shards that tile it
+    assert calls0 == [(0, 20), (40, 60), (80, 92)] and calls1 == [(20, 40), (60, 80), (92, 103)]
