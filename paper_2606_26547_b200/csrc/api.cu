@@ -262,6 +262,8 @@ int do_similarity(hdc_ctx* h, const uint32_t* Hbits, int64_t N, int64_t ldh, con
     if (k->sim == HDC_SIM_COS) colscale = b.take<double>((size_t)K);
     float* amax = b.take<float>(1);
     void* cop = b.take<uint8_t>(sim_tc_operand_bytes(K, k->hv_bits, D_eff));
+    const size_t pbytes = sim_tc_partial_bytes(N, K, k->hv_bits, D_eff, h->sm_count);
+    double* partial = pbytes ? b.take<double>(pbytes / sizeof(double)) : nullptr;
     if (b.off > ws_bytes) return fail(h, HDC_ERR_WORKSPACE, "similarity: workspace too small");
     if (colscale) {
       // norms over the operand as the contraction sees it (permutation-invariant)
@@ -294,8 +296,8 @@ int do_similarity(hdc_ctx* h, const uint32_t* Hbits, int64_t N, int64_t ldh, con
     }
     {
       Timed tm(h, HDC_K_SIM, st);
-      ce = launch_sim_tc(h->tc, Hbits, N, ldh, C_acc, K, ldc, D_eff, k->hv_bits, cop, amax, e, pf, h->sm_count, st,
-                         &h->launches);
+      ce = launch_sim_tc(h->tc, Hbits, N, ldh, C_acc, K, ldc, D_eff, k->hv_bits, cop, amax, e, pf, partial,
+                         h->sm_count, st, &h->launches);
     }
     if (ce == cudaSuccess) return HDC_OK;
     if (ce != cudaErrorNotSupported) return cuda_fail(h, ce, "similarity tcgen05");
@@ -368,8 +370,13 @@ int do_similarity(hdc_ctx* h, const uint32_t* Hbits, int64_t N, int64_t ldh, con
   return ce == cudaSuccess ? HDC_OK : cuda_fail(h, ce, "similarity contraction");
 }
 
-size_t similarity_ws(int K, const hdc_knobs_t* k) {
+size_t similarity_ws(int64_t N, int K, const hdc_knobs_t* k) {
   Bump b(nullptr);
+  {  // split-D partial sums (simtc.cu): at most 8 splits and 64 MB, for any sub-batch of up to N queries
+    size_t pb = (size_t)8 * (size_t)(N > 0 ? N : 1) * (size_t)K * sizeof(double);
+    if (pb > ((size_t)64 << 20)) pb = (size_t)64 << 20;
+    b.take<double>(pb / sizeof(double));
+  }
   const int W = words_of(k->D_eff);
   b.take<double>((size_t)K);
   b.take<int8_t>((size_t)K * round_up(k->D_eff, 16));
@@ -485,12 +492,12 @@ extern "C" size_t hdc_workspace_bytes(hdc_handle_t h, int32_t op, int64_t N, int
       return 0;
     case HDC_OP_SIMILARITY:
     case HDC_OP_CLASSIFY:
-      return similarity_ws(K, &k);
+      return similarity_ws(N, K, &k);
     case HDC_OP_TRAIN_EPOCH: {
       b.take<int32_t>((size_t)K * words_of(k.D_eff) * 32);  // Delta
       b.take<int32_t>((size_t)N);                           // predictions of one mini-batch
       b.take<int32_t>((size_t)K);                           // members per cluster (HDC_TRAIN_KMEANS)
-      return b.off + 256 + similarity_ws(K, &k);
+      return b.off + 256 + similarity_ws(N, K, &k);
     }
     case HDC_OP_INFER_RP_HOST: {
       const int64_t chunk = N < HOST_CHUNK ? N : HOST_CHUNK;
@@ -500,7 +507,7 @@ extern "C" size_t hdc_workspace_bytes(hdc_handle_t h, int32_t op, int64_t N, int
       b.take<int32_t>((size_t)N);
       EncodePlan pl;
       plan_encode(h, chunk, F_or_Q, k.D_eff, &k, false, false, b, pl);
-      return b.off + 512 + similarity_ws(K, &k);
+      return b.off + 512 + similarity_ws(chunk, K, &k);
     }
     default:
       return 0;

@@ -65,6 +65,9 @@ struct SimParams {
   int nparts;   // 1, or 3 for the fp32 class operand
   int m_tiles, n_tiles;
   int num_kb;
+  int splits;       // CTAs that share one m-tile, each reducing kbs k-blocks (split-D for small N)
+  int kbs;          // k-blocks per split (multiple of 16)
+  double* partial;  // [splits][N][K] partial sums when splits > 1
   int kps;          // k-blocks per pipeline group
   int stages;       // ring depth
   int stage_bytes;  // A_BYTES + nparts*kc*KB_BYTES
@@ -123,8 +126,17 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot_ptr;
 
+  // work item = (m-tile, split of the reduction axis); a CTA walks items blockIdx.x, +gridDim.x, ...
+  const int64_t n_items = (int64_t)p.m_tiles * p.splits;
   const int64_t tiles_per_cta =
-      (p.m_tiles > (int)blockIdx.x) ? ((int64_t)(p.m_tiles - 1 - (int)blockIdx.x) / gridDim.x + 1) * p.n_tiles : 0;
+      (n_items > (int64_t)blockIdx.x) ? ((n_items - 1 - (int64_t)blockIdx.x) / gridDim.x + 1) * p.n_tiles : 0;
+  auto item_of = [&](int64_t i, int& mt, int& sp, int& kb_lo, int& kb_hi) {
+    const int64_t item = (int64_t)blockIdx.x + (i / p.n_tiles) * (int64_t)gridDim.x;
+    mt = (int)(item / p.splits);
+    sp = (int)(item - (int64_t)mt * p.splits);
+    kb_lo = sp * p.kbs;
+    kb_hi = kb_lo + p.kbs < p.num_kb ? kb_lo + p.kbs : p.num_kb;
+  };
 
   if (warp == 0) {
     // ================================================================= TMA producer (class tiles)
@@ -132,8 +144,10 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
     uint32_t phase = 0;
     for (int64_t i = 0; i < tiles_per_cta; ++i) {
       const int nt = (int)(i % p.n_tiles);
-      for (int kb0 = 0; kb0 < p.num_kb; kb0 += G) {
-        const int n = p.num_kb - kb0 < G ? p.num_kb - kb0 : G;
+      int mt, sp, kb_lo, kb_hi;
+      item_of(i, mt, sp, kb_lo, kb_hi);
+      for (int kb0 = kb_lo; kb0 < kb_hi; kb0 += G) {
+        const int n = kb_hi - kb0 < G ? kb_hi - kb0 : G;
         mbar_wait(empty_bar(grp), phase ^ 1u);
         mbar_arrive_expect_tx_elect(full_bar(grp), (uint32_t)(n * nb_rows) * KB_BYTES);
         for (int u = 0; u < n; ++u)
@@ -156,8 +170,10 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
       mbar_wait(tempty_bar(acc), acc_phase ^ 1u);
       tc_fence_after();
       const uint32_t d_tmem = tmem_base + (uint32_t)(acc * BN_MAX);
-      for (int kb0 = 0; kb0 < p.num_kb; kb0 += G) {
-        const int n = p.num_kb - kb0 < G ? p.num_kb - kb0 : G;
+      int mt, sp, kb_lo, kb_hi;
+      item_of(i, mt, sp, kb_lo, kb_hi);
+      for (int kb0 = kb_lo; kb0 < kb_hi; kb0 += G) {
+        const int n = kb_hi - kb0 < G ? kb_hi - kb0 : G;
         mbar_wait(full_bar(grp), phase);
         tc_fence_after();
         // whole warp, converged: each call issues once (tc_ptx.cuh, *_elect)
@@ -166,10 +182,10 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
           const uint64_t da = smem_desc(sa), db = smem_desc(sa + A_BYTES);
 #pragma unroll
           for (int k = 0; k < KB_BYTES / 32; ++k)
-            tc_mma_elect<INT8>(d_tmem, da + 2u * k, db + 2u * k, idesc, ((kb0 + u) | k) != 0 ? 1u : 0u);
+            tc_mma_elect<INT8>(d_tmem, da + 2u * k, db + 2u * k, idesc, (kb0 + u != kb_lo || k != 0) ? 1u : 0u);
         }
         tc_commit_elect(empty_bar(grp));  // frees the group's slots when these MMAs retire
-        if (kb0 + n == p.num_kb) tc_commit_elect(tfull_bar(acc));
+        if (kb0 + n == kb_hi) tc_commit_elect(tfull_bar(acc));
         if (++grp == NG) {
           grp = 0;
           phase ^= 1u;
@@ -187,7 +203,8 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
     uint32_t acc_phase = 0;
     Top2 run = Top2{NEG_BIG, INT_MAX, NEG_BIG};
     for (int64_t i = 0; i < tiles_per_cta; ++i) {
-      const int mt = (int)blockIdx.x + (int)(i / p.n_tiles) * (int)gridDim.x;
+      int mt, sp, kb_lo, kb_hi;
+      item_of(i, mt, sp, kb_lo, kb_hi);
       const int nt = (int)(i % p.n_tiles);
       const int64_t row = (int64_t)mt * BM + q * 32 + lane;
       const bool row_ok = row < p.N;
@@ -217,7 +234,11 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
             } else {
               a = (double)__uint_as_float(v0[j]);
             }
-            if (EPI == EPI_SCORE) {
+            if (p.splits > 1) {
+              // partial sum of this split of the reduction axis; split_reduce_kernel adds the splits
+              // in a fixed order and applies the epilogue
+              if (row_ok) p.partial[((int64_t)sp * p.N + row) * p.K + k] = a;
+            } else if (EPI == EPI_SCORE) {
               if (row_ok) {
                 if (p.e.s_i32) {
                   int iv = (int)v0[j];
@@ -248,7 +269,7 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
         acc = 0;
         acc_phase ^= 1u;
       }
-      if (EPI == EPI_ARGMAX && nt == p.n_tiles - 1) {
+      if (EPI == EPI_ARGMAX && nt == p.n_tiles - 1 && p.splits == 1) {
         if (row_ok) {
           double b1 = run.b1, b2 = run.b2;
           if (b2 == NEG_BIG) b2 = b1;  // K == 1
@@ -280,15 +301,15 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
     const uint32_t sw = (uint32_t)(t & 7);
     const uint32_t q_smem = bar0 + 256u;      // ring base (after the barriers)
     const uint32_t* q_ptr = reinterpret_cast<const uint32_t*>(smem_raw + (q_smem - smem_u32(smem_raw)));
-    const int nch = (p.num_kb + KPC - 1) / KPC;
-    const int64_t steps = tiles_per_cta * nch;
-
-    int64_t is_i = 0;   // producer cursor: tile, chunk, ring slot
+    int64_t is_i = 0;   // producer cursor: tile, chunk of the tile's k-block range, ring slot
     int is_c = 0, is_slot = 0;
     auto issue = [&]() {
-      const int mt = (int)blockIdx.x + (int)(is_i / p.n_tiles) * (int)gridDim.x;
+      if (is_i >= tiles_per_cta) return;
+      int mt, sp, kb_lo, kb_hi;
+      item_of(is_i, mt, sp, kb_lo, kb_hi);
+      const int nch = (kb_hi - kb_lo + KPC - 1) / KPC;
       const int64_t m0 = (int64_t)mt * BM;
-      const int w = is_c * QW + lane;
+      const int w = (kb_lo / KPC + is_c) * QW + lane;   // kbs is a multiple of KPC
       const int64_t rows_left = p.N - m0;
       const int nrow = w < p.W ? (rows_left < BM ? (int)rows_left : BM) : 0;
       const uint32_t* src = p.Hbits + (m0 + ew) * p.ldh + w;
@@ -309,7 +330,7 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
       }
     };
     for (int s0 = 0; s0 < Q_SLOTS - 1; ++s0) {
-      if (s0 < steps) issue();
+      issue();
       asm volatile("cp.async.commit_group;" ::: "memory");
     }
 
@@ -346,14 +367,17 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
       }
     };
     for (int64_t i = 0; i < tiles_per_cta; ++i) {
+      int mt, sp, kb_lo, kb_hi;
+      item_of(i, mt, sp, kb_lo, kb_hi);
+      const int nch = (kb_hi - kb_lo + KPC - 1) / KPC;
       for (int c = 0; c < nch; ++c, ++step) {
         asm volatile("cp.async.wait_group %0;" ::"n"(Q_SLOTS - 2) : "memory");
         asm volatile("bar.sync 1, %0;" ::"n"(32 * EXW) : "memory");  // tile visible; previous slot free
-        if (step + Q_SLOTS - 1 < steps) issue();
+        issue();
         asm volatile("cp.async.commit_group;" ::: "memory");
         // this thread's words of the chunk's first k-block (groups never straddle a chunk: G | KPC)
         const uint32_t* qk = q_ptr + slot * Q_SLOT_WORDS + t + part_id * (WPP * Q_LD);
-        int left = p.num_kb - c * KPC;
+        int left = (kb_hi - kb_lo) - c * KPC;
         if (left > KPC) left = KPC;
         while (left > 0) {
           const int n = left < G ? left : G;
@@ -445,6 +469,47 @@ __global__ void class_operand_kernel(const float* __restrict__ C, int K, int D_e
   }
 }
 
+// Adds the split partial sums in split order (fixed: deterministic) and applies the epilogue of
+// sim_tc_kernel: scores (S) or arg-max with best / runner-up.  One thread per query row.
+__global__ void split_reduce_kernel(const double* __restrict__ partial, int splits, int64_t N, int K, Epilogue e) {
+  const int64_t n = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (n >= N) return;
+  Top2 run = Top2{NEG_BIG, INT_MAX, NEG_BIG};
+  for (int k = 0; k < K; ++k) {
+    double a = 0.0;
+    for (int sp = 0; sp < splits; ++sp) a += partial[((int64_t)sp * N + n) * K + k];
+    if (e.kind == EPI_SCORE) {
+      if (e.s_i32) {
+        int iv = (int)a;
+        if (e.ham_D > 0) iv = (e.ham_D - iv) >> 1;
+        reinterpret_cast<int32_t*>(e.S)[n * e.lds + k] = iv;
+      } else {
+        reinterpret_cast<float*>(e.S)[n * e.lds + k] = e.colscale ? (float)(a * e.colscale[k]) : (float)a;
+      }
+    } else {
+      const double sc = e.colscale ? a * e.colscale[k] : a;
+      if (sc > run.b1) {
+        run.b2 = run.b1;
+        run.b1 = sc;
+        run.i1 = k;
+      } else if (sc > run.b2) {
+        run.b2 = sc;
+      }
+    }
+  }
+  if (e.kind == EPI_ARGMAX) {
+    double b1 = run.b1, b2 = run.b2;
+    if (b2 == NEG_BIG) b2 = b1;  // K == 1
+    if (e.ham_D > 0) {
+      b1 = 0.5 * ((double)e.ham_D - b1);
+      b2 = 0.5 * ((double)e.ham_D - b2);
+    }
+    e.labels[n] = run.i1;
+    if (e.best) e.best[n] = (float)b1;
+    if (e.second) e.second[n] = (float)b2;
+  }
+}
+
 template <bool INT8, int EPI>
 cudaError_t launch_one(const CUtensorMap& tmB, const SimParams& p, int grid, cudaStream_t st) {
   static bool attr_set = false;
@@ -479,9 +544,40 @@ size_t sim_tc_operand_bytes(int K, int hv_bits, int D_eff) {
   return (size_t)n_tiles * nparts * kc * num_kb * KB_BYTES;
 }
 
+// Split-D for small N: with fewer m-tiles than half the SMs, `splits` CTAs share an m-tile, each
+// reducing kbs k-blocks (a multiple of 16, so that splits start on ring-chunk boundaries); their
+// partial sums go through a [splits][N][K] double buffer.  Returns 1 when not worth it.
+int sim_tc_splits(int64_t N, int K, int hv_bits, int D_eff, int sm_count, int* kbs_out) {
+  int kc, nparts, n_tiles, num_kb;
+  bool int8;
+  sim_tc_shape(K, hv_bits, D_eff, kc, nparts, n_tiles, num_kb, int8);
+  const int64_t m_tiles = (N + BM - 1) / BM;
+  int splits = 1, kbs = num_kb;
+  if (n_tiles == 1 && m_tiles * 2 <= sm_count && num_kb >= 32) {
+    int want = (int)(sm_count / m_tiles);
+    if (want > 8) want = 8;
+    if (want > num_kb / 16) want = num_kb / 16;
+    if (want >= 2 && (size_t)want * (size_t)N * K * sizeof(double) <= ((size_t)64 << 20)) {
+      kbs = (int)round_up((num_kb + want - 1) / want, 16);
+      splits = (num_kb + kbs - 1) / kbs;
+      if (splits < 2) {
+        splits = 1;
+        kbs = num_kb;
+      }
+    }
+  }
+  if (kbs_out) *kbs_out = kbs;
+  return splits;
+}
+size_t sim_tc_partial_bytes(int64_t N, int K, int hv_bits, int D_eff, int sm_count) {
+  const int splits = sim_tc_splits(N, K, hv_bits, D_eff, sm_count, nullptr);
+  return splits > 1 ? (size_t)splits * (size_t)N * K * sizeof(double) : 0;
+}
+
 cudaError_t launch_sim_tc(TcContext* tc, const uint32_t* Hbits, int64_t N, int64_t ldh, const float* C_acc,
                           int K, int64_t ldc, int D_eff, int hv_bits, void* cop, float* amax_scratch,
-                          const Epilogue& e, Perf pf, int sm_count, cudaStream_t st, int64_t* nlaunch) {
+                          const Epilogue& e, Perf pf, double* partial, int sm_count, cudaStream_t st,
+                          int64_t* nlaunch) {
   if (!tc) return cudaErrorNotSupported;
   if (N <= 0) return cudaSuccess;
   if ((reinterpret_cast<uintptr_t>(cop) & 15) != 0) return cudaErrorNotSupported;
@@ -531,8 +627,19 @@ cudaError_t launch_sim_tc(TcContext* tc, const uint32_t* Hbits, int64_t N, int64
   p.kps = p.stages >= 8 ? 4 : (p.stages >= 4 ? 2 : 1);
   p.stages -= p.stages % p.kps;
   p.e = e;
-  const int grid = p.m_tiles < sm_count ? p.m_tiles : sm_count;
+  p.splits = partial ? sim_tc_splits(N, K, hv_bits, D_eff, sm_count, &p.kbs) : 1;
+  if (p.splits == 1) p.kbs = num_kb;
+  p.partial = partial;
+  const int64_t items = (int64_t)p.m_tiles * p.splits;
+  const int grid = (int)(items < sm_count ? items : sm_count);
   ++*nlaunch;
+  if (p.splits > 1) {
+    ce = int8 ? launch_one<true, EPI_SCORE>(tmB, p, grid, st) : launch_one<false, EPI_SCORE>(tmB, p, grid, st);
+    if (ce != cudaSuccess) return ce;
+    split_reduce_kernel<<<(unsigned)((N + 127) / 128), 128, 0, st>>>(partial, p.splits, N, K, e);
+    ++*nlaunch;
+    return cudaGetLastError();
+  }
   if (int8)
     return e.kind == EPI_SCORE ? launch_one<true, EPI_SCORE>(tmB, p, grid, st)
                                : launch_one<true, EPI_ARGMAX>(tmB, p, grid, st);
