@@ -36,7 +36,7 @@ def rng(*key):
 @pytest.mark.parametrize("N,K,D,D_eff", [(1, 1, 32, 32), (300, 4, 2048, 2048), (300, 4, 2048, 1024),
                                          (257, 26, 10000, 10000), (129, 10, 10000, 4099),
                                          (77, 40, 4500, 33), (64, 3, 100, 1), (50, 70, 2100, 2047),
-                                         (40, 5, 64, 31)])
+                                         (40, 5, 64, 31), (200, 70, 8192, 8000), (300, 100, 16384, 16384)])
 def test_hamming_similarity_and_classify(hd, h, N, K, D, D_eff):
     r = rng(1, N, K, D_eff)
     hb = r.integers(0, 2, size=(N, D), dtype=np.uint8)
