@@ -76,9 +76,9 @@ __device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* tm,
 // CTA; clearing bit 24 gives the same offset in the even (leader) CTA of the pair.
 constexpr uint32_t PEER_MASK = 0xFEFFFFFFu;
 __device__ __forceinline__ uint32_t cluster_ctarank() {
-  uint32_t r;
-  asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
-  return r;
+  // the compiler intrinsic (not inline asm): the value is known to be warp-uniform, which keeps the
+  // code it guards on the uniform datapath
+  return __clusterRelativeBlockRank();
 }
 __device__ __forceinline__ void cluster_sync_all() {
   asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
