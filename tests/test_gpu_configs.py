@@ -236,3 +236,34 @@ def test_c5_large_batch_launch_config_sampled(hd, h, variant):
         lab = h.hdc_classify(Hin, Cd, kn).cpu().numpy()[pos]
         assert np.array_equal(lab, lab_or)
     assert (lab_or[:ns] == w["y"][:ns]).mean() > 0.95
+
+
+def test_c2_bench_launch_configuration_sampled(hd, h):
+    """The step bench.py times: 131072 tiled C2 queries, fp32 encode on CTA pairs (886 waves of 256x256
+    tiles) + cosine classify, and the host entry point.  The oracle checks the first 1559 rows (the
+    test set once) bit by bit / label by label; a property that holds at any size covers the rest:
+    row i is a copy of row i mod 1559, so every hypervector and label must repeat with that period
+    wherever the row sits in a tile, a CTA pair or a chunk of the host pipeline."""
+    w = gen.c2_isolet_shaped()
+    D, K, F = w["D"], w["K"], w["F"]
+    NQ, n_te = 131072, w["Xte"].shape[0]
+    Xq = gen.tile_rows(w["Xte"], NQ)
+    Pd = dev(w["P"])
+    kn_e = hd.knobs(D, precision=hd.HDC_F32)
+    kn = hd.knobs(D, precision=hd.HDC_F32, hv_bits=32, sim=hd.HDC_SIM_COS)
+    Hq = h.hdc_encode_rp(dev(Xq), Pd, kn_e)
+    bte_or, acc_te, ab_te = O.encode_rp(w["Xte"], w["P"], D, O.F32, want_absum=True)
+    check_sign_band(host_bits(Hq[:n_te], D), bte_or, acc_te, ab_te, F)
+    Hw = Hq.cpu().numpy()
+    idx = np.arange(NQ)
+    assert np.array_equal(Hw, Hw[idx % n_te]), "a tiled row encoded differently from its first copy"
+    btr_or, _, _ = O.encode_rp(w["Xtr"][:2048], w["P"], D, O.F32)
+    C_or = O.bundle(btr_or, w["ytr"][:2048], K, D)
+    Cd = dev(C_or)
+    lab = h.hdc_classify(Hq, Cd, kn).cpu().numpy()
+    S_or = O.similarity(bte_or, C_or, D, O.SIM_COS, 32)
+    check_labels_float(lab[:n_te], S_or, O.SIM_COS)
+    assert np.array_equal(lab, lab[idx % n_te])
+    Xh = torch.from_numpy(Xq).pin_memory()
+    lab_host = h.hdc_infer_rp_host(Xh, Pd, Cd, kn).numpy()
+    assert np.array_equal(lab_host, lab), "host pipeline (16384-row chunks) differs from the device path"
