@@ -3,11 +3,15 @@
 //
 //   S[n,k] = sum_{d<D_eff} v[n,d] * c[k,d],   v = 1 - 2*bit
 //
-// The +-1 query operand never exists in HBM: four "expander" warps turn the packed words of a
+// The +-1 query operand never exists in HBM: eight "expander" warps turn the packed words of a
 // 128-query tile into the K-major, 128-byte-swizzled shared-memory tile that tcgen05.mma reads (the
 // layout TMA would have written), while the class operand arrives by TMA.  Roles (14 warps, one
 // persistent CTA per SM): warp 0 = TMA producer (class tiles), warp 1 = MMA issuer + TMEM
-// allocation, warps 2-5 = epilogue (thread = query row), warps 6-13 = expanders (thread = query row x half of a k-block).
+// allocation, warps 2-5 = epilogue (thread = query row), warps 6-13 = expanders (thread = query row
+// x half of a k-block; the packed words reach them through a cp.async ring).  Producer, expanders and
+// issuer hand k-blocks over in groups (one full / empty barrier pair, one proxy fence, one commit per
+// group); for small N the reduction axis is split over several CTAs per m-tile (split_reduce_kernel
+// adds the partial sums in a fixed order).
 //
 // Reduction-axis permutation.  A sum over d is invariant under any permutation of d applied to both
 // operands, so the k-block position kappa <-> dimension map is chosen to make the expansion two or
