@@ -162,6 +162,12 @@ int32_t hdc_encode_levelid(hdc_handle_t h, const uint8_t* levels, int64_t N, int
                            int32_t Q, int64_t ldlv_words, int32_t D, const hdc_knobs_t* knobs,
                            uint32_t* Hbits, int64_t ldh_words, void* ws, size_t ws_bytes,
                            void* stream);
+/* Same with 16-bit level indices, 1 <= Q <= 65535 (PAPER.md L183 N_LEVELS "quantization granularity",
+ * L255: the Micro-HD comparison tunes the number of levels up to 814).  levels [N][ldl] uint16. */
+int32_t hdc_encode_levelid_u16(hdc_handle_t h, const uint16_t* levels, int64_t N, int32_t F, int64_t ldl,
+                               const uint32_t* IDbits, int64_t ldid_words, const uint32_t* LVbits, int32_t Q,
+                               int64_t ldlv_words, int32_t D, const hdc_knobs_t* knobs, uint32_t* Hbits,
+                               int64_t ldh_words, void* ws, size_t ws_bytes, void* stream);
 
 /* ---- (2) similarity -----------------------------------------------------------------------
  * PAPER.md L72-L74 `__hetero_hdc_hamming_distance`, L110 `__hetero_hdc_cos_sim`, L197 dot.

@@ -26,7 +26,8 @@ HDC_FLAG_NONE, HDC_FLAG_SIMT, HDC_FLAG_TC_1CTA, HDC_FLAG_TC_2CTA = 0, 1, 2, 4
 HDC_K_ENCODE_GEMM, HDC_K_SIM, HDC_K_LEVELID, HDC_K_CLASS_UPDATE = 0, 1, 2, 3
 
 EXPORTS = ("hdc_create", "hdc_destroy", "hdc_last_error", "hdc_version", "hdc_launch_count",
-           "hdc_workspace_bytes", "hdc_encode_rp", "hdc_encode_levelid", "hdc_similarity",
+           "hdc_workspace_bytes", "hdc_encode_rp", "hdc_encode_levelid", "hdc_encode_levelid_u16",
+           "hdc_similarity",
            "hdc_classify", "hdc_train_epoch", "hdc_train_delta", "hdc_train_apply", "hdc_infer_rp_host",
            "hdc_kernel_timing", "hdc_kernel_time")
 
@@ -75,6 +76,8 @@ def lib() -> C.CDLL:
     L.hdc_encode_levelid.argtypes = [vp, vp, i64, i32, i64, vp, i64, vp, i32, i64, i32, kp, vp, i64, vp, sz,
                                      vp]
     L.hdc_encode_levelid.restype = i32
+    L.hdc_encode_levelid_u16.argtypes = L.hdc_encode_levelid.argtypes
+    L.hdc_encode_levelid_u16.restype = i32
     L.hdc_similarity.argtypes = [vp, vp, i64, i64, vp, i32, i64, i32, kp, vp, i32, i64, vp, sz, vp]
     L.hdc_similarity.restype = i32
     L.hdc_classify.argtypes = [vp, vp, i64, i64, vp, i32, i64, i32, kp, vp, vp, vp, vp, sz, vp]
@@ -201,7 +204,10 @@ class Handle:
         W = (kn.D_eff + 31) // 32
         if Hbits is None:
             Hbits = torch.empty((N, W), dtype=torch.int32, device=self.device)
-        rc = self._L.hdc_encode_levelid(self._h, _ptr(levels), N, F, _rowmajor(levels, "levels"),
+        if levels.dtype not in (torch.uint8, torch.int16, torch.uint16):
+            raise TypeError("levels must be uint8, or int16 / uint16 (16-bit indices)")
+        fn = self._L.hdc_encode_levelid if levels.dtype == torch.uint8 else self._L.hdc_encode_levelid_u16
+        rc = fn(self._h, _ptr(levels), N, F, _rowmajor(levels, "levels"),
                                         _ptr(IDbits), _rowmajor(IDbits, "IDbits"), _ptr(LVbits), Q,
                                         _rowmajor(LVbits, "LVbits"), D, C.byref(kn), _ptr(Hbits),
                                         _rowmajor(Hbits, "Hbits"), None, 0, self._stream())

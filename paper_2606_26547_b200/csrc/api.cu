@@ -556,17 +556,14 @@ extern "C" int32_t hdc_encode_rp(hdc_handle_t h, const void* X, int32_t x_dtype,
 }
 
 // =================================================================================== (1b)
-extern "C" int32_t hdc_encode_levelid(hdc_handle_t h, const uint8_t* levels, int64_t N, int32_t F,
-                                      int64_t ldl, const uint32_t* IDbits, int64_t ldid_words,
-                                      const uint32_t* LVbits, int32_t Q, int64_t ldlv_words, int32_t D,
-                                      const hdc_knobs_t* knobs, uint32_t* Hbits, int64_t ldh_words, void* ws,
-                                      size_t ws_bytes, void* stream) {
-  (void)ws;
-  (void)ws_bytes;
+static int32_t encode_levelid_impl(hdc_handle_t h, const void* levels, int lvl16, int64_t N, int32_t F, int64_t ldl,
+                                   const uint32_t* IDbits, int64_t ldid_words, const uint32_t* LVbits, int32_t Q,
+                                   int64_t ldlv_words, int32_t D, const hdc_knobs_t* knobs, uint32_t* Hbits,
+                                   int64_t ldh_words, void* stream) {
   if (!h) return HDC_ERR_INVALID_ARG;
   if (((!levels || !Hbits) && N > 0) || !IDbits || !LVbits)
     return fail(h, HDC_ERR_INVALID_ARG, "encode_levelid: NULL pointer");
-  if (N < 0 || F < 1 || F > 65535 || Q < 1 || Q > 256 || D < 1 || ldl < F)
+  if (N < 0 || F < 1 || F > 65535 || Q < 1 || Q > (lvl16 ? 65535 : 256) || D < 1 || ldl < F)
     return fail(h, HDC_ERR_INVALID_ARG, "encode_levelid: bad sizes");
   int rc = check_knobs(h, knobs, D);
   if (rc) return rc;
@@ -576,14 +573,38 @@ extern "C" int32_t hdc_encode_levelid(hdc_handle_t h, const uint8_t* levels, int
   if ((reinterpret_cast<uintptr_t>(IDbits) | reinterpret_cast<uintptr_t>(LVbits) |
        reinterpret_cast<uintptr_t>(Hbits)) & 3)
     return fail(h, HDC_ERR_ALIGNMENT, "encode_levelid: bit matrices must be 4-byte aligned");
+  if (lvl16 && (reinterpret_cast<uintptr_t>(levels) & 1))
+    return fail(h, HDC_ERR_ALIGNMENT, "encode_levelid_u16: levels must be 2-byte aligned");
   if (N == 0) return HDC_OK;
   cudaError_t ce;
   {
     Timed tm(h, HDC_K_LEVELID, (cudaStream_t)stream);
-    ce = launch_levelid(levels, N, F, ldl, IDbits, ldid_words, LVbits, Q, ldlv_words, knobs->D_eff, Hbits,
+    ce = launch_levelid(levels, lvl16, N, F, ldl, IDbits, ldid_words, LVbits, Q, ldlv_words, knobs->D_eff, Hbits,
                         ldh_words, h->sm_count, h->smem_optin, (cudaStream_t)stream, &h->launches);
   }
   return ce == cudaSuccess ? HDC_OK : cuda_fail(h, ce, "encode_levelid");
+}
+
+extern "C" int32_t hdc_encode_levelid(hdc_handle_t h, const uint8_t* levels, int64_t N, int32_t F,
+                                      int64_t ldl, const uint32_t* IDbits, int64_t ldid_words,
+                                      const uint32_t* LVbits, int32_t Q, int64_t ldlv_words, int32_t D,
+                                      const hdc_knobs_t* knobs, uint32_t* Hbits, int64_t ldh_words, void* ws,
+                                      size_t ws_bytes, void* stream) {
+  (void)ws;
+  (void)ws_bytes;
+  return encode_levelid_impl(h, levels, 0, N, F, ldl, IDbits, ldid_words, LVbits, Q, ldlv_words, D, knobs, Hbits,
+                             ldh_words, stream);
+}
+
+extern "C" int32_t hdc_encode_levelid_u16(hdc_handle_t h, const uint16_t* levels, int64_t N, int32_t F,
+                                          int64_t ldl, const uint32_t* IDbits, int64_t ldid_words,
+                                          const uint32_t* LVbits, int32_t Q, int64_t ldlv_words, int32_t D,
+                                          const hdc_knobs_t* knobs, uint32_t* Hbits, int64_t ldh_words, void* ws,
+                                          size_t ws_bytes, void* stream) {
+  (void)ws;
+  (void)ws_bytes;
+  return encode_levelid_impl(h, levels, 1, N, F, ldl, IDbits, ldid_words, LVbits, Q, ldlv_words, D, knobs, Hbits,
+                             ldh_words, stream);
 }
 
 // =================================================================================== (2), (2+3a)

@@ -137,7 +137,8 @@ cudaError_t launch_hamming(const uint32_t* Hbits, int64_t N, int64_t ldh, const 
                            int64_t* nlaunch);
 
 // level-ID encode (levelid.cu)
-cudaError_t launch_levelid(const uint8_t* levels, int64_t N, int F, int64_t ldl, const uint32_t* ID,
+// levels: uint8_t indices, or uint16_t when lvl16 != 0 (general kernel only)
+cudaError_t launch_levelid(const void* levels, int lvl16, int64_t N, int F, int64_t ldl, const uint32_t* ID,
                            int64_t ldid, const uint32_t* LV, int Q, int64_t ldlv, int D_eff,
                            uint32_t* Hbits, int64_t ldh, int sm_count, int smem_optin, cudaStream_t st,
                            int64_t* nlaunch);

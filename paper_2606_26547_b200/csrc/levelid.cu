@@ -30,7 +30,7 @@ constexpr int NTHREADS = NWARPS * 32;
   }
 
 struct LevelIdParams {
-  const uint8_t* levels;
+  const void* levels;  // uint8_t (Q <= 256) or uint16_t level indices
   int64_t N;
   int F;
   int64_t ldl;
@@ -50,13 +50,14 @@ struct LevelIdParams {
   uint32_t mul128;    // 0x8080: dp2a selectors "times 128" of the sparse path
 };
 
-// NP = number of counter planes (p + 1 with 2^p > F); S = samples per warp iteration
-template <int NP, int S>
+// NP = number of counter planes (p + 1 with 2^p > F); S = samples per warp iteration; LT = type of the
+// level indices (uint16_t for Q > 256: PAPER.md L255 tunes the number of levels up to 814)
+template <int NP, int S, typename LT>
 __global__ void __launch_bounds__(NTHREADS, 1) levelid_kernel(const LevelIdParams p) {
   extern __shared__ __align__(16) uint8_t smem[];
   uint32_t* sID = reinterpret_cast<uint32_t*>(smem);                 // [F][SW]
   uint32_t* sLV = sID + (p.tables_in_smem ? (size_t)p.F * SW : 0);    // [Q][SW]
-  uint8_t* sLvl = reinterpret_cast<uint8_t*>(sLV + (p.tables_in_smem ? (size_t)p.Q * SW : 0));
+  LT* sLvl = reinterpret_cast<LT*>(sLV + (p.tables_in_smem ? (size_t)p.Q * SW : 0));
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   constexpr int SB = NWARPS * S;  // samples per batch
@@ -85,7 +86,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) levelid_kernel(const LevelIdParam
     for (int s = warp; s < SB; s += NWARPS) {
       const int64_t n = n0 + s;
       for (int f = lane; f < p.Fpad; f += 32)
-        sLvl[s * p.Fpad + f] = (n < p.N && f < p.F) ? __ldg(p.levels + n * p.ldl + f) : (uint8_t)0;
+        sLvl[s * p.Fpad + f] = (n < p.N && f < p.F) ? __ldg(static_cast<const LT*>(p.levels) + n * p.ldl + f) : (LT)0;
     }
     __syncthreads();
 
@@ -95,7 +96,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) levelid_kernel(const LevelIdParam
 #pragma unroll
       for (int i = 0; i < NP; ++i) pl[j][i] = ((init >> i) & 1u) ? 0xffffffffu : 0u;
 
-    const uint8_t* myl = sLvl + (size_t)(warp * S) * p.Fpad;
+    const LT* myl = sLvl + (size_t)(warp * S) * p.Fpad;
     const uint32_t* idp = p.tables_in_smem ? sID + lane : p.ID + w_glob;
     const uint32_t* lvp = p.tables_in_smem ? sLV + lane : p.LV + w_glob;
     const int64_t idstride = p.tables_in_smem ? SW : p.ldid;
@@ -254,7 +255,7 @@ __global__ void __launch_bounds__(FTHREADS, 1) levelid_fast_kernel(const LevelId
 #pragma unroll
     for (int j = 0; j < FS; ++j) {
       const int64_t n = n0 + j;
-      const uint32_t* row = reinterpret_cast<const uint32_t*>(p.levels + (n < p.N ? n : 0) * p.ldl);
+      const uint32_t* row = reinterpret_cast<const uint32_t*>(static_cast<const uint8_t*>(p.levels) + (n < p.N ? n : 0) * p.ldl);
 #pragma unroll
       for (int i = 0; i < PF_ROW; ++i) {
         const int g = lane + 32 * i;
@@ -553,18 +554,18 @@ __global__ void __launch_bounds__(FTHREADS, 1) levelid_fast_kernel(const LevelId
   }
 }
 
-template <int NP, int S>
+template <int NP, int S, typename LT>
 cudaError_t launch_t(const LevelIdParams& p, int grid, size_t smem, cudaStream_t st) {
-  cudaError_t e = cudaFuncSetAttribute(levelid_kernel<NP, S>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+  cudaError_t e = cudaFuncSetAttribute(levelid_kernel<NP, S, LT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                        (int)smem);
   if (e != cudaSuccess) return e;
-  levelid_kernel<NP, S><<<grid, NTHREADS, smem, st>>>(p);
+  levelid_kernel<NP, S, LT><<<grid, NTHREADS, smem, st>>>(p);
   return cudaGetLastError();
 }
 
 }  // namespace
 
-cudaError_t launch_levelid(const uint8_t* levels, int64_t N, int F, int64_t ldl, const uint32_t* ID,
+cudaError_t launch_levelid(const void* levels, int lvl16, int64_t N, int F, int64_t ldl, const uint32_t* ID,
                            int64_t ldid, const uint32_t* LV, int Q, int64_t ldlv, int D_eff,
                            uint32_t* Hbits, int64_t ldh, int sm_count, int smem_optin, cudaStream_t st,
                            int64_t* nlaunch) {
@@ -573,7 +574,7 @@ cudaError_t launch_levelid(const uint8_t* levels, int64_t N, int F, int64_t ldl,
   {  // fast path
     const size_t fp2 = (size_t)round_up((F + 1) / 2, 8);
     const size_t smem_fast = ((size_t)F + Q) * SW * 4 + (size_t)FSB * fp2 * 4 + (size_t)11 * SW * 4;
-    if (F % 4 == 0 && F < 1024 && (ldl & 3) == 0 && (reinterpret_cast<uintptr_t>(levels) & 3) == 0 &&
+    if (!lvl16 && F % 4 == 0 && F < 1024 && (ldl & 3) == 0 && (reinterpret_cast<uintptr_t>(levels) & 3) == 0 &&
         smem_fast <= (size_t)smem_optin) {
       LevelIdParams p;
       p.levels = levels; p.N = N; p.F = F; p.ldl = ldl;
@@ -605,7 +606,7 @@ cudaError_t launch_levelid(const uint8_t* levels, int64_t N, int F, int64_t ldl,
   const int SB = NWARPS * S;
   p.n_batches = (N + SB - 1) / SB;
   p.Fpad = (int)round_up(F, 16);
-  const size_t lvl_bytes = (size_t)SB * p.Fpad;
+  const size_t lvl_bytes = (size_t)SB * p.Fpad * (lvl16 ? 2 : 1);
   const size_t tab_bytes = ((size_t)F + Q) * SW * 4;
   p.tables_in_smem = (tab_bytes + lvl_bytes <= (size_t)smem_optin) ? 1 : 0;
   const size_t smem = lvl_bytes + (p.tables_in_smem ? tab_bytes : 0);
@@ -613,8 +614,12 @@ cudaError_t launch_levelid(const uint8_t* levels, int64_t N, int F, int64_t ldl,
   const int64_t units = (int64_t)p.n_slices * p.n_batches;
   const int grid = (int)(units < sm_count ? units : sm_count);
   ++*nlaunch;
-  if (F < 1024) return launch_t<11, S>(p, grid, smem, st);
-  return launch_t<17, S>(p, grid, smem, st);
+  if (lvl16) {
+    if (F < 1024) return launch_t<11, S, uint16_t>(p, grid, smem, st);
+    return launch_t<17, S, uint16_t>(p, grid, smem, st);
+  }
+  if (F < 1024) return launch_t<11, S, uint8_t>(p, grid, smem, st);
+  return launch_t<17, S, uint8_t>(p, grid, smem, st);
 }
 
 }  // namespace hdc

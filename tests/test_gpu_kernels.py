@@ -491,3 +491,20 @@ def test_train_delta_of_an_empty_shard_is_zero(hd, h):
     d = torch.full((3, 128), 7, dtype=torch.int32, device="cuda")
     h.hdc_train_delta(H0, y0, Cc, kn, delta=d)
     assert int(d.abs().sum().item()) == 0
+
+
+# ------------------------------------------------------------------------------------ 16-bit level indices
+@pytest.mark.parametrize("N,F,Q,D,D_eff", [(70, 617, 814, 1024, 1024), (33, 617, 814, 1024, 512), (40, 64, 1000, 2048, 1999),
+                                           (20, 1100, 300, 256, 256), (9, 5, 65535, 96, 96)])
+def test_levelid_u16_indices_bit_exact(hd, h, N, F, Q, D, D_eff):
+    """hdc_encode_levelid_u16: more than 256 levels (the Micro-HD comparison runs with up
+    to 814 levels at D = 1024 / 512 on F = 617 features).  Bit-exact against the oracle."""
+    r = rng(14, N, F, Q, D_eff)
+    lv = r.integers(0, Q, size=(N, F)).astype(np.uint16)
+    lv[0] = Q - 1
+    ID = r.integers(0, 2, size=(F, D), dtype=np.uint8)
+    LV = gen.level_table(9, Q, D)
+    bits_or = O.encode_levelid(lv, ID, LV, D_eff)
+    lvd = torch.from_numpy(lv.view(np.int16)).cuda()
+    H = h.hdc_encode_levelid(lvd, dev_bits(ID), dev_bits(LV), D, hd.knobs(D_eff))
+    assert np.array_equal(host_bits(H, D_eff), bits_or)
