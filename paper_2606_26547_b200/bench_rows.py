@@ -227,6 +227,26 @@ def row_c5_stream(h, peaks, reps, hv_bits, sim_name, N=1 << 20, B=65536, F=1024,
     return out
 
 
+def row_levelid_microhd(h, peaks, reps, N=131072, F=617, Q=128, D=1024):
+    """The paper's Micro-HD-Classification reference shape (ISOLET F = 617, D = 1024,
+    L = 128 levels): dense uniform levels, rows of 617 bytes (not word-aligned)."""
+    lv = torch.randint(0, Q, (N, F), dtype=torch.uint8, device="cuda", generator=_gen(31))
+    Wd = (D + 31) // 32
+    ID = _rand_bits(F, Wd, 32)
+    LV = _rand_bits(Q, Wd, 33)
+    H = torch.empty((N, Wd), dtype=torch.int32, device="cuda")
+    kn = hd.knobs(D)
+    fn = lambda: h.hdc_encode_levelid(lv, ID, LV, D, kn, Hbits=H)  # noqa: E731
+    call_ms = _time(fn, reps)
+    ops = 3.0 * F * Wd * N
+    ach = ops / (call_ms * 1e-3) / 1e12
+    peak = 148 * 64 * peaks["sm_max_mhz"] * 1e6 / 1e12
+    return {"what": f"hdc_encode_levelid N={N} F={F} Q={Q} D={D} (Micro-HD reference shape, dense levels)",
+            "call_ms": call_ms, "samples_per_s": N / (call_ms * 1e-3),
+            "roofline": {"bound": "alu", "achieved": ach, "peak": peak, "unit": "Tlop/s (32-bit logic ops)",
+                         "frac": ach / peak, "peak_source": "148 SM x 64 INT lanes x sm_max_mhz"}}
+
+
 def row_c3_pipeline(h, peaks, reps, N=65536, F=784, Q=256, D=10000, K=10):
     """configs[2] inference: level-ID encode + packed Hamming classify against K = 10 classes."""
     from workloads import gen
@@ -330,6 +350,7 @@ ROWS = {
     "c4_classify_cos8": lambda h, p, r: row_classify(h, p, r, 131072, 6, 10000, 8, "cos"),
     "c3_levelid": lambda h, p, r: row_levelid(h, p, r),
     "c3_levelid_dense_input": lambda h, p, r: row_levelid(h, p, r, dense_input=True),
+    "microhd_levelid": lambda h, p, r: row_levelid_microhd(h, p, r),
     "c3_hamming_k10": lambda h, p, r: row_classify(h, p, r, 131072, 10, 10000, 1, "hamming"),
     "c5_encode_bf16": lambda h, p, r: row_encode(h, p, r, 65536, 1024, 16384, "bf16", x_bf16=True),
     "c5_classify_bf16": lambda h, p, r: row_classify(h, p, r, 65536, 1000, 16384, 16, "cos"),

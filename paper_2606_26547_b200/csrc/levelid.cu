@@ -48,6 +48,7 @@ struct LevelIdParams {
   int tables_in_smem;
   uint32_t mul_hi16;  // 0x0101: the dp2a selectors, passed at run time so that they are not strength-reduced
   uint32_t mul128;    // 0x8080: dp2a selectors "times 128" of the sparse path
+  int rows_aligned;   // F % 4 == 0, ldl % 4 == 0 and a 4-byte aligned base: level rows are read as words
 };
 
 // NP = number of counter planes (p + 1 with 2^p > F); S = samples per warp iteration; LT = type of the
@@ -168,7 +169,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) levelid_kernel(const LevelIdParam
 }
 
 // ---------------------------------------------------------------------------------------------
-// Fast path (F % 4 == 0, F < 1024, tables + one batch fit in shared memory, 4-byte aligned level
+// Fast path (uint8 levels, F < 1024, tables + one batch fit in shared memory; word loads of the level
 // rows): same mapping (CTA = 1024-bit slice, lane = word, warp = FS samples at a time) with the
 // instruction stream cut to what the counter needs:
 //   * levels are staged as 16-bit table byte-offsets (level << 7), two per word, read by the warp
@@ -240,7 +241,8 @@ __global__ void __launch_bounds__(FTHREADS, 1) levelid_fast_kernel(const LevelId
   const uint32_t lane4 = (uint32_t)lane * 4u;
   const uint32_t sel_lo = p.mul_hi16 & 0x0001u, sel_hi = p.mul_hi16 & 0x0100u;  // dp2a byte selectors (run-time: not folded)
   const uint32_t sel_id = p.mul128 & 0x0080u, sel_lv = p.mul128 & 0x8000u;      // (16-bit half) * 128
-  const int F4 = p.F >> 2;                                     // level words per sample row
+  const int F4 = (p.F + 3) >> 2;                               // level words per sample row (last one zero-padded)
+  const bool vec_rows = p.rows_aligned != 0;                   // rows readable as 32-bit words
 
   const int64_t units = (int64_t)p.n_slices * p.n_batches;
   const int64_t u_begin = units * blockIdx.x / gridDim.x;
@@ -255,11 +257,22 @@ __global__ void __launch_bounds__(FTHREADS, 1) levelid_fast_kernel(const LevelId
 #pragma unroll
     for (int j = 0; j < FS; ++j) {
       const int64_t n = n0 + j;
-      const uint32_t* row = reinterpret_cast<const uint32_t*>(static_cast<const uint8_t*>(p.levels) + (n < p.N ? n : 0) * p.ldl);
+      const uint8_t* rowb = static_cast<const uint8_t*>(p.levels) + (n < p.N ? n : 0) * p.ldl;
+      const uint32_t* row = reinterpret_cast<const uint32_t*>(rowb);
 #pragma unroll
       for (int i = 0; i < PF_ROW; ++i) {
         const int g = lane + 32 * i;
-        pf[j * PF_ROW + i] = (g < F4 && n < p.N) ? __ldg(row + g) : 0u;
+        uint32_t v = 0u;
+        if (g < F4 && n < p.N) {
+          if (vec_rows) {
+            v = __ldg(row + g);
+          } else {  // any F / ldl / alignment (e.g. ISOLET's F = 617): byte loads, features >= F read as 0
+#pragma unroll
+            for (int b = 0; b < 4; ++b)
+              if (4 * g + b < p.F) v |= (uint32_t)__ldg(rowb + 4 * g + b) << (8 * b);
+          }
+        }
+        pf[j * PF_ROW + i] = v;
       }
     }
   };
@@ -574,8 +587,7 @@ cudaError_t launch_levelid(const void* levels, int lvl16, int64_t N, int F, int6
   {  // fast path
     const size_t fp2 = (size_t)round_up((F + 1) / 2, 8);
     const size_t smem_fast = ((size_t)F + Q) * SW * 4 + (size_t)FSB * fp2 * 4 + (size_t)11 * SW * 4;
-    if (!lvl16 && F % 4 == 0 && F < 1024 && (ldl & 3) == 0 && (reinterpret_cast<uintptr_t>(levels) & 3) == 0 &&
-        smem_fast <= (size_t)smem_optin) {
+    if (!lvl16 && F < 1024 && smem_fast <= (size_t)smem_optin) {
       LevelIdParams p;
       p.levels = levels; p.N = N; p.F = F; p.ldl = ldl;
       p.ID = ID; p.ldid = ldid; p.LV = LV; p.Q = Q; p.ldlv = ldlv;
@@ -587,6 +599,7 @@ cudaError_t launch_levelid(const void* levels, int lvl16, int64_t N, int F, int6
       p.tables_in_smem = 1;
       p.mul_hi16 = 0x0101u;
       p.mul128 = 0x8080u;
+      p.rows_aligned = (F % 4 == 0 && (ldl & 3) == 0 && (reinterpret_cast<uintptr_t>(levels) & 3) == 0) ? 1 : 0;
       const int64_t units = (int64_t)p.n_slices * p.n_batches;
       const int grid = (int)(units < sm_count ? units : sm_count);
       cudaError_t e = cudaFuncSetAttribute(levelid_fast_kernel<11>, cudaFuncAttributeMaxDynamicSharedMemorySize,

@@ -90,7 +90,8 @@ def test_levelid_bit_exact(hd, h, N, F, Q, D, D_eff):
 
 @pytest.mark.parametrize("zeros", [0.8, 0.97, 1.0])
 @pytest.mark.parametrize("N,F,Q,D,D_eff", [(200, 784, 256, 10000, 10000), (97, 100, 16, 3000, 2049), (50, 36, 256, 1100, 1000),
-                                           (130, 1020, 256, 200, 33), (49, 4, 3, 64, 64)])
+                                           (130, 1020, 256, 200, 33), (49, 4, 3, 64, 64),
+                                           (150, 617, 128, 1024, 1024), (60, 1023, 256, 96, 96), (75, 7, 9, 500, 499)])
 def test_levelid_sparse_path_bit_exact(hd, h, zeros, N, F, Q, D, D_eff):
     """Mostly-zero level rows take the sparse path of the fast kernel (per-warp decision, base counter +
     listed features); a few fully dense rows mixed in exercise the per-warp fallback and the list
