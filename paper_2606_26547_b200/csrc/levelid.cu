@@ -226,7 +226,9 @@ __device__ __forceinline__ void ripple(uint32_t (&q)[NP], uint32_t c, int from) 
   }
 }
 
-template <int NP>
+// VEC: level rows are word-aligned and F % 4 == 0 (plain word loads); otherwise aligned words are
+// prefetched and re-aligned by fixup() (any F, any row alignment)
+template <int NP, bool VEC>
 __global__ void __launch_bounds__(FTHREADS, 1) levelid_fast_kernel(const LevelIdParams p) {
   extern __shared__ __align__(16) uint8_t smem[];
   uint32_t* sID = reinterpret_cast<uint32_t*>(smem);          // [F][SW]
@@ -242,7 +244,6 @@ __global__ void __launch_bounds__(FTHREADS, 1) levelid_fast_kernel(const LevelId
   const uint32_t sel_lo = p.mul_hi16 & 0x0001u, sel_hi = p.mul_hi16 & 0x0100u;  // dp2a byte selectors (run-time: not folded)
   const uint32_t sel_id = p.mul128 & 0x0080u, sel_lv = p.mul128 & 0x8000u;      // (16-bit half) * 128
   const int F4 = (p.F + 3) >> 2;                               // level words per sample row (last one zero-padded)
-  const bool vec_rows = p.rows_aligned != 0;                   // rows readable as 32-bit words
 
   const int64_t units = (int64_t)p.n_slices * p.n_batches;
   const int64_t u_begin = units * blockIdx.x / gridDim.x;
@@ -257,22 +258,65 @@ __global__ void __launch_bounds__(FTHREADS, 1) levelid_fast_kernel(const LevelId
 #pragma unroll
     for (int j = 0; j < FS; ++j) {
       const int64_t n = n0 + j;
+      if (VEC) {
+        const uint32_t* row = reinterpret_cast<const uint32_t*>(static_cast<const uint8_t*>(p.levels) +
+                                                                (n < p.N ? n : 0) * p.ldl);
+#pragma unroll
+        for (int i = 0; i < PF_ROW; ++i) {
+          const int g = lane + 32 * i;
+          pf[j * PF_ROW + i] = (g < F4 && n < p.N) ? __ldg(row + g) : 0u;
+        }
+        continue;
+      }
+      // raw ALIGNED words covering the row (the loads have no dependants here: they stay in flight
+      // during the previous unit's arithmetic); row-relative words are formed by fixup() a unit later
       const uint8_t* rowb = static_cast<const uint8_t*>(p.levels) + (n < p.N ? n : 0) * p.ldl;
-      const uint32_t* row = reinterpret_cast<const uint32_t*>(rowb);
+      const uint32_t off = (uint32_t)(reinterpret_cast<uintptr_t>(rowb) & 3u);
+      const uint32_t* row = reinterpret_cast<const uint32_t*>(rowb - off);
+      const int nwords = (int)((off + (uint32_t)p.F + 3u) >> 2);   // aligned words that hold the row
 #pragma unroll
       for (int i = 0; i < PF_ROW; ++i) {
         const int g = lane + 32 * i;
         uint32_t v = 0u;
-        if (g < F4 && n < p.N) {
-          if (vec_rows) {
+        if (g < nwords && n < p.N) {
+          if (g + 1 < nwords || n + 1 < p.N || ((off + (uint32_t)p.F) & 3u) == 0u) {
             v = __ldg(row + g);
-          } else {  // any F / ldl / alignment (e.g. ISOLET's F = 617): byte loads, features >= F read as 0
-#pragma unroll
-            for (int b = 0; b < 4; ++b)
-              if (4 * g + b < p.F) v |= (uint32_t)__ldg(rowb + 4 * g + b) << (8 * b);
+          } else {  // last word of the last row: do not read past the end of the caller's buffer
+            const int nb = (int)((off + (uint32_t)p.F) & 3u);
+            for (int b2 = 0; b2 < nb; ++b2)
+              v |= (uint32_t)__ldg(reinterpret_cast<const uint8_t*>(row + g) + b2) << (8 * b2);
           }
         }
         pf[j * PF_ROW + i] = v;
+      }
+    }
+  };
+  // pf[] of sample j: aligned words -> words relative to the row start, bytes >= F zeroed (level 0)
+  auto fixup = [&](int64_t u) {
+    if (VEC) return;
+    const int64_t n0 = (u % p.n_batches) * FSB + warp * FS;
+#pragma unroll
+    for (int j = 0; j < FS; ++j) {
+      const int64_t n = n0 + j;
+      const uint8_t* rowb = static_cast<const uint8_t*>(p.levels) + (n < p.N ? n : 0) * p.ldl;
+      const uint32_t sh = (uint32_t)(reinterpret_cast<uintptr_t>(rowb) & 3u) * 8u;  // warp-uniform
+      if (sh != 0u) {
+#pragma unroll
+        for (int i = 0; i < PF_ROW; ++i) {
+          const uint32_t lo = pf[j * PF_ROW + i];
+          uint32_t hi = __shfl_down_sync(0xffffffffu, lo, 1);                       // word of lane + 1
+          const uint32_t nxt = i + 1 < PF_ROW ? pf[j * PF_ROW + (i + 1 < PF_ROW ? i + 1 : i)] : 0u;
+          const uint32_t wrap = __shfl_sync(0xffffffffu, nxt, 0);                   // lane 0 of the next round
+          if (lane == 31) hi = wrap;
+          pf[j * PF_ROW + i] = __funnelshift_r(lo, hi, sh);
+        }
+      }
+      if (p.F & 3) {
+#pragma unroll
+        for (int i = 0; i < PF_ROW; ++i) {
+          const int g = lane + 32 * i;
+          if (4 * g + 4 > p.F) pf[j * PF_ROW + i] &= (4 * g < p.F) ? ((1u << (8 * (p.F - 4 * g))) - 1u) : 0u;
+        }
       }
     }
   };
@@ -309,6 +353,7 @@ __global__ void __launch_bounds__(FTHREADS, 1) levelid_fast_kernel(const LevelId
       __syncthreads();
     }
     __syncwarp();  // this warp is done reading its rows of the previous unit
+    fixup(u);
 
     // ---- sparse path (level 0 is the common level: C3's images are ~80 % zeros) ------------------
     // cnt = sum_f b(f, x_f) = base + sum_{f in L} (b(f, x_f) - b(f, 0)) for any list L holding every
@@ -587,7 +632,7 @@ cudaError_t launch_levelid(const void* levels, int lvl16, int64_t N, int F, int6
   {  // fast path
     const size_t fp2 = (size_t)round_up((F + 1) / 2, 8);
     const size_t smem_fast = ((size_t)F + Q) * SW * 4 + (size_t)FSB * fp2 * 4 + (size_t)11 * SW * 4;
-    if (!lvl16 && F < 1024 && smem_fast <= (size_t)smem_optin) {
+    if (!lvl16 && F <= 1020 && smem_fast <= (size_t)smem_optin) {  // (+3 bytes of row misalignment fit the prefetch)
       LevelIdParams p;
       p.levels = levels; p.N = N; p.F = F; p.ldl = ldl;
       p.ID = ID; p.ldid = ldid; p.LV = LV; p.Q = Q; p.ldlv = ldlv;
@@ -602,11 +647,15 @@ cudaError_t launch_levelid(const void* levels, int lvl16, int64_t N, int F, int6
       p.rows_aligned = (F % 4 == 0 && (ldl & 3) == 0 && (reinterpret_cast<uintptr_t>(levels) & 3) == 0) ? 1 : 0;
       const int64_t units = (int64_t)p.n_slices * p.n_batches;
       const int grid = (int)(units < sm_count ? units : sm_count);
-      cudaError_t e = cudaFuncSetAttribute(levelid_fast_kernel<11>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+      cudaError_t e = cudaFuncSetAttribute(levelid_fast_kernel<11, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                            (int)smem_fast);
+      if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(levelid_fast_kernel<11, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 (int)smem_fast);
       if (e != cudaSuccess) return e;
       ++*nlaunch;
-      levelid_fast_kernel<11><<<grid, FTHREADS, smem_fast, st>>>(p);
+      if (p.rows_aligned) levelid_fast_kernel<11, true><<<grid, FTHREADS, smem_fast, st>>>(p);
+      else levelid_fast_kernel<11, false><<<grid, FTHREADS, smem_fast, st>>>(p);
       return cudaGetLastError();
     }
   }

@@ -509,3 +509,20 @@ def test_levelid_u16_indices_bit_exact(hd, h, N, F, Q, D, D_eff):
     lvd = torch.from_numpy(lv.view(np.int16)).cuda()
     H = h.hdc_encode_levelid(lvd, dev_bits(ID), dev_bits(LV), D, hd.knobs(D_eff))
     assert np.array_equal(host_bits(H, D_eff), bits_or)
+
+
+@pytest.mark.parametrize("F,ld,col0", [(617, 617, 0), (617, 620, 0), (616, 621, 1), (100, 107, 3), (1020, 1023, 3), (5, 9, 2)])
+def test_levelid_unaligned_rows_bit_exact(hd, h, F, ld, col0):
+    """Level rows that start at any byte offset (a column slice of a wider uint8 matrix; F not a
+    multiple of 4): the fast kernel reads aligned words and re-aligns them with shuffles."""
+    r = rng(15, F, ld, col0)
+    N, Q, D = 101, 64, 1056
+    big = r.integers(0, Q, size=(N, ld), dtype=np.uint8)
+    big[r.random((N, ld)) < 0.6] = 0
+    lv = big[:, col0:col0 + F]
+    ID = r.integers(0, 2, size=(F, D), dtype=np.uint8)
+    LV = gen.level_table(9, Q, D)
+    bits_or = O.encode_levelid(lv, ID, LV, D)
+    lvd = dev(big)[:, col0:col0 + F]
+    H = h.hdc_encode_levelid(lvd, dev_bits(ID), dev_bits(LV), D, hd.knobs(D))
+    assert np.array_equal(host_bits(H, D), bits_or)
