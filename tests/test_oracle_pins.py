@@ -595,3 +595,53 @@ def test_perforated_training_updates_every_dimension():
     assert np.array_equal(pred, lab) and wrong == int((lab != y).sum()) and wrong > 0
     touched = np.nonzero((C1 != C0).any(axis=0))[0]
     assert (touched % 4 != 2).any()                      # columns outside the visited set changed too
+
+
+# ------------------------------------------------------------------------------------- random shapes
+from hypothesis import given, settings, strategies as st  # noqa: E402
+
+
+@settings(max_examples=40, deadline=None)
+@given(st.integers(1, 8), st.integers(1, 17), st.integers(1, 130), st.integers(0, 2 ** 31 - 1), st.data())
+def test_encode_and_similarity_random_shapes_against_loops(N, F, D, seed, data):
+    """Random small shapes (incl. D_eff = 1, 31, 32, 33 and tails): RP encode bits, Hamming, dot and the
+    arg-extremum against plain python loops."""
+    D_eff = data.draw(st.sampled_from(sorted({1, min(D, 31), min(D, 32), min(D, 33), D})))
+    K = data.draw(st.integers(1, 5))
+    r = np.random.default_rng(seed)
+    X = r.integers(-3, 4, size=(N, F)).astype(np.float32)
+    P = r.integers(-2, 3, size=(D, F)).astype(np.float32)
+    bits, acc, _ = o.encode_rp(X, P, D_eff, o.F32)
+    for n in range(N):
+        for d in range(D_eff):
+            a = sum(float(X[n, f]) * float(P[d, f]) for f in range(F))
+            assert acc[n, d] == a and bits[n, d] == (1 if a < 0 else 0)
+    C = r.integers(-4, 5, size=(K, D)).astype(np.float32)
+    H = o.similarity(bits, C, D_eff, o.SIM_HAMMING, 1)
+    Dt = o.similarity(bits, C, D_eff, o.SIM_DOT, 32)
+    for n in range(N):
+        for k in range(K):
+            assert H[n, k] == sum(int(bits[n, d]) != int(C[k, d] < 0) for d in range(D_eff))
+            assert Dt[n, k] == sum((1 - 2 * int(bits[n, d])) * float(C[k, d]) for d in range(D_eff))
+    lab, best, _ = o.classify(H, o.SIM_HAMMING)
+    for n in range(N):
+        assert lab[n] == min(range(K), key=lambda k: (H[n, k], k)) and best[n] == H[n, lab[n]]
+    lab2, _, _ = o.classify(Dt, o.SIM_DOT)
+    for n in range(N):
+        assert lab2[n] == min(range(K), key=lambda k: (-Dt[n, k], k))
+
+
+@settings(max_examples=40, deadline=None)
+@given(st.integers(1, 6), st.integers(1, 12), st.integers(1, 9), st.integers(1, 70), st.integers(0, 2 ** 31 - 1))
+def test_levelid_random_shapes_against_loops(N, F, Q, D, seed):
+    r = np.random.default_rng(seed)
+    lv = r.integers(0, Q, size=(N, F)).astype(np.uint16)
+    ID = r.integers(0, 2, size=(F, D), dtype=np.uint8)
+    LV = r.integers(0, 2, size=(Q, D), dtype=np.uint8)
+    D_eff = int(r.integers(1, D + 1))
+    bits = o.encode_levelid(lv, ID, LV, D_eff)
+    assert bits.shape == (N, D_eff)
+    for n in range(N):
+        for d in range(D_eff):
+            cnt = sum(int(ID[f, d]) ^ int(LV[lv[n, f], d]) for f in range(F))
+            assert bits[n, d] == (1 if 2 * cnt > F else 0)
