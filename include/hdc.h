@@ -133,7 +133,8 @@ int32_t hdc_kernel_time(hdc_handle_t h, int32_t kernel_id, float* ms_total, int6
 
 /* Bytes of device workspace the given op needs for these sizes and knobs (0 is possible).
  * F_or_Q: F for encode_rp / infer_rp_host, Q for encode_levelid, ignored otherwise.
- * For HDC_OP_TRAIN_EPOCH, N is the mini-batch size actually used (batch, or N when batch = 0). */
+ * For HDC_OP_TRAIN_EPOCH, N is the mini-batch size actually used (batch, or N when batch = 0); for
+ * HDC_TRAIN_KMEANS and hdc_train_delta it is the number of samples of the call. */
 size_t hdc_workspace_bytes(hdc_handle_t h, int32_t op, int64_t N, int32_t F_or_Q, int32_t D,
                            int32_t K, const hdc_knobs_t* knobs);
 

@@ -396,7 +396,7 @@ constexpr int64_t HOST_CHUNK = 16384;
 using namespace hdc;
 
 // =================================================================================== handle
-extern "C" int32_t hdc_version(void) { return 100; }
+extern "C" int32_t hdc_version(void) { return 101; }  // 1.1: perforation knobs, k-means, train_delta/apply, u16 levels
 
 extern "C" int32_t hdc_create(hdc_handle_t* out, int32_t device) {
   if (!out) return HDC_ERR_INVALID_ARG;
