@@ -526,3 +526,43 @@ def test_levelid_unaligned_rows_bit_exact(hd, h, F, ld, col0):
     lvd = dev(big)[:, col0:col0 + F]
     H = h.hdc_encode_levelid(lvd, dev_bits(ID), dev_bits(LV), D, hd.knobs(D))
     assert np.array_equal(host_bits(H, D), bits_or)
+
+
+# ------------------------------------------------------------------------------------ seeded fuzz
+@pytest.mark.parametrize("case", range(48))
+def test_similarity_classify_fuzz(hd, h, case):
+    """Seeded random shapes / knobs through hdc_similarity + hdc_classify (every kernel choice the
+    dispatcher can make: popcount, tensor path, split reduction axis, several n-tiles, perforation)."""
+    r = rng(16, case)
+    N = int(r.choice([1, 2, 31, 127, 128, 129, 300, 700, 2100]))
+    K = int(r.choice([1, 2, 5, 16, 17, 63, 64, 65, 100, 257, 300]))
+    D = int(r.choice([32, 33, 100, 512, 1000, 2048, 4099, 9000]))
+    D_eff = int(r.integers(1, D + 1)) if r.random() < 0.5 else D
+    sim, hv_bits = [("HAMMING", 1), ("DOT", 1), ("DOT", 8), ("COS", 8), ("COS", 32), ("COS", 16), ("DOT", 32),
+                    ("DOT", 16)][int(r.integers(0, 8))]
+    begin, stride = 0, 1
+    if r.random() < 0.35:
+        stride = int(r.choice([2, 3, 8, 32]))
+        begin = int(r.integers(0, min(stride, D_eff)))
+    hb = r.integers(0, 2, size=(N, D), dtype=np.uint8)
+    C = (r.standard_normal((K, D)) * 20).astype(np.float32)
+    C[r.random((K, D)) < 0.02] = 0.0
+    simc = getattr(O, "SIM_" + sim)
+    S_or = O.similarity(hb, C, D_eff, simc, hv_bits, begin, stride)
+    kn = hd.knobs(D_eff, hv_bits=hv_bits, sim=getattr(hd, "HDC_SIM_" + sim), perf_begin=begin, perf_stride=stride)
+    Hd, Cd = dev_bits(hb), dev(C)
+    S = h.hdc_similarity(Hd, Cd, kn).cpu().numpy()
+    lab = h.hdc_classify(Hd, Cd, kn).cpu().numpy()
+    lab_or, _, _ = O.classify(S_or, simc)
+    if hv_bits in (8, 1):
+        if sim == "COS":
+            assert np.allclose(S, S_or, rtol=1e-6, atol=1e-9)
+        else:
+            assert np.array_equal(S.astype(np.float64), S_or.astype(np.float64))
+        assert np.array_equal(lab, lab_or)
+    else:
+        idx = O.perforated_index(D_eff, begin, stride)
+        cop = O.class_operand(C[:, idx], len(idx), hv_bits)
+        floor = 1e-6 * np.sqrt(len(idx)) * np.sqrt((cop * cop).sum(axis=1))[None, :] if sim == "DOT" else 1e-6
+        check_scores(S, S_or, floor)
+        check_labels_float(lab, S_or, simc)
