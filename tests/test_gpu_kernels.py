@@ -566,3 +566,87 @@ def test_similarity_classify_fuzz(hd, h, case):
         floor = 1e-6 * np.sqrt(len(idx)) * np.sqrt((cop * cop).sum(axis=1))[None, :] if sim == "DOT" else 1e-6
         check_scores(S, S_or, floor)
         check_labels_float(lab, S_or, simc)
+
+
+@pytest.mark.parametrize("case", range(32))
+def test_encode_rp_fuzz_exact(hd, h, case):
+    """Seeded random shapes / precisions / kernel flags with integer-exact operands (see
+    test_encode_rp_exact_arithmetic): accumulators and bits equal the oracle bit for bit."""
+    r = rng(17, case)
+    N = int(r.choice([1, 2, 127, 128, 129, 255, 257, 600, 1300]))
+    F = int(r.choice([1, 2, 8, 31, 64, 65, 100, 617, 784, 1024, 1500]))
+    D = int(r.choice([32, 33, 100, 255, 256, 257, 1000, 2048, 3001]))
+    D_eff = int(r.integers(1, D + 1)) if r.random() < 0.5 else D
+    prec = ["F32", "BF16", "I8", "B1"][int(r.integers(0, 4))]
+    flags = int(r.choice([0, 1, 2, 4]))
+    X = r.integers(0, 256, size=(N, F)).astype(np.float32)
+    X[r.random((N, F)) < 0.3] = 0
+    P = (1.0 - 2.0 * r.integers(0, 2, size=(D, F))).astype(np.float32)
+    if prec == "I8":
+        X[:, 0] = np.where(X.max(axis=1) > 0, 254.0, 0.0)
+    bits_or, acc_or, _ = O.encode_rp(X, P, D_eff, getattr(O, prec))
+    bits, raw, words = _encode(hd, h, X, P, D_eff, getattr(hd, "HDC_" + prec), flags)
+    assert np.array_equal(raw.astype(np.float64), acc_or)
+    assert np.array_equal(bits, bits_or)
+    W = (D_eff + 31) // 32
+    if D_eff % 32:
+        assert (words[:, W - 1] >> (D_eff % 32) == 0).all()
+
+
+@pytest.mark.parametrize("case", range(32))
+def test_levelid_fuzz_bit_exact(hd, h, case):
+    """Seeded random (N, F, Q, D, D_eff, zero fraction, level dtype): general, fast dense and fast
+    sparse kernels, aligned and unaligned rows."""
+    r = rng(18, case)
+    N = int(r.choice([1, 3, 4, 5, 47, 48, 49, 200]))
+    F = int(r.choice([1, 2, 15, 16, 17, 63, 64, 65, 100, 617, 784, 1019, 1020, 1021, 1400]))
+    wide = r.random() < 0.25
+    Q = int(r.choice([2, 3, 16, 256])) if not wide else int(r.choice([257, 1000]))
+    D = int(r.choice([32, 40, 100, 1024, 2049, 10000]))
+    D_eff = int(r.integers(1, D + 1)) if r.random() < 0.5 else D
+    zeros = float(r.choice([0.0, 0.5, 0.9, 0.99]))
+    lv = r.integers(0, Q, size=(N, F)).astype(np.uint16 if wide else np.uint8)
+    lv[r.random((N, F)) < zeros] = 0
+    ID = r.integers(0, 2, size=(F, D), dtype=np.uint8)
+    LV = gen.level_table(9, Q, D)
+    bits_or = O.encode_levelid(lv, ID, LV, D_eff)
+    lvd = torch.from_numpy(lv.astype(np.int16)).cuda() if wide else dev(lv)
+    H = h.hdc_encode_levelid(lvd, dev_bits(ID), dev_bits(LV), D, hd.knobs(D_eff))
+    assert np.array_equal(host_bits(H, D_eff), bits_or)
+    W = (D_eff + 31) // 32
+    if D_eff % 32:
+        assert (host_words(H)[:, W - 1] >> (D_eff % 32) == 0).all()
+
+
+@pytest.mark.parametrize("case", range(16))
+def test_perceptron_epoch_fuzz_integer_paths(hd, h, case):
+    """Seeded random (N, K, D, D_eff, batch, lr, perforation) on the integer-similarity paths: two
+    epochs, predictions, wrong counts and accumulators bit-identical to the oracle."""
+    r = rng(19, case)
+    N = int(r.choice([1, 50, 257, 1100]))
+    K = int(r.choice([1, 2, 7, 26, 70]))
+    D = int(r.choice([64, 100, 1000, 2100]))
+    D_eff = int(r.integers(1, D + 1)) if r.random() < 0.5 else D
+    B = int(r.choice([0, 1, 13, 64, 4096]))
+    hv_bits, sim = [(1, "HAMMING"), (8, "COS"), (8, "DOT"), (1, "DOT")][int(r.integers(0, 4))]
+    begin, stride = 0, 1
+    if r.random() < 0.3:
+        stride = int(r.choice([2, 5, 8]))
+        begin = int(r.integers(0, min(stride, D_eff)))
+    lr = float(r.choice([1.0, 0.5, 0.03125]))
+    hb = r.integers(0, 2, size=(N, D), dtype=np.uint8)
+    y = r.integers(0, K, size=N).astype(np.int32)
+    C = r.integers(-5, 6, size=(K, D)).astype(np.float32)
+    simc = getattr(O, "SIM_" + sim)
+    kn = hd.knobs(D_eff, hv_bits=hv_bits, sim=getattr(hd, "HDC_SIM_" + sim), perf_begin=begin, perf_stride=stride)
+    Cd, Hd, yd = dev(C.copy()), dev_bits(hb), dev(y)
+    C_or = C[:, :D_eff].copy()
+    for _ in range(2):
+        C_or, wrong_or, pred_or = O.train_epoch(hb, y, C_or, D_eff, hv_bits, simc, lr, B, begin, stride)
+        pred = torch.empty(N, dtype=torch.int32, device="cuda")
+        nw = torch.zeros(1, dtype=torch.int64, device="cuda")
+        h.hdc_train_epoch(hd.HDC_TRAIN_PERCEPTRON, Hd, yd, Cd, kn, lr=lr, batch=B, pred=pred, n_wrong=nw)
+        assert np.array_equal(pred.cpu().numpy(), pred_or)
+        assert int(nw.item()) == wrong_or
+        assert np.array_equal(Cd.cpu().numpy()[:, :D_eff], C_or)
+    assert np.array_equal(Cd.cpu().numpy()[:, D_eff:], C[:, D_eff:])
