@@ -97,21 +97,34 @@ def rp_operands(X: np.ndarray, P: np.ndarray, precision: int):
 
 
 def encode_rp(X: np.ndarray, P: np.ndarray, D_eff: int, precision: int = F32,
-              want_absum: bool = False):
+              want_absum: bool = False, f_begin: int = 0, f_stride: int = 1):
     """Random-projection encode + sign (Listing 1 L68-L70 `__hetero_hdc_matmul`,
     L155 "matrix-vector dot-product", L161 "{+1,-1} representation"; always binarised: A5).
 
         acc[n,d] = sum_{f<F} x~[n,f] * p~[d,f]      (P is [D][F]: `hypermatrix<2048,617>`, L65)
         bit[n,d] = [acc[n,d] < 0]  for d < D_eff     (sgn(0) = +1, A1)
 
-    The F reduction is never perforated (L157, L187).  float64 accumulation; for INT8 the
-    operands are integers <= 127 so every product and sum is exact in float64.
-    Returns bits [N][D_eff] uint8, acc [N][D_eff] float64 and optionally
-    absum[n,d] = sum_f |x~ p~| (used by the sign-agreement band, S4)."""
-    Xo, Po = rp_operands(np.asarray(X), np.asarray(P)[:D_eff], precision)
-    acc = Xo @ Po.T
+    float64 accumulation; for INT8 the operands are integers <= 127 so every product and sum is
+    exact in float64.  Returns bits [N][D_eff] uint8, acc [N][D_eff] float64 and optionally
+    absum[n,d] = sum_f |x~ p~| (used by the sign-agreement band, S4).
+
+    Reduction perforation of the F axis (off by default: L157 / L187 keep it out of the encoders
+    because it "often degrades the quality-of-service"; L155 defines it: "for operations such as
+    matrix-vector dot products, the results are scaled appropriately to compensate for the skipped
+    iterations"; reading A18): the loop visits f = f_begin, f_begin + f_stride, ... < F, the operands
+    at `precision` are those of the gathered columns (per-row int8 scales over the visited features),
+    and acc (and absum) are multiplied by F / F_visited."""
+    X, P = np.asarray(X), np.asarray(P)[:D_eff]
+    scale = 1.0
+    if f_begin != 0 or f_stride != 1:
+        F = X.shape[1]
+        idx = perforated_index(F, f_begin, f_stride)
+        X, P = X[:, idx], P[:, idx]
+        scale = F / len(idx)
+    Xo, Po = rp_operands(X, P, precision)
+    acc = (Xo @ Po.T) * scale
     bits = (acc < 0).astype(np.uint8)
-    absum = (np.abs(Xo) @ np.abs(Po).T) if want_absum else None
+    absum = (np.abs(Xo) @ np.abs(Po).T) * scale if want_absum else None
     return bits, acc, absum
 
 

@@ -645,3 +645,68 @@ def test_levelid_random_shapes_against_loops(N, F, Q, D, seed):
         for d in range(D_eff):
             cnt = sum(int(ID[f, d]) ^ int(LV[lv[n, f], d]) for f in range(F))
             assert bits[n, d] == (1 if 2 * cnt > F else 0)
+
+
+# ------------------------------------------------------------------------------------- A18 encode perforation
+@pytest.mark.parametrize("begin,stride,F", [(0, 2, 16), (1, 3, 17), (5, 4, 9), (0, 1, 7), (3, 8, 12)])
+def test_perforated_encode_brute_force(begin, stride, F):
+    """the reduction loop skips iterations at a stride and, for matrix-vector dot
+    products, "the results are scaled appropriately to compensate for the skipped iterations"
+    (reading A18: by F / F_visited).  Loops written out by hand, fp32 operands."""
+    r = rng(181)
+    N, D = 5, 11
+    X = r.standard_normal((N, F)).astype(np.float32)
+    P = r.standard_normal((D, F)).astype(np.float32)
+    vis = [f for f in range(F) if f >= begin and (f - begin) % stride == 0]
+    want = np.zeros((N, D))
+    for n in range(N):
+        for d in range(D):
+            t = 0.0
+            for f in vis:
+                t += float(X[n, f]) * float(P[d, f])
+            want[n, d] = t * F / len(vis)
+    bits, acc, absum = o.encode_rp(X, P, D, o.F32, want_absum=True, f_begin=begin, f_stride=stride)
+    assert np.allclose(acc, want, rtol=1e-12, atol=1e-12)
+    assert np.array_equal(bits, (want < 0).astype(np.uint8))
+    assert (absum >= np.abs(acc) - 1e-9).all()
+
+
+def test_perforated_encode_of_a_constant_summand_is_exact():
+    """The compensation is exact when every term of the reduction is the same: x = p = 1 gives
+    acc = F at every stride and offset, also when the stride does not divide F."""
+    F = 617
+    X, P = np.ones((2, F), dtype=np.float32), np.ones((3, F), dtype=np.float32)
+    for begin, stride in [(0, 2), (0, 8), (5, 7), (616, 3), (0, 617)]:
+        _, acc, _ = o.encode_rp(X, P, 3, o.F32, f_begin=begin, f_stride=stride)
+        assert np.allclose(acc, F, rtol=1e-14)
+    # and an alternating summand +1, -1, ... at stride 2 sees only one sign: acc = +F or -F
+    X[:, 1::2] = -1.0
+    _, acc0, _ = o.encode_rp(X, P, 3, o.F32, f_begin=0, f_stride=2)
+    _, acc1, _ = o.encode_rp(X, P, 3, o.F32, f_begin=1, f_stride=2)
+    assert np.allclose(acc0, F) and np.allclose(acc1, -F)
+
+
+def test_perforated_encode_int8_scales_come_from_the_visited_features():
+    """Per-row int8 quantisation of a perforated contraction sees only the gathered columns: a large
+    value in a skipped column must not change the codes of the visited ones."""
+    X = np.array([[1.0, 1000.0, -2.0, 1000.0, 4.0, 1000.0]], dtype=np.float32)
+    P = np.array([[1.0, 9.0, 1.0, 9.0, 1.0, 9.0], [1.0, 9.0, -1.0, 9.0, -1.0, 9.0]], dtype=np.float32)
+    bits, acc, _ = o.encode_rp(X, P, 2, o.I8, f_begin=0, f_stride=2)
+    # visited x = (1, -2, 4): scale 127/4 -> codes (32, -64, 127) (31.75 -> 32, -63.5 -> -64 ties to even);
+    # p rows (1,1,1) and (1,-1,-1) -> (127,127,127) and (127,-127,-127)
+    assert np.array_equal(acc, np.array([[(32 - 64 + 127) * 127 * 2.0, (32 + 64 - 127) * 127 * 2.0]]))
+    assert bits.tolist() == [[0, 1]]
+    # without perforation the 1000s set the scale: x codes (0, 127, 0, 127, 1, 127) (4 * 0.127 = 0.508 -> 1),
+    # p row 0 codes (14, 127, 14, 127, 14, 127) (127/9 = 14.1)
+    _, acc_full, _ = o.encode_rp(X, P, 2, o.I8)
+    assert acc_full[0, 0] == 3 * 127 * 127 + 14
+
+
+def test_unperforated_encode_arguments_change_nothing():
+    r = rng(182)
+    X = r.standard_normal((6, 13)).astype(np.float32)
+    P = r.standard_normal((9, 13)).astype(np.float32)
+    for prec in (o.F32, o.BF16, o.I8):
+        a = o.encode_rp(X, P, 9, prec, want_absum=True)
+        b = o.encode_rp(X, P, 9, prec, want_absum=True, f_begin=0, f_stride=1)
+        assert all(np.array_equal(u, v) for u, v in zip(a, b))
