@@ -97,8 +97,17 @@ enum {
  *             the visited dimensions of both operands; nothing is rescaled (L155); the int8 class
  *             scale and the cosine norms are taken over the visited dimensions.  0 <= perf_begin
  *             < D_eff; perf_stride 0 or 1 = every dimension.  Encoders and class updates are not
- *             perforated (L157, L187).  Not available with HDC_FLAG_SIMT for DOT / COS
- *             (HDC_ERR_UNSUPPORTED).                                                             */
+ *             perforated by these two (L157, L187).  Not available with HDC_FLAG_SIMT for DOT /
+ *             COS (HDC_ERR_UNSUPPORTED).
+ *  enc_perf_begin, enc_perf_stride   reduction perforation of the ENCODE contraction, read by
+ *             hdc_encode_rp and hdc_infer_rp_host only (L155: "for operations such as matrix-vector
+ *             dot products, the results are scaled appropriately to compensate for the skipped
+ *             iterations"): the F reduction visits f = enc_perf_begin + j*enc_perf_stride < F, the
+ *             operands at `precision` are those of the gathered columns (per-row int8 scales over
+ *             the visited features) and the accumulators are multiplied by F / F_visited.  Off
+ *             (0, 0) by default: the paper keeps perforation out of the encoders because it "often
+ *             degrades the quality-of-service" (L157, L187).  0 <= enc_perf_begin < F;
+ *             enc_perf_stride 0 or 1 = every feature.                                            */
 typedef struct {
   int32_t D_eff;
   int32_t precision;
@@ -107,6 +116,8 @@ typedef struct {
   int32_t flags;
   int32_t perf_begin;
   int32_t perf_stride;
+  int32_t enc_perf_begin;
+  int32_t enc_perf_stride;
 } hdc_knobs_t;
 
 /* ---- handle ------------------------------------------------------------------------------ */
@@ -141,11 +152,13 @@ size_t hdc_workspace_bytes(hdc_handle_t h, int32_t op, int64_t N, int32_t F_or_Q
 /* ---- (1a) random-projection encode + sign + pack ------------------------------------------
  * PAPER.md Listing 1 L68-L70 `__hetero_hdc_matmul`, L155, L161 (automatic binarization).
  *   acc[n,d] = sum_{f<F} x~[n,f] * p~[d,f],   bit[n,d] = [acc[n,d] < 0],   d < D_eff
- * (x~, p~ = operands at knobs->precision).  The F reduction is never perforated (L157, L187).
+ * (x~, p~ = operands at knobs->precision).  The F reduction is perforated only when
+ * knobs->enc_perf_* ask for it (see hdc_knobs_t); the bits do not depend on the compensation scale.
  * X [N][ldx] of x_dtype (HDC_F32 or HDC_BF16); P [D][ldp] of p_dtype (HDC_F32 or HDC_BF16).
  * A bf16 input under precision HDC_F32 is widened exactly.  out_kinds: HDC_OUT_BITS writes
  * Hbits [N][ldh_words]; HDC_OUT_RAW additionally writes the accumulators to Hraw [N][ldraw]
- * (float for F32/BF16/B1, int32 for I8).  Unused outputs may be NULL. */
+ * (float for F32/BF16/B1, int32 for I8; with a perforated reduction always float:
+ * fl32(fl32(acc) * fl32(F / F_visited))).  Unused outputs may be NULL. */
 int32_t hdc_encode_rp(hdc_handle_t h, const void* X, int32_t x_dtype, int64_t N, int32_t F,
                       int64_t ldx, const void* P, int32_t p_dtype, int32_t D, int64_t ldp,
                       const hdc_knobs_t* knobs, int32_t out_kinds, uint32_t* Hbits,

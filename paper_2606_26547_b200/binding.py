@@ -35,7 +35,7 @@ EXPORTS = ("hdc_create", "hdc_destroy", "hdc_last_error", "hdc_version", "hdc_la
 class hdc_knobs_t(C.Structure):
     _fields_ = [("D_eff", C.c_int32), ("precision", C.c_int32), ("hv_bits", C.c_int32),
                 ("sim", C.c_int32), ("flags", C.c_int32), ("perf_begin", C.c_int32),
-                ("perf_stride", C.c_int32)]
+                ("perf_stride", C.c_int32), ("enc_perf_begin", C.c_int32), ("enc_perf_stride", C.c_int32)]
 
 
 class HdcError(RuntimeError):
@@ -101,9 +101,10 @@ def lib() -> C.CDLL:
 
 
 def knobs(D_eff: int, precision: int = HDC_F32, hv_bits: int = 32, sim: int = HDC_SIM_COS,
-          flags: int = 0, perf_begin: int = 0, perf_stride: int = 1) -> hdc_knobs_t:
+          flags: int = 0, perf_begin: int = 0, perf_stride: int = 1, enc_perf_begin: int = 0,
+          enc_perf_stride: int = 1) -> hdc_knobs_t:
     return hdc_knobs_t(int(D_eff), int(precision), int(hv_bits), int(sim), int(flags), int(perf_begin),
-                       int(perf_stride))
+                       int(perf_stride), int(enc_perf_begin), int(enc_perf_stride))
 
 
 _DT = {torch.float32: HDC_F32, torch.bfloat16: HDC_BF16, torch.int8: HDC_I8, torch.uint8: HDC_U8,
@@ -187,7 +188,8 @@ class Handle:
         Hraw = None
         if want_raw:
             Hraw = torch.empty((N, kn.D_eff), device=self.device,
-                               dtype=torch.int32 if kn.precision == HDC_I8 else torch.float32)
+                               dtype=torch.int32 if kn.precision == HDC_I8 and kn.enc_perf_begin == 0
+                               and kn.enc_perf_stride <= 1 else torch.float32)
         ws, wsb = self._workspace(self.workspace_bytes(HDC_OP_ENCODE_RP, N, F, D, 0, kn))
         rc = self._L.hdc_encode_rp(self._h, _ptr(X), _DT[X.dtype], N, F, _rowmajor(X, "X"), _ptr(P),
                                    _DT[P.dtype], D, _rowmajor(P, "P"), C.byref(kn),

@@ -90,6 +90,9 @@ int check_sim_knobs(hdc_ctx* h, const hdc_knobs_t* k) {
   return HDC_OK;
 }
 Perf perf_of(const hdc_knobs_t* k) { return Perf{k->perf_begin, k->perf_stride <= 1 ? 1 : k->perf_stride}; }
+Perf enc_perf_of(const hdc_knobs_t* k) {
+  return Perf{k->enc_perf_begin, k->enc_perf_stride <= 1 ? 1 : k->enc_perf_stride};
+}
 
 // ------------------------------------------------------------------------------------- encode
 // Reduction-segment schedule of the fp32-precision contraction over 3-way bf16 splits: segment s
@@ -140,10 +143,9 @@ void plan_encode(const hdc_ctx* h, int64_t N, int F, int D_eff, const hdc_knobs_
   if (!p_inplace) pl.Ps = b.take<__nv_bfloat16>((size_t)D_eff * pl.Fp);
 }
 
-int do_encode_rp(hdc_ctx* h, const void* X, int x_dtype, int64_t N, int F, int64_t ldx, const void* P,
-                 int p_dtype, int D, int64_t ldp, const hdc_knobs_t* k, int out_kinds, uint32_t* Hbits,
-                 int64_t ldh, void* Hraw, int64_t ldraw, Bump& b, size_t ws_bytes, cudaStream_t st) {
-  (void)D;
+int encode_rp_core(hdc_ctx* h, const void* X, int x_dtype, int64_t N, int F, int64_t ldx, const void* P,
+                   int p_dtype, int64_t ldp, const hdc_knobs_t* k, int out_kinds, uint32_t* Hbits,
+                   int64_t ldh, void* Hraw, int64_t ldraw, Bump& b, size_t ws_bytes, cudaStream_t st) {
   const int D_eff = k->D_eff;
   const int prec = k->precision;
   const bool want_raw = (out_kinds & HDC_OUT_RAW) != 0;
@@ -243,6 +245,57 @@ int do_encode_rp(hdc_ctx* h, const void* X, int x_dtype, int64_t N, int F, int64
   const int pr = p_dtype == HDC_BF16 ? OPK_BF16 : OPK_F32_RBF16;
   ce = launch_gemm_simt(Operand{X, ldx, xr}, Operand{P, ldp, pr}, N, D_eff, F, false, e, st, &h->launches);
   return ce == cudaSuccess ? HDC_OK : cuda_fail(h, ce, "encode_rp bf16");
+}
+
+// Workspace of hdc_encode_rp: the compacted operands of a perforated contraction (upper bound: 4-byte
+// elements) followed by the staging buffers of the contraction itself.
+void encode_ws(const hdc_ctx* h, int64_t N, int F, int D_eff, const hdc_knobs_t* k, Bump& b) {
+  const Perf ef = enc_perf_of(k);
+  if (perf_on(ef)) {
+    F = perf_count(ef, F);
+    const int64_t ldg = round_up(F, 16);
+    b.take<float>((size_t)N * ldg);
+    b.take<float>((size_t)D_eff * ldg);
+  }
+  EncodePlan pl;
+  plan_encode(h, N, F, D_eff, k, false, false, b, pl);
+}
+
+// hdc_encode_rp after argument checks.  A perforated F reduction (knobs enc_perf_*; PAPER.md L155,
+// reading A18) is the same contraction over compacted copies of the visited columns, with the raw
+// accumulators multiplied by F / F_visited afterwards (the sign bits do not depend on that scale).
+int do_encode_rp(hdc_ctx* h, const void* X, int x_dtype, int64_t N, int F, int64_t ldx, const void* P,
+                 int p_dtype, int D, int64_t ldp, const hdc_knobs_t* k, int out_kinds, uint32_t* Hbits,
+                 int64_t ldh, void* Hraw, int64_t ldraw, Bump& b, size_t ws_bytes, cudaStream_t st) {
+  (void)D;
+  const Perf ef = enc_perf_of(k);
+  if (!perf_on(ef))
+    return encode_rp_core(h, X, x_dtype, N, F, ldx, P, p_dtype, ldp, k, out_kinds, Hbits, ldh, Hraw, ldraw, b,
+                          ws_bytes, st);
+  const int D_eff = k->D_eff;
+  const int Fv = perf_count(ef, F);
+  const int64_t ldg = round_up(Fv, 16);
+  const int xs = x_dtype == HDC_BF16 ? 2 : 4;
+  const int ps = p_dtype == HDC_BF16 ? 2 : (p_dtype == HDC_I8 ? 1 : 4);
+  void* Xg = b.take<uint8_t>((size_t)N * ldg * xs);
+  void* Pg = b.take<uint8_t>((size_t)D_eff * ldg * ps);
+  {  // the whole workspace is checked before the first launch
+    Bump dry(nullptr);
+    dry.off = b.off;
+    EncodePlan pl;
+    plan_encode(h, N, Fv, D_eff, k, false, false, dry, pl);
+    if (dry.off > ws_bytes) return fail(h, HDC_ERR_WORKSPACE, "encode_rp: workspace too small");
+  }
+  cudaError_t ce = launch_gather_cols(X, xs, N, ldx, ef, Fv, Xg, ldg, st, &h->launches);
+  if (ce != cudaSuccess) return cuda_fail(h, ce, "gather X");
+  ce = launch_gather_cols(P, ps, D_eff, ldp, ef, Fv, Pg, ldg, st, &h->launches);
+  if (ce != cudaSuccess) return cuda_fail(h, ce, "gather P");
+  int rc = encode_rp_core(h, Xg, x_dtype, N, Fv, ldg, Pg, p_dtype, ldg, k, out_kinds, Hbits, ldh, Hraw, ldraw, b,
+                          ws_bytes, st);
+  if (rc != HDC_OK || !(out_kinds & HDC_OUT_RAW)) return rc;
+  const float scale = (float)((double)F / (double)Fv);
+  ce = launch_scale_raw(Hraw, N, D_eff, ldraw, scale, k->precision == HDC_I8, st, &h->launches);
+  return ce == cudaSuccess ? HDC_OK : cuda_fail(h, ce, "scale raw");
 }
 
 // ------------------------------------------------------------------------------------- similarity
@@ -396,7 +449,7 @@ constexpr int64_t HOST_CHUNK = 16384;
 using namespace hdc;
 
 // =================================================================================== handle
-extern "C" int32_t hdc_version(void) { return 101; }  // 1.1: perforation knobs, k-means, train_delta/apply, u16 levels
+extern "C" int32_t hdc_version(void) { return 102; }  // 1.2: + perforation of the encode contraction (enc_perf_*)
 
 extern "C" int32_t hdc_create(hdc_handle_t* out, int32_t device) {
   if (!out) return HDC_ERR_INVALID_ARG;
@@ -484,8 +537,7 @@ extern "C" size_t hdc_workspace_bytes(hdc_handle_t h, int32_t op, int64_t N, int
   Bump b(nullptr);
   switch (op) {
     case HDC_OP_ENCODE_RP: {
-      EncodePlan pl;
-      plan_encode(h, N, F_or_Q, k.D_eff, &k, false, false, b, pl);
+      encode_ws(h, N, F_or_Q, k.D_eff, &k, b);
       return b.off + 256;
     }
     case HDC_OP_ENCODE_LEVELID:
@@ -505,8 +557,7 @@ extern "C" size_t hdc_workspace_bytes(hdc_handle_t h, int32_t op, int64_t N, int
       b.take<float>((size_t)chunk * F_or_Q);
       b.take<uint32_t>((size_t)chunk * words_of(k.D_eff));
       b.take<int32_t>((size_t)N);
-      EncodePlan pl;
-      plan_encode(h, chunk, F_or_Q, k.D_eff, &k, false, false, b, pl);
+      encode_ws(h, chunk, F_or_Q, k.D_eff, &k, b);
       return b.off + 512 + similarity_ws(chunk, K, &k);
     }
     default:
@@ -528,6 +579,8 @@ static int check_encode_rp_args(hdc_ctx* h, const void* X, int x_dtype, int64_t 
     return fail(h, HDC_ERR_INVALID_ARG, "encode_rp: precision");
   if (p_dtype == HDC_I8 && k->precision != HDC_I8)
     return fail(h, HDC_ERR_INVALID_ARG, "encode_rp: int8 P needs precision HDC_I8");
+  if (k->enc_perf_stride < 0 || k->enc_perf_begin < 0 || k->enc_perf_begin >= F)
+    return fail(h, HDC_ERR_INVALID_ARG, "encode_rp: need enc_perf_stride >= 0 and 0 <= enc_perf_begin < F");
   const size_t xa = x_dtype == HDC_BF16 ? 2 : 4, pa = p_dtype == HDC_BF16 ? 2 : (p_dtype == HDC_I8 ? 1 : 4);
   if ((reinterpret_cast<uintptr_t>(X) % xa) || (reinterpret_cast<uintptr_t>(P) % pa))
     return fail(h, HDC_ERR_ALIGNMENT, "encode_rp: operand not element aligned");

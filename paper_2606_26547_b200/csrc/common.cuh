@@ -104,6 +104,12 @@ size_t sim_tc_partial_bytes(int64_t N, int K, int hv_bits, int D_eff, int sm_cou
 cudaError_t launch_tensor_amax(const float* C, int K, int D_eff, int64_t ldc, Perf pf, float* amax,
                                cudaStream_t st, int64_t* nlaunch);
 // mask[w] = bits of word w whose dimension is visited and < D_eff (W words)
+// Perforated encode contraction: compacted copy of the visited columns (esize = element bytes 1/2/4)
+// and the compensation scale applied to the optional raw accumulators.
+cudaError_t launch_gather_cols(const void* src, int esize, int64_t rows, int64_t ld_src, Perf pf, int n_vis,
+                               void* dst, int64_t ld_dst, cudaStream_t st, int64_t* nlaunch);
+cudaError_t launch_scale_raw(void* raw, int64_t rows, int cols, int64_t ld, float scale, int from_i32,
+                             cudaStream_t st, int64_t* nlaunch);
 cudaError_t launch_perf_mask(uint32_t* mask, int W, int D_eff, Perf pf, cudaStream_t st, int64_t* nlaunch);
 
 // fp32/bf16 -> bf16 staging with zero padding of the reduction axis: dst [rows][ld_dst]

@@ -256,6 +256,60 @@ __global__ void perf_mask_kernel(uint32_t* __restrict__ mask, int W, int D_eff, 
 
 }  // namespace
 
+namespace {
+// Perforated encode contraction (reading A18): compacts the visited columns
+// f = begin + j*stride of a row-major matrix; columns >= n_vis of the copy are zero.
+template <typename T>
+__global__ void gather_cols_kernel(const T* __restrict__ src, int64_t rows, int64_t ld_src, Perf pf, int n_vis,
+                                   T* __restrict__ dst, int64_t ld_dst) {
+  const int64_t total = rows * ld_dst;
+  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < total;
+       i += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t r = i / ld_dst;
+    const int j = (int)(i - r * ld_dst);
+    T v = T(0);
+    if (j < n_vis) v = src[r * ld_src + pf.begin + (int64_t)j * pf.stride];
+    dst[i] = v;
+  }
+}
+
+// raw[n,d] = fl32( fl32(acc[n,d]) * scale ), in place (int32 accumulators are converted first).
+__global__ void scale_raw_kernel(void* __restrict__ raw, int64_t rows, int cols, int64_t ld, float scale,
+                                 int from_i32) {
+  const int64_t total = rows * cols;
+  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < total;
+       i += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t r = i / cols;
+    const int64_t idx = r * ld + (i - r * cols);
+    const float a = from_i32 ? (float)reinterpret_cast<const int32_t*>(raw)[idx]
+                             : reinterpret_cast<const float*>(raw)[idx];
+    reinterpret_cast<float*>(raw)[idx] = __fmul_rn(a, scale);
+  }
+}
+}  // namespace
+
+cudaError_t launch_gather_cols(const void* src, int esize, int64_t rows, int64_t ld_src, Perf pf, int n_vis,
+                               void* dst, int64_t ld_dst, cudaStream_t st, int64_t* nlaunch) {
+  if (rows <= 0) return cudaSuccess;
+  const int g = grid_for(rows * ld_dst, 256, 148 * 16);
+  if (esize == 4)
+    gather_cols_kernel<uint32_t><<<g, 256, 0, st>>>((const uint32_t*)src, rows, ld_src, pf, n_vis, (uint32_t*)dst, ld_dst);
+  else if (esize == 2)
+    gather_cols_kernel<uint16_t><<<g, 256, 0, st>>>((const uint16_t*)src, rows, ld_src, pf, n_vis, (uint16_t*)dst, ld_dst);
+  else
+    gather_cols_kernel<uint8_t><<<g, 256, 0, st>>>((const uint8_t*)src, rows, ld_src, pf, n_vis, (uint8_t*)dst, ld_dst);
+  ++*nlaunch;
+  return cudaGetLastError();
+}
+
+cudaError_t launch_scale_raw(void* raw, int64_t rows, int cols, int64_t ld, float scale, int from_i32,
+                             cudaStream_t st, int64_t* nlaunch) {
+  if (rows <= 0) return cudaSuccess;
+  scale_raw_kernel<<<grid_for(rows * cols, 256, 148 * 16), 256, 0, st>>>(raw, rows, cols, ld, scale, from_i32);
+  ++*nlaunch;
+  return cudaGetLastError();
+}
+
 cudaError_t launch_perf_mask(uint32_t* mask, int W, int D_eff, Perf pf, cudaStream_t st, int64_t* nlaunch) {
   perf_mask_kernel<<<(W + 255) / 256, 256, 0, st>>>(mask, W, D_eff, pf);
   ++*nlaunch;

@@ -650,3 +650,99 @@ def test_perceptron_epoch_fuzz_integer_paths(hd, h, case):
         assert int(nw.item()) == wrong_or
         assert np.array_equal(Cd.cpu().numpy()[:, :D_eff], C_or)
     assert np.array_equal(Cd.cpu().numpy()[:, D_eff:], C[:, D_eff:])
+
+
+# ------------------------------------------------------------------------------------ A18 perforated encode
+def _encode_perf(hd, h, X, P, D_eff, prec, begin, stride, flags=0, bf16_inputs=False):
+    kn = hd.knobs(D_eff, precision=prec, flags=flags, enc_perf_begin=begin, enc_perf_stride=stride)
+    Xd, Pd = dev(X), dev(P)
+    if bf16_inputs:
+        Xd, Pd = Xd.to(torch.bfloat16), Pd.to(torch.bfloat16)
+    H, raw = h.hdc_encode_rp(Xd, Pd, kn, want_raw=True)
+    torch.cuda.synchronize()
+    assert raw.dtype == torch.float32
+    return host_bits(H, D_eff), raw.cpu().numpy(), host_words(H)
+
+
+@pytest.mark.parametrize("prec", ["F32", "BF16", "I8", "B1"])
+@pytest.mark.parametrize("flags", [0, 1])
+@pytest.mark.parametrize("N,F,D,D_eff,begin,stride", [(200, 64, 2048, 2048, 0, 2), (131, 617, 1000, 999, 5, 8),
+                                                      (300, 100, 700, 33, 99, 3), (70, 784, 520, 515, 1, 2),
+                                                      (129, 1024, 300, 300, 0, 4), (5, 7, 40, 40, 6, 1)])
+def test_encode_rp_perforated_exact_arithmetic(hd, h, prec, flags, N, F, D, D_eff, begin, stride):
+    """Perforated F reduction (reading A18) on integer-exact operands: bits equal the
+    oracle bit for bit; the scaled accumulators agree to fp32 rounding of the scale (exactly when
+    F / F_visited is a power of two)."""
+    r = rng(20, N, F, D_eff, begin, stride)
+    X = r.integers(0, 256, size=(N, F)).astype(np.float32)
+    X[r.random((N, F)) < 0.3] = 0
+    P = (1.0 - 2.0 * r.integers(0, 2, size=(D, F))).astype(np.float32)
+    if prec == "I8":
+        vis = O.perforated_index(F, begin, stride)
+        X[:, vis[0]] = np.where(X[:, vis].max(axis=1) > 0, 254.0, 0.0)   # row max 254 over the visited columns
+        X[:, np.setdiff1d(np.arange(F), vis)] *= 3.0                     # skipped columns must not set the scale
+    bits_or, acc_or, _ = O.encode_rp(X, P, D_eff, getattr(O, prec), f_begin=begin, f_stride=stride)
+    bits, raw, words = _encode_perf(hd, h, X, P, D_eff, getattr(hd, "HDC_" + prec), begin, stride, flags)
+    assert np.array_equal(bits, bits_or)
+    n_vis = len(O.perforated_index(F, begin, stride))
+    if (F / n_vis) == 2.0 ** round(np.log2(F / n_vis)):
+        assert np.array_equal(raw.astype(np.float64), acc_or)
+    else:
+        assert np.allclose(raw, acc_or, rtol=3e-7, atol=0)
+    W = (D_eff + 31) // 32
+    if D_eff % 32:
+        assert (words[:, W - 1] >> (D_eff % 32) == 0).all()
+
+
+@pytest.mark.parametrize("prec", ["F32", "BF16"])
+def test_encode_rp_perforated_float_c2_shape(hd, h, prec):
+    w = gen.c2_isolet_shaped(D=1500, n_tr=8, n_te=300)
+    X, P, D_eff = w["Xte"], w["P"], 1500
+    for begin, stride, bf in [(0, 2, False), (3, 8, False), (1, 2, True)]:
+        Xo, Po = X, P
+        if bf:   # bf16 inputs handed over as bf16: the compacted copies stay bf16
+            Xo = np.asarray(torch.from_numpy(X).to(torch.bfloat16).float())
+            Po = np.asarray(torch.from_numpy(P).to(torch.bfloat16).float())
+        bits_or, acc_or, absum = O.encode_rp(Xo, Po, D_eff, getattr(O, prec), want_absum=True, f_begin=begin,
+                                             f_stride=stride)
+        bits, raw, _ = _encode_perf(hd, h, Xo, Po, D_eff, getattr(hd, "HDC_" + prec), begin, stride, 0, bf)
+        assert (np.abs(raw - acc_or) <= 1e-3 * np.abs(acc_or) + 1e-6 * absum).all()
+        n = check_sign_band(bits, bits_or, acc_or, absum, X.shape[1])
+        assert n <= 1e-4 * bits.size
+
+
+def test_encode_rp_perforation_argument_errors_and_workspace(hd, h):
+    X = torch.zeros((8, 16), dtype=torch.float32, device="cuda")
+    P = torch.zeros((128, 16), dtype=torch.float32, device="cuda")
+    before = h.launch_count()
+    for kw in ({"enc_perf_begin": 16}, {"enc_perf_begin": -1}, {"enc_perf_stride": -2}):
+        with pytest.raises(hd.HdcError) as ei:
+            h.hdc_encode_rp(X, P, hd.knobs(128, **kw))
+        assert ei.value.code == hd.HDC_ERR_INVALID_ARG
+    assert h.launch_count() == before
+    kn0, kn1 = hd.knobs(128), hd.knobs(128, enc_perf_stride=2)
+    assert h.workspace_bytes(hd.HDC_OP_ENCODE_RP, 8, 16, 128, 0, kn1) > 0
+    # a perforated similarity knob does not touch the encoder and vice versa
+    H0 = h.hdc_encode_rp(X + 1.0, P + 1.0, kn0)
+    H1 = h.hdc_encode_rp(X + 1.0, P + 1.0, hd.knobs(128, perf_begin=3, perf_stride=8))
+    assert torch.equal(H0, H1)
+
+
+def test_infer_rp_host_with_perforated_encode_equals_device_calls(hd, h):
+    """hdc_infer_rp_host reads the same knobs: a perforated encode (enc_perf_*) and a perforated
+    similarity (perf_*) in one call give the labels of the two device calls; integer paths, exact."""
+    r = rng(21)
+    N, F, D, K = 40000, 100, 1100, 7                       # > 2 chunks of the host pipeline
+    X = r.integers(0, 256, size=(N, F)).astype(np.float32)
+    P = (1.0 - 2.0 * r.integers(0, 2, size=(D, F))).astype(np.float32)
+    C = r.integers(-9, 10, size=(K, D)).astype(np.float32)
+    kn = hd.knobs(1000, precision=hd.HDC_BF16, hv_bits=1, sim=hd.HDC_SIM_HAMMING, perf_begin=1, perf_stride=2,
+                  enc_perf_begin=2, enc_perf_stride=3)
+    Pd, Cd = dev(P), dev(C)
+    lab_dev = h.hdc_classify(h.hdc_encode_rp(dev(X), Pd, kn), Cd, kn).cpu().numpy()
+    lab_host = h.hdc_infer_rp_host(torch.from_numpy(X).pin_memory(), Pd, Cd, kn).numpy()
+    assert np.array_equal(lab_host, lab_dev)
+    sub = slice(0, 300)
+    bits_or, _, _ = O.encode_rp(X[sub], P, 1000, O.BF16, f_begin=2, f_stride=3)
+    lab_or, _, _ = O.classify(O.similarity(bits_or, C, 1000, O.SIM_HAMMING, 1, 1, 2), O.SIM_HAMMING)
+    assert np.array_equal(lab_dev[sub], lab_or)
