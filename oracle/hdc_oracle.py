@@ -13,7 +13,9 @@ bipolar identity dot = D_eff - 2*Hamming, near-orthogonality |cos| <~ 3/sqrt(D),
 angle/Hamming closed form for Gaussian projections, majority-bundling recovery probability
 1/2 + C(F-1,(F-1)/2)/2^F, D_eff slice-equivalence and Listing 1's "first 1024 of 2048",
 bf16 RNE against ml_dtypes, perceptron invariants (sum_k Delta = 0; B=1 == textbook online
-perceptron).  Unpinned: accuracy parity with the paper's ISOLET numbers (datasets absent) --
+perceptron); the ADC-quantised chunked dot (S12) against hand loops, the transparent-window case
+(= D_eff - 2*Hamming) and a hand-worked clipped example -- its transfer function itself is a
+reading (A19), the paper prints no formula: "parity unpinned" for the ADC formula.  Unpinned: accuracy parity with the paper's ISOLET numbers (datasets absent) --
 "parity unpinned" for that one item only.
 
 Conventions (S0; paper silent, readings A1-A3): bipolar v in {+1,-1}; bit b = [v == -1], so
@@ -236,6 +238,44 @@ def similarity(hbits: np.ndarray, C_acc: np.ndarray, D_eff: int, sim: int, hv_bi
     if sim == SIM_COS:
         return cosine(hbits, cop, D_eff)
     raise ValueError("sim")
+
+
+# ------------------------------------------------------------------------------------- S12
+def adc_quantize(p: np.ndarray, res: int, step: int, floor: int, ceil: int) -> np.ndarray:
+    """Transfer function of the analogue-to-digital converter that reads one array chunk's partial
+    dot product in the SpecPCM simulator (PAPER.md L273: knobs ADC_RES, ADC_STEP, ADC_FLOOR, ADC_CEIL;
+    "each partial dot product quantized by the ADC before accumulation"; "Clipping below -3 ...
+    narrowing the ADC input range ... allows fewer quantization levels (lower ADC_RES)").  The paper
+    gives no formula; reading A19: the input is clipped to [floor, ceil], converted to the nearest of
+    2^res codes spaced `step` apart starting at `floor` (halves round up, codes saturate at
+    2^res - 1), and read back as floor + code*step.  The paper's baseline window (floor -127, ceil 128,
+    res 8, step 1) is then exactly 256 codes and transparent on [-127, 128].  Integers in, out."""
+    if res < 1 or res > 16 or step < 1 or floor > ceil:
+        raise ValueError("bad ADC parameters")
+    p = np.clip(np.asarray(p, dtype=np.int64), floor, ceil)
+    code = (p - floor + step // 2) // step
+    code = np.minimum(code, (1 << res) - 1)
+    return floor + code * step
+
+
+def similarity_adc(hbits: np.ndarray, C_acc: np.ndarray, D_eff: int, res: int, step: int, floor: int,
+                   ceil: int, chunk: int = 128) -> np.ndarray:
+    """Chunked, ADC-quantised dot-product similarity ("The SpecPCM simulator computes
+    dot-product similarity over 128-element array chunks, with each partial dot product quantized by
+    the ADC before accumulation"; MLC=1, "+-1 encoded hypervectors": query and class operand bipolar,
+    class operand = sign of the accumulators, S5 at hv_bits = 1):
+
+        s[n,k] = sum_j  adc( sum_{d in chunk j, d < D_eff} v[n,d] * c[k,d] )
+
+    chunks are [j*chunk, (j+1)*chunk); the last one may hold fewer than `chunk` dimensions.
+    Returns int64 [N][K]; the label is the arg-max (ties -> lowest index, S7)."""
+    v = bipolar(np.asarray(hbits, dtype=np.uint8)[:, :D_eff]).astype(np.int64)
+    c = bipolar(class_operand(C_acc, D_eff, 1)).astype(np.int64)
+    S = np.zeros((v.shape[0], c.shape[0]), dtype=np.int64)
+    for j0 in range(0, D_eff, chunk):
+        part = v[:, j0:j0 + chunk] @ c[:, j0:j0 + chunk].T
+        S += adc_quantize(part, res, step, floor, ceil)
+    return S
 
 
 # ------------------------------------------------------------------------------------- S7

@@ -710,3 +710,77 @@ def test_unperforated_encode_arguments_change_nothing():
         a = o.encode_rp(X, P, 9, prec, want_absum=True)
         b = o.encode_rp(X, P, 9, prec, want_absum=True, f_begin=0, f_stride=1)
         assert all(np.array_equal(u, v) for u, v in zip(a, b))
+
+
+# ------------------------------------------------------------------------------------- S12 / A19 ADC-quantised chunked dot
+def test_adc_transfer_function_by_hand():
+    """Reading A19 written out on small windows.  Baseline window (L273: floor -127, ceil 128, RES 8,
+    step 1): 256 codes, transparent on [-127, 128], -128 clips to -127."""
+    p = np.arange(-128, 129)
+    q = o.adc_quantize(p, 8, 1, -127, 128)
+    assert np.array_equal(q[1:], p[1:]) and q[0] == -127
+    # the paper's best window: floor -3, ceil 128, RES 8, step 2 -> levels -3, -1, 1, 3, ...
+    q = o.adc_quantize(np.array([-128, -4, -3, -2, -1, 0, 1, 2, 127, 128]), 8, 2, -3, 128)
+    #  clip -> -3,-3,-3,-2,-1,0,1,2,127,128 ; (p+3+1)//2 -> 0,0,0,1,1,2,2,3,65,66 ; -3 + 2*code
+    assert q.tolist() == [-3, -3, -3, -1, -1, 1, 1, 3, 127, 129]
+    # RES limits the code: RES 2, step 9, floor -3 -> levels -3, 6, 15, 24 and nothing above
+    q = o.adc_quantize(np.array([-10, 1, 2, 10, 11, 19, 20, 128]), 2, 9, -3, 128)
+    assert q.tolist() == [-3, -3, 6, 6, 15, 15, 24, 24]
+    # idempotent and monotone
+    for res, step, fl, ce in [(8, 2, -3, 128), (6, 9, -3, 128), (4, 5, -20, 60), (8, 1, -127, 128)]:
+        q = o.adc_quantize(p, res, step, fl, ce)
+        assert (np.diff(q) >= 0).all()
+        assert np.array_equal(o.adc_quantize(q, res, step, fl, max(ce, int(q.max()))), q)
+
+
+@pytest.mark.parametrize("D_eff", [128, 256, 300, 127, 1, 129, 1000])
+def test_adc_similarity_with_a_transparent_window_is_the_bipolar_dot(D_eff):
+    """PAPER.md L273 baseline window is transparent unless a whole chunk is anti-aligned, so the chunked
+    sum is the plain dot = D_eff - 2 * Hamming (S0/S6 identity) -- also with a ragged last chunk."""
+    r = rng(190 + D_eff)
+    hb = r.integers(0, 2, size=(9, 1024), dtype=np.uint8)
+    C = r.standard_normal((5, 1024)).astype(np.float32)
+    C[0, :40] = 0.0
+    S = o.similarity_adc(hb, C, D_eff, 8, 1, -127, 128)
+    ham = o.similarity(hb, C, D_eff, o.SIM_HAMMING, 1)
+    assert np.array_equal(S, D_eff - 2 * ham.astype(np.int64))
+    # an anti-aligned full chunk reads -127, not -128
+    hb2 = np.zeros((1, 256), dtype=np.uint8)
+    C2 = -np.ones((1, 256), dtype=np.float32)
+    assert o.similarity_adc(hb2, C2, 256, 8, 1, -127, 128)[0, 0] == -254
+
+
+@pytest.mark.parametrize("res,step,fl,ce", [(8, 2, -3, 128), (6, 9, -3, 128), (3, 7, -40, 90), (8, 1, -127, 128)])
+def test_adc_similarity_brute_force(res, step, fl, ce):
+    r = rng(195)
+    N, K, D, D_eff, chunk = 4, 3, 400, 300, 128
+    hb = r.integers(0, 2, size=(N, D), dtype=np.uint8)
+    C = r.standard_normal((K, D)).astype(np.float32)
+    S = o.similarity_adc(hb, C, D_eff, res, step, fl, ce)
+    for n in range(N):
+        for k in range(K):
+            total = 0
+            for j0 in range(0, D_eff, chunk):
+                part = 0
+                for d in range(j0, min(j0 + chunk, D_eff)):
+                    v = -1 if hb[n, d] else 1
+                    c = -1 if C[k, d] < 0 else 1
+                    part += v * c
+                x = min(max(part, fl), ce)
+                code = min((x - fl + step // 2) // step, 2 ** res - 1)
+                total += fl + code * step
+            assert S[n, k] == total
+
+
+def test_adc_floor_clipping_keeps_the_label_of_a_separable_query():
+    """L273: "Clipping below -3 therefore preserves the classification outcome": a query equal to one
+    class hypervector keeps its label under the paper's tuned window."""
+    r = rng(196)
+    K, D = 6, 2048
+    C = np.where(r.integers(0, 2, size=(K, D)) == 1, -1.0, 1.0).astype(np.float32)
+    hb = (C < 0).astype(np.uint8)                      # query n == class n
+    flip = r.random((K, D)) < 0.2
+    hb ^= flip.astype(np.uint8)                         # 20 % noise
+    for res, step in [(8, 2), (6, 9)]:
+        lab, _, _ = o.classify(o.similarity_adc(hb, C, D, res, step, -3, 128), o.SIM_DOT)
+        assert lab.tolist() == list(range(K))
