@@ -197,6 +197,29 @@ int32_t hdc_similarity(hdc_handle_t h, const uint32_t* Hbits, int64_t N, int64_t
                        const hdc_knobs_t* knobs, void* S, int32_t s_dtype, int64_t lds, void* ws,
                        size_t ws_bytes, void* stream);
 
+/* ---- (2') chunked, ADC-quantised dot similarity (SpecPCM simulator) --------------------------
+ * "The SpecPCM simulator computes dot-product similarity over 128-element array
+ * chunks, with each partial dot product quantized by the ADC before accumulation"; hardware knobs
+ * ADC_RES, ADC_STEP, ADC_FLOOR, ADC_CEIL; MLC = 1: +-1 hypervectors (class operand = sign of C_acc).
+ *   s[n,k] = sum_j adc( sum_{d in [128 j, 128 j + 128), d < D_eff} v[n,d] * c[k,d] )
+ *   adc(p) = floor + step * min( (clamp(p, floor, ceil) - floor + step/2) / step , 2^res - 1 )
+ * (integer arithmetic, step/2 and the division rounded down: nearest code, halves up; the paper
+ * prints no formula: DESIGN.md reading A19.  floor -127, ceil 128, res 8, step 1 -- the paper's
+ * baseline window -- is transparent on [-127, 128]).  1 <= res <= 16, step >= 1, floor <= ceil,
+ * |floor|, |ceil| <= 32768; only knobs->D_eff is read.  S (int32 [N][lds], nullable) receives the
+ * scores, labels (int32 [N], nullable) the arg-max with ties to the lowest k; at least one of them.
+ * Workspace: hdc_workspace_bytes(HDC_OP_SIMILARITY, ...) suffices. */
+typedef struct {
+  int32_t res;   /* ADC_RES: number of output bits */
+  int32_t step;  /* ADC_STEP: input units per code */
+  int32_t floor; /* ADC_FLOOR: lowest input / level */
+  int32_t ceil;  /* ADC_CEIL: highest input */
+} hdc_adc_t;
+int32_t hdc_similarity_adc(hdc_handle_t h, const uint32_t* Hbits, int64_t N, int64_t ldh_words,
+                           const float* C_acc, int32_t K, int64_t ldc, int32_t D,
+                           const hdc_knobs_t* knobs, const hdc_adc_t* adc, int32_t* S, int64_t lds,
+                           int32_t* labels, void* ws, size_t ws_bytes, void* stream);
+
 /* ---- (2+3a) classify = similarity + arg-extremum, fused (no S matrix) ----------------------
  * PAPER.md Listing 1 L72-L80.  labels[n] = arg-max (DOT, COS) or arg-min (HAMMING) over k, ties
  * to the lowest k.  best / second (nullable, fp32 [N]) receive the winning and runner-up score

@@ -124,6 +124,25 @@ def row_classify(h, peaks, reps, N, K, D, hv_bits, sim_name):
     return out
 
 
+def row_adc(h, peaks, reps, N=131072, K=26, D=1024):
+    """SpecPCM-simulator similarity (PAPER.md L273 best configuration: D = 1024, ADC_RES 8, ADC_STEP 2,
+    ADC_FLOOR -3, ADC_CEIL 128; ISOLET-shaped K = 26): chunked ADC-quantised dot + arg-max."""
+    W = (D + 31) // 32
+    H = _rand_bits(N, W, 3)
+    C = _class_acc(K, D, 4)
+    kn = hd.knobs(D)
+    fn = lambda: h.hdc_similarity_adc(H, C, kn, 8, 2, -3, 128, want_scores=False)  # noqa: E731
+    call_ms = _time(fn, reps)
+    k_ms, _ = _kernel(h, hd.HDC_K_SIM, fn, reps)
+    popc = float(N) * K * W / (k_ms * 1e-3) / 1e12
+    peak = 148 * 16 * peaks["sm_max_mhz"] * 1e6 / 1e12
+    return {"what": f"hdc_similarity_adc N={N} K={K} D={D} window (8, 2, -3, 128), labels only", "call_ms": call_ms,
+            "kernel_ms": k_ms, "queries_per_s": N / (call_ms * 1e-3),
+            "hbm_GBps_query_bits": N * W * 4 / (k_ms * 1e-3) / 1e9,
+            "roofline": {"bound": "alu", "achieved": popc, "peak": peak, "unit": "Tpopc/s", "frac": popc / peak,
+                         "peak_source": "148 SM x 16 POPC lanes x sm_max_mhz"}}
+
+
 # ------------------------------------------------------------------------------------ level-ID row
 def row_levelid(h, peaks, reps, N=65536, F=784, Q=256, D=10000, dense_input=False):
     from workloads import gen
@@ -358,6 +377,8 @@ ROWS = {
     "c3_pipeline": lambda h, p, r: row_c3_pipeline(h, p, r),
     "c5_stream_bf16": lambda h, p, r: row_c5_stream(h, p, r, 16, "cos"),
     "c5_stream_1bit": lambda h, p, r: row_c5_stream(h, p, r, 1, "hamming"),
+    "specpcm_adc_d1024": lambda h, p, r: row_adc(h, p, r, 131072, 26, 1024),
+    "specpcm_adc_d10000": lambda h, p, r: row_adc(h, p, r, 131072, 26, 10000),
     "c2_train_epoch": lambda h, p, r: row_train(h, p, r),
     "c2_kmeans_epoch": lambda h, p, r: row_kmeans(h, p, r),
 }

@@ -27,7 +27,7 @@ HDC_K_ENCODE_GEMM, HDC_K_SIM, HDC_K_LEVELID, HDC_K_CLASS_UPDATE = 0, 1, 2, 3
 
 EXPORTS = ("hdc_create", "hdc_destroy", "hdc_last_error", "hdc_version", "hdc_launch_count",
            "hdc_workspace_bytes", "hdc_encode_rp", "hdc_encode_levelid", "hdc_encode_levelid_u16",
-           "hdc_similarity",
+           "hdc_similarity", "hdc_similarity_adc",
            "hdc_classify", "hdc_train_epoch", "hdc_train_delta", "hdc_train_apply", "hdc_infer_rp_host",
            "hdc_kernel_timing", "hdc_kernel_time")
 
@@ -36,6 +36,10 @@ class hdc_knobs_t(C.Structure):
     _fields_ = [("D_eff", C.c_int32), ("precision", C.c_int32), ("hv_bits", C.c_int32),
                 ("sim", C.c_int32), ("flags", C.c_int32), ("perf_begin", C.c_int32),
                 ("perf_stride", C.c_int32), ("enc_perf_begin", C.c_int32), ("enc_perf_stride", C.c_int32)]
+
+
+class hdc_adc_t(C.Structure):
+    _fields_ = [("res", C.c_int32), ("step", C.c_int32), ("floor", C.c_int32), ("ceil", C.c_int32)]
 
 
 class HdcError(RuntimeError):
@@ -80,6 +84,9 @@ def lib() -> C.CDLL:
     L.hdc_encode_levelid_u16.restype = i32
     L.hdc_similarity.argtypes = [vp, vp, i64, i64, vp, i32, i64, i32, kp, vp, i32, i64, vp, sz, vp]
     L.hdc_similarity.restype = i32
+    L.hdc_similarity_adc.argtypes = [vp, vp, i64, i64, vp, i32, i64, i32, kp, C.POINTER(hdc_adc_t), vp, i64, vp, vp,
+                                     sz, vp]
+    L.hdc_similarity_adc.restype = i32
     L.hdc_classify.argtypes = [vp, vp, i64, i64, vp, i32, i64, i32, kp, vp, vp, vp, vp, sz, vp]
     L.hdc_classify.restype = i32
     L.hdc_train_epoch.argtypes = [vp, i32, vp, i64, i64, vp, vp, i32, i64, i32, kp, C.c_float, i64, vp, vp,
@@ -229,6 +236,22 @@ class Handle:
                                     S.stride(0) if N > 1 else K, ws, wsb, self._stream())
         self._check(rc)
         return S
+
+    def hdc_similarity_adc(self, Hbits, C_acc, kn: hdc_knobs_t, res: int, step: int, floor: int, ceil: int,
+                           want_scores: bool = True, want_labels: bool = True):
+        """Chunked ADC-quantised dot (SpecPCM simulator, include/hdc.h (2')): returns (S int32 [N][K] or None,
+        labels int32 [N] or None)."""
+        N = Hbits.shape[0]
+        K, D = C_acc.shape
+        S = torch.empty((N, K), dtype=torch.int32, device=self.device) if want_scores else None
+        labels = torch.empty(N, dtype=torch.int32, device=self.device) if want_labels else None
+        adc = hdc_adc_t(int(res), int(step), int(floor), int(ceil))
+        ws, wsb = self._workspace(self.workspace_bytes(HDC_OP_SIMILARITY, N, 0, D, K, kn))
+        rc = self._L.hdc_similarity_adc(self._h, _ptr(Hbits), N, _rowmajor(Hbits, "Hbits"), _ptr(C_acc), K,
+                                        _rowmajor(C_acc, "C_acc"), D, C.byref(kn), C.byref(adc), _ptr(S), K,
+                                        _ptr(labels), ws, wsb, self._stream())
+        self._check(rc)
+        return S, labels
 
     # -------------------------------------------------------------------------------- (2+3a)
     def hdc_classify(self, Hbits, C_acc, kn: hdc_knobs_t, want_scores: bool = False, labels=None):

@@ -436,6 +436,7 @@ size_t similarity_ws(int64_t N, int K, const hdc_knobs_t* k) {
   b.take<float>(1);
   b.take<uint32_t>((size_t)K * W);
   b.take<uint32_t>((size_t)W);  // perforation mask
+  b.take<uint32_t>((size_t)((k->D_eff + 127) / 128) * 4 * K);  // [chunk][class] sign bits of hdc_similarity_adc
   b.take<uint8_t>(sim_tc_operand_bytes(K, k->hv_bits == 32 || k->hv_bits == 16 || k->hv_bits == 8 ? k->hv_bits : 1,
                                        k->D_eff));
   return b.off + 1024;
@@ -696,6 +697,56 @@ extern "C" int32_t hdc_similarity(hdc_handle_t h, const uint32_t* Hbits, int64_t
   if (!ws) ws_bytes = 0;
   return do_similarity(h, Hbits, N, ldh_words, C_acc, K, ldc, knobs, S, s_dtype == HDC_I32, lds, nullptr,
                        nullptr, nullptr, b, ws_bytes, (cudaStream_t)stream);
+}
+
+extern "C" int32_t hdc_similarity_adc(hdc_handle_t h, const uint32_t* Hbits, int64_t N, int64_t ldh_words,
+                                      const float* C_acc, int32_t K, int64_t ldc, int32_t D,
+                                      const hdc_knobs_t* knobs, const hdc_adc_t* adc, int32_t* S, int64_t lds,
+                                      int32_t* labels, void* ws, size_t ws_bytes, void* stream) {
+  if (!h) return HDC_ERR_INVALID_ARG;
+  if ((!Hbits && N > 0) || !C_acc || !adc) return fail(h, HDC_ERR_INVALID_ARG, "similarity_adc: NULL operand");
+  if (N < 0 || K < 1 || K > 65535 || D < 1 || ldc < D) return fail(h, HDC_ERR_INVALID_ARG, "similarity_adc: bad sizes");
+  int rc = check_knobs(h, knobs, D);
+  if (rc) return rc;
+  if (ldh_words < words_of(knobs->D_eff)) return fail(h, HDC_ERR_INVALID_ARG, "similarity_adc: ldh_words < W");
+  if (adc->res < 1 || adc->res > 16 || adc->step < 1 || adc->floor > adc->ceil || adc->floor < -32768 ||
+      adc->ceil > 32768)
+    return fail(h, HDC_ERR_INVALID_ARG, "similarity_adc: bad ADC window");
+  if (!S && !labels && N > 0) return fail(h, HDC_ERR_INVALID_ARG, "similarity_adc: S or labels required");
+  if (S && lds < K) return fail(h, HDC_ERR_INVALID_ARG, "similarity_adc: lds < K");
+  if ((reinterpret_cast<uintptr_t>(Hbits) | reinterpret_cast<uintptr_t>(C_acc) | reinterpret_cast<uintptr_t>(S) |
+       reinterpret_cast<uintptr_t>(labels)) & 3)
+    return fail(h, HDC_ERR_ALIGNMENT, "similarity_adc: operands must be 4-byte aligned");
+  if (N == 0) return HDC_OK;
+  const int D_eff = knobs->D_eff;
+  Bump b(ws);
+  if (!ws) ws_bytes = 0;
+  uint32_t* cls = b.take<uint32_t>(adc_class_bytes(K, D_eff) / sizeof(uint32_t));
+  if (b.off > ws_bytes) return fail(h, HDC_ERR_WORKSPACE, "similarity_adc: workspace too small");
+  // the transfer function, tabulated by the number of differing bits of a chunk of n dimensions
+  AdcTables tab;
+  const int n_tail = D_eff - 128 * ((D_eff + 127) / 128 - 1);
+  const long long top = (1ll << adc->res) - 1;
+  auto level = [&](int n, int diff) -> int {
+    long long p = (long long)n - 2ll * diff;
+    if (p < adc->floor) p = adc->floor;
+    if (p > adc->ceil) p = adc->ceil;
+    long long code = (p - adc->floor + adc->step / 2) / adc->step;
+    if (code > top) code = top;
+    return (int)(adc->floor + code * adc->step);
+  };
+  for (int i = 0; i <= 128; ++i) {
+    tab.full[i] = level(128, i);
+    tab.tail[i] = i <= n_tail ? level(n_tail, i) : 0;
+  }
+  cudaError_t ce;
+  {
+    Timed tm(h, HDC_K_SIM, (cudaStream_t)stream);
+    ce = launch_adc_similarity(Hbits, N, ldh_words, C_acc, K, ldc, D_eff, tab, cls, S, lds, labels, h->sm_count,
+                               h->smem_optin, (cudaStream_t)stream, &h->launches);
+  }
+  if (ce == cudaErrorNotSupported) return fail(h, HDC_ERR_UNSUPPORTED, "similarity_adc: D_eff too large for one CTA");
+  return ce == cudaSuccess ? HDC_OK : cuda_fail(h, ce, "similarity_adc");
 }
 
 extern "C" int32_t hdc_classify(hdc_handle_t h, const uint32_t* Hbits, int64_t N, int64_t ldh_words,

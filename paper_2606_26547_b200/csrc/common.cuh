@@ -104,6 +104,18 @@ size_t sim_tc_partial_bytes(int64_t N, int K, int hv_bits, int D_eff, int sm_cou
 cudaError_t launch_tensor_amax(const float* C, int K, int D_eff, int64_t ldc, Perf pf, float* amax,
                                cudaStream_t st, int64_t* nlaunch);
 // mask[w] = bits of word w whose dimension is visited and < D_eff (W words)
+// ADC-quantised chunked dot (adc.cu): transfer function tabulated by the number of
+// differing bits in a chunk -- full[i] for 128-dimension chunks, tail[i] for the ragged last chunk.
+struct AdcTables {
+  int full[129];
+  int tail[129];
+};
+size_t adc_class_bytes(int K, int D_eff);
+cudaError_t launch_adc_similarity(const uint32_t* H, int64_t N, int64_t ldh, const float* C_acc, int K,
+                                  int64_t ldc, int D_eff, const AdcTables& tab, uint32_t* class_ws, int32_t* S,
+                                  int64_t lds, int32_t* labels, int sm_count, int smem_optin, cudaStream_t st,
+                                  int64_t* nlaunch);
+
 // Perforated encode contraction: compacted copy of the visited columns (esize = element bytes 1/2/4)
 // and the compensation scale applied to the optional raw accumulators.
 cudaError_t launch_gather_cols(const void* src, int esize, int64_t rows, int64_t ld_src, Perf pf, int n_vis,

@@ -746,3 +746,55 @@ def test_infer_rp_host_with_perforated_encode_equals_device_calls(hd, h):
     bits_or, _, _ = O.encode_rp(X[sub], P, 1000, O.BF16, f_begin=2, f_stride=3)
     lab_or, _, _ = O.classify(O.similarity(bits_or, C, 1000, O.SIM_HAMMING, 1, 1, 2), O.SIM_HAMMING)
     assert np.array_equal(lab_dev[sub], lab_or)
+
+
+# ------------------------------------------------------------------------------------ S12 / A19 ADC-quantised chunked dot
+@pytest.mark.parametrize("res,step,fl,ce", [(8, 1, -127, 128), (8, 2, -3, 128), (6, 9, -3, 128), (3, 7, -40, 90),
+                                            (16, 1, -128, 128), (1, 50, 0, 128)])
+@pytest.mark.parametrize("N,K,D,D_eff", [(300, 26, 10000, 10000), (77, 6, 1100, 1024), (50, 70, 2100, 2047),
+                                         (33, 1, 256, 129), (9, 40, 128, 1), (130, 33, 4500, 4099),
+                                         (64, 100, 16384, 16384)])
+def test_adc_similarity_bit_exact(hd, h, res, step, fl, ce, N, K, D, D_eff):
+    """hdc_similarity_adc (reading A19): integer scores and labels equal the oracle."""
+    r = rng(22, N, K, D_eff, res, step)
+    hb = r.integers(0, 2, size=(N, D), dtype=np.uint8)
+    C = r.standard_normal((K, D)).astype(np.float32)
+    C[r.random((K, D)) < 0.05] = 0.0
+    if K > 2:
+        C[2] = C[1]                                            # exact tie between classes 1 and 2
+        hb[0] = (C[1] < 0)                                      # query 0 == class 1 == class 2
+    S_or = O.similarity_adc(hb, C, D_eff, res, step, fl, ce)
+    lab_or, _, _ = O.classify(S_or, O.SIM_DOT)
+    S, lab = h.hdc_similarity_adc(dev_bits(hb), dev(C), hd.knobs(D_eff), res, step, fl, ce)
+    assert np.array_equal(S.cpu().numpy().astype(np.int64), S_or)
+    assert np.array_equal(lab.cpu().numpy(), lab_or)
+    _, lab2 = h.hdc_similarity_adc(dev_bits(hb), dev(C), hd.knobs(D_eff), res, step, fl, ce, want_scores=False)
+    assert np.array_equal(lab2.cpu().numpy(), lab_or)
+
+
+def test_adc_similarity_transparent_window_equals_hamming_path(hd, h):
+    """The paper's baseline window is transparent: scores = D_eff - 2 * hdc_similarity(HAMMING)."""
+    r = rng(23)
+    N, K, D, D_eff = 500, 26, 10000, 8400
+    hb = r.integers(0, 2, size=(N, D), dtype=np.uint8)
+    C = r.standard_normal((K, D)).astype(np.float32)
+    Hd, Cd = dev_bits(hb), dev(C)
+    S, _ = h.hdc_similarity_adc(Hd, Cd, hd.knobs(D_eff), 8, 1, -127, 128)
+    ham = h.hdc_similarity(Hd, Cd, hd.knobs(D_eff, hv_bits=1, sim=hd.HDC_SIM_HAMMING))
+    assert torch.equal(S, D_eff - 2 * ham)
+
+
+def test_adc_similarity_argument_errors(hd, h):
+    H = torch.zeros((8, 4), dtype=torch.int32, device="cuda")
+    Cc = torch.ones((3, 128), dtype=torch.float32, device="cuda")
+    before = h.launch_count()
+    for bad in [(0, 1, -3, 128), (17, 1, -3, 128), (8, 0, -3, 128), (8, 1, 5, 4), (8, 1, -40000, 128)]:
+        with pytest.raises(hd.HdcError) as ei:
+            h.hdc_similarity_adc(H, Cc, hd.knobs(128), *bad)
+        assert ei.value.code == hd.HDC_ERR_INVALID_ARG
+    with pytest.raises(hd.HdcError):
+        h.hdc_similarity_adc(H, Cc, hd.knobs(128), 8, 1, -127, 128, want_scores=False, want_labels=False)
+    assert h.launch_count() == before
+    S, lab = h.hdc_similarity_adc(H[:0], Cc, hd.knobs(128), 8, 1, -127, 128)
+    assert S.shape == (0, 3) and lab.shape == (0,)
+    assert h.launch_count() == before
