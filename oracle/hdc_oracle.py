@@ -30,6 +30,7 @@ import numpy as np
 # precision / hv_bits / sim codes mirror include/hdc.h numerically but are typed here by hand
 F32, BF16, I8, B1 = 0, 1, 2, 3
 SIM_DOT, SIM_COS, SIM_HAMMING = 0, 1, 2
+HV_F16 = 17      # hv_bits code (not a width): class operand as 16-bit IEEE half ("FP16")
 
 
 # ------------------------------------------------------------------------------------- S0
@@ -156,13 +157,17 @@ def class_operand(C_acc: np.ndarray, D_eff: int, hv_bits: int) -> np.ndarray:
     """Class operand derived from the fp32 accumulators at the hypervector element width
     (training in high precision, inference "projecting class ... hypervectors
     onto lower-precision integer types"; S5): 32 -> C_acc; 16 -> bf16 RNE; 8 -> per-tensor
-    symmetric int8 over k<K, d<D_eff; 1 -> bit [C_acc < 0].  Returned as float64 values
+    symmetric int8 over k<K, d<D_eff; 1 -> bit [C_acc < 0]; HV_F16 -> IEEE half RNE.  Returned as float64 values
     (bits as uint8)."""
     c = np.asarray(C_acc, dtype=np.float32)[:, :D_eff]
     if hv_bits == 32:
         return c.astype(np.float64)
     if hv_bits == 16:
         return round_bf16(c).astype(np.float64)
+    if hv_bits == HV_F16:
+        # IEEE binary16, round-to-nearest-even (L165 "floating-point types (FP16 or FP32)");
+        # |c| > 65504 overflows to +-inf: outside the contract (S0: finite operands)
+        return c.astype(np.float16).astype(np.float64)
     if hv_bits == 8:
         return quantize_int8_tensor(c).astype(np.float64)
     if hv_bits == 1:

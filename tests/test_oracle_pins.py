@@ -784,3 +784,45 @@ def test_adc_floor_clipping_keeps_the_label_of_a_separable_query():
     for res, step in [(8, 2), (6, 9)]:
         lab, _, _ = o.classify(o.similarity_adc(hb, C, D, res, step, -3, 128), o.SIM_DOT)
         assert lab.tolist() == list(range(K))
+
+
+# ------------------------------------------------------------------------------------- S5 fp16 class operand
+def _half_rne_by_hand(x: float) -> float:
+    """binary16 round-to-nearest-even from the definition (normal and subnormal range, no overflow)."""
+    if x == 0.0:
+        return 0.0
+    s = -1.0 if x < 0 else 1.0
+    a = abs(x)
+    e = max(math.floor(math.log2(a)), -14)           # exponent of the binade; subnormals share 2^-14
+    ulp = 2.0 ** (e - 10)
+    q = a / ulp                                       # exact: power-of-two scaling
+    f = math.floor(q)
+    r = q - f
+    if r > 0.5 or (r == 0.5 and f % 2 == 1):
+        f += 1
+    return s * f * ulp
+
+
+def test_fp16_class_operand_rounding_by_hand():
+    """hv code HV_F16 (PAPER.md L165 FP16): IEEE half RNE, checked against the definition on ties
+    (2049 -> 2048, 2051 -> 2052), the largest finite value, subnormals and random values."""
+    r = rng(200)
+    vals = np.concatenate([np.array([0.0, 1.0, -1.0, 2049.0, 2051.0, -2049.0, 65504.0, 65519.0, 1.0 + 2.0 ** -11,
+                                     1.0 + 3 * 2.0 ** -11, 6e-8, 3e-8, 2.0 ** -25, 1e-5, 0.1, 32.0, -33.3],
+                                    dtype=np.float32),
+                           (r.standard_normal(500) * r.choice([1e-3, 1.0, 40.0, 3000.0], size=500)).astype(np.float32)])
+    got = o.class_operand(vals[None, :], len(vals), o.HV_F16)[0]
+    want = np.array([_half_rne_by_hand(float(v)) for v in vals])
+    assert np.array_equal(got, want)
+    assert got[3] == 2048.0 and got[4] == 2052.0 and got[6] == 65504.0 and got[7] == 65504.0
+    # exact integers up to 2048 are representable: a bundle of <= 2048 hypervectors is held exactly
+    ints = np.arange(-2048, 2049, dtype=np.float32)
+    assert np.array_equal(o.class_operand(ints[None, :], len(ints), o.HV_F16)[0], ints.astype(np.float64))
+
+
+def test_fp16_similarity_equals_fp32_on_small_integer_accumulators():
+    r = rng(201)
+    hb = r.integers(0, 2, size=(7, 300), dtype=np.uint8)
+    C = r.integers(-2048, 2049, size=(4, 300)).astype(np.float32)
+    for sim in (o.SIM_DOT, o.SIM_COS):
+        assert np.array_equal(o.similarity(hb, C, 300, sim, o.HV_F16), o.similarity(hb, C, 300, sim, 32))
