@@ -60,6 +60,8 @@ typedef enum {
 enum { HDC_F32 = 0, HDC_BF16 = 1, HDC_I8 = 2, HDC_B1 = 3, HDC_U8 = 4, HDC_I32 = 5 };
 /* similarity kinds (L167 algorithmic choice) */
 enum { HDC_SIM_DOT = 0, HDC_SIM_COS = 1, HDC_SIM_HAMMING = 2 };
+/* knobs.hv_bits code (not a width) for a 16-bit IEEE half class operand (L165 "FP16") */
+enum { HDC_HV_F16 = 17 };
 /* hdc_train_epoch modes */
 enum { HDC_TRAIN_BUNDLE = 0, HDC_TRAIN_PERCEPTRON = 1, HDC_TRAIN_KMEANS = 2 };
 /* hdc_encode_rp outputs (bit-or) */
@@ -85,7 +87,8 @@ enum {
  *             int32 accumulate.  HDC_B1: packed hypervectors with the real-valued contraction in
  *             bf16 (same contraction as HDC_BF16).
  *  hv_bits    element width of the CLASS hypervectors in similarity / classify / train (L165):
- *             32 fp32 | 16 bf16 (RNE of C_acc) | 8 int8 (per-tensor symmetric over k<K, d<D_eff)
+ *             32 fp32 | 16 bf16 (RNE of C_acc) | HDC_HV_F16 IEEE half (RNE of C_acc; |c| > 65504
+ *             overflows, outside the contract) | 8 int8 (per-tensor symmetric over k<K, d<D_eff)
  *             | 1 sign bit [C_acc < 0].  Query hypervectors are always bipolar (packed bits).
  *  sim        HDC_SIM_*; HDC_SIM_HAMMING requires hv_bits == 1.
  *  flags      HDC_FLAG_*.

@@ -79,8 +79,8 @@ int check_knobs(hdc_ctx* h, const hdc_knobs_t* k, int D) {
   return HDC_OK;
 }
 int check_sim_knobs(hdc_ctx* h, const hdc_knobs_t* k) {
-  if (k->hv_bits != 32 && k->hv_bits != 16 && k->hv_bits != 8 && k->hv_bits != 1)
-    return fail(h, HDC_ERR_INVALID_ARG, "hv_bits must be 32, 16, 8 or 1");
+  if (k->hv_bits != 32 && k->hv_bits != 16 && k->hv_bits != HDC_HV_F16 && k->hv_bits != 8 && k->hv_bits != 1)
+    return fail(h, HDC_ERR_INVALID_ARG, "hv_bits must be 32, 16, HDC_HV_F16, 8 or 1");
   if (k->sim != HDC_SIM_DOT && k->sim != HDC_SIM_COS && k->sim != HDC_SIM_HAMMING)
     return fail(h, HDC_ERR_INVALID_ARG, "bad sim");
   if (k->sim == HDC_SIM_HAMMING && k->hv_bits != 1)
@@ -328,7 +328,10 @@ int do_similarity(hdc_ctx* h, const uint32_t* Hbits, int64_t N, int64_t ldh, con
         if (ce != cudaSuccess) return cuda_fail(h, ce, "quantize C");
         ce = launch_col_scale(Operand{Cq, ldq, OPK_I8}, K, D_eff, 1, pf, colscale, st, &h->launches);
       } else {
-        const int ck = k->hv_bits == 32 ? OPK_F32 : (k->hv_bits == 16 ? OPK_F32_RBF16 : OPK_BITS);
+        const int ck = k->hv_bits == 32   ? OPK_F32
+                       : k->hv_bits == 16 ? OPK_F32_RBF16
+                       : k->hv_bits == HDC_HV_F16 ? OPK_F32_RF16
+                                                  : OPK_BITS;
         ce = launch_col_scale(Operand{C_acc, ldc, ck}, K, D_eff, 1, pf, colscale, st, &h->launches);
       }
       if (ce != cudaSuccess) return cuda_fail(h, ce, "col_scale");
@@ -384,6 +387,8 @@ int do_similarity(hdc_ctx* h, const uint32_t* Hbits, int64_t N, int64_t ldh, con
     B = Operand{C_acc, ldc, OPK_F32};
   } else if (k->hv_bits == 16) {
     B = Operand{C_acc, ldc, OPK_F32_RBF16};
+  } else if (k->hv_bits == HDC_HV_F16) {
+    B = Operand{C_acc, ldc, OPK_F32_RF16};
   } else if (k->hv_bits == 8) {
     const int64_t ldq = round_up(D_eff, 16);
     int8_t* Cq = b.take<int8_t>((size_t)K * ldq);
@@ -437,7 +442,8 @@ size_t similarity_ws(int64_t N, int K, const hdc_knobs_t* k) {
   b.take<uint32_t>((size_t)K * W);
   b.take<uint32_t>((size_t)W);  // perforation mask
   b.take<uint32_t>((size_t)((k->D_eff + 127) / 128) * 4 * K);  // [chunk][class] sign bits of hdc_similarity_adc
-  b.take<uint8_t>(sim_tc_operand_bytes(K, k->hv_bits == 32 || k->hv_bits == 16 || k->hv_bits == 8 ? k->hv_bits : 1,
+  b.take<uint8_t>(sim_tc_operand_bytes(K, k->hv_bits == 32 || k->hv_bits == 16 || k->hv_bits == HDC_HV_F16 ||
+                                               k->hv_bits == 8 ? k->hv_bits : 1,
                                        k->D_eff));
   return b.off + 1024;
 }

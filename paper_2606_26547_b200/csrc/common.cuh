@@ -2,6 +2,7 @@
 // Nothing here is part of the public ABI (include/hdc.h is).  No code is shared with oracle/.
 #pragma once
 #include <cuda_bf16.h>
+#include <cuda_fp16.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -15,7 +16,8 @@ enum OperandKind : int {
   OPK_BF16 = 1,       // __nv_bfloat16, widened exactly
   OPK_F32_RBF16 = 2,  // float rounded to nearest-even bf16 on load (precision BF16 / hv_bits 16)
   OPK_BITS = 3,       // packed hypervector bits: element k -> bit k&31 of word k>>5, value 1-2*bit
-  OPK_I8 = 4          // int8
+  OPK_I8 = 4,         // int8
+  OPK_F32_RF16 = 5    // float rounded to nearest-even IEEE half on load (hv code HDC_HV_F16)
 };
 
 struct Operand {

@@ -183,6 +183,7 @@ __global__ void col_scale_kernel(Operand C, int K, int D_eff, int cos, Perf pf, 
         case OPK_F32_RBF16:
           v = (double)__bfloat162float(__float2bfloat16_rn(__ldg((const float*)C.p + idx)));
           break;
+        case OPK_F32_RF16: v = (double)__half2float(__float2half_rn(__ldg((const float*)C.p + idx))); break;
         case OPK_BITS: v = 1.0; break;
         default: v = (double)((const int8_t*)C.p)[idx]; break;
       }

@@ -40,6 +40,8 @@ __device__ __forceinline__ T load_elem(const Operand& o, int64_t row, int k) {
       return (T)__bfloat162float(((const __nv_bfloat16*)o.p)[row * o.ld + k]);
     case OPK_F32_RBF16:
       return (T)__bfloat162float(__float2bfloat16_rn(__ldg((const float*)o.p + row * o.ld + k)));
+    case OPK_F32_RF16:
+      return (T)__half2float(__float2half_rn(__ldg((const float*)o.p + row * o.ld + k)));
     case OPK_BITS: {
       uint32_t w = __ldg((const uint32_t*)o.p + row * o.ld + (k >> 5));
       return (T)(1 - 2 * (int)((w >> (k & 31)) & 1u));

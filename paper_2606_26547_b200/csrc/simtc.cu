@@ -22,6 +22,7 @@
 // c1+c2+c3 stacked along the class axis of one tile -- the three partial accumulators are summed in
 // the epilogue, so the queries are expanded once; int8 (hv_bits 8) and +-1 int8 (hv_bits 1) with
 // int32 accumulation (exact).
+#include <cuda_fp16.h>
 #include <limits.h>
 
 #include <type_traits>
@@ -75,6 +76,7 @@ struct SimParams {
   int kps;          // k-blocks per pipeline group
   int stages;       // ring depth
   int stage_bytes;  // A_BYTES + nparts*kc*KB_BYTES
+  int f16;          // 16-bit operands are IEEE half instead of bf16 (hv code HDC_HV_F16)
   Epilogue e;
 };
 
@@ -169,7 +171,8 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
     uint32_t phase = 0;
     int acc = 0;
     uint32_t acc_phase = 0;
-    const uint32_t idesc = instr_desc<INT8>(BM, nb_rows);
+    // kind::f16 operand formats (bits 7..9 A, 10..12 B): 1 = bf16, 0 = IEEE half
+    const uint32_t idesc = instr_desc<INT8>(BM, nb_rows) & ((!INT8 && p.f16) ? ~((1u << 7) | (1u << 10)) : ~0u);
     for (int64_t i = 0; i < tiles_per_cta; ++i) {
       mbar_wait(tempty_bar(acc), acc_phase ^ 1u);
       tc_fence_after();
@@ -343,6 +346,7 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
     int slot = 0;
     int64_t step = 0;
     // one k-block of this thread's row half: WPP packed words -> C_PER 16-byte chunks of the A tile
+    const uint32_t one2 = p.f16 ? 0x3C003C00u : 0x3F803F80u;  // two +1.0 in half / bf16; the sign bit makes -1.0
     auto expand = [&](auto part, const uint32_t* qk, uint32_t a_row) {
       constexpr int PART = decltype(part)::value;
       constexpr int C0 = PART * C_PER;
@@ -361,7 +365,7 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
             o[e] = prmt_sign_bytes(w << (7 - (iw & 7))) | 0x01010101u;
           } else {
             const uint32_t w = wq[(iw >> 4) - PART * WPP];
-            o[e] = ((w << (15 - (iw & 15))) & 0x80008000u) | 0x3F803F80u;
+            o[e] = ((w << (15 - (iw & 15))) & 0x80008000u) | one2;
           }
         }
         const uint32_t dst = a_row + ((((uint32_t)cidx) ^ sw) << 4);
@@ -422,8 +426,8 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
 // Stages the class operand of sim_tc_kernel from the fp32 accumulators: staged row r holds class
 // k = tile*kc + (r % (nparts*kc)) % kc, part (r % (nparts*kc)) / kc of tile r / (nparts*kc); staged
 // column kb*BK + kappa holds dimension kb*BK + perm(kappa), zero for d >= D_eff or k >= K.
-// mode: 32 -> bf16 part j of the 3-way split; 16 -> bf16 RNE; 8 -> int8 with scale 127/amax;
-// 1 -> +-1 int8 from the sign.
+// mode: 32 -> bf16 part j of the 3-way split; 16 -> bf16 RNE; HDC_HV_F16 -> IEEE half RNE; 8 -> int8
+// with scale 127/amax; 1 -> +-1 int8 from the sign.
 __device__ __forceinline__ int quant_i8_c(float x, float s) {
   float q = rintf(__fmul_rn(x, s));
   q = fminf(fmaxf(q, -127.0f), 127.0f);
@@ -458,6 +462,8 @@ __global__ void class_operand_kernel(const float* __restrict__ C, int K, int D_e
       int qv = 0;
       if (live) qv = (mode == 8) ? quant_i8_c(x, s) : (x < 0.0f ? -1 : 1);
       reinterpret_cast<int8_t*>(dst)[i] = (int8_t)qv;
+    } else if (mode == HDC_HV_F16) {
+      reinterpret_cast<__half*>(dst)[i] = __float2half_rn(x);
     } else {
       __nv_bfloat16 b1 = __float2bfloat16_rn(x);
       if (mode == 32 && part > 0) {
@@ -623,6 +629,7 @@ cudaError_t launch_sim_tc(TcContext* tc, const uint32_t* Hbits, int64_t N, int64
   p.m_tiles = (int)((N + BM - 1) / BM);
   p.n_tiles = n_tiles;
   p.num_kb = num_kb;
+  p.f16 = hv_bits == HDC_HV_F16;
   p.stage_bytes = A_BYTES + nparts * kc * KB_BYTES;
   p.stages = (SMEM_LIMIT - SMEM_EXTRA - QRING_BYTES) / p.stage_bytes;
   if (p.stages > MAX_STAGES) p.stages = MAX_STAGES;

@@ -182,7 +182,7 @@ def test_encode_rp_bf16_inputs_in_place(hd, h):
 
 # ------------------------------------------------------------------------------------ dot / cos
 @pytest.mark.parametrize("sim", ["DOT", "COS"])
-@pytest.mark.parametrize("hv_bits", [32, 16, 8, 1])
+@pytest.mark.parametrize("hv_bits", [32, 16, 17, 8, 1])   # 17 = HDC_HV_F16: IEEE half class operand
 @pytest.mark.parametrize("N,K,D,D_eff", [(150, 26, 2100, 2100), (64, 6, 10000, 4099), (33, 1, 500, 500),
                                          (140, 70, 1300, 1000), (140, 600, 1300, 1000), (300, 200, 700, 640),
                                          (130, 1000, 520, 520)])
@@ -540,6 +540,8 @@ def test_similarity_classify_fuzz(hd, h, case):
     D_eff = int(r.integers(1, D + 1)) if r.random() < 0.5 else D
     sim, hv_bits = [("HAMMING", 1), ("DOT", 1), ("DOT", 8), ("COS", 8), ("COS", 32), ("COS", 16), ("DOT", 32),
                     ("DOT", 16)][int(r.integers(0, 8))]
+    if hv_bits == 16 and case % 2:
+        hv_bits = 17                                           # HDC_HV_F16
     begin, stride = 0, 1
     if r.random() < 0.35:
         stride = int(r.choice([2, 3, 8, 32]))
@@ -798,3 +800,46 @@ def test_adc_similarity_argument_errors(hd, h):
     S, lab = h.hdc_similarity_adc(H[:0], Cc, hd.knobs(128), 8, 1, -127, 128)
     assert S.shape == (0, 3) and lab.shape == (0,)
     assert h.launch_count() == before
+
+
+# ------------------------------------------------------------------------------------ fp16 class operand (L165)
+@pytest.mark.parametrize("flags", [0, 1])
+def test_fp16_class_operand_exact_on_small_integer_accumulators(hd, h, flags):
+    """Accumulators that are integers of magnitude <= 2048 are exact in IEEE half (not in bf16), so the
+    HDC_HV_F16 contraction (tcgen05 kind::f16 with half operands, or the CUDA-core kernel) must give
+    the exact integer dot products -- and differ from the bf16 operand's."""
+    r = rng(24, flags)
+    N, K, D, D_eff = 300, 26, 2100, 2047
+    hb = r.integers(0, 2, size=(N, D), dtype=np.uint8)
+    C = r.integers(-2048, 2049, size=(K, D)).astype(np.float32)
+    S_or = O.similarity(hb, C, D_eff, O.SIM_DOT, O.HV_F16)
+    assert np.array_equal(S_or, O.similarity(hb, C, D_eff, O.SIM_DOT, 32))
+    kn = hd.knobs(D_eff, hv_bits=hd.HDC_HV_F16, sim=hd.HDC_SIM_DOT, flags=flags)
+    S = h.hdc_similarity(dev_bits(hb), dev(C), kn).cpu().numpy()
+    assert np.array_equal(S.astype(np.float64), S_or)          # |s| < 2^24: exact in the fp32 accumulator
+    lab = h.hdc_classify(dev_bits(hb), dev(C), kn).cpu().numpy()
+    assert np.array_equal(lab, O.classify(S_or, O.SIM_DOT)[0])
+    S16 = h.hdc_similarity(dev_bits(hb), dev(C), hd.knobs(D_eff, hv_bits=16, sim=hd.HDC_SIM_DOT, flags=flags))
+    assert not np.array_equal(S16.cpu().numpy(), S)
+
+
+def test_fp16_perceptron_epoch_teacher_forced(hd, h):
+    w = gen.c2_isolet_shaped(D=2000, n_tr=1200, n_te=8)
+    hb, _, _ = O.encode_rp(w["Xtr"], w["P"], 2000, O.F32)
+    y, K, D_eff = w["ytr"], w["K"], 2000
+    C_or = O.bundle(hb, y, K, D_eff)
+    kn = hd.knobs(D_eff, hv_bits=hd.HDC_HV_F16, sim=hd.HDC_SIM_COS)
+    Hd, yd = dev_bits(hb), dev(y)
+    for _ in range(2):
+        S_or = O.similarity(hb, C_or, D_eff, O.SIM_COS, O.HV_F16)
+        C_next, wrong_or, pred_or = O.train_epoch(hb, y, C_or, D_eff, O.HV_F16, O.SIM_COS, 0.05, 0)
+        Cd = dev(C_or.copy())
+        pred = torch.empty(len(y), dtype=torch.int32, device="cuda")
+        h.hdc_train_epoch(hd.HDC_TRAIN_PERCEPTRON, Hd, yd, Cd, kn, lr=0.05, batch=0, pred=pred)
+        pred = pred.cpu().numpy()
+        check_labels_float(pred, S_or, O.SIM_COS)
+        near = np.nonzero(pred != pred_or)[0]
+        touched = set(y[near]) | set(pred[near]) | set(pred_or[near])
+        rows = [k for k in range(K) if k not in touched]
+        assert np.array_equal(Cd.cpu().numpy()[rows], C_next[rows])
+        C_or = C_next
