@@ -29,6 +29,7 @@ import numpy as np
 
 # precision / hv_bits / sim codes mirror include/hdc.h numerically but are typed here by hand
 F32, BF16, I8, B1 = 0, 1, 2, 3
+F16 = 6         # encode operands as IEEE half ("floating-point types (FP16 or FP32)")
 SIM_DOT, SIM_COS, SIM_HAMMING = 0, 1, 2
 HV_F16 = 17      # hv_bits code (not a width): class operand as 16-bit IEEE half ("FP16")
 
@@ -88,12 +89,16 @@ def quantize_int8_tensor(c: np.ndarray) -> np.ndarray:
 
 def rp_operands(X: np.ndarray, P: np.ndarray, precision: int):
     """Operands of the random-projection contraction at `precision` (S1): FP32 identity;
-    BF16 RNE of both; INT8 per-row of X and per-row (per projection d) of P.  B1 means packed
+    BF16 RNE of both; F16 IEEE-half RNE of both; INT8 per-row of X and per-row (per projection d) of P.  B1 means packed
     hypervectors with the real-valued contraction done in bf16 (reading A6)."""
     if precision == F32:
         return X.astype(np.float64), P.astype(np.float64)
     if precision in (BF16, B1):
         return round_bf16(X).astype(np.float64), round_bf16(P).astype(np.float64)
+    if precision == F16:
+        # IEEE binary16 RNE of both operands, products and sums exact / float64 (fp32 accumulate on the GPU)
+        return (np.asarray(X, dtype=np.float32).astype(np.float16).astype(np.float64),
+                np.asarray(P, dtype=np.float32).astype(np.float16).astype(np.float64))
     if precision == I8:
         return quantize_int8_rows(X).astype(np.float64), quantize_int8_rows(P).astype(np.float64)
     raise ValueError("precision")

@@ -826,3 +826,24 @@ def test_fp16_similarity_equals_fp32_on_small_integer_accumulators():
     C = r.integers(-2048, 2049, size=(4, 300)).astype(np.float32)
     for sim in (o.SIM_DOT, o.SIM_COS):
         assert np.array_equal(o.similarity(hb, C, 300, sim, o.HV_F16), o.similarity(hb, C, 300, sim, 32))
+
+
+def test_fp16_encode_operands_by_hand():
+    """precision F16: both operands rounded to binary16 (definition written out in
+    _half_rne_by_hand), then the plain contraction."""
+    r = rng(202)
+    X = (r.standard_normal((5, 9)) * 3).astype(np.float32)
+    P = r.standard_normal((7, 9)).astype(np.float32)
+    Xh = np.array([[_half_rne_by_hand(float(v)) for v in row] for row in X])
+    Ph = np.array([[_half_rne_by_hand(float(v)) for v in row] for row in P])
+    want = np.zeros((5, 7))
+    for n in range(5):
+        for d in range(7):
+            want[n, d] = sum(Xh[n, f] * Ph[d, f] for f in range(9))
+    bits, acc, _ = o.encode_rp(X, P, 7, o.F16)
+    assert np.allclose(acc, want, rtol=1e-14, atol=1e-14)
+    assert np.array_equal(bits, (want < 0).astype(np.uint8))
+    # operands already representable in half: identical to fp32
+    Xi = r.integers(0, 256, size=(4, 9)).astype(np.float32)
+    Pi = (1.0 - 2.0 * r.integers(0, 2, size=(6, 9))).astype(np.float32)
+    assert np.array_equal(o.encode_rp(Xi, Pi, 6, o.F16)[1], o.encode_rp(Xi, Pi, 6, o.F32)[1])
