@@ -57,7 +57,7 @@ typedef enum {
 } hdc_status;
 
 /* element types of buffers */
-enum { HDC_F32 = 0, HDC_BF16 = 1, HDC_I8 = 2, HDC_B1 = 3, HDC_U8 = 4, HDC_I32 = 5 };
+enum { HDC_F32 = 0, HDC_BF16 = 1, HDC_I8 = 2, HDC_B1 = 3, HDC_U8 = 4, HDC_I32 = 5, HDC_F16 = 6 };
 /* similarity kinds (L167 algorithmic choice) */
 enum { HDC_SIM_DOT = 0, HDC_SIM_COS = 1, HDC_SIM_HAMMING = 2 };
 /* knobs.hv_bits code (not a width) for a 16-bit IEEE half class operand (L165 "FP16") */
@@ -81,7 +81,8 @@ enum {
 
 /* Approximation knobs (section 4.2).
  *  D_eff      effective dimensionality, 1..D (L61, L155, L163).
- *  precision  operand type of the encode contraction (L165): HDC_F32 | HDC_BF16 | HDC_I8 | HDC_B1.
+ *  precision  operand type of the encode contraction (L165): HDC_F32 | HDC_BF16 | HDC_F16 | HDC_I8 |
+ *             HDC_B1.  HDC_F16: operands rounded to nearest-even IEEE half, fp32 accumulate.
  *             HDC_BF16: operands rounded to nearest-even bf16, fp32 accumulate.  HDC_I8: per-row
  *             symmetric int8 of X and of P (a = max|row|, s = 127/a, q = clamp(rint(x*s),+-127)),
  *             int32 accumulate.  HDC_B1: packed hypervectors with the real-valued contraction in

@@ -68,7 +68,7 @@ def _class_acc(K, D, seed, per_class=32):
 
 # ------------------------------------------------------------------------------------ encode rows
 def row_encode(h, peaks, reps, N, F, D, prec_name, x_bf16=False):
-    prec = {"f32": hd.HDC_F32, "bf16": hd.HDC_BF16, "i8": hd.HDC_I8}[prec_name]
+    prec = {"f32": hd.HDC_F32, "bf16": hd.HDC_BF16, "f16": hd.HDC_F16, "i8": hd.HDC_I8}[prec_name]
     X = torch.randn((N, F), device="cuda", generator=_gen(1))
     P = torch.randn((D, F), device="cuda", generator=_gen(2))
     if x_bf16:
@@ -79,7 +79,7 @@ def row_encode(h, peaks, reps, N, F, D, prec_name, x_bf16=False):
     call_ms = _time(fn, reps)
     k_ms, _ = _kernel(h, hd.HDC_K_ENCODE_GEMM, fn, reps)
     flops = 2.0 * N * F * D
-    mult = {"f32": 1.0 / 6.0, "bf16": 1.0, "i8": 2.0}[prec_name]
+    mult = {"f32": 1.0 / 6.0, "bf16": 1.0, "f16": 1.0, "i8": 2.0}[prec_name]
     peak = peaks["bf16_tflops"] * mult
     ach = flops / (k_ms * 1e-3) / 1e12
     return {"what": f"hdc_encode_rp N={N} F={F} D={D} precision={prec_name}" + (" (bf16 inputs in place)" if x_bf16 else ""),
@@ -364,6 +364,7 @@ def row_kmeans(h, peaks, reps, N=7797, K=26, D=10000, hv_bits=32, sim_name="cos"
 ROWS = {
     "c2_encode_f32": lambda h, p, r: row_encode(h, p, r, 131072, 617, 10000, "f32"),
     "c2_encode_bf16": lambda h, p, r: row_encode(h, p, r, 131072, 617, 10000, "bf16"),
+    "c2_encode_f16": lambda h, p, r: row_encode(h, p, r, 131072, 617, 10000, "f16"),
     "c2_encode_i8": lambda h, p, r: row_encode(h, p, r, 131072, 617, 10000, "i8"),
     "c2_classify_cos32": lambda h, p, r: row_classify(h, p, r, 131072, 26, 10000, 32, "cos"),
     "c4_classify_cos8": lambda h, p, r: row_classify(h, p, r, 131072, 6, 10000, 8, "cos"),

@@ -16,7 +16,7 @@ _LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "lib", "lib
 HDC_OK = 0
 HDC_ERR_INVALID_ARG, HDC_ERR_UNSUPPORTED, HDC_ERR_ALIGNMENT = -1, -2, -3
 HDC_ERR_WORKSPACE, HDC_ERR_CUDA, HDC_ERR_ARCH = -4, -5, -6
-HDC_F32, HDC_BF16, HDC_I8, HDC_B1, HDC_U8, HDC_I32 = 0, 1, 2, 3, 4, 5
+HDC_F32, HDC_BF16, HDC_I8, HDC_B1, HDC_U8, HDC_I32, HDC_F16 = 0, 1, 2, 3, 4, 5, 6
 HDC_SIM_DOT, HDC_SIM_COS, HDC_SIM_HAMMING = 0, 1, 2
 HDC_TRAIN_BUNDLE, HDC_TRAIN_PERCEPTRON, HDC_TRAIN_KMEANS = 0, 1, 2
 HDC_OUT_BITS, HDC_OUT_RAW = 1, 4

@@ -136,8 +136,9 @@ void plan_encode(const hdc_ctx* h, int64_t N, int F, int D_eff, const hdc_knobs_
     if (!p_inplace) pl.Ps = b.take<int8_t>((size_t)D_eff * pl.Fp);
     return;
   }
-  // BF16 / B1
+  // BF16 / B1 / F16 (half operands are always staged: the inputs are fp32 or bf16)
   if (!pl.tc) return;  // CUDA-core kernel rounds on load, no staging
+  if (prec == HDC_F16) x_inplace = p_inplace = false;
   pl.ldxs = pl.ldps = pl.Fp;
   if (!x_inplace) pl.Xs = b.take<__nv_bfloat16>((size_t)N * pl.Fp);
   if (!p_inplace) pl.Ps = b.take<__nv_bfloat16>((size_t)D_eff * pl.Fp);
@@ -212,6 +213,28 @@ int encode_rp_core(hdc_ctx* h, const void* X, int x_dtype, int64_t N, int F, int
     ce = launch_gemm_simt(Operand{pl.Xs, pl.ldxs, OPK_I8}, Operand{Pq, ldpq, OPK_I8}, N, D_eff, F, true, e,
                           st, &h->launches);
     return ce == cudaSuccess ? HDC_OK : cuda_fail(h, ce, "encode_rp int8");
+  }
+
+  if (prec == HDC_F16) {
+    plan_encode(h, N, F, D_eff, k, false, false, b, pl);
+    if (b.off > ws_bytes) return fail(h, HDC_ERR_WORKSPACE, "encode_rp: workspace too small");
+    if (pl.tc) {
+      ce = launch_convert_f16(X, xk, N, F, ldx, (__half*)pl.Xs, pl.ldxs, st, &h->launches);
+      if (ce != cudaSuccess) return cuda_fail(h, ce, "convert X");
+      ce = launch_convert_f16(P, pk, D_eff, F, ldp, (__half*)pl.Ps, pl.ldps, st, &h->launches);
+      if (ce != cudaSuccess) return cuda_fail(h, ce, "convert P");
+      TcOperands o{pl.Xs, pl.Ps, OPK_F16, pl.ldxs, pl.ldps, F, F, F, 1, 0u, 0u, 0};
+      {
+        Timed tm(h, HDC_K_ENCODE_GEMM, st);
+        ce = launch_gemm_tc(h->tc, o, N, D_eff, e, h->sm_count, tc_cta_group(k), st, &h->launches);
+      }
+      if (ce == cudaSuccess) return HDC_OK;
+      if (ce != cudaErrorNotSupported) return cuda_fail(h, ce, "encode_rp fp16 tcgen05");
+    }
+    const int xr = x_dtype == HDC_BF16 ? OPK_BF16_RF16 : OPK_F32_RF16;
+    const int pr = p_dtype == HDC_BF16 ? OPK_BF16_RF16 : OPK_F32_RF16;
+    ce = launch_gemm_simt(Operand{X, ldx, xr}, Operand{P, ldp, pr}, N, D_eff, F, false, e, st, &h->launches);
+    return ce == cudaSuccess ? HDC_OK : cuda_fail(h, ce, "encode_rp fp16");
   }
 
   // BF16 / B1
@@ -582,7 +605,8 @@ static int check_encode_rp_args(hdc_ctx* h, const void* X, int x_dtype, int64_t 
     return fail(h, HDC_ERR_INVALID_ARG, "encode_rp: p_dtype");
   int rc = check_knobs(h, k, D);
   if (rc) return rc;
-  if (k->precision != HDC_F32 && k->precision != HDC_BF16 && k->precision != HDC_I8 && k->precision != HDC_B1)
+  if (k->precision != HDC_F32 && k->precision != HDC_BF16 && k->precision != HDC_I8 && k->precision != HDC_B1 &&
+      k->precision != HDC_F16)
     return fail(h, HDC_ERR_INVALID_ARG, "encode_rp: precision");
   if (p_dtype == HDC_I8 && k->precision != HDC_I8)
     return fail(h, HDC_ERR_INVALID_ARG, "encode_rp: int8 P needs precision HDC_I8");

@@ -17,7 +17,9 @@ enum OperandKind : int {
   OPK_F32_RBF16 = 2,  // float rounded to nearest-even bf16 on load (precision BF16 / hv_bits 16)
   OPK_BITS = 3,       // packed hypervector bits: element k -> bit k&31 of word k>>5, value 1-2*bit
   OPK_I8 = 4,         // int8
-  OPK_F32_RF16 = 5    // float rounded to nearest-even IEEE half on load (hv code HDC_HV_F16)
+  OPK_F32_RF16 = 5,   // float rounded to nearest-even IEEE half on load (hv code HDC_HV_F16, precision HDC_F16)
+  OPK_BF16_RF16 = 6,  // __nv_bfloat16 widened, then rounded to IEEE half (precision HDC_F16 on bf16 inputs)
+  OPK_F16 = 7         // __half (staged operands of the tcgen05 path)
 };
 
 struct Operand {
@@ -80,7 +82,7 @@ void tc_context_destroy(TcContext*);
 struct TcOperands {
   const void* A;
   const void* B;
-  int elem_kind;  // OPK_BF16 | OPK_I8
+  int elem_kind;  // OPK_BF16 | OPK_F16 | OPK_I8
   int64_t lda, ldb;
   int64_t cols_a, cols_b;
   int Kr;
@@ -127,6 +129,8 @@ cudaError_t launch_scale_raw(void* raw, int64_t rows, int cols, int64_t ld, floa
 cudaError_t launch_perf_mask(uint32_t* mask, int W, int D_eff, Perf pf, cudaStream_t st, int64_t* nlaunch);
 
 // fp32/bf16 -> bf16 staging with zero padding of the reduction axis: dst [rows][ld_dst]
+cudaError_t launch_convert_f16(const void* src, int src_kind, int64_t rows, int cols, int64_t ld_src,
+                               __half* dst, int64_t ld_dst, cudaStream_t st, int64_t* nlaunch);
 cudaError_t launch_convert_bf16(const void* src, int src_kind, int64_t rows, int cols, int64_t ld_src,
                                 __nv_bfloat16* dst, int64_t ld_dst, cudaStream_t st, int64_t* nlaunch);
 // fp32/bf16 -> three bf16 segments [x1 | x2 | x3] with x1 = bf16(x), x2 = bf16(x - x1),

@@ -43,6 +43,25 @@ __global__ void convert_bf16_kernel(const void* __restrict__ src, int src_kind, 
   }
 }
 
+// ---------------------------------------------------------------------------------- fp16 staging
+// Same layout as convert_bf16_kernel with IEEE half RNE (precision HDC_F16).
+__global__ void convert_f16_kernel(const void* __restrict__ src, int src_kind, int64_t rows, int cols,
+                                   int64_t ld_src, __half* __restrict__ dst, int64_t ld_dst) {
+  const int chunks = (int)(ld_dst >> 3);
+  const int64_t total = rows * chunks;
+  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < total;
+       i += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t r = i / chunks;
+    const int c0 = (int)(i - r * chunks) << 3;
+    __align__(16) __half v[8];
+    const int64_t base = r * ld_src + c0;
+#pragma unroll
+    for (int j = 0; j < 8; ++j)
+      v[j] = __float2half_rn((c0 + j < cols) ? load_as_f32(src, src_kind, base + j) : 0.0f);
+    *reinterpret_cast<uint4*>(dst + r * ld_dst + c0) = *reinterpret_cast<const uint4*>(v);
+  }
+}
+
 // ---------------------------------------------------------------------------------- bf16 x3 split
 // x = x1 + x2 + x3 (+ O(2^-25 |x|)): x1 = bf16(x), x2 = bf16(x - x1), x3 = bf16(x - x1 - x2); both
 // residuals are exact fp32 subtractions.  dst [rows][3*seg]: segment s holds x_{s+1}; columns >=
@@ -221,6 +240,15 @@ cudaError_t launch_convert_bf16(const void* src, int src_kind, int64_t rows, int
   const int64_t total = rows * (ld_dst >> 3);
   convert_bf16_kernel<<<grid_for(total, 256, 148 * 16), 256, 0, st>>>(src, src_kind, rows, cols, ld_src,
                                                                      dst, ld_dst);
+  ++*nlaunch;
+  return cudaGetLastError();
+}
+
+cudaError_t launch_convert_f16(const void* src, int src_kind, int64_t rows, int cols, int64_t ld_src,
+                               __half* dst, int64_t ld_dst, cudaStream_t st, int64_t* nlaunch) {
+  if (rows <= 0) return cudaSuccess;
+  const int64_t total = rows * (ld_dst >> 3);
+  convert_f16_kernel<<<grid_for(total, 256, 148 * 16), 256, 0, st>>>(src, src_kind, rows, cols, ld_src, dst, ld_dst);
   ++*nlaunch;
   return cudaGetLastError();
 }

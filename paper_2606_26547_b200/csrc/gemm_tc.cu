@@ -98,6 +98,7 @@ struct TcParams {
   uint32_t a_segs, b_segs;      // 4 bits per segment: which operand segment it reads
   int seg_stride;               // elements between operand segments
   int group_m;                  // m-tiles per rasterisation group (EPI_SIGN / EPI_SCORE)
+  int f16;                      // 16-bit operands are IEEE half instead of bf16
   Epilogue e;
 };
 
@@ -227,7 +228,9 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     for (int64_t i = 0; rank == 0 && tile_at<EPI, CG>(p, i, mt, nt); ++i) {
       int n_valid = p.Nc - nt * BN;
       if (n_valid > BN) n_valid = BN;
-      const uint32_t idesc = instr_desc<INT8>(BM * CG, (n_valid + 15) & ~15);
+      // kind::f16 operand formats (bits 7..9 A, 10..12 B): 1 = bf16, 0 = IEEE half
+      const uint32_t idesc = instr_desc<INT8>(BM * CG, (n_valid + 15) & ~15) &
+                             ((!INT8 && p.f16) ? ~((1u << 7) | (1u << 10)) : ~0u);
       mbar_wait(tempty_bar(acc), acc_phase ^ 1u);
       tc_fence_after();
       const uint32_t d_tmem = tmem_base + (uint32_t)(acc * BN);
@@ -468,6 +471,7 @@ cudaError_t launch_gemm_tc(TcContext* tc, const TcOperands& o, int64_t M, int Nc
   p.b_segs = o.b_segs;
   p.seg_stride = o.seg_stride;
   p.group_m = 16 / cg;
+  p.f16 = o.elem_kind == OPK_F16;
   p.e = e;
   CUtensorMap tmA, tmB;
   if (!tc_make_map(tc, &tmA, o.A, int8, M, o.cols_a, o.lda, BM)) return cudaErrorInvalidValue;

@@ -123,7 +123,7 @@ def _encode(hd, h, X, P, D_eff, prec, flags=0, bf16_inputs=False):
     return host_bits(H, D_eff), raw.cpu().numpy(), host_words(H)
 
 
-@pytest.mark.parametrize("prec", ["F32", "BF16", "I8", "B1"])
+@pytest.mark.parametrize("prec", ["F32", "BF16", "F16", "I8", "B1"])
 @pytest.mark.parametrize("flags", [0, 1, 2, 4])
 @pytest.mark.parametrize("N,F,D,D_eff", [(200, 64, 2048, 2048), (131, 617, 1000, 999), (300, 100, 700, 33),
                                          (3, 7, 40, 40), (520, 784, 520, 515)])
@@ -151,7 +151,7 @@ def test_encode_rp_exact_arithmetic(hd, h, prec, flags, N, F, D, D_eff):
         assert (words[:, W - 1] >> (D_eff % 32) == 0).all()
 
 
-@pytest.mark.parametrize("prec", ["F32", "BF16", "I8"])
+@pytest.mark.parametrize("prec", ["F32", "BF16", "F16", "I8"])
 @pytest.mark.parametrize("flags", [0, 1, 2, 4])
 def test_encode_rp_float_c2_shape(hd, h, prec, flags):
     """Gaussian features / projection at the C2 shape (F=617, D=10000 sliced): raw accumulators
@@ -580,6 +580,8 @@ def test_encode_rp_fuzz_exact(hd, h, case):
     D = int(r.choice([32, 33, 100, 255, 256, 257, 1000, 2048, 3001]))
     D_eff = int(r.integers(1, D + 1)) if r.random() < 0.5 else D
     prec = ["F32", "BF16", "I8", "B1"][int(r.integers(0, 4))]
+    if prec == "BF16" and case % 2:
+        prec = "F16"
     flags = int(r.choice([0, 1, 2, 4]))
     X = r.integers(0, 256, size=(N, F)).astype(np.float32)
     X[r.random((N, F)) < 0.3] = 0
@@ -666,7 +668,7 @@ def _encode_perf(hd, h, X, P, D_eff, prec, begin, stride, flags=0, bf16_inputs=F
     return host_bits(H, D_eff), raw.cpu().numpy(), host_words(H)
 
 
-@pytest.mark.parametrize("prec", ["F32", "BF16", "I8", "B1"])
+@pytest.mark.parametrize("prec", ["F32", "BF16", "F16", "I8", "B1"])
 @pytest.mark.parametrize("flags", [0, 1])
 @pytest.mark.parametrize("N,F,D,D_eff,begin,stride", [(200, 64, 2048, 2048, 0, 2), (131, 617, 1000, 999, 5, 8),
                                                       (300, 100, 700, 33, 99, 3), (70, 784, 520, 515, 1, 2),
@@ -843,3 +845,15 @@ def test_fp16_perceptron_epoch_teacher_forced(hd, h):
         rows = [k for k in range(K) if k not in touched]
         assert np.array_equal(Cd.cpu().numpy()[rows], C_next[rows])
         C_or = C_next
+
+
+def test_encode_rp_fp16_precision_on_bf16_inputs(hd, h):
+    """precision HDC_F16 with bf16 inputs: widened exactly, then rounded to half (both kernels)."""
+    w = gen.c5_large_batch(n=200, D=768, K=10, F=1024, per_class=1)
+    Xb = np.asarray(torch.from_numpy(w["X"]).to(torch.bfloat16).float())
+    Pb = np.asarray(torch.from_numpy(w["P"]).to(torch.bfloat16).float())
+    bits_or, acc_or, absum = O.encode_rp(Xb, Pb, 768, O.F16, want_absum=True)
+    for flags in (0, 1):
+        bits, raw, _ = _encode(hd, h, Xb, Pb, 768, hd.HDC_F16, flags, bf16_inputs=True)
+        assert (np.abs(raw - acc_or) <= 1e-3 * np.abs(acc_or) + 1e-6 * absum).all()
+        check_sign_band(bits, bits_or, acc_or, absum, 1024)
