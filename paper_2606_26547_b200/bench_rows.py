@@ -344,6 +344,39 @@ def c4_sweep(h, peaks, reps=5, NQ=131072):
     return points
 
 
+def adc_sweep(h, peaks, reps=5, NQ=131072):
+    """SpecPCM-simulator knobs on the ISOLET-shaped mixture (D = 1024, TRAINING_ITER = 2, MLC = 1):
+    test accuracy and queries/s of hdc_similarity_adc for the paper's ADC windows, beside the exact
+    Hamming classify at the same D.  Accuracy parity with the oracle: tests/test_gpu_kernels.py."""
+    from workloads import gen
+    import numpy as np
+    w = gen.c2_isolet_shaped()
+    K, D = w["K"], w["D"]
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()  # noqa: E731
+    Xtr, Xte, ytr, P = dev(w["Xtr"]), dev(w["Xte"]), dev(w["ytr"]), dev(w["P"])
+    yte = w["yte"]
+    out = []
+    for D_eff in (1024, 2048, 10000):
+        kn_e = hd.knobs(D_eff, precision=hd.HDC_F32)
+        kn = hd.knobs(D_eff, hv_bits=1, sim=hd.HDC_SIM_HAMMING)
+        Htr, Hte = h.hdc_encode_rp(Xtr, P, kn_e), h.hdc_encode_rp(Xte, P, kn_e)
+        C = torch.zeros((K, D), dtype=torch.float32, device="cuda")
+        h.hdc_train_epoch(hd.HDC_TRAIN_BUNDLE, Htr, ytr, C, kn)
+        for _ in range(2):
+            h.hdc_train_epoch(hd.HDC_TRAIN_PERCEPTRON, Htr, ytr, C, kn, lr=w["lr"], batch=0)
+        Hq = dev(gen.tile_rows(Hte.cpu().numpy(), NQ))
+        lab = h.hdc_classify(Hte, C, kn).cpu().numpy()
+        ms = _time(lambda: h.hdc_classify(Hq, C, kn), reps)
+        out.append({"D_eff": D_eff, "similarity": "hamming (exact)", "accuracy": float((lab == yte).mean()),
+                    "queries_per_s": NQ / (ms * 1e-3)})
+        for res, step, fl, ce in [(8, 1, -127, 128), (8, 2, -3, 128), (6, 9, -3, 128), (4, 9, -3, 128), (2, 32, -3, 128)]:
+            _, lab = h.hdc_similarity_adc(Hte, C, kn, res, step, fl, ce, want_scores=False)
+            ms = _time(lambda: h.hdc_similarity_adc(Hq, C, kn, res, step, fl, ce, want_scores=False), reps)
+            out.append({"D_eff": D_eff, "similarity": f"adc res={res} step={step} floor={fl} ceil={ce}",
+                        "accuracy": float((lab.cpu().numpy() == yte).mean()), "queries_per_s": NQ / (ms * 1e-3)})
+    return out
+
+
 def row_kmeans(h, peaks, reps, N=7797, K=26, D=10000, hv_bits=32, sim_name="cos"):
     """HD-Clustering epoch (assign + re-bundle) on noisy copies of K prototypes, ISOLET-sized."""
     sim = {"cos": hd.HDC_SIM_COS, "hamming": hd.HDC_SIM_HAMMING}[sim_name]
@@ -401,6 +434,7 @@ def main():
     ap.add_argument("--row", default=None, choices=sorted(ROWS))
     ap.add_argument("--reps", type=int, default=5)
     ap.add_argument("--c4-sweep", action="store_true", help="configs[3]: D_eff x precision x epochs table")
+    ap.add_argument("--adc-sweep", action="store_true", help="SpecPCM ADC windows (PAPER.md L273): accuracy, queries/s")
     a = ap.parse_args()
     pk = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(pk):
@@ -413,6 +447,11 @@ def main():
     if a.c4_sweep:
         for pt in c4_sweep(h, peaks, a.reps):
             print(json.dumps({"c4_sweep": pt}), flush=True)
+        h.close()
+        return
+    if a.adc_sweep:
+        for pt in adc_sweep(h, peaks, a.reps):
+            print(json.dumps({"adc_sweep": pt}), flush=True)
         h.close()
         return
     res = run(h, peaks, a.reps, a.row)
