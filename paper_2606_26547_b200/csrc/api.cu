@@ -21,6 +21,9 @@ struct hdc_ctx {
   cudaEvent_t ev_done[2] = {nullptr, nullptr};
   cudaEvent_t ev_entry = nullptr;
   bool timing = false;
+  // set by hdc_infer_rp_host for chunks after the first of equal size: the staged projection and the
+  // prepared class operand of the previous chunk still sit at the same workspace addresses
+  bool reuse_prep = false;
   std::vector<std::pair<cudaEvent_t, cudaEvent_t>> tev[HDC_K_COUNT];  // event pool per kernel id
   size_t tused[HDC_K_COUNT] = {0, 0, 0, 0};
 };
@@ -167,8 +170,10 @@ int encode_rp_core(hdc_ctx* h, const void* X, int x_dtype, int64_t N, int F, int
     if (pl.tc) {
       ce = launch_split3_bf16(X, xk, N, F, ldx, (__nv_bfloat16*)pl.Xs, pl.Fp, st, &h->launches);
       if (ce != cudaSuccess) return cuda_fail(h, ce, "split X");
-      ce = launch_split3_bf16(P, pk, D_eff, F, ldp, (__nv_bfloat16*)pl.Ps, pl.Fp, st, &h->launches);
-      if (ce != cudaSuccess) return cuda_fail(h, ce, "split P");
+      if (!h->reuse_prep) {
+        ce = launch_split3_bf16(P, pk, D_eff, F, ldp, (__nv_bfloat16*)pl.Ps, pl.Fp, st, &h->launches);
+        if (ce != cudaSuccess) return cuda_fail(h, ce, "split P");
+      }
       TcOperands o{pl.Xs, pl.Ps, OPK_BF16, pl.ldxs, pl.ldps, pl.ldxs, pl.ldps, pl.Fp, 6,
                    SPLIT_A_SEGS, SPLIT_B_SEGS, pl.Fp};
       {
@@ -196,8 +201,10 @@ int encode_rp_core(hdc_ctx* h, const void* X, int x_dtype, int64_t N, int F, int
     const void* Pq = P;
     int64_t ldpq = ldp;
     if (!p_in) {
-      ce = launch_quantize_rows_i8(P, pk, D_eff, F, ldp, (int8_t*)pl.Ps, pl.ldps, st, &h->launches);
-      if (ce != cudaSuccess) return cuda_fail(h, ce, "quantize P");
+      if (!h->reuse_prep) {
+        ce = launch_quantize_rows_i8(P, pk, D_eff, F, ldp, (int8_t*)pl.Ps, pl.ldps, st, &h->launches);
+        if (ce != cudaSuccess) return cuda_fail(h, ce, "quantize P");
+      }
       Pq = pl.Ps;
       ldpq = pl.ldps;
     }
@@ -221,8 +228,10 @@ int encode_rp_core(hdc_ctx* h, const void* X, int x_dtype, int64_t N, int F, int
     if (pl.tc) {
       ce = launch_convert_f16(X, xk, N, F, ldx, (__half*)pl.Xs, pl.ldxs, st, &h->launches);
       if (ce != cudaSuccess) return cuda_fail(h, ce, "convert X");
-      ce = launch_convert_f16(P, pk, D_eff, F, ldp, (__half*)pl.Ps, pl.ldps, st, &h->launches);
-      if (ce != cudaSuccess) return cuda_fail(h, ce, "convert P");
+      if (!h->reuse_prep) {
+        ce = launch_convert_f16(P, pk, D_eff, F, ldp, (__half*)pl.Ps, pl.ldps, st, &h->launches);
+        if (ce != cudaSuccess) return cuda_fail(h, ce, "convert P");
+      }
       TcOperands o{pl.Xs, pl.Ps, OPK_F16, pl.ldxs, pl.ldps, F, F, F, 1, 0u, 0u, 0};
       {
         Timed tm(h, HDC_K_ENCODE_GEMM, st);
@@ -251,8 +260,10 @@ int encode_rp_core(hdc_ctx* h, const void* X, int x_dtype, int64_t N, int F, int
       ldxb = pl.ldxs;
     }
     if (!tc_ok_p) {
-      ce = launch_convert_bf16(P, pk, D_eff, F, ldp, (__nv_bfloat16*)pl.Ps, pl.ldps, st, &h->launches);
-      if (ce != cudaSuccess) return cuda_fail(h, ce, "convert P");
+      if (!h->reuse_prep) {
+        ce = launch_convert_bf16(P, pk, D_eff, F, ldp, (__nv_bfloat16*)pl.Ps, pl.ldps, st, &h->launches);
+        if (ce != cudaSuccess) return cuda_fail(h, ce, "convert P");
+      }
       Pb = pl.Ps;
       ldpb = pl.ldps;
     }
@@ -341,7 +352,7 @@ int do_similarity(hdc_ctx* h, const uint32_t* Hbits, int64_t N, int64_t ldh, con
     const size_t pbytes = sim_tc_partial_bytes(N, K, k->hv_bits, D_eff, h->sm_count);
     double* partial = pbytes ? b.take<double>(pbytes / sizeof(double)) : nullptr;
     if (b.off > ws_bytes) return fail(h, HDC_ERR_WORKSPACE, "similarity: workspace too small");
-    if (colscale) {
+    if (colscale && !h->reuse_prep) {
       // norms over the operand as the contraction sees it (permutation-invariant)
       if (k->hv_bits == 8) {
         const int64_t ldq = round_up(D_eff, 16);
@@ -376,7 +387,7 @@ int do_similarity(hdc_ctx* h, const uint32_t* Hbits, int64_t N, int64_t ldh, con
     {
       Timed tm(h, HDC_K_SIM, st);
       ce = launch_sim_tc(h->tc, Hbits, N, ldh, C_acc, K, ldc, D_eff, k->hv_bits, cop, amax, e, pf, partial,
-                         h->sm_count, st, &h->launches);
+                         h->reuse_prep, h->sm_count, st, &h->launches);
     }
     if (ce == cudaSuccess) return HDC_OK;
     if (ce != cudaErrorNotSupported) return cuda_fail(h, ce, "similarity tcgen05");
@@ -384,14 +395,18 @@ int do_similarity(hdc_ctx* h, const uint32_t* Hbits, int64_t N, int64_t ldh, con
   if (k->sim == HDC_SIM_HAMMING) {
     uint32_t* cbits = b.take<uint32_t>((size_t)K * W);
     if (b.off > ws_bytes) return fail(h, HDC_ERR_WORKSPACE, "similarity: workspace too small");
-    ce = launch_sign_bits(C_acc, K, D_eff, ldc, cbits, W, st, &h->launches);
-    if (ce != cudaSuccess) return cuda_fail(h, ce, "sign_bits");
+    if (!h->reuse_prep) {
+      ce = launch_sign_bits(C_acc, K, D_eff, ldc, cbits, W, st, &h->launches);
+      if (ce != cudaSuccess) return cuda_fail(h, ce, "sign_bits");
+    }
     uint32_t* pmask = nullptr;
     if (perf_on(pf)) {
       pmask = b.take<uint32_t>((size_t)W);
       if (b.off > ws_bytes) return fail(h, HDC_ERR_WORKSPACE, "similarity: workspace too small");
-      ce = launch_perf_mask(pmask, W, D_eff, pf, st, &h->launches);
-      if (ce != cudaSuccess) return cuda_fail(h, ce, "perforation mask");
+      if (!h->reuse_prep) {
+        ce = launch_perf_mask(pmask, W, D_eff, pf, st, &h->launches);
+        if (ce != cudaSuccess) return cuda_fail(h, ce, "perforation mask");
+      }
     }
     {
       Timed tm(h, HDC_K_SIM, st);
@@ -951,11 +966,14 @@ extern "C" int32_t hdc_infer_rp_host(hdc_handle_t h, const void* X_host, int32_t
     cudaStreamWaitEvent(st, h->ev_copied[buf], 0);
     Bump be(ws);
     be.off = base_off;
+    // same chunk size => same workspace layout: P staging and class-operand preparation of chunk 0 are reused
+    h->reuse_prep = c > 0 && nb == chunk;
     rc = do_encode_rp(h, Xd[buf], x_dtype, nb, F, F, P, p_dtype, D, ldp, knobs, HDC_OUT_BITS, Hd, W, nullptr, 0,
                       be, ws_bytes, st);
-    if (rc) return rc;
-    rc = do_similarity(h, Hd, nb, W, C_acc, K, ldc, knobs, nullptr, 0, 0, Ld + n0, nullptr, nullptr, be,
-                       ws_bytes, st);
+    if (rc == HDC_OK)
+      rc = do_similarity(h, Hd, nb, W, C_acc, K, ldc, knobs, nullptr, 0, 0, Ld + n0, nullptr, nullptr, be,
+                         ws_bytes, st);
+    h->reuse_prep = false;
     if (rc) return rc;
     cudaEventRecord(h->ev_done[buf], st);
   }

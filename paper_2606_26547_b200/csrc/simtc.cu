@@ -586,8 +586,8 @@ size_t sim_tc_partial_bytes(int64_t N, int K, int hv_bits, int D_eff, int sm_cou
 
 cudaError_t launch_sim_tc(TcContext* tc, const uint32_t* Hbits, int64_t N, int64_t ldh, const float* C_acc,
                           int K, int64_t ldc, int D_eff, int hv_bits, void* cop, float* amax_scratch,
-                          const Epilogue& e, Perf pf, double* partial, int sm_count, cudaStream_t st,
-                          int64_t* nlaunch) {
+                          const Epilogue& e, Perf pf, double* partial, bool cop_ready, int sm_count,
+                          cudaStream_t st, int64_t* nlaunch) {
   if (!tc) return cudaErrorNotSupported;
   if (N <= 0) return cudaSuccess;
   if ((reinterpret_cast<uintptr_t>(cop) & 15) != 0) return cudaErrorNotSupported;
@@ -598,11 +598,11 @@ cudaError_t launch_sim_tc(TcContext* tc, const uint32_t* Hbits, int64_t N, int64
   const int BK = int8 ? 128 : 64;
   const int64_t ld = (int64_t)num_kb * BK;
   cudaError_t ce;
-  if (hv_bits == 8) {
+  if (hv_bits == 8 && !cop_ready) {
     ce = launch_tensor_amax(C_acc, K, D_eff, ldc, pf, amax_scratch, st, nlaunch);
     if (ce != cudaSuccess) return ce;
   }
-  {
+  if (!cop_ready) {
     const int64_t total = (int64_t)rows_total * ld;
     int64_t g = (total + 255) / 256;
     if (g > (int64_t)sm_count * 16) g = (int64_t)sm_count * 16;

@@ -857,3 +857,29 @@ def test_encode_rp_fp16_precision_on_bf16_inputs(hd, h):
         bits, raw, _ = _encode(hd, h, Xb, Pb, 768, hd.HDC_F16, flags, bf16_inputs=True)
         assert (np.abs(raw - acc_or) <= 1e-3 * np.abs(acc_or) + 1e-6 * absum).all()
         check_sign_band(bits, bits_or, acc_or, absum, 1024)
+
+
+@pytest.mark.parametrize("prec,hv_bits,sim,K,perf", [("F32", 32, "COS", 26, False), ("I8", 8, "COS", 6, False),
+                                                     ("BF16", 1, "HAMMING", 10, True), ("F16", 17, "DOT", 7, False),
+                                                     ("B1", 1, "HAMMING", 100, False), ("BF16", 16, "COS", 3, True)])
+def test_infer_rp_host_chunks_reuse_staged_operands(hd, h, prec, hv_bits, sim, K, perf):
+    """hdc_infer_rp_host stages P and prepares the class operand once and reuses them for the following
+    chunks of equal size (the last, shorter chunk prepares again): labels equal the two device calls on
+    the whole batch, for every precision / class-operand kind; exact-integer operands."""
+    r = rng(25, K, hv_bits)
+    N, F, D, D_eff = 16384 * 2 + 5000, 64, 1100, 1000
+    X = r.integers(0, 256, size=(N, F)).astype(np.float32)
+    P = (1.0 - 2.0 * r.integers(0, 2, size=(D, F))).astype(np.float32)
+    C = r.integers(-20, 21, size=(K, D)).astype(np.float32)
+    kw = dict(perf_begin=3, perf_stride=4) if perf else {}
+    kn = hd.knobs(D_eff, precision=getattr(hd, "HDC_" + prec), hv_bits=hv_bits, sim=getattr(hd, "HDC_SIM_" + sim), **kw)
+    Pd, Cd = dev(P), dev(C)
+    lab_dev = h.hdc_classify(h.hdc_encode_rp(dev(X), Pd, kn), Cd, kn).cpu().numpy()
+    lab_host = h.hdc_infer_rp_host(torch.from_numpy(X).pin_memory(), Pd, Cd, kn).numpy()
+    assert np.array_equal(lab_host, lab_dev)
+    # a second call with another class model through the same workspace must not see stale operands
+    C2 = -C
+    lab_dev2 = h.hdc_classify(h.hdc_encode_rp(dev(X), Pd, kn), dev(C2), kn).cpu().numpy()
+    lab_host2 = h.hdc_infer_rp_host(torch.from_numpy(X).pin_memory(), Pd, dev(C2), kn).numpy()
+    assert np.array_equal(lab_host2, lab_dev2)
+    assert not np.array_equal(lab_host2, lab_host)
