@@ -68,18 +68,22 @@ def _class_acc(K, D, seed, per_class=32):
 
 # ------------------------------------------------------------------------------------ encode rows
 def row_encode(h, peaks, reps, N, F, D, prec_name, x_bf16=False):
-    prec = {"f32": hd.HDC_F32, "bf16": hd.HDC_BF16, "f16": hd.HDC_F16, "i8": hd.HDC_I8}[prec_name]
+    flags = 0
+    if prec_name == "f32_fast":   # HDC_FLAG_F32_FAST: 2-way half splits, three products
+        flags = hd.HDC_FLAG_F32_FAST
+    prec = {"f32": hd.HDC_F32, "f32_fast": hd.HDC_F32, "bf16": hd.HDC_BF16, "f16": hd.HDC_F16,
+            "i8": hd.HDC_I8}[prec_name]
     X = torch.randn((N, F), device="cuda", generator=_gen(1))
     P = torch.randn((D, F), device="cuda", generator=_gen(2))
     if x_bf16:
         X, P = X.to(torch.bfloat16), P.to(torch.bfloat16)
-    kn = hd.knobs(D, precision=prec)
+    kn = hd.knobs(D, precision=prec, flags=flags)
     H = torch.empty((N, (D + 31) // 32), dtype=torch.int32, device="cuda")
     fn = lambda: h.hdc_encode_rp(X, P, kn, Hbits=H)  # noqa: E731
     call_ms = _time(fn, reps)
     k_ms, _ = _kernel(h, hd.HDC_K_ENCODE_GEMM, fn, reps)
     flops = 2.0 * N * F * D
-    mult = {"f32": 1.0 / 6.0, "bf16": 1.0, "f16": 1.0, "i8": 2.0}[prec_name]
+    mult = {"f32": 1.0 / 6.0, "f32_fast": 1.0 / 3.0, "bf16": 1.0, "f16": 1.0, "i8": 2.0}[prec_name]
     peak = peaks["bf16_tflops"] * mult
     ach = flops / (k_ms * 1e-3) / 1e12
     return {"what": f"hdc_encode_rp N={N} F={F} D={D} precision={prec_name}" + (" (bf16 inputs in place)" if x_bf16 else ""),
@@ -396,6 +400,7 @@ def row_kmeans(h, peaks, reps, N=7797, K=26, D=10000, hv_bits=32, sim_name="cos"
 
 ROWS = {
     "c2_encode_f32": lambda h, p, r: row_encode(h, p, r, 131072, 617, 10000, "f32"),
+    "c2_encode_f32_fast": lambda h, p, r: row_encode(h, p, r, 131072, 617, 10000, "f32_fast"),
     "c2_encode_bf16": lambda h, p, r: row_encode(h, p, r, 131072, 617, 10000, "bf16"),
     "c2_encode_f16": lambda h, p, r: row_encode(h, p, r, 131072, 617, 10000, "f16"),
     "c2_encode_i8": lambda h, p, r: row_encode(h, p, r, 131072, 617, 10000, "i8"),

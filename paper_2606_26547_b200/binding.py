@@ -22,7 +22,7 @@ HDC_TRAIN_BUNDLE, HDC_TRAIN_PERCEPTRON, HDC_TRAIN_KMEANS = 0, 1, 2
 HDC_OUT_BITS, HDC_OUT_RAW = 1, 4
 HDC_OP_ENCODE_RP, HDC_OP_ENCODE_LEVELID, HDC_OP_SIMILARITY = 0, 1, 2
 HDC_OP_CLASSIFY, HDC_OP_TRAIN_EPOCH, HDC_OP_INFER_RP_HOST = 3, 4, 5
-HDC_FLAG_NONE, HDC_FLAG_SIMT, HDC_FLAG_TC_1CTA, HDC_FLAG_TC_2CTA = 0, 1, 2, 4
+HDC_FLAG_NONE, HDC_FLAG_SIMT, HDC_FLAG_TC_1CTA, HDC_FLAG_TC_2CTA, HDC_FLAG_F32_FAST = 0, 1, 2, 4, 8
 HDC_HV_F16 = 17
 HDC_K_ENCODE_GEMM, HDC_K_SIM, HDC_K_LEVELID, HDC_K_CLASS_UPDATE = 0, 1, 2, 3
 

@@ -102,6 +102,9 @@ Perf enc_perf_of(const hdc_knobs_t* k) {
 // multiplies A part a(s) with B part b(s); smallest terms first (x3p1, x2p2, x1p3, x2p1, x1p2, x1p1).
 constexpr uint32_t SPLIT_A_SEGS = 0x001012u;  // nibble s = a(s): 2,1,0,1,0,0
 constexpr uint32_t SPLIT_B_SEGS = 0x010210u;  // nibble s = b(s): 0,1,2,0,1,0
+// HDC_FLAG_F32_FAST: 2-way half splits, three products (h2 p1, h1 p2, h1 p1)
+constexpr uint32_t SPLIT2_A_SEGS = 0x001u;  // a(s): 1,0,0
+constexpr uint32_t SPLIT2_B_SEGS = 0x010u;  // b(s): 0,1,0
 
 struct EncodePlan {
   bool tc = false;         // tensor-core kernel
@@ -109,6 +112,8 @@ struct EncodePlan {
   void* Ps = nullptr;      // staged P
   int64_t ldxs = 0, ldps = 0;
   int Fp = 0;
+  int* ex = nullptr;       // HDC_FLAG_F32_FAST: per-row scale exponents of X and of P
+  int* ep = nullptr;
 };
 
 // 1 / 2 when the knobs force the 1-CTA / CTA-pair contraction kernel, 0 = by problem size
@@ -128,6 +133,14 @@ void plan_encode(const hdc_ctx* h, int64_t N, int F, int D_eff, const hdc_knobs_
   pl.Fp = (int)round_up(F, 64);
   if (prec == HDC_F32) {
     if (!pl.tc) return;  // FFMA kernel reads the operands in place
+    if (k->flags & HDC_FLAG_F32_FAST) {
+      pl.ldxs = pl.ldps = 2 * (int64_t)pl.Fp;
+      pl.Xs = b.take<__half>((size_t)N * pl.ldxs);
+      pl.Ps = b.take<__half>((size_t)D_eff * pl.ldps);
+      pl.ex = b.take<int>((size_t)N);
+      pl.ep = b.take<int>((size_t)D_eff);
+      return;
+    }
     pl.ldxs = pl.ldps = 3 * (int64_t)pl.Fp;
     pl.Xs = b.take<__nv_bfloat16>((size_t)N * pl.ldxs);
     pl.Ps = b.take<__nv_bfloat16>((size_t)D_eff * pl.ldps);
@@ -167,6 +180,24 @@ int encode_rp_core(hdc_ctx* h, const void* X, int x_dtype, int64_t N, int F, int
   if (prec == HDC_F32) {
     plan_encode(h, N, F, D_eff, k, false, false, b, pl);
     if (b.off > ws_bytes) return fail(h, HDC_ERR_WORKSPACE, "encode_rp: workspace too small");
+    if (pl.tc && (k->flags & HDC_FLAG_F32_FAST)) {
+      ce = launch_split2_f16(X, xk, N, F, ldx, (__half*)pl.Xs, pl.Fp, pl.ex, st, &h->launches);
+      if (ce != cudaSuccess) return cuda_fail(h, ce, "split X");
+      if (!h->reuse_prep) {
+        ce = launch_split2_f16(P, pk, D_eff, F, ldp, (__half*)pl.Ps, pl.Fp, pl.ep, st, &h->launches);
+        if (ce != cudaSuccess) return cuda_fail(h, ce, "split P");
+      }
+      TcOperands o{pl.Xs, pl.Ps, OPK_F16, pl.ldxs, pl.ldps, pl.ldxs, pl.ldps, pl.Fp, 3,
+                   SPLIT2_A_SEGS, SPLIT2_B_SEGS, pl.Fp};
+      {
+        Timed tm(h, HDC_K_ENCODE_GEMM, st);
+        ce = launch_gemm_tc(h->tc, o, N, D_eff, e, h->sm_count, tc_cta_group(k), st, &h->launches);
+      }
+      if (ce == cudaSuccess && want_raw)
+        ce = launch_unscale_raw((float*)Hraw, N, D_eff, ldraw, pl.ex, pl.ep, st, &h->launches);
+      if (ce == cudaSuccess) return HDC_OK;
+      if (ce != cudaErrorNotSupported) return cuda_fail(h, ce, "encode_rp fp32 (2 x fp16) tcgen05");
+    }
     if (pl.tc) {
       ce = launch_split3_bf16(X, xk, N, F, ldx, (__nv_bfloat16*)pl.Xs, pl.Fp, st, &h->launches);
       if (ce != cudaSuccess) return cuda_fail(h, ce, "split X");

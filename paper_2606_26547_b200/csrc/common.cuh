@@ -130,6 +130,12 @@ cudaError_t launch_scale_raw(void* raw, int64_t rows, int cols, int64_t ld, floa
 cudaError_t launch_perf_mask(uint32_t* mask, int W, int D_eff, Perf pf, cudaStream_t st, int64_t* nlaunch);
 
 // fp32/bf16 -> bf16 staging with zero padding of the reduction axis: dst [rows][ld_dst]
+// HDC_FLAG_F32_FAST staging: per-row power-of-two scale + 2-way half split ([h1 | h2], seg columns each);
+// expo[row] = the exponent applied; launch_unscale_raw undoes both operands' scales on raw accumulators.
+cudaError_t launch_split2_f16(const void* src, int src_kind, int64_t rows, int cols, int64_t ld_src, __half* dst,
+                              int seg, int* expo, cudaStream_t st, int64_t* nlaunch);
+cudaError_t launch_unscale_raw(float* raw, int64_t rows, int cols, int64_t ld, const int* ex, const int* ep,
+                               cudaStream_t st, int64_t* nlaunch);
 cudaError_t launch_convert_f16(const void* src, int src_kind, int64_t rows, int cols, int64_t ld_src,
                                __half* dst, int64_t ld_dst, cudaStream_t st, int64_t* nlaunch);
 cudaError_t launch_convert_bf16(const void* src, int src_kind, int64_t rows, int cols, int64_t ld_src,

@@ -102,6 +102,50 @@ __global__ void split3_bf16_kernel(const void* __restrict__ src, int src_kind, i
   }
 }
 
+// ---------------------------------------------------------------------------------- fp16 x2 split
+// HDC_FLAG_F32_FAST: x * 2^e = h1 + h2 (+ O(2^-22 |x|)), h1 = half(x 2^e), h2 = half(x 2^e - h1), with the
+// per-row exponent e chosen so that the row maximum lands in [2^14, 2^15): every element within 2^-18
+// of the row maximum keeps 22 mantissa bits, smaller ones are held to 2^-25 absolute (half subnormals),
+// i.e. 2^-40 of the row maximum.  Power-of-two row scales change no sign and are undone exactly on
+// the optional raw accumulators.  dst [rows][2*seg]: segment 0 = h1, segment 1 = h2; columns >= cols
+// are zero.  One warp per row.
+__global__ void split2_f16_rows_kernel(const void* __restrict__ src, int src_kind, int64_t rows, int cols,
+                                       int64_t ld_src, __half* __restrict__ dst, int seg,
+                                       int* __restrict__ expo) {
+  const int lane = threadIdx.x & 31;
+  const int64_t warp = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
+  const int64_t nwarps = ((int64_t)gridDim.x * blockDim.x) >> 5;
+  for (int64_t r = warp; r < rows; r += nwarps) {
+    float a = 0.0f;
+    for (int c = lane; c < cols; c += 32) a = fmaxf(a, fabsf(load_as_f32(src, src_kind, r * ld_src + c)));
+#pragma unroll
+    for (int off = 16; off; off >>= 1) a = fmaxf(a, __shfl_xor_sync(0xffffffffu, a, off));
+    const int e = a > 0.0f ? 14 - ilogbf(a) : 0;
+    if (lane == 0) expo[r] = e;
+    __half* o = dst + r * (int64_t)(2 * seg);
+    for (int c = lane; c < seg; c += 32) {
+      float xs = 0.0f;
+      if (c < cols) xs = scalbnf(load_as_f32(src, src_kind, r * ld_src + c), e);
+      const __half h1 = __float2half_rn(xs);
+      const __half h2 = __float2half_rn(__fsub_rn(xs, __half2float(h1)));
+      o[c] = h1;
+      o[seg + c] = h2;
+    }
+  }
+}
+
+// raw[n,d] = raw[n,d] * 2^-(ex[n] + ep[d])   (exact)
+__global__ void unscale_raw_kernel(float* __restrict__ raw, int64_t rows, int cols, int64_t ld,
+                                   const int* __restrict__ ex, const int* __restrict__ ep) {
+  const int64_t total = rows * cols;
+  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < total;
+       i += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t r = i / cols;
+    const int d = (int)(i - r * cols);
+    raw[r * ld + d] = scalbnf(raw[r * ld + d], -(ex[r] + ep[d]));
+  }
+}
+
 // ---------------------------------------------------------------------------------- int8 per row
 __device__ __forceinline__ int quant_i8(float x, float s) {
   float q = rintf(__fmul_rn(x, s));  // round-half-even, one rounded multiply (no FMA contraction)
@@ -258,6 +302,23 @@ cudaError_t launch_split3_bf16(const void* src, int src_kind, int64_t rows, int 
   if (rows <= 0) return cudaSuccess;
   const int64_t total = rows * (seg >> 3);
   split3_bf16_kernel<<<grid_for(total, 256, 148 * 16), 256, 0, st>>>(src, src_kind, rows, cols, ld_src, dst, seg);
+  ++*nlaunch;
+  return cudaGetLastError();
+}
+
+cudaError_t launch_split2_f16(const void* src, int src_kind, int64_t rows, int cols, int64_t ld_src, __half* dst,
+                              int seg, int* expo, cudaStream_t st, int64_t* nlaunch) {
+  if (rows <= 0) return cudaSuccess;
+  split2_f16_rows_kernel<<<grid_for(rows * 32, 256, 148 * 16), 256, 0, st>>>(src, src_kind, rows, cols, ld_src, dst,
+                                                                            seg, expo);
+  ++*nlaunch;
+  return cudaGetLastError();
+}
+
+cudaError_t launch_unscale_raw(float* raw, int64_t rows, int cols, int64_t ld, const int* ex, const int* ep,
+                               cudaStream_t st, int64_t* nlaunch) {
+  if (rows <= 0) return cudaSuccess;
+  unscale_raw_kernel<<<grid_for(rows * cols, 256, 148 * 16), 256, 0, st>>>(raw, rows, cols, ld, ex, ep);
   ++*nlaunch;
   return cudaGetLastError();
 }

@@ -883,3 +883,57 @@ def test_infer_rp_host_chunks_reuse_staged_operands(hd, h, prec, hv_bits, sim, K
     lab_host2 = h.hdc_infer_rp_host(torch.from_numpy(X).pin_memory(), Pd, dev(C2), kn).numpy()
     assert np.array_equal(lab_host2, lab_dev2)
     assert not np.array_equal(lab_host2, lab_host)
+
+
+# ------------------------------------------------------------------------------------ HDC_FLAG_F32_FAST (2 x fp16 split)
+@pytest.mark.parametrize("flags", [8, 8 | 2, 8 | 4])
+@pytest.mark.parametrize("N,F,D,D_eff", [(200, 64, 2048, 2048), (131, 617, 1000, 999), (300, 100, 700, 33),
+                                         (3, 7, 40, 40), (520, 784, 520, 515)])
+def test_encode_rp_f32_fast_exact_arithmetic(hd, h, flags, N, F, D, D_eff):
+    """Integer features and +-1 projections are exact in the row-scaled half split, so the 3-product
+    contraction must match the oracle bit for bit, raw accumulators (scales undone exactly) included."""
+    r = rng(26, N, F, D_eff)
+    X = r.integers(0, 256, size=(N, F)).astype(np.float32)
+    X[r.random((N, F)) < 0.3] = 0
+    X[0] = 0
+    X[1 % N] *= 2.0 ** -20                                   # a tiny row: its own scale
+    P = (1.0 - 2.0 * r.integers(0, 2, size=(D, F))).astype(np.float32)
+    P[2 % D] *= 2.0 ** 9
+    bits_or, acc_or, _ = O.encode_rp(X, P, D_eff, O.F32)
+    bits, raw, words = _encode(hd, h, X, P, D_eff, hd.HDC_F32, flags)
+    assert np.array_equal(raw.astype(np.float64), acc_or)
+    assert np.array_equal(bits, bits_or)
+    W = (D_eff + 31) // 32
+    if D_eff % 32:
+        assert (words[:, W - 1] >> (D_eff % 32) == 0).all()
+
+
+def test_encode_rp_f32_fast_error_bound_and_sign_band(hd, h):
+    """Gaussian operands with a wide dynamic range inside each row (magnitudes over 2^-24 .. 1): the
+    accumulators are as close to the float64 oracle as the CUDA-core fp32 FFMA kernel's, sign mismatches
+    only inside the fp32 rounding band, and the result passes the same checks as the 6-product path."""
+    r = rng(27)
+    N, F, D = 300, 617, 1500
+    X = (r.standard_normal((N, F)) * np.exp2(-24.0 * r.random((N, F)))).astype(np.float32)
+    P = (r.standard_normal((D, F)) * np.exp2(-10.0 * r.random((D, F)))).astype(np.float32)
+    X[:, 0] = 3.0                                            # one dominant element per row
+    bits_or, acc_or, absum = O.encode_rp(X, P, D, O.F32, want_absum=True)
+    bits, raw, _ = _encode(hd, h, X, P, D, hd.HDC_F32, hd.HDC_FLAG_F32_FAST)
+    err = np.abs(raw - acc_or)
+    # operand truncation is bounded by 3 * 2^-22 * sum|x p|; on top sits the fp32 accumulation error every
+    # fp32 kernel has (here, with one dominant term per row, the larger of the two): hold the fast path to
+    # the CUDA-core FFMA kernel's measured error on the same data
+    _, raw_ffma, _ = _encode(hd, h, X, P, D, hd.HDC_F32, hd.HDC_FLAG_SIMT)
+    ref = (np.abs(raw_ffma - acc_or) / absum).max()
+    assert (err / absum).max() <= 1.5 * ref + 3 * 2.0 ** -22
+    assert (err <= 4 * F * 2.0 ** -24 * absum).all()
+    n = check_sign_band(bits, bits_or, acc_or, absum, F)
+    assert n <= 1e-4 * bits.size
+    # C2-shaped data: same tolerances as test_encode_rp_float_c2_shape
+    w = gen.c2_isolet_shaped(D=1500, n_tr=8, n_te=300)
+    bits_or, acc_or, absum = O.encode_rp(w["Xte"], w["P"], 1500, O.F32, want_absum=True)
+    bits, raw, _ = _encode(hd, h, w["Xte"], w["P"], 1500, hd.HDC_F32, hd.HDC_FLAG_F32_FAST)
+    assert (np.abs(raw - acc_or) <= 1e-3 * np.abs(acc_or) + 1e-6 * absum).all()
+    n = check_sign_band(bits, bits_or, acc_or, absum, 617)
+    assert n <= 1e-4 * bits.size
+    print("f32_fast: max err / absum =", float((np.abs(raw - acc_or) / absum).max()), "sign mismatches", n)
