@@ -123,13 +123,17 @@ __global__ void split2_f16_rows_kernel(const void* __restrict__ src, int src_kin
     const int e = a > 0.0f ? 14 - ilogbf(a) : 0;
     if (lane == 0) expo[r] = e;
     __half* o = dst + r * (int64_t)(2 * seg);
-    for (int c = lane; c < seg; c += 32) {
-      float xs = 0.0f;
-      if (c < cols) xs = scalbnf(load_as_f32(src, src_kind, r * ld_src + c), e);
-      const __half h1 = __float2half_rn(xs);
-      const __half h2 = __float2half_rn(__fsub_rn(xs, __half2float(h1)));
-      o[c] = h1;
-      o[seg + c] = h2;
+    for (int c0 = lane * 8; c0 < seg; c0 += 256) {  // seg is a multiple of 64: whole 16-byte stores
+      __align__(16) __half v1[8], v2[8];
+#pragma unroll
+      for (int j = 0; j < 8; ++j) {
+        float xs = 0.0f;
+        if (c0 + j < cols) xs = scalbnf(load_as_f32(src, src_kind, r * ld_src + c0 + j), e);
+        v1[j] = __float2half_rn(xs);
+        v2[j] = __float2half_rn(__fsub_rn(xs, __half2float(v1[j])));
+      }
+      *reinterpret_cast<uint4*>(o + c0) = *reinterpret_cast<const uint4*>(v1);
+      *reinterpret_cast<uint4*>(o + seg + c0) = *reinterpret_cast<const uint4*>(v2);
     }
   }
 }
