@@ -937,3 +937,19 @@ def test_encode_rp_f32_fast_error_bound_and_sign_band(hd, h):
     n = check_sign_band(bits, bits_or, acc_or, absum, 617)
     assert n <= 1e-4 * bits.size
     print("f32_fast: max err / absum =", float((np.abs(raw - acc_or) / absum).max()), "sign mismatches", n)
+
+
+def test_infer_rp_host_with_f32_fast_flag(hd, h):
+    r = rng(28)
+    N, F, D, K = 40000, 100, 1100, 7
+    X = r.integers(0, 256, size=(N, F)).astype(np.float32)
+    P = (1.0 - 2.0 * r.integers(0, 2, size=(D, F))).astype(np.float32)
+    C = r.integers(-9, 10, size=(K, D)).astype(np.float32)
+    kn = hd.knobs(1000, precision=hd.HDC_F32, hv_bits=8, sim=hd.HDC_SIM_COS, flags=hd.HDC_FLAG_F32_FAST)
+    Pd, Cd = dev(P), dev(C)
+    lab_dev = h.hdc_classify(h.hdc_encode_rp(dev(X), Pd, kn), Cd, kn).cpu().numpy()
+    lab_host = h.hdc_infer_rp_host(torch.from_numpy(X).pin_memory(), Pd, Cd, kn).numpy()
+    assert np.array_equal(lab_host, lab_dev)
+    bits_or, _, _ = O.encode_rp(X[:300], P, 1000, O.F32)
+    lab_or, _, _ = O.classify(O.similarity(bits_or, C, 1000, O.SIM_COS, 8), O.SIM_COS)
+    assert np.array_equal(lab_dev[:300], lab_or)
