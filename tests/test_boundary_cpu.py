@@ -88,3 +88,18 @@ def test_sass_has_tcgen05_tmem_and_tma(libpath):
     assert re.search(r"\bUTC[A-Z]*MMA\b", sass), "no tcgen05.mma (UTC*MMA) in libhdc.so"
     assert "LDTM" in sass, "no tcgen05.ld (LDTM) in libhdc.so"
     assert "UTMALDG" in sass, "no TMA tensor load (UTMALDG) in libhdc.so"
+
+
+def test_binding_structs_match_header_field_for_field():
+    """hdc_knobs_t / hdc_adc_t cross the ABI by value layout: same int32 fields, same order, on both sides."""
+    from paper_2606_26547_b200 import binding
+    import ctypes as C
+    src = open(HEADER).read()
+    for cname, cls in (("hdc_knobs_t", binding.hdc_knobs_t), ("hdc_adc_t", binding.hdc_adc_t)):
+        m = re.search(r"typedef struct \{([^}]*)\}\s*" + cname + r"\s*;", src)
+        assert m, cname
+        body = re.sub(r"/\*.*?\*/", "", m.group(1), flags=re.S)
+        fields = re.findall(r"int32_t\s+(\w+)\s*;", body)
+        assert fields == [f[0] for f in cls._fields_], cname
+        assert all(f[1] is C.c_int32 for f in cls._fields_)
+        assert C.sizeof(cls) == 4 * len(fields)
