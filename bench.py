@@ -304,6 +304,13 @@ def run_gpu(args):
     h.hdc_encode_rp(Xd, Pd, kn_e, Hbits=Hq)                  # leave Hq / labels as the headline path wrote them
     h.hdc_classify(Hq, C, kn, labels=labels)
 
+    # ---- fingerprint of the seeded inputs (a run is reproducible even if the RNG library changes)
+    import hashlib
+    hsh = hashlib.sha256()
+    for a in (w["Xte"], w["yte"], w["Xtr"], w["ytr"], w["P"]):
+        hsh.update(np.ascontiguousarray(a).tobytes())
+    inputs_sha = hsh.hexdigest()[:16]
+
     # ---- single-pass latency at the true test-set size: one encode + classify of the
     # 1559 C2 test queries, device-resident, median of 20 passes
     Xt = dev(w["Xte"])
@@ -346,7 +353,7 @@ def run_gpu(args):
                 "config": {"workload": "C2 ISOLET-shaped: F=617 fp32, K=26, D=10000 fp32 RP encode + cosine + argmax",
                            "queries_per_step_per_gpu": NQ, "l2": "inputs (323 MB/step) larger than L2",
                            "sharding": "queries split across ranks, P and C replicated, no collective",
-                           "test_accuracy": acc},
+                           "test_accuracy": acc, "inputs_sha256": inputs_sha},
                 "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
                 "f32_fast_variant": f32_fast, "latency_true_size": latency,
                 "train": {"samples_per_s": train_sps, "what": "C2 retraining epochs (classify + class update), B=N",
