@@ -213,7 +213,7 @@ int32_t hdc_similarity(hdc_handle_t h, const uint32_t* Hbits, int64_t N, int64_t
  *   adc(p) = floor + step * min( (clamp(p, floor, ceil) - floor + step/2) / step , 2^res - 1 )
  * (integer arithmetic, step/2 and the division rounded down: nearest code, halves up; the paper
  * prints no formula: DESIGN.md reading A19.  floor -127, ceil 128, res 8, step 1 -- the paper's
- * baseline window -- is transparent on [-127, 128]).  1 <= res <= 16, step >= 1, floor <= ceil,
+ * baseline window -- is transparent on [-127, 128]).  1 <= res <= 16, 1 <= step <= 65536, floor <= ceil,
  * |floor|, |ceil| <= 32768; only knobs->D_eff is read.  S (int32 [N][lds], nullable) receives the
  * scores, labels (int32 [N], nullable) the arg-max with ties to the lowest k; at least one of them.
  * Workspace: hdc_workspace_bytes(HDC_OP_SIMILARITY, ...) suffices. */

@@ -785,8 +785,8 @@ extern "C" int32_t hdc_similarity_adc(hdc_handle_t h, const uint32_t* Hbits, int
   int rc = check_knobs(h, knobs, D);
   if (rc) return rc;
   if (ldh_words < words_of(knobs->D_eff)) return fail(h, HDC_ERR_INVALID_ARG, "similarity_adc: ldh_words < W");
-  if (adc->res < 1 || adc->res > 16 || adc->step < 1 || adc->floor > adc->ceil || adc->floor < -32768 ||
-      adc->ceil > 32768)
+  if (adc->res < 1 || adc->res > 16 || adc->step < 1 || adc->step > 65536 || adc->floor > adc->ceil ||
+      adc->floor < -32768 || adc->ceil > 32768)
     return fail(h, HDC_ERR_INVALID_ARG, "similarity_adc: bad ADC window");
   if (!S && !labels && N > 0) return fail(h, HDC_ERR_INVALID_ARG, "similarity_adc: S or labels required");
   if (S && lds < K) return fail(h, HDC_ERR_INVALID_ARG, "similarity_adc: lds < K");

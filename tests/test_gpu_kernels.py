@@ -792,7 +792,8 @@ def test_adc_similarity_argument_errors(hd, h):
     H = torch.zeros((8, 4), dtype=torch.int32, device="cuda")
     Cc = torch.ones((3, 128), dtype=torch.float32, device="cuda")
     before = h.launch_count()
-    for bad in [(0, 1, -3, 128), (17, 1, -3, 128), (8, 0, -3, 128), (8, 1, 5, 4), (8, 1, -40000, 128)]:
+    for bad in [(0, 1, -3, 128), (17, 1, -3, 128), (8, 0, -3, 128), (8, 1, 5, 4), (8, 1, -40000, 128),
+                (8, 65537, -3, 128)]:
         with pytest.raises(hd.HdcError) as ei:
             h.hdc_similarity_adc(H, Cc, hd.knobs(128), *bad)
         assert ei.value.code == hd.HDC_ERR_INVALID_ARG
