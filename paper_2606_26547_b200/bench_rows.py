@@ -253,7 +253,10 @@ def row_c5_stream(h, peaks, reps, hv_bits, sim_name, N=1 << 20, B=65536, F=1024,
 def row_levelid_microhd(h, peaks, reps, N=131072, F=617, Q=128, D=1024):
     """The paper's Micro-HD-Classification reference shape (ISOLET F = 617, D = 1024,
     L = 128 levels): dense uniform levels, rows of 617 bytes (not word-aligned)."""
-    lv = torch.randint(0, Q, (N, F), dtype=torch.uint8, device="cuda", generator=_gen(31))
+    if Q <= 256:
+        lv = torch.randint(0, Q, (N, F), dtype=torch.uint8, device="cuda", generator=_gen(31))
+    else:   # 16-bit level indices (hdc_encode_levelid_u16): L255 tunes the level count up to 814
+        lv = torch.randint(0, Q, (N, F), dtype=torch.int16, device="cuda", generator=_gen(31))
     Wd = (D + 31) // 32
     ID = _rand_bits(F, Wd, 32)
     LV = _rand_bits(Q, Wd, 33)
@@ -409,6 +412,7 @@ ROWS = {
     "c3_levelid": lambda h, p, r: row_levelid(h, p, r),
     "c3_levelid_dense_input": lambda h, p, r: row_levelid(h, p, r, dense_input=True),
     "microhd_levelid": lambda h, p, r: row_levelid_microhd(h, p, r),
+    "microhd_levelid_q814": lambda h, p, r: row_levelid_microhd(h, p, r, Q=814),
     "c3_hamming_k10": lambda h, p, r: row_classify(h, p, r, 131072, 10, 10000, 1, "hamming"),
     "c5_encode_bf16": lambda h, p, r: row_encode(h, p, r, 65536, 1024, 16384, "bf16", x_bf16=True),
     "c5_classify_bf16": lambda h, p, r: row_classify(h, p, r, 65536, 1000, 16384, 16, "cos"),
