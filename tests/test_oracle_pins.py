@@ -419,6 +419,120 @@ def test_train_update_two_rounded_fp32_ops():
         assert Cn[1, d] == np.float32(C[1, d] + np.float32(lr * np.float32(-v)))
 
 
+# ------------------------------------------------------------------ S5 per-tensor int8, by hand
+def test_int8_tensor_rounding_mode_and_scale_by_hand():
+    """quantize_int8_tensor (S5 / A7; "projecting ... onto lower-precision integer
+    types"): ONE scale for the whole array, s = fl32(127 / max|c|), q = rint-to-nearest-EVEN of
+    fl32(c*s).  Worked by hand, non-unit scales, with halves of both parities so that truncation,
+    round-half-up, round-half-away and a per-row scale each fail."""
+    # max|c| = 2  ->  s = 63.5 (exact in fp32)
+    #   2.0*63.5 = 127        -> 127
+    #   1.0*63.5 = 63.5       -> 64   (tie, 64 is even; trunc gives 63)
+    #   0.5*63.5 = 31.75      -> 32   (trunc gives 31)
+    #  -0.75*63.5 = -47.625   -> -48  (trunc gives -47)
+    #   0.0123*63.5 = 0.78..  -> 1    (trunc gives 0)
+    c = np.array([[2.0, 1.0, 0.5, -0.75, 0.0123]], dtype=np.float32)
+    assert o.quantize_int8_tensor(c).tolist() == [[127, 64, 32, -48, 1]]
+    # max|c| = 254 -> s = 0.5 (exact): products are exact halves
+    #   125*0.5 = 62.5 -> 62 (tie to EVEN; half-up and half-away give 63)
+    #   127*0.5 = 63.5 -> 64 (tie to even; trunc gives 63)
+    #  -125*0.5 = -62.5 -> -62 (half-away gives -63);  -127*0.5 = -63.5 -> -64
+    #   -254*0.5 = -127 -> -127 (the negative extreme is -127, never -128);  1*0.5 = 0.5 -> 0;  3*0.5 = 1.5 -> 2
+    c = np.array([[125.0, 127.0, -125.0, -127.0], [-254.0, 1.0, 3.0, 0.0]], dtype=np.float32)
+    assert o.quantize_int8_tensor(c).tolist() == [[62, 64, -62, -64], [-127, 0, 2, 0]]
+    # the scale is per TENSOR: the second row is quantised with the first row's maximum
+    # (a per-row scheme would give [[127, 64], [127, 64]])
+    c = np.array([[2.0, 1.0], [0.5, 0.25]], dtype=np.float32)
+    assert o.quantize_int8_tensor(c).tolist() == [[127, 64], [32, 16]]         # 0.25*63.5 = 15.875 -> 16
+    # the class operand at hv_bits = 8 takes the scale over d < D_eff only (S5): the large entry in the
+    # truncated column must not change it
+    C = np.array([[2.0, 1.0, 1000.0], [0.5, 0.25, -1000.0]], dtype=np.float32)
+    assert o.class_operand(C, 2, 8).tolist() == [[127.0, 64.0], [32.0, 16.0]]
+    # all-zero tensor: scale 1, codes 0
+    assert o.quantize_int8_tensor(np.zeros((2, 3), dtype=np.float32)).tolist() == [[0, 0, 0], [0, 0, 0]]
+
+
+# ------------------------------------------------------------------ S9 mini-batches 1 < B < N, brute force
+def _py_round_half_even(x: float) -> int:
+    return int(round(x))          # python's round() is round-half-to-even on floats
+
+
+def _brute_minibatch_epoch(hb, y, C0, lr, B, hv_bits, sim, epoch_start_model=False, drop_partial=False):
+    """S9 written out with python loops only, sharing nothing with the oracle: for every mini-batch
+    [b0, b0+B) in index order -- including the shorter last one -- (i) re-derive the class operand from
+    the CURRENT accumulators, (ii) predict each sample of the batch against it, (iii) integer Delta over the
+    batch's mispredictions, (iv) C = fl32(C + fl32(lr*Delta)).  The two keyword switches build the MUTANTS
+    the pin has to reject (every batch predicted from the epoch-start model; last partial batch dropped)."""
+    N, D = hb.shape
+    K = C0.shape[0]
+    C = [[np.float32(C0[k, d]) for d in range(D)] for k in range(K)]
+    Cstart = [row[:] for row in C]
+    pred, wrong = [-1] * N, 0
+
+    def operand(Cm):
+        if hv_bits == 32:
+            return [[float(v) for v in row] for row in Cm]
+        amax = max(abs(float(v)) for row in Cm for v in row)
+        s = np.float32(127.0) / np.float32(amax) if amax > 0 else np.float32(1.0)
+        return [[float(max(-127, min(127, _py_round_half_even(float(np.float32(v * s)))))) for v in row] for row in Cm]
+
+    for b0 in range(0, N, B):
+        b1 = min(N, b0 + B)
+        if drop_partial and b1 - b0 < B:
+            break
+        op = operand(Cstart if epoch_start_model else C)
+        nrm = [math.sqrt(sum(c * c for c in op[k])) for k in range(K)]
+        delta = [[0] * D for _ in range(K)]
+        for n in range(b0, b1):
+            v = [1 - 2 * int(hb[n, d]) for d in range(D)]
+            sc = []
+            for k in range(K):
+                t = float(sum(v[d] * op[k][d] for d in range(D)))
+                if sim == o.SIM_COS:
+                    t = t / (math.sqrt(D) * nrm[k]) if nrm[k] > 0 else 0.0
+                sc.append(t)
+            yh = max(range(K), key=lambda k: (sc[k], -k))          # arg-max, ties -> lowest index
+            pred[n] = yh
+            if yh != int(y[n]):
+                wrong += 1
+                for d in range(D):
+                    delta[int(y[n])][d] += v[d]
+                    delta[yh][d] -= v[d]
+        for k in range(K):
+            for d in range(D):
+                C[k][d] = np.float32(C[k][d] + np.float32(np.float32(lr) * np.float32(delta[k][d])))
+    return np.array(C, dtype=np.float32), wrong, pred
+
+
+@pytest.mark.parametrize("hv_bits,sim", [(32, o.SIM_DOT), (32, o.SIM_COS), (8, o.SIM_DOT)])
+def test_train_epoch_minibatches_brute_force(hv_bits, sim):
+    """1 < B < N with B not dividing N (N = 23, B = 5: batches of 5,5,5,5,3), K = 3, D = 40, two epochs,
+    lr = 0.25 (a power of two: no score is decided by a rounding).  Pins S9 step (i) -- the operand is
+    re-derived and the batch re-predicted from the CURRENT accumulators -- and the ragged last batch."""
+    r = rng(61)
+    N, B, K, D = 23, 5, 3, 40
+    protos = r.integers(0, 2, size=(K, D), dtype=np.uint8)
+    y = r.integers(0, K, size=N)
+    hb = protos[y] ^ (r.random((N, D)) < 0.35).astype(np.uint8)
+    C = o.bundle(hb[:6], y[:6], K, D)                    # a weak start so that several batches hold mistakes
+    Cm, Cd = C.copy(), C.copy()
+    differs_start = differs_drop = False
+    for _ in range(2):
+        want_C, want_wrong, want_pred = _brute_minibatch_epoch(hb, y, C, 0.25, B, hv_bits, sim)
+        got_C, got_wrong, got_pred = o.train_epoch(hb, y, C, D, hv_bits, sim, 0.25, B)
+        assert np.array_equal(got_C, want_C) and got_wrong == want_wrong and got_pred.tolist() == want_pred
+        assert want_wrong > 0
+        # the two mutants, built from the same brute force, must be distinguishable on this data --
+        # otherwise the equality above would not pin what it says it pins
+        m_C, m_wrong, m_pred = _brute_minibatch_epoch(hb, y, C, 0.25, B, hv_bits, sim, epoch_start_model=True)
+        differs_start |= (not np.array_equal(m_C, want_C)) or m_pred != want_pred
+        d_C, d_wrong, d_pred = _brute_minibatch_epoch(hb, y, C, 0.25, B, hv_bits, sim, drop_partial=True)
+        differs_drop |= (not np.array_equal(d_C, want_C)) or d_pred != want_pred
+        C = got_C
+    assert differs_start, "data does not separate per-batch re-prediction from the epoch-start model"
+    assert differs_drop, "data does not exercise the ragged last mini-batch"
+
+
 # ------------------------------------------------------------------ end-to-end sanity (not parity)
 def test_pipeline_sanity_c1():
     c = wl.c1_tiny()
