@@ -6,19 +6,28 @@ bundling + 20 retraining epochs (lr 0.05); the 1559-query test set is tiled to 1
 step so that the timed inputs (323 MB) exceed L2.  One step = hdc_encode_rp + hdc_classify over
 that batch, through the C ABI.  Synthetic seeded data (workloads/gen.py) stands in for ISOLET.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--rows]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--rows] [--no-rows]
 
-Prints ONE JSON line (rank 0).  `--impl reference` times the CPU oracle (oracle/hdc_oracle.py, as
-it stands) on the host cores for the same metric / config.  `--rows` adds per-row measurements of
-the other hot-path steps (level-ID encode, Hamming, training, bf16 / int8 precisions).
+`--gpus N` with N > 1 and no torchrun environment re-executes itself as N ranks (one per GPU) under
+`python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1`; launched by
+torchrun it checks WORLD_SIZE == N.  Queries are sharded over the ranks (weak scaling, no collective
+on the inference path); the `train_sharded` block times data-parallel retraining (one int32 all-reduce
+of the class update per mini-batch: paper_2606_26547_b200/shard.py) and checks it against a single-rank
+epoch bit for bit.
+
+Prints ONE JSON line (rank 0).  Besides the headline it carries `rows`: the other hot-path rows
+(bench_rows.DEFAULT_ROWS: bf16 / int8 encode, the C4 precision points, level-ID, Hamming, C5, retraining),
+each with its own SM-clock sample, and -- at N = 1 -- the oracle timed beside them (`rows_cpu_baseline`).
+`--rows` measures every row of bench_rows.ROWS, `--no-rows` none.  `--impl reference` times the CPU oracle
+(oracle/hdc_oracle.py, as it stands) on the host cores for the same metric / config.
 """
 from __future__ import annotations
 
 import argparse
 import json
 import os
+import socket
 import sys
-import threading
 import time
 
 import numpy as np
@@ -29,75 +38,55 @@ if ROOT not in sys.path:
 
 METRIC = "hdc_inference_queries_per_sec_D10000"
 UNIT = "queries/s"
-NQ = 131072            # queries per step (test set tiled)
+NQ = 131072            # queries per step and rank (test set tiled)
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the headline contraction kernel, from the
+# `ncu --set full` capture named beside it (a static figure: ncu cannot run inside the timed bench)
 NCU_TRAFFIC_BYTES = 804.4e6
 NCU_TRAFFIC_SOURCE = "profiles/r1_final_kernels.md (gemm_tc_kernel, fp32-precision encode, 131072 x 617 x 10000)"
 SM_COUNT = 148
 FP32_LANES = 128       # FFMA lanes per SM per clock
+NOMINAL_BF16_TFLOPS = 2250.0   # dense, at sm_max_mhz (guide)
 
 
-def load_peaks():
-    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
-    if os.path.exists(p):
-        with open(p) as f:
-            d = json.load(f)
-        d["_source"] = "measured"
-        return d
-    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0,
-            "sm_max_mhz": 1965.0, "_source": "fallback"}
+# ------------------------------------------------------------------------------------ launcher
+def launcher_command(gpus: int, argv: list, port: int) -> list:
+    """Command line that runs this file as `gpus` ranks, one per GPU, over NCCL (the form the driver uses)."""
+    return [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={int(gpus)}",
+            "--master-addr", "127.0.0.1", "--master-port", str(int(port)), os.path.abspath(__file__)] + list(argv)
 
 
-class ClockSampler:
-    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+def free_port() -> int:
+    with socket.socket(socket.AF_INET, socket.SOCK_STREAM) as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
 
-    def __init__(self, index: int):
-        self.ok = False
-        self.samples, self.reasons = [], set()
-        self._stop = threading.Event()
-        try:
-            import pynvml
-            self.nv = pynvml
-            pynvml.nvmlInit()
-            self.dev = pynvml.nvmlDeviceGetHandleByIndex(index)
-            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self.dev, pynvml.NVML_CLOCK_SM))
-            self.ok = True
-        except Exception:
-            self.max_mhz = None
 
-    def _run(self):
-        nv = self.nv
-        names = {nv.nvmlClocksThrottleReasonSwPowerCap: "sw_power_cap",
-                 nv.nvmlClocksThrottleReasonHwSlowdown: "hw_slowdown",
-                 nv.nvmlClocksThrottleReasonSwThermalSlowdown: "sw_thermal_slowdown",
-                 nv.nvmlClocksThrottleReasonHwThermalSlowdown: "hw_thermal_slowdown",
-                 nv.nvmlClocksThrottleReasonHwPowerBrakeSlowdown: "hw_power_brake"}
-        while not self._stop.is_set():
-            try:
-                self.samples.append(int(nv.nvmlDeviceGetClockInfo(self.dev, nv.NVML_CLOCK_SM)))
-                r = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.dev))
-                for bit, nm in names.items():
-                    if r & bit:
-                        self.reasons.add(nm)
-            except Exception:
-                pass
-            self._stop.wait(0.004)
+def resolve_world(gpus: int, env=os.environ):
+    """(world, rank, local_rank, must_spawn).  Under torchrun WORLD_SIZE must equal --gpus; without it
+    --gpus > 1 asks for a re-exec under the launcher.  Never falls back to fewer ranks than asked."""
+    if gpus < 1:
+        raise SystemExit("bench.py: --gpus must be >= 1")
+    if "WORLD_SIZE" in env:
+        world = int(env["WORLD_SIZE"])
+        if world != gpus:
+            raise SystemExit(f"bench.py: --gpus {gpus} but the launcher started WORLD_SIZE={world} ranks")
+        return world, int(env.get("RANK", "0")), int(env.get("LOCAL_RANK", "0")), False
+    return gpus, 0, 0, gpus > 1
 
-    def __enter__(self):
-        if self.ok:
-            self.t = threading.Thread(target=self._run, daemon=True)
-            self.t.start()
-        return self
 
-    def __exit__(self, *a):
-        if self.ok:
-            self._stop.set()
-            self.t.join()
+def spawn_ranks(args):
+    """Re-exec as args.gpus ranks.  Fails loudly when the box has fewer GPUs (no silent 1-rank run)."""
+    import torch
+    have = torch.cuda.device_count() if torch.cuda.is_available() else 0
+    if have < args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} needs {args.gpus} CUDA devices, this box has {have} "
+                         "(there is no CPU or fewer-rank fallback)")
+    cmd = launcher_command(args.gpus, sys.argv[1:], free_port())
+    sys.stdout.flush()
+    os.execv(cmd[0], cmd)
 
-    def summary(self):
-        if not self.ok or not self.samples:
-            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["nvml unavailable"]}
-        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz,
-                "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+from bench_rows import ClockSampler, load_peaks, sustained_clock_mhz  # noqa: E402  (imports torch)
 
 
 def c2_workload(world: int = 1, rank: int = 0):
@@ -128,7 +117,7 @@ def oracle_model(O, w, n_train=1024):
 
 
 def run_reference(args):
-    rank = int(os.environ.get("RANK", "0"))
+    world, rank, _, _ = resolve_world(args.gpus) if "WORLD_SIZE" in os.environ else (1, 0, 0, False)
     if rank != 0:
         return
     from oracle import hdc_oracle as O
@@ -144,12 +133,12 @@ def run_reference(args):
     dt = time.perf_counter() - t0
     val = sample * args.steps / dt
     cores = os.cpu_count()
-    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": world,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
             "data": "synthetic",
             "config": {"workload": "C2 ISOLET-shaped: F=617 fp32, K=26, D=10000 RP encode + cosine + argmax",
-                       "queries_per_step": sample, "timing": "host wall clock"},
+                       "queries_per_step": sample, "timing": "host wall clock; rank 0 only, no GPU is used"},
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle",
                              "sample": f"{sample} queries of the tiled C2 test set per step"},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -158,16 +147,59 @@ def run_reference(args):
 
 
 # ------------------------------------------------------------------------------------ own arm
+def train_sharded_block(h, hd, shard, dist, world, rank, local, w, Htr, ytr, kn, epochs):
+    """Data-parallel retraining: every mini-batch (B = N here) is split over the ranks,
+    each rank computes the int32 class update of its shard (hdc_train_delta), ONE all-reduce(sum) per
+    mini-batch (NCCL when world > 1) hands every rank the same integers, hdc_train_apply performs the
+    identical fp32 update.  Checked bit for bit against hdc_train_epoch run by this rank alone."""
+    import torch
+    K, D = w["K"], w["D"]
+    N = Htr.shape[0]
+    C0 = torch.zeros((K, D), dtype=torch.float32, device="cuda")
+    h.hdc_train_epoch(hd.HDC_TRAIN_BUNDLE, Htr, ytr, C0, kn)
+    C_single = C0.clone()
+    for _ in range(epochs):
+        h.hdc_train_epoch(hd.HDC_TRAIN_PERCEPTRON, Htr, ytr, C_single, kn, lr=w["lr"], batch=0)
+    C = C0.clone()
+    delta = torch.empty((K, ((D + 31) // 32) * 32), dtype=torch.int32, device="cuda")
+    delta_fn = lambda lo, hi: h.hdc_train_delta(Htr[lo:hi], ytr[lo:hi], C, kn, delta=delta)   # noqa: E731
+    apply_fn = lambda d: h.hdc_train_apply(C, kn, d, w["lr"])                                    # noqa: E731
+    shard.train_epoch_sharded(delta_fn, apply_fn, N, 0)            # warm-up epoch (NCCL communicator, workspaces)
+    C.copy_(C0)
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    ev[0].record()
+    for _ in range(epochs):
+        shard.train_epoch_sharded(delta_fn, apply_fn, N, 0)
+    ev[1].record()
+    torch.cuda.synchronize()
+    ms = shard.max_over_ranks(ev[0].elapsed_time(ev[1]), torch.device("cuda", local))
+    same = bool(torch.equal(C, C_single))
+    if world > 1:
+        flag = torch.tensor([1 if same else 0], device="cuda")
+        dist.all_reduce(flag, op=dist.ReduceOp.MIN)
+        same = bool(flag.item())
+    if not same:
+        raise RuntimeError("sharded retraining differs from the single-rank epochs (replicas must be bit-identical)")
+    return {"samples_per_s": epochs * N / (ms * 1e-3), "ms": ms, "epochs": epochs, "ranks": world,
+            "scaling": "strong (the 6238 C2 training samples are split over the ranks)",
+            "collective": "none (1 rank)" if world == 1 else "all_reduce(sum) of int32 Delta[K x D] per mini-batch, NCCL",
+            "bit_identical_to_single_rank": same,
+            "what": "C2 retraining epochs as hdc_train_delta -> all-reduce -> hdc_train_apply, B = N"}
+
+
 def run_gpu(args):
+    world, rank, local, must_spawn = resolve_world(args.gpus)
+    if must_spawn:
+        spawn_ranks(args)          # does not return
     import torch
     import torch.distributed as dist
 
     import paper_2606_26547_b200 as hd
     from paper_2606_26547_b200 import shard
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a CUDA device (there is no CPU fallback)")
     torch.cuda.set_device(local)
@@ -179,11 +211,12 @@ def run_gpu(args):
 
     w, Xq = c2_workload(world, rank)
     D, K, F = w["D"], w["K"], w["F"]
+    Fp = -(-F // 64) * 64            # reduction axis as staged (k-blocks of 64 bf16)
     Pd = dev(w["P"])
     kn_e = hd.knobs(D, precision=hd.HDC_F32)
     kn = hd.knobs(D, precision=hd.HDC_F32, hv_bits=32, sim=hd.HDC_SIM_COS)
 
-    # ---- model: encode train, bundle, 20 retraining epochs (setup; also timed as training rows)
+    # ---- model: encode train, bundle, 20 retraining epochs (setup; warm epochs are timed afterwards)
     Xtr, ytr = dev(w["Xtr"]), dev(w["ytr"])
     Htr = h.hdc_encode_rp(Xtr, Pd, kn_e)
     C = torch.zeros((K, D), dtype=torch.float32, device="cuda")
@@ -195,8 +228,16 @@ def run_gpu(args):
         h.hdc_train_epoch(hd.HDC_TRAIN_PERCEPTRON, Htr, ytr, C, kn, lr=w["lr"], batch=0)
     ev[1].record()
     torch.cuda.synchronize()
+    train_cold_ms = ev[0].elapsed_time(ev[1])
+    Cw = C.clone()                                       # the same epochs again, warm (model already converged)
+    ev[0].record()
+    for _ in range(w["epochs"]):
+        h.hdc_train_epoch(hd.HDC_TRAIN_PERCEPTRON, Htr, ytr, Cw, kn, lr=w["lr"], batch=0)
+    ev[1].record()
+    torch.cuda.synchronize()
     train_ms = ev[0].elapsed_time(ev[1])
     train_sps = w["epochs"] * Xtr.shape[0] / (train_ms * 1e-3)
+    del Cw
 
     # ---- timed inference steps (device-resident inputs)
     Xd = dev(Xq)
@@ -235,9 +276,10 @@ def run_gpu(args):
     # re-run of the timed steps (sustained regime) and (b) alone, back to back (burst regime).
     h.kernel_timing(True)
     torch.cuda.synchronize()
-    for _ in range(args.steps):
-        step()
-    torch.cuda.synchronize()
+    with ClockSampler(local) as cs_k:
+        for _ in range(args.steps):
+            step()
+        torch.cuda.synchronize()
     enc_ms_tot, enc_n = h.kernel_time(hd.HDC_K_ENCODE_GEMM)
     sim_ms_tot, sim_n = h.kernel_time(hd.HDC_K_SIM)
     enc_ms = enc_ms_tot / max(1, enc_n)
@@ -258,25 +300,42 @@ def run_gpu(args):
     achieved = flops / (enc_ms * 1e-3) / 1e12
     peak = peaks["bf16_tflops_sustained"] / 6.0
     clocks = cs.summary()
+    clk_k = cs_k.summary()
+    # the same fraction against the peak RESCALED to the SM clock sampled while the kernel ran:
+    # (a) the measured sustained cuBLAS rate per MHz of the clock it was measured at, (b) the nominal dense rate
+    f_k = clk_k.get("sm_mhz") or clocks.get("sm_mhz")
+    rescaled = None
+    if f_k:
+        pk_meas = peaks["bf16_tflops_sustained"] * f_k / sustained_clock_mhz(peaks) / 6.0
+        pk_nom = NOMINAL_BF16_TFLOPS * f_k / peaks["sm_max_mhz"] / 6.0
+        rescaled = {"sm_mhz_during_kernel_pass": f_k,
+                    "peak_measured_rate_at_this_clock": pk_meas, "frac_of_measured_rate_at_this_clock": achieved / pk_meas,
+                    "peak_nominal_at_this_clock": pk_nom, "frac_of_nominal_at_this_clock": achieved / pk_nom,
+                    "how": "bf16_tflops_sustained x sm_mhz / (clock the driver measured it at) / 6; "
+                           "2250 TFLOP/s nominal dense x sm_mhz / sm_max_mhz / 6"}
     roofline = {"bound": "tensor",
                 "kernel": "gemm_tc_kernel<bf16,EPI_SIGN,cta_group::2> (tcgen05 fp32-precision encode on CTA pairs: 6 "
                           "bf16 segment products per MAC over 3-way split operands, sign+pack epilogue)",
                 "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
                 "peak_source": f"bf16_tflops_sustained / 6 ({peaks['_source']} MEASURED_PEAKS.json; kernel timed "
                                "inside the step loop)",
+                "frac_of_burst_peak": achieved / (peaks["bf16_tflops"] / 6.0),
+                "clock_rescaled": rescaled,
                 "algorithmic_flops_per_launch": flops, "ms_per_launch": enc_ms,
-                "executed_bf16_tflops": 6.0 * 2.0 * NQ * 640 * D / (enc_ms * 1e-3) / 1e12,
+                "executed_bf16_tflops": 6.0 * 2.0 * NQ * Fp * D / (enc_ms * 1e-3) / 1e12,
                 "alone": {"ms_per_launch": enc_alone_ms, "achieved": flops / (enc_alone_ms * 1e-3) / 1e12,
                           "peak": peaks["bf16_tflops"] / 6.0,
                           "frac": flops / (enc_alone_ms * 1e-3) / 1e12 / (peaks["bf16_tflops"] / 6.0),
                           "peak_source": "bf16_tflops (burst) / 6"},
                 "encode_call_ms": enc_call_ms, "classify_kernel_ms": cls_ms,
+                "later_passes": "ms_per_launch and classify_kernel_ms come from a second pass over the same steps with "
+                                "the library's per-kernel events on, encode_call_ms and `alone` from a third pass of "
+                                "encode calls only; each ran after the timed region, at the clocks the part had then, "
+                                "so they need not add up to ms_per_step",
                 "share_of_step": enc_ms / (ms / args.steps),
                 "fp32_alu_peak_tflops": SM_COUNT * FP32_LANES * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12,
-                # dram__bytes_read.sum + dram__bytes_write.sum of this kernel at this shape, one launch, from
-                # the ncu --set full capture summarised in profiles/ (bytes)
                 "traffic": NCU_TRAFFIC_BYTES, "traffic_source": NCU_TRAFFIC_SOURCE,
-                "algorithmic_bytes_per_launch": float(NQ) * 3 * 640 * 2 + float(D) * 3 * 640 * 2 + float(NQ) * W * 4}
+                "algorithmic_bytes_per_launch": float(NQ) * 3 * Fp * 2 + float(D) * 3 * Fp * 2 + float(NQ) * W * 4}
 
     # ---- NOT the headline: the same step with the opt-in HDC_FLAG_F32_FAST encode (fp32 operands as 2-way
     # IEEE-half splits, 22 mantissa bits, three tensor-core products instead of six).  Reported beside the
@@ -328,22 +387,24 @@ def run_gpu(args):
     latency = {"queries": int(n_te), "ms_median": float(np.median(lat)), "ms_best": float(min(lat))}
 
     # ---- end to end through the host entry point (pinned host buffers, H2D + D2H inside)
-    e2e = None
-    if rank == 0 or world > 1:
-        Xh = torch.from_numpy(Xq).pin_memory()
-        Lh = torch.empty(NQ, dtype=torch.int32).pin_memory()
-        h.hdc_infer_rp_host(Xh, Pd, C, kn, labels_host=Lh)
-        torch.cuda.synchronize()
-        if world > 1:
-            dist.barrier()
-        t0 = time.perf_counter()
-        for _ in range(args.steps):
-            h.hdc_infer_rp_host(Xh, Pd, C, kn, labels_host=Lh)      # synchronises before returning
-        dt = time.perf_counter() - t0
-        dt = shard.max_over_ranks(dt, torch.device("cuda", local))
-        assert np.array_equal(Lh.numpy(), labels.cpu().numpy()), "e2e labels differ from the device path"
-        e2e = {"value": world * NQ * args.steps / dt, "unit": UNIT, "h2d_bytes_per_step": int(Xh.numel() * 4),
-               "d2h_bytes_per_step": int(NQ * 4), "api": "hdc_infer_rp_host"}
+    Xh = torch.from_numpy(Xq).pin_memory()
+    Lh = torch.empty(NQ, dtype=torch.int32).pin_memory()
+    h.hdc_infer_rp_host(Xh, Pd, C, kn, labels_host=Lh)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        h.hdc_infer_rp_host(Xh, Pd, C, kn, labels_host=Lh)      # synchronises before returning
+    dt = time.perf_counter() - t0
+    dt = shard.max_over_ranks(dt, torch.device("cuda", local))
+    assert np.array_equal(Lh.numpy(), labels.cpu().numpy()), "e2e labels differ from the device path"
+    e2e = {"value": world * NQ * args.steps / dt, "unit": UNIT, "h2d_bytes_per_step": int(world * Xh.numel() * 4),
+           "d2h_bytes_per_step": int(world * NQ * 4), "api": "hdc_infer_rp_host"}
+    del Xh, Lh
+
+    # ---- data-parallel retraining (every N; NCCL all-reduce when N > 1)
+    train_sharded = train_sharded_block(h, hd, shard, dist, world, rank, local, w, Htr, ytr, kn, w["epochs"])
 
     line = None
     if rank == 0:
@@ -356,13 +417,23 @@ def run_gpu(args):
                            "test_accuracy": acc, "inputs_sha256": inputs_sha},
                 "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
                 "f32_fast_variant": f32_fast, "latency_true_size": latency,
-                "train": {"samples_per_s": train_sps, "what": "C2 retraining epochs (classify + class update), B=N",
-                          "epochs": w["epochs"], "ms": train_ms}}
-        if world == 1:
-            line["cpu_baseline"] = cpu_baseline(w, Xq)
-        if args.rows and world == 1:
-            from paper_2606_26547_b200 import bench_rows
-            line["rows"] = bench_rows.run(h, peaks)
+                "train": {"samples_per_s": train_sps, "what": "C2 retraining epochs (classify + class update), B=N, "
+                          "warm (second run of the 20 epochs)", "epochs": w["epochs"], "ms": train_ms,
+                          "first_run_ms": train_cold_ms},
+                "train_sharded": train_sharded}
+    # ---- the other hot-path rows, each with its own clock sample (rank 0's GPU; N = 1 only: they are 1-GPU rows)
+    if rank == 0 and world == 1 and not args.no_rows:
+        import bench_rows
+        del Xd, Hq, Xt, Ht
+        torch.cuda.empty_cache()
+        t0 = time.perf_counter()
+        line["rows"] = bench_rows.run(h, peaks, reps=5, only=None if args.rows else bench_rows.DEFAULT_ROWS)
+        line["rows_wall_s"] = round(time.perf_counter() - t0, 1)
+        line["cpu_baseline"] = cpu_baseline(w, Xq)
+        line["rows_cpu_baseline"] = rows_cpu_baseline(w)
+    elif rank == 0 and world == 1:
+        line["cpu_baseline"] = cpu_baseline(w, Xq)
+    if rank == 0:
         print(json.dumps(line), flush=True)
     if world > 1:
         dist.barrier()
@@ -384,13 +455,72 @@ def cpu_baseline(w, Xq):
             "sample": f"{sample} queries of the tiled C2 test set (encode + cosine + argmax), {dt:.1f} s"}
 
 
+def rows_cpu_baseline(w):
+    """The oracle, as it stands, timed on the host cores beside the rows of `rows` (north_star: "absolute
+    queries/sec and training samples/sec ... beside the oracle timed on the box's host cores in the same
+    run"): bounded samples, wall clock, each labelled; a baseline, not a target."""
+    from oracle import hdc_oracle as O
+    from workloads import gen
+    cores = os.cpu_count()
+    out = {}
+
+    def timed(fn):
+        t0 = time.perf_counter()
+        r = fn()
+        return r, time.perf_counter() - t0
+
+    # retraining epoch, C2 (train set encoded by the oracle first; one epoch B = N timed)
+    n_tr = w["Xtr"].shape[0]
+    btr, _, _ = O.encode_rp(w["Xtr"][:n_tr], w["P"], w["D"], O.F32)
+    C = O.bundle(btr, w["ytr"][:n_tr], w["K"], w["D"])
+    _, dt = timed(lambda: O.train_epoch(btr, w["ytr"][:n_tr], C, w["D"], 32, O.SIM_COS, w["lr"], 0))
+    out["c2_train_epoch"] = {"value": n_tr / dt, "unit": "samples/s", "cores": cores, "kind": "oracle",
+                             "sample": f"one retraining epoch (B=N) over the {n_tr} C2 training samples (pre-encoded), {dt:.2f} s"}
+    # level-ID encode, C3
+    c3 = gen.c3_mnist_shaped(n_tr=16, n_te=256)
+    hb3, dt = timed(lambda: O.encode_levelid(c3["Lte"], c3["ID"], c3["LV"], c3["D"]))
+    out["c3_levelid"] = {"value": 256 / dt, "unit": "samples/s", "cores": cores, "kind": "oracle",
+                         "sample": f"256 C3-shaped images (F=784, Q=256, D=10000), {dt:.2f} s; the oracle loops over "
+                                   "samples in python: one core"}
+    # Hamming similarity + arg-min, C3 shape (K = 10)
+    C3 = O.bundle(hb3, c3["yte"], c3["K"], c3["D"])
+    reps = 16
+    q = np.concatenate([hb3] * reps, axis=0)
+    _, dt = timed(lambda: O.infer(q, C3, c3["D"], O.SIM_HAMMING, 1))
+    out["c3_hamming_k10"] = {"value": q.shape[0] / dt, "unit": "queries/s", "cores": cores, "kind": "oracle",
+                             "sample": f"{q.shape[0]} encoded C3 queries (256 tiled x{reps}) against K=10, {dt:.2f} s"}
+    out["c3_pipeline"] = {"value": 1.0 / (1.0 / out["c3_levelid"]["value"] + 1.0 / out["c3_hamming_k10"]["value"]),
+                          "unit": "queries/s", "cores": cores, "kind": "oracle",
+                          "sample": "harmonic combination of the two rows above (same samples)"}
+    # C5: the SURVEY 8(d) subsample -- first 4096 queries of batch 0 + 64 of each remaining batch = 5056 queries
+    c5 = gen.c5_large_batch(4096, batch=0)
+    X5 = np.concatenate([c5["X"]] + [gen.c5_large_batch(64, batch=i, per_class=1)["X"] for i in range(1, 16)], axis=0)
+    btr5, _, _ = O.encode_rp(c5["Xtr"], c5["P"], c5["D"], O.BF16)
+    C5 = O.bundle(btr5, c5["ytr"], c5["K"], c5["D"])
+    (hb5, _, _), dt_e = timed(lambda: O.encode_rp(X5, c5["P"], c5["D"], O.BF16))
+    _, dt_c = timed(lambda: O.infer(hb5, C5, c5["D"], O.SIM_COS, 16))
+    n5h = 512                        # the oracle's Hamming loops over the 1000 classes: a smaller sample
+    _, dt_h = timed(lambda: O.infer(hb5[:n5h], C5, c5["D"], O.SIM_HAMMING, 1))
+    dt_h *= X5.shape[0] / n5h
+    n5 = X5.shape[0]
+    out["c5_stream_bf16"] = {"value": n5 / (dt_e + dt_c), "unit": "queries/s", "cores": cores, "kind": "oracle",
+                             "sample": f"{n5}-query subsample (4096 of batch 0 + 64 of each other batch): encode {dt_e:.1f} s "
+                                       f"+ bf16 cosine classify {dt_c:.1f} s; extrapolated linearly to 2^20 queries: "
+                                       f"{(dt_e + dt_c) * (1 << 20) / n5:.0f} s"}
+    out["c5_stream_1bit"] = {"value": n5 / (dt_e + dt_h), "unit": "queries/s", "cores": cores, "kind": "oracle",
+                             "sample": f"same subsample: encode {dt_e:.1f} s + Hamming classify {dt_h:.1f} s (timed on its first {n5h} queries, scaled); extrapolated "
+                                       f"linearly to 2^20 queries: {(dt_e + dt_h) * (1 << 20) / n5:.0f} s"}
+    return out
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="own", choices=["own", "reference"])
-    ap.add_argument("--rows", action="store_true", help="also measure the other hot-path rows")
+    ap.add_argument("--rows", action="store_true", help="measure every row of bench_rows.ROWS (default: DEFAULT_ROWS)")
+    ap.add_argument("--no-rows", action="store_true", help="headline only")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
