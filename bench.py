@@ -242,7 +242,7 @@ def run_gpu(args):
     # ---- timed inference steps (device-resident inputs)
     Xd = dev(Xq)
     W = (D + 31) // 32
-    Hq = torch.empty((NQ, W), dtype=torch.int32, device="cuda")
+    Hq = h.alloc_hbits(NQ, D)
     labels = torch.empty(NQ, dtype=torch.int32, device="cuda")
 
     def step():
@@ -373,7 +373,7 @@ def run_gpu(args):
     # ---- single-pass latency at the true test-set size: one encode + classify of the
     # 1559 C2 test queries, device-resident, median of 20 passes
     Xt = dev(w["Xte"])
-    Ht = torch.empty((n_te, W), dtype=torch.int32, device="cuda")
+    Ht = h.alloc_hbits(n_te, D)
     lt = torch.empty(n_te, dtype=torch.int32, device="cuda")
     lat = []
     for i in range(23):

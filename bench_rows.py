@@ -180,7 +180,7 @@ def row_encode(h, peaks, reps, cfg, N, prec_name):
         X, P = _dev(gen.tile_rows(w["Xte"], N)), _dev(w["P"])
     F, D = X.shape[1], P.shape[0]
     kn = hd.knobs(D, precision=prec, flags=flags)
-    H = torch.empty((N, (D + 31) // 32), dtype=torch.int32, device="cuda")
+    H = h.alloc_hbits(N, D)
     fn = lambda: h.hdc_encode_rp(X, P, kn, Hbits=H)  # noqa: E731
     call_ms = _time(fn, reps)
     k_ms, _ = _kernel(h, hd.HDC_K_ENCODE_GEMM, fn, reps)
@@ -207,7 +207,7 @@ def row_point(h, peaks, reps, cfg, N, prec_name):
     Htr = h.hdc_encode_rp(_dev(w["Xtr"]), P, kn_e)
     C = torch.zeros((K, D), dtype=torch.float32, device="cuda")
     h.hdc_train_epoch(hd.HDC_TRAIN_BUNDLE, Htr, _dev(w["ytr"]), C, kn)
-    H = torch.empty((N, (D + 31) // 32), dtype=torch.int32, device="cuda")
+    H = h.alloc_hbits(N, D)
     lab = torch.empty(N, dtype=torch.int32, device="cuda")
 
     def fn():
@@ -293,7 +293,7 @@ def row_levelid(h, peaks, reps, N=65536, F=784, Q=256, D=10000, dense_input=Fals
         lv = _dev(gen.rng_for(3, "rows_dense_levels").integers(0, Q, size=(N, F), dtype=np.uint8))
     ID, LV = _bits(w["ID"]), _bits(w["LV"])
     Wd = (D + 31) // 32
-    H = torch.empty((N, Wd), dtype=torch.int32, device="cuda")
+    H = h.alloc_hbits(N, D)
     kn = hd.knobs(D)
     fn = lambda: h.hdc_encode_levelid(lv, ID, LV, D, kn, Hbits=H)  # noqa: E731
     call_ms = _time(fn, reps)
@@ -375,7 +375,7 @@ def row_c5_stream(h, peaks, reps, hv_bits, sim_name, N=1 << 20, B=65536, F=1024,
     Xs, P, C, y0 = _c5_setup(h, 4, B, D, K, F)
     kn_e = hd.knobs(D, precision=hd.HDC_BF16)
     kn = hd.knobs(D, hv_bits=hv_bits, sim=sim)
-    H = torch.empty((B, (D + 31) // 32), dtype=torch.int32, device="cuda")
+    H = h.alloc_hbits(B, D)
     lab = torch.empty(N, dtype=torch.int32, device="cuda")
 
     def fn():
@@ -434,7 +434,7 @@ def row_levelid_microhd(h, peaks, reps, N=131072, F=617, Q=128, D=1024):
     lv = _dev(lv)    # Q > 256: 16-bit level indices (hdc_encode_levelid_u16): L255 tunes the level count up to 814
     Wd = (D + 31) // 32
     ID, LV = _bits(gen.id_table(0, F, D)), _bits(gen.level_table(0, Q, D))
-    H = torch.empty((N, Wd), dtype=torch.int32, device="cuda")
+    H = h.alloc_hbits(N, D)
     kn = hd.knobs(D)
     fn = lambda: h.hdc_encode_levelid(lv, ID, LV, D, kn, Hbits=H)  # noqa: E731
     call_ms = _time(fn, reps)
@@ -452,7 +452,7 @@ def row_c3_pipeline(h, peaks, reps, N=65536, F=784, Q=256, D=10000, K=10):
     w = gen.c3_mnist_shaped(D=D, n_tr=16, n_te=4096, Q=Q)
     lv = _dev(gen.tile_rows(w["Lte"], N))
     ID, LV = _bits(w["ID"]), _bits(w["LV"])
-    H = torch.empty((N, (D + 31) // 32), dtype=torch.int32, device="cuda")
+    H = h.alloc_hbits(N, D)
     C = _class_acc(K, D, "rows_class_acc")
     lab = torch.empty(N, dtype=torch.int32, device="cuda")
     kn_e, kn = hd.knobs(D), hd.knobs(D, hv_bits=1, sim=hd.HDC_SIM_HAMMING)
@@ -504,7 +504,7 @@ def c4_sweep(h, peaks, reps=5, NQ=131072):
             Ct = C.clone()
             ep_ms = _time(lambda: h.hdc_train_epoch(hd.HDC_TRAIN_PERCEPTRON, Htr, ytr, Ct, kn, lr=w["lr"], batch=0),
                           reps)
-            Hq = torch.empty((NQ, (D_eff + 31) // 32), dtype=torch.int32, device="cuda")
+            Hq = h.alloc_hbits(NQ, D_eff)
             lab_q = torch.empty(NQ, dtype=torch.int32, device="cuda")
 
             def infer():

@@ -182,6 +182,13 @@ class Handle:
             self._ws = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
         return C.c_void_p(self._ws.data_ptr()), self._ws.numel()
 
+    def alloc_hbits(self, N: int, D_eff: int) -> torch.Tensor:
+        """[N][W] int32 view of packed-hypervector rows whose stride is W rounded up to 4 words: 16-byte
+        aligned rows let the encode epilogue write one 16-byte store per thread (include/hdc.h: ldh_words)."""
+        W = (int(D_eff) + 31) // 32
+        ld = (W + 3) // 4 * 4
+        return torch.empty((int(N), ld), dtype=torch.int32, device=self.device)[:, :W]
+
     @staticmethod
     def _stream():
         return C.c_void_p(torch.cuda.current_stream().cuda_stream)
@@ -192,7 +199,7 @@ class Handle:
         D = P.shape[0]
         W = (kn.D_eff + 31) // 32
         if Hbits is None:
-            Hbits = torch.empty((N, W), dtype=torch.int32, device=self.device)
+            Hbits = self.alloc_hbits(N, kn.D_eff)
         Hraw = None
         if want_raw:
             Hraw = torch.empty((N, kn.D_eff), device=self.device,
@@ -213,7 +220,7 @@ class Handle:
         Q = LVbits.shape[0]
         W = (kn.D_eff + 31) // 32
         if Hbits is None:
-            Hbits = torch.empty((N, W), dtype=torch.int32, device=self.device)
+            Hbits = self.alloc_hbits(N, kn.D_eff)
         if levels.dtype not in (torch.uint8, torch.int16, torch.uint16):
             raise TypeError("levels must be uint8, or int16 / uint16 (16-bit indices)")
         fn = self._L.hdc_encode_levelid if levels.dtype == torch.uint8 else self._L.hdc_encode_levelid_u16

@@ -99,6 +99,7 @@ struct TcParams {
   int seg_stride;               // elements between operand segments
   int group_m;                  // m-tiles per rasterisation group (EPI_SIGN / EPI_SCORE)
   int f16;                      // 16-bit operands are IEEE half instead of bf16
+  int bits_vec4;                // EPI_SIGN: rows of e.bits are 16-byte aligned (base and ldbits % 4 == 0)
   Epilogue e;
 };
 
@@ -286,36 +287,58 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
         // column first, so column j lands in bit j); for floats x + (+0.0) first turns -0.0 into
         // +0.0 (reading A1: sgn(-0.0) = +1) on the FMA pipe, leaving the ALU pipe one op per value.
         uint32_t va[32], vb[32];
-        auto pack_store = [&](const uint32_t (&v)[32], int c) {
-          uint32_t word = 0;
+        uint32_t words[4] = {0u, 0u, 0u, 0u};   // this warp's (up to) four packed words of the row
+        auto pack = [&](const uint32_t (&v)[32], int c) -> uint32_t {
+          // four independent funnel-shift chains of eight (a single chain of 32 dependent shifts made the
+          // epilogue latency, not its instruction count, the pace of short-reduction tiles)
+          uint32_t w4[4] = {0u, 0u, 0u, 0u};
 #pragma unroll
-          for (int j = 31; j >= 0; --j) {
-            const uint32_t u = INT8 ? v[j] : __float_as_uint(__fadd_rn(__uint_as_float(v[j]), 0.0f));
-            word = __funnelshift_l(u, word, 1);
-          }
-          const int valid = n_valid - c * 32;  // >= 1
-          if (valid < 32) word &= (1u << valid) - 1u;
-          if (row_ok) {
-            p.e.bits[row * p.e.ldbits + (n0 >> 5) + c] = word;
-            if (p.e.raw) {
-              uint32_t* out = reinterpret_cast<uint32_t*>(p.e.raw) + row * p.e.ldraw + n0 + c * 32;
+          for (int j = 7; j >= 0; --j) {
 #pragma unroll
-              for (int j = 0; j < 32; ++j)
-                if (j < valid) out[j] = v[j];
+            for (int g = 0; g < 4; ++g) {
+              const uint32_t x = v[8 * g + j];
+              const uint32_t u = INT8 ? x : __float_as_uint(__fadd_rn(__uint_as_float(x), 0.0f));
+              w4[g] = __funnelshift_l(u, w4[g], 1);
             }
           }
+          uint32_t word = (w4[0] | (w4[1] << 8)) | ((w4[2] << 16) | (w4[3] << 24));
+          const int valid = n_valid - c * 32;  // >= 1
+          if (valid < 32) word &= (1u << valid) - 1u;
+          if (row_ok && p.e.raw) {
+            uint32_t* out = reinterpret_cast<uint32_t*>(p.e.raw) + row * p.e.ldraw + n0 + c * 32;
+#pragma unroll
+            for (int j = 0; j < 32; ++j)
+              if (j < valid) out[j] = v[j];
+          }
+          return word;
         };
         const int c_begin = ehalf * 4;
         const int c_end = nchunks < c_begin + 4 ? nchunks : c_begin + 4;
-        if (c_begin < c_end) tmem_ld32(taddr + (uint32_t)(c_begin * 32), va);
-        for (int c = c_begin; c < c_end; c += 2) {
-          tmem_ld_wait();
-          if (c + 1 < c_end) tmem_ld32(taddr + (uint32_t)((c + 1) * 32), vb);
-          pack_store(va, c);
-          if (c + 1 < c_end) {
+        const int nleft = c_end - c_begin;   // 0..4 chunks for this warp
+        if (nleft > 0) tmem_ld32(taddr + (uint32_t)(c_begin * 32), va);
+#pragma unroll
+        for (int i = 0; i < 4; i += 2) {
+          if (i < nleft) {
             tmem_ld_wait();
-            if (c + 2 < c_end) tmem_ld32(taddr + (uint32_t)((c + 2) * 32), va);
-            pack_store(vb, c + 1);
+            if (i + 1 < nleft) tmem_ld32(taddr + (uint32_t)((c_begin + i + 1) * 32), vb);
+            words[i] = pack(va, c_begin + i);
+            if (i + 1 < nleft) {
+              tmem_ld_wait();
+              if (i + 2 < nleft) tmem_ld32(taddr + (uint32_t)((c_begin + i + 2) * 32), va);
+              words[i + 1] = pack(vb, c_begin + i + 1);
+            }
+          }
+        }
+        // one 16-byte store per thread when the row segment is aligned and complete (each warp of a lane
+        // quadrant writes half of the row's 32-byte sector of this tile), else word by word
+        if (row_ok && c_begin < c_end) {
+          uint32_t* dst = p.e.bits + row * p.e.ldbits + (n0 >> 5) + c_begin;
+          if (c_end - c_begin == 4 && p.bits_vec4) {
+            *reinterpret_cast<uint4*>(dst) = make_uint4(words[0], words[1], words[2], words[3]);
+          } else {
+#pragma unroll
+            for (int c = 0; c < 4; ++c)
+              if (c_begin + c < c_end) dst[c] = words[c];
           }
         }
       }
@@ -362,7 +385,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
       tc_fence_before();
       __syncwarp();
       if (lane == 0) {
-        if (CG == 2) mbar_arrive_cluster(tempty_bar(acc) & PEER_MASK);  // the leader's barrier
+        if (CG == 2) mbar_arrive_cluster_relaxed(tempty_bar(acc) & PEER_MASK);  // the leader's barrier
         else mbar_arrive(tempty_bar(acc));
       }
       if (++acc == 2) {
@@ -472,6 +495,7 @@ cudaError_t launch_gemm_tc(TcContext* tc, const TcOperands& o, int64_t M, int Nc
   p.seg_stride = o.seg_stride;
   p.group_m = 16 / cg;
   p.f16 = o.elem_kind == OPK_F16;
+  p.bits_vec4 = e.kind == EPI_SIGN && (reinterpret_cast<uintptr_t>(e.bits) & 15) == 0 && (e.ldbits & 3) == 0;
   p.e = e;
   CUtensorMap tmA, tmB;
   if (!tc_make_map(tc, &tmA, o.A, int8, M, o.cols_a, o.lda, BM)) return cudaErrorInvalidValue;

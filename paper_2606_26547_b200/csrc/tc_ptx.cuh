@@ -87,6 +87,14 @@ __device__ __forceinline__ void cluster_sync_all() {
 __device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_addr) {
   asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
 }
+// Same without memory ordering.  For hand-offs that publish no generic-proxy memory: an epilogue warp
+// returning a TMEM accumulator has already waited for its tcgen05.ld (tcgen05.wait::ld) and fenced the
+// tensor proxy (tcgen05.fence::before_thread_sync).  The .release.cluster form compiles to MEMBAR.ALL.GPU +
+// ERRBAR in front of the arrive, which makes the warp wait for the acknowledgement of its global stores of
+// the tile on every hand-off (measured: profiles/r2_encode_epilogue.md).
+__device__ __forceinline__ void mbar_arrive_cluster_relaxed(uint32_t cluster_addr) {
+  asm volatile("mbarrier.arrive.relaxed.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
+}
 // each CTA of the pair loads into its own shared memory; the bytes complete on `bar` (a
 // shared::cluster address, normally the leader's barrier)
 __device__ __forceinline__ void tma_load_2d_2sm(uint32_t dst, const CUtensorMap* tm, uint32_t bar, int c0, int c1) {

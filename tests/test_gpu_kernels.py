@@ -151,6 +151,36 @@ def test_encode_rp_exact_arithmetic(hd, h, prec, flags, N, F, D, D_eff):
         assert (words[:, W - 1] >> (D_eff % 32) == 0).all()
 
 
+@pytest.mark.parametrize("prec", ["F32", "BF16", "I8"])
+@pytest.mark.parametrize("flags", [0, 2, 4])
+@pytest.mark.parametrize("D_eff,pad,off", [(10000, 0, 0), (10000, 3, 0), (10000, 7, 0), (10000, 3, 1), (4100, 0, 0),
+                                           (4100, 3, 4), (8192, 0, 0), (8192, 4, 2), (240, 0, 0), (240, 4, 0)])
+def test_encode_rp_row_stride_and_alignment_of_hbits(hd, h, prec, flags, D_eff, pad, off):
+    """The sign+pack epilogue writes one 16-byte store per thread when the rows of Hbits are 16-byte aligned
+    (ldh_words % 4 == 0 and an aligned base) and single words otherwise: every (ld, base offset) must give
+    the oracle's bits, exactly W words per row, nothing else in the buffer touched (include/hdc.h)."""
+    N, F = 300, 72
+    r = rng(41, D_eff, pad, off)
+    X = r.integers(0, 256, size=(N, F)).astype(np.float32)
+    P = (1.0 - 2.0 * r.integers(0, 2, size=(D_eff, F))).astype(np.float32)
+    bits_or, _, _ = O.encode_rp(X, P, D_eff, getattr(O, prec))
+    W = (D_eff + 31) // 32
+    ld = W + pad
+    SENT = 0x5A5A5A5A
+    buf = torch.full((N * ld + off + 8,), SENT, dtype=torch.int32, device="cuda")
+    H = buf[off:off + N * ld].view(N, ld)[:, :W]
+    kn = hd.knobs(D_eff, precision=getattr(hd, "HDC_" + prec), flags=flags)
+    h.hdc_encode_rp(dev(X), dev(P), kn, Hbits=H)
+    torch.cuda.synchronize()
+    assert np.array_equal(host_bits(H, D_eff), bits_or)
+    full = buf.cpu().numpy()
+    assert (full[:off] == SENT).all() and (full[off + N * ld:] == SENT).all()
+    if pad:
+        assert (full[off:off + N * ld].reshape(N, ld)[:, W:] == SENT).all()
+    if D_eff % 32:
+        assert (host_words(H)[:, W - 1] >> (D_eff % 32) == 0).all()
+
+
 @pytest.mark.parametrize("prec", ["F32", "BF16", "F16", "I8"])
 @pytest.mark.parametrize("flags", [0, 1, 2, 4])
 def test_encode_rp_float_c2_shape(hd, h, prec, flags):
