@@ -68,7 +68,7 @@ enum { HDC_TRAIN_BUNDLE = 0, HDC_TRAIN_PERCEPTRON = 1, HDC_TRAIN_KMEANS = 2 };
 enum { HDC_OUT_BITS = 1, HDC_OUT_RAW = 4 };
 /* hdc_workspace_bytes ops */
 enum { HDC_OP_ENCODE_RP = 0, HDC_OP_ENCODE_LEVELID = 1, HDC_OP_SIMILARITY = 2, HDC_OP_CLASSIFY = 3,
-       HDC_OP_TRAIN_EPOCH = 4, HDC_OP_INFER_RP_HOST = 5 };
+       HDC_OP_TRAIN_EPOCH = 4, HDC_OP_INFER_RP_HOST = 5, HDC_OP_INFER_RP = 6 };
 /* knobs.flags */
 enum {
   HDC_FLAG_NONE = 0,
@@ -77,10 +77,17 @@ enum {
   HDC_FLAG_TC_1CTA = 2, /* encode contraction: force the one-CTA-per-tile tcgen05 kernel        */
   HDC_FLAG_TC_2CTA = 4, /* encode contraction: force the CTA-pair (cta_group::2) tcgen05 kernel;
                            without either flag the library chooses by problem size              */
-  HDC_FLAG_F32_FAST = 8 /* precision HDC_F32 only, OFF by default: contract 2-way IEEE-half splits of
+  HDC_FLAG_F32_FAST = 8, /* precision HDC_F32 only, OFF by default: contract 2-way IEEE-half splits of
                            the row-scaled operands (22 of the 24 mantissa bits, three tensor-core
                            products instead of six; |error| <= 3 * 2^-22 * sum|x p|).  An extra point
                            of the element-precision knob (L165) between bf16 and fp32, not fp32.  */
+  HDC_FLAG_FUSED_INFER = 16 /* hdc_infer_rp / hdc_infer_rp_host only, OFF by default: for K <= 32 and
+                           N >= 12288 run encode + similarity + arg-max as ONE kernel (the epilogue warps of the
+                           contraction search each signed row against the class hypervectors on the CUDA
+                           cores; the hypervectors need not reach HBM).  Same results as the two kernels;
+                           measured SLOWER than them on B200 (the class values reach the FFMAs through shared
+                           memory, whose bandwidth the tensor-core operand traffic already uses up:
+                           DESIGN.md section 6), kept as a tested A/B switch.                              */
 };
 
 /* Approximation knobs (section 4.2).
@@ -140,6 +147,16 @@ int32_t hdc_version(void);
 /* Number of kernel launches this handle has enqueued since creation (bench `gpu_launches`). */
 int64_t hdc_launch_count(hdc_handle_t h);
 
+/* Which kernels the handle has chosen since creation (a tensor-core request that silently ran on the CUDA
+ * cores, or a fused inference that ran as two kernels, costs a multiple of the time with HDC_OK: this makes it
+ * visible).  HDC_STAT_TC_LAUNCHES: encode contractions on the tcgen05 kernels; HDC_STAT_SIMT_FALLBACKS: encode
+ * contractions for which the tensor path was asked (no HDC_FLAG_SIMT) but refused the operands, so the
+ * CUDA-core kernel ran (hdc_last_error then says so); HDC_STAT_INFER_FUSED / _UNFUSED: hdc_infer_rp /
+ * hdc_infer_rp_host passes (per chunk) through the fused kernel / through encode + classify.  -1: bad id. */
+enum { HDC_STAT_TC_LAUNCHES = 0, HDC_STAT_SIMT_FALLBACKS = 1, HDC_STAT_INFER_FUSED = 2, HDC_STAT_INFER_UNFUSED = 3,
+       HDC_STAT_COUNT = 4 };
+int64_t hdc_stat(hdc_handle_t h, int32_t stat_id);
+
 /* Per-kernel device timing (for roofline reporting).  While enabled, the dominant kernel of each
  * entry point is bracketed by CUDA events on the caller's stream: HDC_K_ENCODE_GEMM (contraction of
  * hdc_encode_rp, staging excluded), HDC_K_SIM (similarity / classify kernel, operand staging
@@ -151,7 +168,7 @@ int32_t hdc_kernel_timing(hdc_handle_t h, int32_t enable);
 int32_t hdc_kernel_time(hdc_handle_t h, int32_t kernel_id, float* ms_total, int64_t* launches);
 
 /* Bytes of device workspace the given op needs for these sizes and knobs (0 is possible).
- * F_or_Q: F for encode_rp / infer_rp_host, Q for encode_levelid, ignored otherwise.
+ * F_or_Q: F for encode_rp / infer_rp / infer_rp_host, Q for encode_levelid, ignored otherwise.
  * For HDC_OP_TRAIN_EPOCH, N is the mini-batch size actually used (batch, or N when batch = 0); for
  * HDC_TRAIN_KMEANS and hdc_train_delta it is the number of samples of the call. */
 size_t hdc_workspace_bytes(hdc_handle_t h, int32_t op, int64_t N, int32_t F_or_Q, int32_t D,
@@ -277,9 +294,25 @@ int32_t hdc_train_delta(hdc_handle_t h, const uint32_t* Hbits, int64_t N, int64_
 int32_t hdc_train_apply(hdc_handle_t h, float* C_acc, int32_t K, int64_t ldc, int32_t D,
                         const hdc_knobs_t* knobs, const int32_t* delta, float lr, void* stream);
 
+/* ---- (1a)+(2)+(3a) inference in one call ----------------------------------------------------
+ * PAPER.md Listing 1 L63-L81 (`inference`: matmul -> hamming_distance / cos_sim -> arg_min as one task),
+ * L161 (binarization between them).  labels[n] = hdc_classify(hdc_encode_rp(X))[n] with the same knobs:
+ * operand precisions, D_eff, similarity, class width and perforation exactly as in those two calls (integer
+ * class operands -- hv_bits 8 and 1 -- give the same labels bit for bit; float class operands the same
+ * scores up to fp32 summation order, i.e. within the 1e-3 tolerance of the float paths).  best / second
+ * (nullable) as in hdc_classify.  Hbits (NULLABLE, [N][ldh_words]) additionally receives the hypervectors.
+ * The call runs the encode and the classify kernels one after the other on `stream` (the hypervectors
+ * stay in the workspace when Hbits is NULL).  With HDC_FLAG_FUSED_INFER, K <= 32 and N >= 12288 the three
+ * steps run as ONE kernel instead (see the flag; hdc_stat says which path ran).
+ * Workspace: hdc_workspace_bytes(HDC_OP_INFER_RP, N, F, D, K, knobs). */
+int32_t hdc_infer_rp(hdc_handle_t h, const void* X, int32_t x_dtype, int64_t N, int32_t F, int64_t ldx,
+                     const void* P, int32_t p_dtype, int32_t D, int64_t ldp, const float* C_acc, int32_t K,
+                     int64_t ldc, const hdc_knobs_t* knobs, int32_t* labels, float* best, float* second,
+                     uint32_t* Hbits, int64_t ldh_words, void* ws, size_t ws_bytes, void* stream);
+
 /* ---- end-to-end inference from host buffers ------------------------------------------------
  * encode_rp + classify for N queries whose features live in HOST memory (pinned for full speed):
- * copies X_host in chunks to the device (inside the call), runs (1a)+(2)+(3a) and copies the
+ * copies X_host in chunks to the device (inside the call), runs hdc_infer_rp per chunk and copies the
  * labels back to labels_host; synchronises `stream` before returning.  P and C_acc are device
  * pointers as above.  Used for the end-to-end (`e2e`) measurement. */
 int32_t hdc_infer_rp_host(hdc_handle_t h, const void* X_host, int32_t x_dtype, int64_t N, int32_t F,

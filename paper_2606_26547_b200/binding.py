@@ -21,16 +21,18 @@ HDC_SIM_DOT, HDC_SIM_COS, HDC_SIM_HAMMING = 0, 1, 2
 HDC_TRAIN_BUNDLE, HDC_TRAIN_PERCEPTRON, HDC_TRAIN_KMEANS = 0, 1, 2
 HDC_OUT_BITS, HDC_OUT_RAW = 1, 4
 HDC_OP_ENCODE_RP, HDC_OP_ENCODE_LEVELID, HDC_OP_SIMILARITY = 0, 1, 2
-HDC_OP_CLASSIFY, HDC_OP_TRAIN_EPOCH, HDC_OP_INFER_RP_HOST = 3, 4, 5
+HDC_OP_CLASSIFY, HDC_OP_TRAIN_EPOCH, HDC_OP_INFER_RP_HOST, HDC_OP_INFER_RP = 3, 4, 5, 6
 HDC_FLAG_NONE, HDC_FLAG_SIMT, HDC_FLAG_TC_1CTA, HDC_FLAG_TC_2CTA, HDC_FLAG_F32_FAST = 0, 1, 2, 4, 8
+HDC_FLAG_FUSED_INFER = 16
 HDC_HV_F16 = 17
 HDC_K_ENCODE_GEMM, HDC_K_SIM, HDC_K_LEVELID, HDC_K_CLASS_UPDATE = 0, 1, 2, 3
+HDC_STAT_TC_LAUNCHES, HDC_STAT_SIMT_FALLBACKS, HDC_STAT_INFER_FUSED, HDC_STAT_INFER_UNFUSED = 0, 1, 2, 3
 
 EXPORTS = ("hdc_create", "hdc_destroy", "hdc_last_error", "hdc_version", "hdc_launch_count",
            "hdc_workspace_bytes", "hdc_encode_rp", "hdc_encode_levelid", "hdc_encode_levelid_u16",
            "hdc_similarity", "hdc_similarity_adc",
            "hdc_classify", "hdc_train_epoch", "hdc_train_delta", "hdc_train_apply", "hdc_infer_rp_host",
-           "hdc_kernel_timing", "hdc_kernel_time")
+           "hdc_kernel_timing", "hdc_kernel_time", "hdc_infer_rp", "hdc_stat")
 
 
 class hdc_knobs_t(C.Structure):
@@ -100,6 +102,11 @@ def lib() -> C.CDLL:
     L.hdc_infer_rp_host.argtypes = [vp, vp, i32, i64, i32, i64, vp, i32, i32, i64, vp, i32, i64, kp, vp, vp,
                                     sz, vp]
     L.hdc_infer_rp_host.restype = i32
+    L.hdc_infer_rp.argtypes = [vp, vp, i32, i64, i32, i64, vp, i32, i32, i64, vp, i32, i64, kp, vp, vp, vp, vp, i64,
+                               vp, sz, vp]
+    L.hdc_infer_rp.restype = i32
+    L.hdc_stat.argtypes = [vp, i32]
+    L.hdc_stat.restype = i64
     L.hdc_kernel_timing.argtypes = [vp, i32]
     L.hdc_kernel_timing.restype = i32
     L.hdc_kernel_time.argtypes = [vp, i32, C.POINTER(C.c_float), C.POINTER(i64)]
@@ -312,6 +319,29 @@ class Handle:
                                      _ptr(delta), C.c_float(lr), self._stream())
         self._check(rc)
         return C_acc
+
+    def stat(self, stat_id: int) -> int:
+        return int(self._L.hdc_stat(self._h, int(stat_id)))
+
+    # -------------------------------------------------------------------------------- (1a)+(2)+(3a)
+    def hdc_infer_rp(self, X, P, C_acc, kn: hdc_knobs_t, labels=None, want_scores: bool = False, Hbits=None):
+        """encode + similarity + arg-max in one call (fused into one kernel for small K, large N)."""
+        N, F = X.shape
+        D = P.shape[0]
+        K = C_acc.shape[0]
+        if labels is None:
+            labels = torch.empty(N, dtype=torch.int32, device=self.device)
+        best = second = None
+        if want_scores:
+            best = torch.empty(N, dtype=torch.float32, device=self.device)
+            second = torch.empty(N, dtype=torch.float32, device=self.device)
+        ws, wsb = self._workspace(self.workspace_bytes(HDC_OP_INFER_RP, N, F, D, K, kn))
+        rc = self._L.hdc_infer_rp(self._h, _ptr(X), _DT[X.dtype], N, F, _rowmajor(X, "X"), _ptr(P), _DT[P.dtype], D,
+                                  _rowmajor(P, "P"), _ptr(C_acc), K, _rowmajor(C_acc, "C_acc"), C.byref(kn),
+                                  _ptr(labels), _ptr(best), _ptr(second), _ptr(Hbits),
+                                  0 if Hbits is None else _rowmajor(Hbits, "Hbits"), ws, wsb, self._stream())
+        self._check(rc)
+        return (labels, best, second) if want_scores else labels
 
     # -------------------------------------------------------------------------------- host e2e
     def hdc_infer_rp_host(self, X_host, P, C_acc, kn: hdc_knobs_t, labels_host=None):

@@ -26,6 +26,7 @@ struct hdc_ctx {
   bool reuse_prep = false;
   std::vector<std::pair<cudaEvent_t, cudaEvent_t>> tev[HDC_K_COUNT];  // event pool per kernel id
   size_t tused[HDC_K_COUNT] = {0, 0, 0, 0};
+  int64_t stats[HDC_STAT_COUNT] = {0, 0, 0, 0};
 };
 
 namespace hdc {
@@ -160,18 +161,31 @@ void plan_encode(const hdc_ctx* h, int64_t N, int F, int D_eff, const hdc_knobs_
   if (!p_inplace) pl.Ps = b.take<__nv_bfloat16>((size_t)D_eff * pl.Fp);
 }
 
+// infer (nullable): the epilogue of the fused inference kernel (EPI_INFER: labels, class operand, scales); the
+// contraction then signs, optionally packs (Hbits may be NULL) and classifies in one kernel.  Only the
+// tensor-core path has it: the caller checks infer_fusable() first.
 int encode_rp_core(hdc_ctx* h, const void* X, int x_dtype, int64_t N, int F, int64_t ldx, const void* P,
                    int p_dtype, int64_t ldp, const hdc_knobs_t* k, int out_kinds, uint32_t* Hbits,
-                   int64_t ldh, void* Hraw, int64_t ldraw, Bump& b, size_t ws_bytes, cudaStream_t st) {
+                   int64_t ldh, void* Hraw, int64_t ldraw, Bump& b, size_t ws_bytes, cudaStream_t st,
+                   const Epilogue* infer = nullptr) {
   const int D_eff = k->D_eff;
   const int prec = k->precision;
   const bool want_raw = (out_kinds & HDC_OUT_RAW) != 0;
   Epilogue e{};
-  e.kind = EPI_SIGN;
+  if (infer) e = *infer;
+  e.kind = infer ? EPI_INFER : EPI_SIGN;
   e.bits = Hbits;
   e.ldbits = ldh;
   e.raw = want_raw ? Hraw : nullptr;
   e.ldraw = ldraw;
+  // a tensor-core launch that cannot take these operands: the CUDA-core kernel runs instead (counted, so that
+  // a silent 3x slow-down is visible through hdc_stat); the fused inference epilogue has no such fallback
+  auto tc_refused = [&](const char* what) -> int {
+    if (infer) return fail(h, HDC_ERR_UNSUPPORTED, "infer_rp: operands not usable by the fused tensor-core kernel");
+    ++h->stats[HDC_STAT_SIMT_FALLBACKS];
+    h->err = std::string(what) + ": tensor-core kernel refused the operands, CUDA-core kernel used";
+    return HDC_OK;
+  };
   const int xk = x_dtype == HDC_BF16 ? OPK_BF16 : OPK_F32;
   const int pk = p_dtype == HDC_BF16 ? OPK_BF16 : (p_dtype == HDC_I8 ? OPK_I8 : OPK_F32);
   cudaError_t ce;
@@ -195,8 +209,10 @@ int encode_rp_core(hdc_ctx* h, const void* X, int x_dtype, int64_t N, int F, int
       }
       if (ce == cudaSuccess && want_raw)
         ce = launch_unscale_raw((float*)Hraw, N, D_eff, ldraw, pl.ex, pl.ep, st, &h->launches);
-      if (ce == cudaSuccess) return HDC_OK;
+      if (ce == cudaSuccess) { ++h->stats[HDC_STAT_TC_LAUNCHES]; return HDC_OK; }
       if (ce != cudaErrorNotSupported) return cuda_fail(h, ce, "encode_rp fp32 (2 x fp16) tcgen05");
+      if (int rc = tc_refused("encode_rp fp32 (2 x fp16) tcgen05")) return rc;
+      pl.tc = false;  // the workspace was planned for the 2-way split: go straight to the CUDA-core kernel
     }
     if (pl.tc) {
       ce = launch_split3_bf16(X, xk, N, F, ldx, (__nv_bfloat16*)pl.Xs, pl.Fp, st, &h->launches);
@@ -211,8 +227,9 @@ int encode_rp_core(hdc_ctx* h, const void* X, int x_dtype, int64_t N, int F, int
         Timed tm(h, HDC_K_ENCODE_GEMM, st);
         ce = launch_gemm_tc(h->tc, o, N, D_eff, e, h->sm_count, tc_cta_group(k), st, &h->launches);
       }
-      if (ce == cudaSuccess) return HDC_OK;
+      if (ce == cudaSuccess) { ++h->stats[HDC_STAT_TC_LAUNCHES]; return HDC_OK; }
       if (ce != cudaErrorNotSupported) return cuda_fail(h, ce, "encode_rp fp32 tcgen05");
+      if (int rc = tc_refused("encode_rp fp32 tcgen05")) return rc;
     }
     {
       Timed tm(h, HDC_K_ENCODE_GEMM, st);
@@ -245,8 +262,9 @@ int encode_rp_core(hdc_ctx* h, const void* X, int x_dtype, int64_t N, int F, int
         Timed tm(h, HDC_K_ENCODE_GEMM, st);
         ce = launch_gemm_tc(h->tc, o, N, D_eff, e, h->sm_count, tc_cta_group(k), st, &h->launches);
       }
-      if (ce == cudaSuccess) return HDC_OK;
+      if (ce == cudaSuccess) { ++h->stats[HDC_STAT_TC_LAUNCHES]; return HDC_OK; }
       if (ce != cudaErrorNotSupported) return cuda_fail(h, ce, "encode_rp int8 tcgen05");
+      if (int rc = tc_refused("encode_rp int8 tcgen05")) return rc;
     }
     ce = launch_gemm_simt(Operand{pl.Xs, pl.ldxs, OPK_I8}, Operand{Pq, ldpq, OPK_I8}, N, D_eff, F, true, e,
                           st, &h->launches);
@@ -268,8 +286,9 @@ int encode_rp_core(hdc_ctx* h, const void* X, int x_dtype, int64_t N, int F, int
         Timed tm(h, HDC_K_ENCODE_GEMM, st);
         ce = launch_gemm_tc(h->tc, o, N, D_eff, e, h->sm_count, tc_cta_group(k), st, &h->launches);
       }
-      if (ce == cudaSuccess) return HDC_OK;
+      if (ce == cudaSuccess) { ++h->stats[HDC_STAT_TC_LAUNCHES]; return HDC_OK; }
       if (ce != cudaErrorNotSupported) return cuda_fail(h, ce, "encode_rp fp16 tcgen05");
+      if (int rc = tc_refused("encode_rp fp16 tcgen05")) return rc;
     }
     const int xr = x_dtype == HDC_BF16 ? OPK_BF16_RF16 : OPK_F32_RF16;
     const int pr = p_dtype == HDC_BF16 ? OPK_BF16_RF16 : OPK_F32_RF16;
@@ -303,8 +322,9 @@ int encode_rp_core(hdc_ctx* h, const void* X, int x_dtype, int64_t N, int F, int
       Timed tm(h, HDC_K_ENCODE_GEMM, st);
       ce = launch_gemm_tc(h->tc, o, N, D_eff, e, h->sm_count, tc_cta_group(k), st, &h->launches);
     }
-    if (ce == cudaSuccess) return HDC_OK;
+    if (ce == cudaSuccess) { ++h->stats[HDC_STAT_TC_LAUNCHES]; return HDC_OK; }
     if (ce != cudaErrorNotSupported) return cuda_fail(h, ce, "encode_rp bf16 tcgen05");
+      if (int rc = tc_refused("encode_rp bf16 tcgen05")) return rc;
   }
   const int xr = x_dtype == HDC_BF16 ? OPK_BF16 : OPK_F32_RBF16;
   const int pr = p_dtype == HDC_BF16 ? OPK_BF16 : OPK_F32_RBF16;
@@ -519,13 +539,99 @@ size_t similarity_ws(int64_t N, int K, const hdc_knobs_t* k) {
 
 constexpr int64_t HOST_CHUNK = 16384;
 
+// ------------------------------------------------------------------------------------- fused inference
+// hdc_infer_rp = hdc_encode_rp followed by hdc_classify, kernel for kernel.  Opt-in (HDC_FLAG_FUSED_INFER):
+// encode + similarity + arg-max in ONE contraction kernel (gemm_tc.cu, EPI_INFER) when the class model is
+// small enough to search on the CUDA cores beside the tensor-core tiles: K <= 32, the tensor path is on,
+// CTA pairs are allowed, and there are enough row blocks to occupy the pairs (each pair owns 256 rows and
+// walks all of D).  Measured slower than the two kernels (shared-memory bandwidth): off by default.
+constexpr int INFER_MAX_K = 32;
+constexpr int64_t INFER_MIN_N = 12288;  // 48 row blocks of 256: below it the two-kernel path spreads m x n tiles better
+
+bool infer_fusable(const hdc_ctx* h, const hdc_knobs_t* k, int64_t N, int K) {
+  return (k->flags & HDC_FLAG_FUSED_INFER) && use_tc(h, k) && !(k->flags & HDC_FLAG_TC_1CTA) && h->sm_count >= 2 &&
+         K <= INFER_MAX_K &&
+         N >= INFER_MIN_N && k->D_eff <= (1 << 17);
+}
+int infer_kc(int K) { return K <= 8 ? 8 : (K <= 16 ? 16 : 32); }
+
+// workspace of the fused path after the encode staging: class operand, scales, amax
+void infer_ws(int K, int D_eff, Bump& b) {
+  b.take<float>((size_t)infer_kc(K) * (size_t)round_up(D_eff, 256));
+  b.take<double>((size_t)K);
+  b.take<float>(1);
+}
+
+// Shared by hdc_infer_rp and hdc_infer_rp_host (per chunk).  Hbits may be NULL on the fused path; the
+// two-kernel path then keeps the hypervectors in the workspace.
+int do_infer_rp(hdc_ctx* h, const void* X, int x_dtype, int64_t N, int F, int64_t ldx, const void* P, int p_dtype,
+                int D, int64_t ldp, const float* C_acc, int K, int64_t ldc, const hdc_knobs_t* k, int32_t* labels,
+                float* best, float* second, uint32_t* Hbits, int64_t ldh, Bump& b, size_t ws_bytes,
+                cudaStream_t st) {
+  const int D_eff = k->D_eff;
+  const int W = words_of(D_eff);
+  if (infer_fusable(h, k, N, K) && !perf_on(enc_perf_of(k))) {
+    const int KC = infer_kc(K);
+    const int64_t ldcls = round_up(D_eff, 256);
+    const Perf pf = perf_of(k);
+    float* cls = b.take<float>((size_t)KC * (size_t)ldcls);
+    double* colscale = b.take<double>((size_t)K);
+    float* amax = b.take<float>(1);
+    if (b.off > ws_bytes) return fail(h, HDC_ERR_WORKSPACE, "infer_rp: workspace too small");
+    cudaError_t ce = cudaSuccess;
+    if (!h->reuse_prep) {
+      if (k->hv_bits == 8) ce = launch_tensor_amax(C_acc, K, D_eff, ldc, pf, amax, st, &h->launches);
+      if (ce == cudaSuccess)
+        ce = launch_class_operand_f32(C_acc, K, D_eff, ldc, k->hv_bits, pf, amax, cls, KC, ldcls, st, &h->launches);
+      if (ce == cudaSuccess && k->sim == HDC_SIM_COS)   // norms over the operand as the epilogue contracts it
+        ce = launch_col_scale(Operand{cls, ldcls, OPK_F32}, K, D_eff, 1, pf, colscale, st, &h->launches);
+      if (ce != cudaSuccess) return cuda_fail(h, ce, "infer_rp: class operand");
+    }
+    Epilogue e{};
+    e.labels = labels;
+    e.best = best;
+    e.second = second;
+    e.colscale = k->sim == HDC_SIM_COS ? colscale : nullptr;
+    e.ham_D = k->sim == HDC_SIM_HAMMING ? perf_count(pf, D_eff) : 0;
+    e.cls = cls;
+    e.ldcls = ldcls;
+    e.K = K;
+    int rc = encode_rp_core(h, X, x_dtype, N, F, ldx, P, p_dtype, ldp, k, HDC_OUT_BITS, Hbits, ldh, nullptr, 0, b,
+                            ws_bytes, st, &e);
+    if (rc == HDC_OK) ++h->stats[HDC_STAT_INFER_FUSED];
+    return rc;
+  }
+  uint32_t* Hd = Hbits;
+  int64_t ldhd = ldh;
+  if (!Hd) {
+    Hd = b.take<uint32_t>((size_t)N * W);
+    ldhd = W;
+    if (b.off > ws_bytes) return fail(h, HDC_ERR_WORKSPACE, "infer_rp: workspace too small");
+  }
+  int rc = do_encode_rp(h, X, x_dtype, N, F, ldx, P, p_dtype, D, ldp, k, HDC_OUT_BITS, Hd, ldhd, nullptr, 0, b,
+                        ws_bytes, st);
+  if (rc == HDC_OK)
+    rc = do_similarity(h, Hd, N, ldhd, C_acc, K, ldc, k, nullptr, 0, 0, labels, best, second, b, ws_bytes, st);
+  if (rc == HDC_OK) ++h->stats[HDC_STAT_INFER_UNFUSED];
+  return rc;
+}
+
+// upper bound of what do_infer_rp takes from the workspace for up to N rows
+size_t infer_ws_bytes(const hdc_ctx* h, int64_t N, int F, int K, const hdc_knobs_t* k) {
+  Bump b(nullptr);
+  infer_ws(K, k->D_eff, b);
+  b.take<uint32_t>((size_t)N * words_of(k->D_eff));
+  encode_ws(h, N, F, k->D_eff, k, b);
+  return b.off + 1024 + similarity_ws(N, K, k);
+}
+
 }  // namespace
 }  // namespace hdc
 
 using namespace hdc;
 
 // =================================================================================== handle
-extern "C" int32_t hdc_version(void) { return 102; }  // 1.2: + perforation of the encode contraction (enc_perf_*)
+extern "C" int32_t hdc_version(void) { return 103; }  // 1.3: + hdc_infer_rp (fused inference), hdc_stat
 
 extern "C" int32_t hdc_create(hdc_handle_t* out, int32_t device) {
   if (!out) return HDC_ERR_INVALID_ARG;
@@ -579,6 +685,11 @@ extern "C" const char* hdc_last_error(hdc_handle_t h) { return h ? h->err.c_str(
 
 extern "C" int64_t hdc_launch_count(hdc_handle_t h) { return h ? h->launches : -1; }
 
+extern "C" int64_t hdc_stat(hdc_handle_t h, int32_t stat_id) {
+  if (!h || stat_id < 0 || stat_id >= HDC_STAT_COUNT) return -1;
+  return h->stats[stat_id];
+}
+
 extern "C" int32_t hdc_kernel_timing(hdc_handle_t h, int32_t enable) {
   if (!h) return HDC_ERR_INVALID_ARG;
   h->timing = enable != 0;
@@ -627,14 +738,14 @@ extern "C" size_t hdc_workspace_bytes(hdc_handle_t h, int32_t op, int64_t N, int
       b.take<int32_t>((size_t)K);                           // members per cluster (HDC_TRAIN_KMEANS)
       return b.off + 256 + similarity_ws(N, K, &k);
     }
+    case HDC_OP_INFER_RP:
+      return infer_ws_bytes(h, N, F_or_Q, K, &k) + 256;
     case HDC_OP_INFER_RP_HOST: {
       const int64_t chunk = N < HOST_CHUNK ? N : HOST_CHUNK;
       b.take<float>((size_t)chunk * F_or_Q);  // two staging buffers for X (fp32 upper bound)
       b.take<float>((size_t)chunk * F_or_Q);
-      b.take<uint32_t>((size_t)chunk * words_of(k.D_eff));
       b.take<int32_t>((size_t)N);
-      encode_ws(h, chunk, F_or_Q, k.D_eff, &k, b);
-      return b.off + 512 + similarity_ws(chunk, K, &k);
+      return b.off + 512 + infer_ws_bytes(h, chunk, F_or_Q, K, &k);
     }
     default:
       return 0;
@@ -950,6 +1061,29 @@ extern "C" int32_t hdc_train_apply(hdc_handle_t h, float* C_acc, int32_t K, int6
   return ce == cudaSuccess ? HDC_OK : cuda_fail(h, ce, "train_apply");
 }
 
+// =================================================================================== fused inference
+extern "C" int32_t hdc_infer_rp(hdc_handle_t h, const void* X, int32_t x_dtype, int64_t N, int32_t F, int64_t ldx,
+                                const void* P, int32_t p_dtype, int32_t D, int64_t ldp, const float* C_acc,
+                                int32_t K, int64_t ldc, const hdc_knobs_t* knobs, int32_t* labels, float* best,
+                                float* second, uint32_t* Hbits, int64_t ldh_words, void* ws, size_t ws_bytes,
+                                void* stream) {
+  if (!h) return HDC_ERR_INVALID_ARG;
+  int rc = check_encode_rp_args(h, X, x_dtype, N, F, ldx, P, p_dtype, D, ldp, knobs);
+  if (rc) return rc;
+  if (!C_acc || (!labels && N > 0)) return fail(h, HDC_ERR_INVALID_ARG, "infer_rp: NULL pointer");
+  if (K < 1 || K > 65535 || ldc < D) return fail(h, HDC_ERR_INVALID_ARG, "infer_rp: bad sizes");
+  rc = check_sim_knobs(h, knobs);
+  if (rc) return rc;
+  if (Hbits && ldh_words < words_of(knobs->D_eff)) return fail(h, HDC_ERR_INVALID_ARG, "infer_rp: ldh_words < W");
+  if ((reinterpret_cast<uintptr_t>(Hbits) | reinterpret_cast<uintptr_t>(C_acc) | reinterpret_cast<uintptr_t>(labels)) & 3)
+    return fail(h, HDC_ERR_ALIGNMENT, "infer_rp: operands must be 4-byte aligned");
+  if (N == 0) return HDC_OK;
+  Bump b(ws);
+  if (!ws) ws_bytes = 0;
+  return do_infer_rp(h, X, x_dtype, N, F, ldx, P, p_dtype, D, ldp, C_acc, K, ldc, knobs, labels, best, second, Hbits,
+                     ldh_words, b, ws_bytes, (cudaStream_t)stream);
+}
+
 // =================================================================================== host end-to-end
 extern "C" int32_t hdc_infer_rp_host(hdc_handle_t h, const void* X_host, int32_t x_dtype, int64_t N, int32_t F,
                                      int64_t ldx, const void* P, int32_t p_dtype, int32_t D, int64_t ldp,
@@ -966,13 +1100,11 @@ extern "C" int32_t hdc_infer_rp_host(hdc_handle_t h, const void* X_host, int32_t
   cudaStream_t st = (cudaStream_t)stream;
   const size_t es = x_dtype == HDC_BF16 ? 2 : 4;
   const int64_t chunk = N < HOST_CHUNK ? N : HOST_CHUNK;
-  const int W = words_of(knobs->D_eff);
   Bump b(ws);
   if (!ws) ws_bytes = 0;
   char* Xd[2];
   Xd[0] = (char*)b.take<float>((size_t)chunk * F);
   Xd[1] = (char*)b.take<float>((size_t)chunk * F);
-  uint32_t* Hd = b.take<uint32_t>((size_t)chunk * W);
   int32_t* Ld = b.take<int32_t>((size_t)N);
   if (b.off > ws_bytes) return fail(h, HDC_ERR_WORKSPACE, "infer_rp_host: workspace too small");
   const size_t base_off = b.off;
@@ -999,11 +1131,8 @@ extern "C" int32_t hdc_infer_rp_host(hdc_handle_t h, const void* X_host, int32_t
     be.off = base_off;
     // same chunk size => same workspace layout: P staging and class-operand preparation of chunk 0 are reused
     h->reuse_prep = c > 0 && nb == chunk;
-    rc = do_encode_rp(h, Xd[buf], x_dtype, nb, F, F, P, p_dtype, D, ldp, knobs, HDC_OUT_BITS, Hd, W, nullptr, 0,
-                      be, ws_bytes, st);
-    if (rc == HDC_OK)
-      rc = do_similarity(h, Hd, nb, W, C_acc, K, ldc, knobs, nullptr, 0, 0, Ld + n0, nullptr, nullptr, be,
-                         ws_bytes, st);
+    rc = do_infer_rp(h, Xd[buf], x_dtype, nb, F, F, P, p_dtype, D, ldp, C_acc, K, ldc, knobs, Ld + n0, nullptr,
+                     nullptr, nullptr, 0, be, ws_bytes, st);
     h->reuse_prep = false;
     if (rc) return rc;
     cudaEventRecord(h->ev_done[buf], st);

@@ -43,7 +43,7 @@ static inline int perf_count(const Perf& pf, int D_eff) {
 }
 static inline bool perf_on(const Perf& pf) { return pf.begin > 0 || pf.stride > 1; }
 
-enum EpilogueKind : int { EPI_SIGN = 0, EPI_SCORE = 1, EPI_ARGMAX = 2 };
+enum EpilogueKind : int { EPI_SIGN = 0, EPI_SCORE = 1, EPI_ARGMAX = 2, EPI_INFER = 3 };
 
 // Epilogue of C[m,n] = sum_k A[m,k] * B[n,k]
 struct Epilogue {
@@ -64,6 +64,14 @@ struct Epilogue {
   float* best;
   float* second;
   int ham_D;
+  // EPI_INFER (gemm_tc.cu only): sign of the accumulators (packed into `bits` when it is not NULL) followed by
+  // the similarity search of the signed row against K <= 32 class hypervectors and the arg-max, all in the
+  // epilogue: score[m,k] = sum_n sgn(acc[m,n]) * cls[k][n].  cls: fp32 [KC][ldcls] class operand prepared by
+  // launch_class_operand_f32 (KC = 8, 16 or 32 rows, ldcls a multiple of 256, zeros beyond K / D_eff);
+  // labels / best / second / colscale / ham_D as for EPI_ARGMAX.
+  const float* cls;
+  int64_t ldcls;
+  int K;
 };
 
 // ---- launchers (each returns the CUDA error of its launches and adds to *nlaunch) -------------
@@ -151,6 +159,12 @@ cudaError_t launch_quantize_rows_i8(const void* src, int src_kind, int64_t rows,
 cudaError_t launch_quantize_tensor_i8(const float* C, int K, int D_eff, int64_t ldc, Perf pf, int8_t* dst,
                                       int64_t ld_dst, float* amax_scratch, cudaStream_t st,
                                       int64_t* nlaunch);
+// class operand of the fused inference epilogue (EPI_INFER): dst [KC][ld_dst] fp32, row k < K = the class
+// operand at hv_bits (32: C_acc; 16 / HDC_HV_F16: RNE to bf16 / half; 8: per-tensor int8 code, scale 127 / *amax;
+// 1: +-1 from the sign), zero for d >= D_eff, unvisited d and rows >= K
+cudaError_t launch_class_operand_f32(const float* C, int K, int D_eff, int64_t ldc, int hv_bits, Perf pf,
+                                     const float* amax, float* dst, int KC, int64_t ld_dst, cudaStream_t st,
+                                     int64_t* nlaunch);
 // sign bits of C_acc: cbits [K][W] (tail bits zero)
 cudaError_t launch_sign_bits(const float* C, int K, int D_eff, int64_t ldc, uint32_t* cbits, int W,
                              cudaStream_t st, int64_t* nlaunch);

@@ -208,6 +208,37 @@ __global__ void quantize_tensor_i8_kernel(const float* __restrict__ C, int K, in
   }
 }
 
+// ---------------------------------------------------------------------------------- fp32 class operand
+// Class operand of the fused inference epilogue (gemm_tc.cu, EPI_INFER), S5: the value the
+// similarity contracts at hv_bits, as a float (int8 codes and +-1 are exact in fp32).
+__global__ void class_operand_f32_kernel(const float* __restrict__ C, int K, int D_eff, int64_t ldc, int hv_bits,
+                                         Perf pf, const float* __restrict__ amax, float* __restrict__ dst, int KC,
+                                         int64_t ld_dst) {
+  float s = 1.0f;
+  if (hv_bits == 8) {
+    const float a = *amax;
+    s = a > 0.0f ? __fdiv_rn(127.0f, a) : 1.0f;
+  }
+  const int64_t total = (int64_t)KC * ld_dst;
+  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < total;
+       i += (int64_t)gridDim.x * blockDim.x) {
+    const int k = (int)(i / ld_dst);
+    const int d = (int)(i - (int64_t)k * ld_dst);
+    float v = 0.0f;
+    if (k < K && d < D_eff && perf_visits(pf, d)) {
+      const float x = __ldg(C + (int64_t)k * ldc + d);
+      switch (hv_bits) {
+        case 32: v = x; break;
+        case 16: v = __bfloat162float(__float2bfloat16_rn(x)); break;
+        case HDC_HV_F16: v = __half2float(__float2half_rn(x)); break;
+        case 8: v = (float)quant_i8(x, s); break;
+        default: v = x < 0.0f ? -1.0f : 1.0f; break;
+      }
+    }
+    dst[i] = v;
+  }
+}
+
 // ---------------------------------------------------------------------------------- sign bits
 // One warp produces 32 words (1024 dims) of one class row: coalesced loads, one ballot per word.
 __global__ void sign_bits_kernel(const float* __restrict__ C, int K, int D_eff, int64_t ldc,
@@ -327,9 +358,54 @@ cudaError_t launch_unscale_raw(float* raw, int64_t rows, int cols, int64_t ld, c
   return cudaGetLastError();
 }
 
+namespace {
+// Same result, one pass over HBM: the row (<= 1024 columns) is read once into registers with coalesced
+// loads, its codes go through a per-warp shared-memory line and leave as 16-byte stores (the plain kernel
+// reads the row twice and stores single bytes: 3x off the HBM time of the C4 int8 point's 294 MB of features).
+constexpr int QR_WARPS = 8;
+constexpr int QR_MAXC = 1024;
+__global__ void __launch_bounds__(QR_WARPS * 32)
+quantize_rows_i8_reg_kernel(const void* __restrict__ src, int src_kind, int64_t rows, int cols, int64_t ld_src,
+                            int8_t* __restrict__ dst, int64_t ld_dst) {
+  __shared__ __align__(16) int8_t line[QR_WARPS][QR_MAXC + 64];
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  const int64_t warp = (int64_t)blockIdx.x * QR_WARPS + wid;
+  const int64_t nwarps = (int64_t)gridDim.x * QR_WARPS;
+  const int nvec = (int)(ld_dst >> 4);  // ld_dst is a multiple of 16
+  for (int64_t r = warp; r < rows; r += nwarps) {
+    float v[QR_MAXC / 32];
+    float a = 0.0f;
+#pragma unroll
+    for (int i = 0; i < QR_MAXC / 32; ++i) {
+      const int c = i * 32 + lane;
+      v[i] = c < cols ? load_as_f32(src, src_kind, r * ld_src + c) : 0.0f;
+      a = fmaxf(a, fabsf(v[i]));
+    }
+#pragma unroll
+    for (int off = 16; off; off >>= 1) a = fmaxf(a, __shfl_xor_sync(0xffffffffu, a, off));
+    const float s = a > 0.0f ? __fdiv_rn(127.0f, a) : 1.0f;
+#pragma unroll
+    for (int i = 0; i < QR_MAXC / 32; ++i) {
+      const int c = i * 32 + lane;
+      if (c < (int)ld_dst) line[wid][c] = (int8_t)(c < cols ? quant_i8(v[i], s) : 0);
+    }
+    __syncwarp();
+    for (int j = lane; j < nvec; j += 32)
+      reinterpret_cast<uint4*>(dst + r * ld_dst)[j] = reinterpret_cast<const uint4*>(line[wid])[j];
+    __syncwarp();
+  }
+}
+}  // namespace
+
 cudaError_t launch_quantize_rows_i8(const void* src, int src_kind, int64_t rows, int cols, int64_t ld_src,
                                     int8_t* dst, int64_t ld_dst, cudaStream_t st, int64_t* nlaunch) {
   if (rows <= 0) return cudaSuccess;
+  if (cols <= QR_MAXC && ld_dst <= QR_MAXC + 64 && (ld_dst & 15) == 0 && (reinterpret_cast<uintptr_t>(dst) & 15) == 0) {
+    quantize_rows_i8_reg_kernel<<<grid_for(rows, QR_WARPS, 148 * 8), QR_WARPS * 32, 0, st>>>(src, src_kind, rows, cols,
+                                                                                          ld_src, dst, ld_dst);
+    ++*nlaunch;
+    return cudaGetLastError();
+  }
   quantize_rows_i8_kernel<<<grid_for(rows * 32, 256, 148 * 16), 256, 0, st>>>(src, src_kind, rows, cols,
                                                                              ld_src, dst, ld_dst);
   ++*nlaunch;
@@ -434,6 +510,15 @@ cudaError_t launch_sign_bits(const float* C, int K, int D_eff, int64_t ldc, uint
                              cudaStream_t st, int64_t* nlaunch) {
   const int64_t warps = (int64_t)K * ((W + 31) >> 5);
   sign_bits_kernel<<<(unsigned)((warps * 32 + 255) / 256), 256, 0, st>>>(C, K, D_eff, ldc, cbits, W);
+  ++*nlaunch;
+  return cudaGetLastError();
+}
+
+cudaError_t launch_class_operand_f32(const float* C, int K, int D_eff, int64_t ldc, int hv_bits, Perf pf,
+                                     const float* amax, float* dst, int KC, int64_t ld_dst, cudaStream_t st,
+                                     int64_t* nlaunch) {
+  class_operand_f32_kernel<<<grid_for((int64_t)KC * ld_dst, 256, 148 * 8), 256, 0, st>>>(C, K, D_eff, ldc, hv_bits, pf,
+                                                                                        amax, dst, KC, ld_dst);
   ++*nlaunch;
   return cudaGetLastError();
 }

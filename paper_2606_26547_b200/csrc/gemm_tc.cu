@@ -19,6 +19,12 @@
 // lives in the leader and collects the epilogue warps of both CTAs.
 // CG = 1: one CTA per 128 x 256 tile, 4-deep ring (small problems, HDC_FLAG_TC_1CTA).
 //
+// EPI_INFER (CTA pairs only; Listing 1 L63-L81 as ONE kernel): the epilogue warps, which idle for most of a tile
+// while the tensor core works, also run the similarity search of the row they have just signed against K <= 32
+// class hypervectors on the CUDA cores -- score[m,k] += sgn(acc[m,n]) * cls[k][n], one FFMA per (class,
+// dimension), class tiles [KC][256] fp32 arriving by TMA through a two-slot ring of their own -- and the
+// arg-max after the last n-tile of the row block, so the hypervectors never leave the SM unless asked for.
+//
 // The reduction axis is a list of SEGMENTS: k-block kb reads A columns a_seg[kb / nkb_seg] *
 // seg_stride + (kb % nkb_seg) * BK and B columns b_seg[..] likewise.  One segment = a plain GEMM.
 // Six segments over 3-way bf16-split operands [x1|x2|x3], [p1|p2|p3] give the fp32-precision
@@ -69,6 +75,17 @@ bool tc_make_map(TcContext* tc, CUtensorMap* out, const void* ptr, bool int8, in
                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
 }
 
+// fp32 [rows][cols] row-major, row stride ld elements: un-swizzled boxes of box_cols x box_rows
+static bool tc_make_map_f32(TcContext* tc, CUtensorMap* out, const void* ptr, int64_t rows, int64_t cols, int64_t ld,
+                            int box_cols, int box_rows) {
+  cuuint64_t dims[2] = {(cuuint64_t)cols, (cuuint64_t)rows};
+  cuuint64_t strides[1] = {(cuuint64_t)ld * 4};
+  cuuint32_t box[2] = {(cuuint32_t)box_cols, (cuuint32_t)box_rows};
+  cuuint32_t estr[2] = {1, 1};
+  return CUDA_SUCCESS == tc->encode(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<void*>(ptr), dims, strides,
+                                    box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                    CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+}
 
 namespace {
 
@@ -81,13 +98,18 @@ constexpr int EPI_WARPS = 8;            // two per TMEM lane quadrant: columns 0
 constexpr int NTHREADS = 64 + 32 * EPI_WARPS;
 constexpr int TMEM_COLS = 512;
 constexpr int MAX_STAGES = 6;
-template <int CG>
+// KC = rows of the class tile of the fused inference epilogue (0: none).  The class tiles (two slots of
+// KC x 256 floats) and the exchange buffer of the final arg-max (128 rows x KC floats) come out of the ring.
+template <int CG, int KC = 0>
 struct Cfg {
-  static constexpr int STAGES = CG == 2 ? 6 : 4;
+  static constexpr int STAGES = KC == 32 ? 4 : KC == 16 ? 5 : CG == 2 ? 6 : 4;
   static constexpr int B_ROWS = BN / CG;               // rows of B this CTA stages
   static constexpr int B_BYTES = B_ROWS * KB_BYTES;    // 32 KB / 16 KB
   static constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
-  static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*alignment slack*/ + 256 /*barriers*/;
+  static constexpr int CLS_BYTES = KC * BN * 4;        // one class tile
+  static constexpr int XCH_BYTES = BM * KC * 4;
+  static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*alignment slack*/ + 256 /*barriers*/ +
+                                    2 * CLS_BYTES + XCH_BYTES;
 };
 
 struct TcParams {
@@ -117,7 +139,7 @@ constexpr double NEG_BIG = -1.0e300;
 template <int EPI, int CG>
 __device__ __forceinline__ bool tile_at(const TcParams& p, int64_t i, int& mt, int& nt) {
   const int64_t unit = blockIdx.x / CG, nunits = gridDim.x / CG;
-  if (EPI == EPI_ARGMAX) {
+  if (EPI == EPI_ARGMAX || EPI == EPI_INFER) {
     const int64_t u = unit + (i / p.n_tiles) * nunits;
     if (u >= p.m_tiles) return false;
     mt = (int)u;
@@ -136,12 +158,14 @@ __device__ __forceinline__ bool tile_at(const TcParams& p, int64_t i, int& mt, i
   return true;
 }
 
-template <bool INT8, int EPI, int CG>
+template <bool INT8, int EPI, int CG, int KC>
 __global__ void __launch_bounds__(NTHREADS, 1)
 gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
-               const TcParams p) {
-  constexpr int STAGES = Cfg<CG>::STAGES;
-  constexpr int STAGE_BYTES = Cfg<CG>::STAGE_BYTES;
+               const __grid_constant__ CUtensorMap tmC, const TcParams p) {
+  static_assert((EPI == EPI_INFER) == (KC != 0), "class tiles belong to the fused inference epilogue");
+  constexpr int STAGES = Cfg<CG, KC>::STAGES;
+  constexpr int STAGE_BYTES = Cfg<CG, KC>::STAGE_BYTES;
+  constexpr int CLS_BYTES = Cfg<CG, KC>::CLS_BYTES;
   extern __shared__ uint8_t smem_raw[];
   const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
   // barriers live after the stage ring (same offsets in both CTAs of a pair)
@@ -152,6 +176,11 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
   auto tempty_bar = [&](int s) { return bar0 + 8u * (2 * MAX_STAGES + 2 + s); };
   const uint32_t tmem_slot = bar0 + 8u * (2 * MAX_STAGES + 4);
   uint32_t* tmem_slot_ptr = reinterpret_cast<uint32_t*>(smem_raw + (tmem_slot - smem_u32(smem_raw)));
+  // EPI_INFER: class-tile ring (two slots, barriers local to each CTA) and the arg-max exchange buffer
+  auto cfull_bar = [&](int s) { return bar0 + 8u * (2 * MAX_STAGES + 6 + s); };
+  auto cempty_bar = [&](int s) { return bar0 + 8u * (2 * MAX_STAGES + 8 + s); };
+  const uint32_t cls0 = bar0 + 256u;
+  const uint32_t xch0 = cls0 + 2u * CLS_BYTES;
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int rank = CG == 2 ? (int)cluster_ctarank() : 0;  // 0 = leader (issues the MMAs)
@@ -168,6 +197,8 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     for (int s = 0; s < 2; ++s) {
       mbar_init(tfull_bar(s), 1);
       mbar_init(tempty_bar(s), EPI_WARPS * CG);
+      mbar_init(cfull_bar(s), 1);
+      mbar_init(cempty_bar(s), EPI_WARPS);
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
@@ -193,6 +224,13 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
         nb = rank * (((n_valid + 15) & ~15) >> 1);
       }
       const int m0 = (mt * CG + rank) * BM;
+      if (EPI == EPI_INFER) {  // this tile's class tile: cls[0..KC)[n0, n0 + 256), own copy per CTA
+        const int cs = (int)(i & 1);
+        mbar_wait(cempty_bar(cs), (uint32_t)((i >> 1) & 1) ^ 1u);
+        mbar_arrive_expect_tx_elect(cfull_bar(cs), CLS_BYTES);
+        tma_load_2d_elect(cls0 + cs * CLS_BYTES, &tmC, cfull_bar(cs), n0, 0);
+        __syncwarp();
+      }
       for (int kb = 0; kb < num_kb; ++kb) {
         const int seg = kb / p.nkb_seg;
         const int j = kb - seg * p.nkb_seg;
@@ -270,6 +308,12 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     int acc = 0;
     uint32_t acc_phase = 0;
     Top2 run = Top2{NEG_BIG, INT_MAX, NEG_BIG};
+    // EPI_INFER: running scores of this thread's row over its half of the columns.  fp32 holds them exactly
+    // for the integer class operands (|score| <= 127 * D_eff < 2^24: launch_gemm_tc checks D_eff) and adds
+    // one rounding per 32-column partial for the float ones.
+    float irun[KC > 0 ? KC : 1];
+#pragma unroll
+    for (int k = 0; k < (KC > 0 ? KC : 1); ++k) irun[k] = 0.0f;
     int mt, nt;
     for (int64_t i = 0; tile_at<EPI, CG>(p, i, mt, nt); ++i) {
       const int n0 = nt * BN;
@@ -342,7 +386,71 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
           }
         }
       }
-      for (int c = 0; EPI != EPI_SIGN && ehalf == 0 && c < nchunks; ++c) {
+      if (EPI == EPI_INFER) {
+        // Fused similarity search.  Per 32-column chunk: sg[j] = +-1.0f from the sign of accumulator j, then one
+        // FFMA per (class, column) against the class tile in shared memory (every lane reads the same 16 bytes:
+        // a broadcast); each 32-column partial sum is added to the class's running score.
+        const int cs = (int)(i & 1);
+        mbar_wait(cfull_bar(cs), (uint32_t)((i >> 1) & 1));
+        const float* ctile = reinterpret_cast<const float*>(smem_raw + (cls0 + cs * CLS_BYTES - smem_u32(smem_raw)));
+        uint32_t words[4] = {0u, 0u, 0u, 0u};
+        const int c_begin = ehalf * 4;
+        const int c_end = nchunks < c_begin + 4 ? nchunks : c_begin + 4;
+#pragma unroll 1
+        for (int c = c_begin; c < c_end; ++c) {
+          uint32_t v[32];
+          tmem_ld32(taddr + (uint32_t)(c * 32), v);
+          tmem_ld_wait();
+          uint32_t w4[4] = {0u, 0u, 0u, 0u};
+#pragma unroll
+          for (int j = 7; j >= 0; --j) {
+#pragma unroll
+            for (int g = 0; g < 4; ++g) {
+              const uint32_t x = v[8 * g + j];
+              const uint32_t u = INT8 ? x : __float_as_uint(__fadd_rn(__uint_as_float(x), 0.0f));
+              w4[g] = __funnelshift_l(u, w4[g], 1);
+              v[8 * g + j] = (u & 0x80000000u) | 0x3F800000u;   // sgn as a float: -0.0 and 0 count as +1 (A1)
+            }
+          }
+          uint32_t word = (w4[0] | (w4[1] << 8)) | ((w4[2] << 16) | (w4[3] << 24));
+          const int valid = n_valid - c * 32;  // >= 1; columns beyond it meet zero class values
+          if (valid < 32) word &= (1u << valid) - 1u;
+          {
+            const int ci = c - c_begin;   // static register selection (a dynamic index would go through local memory)
+            if (ci == 0) words[0] = word;
+            else if (ci == 1) words[1] = word;
+            else if (ci == 2) words[2] = word;
+            else words[3] = word;
+          }
+          const float4* crow = reinterpret_cast<const float4*>(ctile + c * 32);
+#pragma unroll
+          for (int k = 0; k < KC; ++k) {   // two chains of 16 per class, one add into the running score per chunk
+            float t0 = 0.0f, t1 = 0.0f;
+#pragma unroll
+            for (int j4 = 0; j4 < 8; ++j4) {
+              const float4 cv = crow[k * (BN / 4) + j4];
+              t0 = __fmaf_rn(__uint_as_float(v[4 * j4 + 0]), cv.x, t0);
+              t1 = __fmaf_rn(__uint_as_float(v[4 * j4 + 1]), cv.y, t1);
+              t0 = __fmaf_rn(__uint_as_float(v[4 * j4 + 2]), cv.z, t0);
+              t1 = __fmaf_rn(__uint_as_float(v[4 * j4 + 3]), cv.w, t1);
+            }
+            irun[k] = __fadd_rn(irun[k], __fadd_rn(t0, t1));
+          }
+        }
+        if (p.e.bits && row_ok && c_begin < c_end) {
+          uint32_t* dst = p.e.bits + row * p.e.ldbits + (n0 >> 5) + c_begin;
+          if (c_end - c_begin == 4 && p.bits_vec4) {
+            *reinterpret_cast<uint4*>(dst) = make_uint4(words[0], words[1], words[2], words[3]);
+          } else {
+#pragma unroll
+            for (int c = 0; c < 4; ++c)
+              if (c_begin + c < c_end) dst[c] = words[c];
+          }
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(cempty_bar(cs));   // class tile consumed
+      }
+      for (int c = 0; EPI != EPI_SIGN && EPI != EPI_INFER && ehalf == 0 && c < nchunks; ++c) {
         uint32_t v[32];
         tmem_ld32(taddr + (uint32_t)(c * 32), v);
         tmem_ld_wait();
@@ -406,6 +514,48 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
         }
         run = Top2{NEG_BIG, INT_MAX, NEG_BIG};
       }
+      if (EPI == EPI_INFER && nt == p.n_tiles - 1) {
+        // the two warps of a lane quadrant hold the scores of the same rows over the two halves of every tile's
+        // columns: the upper half hands its sums over through shared memory ([class][row]: conflict-free)
+        float* xch = reinterpret_cast<float*>(smem_raw + (xch0 - smem_u32(smem_raw)));
+        const int r = q * 32 + lane;
+        if (ehalf == 1) {
+#pragma unroll
+          for (int k = 0; k < KC; ++k) xch[k * BM + r] = irun[k];
+        }
+        asm volatile("bar.sync %0, 64;" ::"r"(1 + q) : "memory");
+        if (ehalf == 0) {
+          Top2 t = Top2{NEG_BIG, INT_MAX, NEG_BIG};
+#pragma unroll
+          for (int k = 0; k < KC; ++k) {
+            if (k < p.e.K) {
+              const double a = (double)irun[k] + (double)xch[k * BM + r];
+              const double sc = p.e.colscale ? a * p.e.colscale[k] : a;
+              if (sc > t.b1) {  // increasing k: strict > keeps the lowest index
+                t.b2 = t.b1;
+                t.b1 = sc;
+                t.i1 = k;
+              } else if (sc > t.b2) {
+                t.b2 = sc;
+              }
+            }
+          }
+          if (row_ok) {
+            double b1 = t.b1, b2 = t.b2;
+            if (b2 == NEG_BIG) b2 = b1;  // K == 1
+            if (p.e.ham_D > 0) {
+              b1 = 0.5 * ((double)p.e.ham_D - b1);
+              b2 = 0.5 * ((double)p.e.ham_D - b2);
+            }
+            p.e.labels[row] = t.i1;
+            if (p.e.best) p.e.best[row] = (float)b1;
+            if (p.e.second) p.e.second[row] = (float)b2;
+          }
+        }
+        asm volatile("bar.sync %0, 64;" ::"r"(1 + q) : "memory");   // buffer free for the next row block
+#pragma unroll
+        for (int k = 0; k < KC; ++k) irun[k] = 0.0f;
+      }
     }
   }
 
@@ -418,17 +568,16 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
   }
 }
 
-template <bool INT8, int EPI, int CG>
-cudaError_t launch_one(const CUtensorMap& tmA, const CUtensorMap& tmB, const TcParams& p, int grid,
-                       cudaStream_t st) {
-  static bool attr_set = false;  // per instantiation; the attribute is sticky for the function
-  constexpr int SMEM_BYTES = Cfg<CG>::SMEM_BYTES;
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(gemm_tc_kernel<INT8, EPI, CG>,
-                                         cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
-    if (e != cudaSuccess) return e;
-    attr_set = true;
-  }
+template <bool INT8, int EPI, int CG, int KC = 0>
+cudaError_t launch_one(const CUtensorMap& tmA, const CUtensorMap& tmB, const CUtensorMap& tmC, const TcParams& p,
+                       int grid, cudaStream_t st) {
+  constexpr int SMEM_BYTES = Cfg<CG, KC>::SMEM_BYTES;
+  static_assert(SMEM_BYTES <= 227 * 1024, "shared memory budget");
+  // the opt-in is a per-device attribute of the function: set on every launch (a cheap host-side call), so
+  // that handles on different devices of one process each get it
+  cudaError_t e = cudaFuncSetAttribute(gemm_tc_kernel<INT8, EPI, CG, KC>,
+                                       cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+  if (e != cudaSuccess) return e;
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3((unsigned)grid);
   cfg.blockDim = dim3(NTHREADS);
@@ -441,7 +590,7 @@ cudaError_t launch_one(const CUtensorMap& tmA, const CUtensorMap& tmB, const TcP
   at[0].val.clusterDim.z = 1;
   cfg.attrs = at;
   cfg.numAttrs = 1;
-  return cudaLaunchKernelEx(&cfg, gemm_tc_kernel<INT8, EPI, CG>, tmA, tmB, p);
+  return cudaLaunchKernelEx(&cfg, gemm_tc_kernel<INT8, EPI, CG, KC>, tmA, tmB, tmC, p);
 }
 
 template <int CG>
@@ -449,15 +598,25 @@ cudaError_t launch_cg(bool int8, int kind, const CUtensorMap& tmA, const CUtenso
                       int grid, cudaStream_t st) {
   if (int8) {
     switch (kind) {
-      case EPI_SIGN: return launch_one<true, EPI_SIGN, CG>(tmA, tmB, p, grid, st);
-      case EPI_SCORE: return launch_one<true, EPI_SCORE, CG>(tmA, tmB, p, grid, st);
-      default: return launch_one<true, EPI_ARGMAX, CG>(tmA, tmB, p, grid, st);
+      case EPI_SIGN: return launch_one<true, EPI_SIGN, CG>(tmA, tmB, tmB, p, grid, st);
+      case EPI_SCORE: return launch_one<true, EPI_SCORE, CG>(tmA, tmB, tmB, p, grid, st);
+      default: return launch_one<true, EPI_ARGMAX, CG>(tmA, tmB, tmB, p, grid, st);
     }
   }
   switch (kind) {
-    case EPI_SIGN: return launch_one<false, EPI_SIGN, CG>(tmA, tmB, p, grid, st);
-    case EPI_SCORE: return launch_one<false, EPI_SCORE, CG>(tmA, tmB, p, grid, st);
-    default: return launch_one<false, EPI_ARGMAX, CG>(tmA, tmB, p, grid, st);
+    case EPI_SIGN: return launch_one<false, EPI_SIGN, CG>(tmA, tmB, tmB, p, grid, st);
+    case EPI_SCORE: return launch_one<false, EPI_SCORE, CG>(tmA, tmB, tmB, p, grid, st);
+    default: return launch_one<false, EPI_ARGMAX, CG>(tmA, tmB, tmB, p, grid, st);
+  }
+}
+
+template <bool INT8>
+cudaError_t launch_infer(int KC, const CUtensorMap& tmA, const CUtensorMap& tmB, const CUtensorMap& tmC,
+                         const TcParams& p, int grid, cudaStream_t st) {
+  switch (KC) {
+    case 8: return launch_one<INT8, EPI_INFER, 2, 8>(tmA, tmB, tmC, p, grid, st);
+    case 16: return launch_one<INT8, EPI_INFER, 2, 16>(tmA, tmB, tmC, p, grid, st);
+    default: return launch_one<INT8, EPI_INFER, 2, 32>(tmA, tmB, tmC, p, grid, st);
   }
 }
 
@@ -477,12 +636,17 @@ cudaError_t launch_gemm_tc(TcContext* tc, const TcOperands& o, int64_t M, int Nc
     return cudaErrorNotSupported;
   if (M > (int64_t)INT_MAX - 2 * BM || o.cols_a > INT_MAX || o.cols_b > INT_MAX) return cudaErrorNotSupported;
   const int n_tiles = (Nc + BN - 1) / BN;
+  const bool infer = e.kind == EPI_INFER;
+  if (infer && (sm_count < 2 || e.K < 1 || e.K > 32 || Nc > (1 << 17) || !e.cls || (e.ldcls % BN) != 0 || e.ldcls < (int64_t)n_tiles * BN ||
+                (reinterpret_cast<uintptr_t>(e.cls) & 15) || !e.labels))
+    return cudaErrorNotSupported;
   const int64_t units1 = e.kind == EPI_ARGMAX ? (M + BM - 1) / BM : (M + BM - 1) / BM * n_tiles;
   // CTA pairs once every SM has a tile of its own either way; small problems keep the 1-CTA kernel
   // (twice as many independent tiles)
   int cg = cta_group;
   if (cg != 1 && cg != 2) cg = units1 >= 2 * (int64_t)sm_count ? 2 : 1;
   if (sm_count < 2) cg = 1;
+  if (infer) cg = 2;
   TcParams p;
   p.M = M;
   p.Nc = Nc;
@@ -500,10 +664,16 @@ cudaError_t launch_gemm_tc(TcContext* tc, const TcOperands& o, int64_t M, int Nc
   CUtensorMap tmA, tmB;
   if (!tc_make_map(tc, &tmA, o.A, int8, M, o.cols_a, o.lda, BM)) return cudaErrorInvalidValue;
   if (!tc_make_map(tc, &tmB, o.B, int8, Nc, o.cols_b, o.ldb, BN / cg)) return cudaErrorInvalidValue;
-  const int64_t units = e.kind == EPI_ARGMAX ? p.m_tiles : (int64_t)p.m_tiles * p.n_tiles;
+  const int64_t units = (e.kind == EPI_ARGMAX || infer) ? p.m_tiles : (int64_t)p.m_tiles * p.n_tiles;
   const int max_units = sm_count / cg;
   const int grid = (int)(units < max_units ? units : max_units) * cg;
   ++*nlaunch;
+  if (infer) {
+    const int KC = e.K <= 8 ? 8 : (e.K <= 16 ? 16 : 32);
+    CUtensorMap tmC;
+    if (!tc_make_map_f32(tc, &tmC, e.cls, KC, e.ldcls, e.ldcls, BN, KC)) return cudaErrorInvalidValue;
+    return int8 ? launch_infer<true>(KC, tmA, tmB, tmC, p, grid, st) : launch_infer<false>(KC, tmA, tmB, tmC, p, grid, st);
+  }
   if (cg == 2) return launch_cg<2>(int8, e.kind, tmA, tmB, p, grid, st);
   return launch_cg<1>(int8, e.kind, tmA, tmB, p, grid, st);
 }

@@ -266,4 +266,7 @@ def test_c2_bench_launch_configuration_sampled(hd, h):
     assert np.array_equal(lab, lab[idx % n_te])
     Xh = torch.from_numpy(Xq).pin_memory()
     lab_host = h.hdc_infer_rp_host(Xh, Pd, Cd, kn).numpy()
-    assert np.array_equal(lab_host, lab), "host pipeline (16384-row chunks) differs from the device path"
+    # the host pipeline runs the fused kernel per chunk: same hypervectors, scores summed in another order, so
+    # it answers to the oracle by the same rule rather than to the two-kernel path bit for bit
+    check_labels_float(lab_host[:n_te], S_or, O.SIM_COS)
+    assert np.array_equal(lab_host, lab_host[idx % n_te])
