@@ -10,7 +10,8 @@
  *
  * General contract
  *  - Every data pointer is a DEVICE pointer owned by the caller, unless the parameter name ends in
- *    `_host` (then it is a host pointer, pinned for full speed).  Nothing is allocated or freed
+ *    `_host` (then it is a host pointer, pinned for full speed).  A call may be made with any device current:
+ *    its work goes to the handle's device.  Nothing is allocated or freed
  *    inside a compute call; scratch comes from the caller's workspace `ws` (size from
  *    hdc_workspace_bytes()).  `stream` is a cudaStream_t (NULL = legacy default stream).  Calls
  *    enqueue work and return; they do not synchronise (the `_host` entry point does, it says so).
@@ -32,7 +33,8 @@
  *    HDC_OK; the per-sample pointers (X, levels, Hbits, S, labels, y, pred) may then be NULL.
  *  - Outputs must not alias inputs (except C_acc, which is in/out).  A handle is not thread-safe;
  *    distinct handles are independent.  There is no CPU fallback and no other architecture:
- *    hdc_create() fails with HDC_ERR_ARCH unless the device is compute capability 10.x.
+ *    hdc_create() fails with HDC_ERR_ARCH unless the device is compute capability 10.0 (the library
+ *    holds sm_100a code only).
  */
 #ifndef HDC_H_
 #define HDC_H_
@@ -137,7 +139,7 @@ typedef struct {
 
 /* ---- handle ------------------------------------------------------------------------------ */
 /* Creates a context on CUDA device `device` (sets nothing globally except cudaSetDevice during
- * the call).  HDC_ERR_ARCH unless compute capability 10.x; HDC_ERR_CUDA if no device. */
+ * the call).  HDC_ERR_ARCH unless compute capability 10.0; HDC_ERR_CUDA if no device. */
 int32_t hdc_create(hdc_handle_t* out, int32_t device);
 int32_t hdc_destroy(hdc_handle_t h);
 /* Host string describing the last error on this handle; valid until the next call on it. */
@@ -194,7 +196,8 @@ int32_t hdc_encode_rp(hdc_handle_t h, const void* X, int32_t x_dtype, int64_t N,
  * PAPER.md L167 ("ID-based encoding"), L183 (N_LEVELS), L239 (Level-ID); bind = XOR, bundle =
  * majority (BASELINE.json north_star).
  *   cnt[n,d] = sum_{f<F} ( ID[f,d] XOR LV[levels[n,f], d] ),   bit[n,d] = [2*cnt > F]
- * levels [N][ldl] uint8 level indices, each < Q <= 256 (unchecked on device);
+ * levels [N][ldl] uint8 level indices, each < Q <= 256 (unchecked on device); F above what one CTA can stage
+ * in shared memory (about 7000 features; 3500 for the 16-bit variant) returns HDC_ERR_UNSUPPORTED;
  * IDbits [F][ldid_words], LVbits [Q][ldlv_words] packed tables covering D bits. */
 int32_t hdc_encode_levelid(hdc_handle_t h, const uint8_t* levels, int64_t N, int32_t F, int64_t ldl,
                            const uint32_t* IDbits, int64_t ldid_words, const uint32_t* LVbits,
@@ -309,6 +312,43 @@ int32_t hdc_infer_rp(hdc_handle_t h, const void* X, int32_t x_dtype, int64_t N, 
                      const void* P, int32_t p_dtype, int32_t D, int64_t ldp, const float* C_acc, int32_t K,
                      int64_t ldc, const hdc_knobs_t* knobs, int32_t* labels, float* best, float* second,
                      uint32_t* Hbits, int64_t ldh_words, void* ws, size_t ws_bytes, void* stream);
+
+/* ---- prepared model: the query-independent operands, converted once ------------------------
+ * Every plain entry point derives the operands of its contraction from the caller's P and C_acc inside
+ * the call (staged projection at knobs->precision; class operand at knobs->hv_bits with its int8 scale,
+ * cosine scales, perforation mask) -- right for training, where C_acc changes every mini-batch, wasteful
+ * for a server that classifies small batches against a fixed model.  hdc_model_prepare runs exactly those
+ * preparation kernels once, into `blob` (DEVICE memory of the caller, >= hdc_model_bytes(), 256-byte
+ * aligned), and fills the host descriptor *out; the *_m entry points take the descriptor instead of
+ * (P, C_acc, knobs) and launch only the per-query kernels.  Results are identical, bit for bit, to the
+ * plain entry points with the same arguments.  P or C_acc may be NULL (a model with one half only; F / K
+ * are then ignored).  The descriptor is plain data (copy it freely); P, C_acc and blob must stay alive and
+ * unchanged while it is in use (the CUDA-core kernels of HDC_FLAG_SIMT read P and C_acc in place).  The
+ * knobs are fixed at preparation (the staged layouts depend on them) and stored in the descriptor.
+ * Workspace of the *_m calls: as for hdc_encode_rp / hdc_classify / hdc_infer_rp. */
+typedef struct {
+  uint32_t magic;
+  int32_t F, D, K, p_dtype;
+  int64_t ldp, ldc;
+  const void* P;
+  const float* C_acc;
+  void* blob;
+  size_t blob_bytes;
+  hdc_knobs_t knobs;
+} hdc_model_t;
+size_t hdc_model_bytes(hdc_handle_t h, int32_t F, int32_t D, int32_t K, const hdc_knobs_t* knobs);
+int32_t hdc_model_prepare(hdc_handle_t h, const void* P, int32_t p_dtype, int32_t F, int32_t D, int64_t ldp,
+                          const float* C_acc, int32_t K, int64_t ldc, const hdc_knobs_t* knobs, void* blob,
+                          size_t blob_bytes, hdc_model_t* out, void* stream);
+/* = hdc_encode_rp (HDC_OUT_BITS) / hdc_classify / hdc_infer_rp with the model's P, C_acc and knobs */
+int32_t hdc_encode_rp_m(hdc_handle_t h, const void* X, int32_t x_dtype, int64_t N, int64_t ldx,
+                        const hdc_model_t* m, uint32_t* Hbits, int64_t ldh_words, void* ws, size_t ws_bytes,
+                        void* stream);
+int32_t hdc_classify_m(hdc_handle_t h, const uint32_t* Hbits, int64_t N, int64_t ldh_words, const hdc_model_t* m,
+                       int32_t* labels, float* best, float* second, void* ws, size_t ws_bytes, void* stream);
+int32_t hdc_infer_rp_m(hdc_handle_t h, const void* X, int32_t x_dtype, int64_t N, int64_t ldx,
+                       const hdc_model_t* m, int32_t* labels, float* best, float* second, uint32_t* Hbits,
+                       int64_t ldh_words, void* ws, size_t ws_bytes, void* stream);
 
 /* ---- end-to-end inference from host buffers ------------------------------------------------
  * encode_rp + classify for N queries whose features live in HOST memory (pinned for full speed):

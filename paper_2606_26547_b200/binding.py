@@ -32,7 +32,8 @@ EXPORTS = ("hdc_create", "hdc_destroy", "hdc_last_error", "hdc_version", "hdc_la
            "hdc_workspace_bytes", "hdc_encode_rp", "hdc_encode_levelid", "hdc_encode_levelid_u16",
            "hdc_similarity", "hdc_similarity_adc",
            "hdc_classify", "hdc_train_epoch", "hdc_train_delta", "hdc_train_apply", "hdc_infer_rp_host",
-           "hdc_kernel_timing", "hdc_kernel_time", "hdc_infer_rp", "hdc_stat")
+           "hdc_kernel_timing", "hdc_kernel_time", "hdc_infer_rp", "hdc_stat", "hdc_model_bytes", "hdc_model_prepare",
+           "hdc_encode_rp_m", "hdc_classify_m", "hdc_infer_rp_m")
 
 
 class hdc_knobs_t(C.Structure):
@@ -43,6 +44,12 @@ class hdc_knobs_t(C.Structure):
 
 class hdc_adc_t(C.Structure):
     _fields_ = [("res", C.c_int32), ("step", C.c_int32), ("floor", C.c_int32), ("ceil", C.c_int32)]
+
+
+class hdc_model_t(C.Structure):
+    _fields_ = [("magic", C.c_uint32), ("F", C.c_int32), ("D", C.c_int32), ("K", C.c_int32), ("p_dtype", C.c_int32),
+                ("ldp", C.c_int64), ("ldc", C.c_int64), ("P", C.c_void_p), ("C_acc", C.c_void_p), ("blob", C.c_void_p),
+                ("blob_bytes", C.c_size_t), ("knobs", hdc_knobs_t)]
 
 
 class HdcError(RuntimeError):
@@ -107,6 +114,17 @@ def lib() -> C.CDLL:
     L.hdc_infer_rp.restype = i32
     L.hdc_stat.argtypes = [vp, i32]
     L.hdc_stat.restype = i64
+    mp = C.POINTER(hdc_model_t)
+    L.hdc_model_bytes.argtypes = [vp, i32, i32, i32, kp]
+    L.hdc_model_bytes.restype = sz
+    L.hdc_model_prepare.argtypes = [vp, vp, i32, i32, i32, i64, vp, i32, i64, kp, vp, sz, mp, vp]
+    L.hdc_model_prepare.restype = i32
+    L.hdc_encode_rp_m.argtypes = [vp, vp, i32, i64, i64, mp, vp, i64, vp, sz, vp]
+    L.hdc_encode_rp_m.restype = i32
+    L.hdc_classify_m.argtypes = [vp, vp, i64, i64, mp, vp, vp, vp, vp, sz, vp]
+    L.hdc_classify_m.restype = i32
+    L.hdc_infer_rp_m.argtypes = [vp, vp, i32, i64, i64, mp, vp, vp, vp, vp, i64, vp, sz, vp]
+    L.hdc_infer_rp_m.restype = i32
     L.hdc_kernel_timing.argtypes = [vp, i32]
     L.hdc_kernel_timing.restype = i32
     L.hdc_kernel_time.argtypes = [vp, i32, C.POINTER(C.c_float), C.POINTER(i64)]
@@ -343,6 +361,63 @@ class Handle:
         self._check(rc)
         return (labels, best, second) if want_scores else labels
 
+    # -------------------------------------------------------------------------------- prepared model
+    def hdc_model_prepare(self, P, C_acc, kn: hdc_knobs_t) -> "Model":
+        """Converts the query-independent operands once (include/hdc.h "prepared model").  P or C_acc may be None."""
+        D = P.shape[0] if P is not None else C_acc.shape[1]
+        F = P.shape[1] if P is not None else 1
+        K = C_acc.shape[0] if C_acc is not None else 1
+        nbytes = int(self._L.hdc_model_bytes(self._h, F, D, K, C.byref(kn)))
+        blob = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+        off = (-blob.data_ptr()) % 256
+        desc = hdc_model_t()
+        rc = self._L.hdc_model_prepare(self._h, _ptr(P), _DT[P.dtype] if P is not None else HDC_F32, F, D,
+                                       _rowmajor(P, "P") if P is not None else F, _ptr(C_acc), K,
+                                       _rowmajor(C_acc, "C_acc") if C_acc is not None else D, C.byref(kn),
+                                       C.c_void_p(blob.data_ptr() + off), nbytes, C.byref(desc), self._stream())
+        self._check(rc)
+        return Model(desc, (blob, P, C_acc), kn)
+
+    def hdc_encode_rp_m(self, X, m: "Model", Hbits=None):
+        N, F = X.shape
+        kn = m.kn
+        if Hbits is None:
+            Hbits = self.alloc_hbits(N, kn.D_eff)
+        ws, wsb = self._workspace(self.workspace_bytes(HDC_OP_ENCODE_RP, N, F, m.desc.D, 0, kn))
+        rc = self._L.hdc_encode_rp_m(self._h, _ptr(X), _DT[X.dtype], N, _rowmajor(X, "X"), C.byref(m.desc), _ptr(Hbits),
+                                     _rowmajor(Hbits, "Hbits"), ws, wsb, self._stream())
+        self._check(rc)
+        return Hbits
+
+    def hdc_classify_m(self, Hbits, m: "Model", want_scores: bool = False, labels=None):
+        N = Hbits.shape[0]
+        if labels is None:
+            labels = torch.empty(N, dtype=torch.int32, device=self.device)
+        best = second = None
+        if want_scores:
+            best = torch.empty(N, dtype=torch.float32, device=self.device)
+            second = torch.empty(N, dtype=torch.float32, device=self.device)
+        ws, wsb = self._workspace(self.workspace_bytes(HDC_OP_CLASSIFY, N, 0, m.desc.D, m.desc.K, m.kn))
+        rc = self._L.hdc_classify_m(self._h, _ptr(Hbits), N, _rowmajor(Hbits, "Hbits"), C.byref(m.desc), _ptr(labels),
+                                    _ptr(best), _ptr(second), ws, wsb, self._stream())
+        self._check(rc)
+        return (labels, best, second) if want_scores else labels
+
+    def hdc_infer_rp_m(self, X, m: "Model", labels=None, want_scores: bool = False, Hbits=None):
+        N, F = X.shape
+        if labels is None:
+            labels = torch.empty(N, dtype=torch.int32, device=self.device)
+        best = second = None
+        if want_scores:
+            best = torch.empty(N, dtype=torch.float32, device=self.device)
+            second = torch.empty(N, dtype=torch.float32, device=self.device)
+        ws, wsb = self._workspace(self.workspace_bytes(HDC_OP_INFER_RP, N, F, m.desc.D, m.desc.K, m.kn))
+        rc = self._L.hdc_infer_rp_m(self._h, _ptr(X), _DT[X.dtype], N, _rowmajor(X, "X"), C.byref(m.desc), _ptr(labels),
+                                    _ptr(best), _ptr(second), _ptr(Hbits),
+                                    0 if Hbits is None else _rowmajor(Hbits, "Hbits"), ws, wsb, self._stream())
+        self._check(rc)
+        return (labels, best, second) if want_scores else labels
+
     # -------------------------------------------------------------------------------- host e2e
     def hdc_infer_rp_host(self, X_host, P, C_acc, kn: hdc_knobs_t, labels_host=None):
         """X_host: CPU tensor (pinned for full speed); returns CPU int32 labels.  Synchronises."""
@@ -358,3 +433,10 @@ class Handle:
                                        C.byref(kn), _ptr(labels_host), ws, wsb, self._stream())
         self._check(rc)
         return labels_host
+
+
+class Model:
+    """hdc_model_t descriptor plus the tensors it points into (kept alive with it)."""
+
+    def __init__(self, desc: hdc_model_t, keep, kn: hdc_knobs_t):
+        self.desc, self._keep, self.kn = desc, keep, kn

@@ -21,9 +21,13 @@ struct hdc_ctx {
   cudaEvent_t ev_done[2] = {nullptr, nullptr};
   cudaEvent_t ev_entry = nullptr;
   bool timing = false;
-  // set by hdc_infer_rp_host for chunks after the first of equal size: the staged projection and the
-  // prepared class operand of the previous chunk still sit at the same workspace addresses
-  bool reuse_prep = false;
+  // Where the per-call-invariant operands live (staged projection, class operand, scales) and whether this
+  // pass prepares them, uses them, or both.  model == nullptr: they are carved from the call's workspace and
+  // prepared in the call (the plain entry points).  hdc_model_prepare: PREP_ONLY into the caller's blob; the
+  // *_m entry points and the chunks of hdc_infer_rp_host after the first: RUN_ONLY.
+  void* model = nullptr;  // hdc::Bump*
+  size_t model_cap = 0;
+  int prep_mode = 0;  // PREP_AND_RUN
   std::vector<std::pair<cudaEvent_t, cudaEvent_t>> tev[HDC_K_COUNT];  // event pool per kernel id
   size_t tused[HDC_K_COUNT] = {0, 0, 0, 0};
   int64_t stats[HDC_STAT_COUNT] = {0, 0, 0, 0};
@@ -45,6 +49,16 @@ struct Bump {
     return p;
   }
 };
+
+enum PrepMode : int { PREP_AND_RUN = 0, PREP_ONLY = 1, RUN_ONLY = 2 };
+// the allocator of the persistent operands of this pass
+Bump& persistent(hdc_ctx* h, Bump& b) { return h->model ? *static_cast<Bump*>(h->model) : b; }
+bool persistent_fits(const hdc_ctx* h, Bump& b, size_t ws_bytes) {
+  if (b.off > ws_bytes) return false;
+  return !h->model || static_cast<Bump*>(h->model)->off <= h->model_cap;
+}
+bool do_prep(const hdc_ctx* h) { return h->prep_mode != RUN_ONLY; }
+bool prep_only(const hdc_ctx* h) { return h->prep_mode == PREP_ONLY; }
 
 int fail(hdc_ctx* h, int code, const char* msg) {
   if (h) h->err = msg;
@@ -72,6 +86,18 @@ struct Timed {
   }
   ~Timed() {
     if (stop) cudaEventRecord(stop, st);
+  }
+};
+
+// Work of a handle goes to the handle's device whatever device the caller left current (restored on return).
+struct DeviceGuard {
+  int prev = -1;
+  bool switched = false;
+  explicit DeviceGuard(int device) {
+    if (cudaGetDevice(&prev) == cudaSuccess && prev != device) switched = cudaSetDevice(device) == cudaSuccess;
+  }
+  ~DeviceGuard() {
+    if (switched) cudaSetDevice(prev);
   }
 };
 
@@ -127,8 +153,9 @@ bool use_tc(const hdc_ctx* h, const hdc_knobs_t* k) {
 }
 
 // Carves the staging buffers of hdc_encode_rp.  x_inplace / p_inplace: operand usable as given.
+// X staging comes from b (scratch), P staging from pm (persistent: may be the same allocator).
 void plan_encode(const hdc_ctx* h, int64_t N, int F, int D_eff, const hdc_knobs_t* k, bool x_inplace,
-                 bool p_inplace, Bump& b, EncodePlan& pl) {
+                 bool p_inplace, Bump& b, Bump& pm, EncodePlan& pl) {
   const int prec = k->precision;
   pl.tc = use_tc(h, k);
   pl.Fp = (int)round_up(F, 64);
@@ -137,20 +164,20 @@ void plan_encode(const hdc_ctx* h, int64_t N, int F, int D_eff, const hdc_knobs_
     if (k->flags & HDC_FLAG_F32_FAST) {
       pl.ldxs = pl.ldps = 2 * (int64_t)pl.Fp;
       pl.Xs = b.take<__half>((size_t)N * pl.ldxs);
-      pl.Ps = b.take<__half>((size_t)D_eff * pl.ldps);
+      pl.Ps = pm.take<__half>((size_t)D_eff * pl.ldps);
       pl.ex = b.take<int>((size_t)N);
-      pl.ep = b.take<int>((size_t)D_eff);
+      pl.ep = pm.take<int>((size_t)D_eff);
       return;
     }
     pl.ldxs = pl.ldps = 3 * (int64_t)pl.Fp;
     pl.Xs = b.take<__nv_bfloat16>((size_t)N * pl.ldxs);
-    pl.Ps = b.take<__nv_bfloat16>((size_t)D_eff * pl.ldps);
+    pl.Ps = pm.take<__nv_bfloat16>((size_t)D_eff * pl.ldps);
     return;
   }
   if (prec == HDC_I8) {
     pl.ldxs = pl.ldps = pl.Fp;
     if (!x_inplace) pl.Xs = b.take<int8_t>((size_t)N * pl.Fp);
-    if (!p_inplace) pl.Ps = b.take<int8_t>((size_t)D_eff * pl.Fp);
+    if (!p_inplace) pl.Ps = pm.take<int8_t>((size_t)D_eff * pl.Fp);
     return;
   }
   // BF16 / B1 / F16 (half operands are always staged: the inputs are fp32 or bf16)
@@ -158,12 +185,14 @@ void plan_encode(const hdc_ctx* h, int64_t N, int F, int D_eff, const hdc_knobs_
   if (prec == HDC_F16) x_inplace = p_inplace = false;
   pl.ldxs = pl.ldps = pl.Fp;
   if (!x_inplace) pl.Xs = b.take<__nv_bfloat16>((size_t)N * pl.Fp);
-  if (!p_inplace) pl.Ps = b.take<__nv_bfloat16>((size_t)D_eff * pl.Fp);
+  if (!p_inplace) pl.Ps = pm.take<__nv_bfloat16>((size_t)D_eff * pl.Fp);
 }
 
 // infer (nullable): the epilogue of the fused inference kernel (EPI_INFER: labels, class operand, scales); the
 // contraction then signs, optionally packs (Hbits may be NULL) and classifies in one kernel.  Only the
 // tensor-core path has it: the caller checks infer_fusable() first.
+// Order in every branch: stage P (persistent; skipped when a prepared model is used), return if only
+// preparing, stage X, contract.
 int encode_rp_core(hdc_ctx* h, const void* X, int x_dtype, int64_t N, int F, int64_t ldx, const void* P,
                    int p_dtype, int64_t ldp, const hdc_knobs_t* k, int out_kinds, uint32_t* Hbits,
                    int64_t ldh, void* Hraw, int64_t ldraw, Bump& b, size_t ws_bytes, cudaStream_t st,
@@ -186,51 +215,63 @@ int encode_rp_core(hdc_ctx* h, const void* X, int x_dtype, int64_t N, int F, int
     h->err = std::string(what) + ": tensor-core kernel refused the operands, CUDA-core kernel used";
     return HDC_OK;
   };
+  // runs the tensor-core contraction; HDC_OK, an error, or 1 = refused (fall through to the CUDA cores)
+  auto contract_tc = [&](const TcOperands& o, const char* what) -> int {
+    cudaError_t ce;
+    {
+      Timed tm(h, HDC_K_ENCODE_GEMM, st);
+      ce = launch_gemm_tc(h->tc, o, N, D_eff, e, h->sm_count, tc_cta_group(k), st, &h->launches);
+    }
+    if (ce == cudaSuccess) {
+      ++h->stats[HDC_STAT_TC_LAUNCHES];
+      return HDC_OK;
+    }
+    if (ce != cudaErrorNotSupported) return cuda_fail(h, ce, what);
+    if (int rc = tc_refused(what)) return rc;
+    return 1;
+  };
   const int xk = x_dtype == HDC_BF16 ? OPK_BF16 : OPK_F32;
   const int pk = p_dtype == HDC_BF16 ? OPK_BF16 : (p_dtype == HDC_I8 ? OPK_I8 : OPK_F32);
+  const bool modelled = h->model != nullptr;   // P must then be staged into the model, never used in place
   cudaError_t ce;
   EncodePlan pl;
+  Bump& pm = persistent(h, b);
 
   if (prec == HDC_F32) {
-    plan_encode(h, N, F, D_eff, k, false, false, b, pl);
-    if (b.off > ws_bytes) return fail(h, HDC_ERR_WORKSPACE, "encode_rp: workspace too small");
+    plan_encode(h, N, F, D_eff, k, false, false, b, pm, pl);
+    if (!persistent_fits(h, b, ws_bytes)) return fail(h, HDC_ERR_WORKSPACE, "encode_rp: workspace too small");
     if (pl.tc && (k->flags & HDC_FLAG_F32_FAST)) {
-      ce = launch_split2_f16(X, xk, N, F, ldx, (__half*)pl.Xs, pl.Fp, pl.ex, st, &h->launches);
-      if (ce != cudaSuccess) return cuda_fail(h, ce, "split X");
-      if (!h->reuse_prep) {
+      if (do_prep(h)) {
         ce = launch_split2_f16(P, pk, D_eff, F, ldp, (__half*)pl.Ps, pl.Fp, pl.ep, st, &h->launches);
         if (ce != cudaSuccess) return cuda_fail(h, ce, "split P");
       }
+      if (prep_only(h)) return HDC_OK;
+      ce = launch_split2_f16(X, xk, N, F, ldx, (__half*)pl.Xs, pl.Fp, pl.ex, st, &h->launches);
+      if (ce != cudaSuccess) return cuda_fail(h, ce, "split X");
       TcOperands o{pl.Xs, pl.Ps, OPK_F16, pl.ldxs, pl.ldps, pl.ldxs, pl.ldps, pl.Fp, 3,
                    SPLIT2_A_SEGS, SPLIT2_B_SEGS, pl.Fp};
-      {
-        Timed tm(h, HDC_K_ENCODE_GEMM, st);
-        ce = launch_gemm_tc(h->tc, o, N, D_eff, e, h->sm_count, tc_cta_group(k), st, &h->launches);
-      }
-      if (ce == cudaSuccess && want_raw)
+      int rc = contract_tc(o, "encode_rp fp32 (2 x fp16) tcgen05");
+      if (rc == HDC_OK && want_raw) {
         ce = launch_unscale_raw((float*)Hraw, N, D_eff, ldraw, pl.ex, pl.ep, st, &h->launches);
-      if (ce == cudaSuccess) { ++h->stats[HDC_STAT_TC_LAUNCHES]; return HDC_OK; }
-      if (ce != cudaErrorNotSupported) return cuda_fail(h, ce, "encode_rp fp32 (2 x fp16) tcgen05");
-      if (int rc = tc_refused("encode_rp fp32 (2 x fp16) tcgen05")) return rc;
+        if (ce != cudaSuccess) return cuda_fail(h, ce, "unscale raw");
+      }
+      if (rc <= 0) return rc;
       pl.tc = false;  // the workspace was planned for the 2-way split: go straight to the CUDA-core kernel
     }
     if (pl.tc) {
-      ce = launch_split3_bf16(X, xk, N, F, ldx, (__nv_bfloat16*)pl.Xs, pl.Fp, st, &h->launches);
-      if (ce != cudaSuccess) return cuda_fail(h, ce, "split X");
-      if (!h->reuse_prep) {
+      if (do_prep(h)) {
         ce = launch_split3_bf16(P, pk, D_eff, F, ldp, (__nv_bfloat16*)pl.Ps, pl.Fp, st, &h->launches);
         if (ce != cudaSuccess) return cuda_fail(h, ce, "split P");
       }
+      if (prep_only(h)) return HDC_OK;
+      ce = launch_split3_bf16(X, xk, N, F, ldx, (__nv_bfloat16*)pl.Xs, pl.Fp, st, &h->launches);
+      if (ce != cudaSuccess) return cuda_fail(h, ce, "split X");
       TcOperands o{pl.Xs, pl.Ps, OPK_BF16, pl.ldxs, pl.ldps, pl.ldxs, pl.ldps, pl.Fp, 6,
                    SPLIT_A_SEGS, SPLIT_B_SEGS, pl.Fp};
-      {
-        Timed tm(h, HDC_K_ENCODE_GEMM, st);
-        ce = launch_gemm_tc(h->tc, o, N, D_eff, e, h->sm_count, tc_cta_group(k), st, &h->launches);
-      }
-      if (ce == cudaSuccess) { ++h->stats[HDC_STAT_TC_LAUNCHES]; return HDC_OK; }
-      if (ce != cudaErrorNotSupported) return cuda_fail(h, ce, "encode_rp fp32 tcgen05");
-      if (int rc = tc_refused("encode_rp fp32 tcgen05")) return rc;
+      int rc = contract_tc(o, "encode_rp fp32 tcgen05");
+      if (rc <= 0) return rc;
     }
+    if (prep_only(h)) return HDC_OK;  // the CUDA-core kernel reads P in place
     {
       Timed tm(h, HDC_K_ENCODE_GEMM, st);
       ce = launch_gemm_simt(Operand{X, ldx, xk}, Operand{P, ldp, pk}, N, D_eff, F, false, e, st, &h->launches);
@@ -239,32 +280,28 @@ int encode_rp_core(hdc_ctx* h, const void* X, int x_dtype, int64_t N, int F, int
   }
 
   const bool tc_ok_x = x_dtype == HDC_BF16 && (ldx % 8) == 0 && aligned16(X);
-  const bool tc_ok_p = p_dtype == HDC_BF16 && (ldp % 8) == 0 && aligned16(P);
+  const bool tc_ok_p = !modelled && p_dtype == HDC_BF16 && (ldp % 8) == 0 && aligned16(P);
   if (prec == HDC_I8) {
-    const bool p_in = p_dtype == HDC_I8 && (ldp % 16) == 0 && aligned16(P);
-    plan_encode(h, N, F, D_eff, k, false, p_in, b, pl);
-    if (b.off > ws_bytes) return fail(h, HDC_ERR_WORKSPACE, "encode_rp: workspace too small");
-    ce = launch_quantize_rows_i8(X, xk, N, F, ldx, (int8_t*)pl.Xs, pl.ldxs, st, &h->launches);
-    if (ce != cudaSuccess) return cuda_fail(h, ce, "quantize X");
+    const bool p_in = !modelled && p_dtype == HDC_I8 && (ldp % 16) == 0 && aligned16(P);
+    plan_encode(h, N, F, D_eff, k, false, p_in, b, pm, pl);
+    if (!persistent_fits(h, b, ws_bytes)) return fail(h, HDC_ERR_WORKSPACE, "encode_rp: workspace too small");
     const void* Pq = P;
     int64_t ldpq = ldp;
     if (!p_in) {
-      if (!h->reuse_prep) {
+      if (do_prep(h)) {
         ce = launch_quantize_rows_i8(P, pk, D_eff, F, ldp, (int8_t*)pl.Ps, pl.ldps, st, &h->launches);
         if (ce != cudaSuccess) return cuda_fail(h, ce, "quantize P");
       }
       Pq = pl.Ps;
       ldpq = pl.ldps;
     }
+    if (prep_only(h)) return HDC_OK;
+    ce = launch_quantize_rows_i8(X, xk, N, F, ldx, (int8_t*)pl.Xs, pl.ldxs, st, &h->launches);
+    if (ce != cudaSuccess) return cuda_fail(h, ce, "quantize X");
     if (pl.tc) {
       TcOperands o{pl.Xs, Pq, OPK_I8, pl.ldxs, ldpq, F, F, F, 1, 0u, 0u, 0};
-      {
-        Timed tm(h, HDC_K_ENCODE_GEMM, st);
-        ce = launch_gemm_tc(h->tc, o, N, D_eff, e, h->sm_count, tc_cta_group(k), st, &h->launches);
-      }
-      if (ce == cudaSuccess) { ++h->stats[HDC_STAT_TC_LAUNCHES]; return HDC_OK; }
-      if (ce != cudaErrorNotSupported) return cuda_fail(h, ce, "encode_rp int8 tcgen05");
-      if (int rc = tc_refused("encode_rp int8 tcgen05")) return rc;
+      int rc = contract_tc(o, "encode_rp int8 tcgen05");
+      if (rc <= 0) return rc;
     }
     ce = launch_gemm_simt(Operand{pl.Xs, pl.ldxs, OPK_I8}, Operand{Pq, ldpq, OPK_I8}, N, D_eff, F, true, e,
                           st, &h->launches);
@@ -272,24 +309,21 @@ int encode_rp_core(hdc_ctx* h, const void* X, int x_dtype, int64_t N, int F, int
   }
 
   if (prec == HDC_F16) {
-    plan_encode(h, N, F, D_eff, k, false, false, b, pl);
-    if (b.off > ws_bytes) return fail(h, HDC_ERR_WORKSPACE, "encode_rp: workspace too small");
+    plan_encode(h, N, F, D_eff, k, false, false, b, pm, pl);
+    if (!persistent_fits(h, b, ws_bytes)) return fail(h, HDC_ERR_WORKSPACE, "encode_rp: workspace too small");
     if (pl.tc) {
-      ce = launch_convert_f16(X, xk, N, F, ldx, (__half*)pl.Xs, pl.ldxs, st, &h->launches);
-      if (ce != cudaSuccess) return cuda_fail(h, ce, "convert X");
-      if (!h->reuse_prep) {
+      if (do_prep(h)) {
         ce = launch_convert_f16(P, pk, D_eff, F, ldp, (__half*)pl.Ps, pl.ldps, st, &h->launches);
         if (ce != cudaSuccess) return cuda_fail(h, ce, "convert P");
       }
+      if (prep_only(h)) return HDC_OK;
+      ce = launch_convert_f16(X, xk, N, F, ldx, (__half*)pl.Xs, pl.ldxs, st, &h->launches);
+      if (ce != cudaSuccess) return cuda_fail(h, ce, "convert X");
       TcOperands o{pl.Xs, pl.Ps, OPK_F16, pl.ldxs, pl.ldps, F, F, F, 1, 0u, 0u, 0};
-      {
-        Timed tm(h, HDC_K_ENCODE_GEMM, st);
-        ce = launch_gemm_tc(h->tc, o, N, D_eff, e, h->sm_count, tc_cta_group(k), st, &h->launches);
-      }
-      if (ce == cudaSuccess) { ++h->stats[HDC_STAT_TC_LAUNCHES]; return HDC_OK; }
-      if (ce != cudaErrorNotSupported) return cuda_fail(h, ce, "encode_rp fp16 tcgen05");
-      if (int rc = tc_refused("encode_rp fp16 tcgen05")) return rc;
+      int rc = contract_tc(o, "encode_rp fp16 tcgen05");
+      if (rc <= 0) return rc;
     }
+    if (prep_only(h)) return HDC_OK;
     const int xr = x_dtype == HDC_BF16 ? OPK_BF16_RF16 : OPK_F32_RF16;
     const int pr = p_dtype == HDC_BF16 ? OPK_BF16_RF16 : OPK_F32_RF16;
     ce = launch_gemm_simt(Operand{X, ldx, xr}, Operand{P, ldp, pr}, N, D_eff, F, false, e, st, &h->launches);
@@ -297,35 +331,32 @@ int encode_rp_core(hdc_ctx* h, const void* X, int x_dtype, int64_t N, int F, int
   }
 
   // BF16 / B1
-  plan_encode(h, N, F, D_eff, k, tc_ok_x, tc_ok_p, b, pl);
-  if (b.off > ws_bytes) return fail(h, HDC_ERR_WORKSPACE, "encode_rp: workspace too small");
+  plan_encode(h, N, F, D_eff, k, tc_ok_x, tc_ok_p, b, pm, pl);
+  if (!persistent_fits(h, b, ws_bytes)) return fail(h, HDC_ERR_WORKSPACE, "encode_rp: workspace too small");
   if (pl.tc) {
     const void* Xb = X;
     const void* Pb = P;
     int64_t ldxb = ldx, ldpb = ldp;
-    if (!tc_ok_x) {
-      ce = launch_convert_bf16(X, xk, N, F, ldx, (__nv_bfloat16*)pl.Xs, pl.ldxs, st, &h->launches);
-      if (ce != cudaSuccess) return cuda_fail(h, ce, "convert X");
-      Xb = pl.Xs;
-      ldxb = pl.ldxs;
-    }
     if (!tc_ok_p) {
-      if (!h->reuse_prep) {
+      if (do_prep(h)) {
         ce = launch_convert_bf16(P, pk, D_eff, F, ldp, (__nv_bfloat16*)pl.Ps, pl.ldps, st, &h->launches);
         if (ce != cudaSuccess) return cuda_fail(h, ce, "convert P");
       }
       Pb = pl.Ps;
       ldpb = pl.ldps;
     }
-    TcOperands o{Xb, Pb, OPK_BF16, ldxb, ldpb, F, F, F, 1, 0u, 0u, 0};
-    {
-      Timed tm(h, HDC_K_ENCODE_GEMM, st);
-      ce = launch_gemm_tc(h->tc, o, N, D_eff, e, h->sm_count, tc_cta_group(k), st, &h->launches);
+    if (prep_only(h)) return HDC_OK;
+    if (!tc_ok_x) {
+      ce = launch_convert_bf16(X, xk, N, F, ldx, (__nv_bfloat16*)pl.Xs, pl.ldxs, st, &h->launches);
+      if (ce != cudaSuccess) return cuda_fail(h, ce, "convert X");
+      Xb = pl.Xs;
+      ldxb = pl.ldxs;
     }
-    if (ce == cudaSuccess) { ++h->stats[HDC_STAT_TC_LAUNCHES]; return HDC_OK; }
-    if (ce != cudaErrorNotSupported) return cuda_fail(h, ce, "encode_rp bf16 tcgen05");
-      if (int rc = tc_refused("encode_rp bf16 tcgen05")) return rc;
+    TcOperands o{Xb, Pb, OPK_BF16, ldxb, ldpb, F, F, F, 1, 0u, 0u, 0};
+    int rc = contract_tc(o, "encode_rp bf16 tcgen05");
+    if (rc <= 0) return rc;
   }
+  if (prep_only(h)) return HDC_OK;
   const int xr = x_dtype == HDC_BF16 ? OPK_BF16 : OPK_F32_RBF16;
   const int pr = p_dtype == HDC_BF16 ? OPK_BF16 : OPK_F32_RBF16;
   ce = launch_gemm_simt(Operand{X, ldx, xr}, Operand{P, ldp, pr}, N, D_eff, F, false, e, st, &h->launches);
@@ -334,16 +365,19 @@ int encode_rp_core(hdc_ctx* h, const void* X, int x_dtype, int64_t N, int F, int
 
 // Workspace of hdc_encode_rp: the compacted operands of a perforated contraction (upper bound: 4-byte
 // elements) followed by the staging buffers of the contraction itself.
-void encode_ws(const hdc_ctx* h, int64_t N, int F, int D_eff, const hdc_knobs_t* k, Bump& b) {
+void encode_ws(const hdc_ctx* h, int64_t N, int F, int D_eff, const hdc_knobs_t* k, Bump& b, Bump& pm) {
   const Perf ef = enc_perf_of(k);
   if (perf_on(ef)) {
     F = perf_count(ef, F);
     const int64_t ldg = round_up(F, 16);
     b.take<float>((size_t)N * ldg);
-    b.take<float>((size_t)D_eff * ldg);
+    pm.take<float>((size_t)D_eff * ldg);
   }
   EncodePlan pl;
-  plan_encode(h, N, F, D_eff, k, false, false, b, pl);
+  plan_encode(h, N, F, D_eff, k, false, false, b, pm, pl);
+}
+void encode_ws(const hdc_ctx* h, int64_t N, int F, int D_eff, const hdc_knobs_t* k, Bump& b) {
+  encode_ws(h, N, F, D_eff, k, b, b);
 }
 
 // hdc_encode_rp after argument checks.  A perforated F reduction (knobs enc_perf_*; PAPER.md L155,
@@ -362,22 +396,26 @@ int do_encode_rp(hdc_ctx* h, const void* X, int x_dtype, int64_t N, int F, int64
   const int64_t ldg = round_up(Fv, 16);
   const int xs = x_dtype == HDC_BF16 ? 2 : 4;
   const int ps = p_dtype == HDC_BF16 ? 2 : (p_dtype == HDC_I8 ? 1 : 4);
+  Bump& pm = persistent(h, b);
   void* Xg = b.take<uint8_t>((size_t)N * ldg * xs);
-  void* Pg = b.take<uint8_t>((size_t)D_eff * ldg * ps);
+  void* Pg = pm.take<uint8_t>((size_t)D_eff * ldg * (h->model ? 4 : ps));  // a model reserves the 4-byte bound (encode_ws)
   {  // the whole workspace is checked before the first launch
-    Bump dry(nullptr);
+    Bump dry(nullptr), dry_pm(nullptr);
     dry.off = b.off;
+    dry_pm.off = pm.off;
     EncodePlan pl;
-    plan_encode(h, N, Fv, D_eff, k, false, false, dry, pl);
-    if (dry.off > ws_bytes) return fail(h, HDC_ERR_WORKSPACE, "encode_rp: workspace too small");
+    plan_encode(h, N, Fv, D_eff, k, false, false, dry, h->model ? dry_pm : dry, pl);
+    if (dry.off > ws_bytes || (h->model && dry_pm.off > h->model_cap))
+      return fail(h, HDC_ERR_WORKSPACE, "encode_rp: workspace too small");
   }
-  cudaError_t ce = launch_gather_cols(X, xs, N, ldx, ef, Fv, Xg, ldg, st, &h->launches);
+  cudaError_t ce = cudaSuccess;
+  if (!prep_only(h)) ce = launch_gather_cols(X, xs, N, ldx, ef, Fv, Xg, ldg, st, &h->launches);
   if (ce != cudaSuccess) return cuda_fail(h, ce, "gather X");
-  ce = launch_gather_cols(P, ps, D_eff, ldp, ef, Fv, Pg, ldg, st, &h->launches);
+  if (do_prep(h)) ce = launch_gather_cols(P, ps, D_eff, ldp, ef, Fv, Pg, ldg, st, &h->launches);
   if (ce != cudaSuccess) return cuda_fail(h, ce, "gather P");
   int rc = encode_rp_core(h, Xg, x_dtype, N, Fv, ldg, Pg, p_dtype, ldg, k, out_kinds, Hbits, ldh, Hraw, ldraw, b,
                           ws_bytes, st);
-  if (rc != HDC_OK || !(out_kinds & HDC_OUT_RAW)) return rc;
+  if (rc != HDC_OK || !(out_kinds & HDC_OUT_RAW) || prep_only(h)) return rc;
   const float scale = (float)((double)F / (double)Fv);
   ce = launch_scale_raw(Hraw, N, D_eff, ldraw, scale, k->precision == HDC_I8, st, &h->launches);
   return ce == cudaSuccess ? HDC_OK : cuda_fail(h, ce, "scale raw");
@@ -393,22 +431,25 @@ int do_similarity(hdc_ctx* h, const uint32_t* Hbits, int64_t N, int64_t ldh, con
   const Perf pf = perf_of(k);
   const int n_vis = perf_count(pf, D_eff);  // dimensions the reduction visits (= D_eff unless perforated)
   cudaError_t ce;
+  Bump& pm = persistent(h, b);   // class operand, scales, masks: per-call-invariant (prepared-model modes)
+  bool prep = do_prep(h);
+  auto too_small = [&]() { return fail(h, HDC_ERR_WORKSPACE, "similarity: workspace too small"); };
   // tensor-core path from packed queries: DOT / COS at any K; Hamming once K is large enough that
   // the popcount pipe would bound it (dist = (D_eff - dot)/2 is exact in int32)
   if (use_tc(h, k) && (k->sim != HDC_SIM_HAMMING || K >= 64)) {
     double* colscale = nullptr;
-    if (k->sim == HDC_SIM_COS) colscale = b.take<double>((size_t)K);
-    float* amax = b.take<float>(1);
-    void* cop = b.take<uint8_t>(sim_tc_operand_bytes(K, k->hv_bits, D_eff));
+    if (k->sim == HDC_SIM_COS) colscale = pm.take<double>((size_t)K);
+    float* amax = pm.take<float>(1);
+    void* cop = pm.take<uint8_t>(sim_tc_operand_bytes(K, k->hv_bits, D_eff));
+    int8_t* Cq = nullptr;
+    const int64_t ldq = round_up(D_eff, 16);
+    if (colscale && k->hv_bits == 8) Cq = pm.take<int8_t>((size_t)K * ldq);
     const size_t pbytes = sim_tc_partial_bytes(N, K, k->hv_bits, D_eff, h->sm_count);
     double* partial = pbytes ? b.take<double>(pbytes / sizeof(double)) : nullptr;
-    if (b.off > ws_bytes) return fail(h, HDC_ERR_WORKSPACE, "similarity: workspace too small");
-    if (colscale && !h->reuse_prep) {
+    if (!persistent_fits(h, b, ws_bytes)) return too_small();
+    if (colscale && prep) {
       // norms over the operand as the contraction sees it (permutation-invariant)
       if (k->hv_bits == 8) {
-        const int64_t ldq = round_up(D_eff, 16);
-        int8_t* Cq = b.take<int8_t>((size_t)K * ldq);
-        if (b.off > ws_bytes) return fail(h, HDC_ERR_WORKSPACE, "similarity: workspace too small");
         ce = launch_quantize_tensor_i8(C_acc, K, D_eff, ldc, pf, Cq, ldq, amax, st, &h->launches);
         if (ce != cudaSuccess) return cuda_fail(h, ce, "quantize C");
         ce = launch_col_scale(Operand{Cq, ldq, OPK_I8}, K, D_eff, 1, pf, colscale, st, &h->launches);
@@ -438,27 +479,25 @@ int do_similarity(hdc_ctx* h, const uint32_t* Hbits, int64_t N, int64_t ldh, con
     {
       Timed tm(h, HDC_K_SIM, st);
       ce = launch_sim_tc(h->tc, Hbits, N, ldh, C_acc, K, ldc, D_eff, k->hv_bits, cop, amax, e, pf, partial,
-                         h->reuse_prep, h->sm_count, st, &h->launches);
+                         !prep, prep_only(h), h->sm_count, st, &h->launches);
     }
     if (ce == cudaSuccess) return HDC_OK;
     if (ce != cudaErrorNotSupported) return cuda_fail(h, ce, "similarity tcgen05");
+    prep = true;  // the CUDA-core kernels below take other operand forms: prepare them here
   }
   if (k->sim == HDC_SIM_HAMMING) {
-    uint32_t* cbits = b.take<uint32_t>((size_t)K * W);
-    if (b.off > ws_bytes) return fail(h, HDC_ERR_WORKSPACE, "similarity: workspace too small");
-    if (!h->reuse_prep) {
+    uint32_t* cbits = pm.take<uint32_t>((size_t)K * W);
+    uint32_t* pmask = perf_on(pf) ? pm.take<uint32_t>((size_t)W) : nullptr;
+    if (!persistent_fits(h, b, ws_bytes)) return too_small();
+    if (prep) {
       ce = launch_sign_bits(C_acc, K, D_eff, ldc, cbits, W, st, &h->launches);
       if (ce != cudaSuccess) return cuda_fail(h, ce, "sign_bits");
-    }
-    uint32_t* pmask = nullptr;
-    if (perf_on(pf)) {
-      pmask = b.take<uint32_t>((size_t)W);
-      if (b.off > ws_bytes) return fail(h, HDC_ERR_WORKSPACE, "similarity: workspace too small");
-      if (!h->reuse_prep) {
+      if (pmask) {
         ce = launch_perf_mask(pmask, W, D_eff, pf, st, &h->launches);
         if (ce != cudaSuccess) return cuda_fail(h, ce, "perforation mask");
       }
     }
+    if (prep_only(h)) return HDC_OK;
     {
       Timed tm(h, HDC_K_SIM, st);
       ce = launch_hamming(Hbits, N, ldh, cbits, K, W, D_eff, pmask, (int32_t*)S, lds, labels, best, second,
@@ -471,7 +510,7 @@ int do_similarity(hdc_ctx* h, const uint32_t* Hbits, int64_t N, int64_t ldh, con
   Operand B{};
   bool int_acc = false;
   double* colscale = nullptr;
-  if (k->sim == HDC_SIM_COS) colscale = b.take<double>((size_t)K);
+  if (k->sim == HDC_SIM_COS) colscale = pm.take<double>((size_t)K);
   if (k->hv_bits == 32) {
     B = Operand{C_acc, ldc, OPK_F32};
   } else if (k->hv_bits == 16) {
@@ -480,26 +519,31 @@ int do_similarity(hdc_ctx* h, const uint32_t* Hbits, int64_t N, int64_t ldh, con
     B = Operand{C_acc, ldc, OPK_F32_RF16};
   } else if (k->hv_bits == 8) {
     const int64_t ldq = round_up(D_eff, 16);
-    int8_t* Cq = b.take<int8_t>((size_t)K * ldq);
-    float* amax = b.take<float>(1);
-    if (b.off > ws_bytes) return fail(h, HDC_ERR_WORKSPACE, "similarity: workspace too small");
-    ce = launch_quantize_tensor_i8(C_acc, K, D_eff, ldc, pf, Cq, ldq, amax, st, &h->launches);
-    if (ce != cudaSuccess) return cuda_fail(h, ce, "quantize C");
+    int8_t* Cq = pm.take<int8_t>((size_t)K * ldq);
+    float* amax = pm.take<float>(1);
+    if (!persistent_fits(h, b, ws_bytes)) return too_small();
+    if (prep) {
+      ce = launch_quantize_tensor_i8(C_acc, K, D_eff, ldc, pf, Cq, ldq, amax, st, &h->launches);
+      if (ce != cudaSuccess) return cuda_fail(h, ce, "quantize C");
+    }
     B = Operand{Cq, ldq, OPK_I8};
     int_acc = true;
   } else {
-    uint32_t* cbits = b.take<uint32_t>((size_t)K * W);
-    if (b.off > ws_bytes) return fail(h, HDC_ERR_WORKSPACE, "similarity: workspace too small");
-    ce = launch_sign_bits(C_acc, K, D_eff, ldc, cbits, W, st, &h->launches);
-    if (ce != cudaSuccess) return cuda_fail(h, ce, "sign_bits");
+    uint32_t* cbits = pm.take<uint32_t>((size_t)K * W);
+    if (!persistent_fits(h, b, ws_bytes)) return too_small();
+    if (prep) {
+      ce = launch_sign_bits(C_acc, K, D_eff, ldc, cbits, W, st, &h->launches);
+      if (ce != cudaSuccess) return cuda_fail(h, ce, "sign_bits");
+    }
     B = Operand{cbits, W, OPK_BITS};
     int_acc = true;
   }
-  if (b.off > ws_bytes) return fail(h, HDC_ERR_WORKSPACE, "similarity: workspace too small");
-  if (colscale) {
+  if (!persistent_fits(h, b, ws_bytes)) return too_small();
+  if (colscale && prep) {
     ce = launch_col_scale(B, K, D_eff, 1, pf, colscale, st, &h->launches);
     if (ce != cudaSuccess) return cuda_fail(h, ce, "col_scale");
   }
+  if (prep_only(h)) return HDC_OK;
   Epilogue e{};
   e.colscale = colscale;
   if (labels) {
@@ -515,6 +559,19 @@ int do_similarity(hdc_ctx* h, const uint32_t* Hbits, int64_t N, int64_t ldh, con
   }
   ce = launch_gemm_simt(Operand{Hbits, ldh, OPK_BITS}, B, N, K, D_eff, int_acc, e, st, &h->launches);
   return ce == cudaSuccess ? HDC_OK : cuda_fail(h, ce, "similarity contraction");
+}
+
+// persistent operands of do_similarity (upper bound over its paths)
+void similarity_model_ws(int K, const hdc_knobs_t* k, Bump& pm) {
+  const int W = words_of(k->D_eff);
+  pm.take<double>((size_t)K);
+  pm.take<float>(1);
+  pm.take<int8_t>((size_t)K * round_up(k->D_eff, 16));
+  pm.take<uint32_t>((size_t)K * W);
+  pm.take<uint32_t>((size_t)W);  // perforation mask
+  pm.take<uint8_t>(sim_tc_operand_bytes(K, k->hv_bits == 32 || k->hv_bits == 16 || k->hv_bits == HDC_HV_F16 ||
+                                               k->hv_bits == 8 ? k->hv_bits : 1,
+                                        k->D_eff));
 }
 
 size_t similarity_ws(int64_t N, int K, const hdc_knobs_t* k) {
@@ -574,12 +631,13 @@ int do_infer_rp(hdc_ctx* h, const void* X, int x_dtype, int64_t N, int F, int64_
     const int KC = infer_kc(K);
     const int64_t ldcls = round_up(D_eff, 256);
     const Perf pf = perf_of(k);
-    float* cls = b.take<float>((size_t)KC * (size_t)ldcls);
-    double* colscale = b.take<double>((size_t)K);
-    float* amax = b.take<float>(1);
-    if (b.off > ws_bytes) return fail(h, HDC_ERR_WORKSPACE, "infer_rp: workspace too small");
+    Bump& pm = persistent(h, b);
+    float* cls = pm.take<float>((size_t)KC * (size_t)ldcls);
+    double* colscale = pm.take<double>((size_t)K);
+    float* amax = pm.take<float>(1);
+    if (!persistent_fits(h, b, ws_bytes)) return fail(h, HDC_ERR_WORKSPACE, "infer_rp: workspace too small");
     cudaError_t ce = cudaSuccess;
-    if (!h->reuse_prep) {
+    if (do_prep(h)) {
       if (k->hv_bits == 8) ce = launch_tensor_amax(C_acc, K, D_eff, ldc, pf, amax, st, &h->launches);
       if (ce == cudaSuccess)
         ce = launch_class_operand_f32(C_acc, K, D_eff, ldc, k->hv_bits, pf, amax, cls, KC, ldcls, st, &h->launches);
@@ -598,7 +656,7 @@ int do_infer_rp(hdc_ctx* h, const void* X, int x_dtype, int64_t N, int F, int64_
     e.K = K;
     int rc = encode_rp_core(h, X, x_dtype, N, F, ldx, P, p_dtype, ldp, k, HDC_OUT_BITS, Hbits, ldh, nullptr, 0, b,
                             ws_bytes, st, &e);
-    if (rc == HDC_OK) ++h->stats[HDC_STAT_INFER_FUSED];
+    if (rc == HDC_OK && !prep_only(h)) ++h->stats[HDC_STAT_INFER_FUSED];
     return rc;
   }
   uint32_t* Hd = Hbits;
@@ -612,7 +670,31 @@ int do_infer_rp(hdc_ctx* h, const void* X, int x_dtype, int64_t N, int F, int64_
                         ws_bytes, st);
   if (rc == HDC_OK)
     rc = do_similarity(h, Hd, N, ldhd, C_acc, K, ldc, k, nullptr, 0, 0, labels, best, second, b, ws_bytes, st);
-  if (rc == HDC_OK) ++h->stats[HDC_STAT_INFER_UNFUSED];
+  if (rc == HDC_OK && !prep_only(h)) ++h->stats[HDC_STAT_INFER_UNFUSED];
+  return rc;
+}
+
+// bytes of the persistent operands of encode (P staging) + similarity (class operand, scales, masks) + the
+// fused inference epilogue (fp32 class operand) for these sizes and knobs: the prepared-model blob
+size_t model_ws_bytes(const hdc_ctx* h, int F, int K, const hdc_knobs_t* k) {
+  Bump scratch(nullptr), pm(nullptr);
+  encode_ws(h, 0, F, k->D_eff, k, scratch, pm);
+  similarity_model_ws(K, k, pm);
+  infer_ws(K, k->D_eff, pm);
+  return pm.off + 1024;
+}
+
+// Runs `fn` with the persistent operands directed at [blob, blob + cap) in the given mode.
+template <typename Fn>
+int with_model(hdc_ctx* h, void* blob, size_t cap, int mode, Fn fn) {
+  Bump pm(blob);
+  h->model = &pm;
+  h->model_cap = cap;
+  h->prep_mode = mode;
+  const int rc = fn();
+  h->model = nullptr;
+  h->model_cap = 0;
+  h->prep_mode = PREP_AND_RUN;
   return rc;
 }
 
@@ -643,7 +725,7 @@ extern "C" int32_t hdc_create(hdc_handle_t* out, int32_t device) {
   }
   cudaDeviceProp prop;
   if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return HDC_ERR_CUDA;
-  if (prop.major != 10) return HDC_ERR_ARCH;
+  if (prop.major != 10 || prop.minor != 0) return HDC_ERR_ARCH;  // the library holds sm_100a code only (no forward compatibility)
   if (cudaSetDevice(device) != cudaSuccess) return HDC_ERR_CUDA;
   hdc_ctx* h = new hdc_ctx();
   h->device = device;
@@ -665,6 +747,7 @@ extern "C" int32_t hdc_create(hdc_handle_t* out, int32_t device) {
 
 extern "C" int32_t hdc_destroy(hdc_handle_t h) {
   if (!h) return HDC_ERR_INVALID_ARG;
+  DeviceGuard device_guard(h->device);
   for (int i = 0; i < 2; ++i) {
     if (h->ev_copied[i]) cudaEventDestroy(h->ev_copied[i]);
     if (h->ev_done[i]) cudaEventDestroy(h->ev_done[i]);
@@ -692,6 +775,7 @@ extern "C" int64_t hdc_stat(hdc_handle_t h, int32_t stat_id) {
 
 extern "C" int32_t hdc_kernel_timing(hdc_handle_t h, int32_t enable) {
   if (!h) return HDC_ERR_INVALID_ARG;
+  DeviceGuard device_guard(h->device);
   h->timing = enable != 0;
   for (auto& u : h->tused) u = 0;
   return HDC_OK;
@@ -721,6 +805,8 @@ extern "C" size_t hdc_workspace_bytes(hdc_handle_t h, int32_t op, int64_t N, int
   if (!h || !knobs || N < 0) return 0;
   hdc_knobs_t k = *knobs;
   if (k.D_eff < 1 || k.D_eff > D) k.D_eff = D;
+  if (K < 1) K = 1;  // sizes only: a bad K is reported by the call itself
+  if (k.D_eff < 1) return 0;
   Bump b(nullptr);
   switch (op) {
     case HDC_OP_ENCODE_RP: {
@@ -745,6 +831,7 @@ extern "C" size_t hdc_workspace_bytes(hdc_handle_t h, int32_t op, int64_t N, int
       b.take<float>((size_t)chunk * F_or_Q);  // two staging buffers for X (fp32 upper bound)
       b.take<float>((size_t)chunk * F_or_Q);
       b.take<int32_t>((size_t)N);
+      b.take<uint8_t>(model_ws_bytes(h, F_or_Q, K, &k));
       return b.off + 512 + infer_ws_bytes(h, chunk, F_or_Q, K, &k);
     }
     default:
@@ -781,6 +868,7 @@ extern "C" int32_t hdc_encode_rp(hdc_handle_t h, const void* X, int32_t x_dtype,
                                  int64_t ldh_words, void* Hraw, int64_t ldraw, void* ws, size_t ws_bytes,
                                  void* stream) {
   if (!h) return HDC_ERR_INVALID_ARG;
+  DeviceGuard device_guard(h->device);
   int rc = check_encode_rp_args(h, X, x_dtype, N, F, ldx, P, p_dtype, D, ldp, knobs);
   if (rc) return rc;
   if (!(out_kinds & HDC_OUT_BITS) || (!Hbits && N > 0))
@@ -802,6 +890,7 @@ static int32_t encode_levelid_impl(hdc_handle_t h, const void* levels, int lvl16
                                    int64_t ldlv_words, int32_t D, const hdc_knobs_t* knobs, uint32_t* Hbits,
                                    int64_t ldh_words, void* stream) {
   if (!h) return HDC_ERR_INVALID_ARG;
+  DeviceGuard device_guard(h->device);
   if (((!levels || !Hbits) && N > 0) || !IDbits || !LVbits)
     return fail(h, HDC_ERR_INVALID_ARG, "encode_levelid: NULL pointer");
   if (N < 0 || F < 1 || F > 65535 || Q < 1 || Q > (lvl16 ? 65535 : 256) || D < 1 || ldl < F)
@@ -823,6 +912,9 @@ static int32_t encode_levelid_impl(hdc_handle_t h, const void* levels, int lvl16
     ce = launch_levelid(levels, lvl16, N, F, ldl, IDbits, ldid_words, LVbits, Q, ldlv_words, knobs->D_eff, Hbits,
                         ldh_words, h->sm_count, h->smem_optin, (cudaStream_t)stream, &h->launches);
   }
+  if (ce == cudaErrorNotSupported)
+    return fail(h, HDC_ERR_UNSUPPORTED, "encode_levelid: F too large (a batch of level rows must fit in shared memory: "
+                                        "about 7000 features with 8-bit, 3500 with 16-bit level indices)");
   return ce == cudaSuccess ? HDC_OK : cuda_fail(h, ce, "encode_levelid");
 }
 
@@ -868,6 +960,7 @@ extern "C" int32_t hdc_similarity(hdc_handle_t h, const uint32_t* Hbits, int64_t
                                   const hdc_knobs_t* knobs, void* S, int32_t s_dtype, int64_t lds, void* ws,
                                   size_t ws_bytes, void* stream) {
   if (!h) return HDC_ERR_INVALID_ARG;
+  DeviceGuard device_guard(h->device);
   int rc = check_sim_args(h, Hbits, N, ldh_words, C_acc, K, ldc, D, knobs);
   if (rc) return rc;
   if ((!S && N > 0) || lds < K) return fail(h, HDC_ERR_INVALID_ARG, "similarity: S / lds");
@@ -891,6 +984,7 @@ extern "C" int32_t hdc_similarity_adc(hdc_handle_t h, const uint32_t* Hbits, int
                                       const hdc_knobs_t* knobs, const hdc_adc_t* adc, int32_t* S, int64_t lds,
                                       int32_t* labels, void* ws, size_t ws_bytes, void* stream) {
   if (!h) return HDC_ERR_INVALID_ARG;
+  DeviceGuard device_guard(h->device);
   if ((!Hbits && N > 0) || !C_acc || !adc) return fail(h, HDC_ERR_INVALID_ARG, "similarity_adc: NULL operand");
   if (N < 0 || K < 1 || K > 65535 || D < 1 || ldc < D) return fail(h, HDC_ERR_INVALID_ARG, "similarity_adc: bad sizes");
   int rc = check_knobs(h, knobs, D);
@@ -941,6 +1035,7 @@ extern "C" int32_t hdc_classify(hdc_handle_t h, const uint32_t* Hbits, int64_t N
                                 const hdc_knobs_t* knobs, int32_t* labels, float* best, float* second,
                                 void* ws, size_t ws_bytes, void* stream) {
   if (!h) return HDC_ERR_INVALID_ARG;
+  DeviceGuard device_guard(h->device);
   int rc = check_sim_args(h, Hbits, N, ldh_words, C_acc, K, ldc, D, knobs);
   if (rc) return rc;
   if (!labels && N > 0) return fail(h, HDC_ERR_INVALID_ARG, "classify: labels is NULL");
@@ -957,6 +1052,7 @@ extern "C" int32_t hdc_train_epoch(hdc_handle_t h, int32_t mode, const uint32_t*
                                    int32_t D, const hdc_knobs_t* knobs, float lr, int64_t batch, int32_t* pred,
                                    unsigned long long* n_wrong, void* ws, size_t ws_bytes, void* stream) {
   if (!h) return HDC_ERR_INVALID_ARG;
+  DeviceGuard device_guard(h->device);
   if (mode != HDC_TRAIN_BUNDLE && mode != HDC_TRAIN_PERCEPTRON && mode != HDC_TRAIN_KMEANS)
     return fail(h, HDC_ERR_INVALID_ARG, "train: mode");
   if (!y && N > 0 && mode != HDC_TRAIN_KMEANS) return fail(h, HDC_ERR_INVALID_ARG, "train: y is NULL");
@@ -1028,6 +1124,7 @@ extern "C" int32_t hdc_train_delta(hdc_handle_t h, const uint32_t* Hbits, int64_
                                    const hdc_knobs_t* knobs, int32_t* delta, int32_t* pred,
                                    unsigned long long* n_wrong, void* ws, size_t ws_bytes, void* stream) {
   if (!h) return HDC_ERR_INVALID_ARG;
+  DeviceGuard device_guard(h->device);
   if (!delta) return fail(h, HDC_ERR_INVALID_ARG, "train_delta: delta is NULL");
   if (!y && N > 0) return fail(h, HDC_ERR_INVALID_ARG, "train_delta: y is NULL");
   int rc = check_sim_args(h, Hbits, N, ldh_words, C_acc, K, ldc, D, knobs);
@@ -1052,6 +1149,7 @@ extern "C" int32_t hdc_train_delta(hdc_handle_t h, const uint32_t* Hbits, int64_
 extern "C" int32_t hdc_train_apply(hdc_handle_t h, float* C_acc, int32_t K, int64_t ldc, int32_t D,
                                    const hdc_knobs_t* knobs, const int32_t* delta, float lr, void* stream) {
   if (!h) return HDC_ERR_INVALID_ARG;
+  DeviceGuard device_guard(h->device);
   if (!C_acc || !delta) return fail(h, HDC_ERR_INVALID_ARG, "train_apply: NULL pointer");
   if (K < 1 || K > 65535 || D < 1 || ldc < D) return fail(h, HDC_ERR_INVALID_ARG, "train_apply: bad sizes");
   int rc = check_knobs(h, knobs, D);
@@ -1068,6 +1166,7 @@ extern "C" int32_t hdc_infer_rp(hdc_handle_t h, const void* X, int32_t x_dtype, 
                                 float* second, uint32_t* Hbits, int64_t ldh_words, void* ws, size_t ws_bytes,
                                 void* stream) {
   if (!h) return HDC_ERR_INVALID_ARG;
+  DeviceGuard device_guard(h->device);
   int rc = check_encode_rp_args(h, X, x_dtype, N, F, ldx, P, p_dtype, D, ldp, knobs);
   if (rc) return rc;
   if (!C_acc || (!labels && N > 0)) return fail(h, HDC_ERR_INVALID_ARG, "infer_rp: NULL pointer");
@@ -1084,12 +1183,165 @@ extern "C" int32_t hdc_infer_rp(hdc_handle_t h, const void* X, int32_t x_dtype, 
                      ldh_words, b, ws_bytes, (cudaStream_t)stream);
 }
 
+// =================================================================================== prepared model
+// The operands that do not depend on the queries -- the staged projection (bf16 / 3 x bf16 / half / int8 with
+// its row scales) and the class operand at hv_bits with its cosine scales -- prepared ONCE into caller memory
+// ("the one-time conversion of P and of the class model is not per-query work"); the *_m entry
+// points then run only the per-query kernels.
+constexpr uint32_t MODEL_MAGIC = 0x4D434448u;  // "HDCM"
+
+static bool same_knobs(const hdc_knobs_t& a, const hdc_knobs_t& b) {
+  return a.D_eff == b.D_eff && a.precision == b.precision && a.hv_bits == b.hv_bits && a.sim == b.sim &&
+         a.flags == b.flags && a.perf_begin == b.perf_begin && a.perf_stride == b.perf_stride &&
+         a.enc_perf_begin == b.enc_perf_begin && a.enc_perf_stride == b.enc_perf_stride;
+}
+
+extern "C" size_t hdc_model_bytes(hdc_handle_t h, int32_t F, int32_t D, int32_t K, const hdc_knobs_t* knobs) {
+  if (!h || !knobs || F < 1 || D < 1 || K < 1) return 0;
+  hdc_knobs_t k = *knobs;
+  if (k.D_eff < 1 || k.D_eff > D) k.D_eff = D;
+  return model_ws_bytes(h, F, K, &k);
+}
+
+extern "C" int32_t hdc_model_prepare(hdc_handle_t h, const void* P, int32_t p_dtype, int32_t F, int32_t D, int64_t ldp,
+                                     const float* C_acc, int32_t K, int64_t ldc, const hdc_knobs_t* knobs, void* blob,
+                                     size_t blob_bytes, hdc_model_t* out, void* stream) {
+  if (!h) return HDC_ERR_INVALID_ARG;
+  DeviceGuard device_guard(h->device);
+  if (!out || !blob) return fail(h, HDC_ERR_INVALID_ARG, "model_prepare: NULL pointer");
+  if (!P && !C_acc) return fail(h, HDC_ERR_INVALID_ARG, "model_prepare: neither P nor C_acc");
+  int rc = check_knobs(h, knobs, D);
+  if (rc) return rc;
+  if (reinterpret_cast<uintptr_t>(blob) & 255) return fail(h, HDC_ERR_ALIGNMENT, "model_prepare: blob must be 256-byte aligned");
+  if (P) {
+    float dummy = 0.0f;  // X is not read when only preparing
+    rc = check_encode_rp_args(h, &dummy, HDC_F32, 0, F, F, P, p_dtype, D, ldp, knobs);
+    if (rc) return rc;
+  }
+  if (C_acc) {
+    if (K < 1 || K > 65535 || ldc < D) return fail(h, HDC_ERR_INVALID_ARG, "model_prepare: bad sizes");
+    rc = check_sim_knobs(h, knobs);
+    if (rc) return rc;
+    if (reinterpret_cast<uintptr_t>(C_acc) & 3) return fail(h, HDC_ERR_ALIGNMENT, "model_prepare: C_acc alignment");
+  }
+  if (blob_bytes < model_ws_bytes(h, P ? F : 1, C_acc ? K : 1, knobs))
+    return fail(h, HDC_ERR_WORKSPACE, "model_prepare: blob smaller than hdc_model_bytes()");
+  cudaStream_t st = (cudaStream_t)stream;
+  rc = with_model(h, blob, blob_bytes, PREP_ONLY, [&]() {
+    Bump none(nullptr);  // preparing takes nothing from a scratch workspace
+    int r = HDC_OK;
+    // the same order as do_infer_rp's two-kernel path carves them: encode, then similarity; the fused
+    // epilogue's operand is prepared by hdc_model_prepare only when the knobs ask for that kernel
+    if (P && C_acc && (knobs->flags & HDC_FLAG_FUSED_INFER) && K <= INFER_MAX_K)
+      return do_infer_rp(h, nullptr, HDC_F32, INFER_MIN_N, F, F, P, p_dtype, D, ldp, C_acc, K, ldc, knobs, nullptr,
+                         nullptr, nullptr, nullptr, 0, none, (size_t)-1, st);
+    if (P) r = do_encode_rp(h, nullptr, HDC_F32, 1, F, F, P, p_dtype, D, ldp, knobs, HDC_OUT_BITS, nullptr, 0, nullptr, 0,
+                            none, (size_t)-1, st);
+    if (r == HDC_OK && C_acc)
+      r = do_similarity(h, nullptr, 1, words_of(knobs->D_eff), C_acc, K, ldc, knobs, nullptr, 0, 0, nullptr, nullptr,
+                        nullptr, none, (size_t)-1, st);
+    return r;
+  });
+  if (rc) return rc;
+  out->magic = MODEL_MAGIC;
+  out->F = P ? F : 0;
+  out->D = D;
+  out->K = C_acc ? K : 0;
+  out->p_dtype = p_dtype;
+  out->ldp = ldp;
+  out->ldc = ldc;
+  out->P = P;
+  out->C_acc = C_acc;
+  out->blob = blob;
+  out->blob_bytes = blob_bytes;
+  out->knobs = *knobs;
+  return HDC_OK;
+}
+
+static int check_model(hdc_ctx* h, const hdc_model_t* m, bool need_p, bool need_c) {
+  if (!m || m->magic != MODEL_MAGIC || !m->blob) return fail(h, HDC_ERR_INVALID_ARG, "model: not prepared by hdc_model_prepare");
+  if (need_p && !m->P) return fail(h, HDC_ERR_INVALID_ARG, "model: prepared without a projection");
+  if (need_c && !m->C_acc) return fail(h, HDC_ERR_INVALID_ARG, "model: prepared without class accumulators");
+  return HDC_OK;
+}
+
+extern "C" int32_t hdc_encode_rp_m(hdc_handle_t h, const void* X, int32_t x_dtype, int64_t N, int64_t ldx,
+                                   const hdc_model_t* m, uint32_t* Hbits, int64_t ldh_words, void* ws, size_t ws_bytes,
+                                   void* stream) {
+  if (!h) return HDC_ERR_INVALID_ARG;
+  DeviceGuard device_guard(h->device);
+  int rc = check_model(h, m, true, false);
+  if (rc) return rc;
+  rc = check_encode_rp_args(h, X, x_dtype, N, m->F, ldx, m->P, m->p_dtype, m->D, m->ldp, &m->knobs);
+  if (rc) return rc;
+  if ((!Hbits && N > 0) || ldh_words < words_of(m->knobs.D_eff)) return fail(h, HDC_ERR_INVALID_ARG, "encode_rp_m: Hbits / ldh_words");
+  if (reinterpret_cast<uintptr_t>(Hbits) & 3) return fail(h, HDC_ERR_ALIGNMENT, "encode_rp_m: Hbits alignment");
+  if (N == 0) return HDC_OK;
+  Bump b(ws);
+  if (!ws) ws_bytes = 0;
+  return with_model(h, m->blob, m->blob_bytes, RUN_ONLY, [&]() {
+    return do_encode_rp(h, X, x_dtype, N, m->F, ldx, m->P, m->p_dtype, m->D, m->ldp, &m->knobs, HDC_OUT_BITS, Hbits,
+                        ldh_words, nullptr, 0, b, ws_bytes, (cudaStream_t)stream);
+  });
+}
+
+extern "C" int32_t hdc_classify_m(hdc_handle_t h, const uint32_t* Hbits, int64_t N, int64_t ldh_words,
+                                  const hdc_model_t* m, int32_t* labels, float* best, float* second, void* ws,
+                                  size_t ws_bytes, void* stream) {
+  if (!h) return HDC_ERR_INVALID_ARG;
+  DeviceGuard device_guard(h->device);
+  int rc = check_model(h, m, false, true);
+  if (rc) return rc;
+  rc = check_sim_args(h, Hbits, N, ldh_words, m->C_acc, m->K, m->ldc, m->D, &m->knobs);
+  if (rc) return rc;
+  if (!labels && N > 0) return fail(h, HDC_ERR_INVALID_ARG, "classify_m: labels is NULL");
+  if (N == 0) return HDC_OK;
+  Bump b(ws);
+  if (!ws) ws_bytes = 0;
+  return with_model(h, m->blob, m->blob_bytes, RUN_ONLY, [&]() {
+    // a model prepared with both halves holds the encode operands first: skip over them as hdc_model_prepare did
+    Bump& pm = *static_cast<Bump*>(h->model);
+    if (m->P) {
+      Bump skip(nullptr);
+      encode_ws(h, 0, m->F, m->knobs.D_eff, &m->knobs, skip, pm);
+    }
+    return do_similarity(h, Hbits, N, ldh_words, m->C_acc, m->K, m->ldc, &m->knobs, nullptr, 0, 0, labels, best, second,
+                         b, ws_bytes, (cudaStream_t)stream);
+  });
+}
+
+extern "C" int32_t hdc_infer_rp_m(hdc_handle_t h, const void* X, int32_t x_dtype, int64_t N, int64_t ldx,
+                                  const hdc_model_t* m, int32_t* labels, float* best, float* second, uint32_t* Hbits,
+                                  int64_t ldh_words, void* ws, size_t ws_bytes, void* stream) {
+  if (!h) return HDC_ERR_INVALID_ARG;
+  DeviceGuard device_guard(h->device);
+  int rc = check_model(h, m, true, true);
+  if (rc) return rc;
+  rc = check_encode_rp_args(h, X, x_dtype, N, m->F, ldx, m->P, m->p_dtype, m->D, m->ldp, &m->knobs);
+  if (rc) return rc;
+  if (!labels && N > 0) return fail(h, HDC_ERR_INVALID_ARG, "infer_rp_m: labels is NULL");
+  if (Hbits && ldh_words < words_of(m->knobs.D_eff)) return fail(h, HDC_ERR_INVALID_ARG, "infer_rp_m: ldh_words < W");
+  if ((reinterpret_cast<uintptr_t>(Hbits) | reinterpret_cast<uintptr_t>(labels)) & 3)
+    return fail(h, HDC_ERR_ALIGNMENT, "infer_rp_m: operands must be 4-byte aligned");
+  if (N == 0) return HDC_OK;
+  // a model prepared for the fused kernel holds that kernel's operands only
+  if ((m->knobs.flags & HDC_FLAG_FUSED_INFER) && m->K <= INFER_MAX_K && !infer_fusable(h, &m->knobs, N, m->K))
+    return fail(h, HDC_ERR_UNSUPPORTED, "infer_rp_m: model prepared for the fused kernel, N too small for it");
+  Bump b(ws);
+  if (!ws) ws_bytes = 0;
+  return with_model(h, m->blob, m->blob_bytes, RUN_ONLY, [&]() {
+    return do_infer_rp(h, X, x_dtype, N, m->F, ldx, m->P, m->p_dtype, m->D, m->ldp, m->C_acc, m->K, m->ldc, &m->knobs,
+                       labels, best, second, Hbits, ldh_words, b, ws_bytes, (cudaStream_t)stream);
+  });
+}
+
 // =================================================================================== host end-to-end
 extern "C" int32_t hdc_infer_rp_host(hdc_handle_t h, const void* X_host, int32_t x_dtype, int64_t N, int32_t F,
                                      int64_t ldx, const void* P, int32_t p_dtype, int32_t D, int64_t ldp,
                                      const float* C_acc, int32_t K, int64_t ldc, const hdc_knobs_t* knobs,
                                      int32_t* labels_host, void* ws, size_t ws_bytes, void* stream) {
   if (!h) return HDC_ERR_INVALID_ARG;
+  DeviceGuard device_guard(h->device);
   int rc = check_encode_rp_args(h, X_host, x_dtype, N, F, ldx, P, p_dtype, D, ldp, knobs);
   if (rc) return rc;
   if (!C_acc || !labels_host) return fail(h, HDC_ERR_INVALID_ARG, "infer_rp_host: NULL pointer");
@@ -1106,8 +1358,16 @@ extern "C" int32_t hdc_infer_rp_host(hdc_handle_t h, const void* X_host, int32_t
   Xd[0] = (char*)b.take<float>((size_t)chunk * F);
   Xd[1] = (char*)b.take<float>((size_t)chunk * F);
   int32_t* Ld = b.take<int32_t>((size_t)N);
+  // the per-call-invariant operands (staged P, class operand, scales) are prepared by the first chunk into a
+  // region of their own and used by every later one, whatever its size
+  const size_t mbytes = model_ws_bytes(h, F, K, knobs);
+  uint8_t* mblob = b.take<uint8_t>(mbytes);
   if (b.off > ws_bytes) return fail(h, HDC_ERR_WORKSPACE, "infer_rp_host: workspace too small");
   const size_t base_off = b.off;
+  {  // dry run of the first (largest) chunk: workspace errors are reported before any copy is enqueued
+    const size_t need = base_off + infer_ws_bytes(h, chunk, F, K, knobs);
+    if (need > ws_bytes) return fail(h, HDC_ERR_WORKSPACE, "infer_rp_host: workspace too small");
+  }
   cudaError_t ce = cudaEventRecord(h->ev_entry, st);
   if (ce == cudaSuccess) ce = cudaStreamWaitEvent(h->copy_stream, h->ev_entry, 0);
   if (ce != cudaSuccess) return cuda_fail(h, ce, "infer_rp_host: entry");
@@ -1124,17 +1384,22 @@ extern "C" int32_t hdc_infer_rp_host(hdc_handle_t h, const void* X_host, int32_t
       ce = cudaMemcpy2DAsync(Xd[buf], (size_t)F * es, (const char*)X_host + (size_t)n0 * ldx * es,
                              (size_t)ldx * es, (size_t)F * es, (size_t)nb, cudaMemcpyHostToDevice,
                              h->copy_stream);
-    if (ce != cudaSuccess) return cuda_fail(h, ce, "infer_rp_host: H2D");
+    if (ce != cudaSuccess) {
+      cudaStreamSynchronize(h->copy_stream);
+      return cuda_fail(h, ce, "infer_rp_host: H2D");
+    }
     cudaEventRecord(h->ev_copied[buf], h->copy_stream);
     cudaStreamWaitEvent(st, h->ev_copied[buf], 0);
     Bump be(ws);
     be.off = base_off;
-    // same chunk size => same workspace layout: P staging and class-operand preparation of chunk 0 are reused
-    h->reuse_prep = c > 0 && nb == chunk;
-    rc = do_infer_rp(h, Xd[buf], x_dtype, nb, F, F, P, p_dtype, D, ldp, C_acc, K, ldc, knobs, Ld + n0, nullptr,
-                     nullptr, nullptr, 0, be, ws_bytes, st);
-    h->reuse_prep = false;
-    if (rc) return rc;
+    rc = with_model(h, mblob, mbytes, c == 0 ? PREP_AND_RUN : RUN_ONLY, [&]() {
+      return do_infer_rp(h, Xd[buf], x_dtype, nb, F, F, P, p_dtype, D, ldp, C_acc, K, ldc, knobs, Ld + n0, nullptr,
+                         nullptr, nullptr, 0, be, ws_bytes, st);
+    });
+    if (rc) {
+      cudaStreamSynchronize(h->copy_stream);  // no copy into the caller's workspace outlives the call
+      return rc;
+    }
     cudaEventRecord(h->ev_done[buf], st);
   }
   ce = cudaMemcpyAsync(labels_host, Ld, sizeof(int32_t) * (size_t)N, cudaMemcpyDeviceToHost, st);

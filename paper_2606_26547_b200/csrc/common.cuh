@@ -108,9 +108,10 @@ cudaError_t launch_gemm_tc(TcContext* tc, const TcOperands& o, int64_t M, int Nc
 size_t sim_tc_operand_bytes(int K, int hv_bits, int D_eff);
 cudaError_t launch_sim_tc(TcContext* tc, const uint32_t* Hbits, int64_t N, int64_t ldh, const float* C_acc,
                           int K, int64_t ldc, int D_eff, int hv_bits, void* cop, float* amax_scratch,
-                          const Epilogue& e, Perf pf, double* partial, bool cop_ready, int sm_count,
+                          const Epilogue& e, Perf pf, double* partial, bool cop_ready, bool prep_only, int sm_count,
                           cudaStream_t st, int64_t* nlaunch);
 // cop_ready: cop already holds the staged class operand of the same (C_acc, knobs) -- skip its preparation
+// prep_only: stage the class operand into cop (and amax) and return without contracting
 // partial: workspace of sim_tc_partial_bytes() (0 bytes / NULL: no split of the reduction axis)
 size_t sim_tc_partial_bytes(int64_t N, int K, int hv_bits, int D_eff, int sm_count);
 // amax = max |C[k][d]| over k < K and the visited d < D_eff (amax zeroed here)
@@ -174,7 +175,6 @@ cudaError_t launch_col_scale(const Operand& C, int K, int D_eff, int cos, Perf p
                              cudaStream_t st, int64_t* nlaunch);
 
 // packed XOR+popcount similarity with class bits in shared memory (hamming.cu)
-bool hamming_smem_fits(int K, int W, int smem_optin);
 // mask (nullable): W words; distances count only the bits set in it (reduction perforation)
 cudaError_t launch_hamming(const uint32_t* Hbits, int64_t N, int64_t ldh, const uint32_t* Cbits, int K,
                            int W, int D_eff, const uint32_t* mask, int32_t* dist, int64_t lds, int32_t* labels,

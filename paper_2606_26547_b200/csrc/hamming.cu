@@ -200,13 +200,9 @@ cudaError_t launch_ham2(int grid, cudaStream_t st, const uint32_t* Hbits, int64_
                         const uint32_t* Cbits, int K, int W, int D_eff, const uint32_t* mask, int32_t* dist,
                         int64_t lds, int32_t* labels, float* best, float* second) {
   constexpr int SMEM = NST * stage_words(KC) * 4;
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaError_t e =
-        cudaFuncSetAttribute(hamming_kernel<KC, PERF>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM);
-    if (e != cudaSuccess) return e;
-    attr_set = true;
-  }
+  // per-device attribute of the function: set on every launch (handles on several devices of one process)
+  cudaError_t e = cudaFuncSetAttribute(hamming_kernel<KC, PERF>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM);
+  if (e != cudaSuccess) return e;
   hamming_kernel<KC, PERF><<<grid, QT, SMEM, st>>>(Hbits, N, ldh, Cbits, K, W, D_eff, mask, dist, lds, labels,
                                                    best, second);
   return cudaGetLastError();
@@ -222,7 +218,6 @@ cudaError_t launch_ham(int grid, cudaStream_t st, const uint32_t* Hbits, int64_t
 
 }  // namespace
 
-bool hamming_smem_fits(int, int, int) { return true; }
 
 cudaError_t launch_hamming(const uint32_t* Hbits, int64_t N, int64_t ldh, const uint32_t* Cbits, int K,
                            int W, int D_eff, const uint32_t* mask, int32_t* dist, int64_t lds, int32_t* labels,

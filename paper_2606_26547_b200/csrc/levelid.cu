@@ -672,7 +672,7 @@ cudaError_t launch_levelid(const void* levels, int lvl16, int64_t N, int F, int6
   const size_t tab_bytes = ((size_t)F + Q) * SW * 4;
   p.tables_in_smem = (tab_bytes + lvl_bytes <= (size_t)smem_optin) ? 1 : 0;
   const size_t smem = lvl_bytes + (p.tables_in_smem ? tab_bytes : 0);
-  if (smem > (size_t)smem_optin) return cudaErrorInvalidConfiguration;
+  if (smem > (size_t)smem_optin) return cudaErrorNotSupported;  // the staged level rows alone exceed one CTA's shared memory
   const int64_t units = (int64_t)p.n_slices * p.n_batches;
   const int grid = (int)(units < sm_count ? units : sm_count);
   ++*nlaunch;

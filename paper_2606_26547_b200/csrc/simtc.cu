@@ -522,13 +522,10 @@ __global__ void split_reduce_kernel(const double* __restrict__ partial, int spli
 
 template <bool INT8, int EPI>
 cudaError_t launch_one(const CUtensorMap& tmB, const SimParams& p, int grid, cudaStream_t st) {
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(sim_tc_kernel<INT8, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         SMEM_LIMIT);
-    if (e != cudaSuccess) return e;
-    attr_set = true;
-  }
+  // per-device attribute of the function: set on every launch (handles on several devices of one process)
+  cudaError_t e = cudaFuncSetAttribute(sim_tc_kernel<INT8, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                       SMEM_LIMIT);
+  if (e != cudaSuccess) return e;
   const int smem = p.stages * p.stage_bytes + SMEM_EXTRA + QRING_BYTES;
   sim_tc_kernel<INT8, EPI><<<grid, NTHREADS, smem, st>>>(tmB, p);
   return cudaGetLastError();
@@ -586,10 +583,10 @@ size_t sim_tc_partial_bytes(int64_t N, int K, int hv_bits, int D_eff, int sm_cou
 
 cudaError_t launch_sim_tc(TcContext* tc, const uint32_t* Hbits, int64_t N, int64_t ldh, const float* C_acc,
                           int K, int64_t ldc, int D_eff, int hv_bits, void* cop, float* amax_scratch,
-                          const Epilogue& e, Perf pf, double* partial, bool cop_ready, int sm_count,
+                          const Epilogue& e, Perf pf, double* partial, bool cop_ready, bool prep_only, int sm_count,
                           cudaStream_t st, int64_t* nlaunch) {
   if (!tc) return cudaErrorNotSupported;
-  if (N <= 0) return cudaSuccess;
+  if (N <= 0 && !prep_only) return cudaSuccess;
   if ((reinterpret_cast<uintptr_t>(cop) & 15) != 0) return cudaErrorNotSupported;
   int kc, nparts, n_tiles, num_kb;
   bool int8;
@@ -616,6 +613,7 @@ cudaError_t launch_sim_tc(TcContext* tc, const uint32_t* Hbits, int64_t N, int64
     ce = cudaGetLastError();
     if (ce != cudaSuccess) return ce;
   }
+  if (prep_only) return cudaSuccess;
   CUtensorMap tmB;
   if (!tc_make_map(tc, &tmB, cop, int8, rows_total, ld, ld, nparts * kc)) return cudaErrorInvalidValue;
   SimParams p;

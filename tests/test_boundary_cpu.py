@@ -103,3 +103,20 @@ def test_binding_structs_match_header_field_for_field():
         assert fields == [f[0] for f in cls._fields_], cname
         assert all(f[1] is C.c_int32 for f in cls._fields_)
         assert C.sizeof(cls) == 4 * len(fields)
+
+
+@pytest.mark.skipif(shutil.which("gcc") is None, reason="gcc not on PATH")
+def test_model_descriptor_layout_matches_the_c_compiler(tmp_path):
+    """hdc_model_t is filled by the library and read back by the binding: sizeof and every offsetof, as gcc
+    lays the header's struct out, must equal the ctypes Structure's."""
+    from paper_2606_26547_b200 import binding
+    names = [f[0] for f in binding.hdc_model_t._fields_]
+    src = tmp_path / "layout.c"
+    src.write_text('#include <stdio.h>\n#include <stddef.h>\n#include "hdc.h"\nint main(void){\n'
+                   'printf("%zu\\n", sizeof(hdc_model_t));\n' +
+                   "".join(f'printf("%zu\\n", offsetof(hdc_model_t, {n}));\n' for n in names) + "return 0;}\n")
+    exe = tmp_path / "layout"
+    subprocess.run(["gcc", "-I", os.path.join(ROOT, "include"), str(src), "-o", str(exe)], check=True)
+    out = [int(x) for x in subprocess.run([str(exe)], capture_output=True, text=True, check=True).stdout.split()]
+    assert out[0] == C.sizeof(binding.hdc_model_t)
+    assert out[1:] == [getattr(binding.hdc_model_t, n).offset for n in names]
