@@ -49,6 +49,7 @@ struct LevelIdParams {
   uint32_t mul_hi16;  // 0x0101: the dp2a selectors, passed at run time so that they are not strength-reduced
   uint32_t mul128;    // 0x8080: dp2a selectors "times 128" of the sparse path
   int rows_aligned;   // F % 4 == 0, ldl % 4 == 0 and a 4-byte aligned base: level rows are read as words
+  int chunk;          // 16-bit levels on the fast kernel: features staged per pass (multiple of 64)
 };
 
 // NP = number of counter planes (p + 1 with 2^p > F); S = samples per warp iteration; LT = type of the
@@ -228,8 +229,17 @@ __device__ __forceinline__ void ripple(uint32_t (&q)[NP], uint32_t c, int from) 
 
 // VEC: level rows are word-aligned and F % 4 == 0 (plain word loads); otherwise aligned words are
 // prefetched and re-aligned by fixup() (any F, any row alignment)
-template <int NP, bool VEC>
-__global__ void __launch_bounds__(FTHREADS, 1) levelid_fast_kernel(const LevelIdParams p) {
+// L16: 16-bit level indices (PAPER.md L245 / L255: up to 1024 levels; the Micro-HD comparison tunes 814).  The staged
+// offsets are then the raw indices, two per word, and the "* 128" of the table address moves into the dp2a
+// selector.  A 1024-bit slice of an 814-level table is 104 KB, so the level rows of the 12 warps are staged in
+// chunks of p.chunk features by plain loads (measured: the kernel's rate follows the number of warps, 8 warps
+// with or without the register prefetch gave 114 M samples/s); the sparse path is left out.
+template <int NP, bool VEC, bool L16, int NW>
+__global__ void __launch_bounds__(NW * 32, 1) levelid_fast_kernel(const LevelIdParams p) {
+  constexpr int FSB = NW * FS;      // samples per batch (shadows the 12-warp constant)
+  constexpr int FWARPS = NW;
+  constexpr int PFR = PF_ROW;                      // prefetched words per lane per row (8-bit levels only)
+  constexpr int LB = L16 ? 2 : 1;                  // bytes per level index
   extern __shared__ __align__(16) uint8_t smem[];
   uint32_t* sID = reinterpret_cast<uint32_t*>(smem);          // [F][SW]
   uint32_t* sLV = sID + (size_t)p.F * SW;                      // [Q][SW]
@@ -241,9 +251,11 @@ __global__ void __launch_bounds__(FTHREADS, 1) levelid_fast_kernel(const LevelId
   constexpr int P = NP - 1;
   const uint32_t init = (1u << P) - (uint32_t)(p.F / 2 + 1);
   const uint32_t lane4 = (uint32_t)lane * 4u;
-  const uint32_t sel_lo = p.mul_hi16 & 0x0001u, sel_hi = p.mul_hi16 & 0x0100u;  // dp2a byte selectors (run-time: not folded)
   const uint32_t sel_id = p.mul128 & 0x0080u, sel_lv = p.mul128 & 0x8000u;      // (16-bit half) * 128
-  const int F4 = (p.F + 3) >> 2;                               // level words per sample row (last one zero-padded)
+  // dp2a byte selectors (run-time: not folded): staged half * 1 (8-bit levels, pre-multiplied) or * 128 (L16)
+  const uint32_t sel_lo = L16 ? sel_id : (p.mul_hi16 & 0x0001u), sel_hi = L16 ? sel_lv : (p.mul_hi16 & 0x0100u);
+  const int RB = p.F * LB;                                     // bytes of a level row
+  const int F4 = (RB + 3) >> 2;                                // level words per sample row (last one zero-padded)
 
   const int64_t units = (int64_t)p.n_slices * p.n_batches;
   const int64_t u_begin = units * blockIdx.x / gridDim.x;
@@ -252,7 +264,7 @@ __global__ void __launch_bounds__(FTHREADS, 1) levelid_fast_kernel(const LevelId
 
   // Each warp stages the level rows of its own FS samples (lanes stride over the row's words), so
   // a unit needs no block-wide barrier unless the slice -- and with it the tables -- changes.
-  uint32_t pf[PF_MAX];
+  uint32_t pf[FS * PFR];
   auto prefetch = [&](int64_t u) {
     const int64_t n0 = (u % p.n_batches) * FSB + warp * FS;
 #pragma unroll
@@ -270,24 +282,24 @@ __global__ void __launch_bounds__(FTHREADS, 1) levelid_fast_kernel(const LevelId
       }
       // raw ALIGNED words covering the row (the loads have no dependants here: they stay in flight
       // during the previous unit's arithmetic); row-relative words are formed by fixup() a unit later
-      const uint8_t* rowb = static_cast<const uint8_t*>(p.levels) + (n < p.N ? n : 0) * p.ldl;
+      const uint8_t* rowb = static_cast<const uint8_t*>(p.levels) + (n < p.N ? n : 0) * p.ldl * LB;
       const uint32_t off = (uint32_t)(reinterpret_cast<uintptr_t>(rowb) & 3u);
       const uint32_t* row = reinterpret_cast<const uint32_t*>(rowb - off);
-      const int nwords = (int)((off + (uint32_t)p.F + 3u) >> 2);   // aligned words that hold the row
+      const int nwords = (int)((off + (uint32_t)RB + 3u) >> 2);   // aligned words that hold the row
 #pragma unroll
-      for (int i = 0; i < PF_ROW; ++i) {
+      for (int i = 0; i < PFR; ++i) {
         const int g = lane + 32 * i;
         uint32_t v = 0u;
         if (g < nwords && n < p.N) {
-          if (g + 1 < nwords || n + 1 < p.N || ((off + (uint32_t)p.F) & 3u) == 0u) {
+          if (g + 1 < nwords || n + 1 < p.N || ((off + (uint32_t)RB) & 3u) == 0u) {
             v = __ldg(row + g);
           } else {  // last word of the last row: do not read past the end of the caller's buffer
-            const int nb = (int)((off + (uint32_t)p.F) & 3u);
+            const int nb = (int)((off + (uint32_t)RB) & 3u);
             for (int b2 = 0; b2 < nb; ++b2)
               v |= (uint32_t)__ldg(reinterpret_cast<const uint8_t*>(row + g) + b2) << (8 * b2);
           }
         }
-        pf[j * PF_ROW + i] = v;
+        pf[j * PFR + i] = v;
       }
     }
   };
@@ -298,29 +310,29 @@ __global__ void __launch_bounds__(FTHREADS, 1) levelid_fast_kernel(const LevelId
 #pragma unroll
     for (int j = 0; j < FS; ++j) {
       const int64_t n = n0 + j;
-      const uint8_t* rowb = static_cast<const uint8_t*>(p.levels) + (n < p.N ? n : 0) * p.ldl;
+      const uint8_t* rowb = static_cast<const uint8_t*>(p.levels) + (n < p.N ? n : 0) * p.ldl * LB;
       const uint32_t sh = (uint32_t)(reinterpret_cast<uintptr_t>(rowb) & 3u) * 8u;  // warp-uniform
       if (sh != 0u) {
 #pragma unroll
-        for (int i = 0; i < PF_ROW; ++i) {
-          const uint32_t lo = pf[j * PF_ROW + i];
+        for (int i = 0; i < PFR; ++i) {
+          const uint32_t lo = pf[j * PFR + i];
           uint32_t hi = __shfl_down_sync(0xffffffffu, lo, 1);                       // word of lane + 1
-          const uint32_t nxt = i + 1 < PF_ROW ? pf[j * PF_ROW + (i + 1 < PF_ROW ? i + 1 : i)] : 0u;
+          const uint32_t nxt = i + 1 < PFR ? pf[j * PFR + (i + 1 < PFR ? i + 1 : i)] : 0u;
           const uint32_t wrap = __shfl_sync(0xffffffffu, nxt, 0);                   // lane 0 of the next round
           if (lane == 31) hi = wrap;
-          pf[j * PF_ROW + i] = __funnelshift_r(lo, hi, sh);
+          pf[j * PFR + i] = __funnelshift_r(lo, hi, sh);
         }
       }
-      if (p.F & 3) {
+      if (RB & 3) {
 #pragma unroll
-        for (int i = 0; i < PF_ROW; ++i) {
+        for (int i = 0; i < PFR; ++i) {
           const int g = lane + 32 * i;
-          if (4 * g + 4 > p.F) pf[j * PF_ROW + i] &= (4 * g < p.F) ? ((1u << (8 * (p.F - 4 * g))) - 1u) : 0u;
+          if (4 * g + 4 > RB) pf[j * PFR + i] &= (4 * g < RB) ? ((1u << (8 * (RB - 4 * g))) - 1u) : 0u;
         }
       }
     }
   };
-  if (u_begin < u_end) prefetch(u_begin);
+  if (!L16 && u_begin < u_end) prefetch(u_begin);
 
   for (int64_t u = u_begin; u < u_end; ++u) {
     const int slice = (int)(u / p.n_batches);
@@ -353,7 +365,7 @@ __global__ void __launch_bounds__(FTHREADS, 1) levelid_fast_kernel(const LevelId
       __syncthreads();
     }
     __syncwarp();  // this warp is done reading its rows of the previous unit
-    fixup(u);
+    if (!L16) fixup(u);
 
     // ---- sparse path (level 0 is the common level: C3's images are ~80 % zeros) ------------------
     // cnt = sum_f b(f, x_f) = base + sum_{f in L} (b(f, x_f) - b(f, 0)) for any list L holding every
@@ -363,7 +375,7 @@ __global__ void __launch_bounds__(FTHREADS, 1) levelid_fast_kernel(const LevelId
     // the counter starts at base + init - |L|.  Exact for every input; chosen per warp when fewer
     // than 40 % of its FS samples' features are nonzero (the dense path costs 3.1 LOP3 per
     // feature, this one 6.3 per listed feature).
-    {
+    if (!L16) {
       int nz = 0, nz_max = 0;
 #pragma unroll
       for (int j = 0; j < FS; ++j) {
@@ -478,23 +490,25 @@ __global__ void __launch_bounds__(FTHREADS, 1) levelid_fast_kernel(const LevelId
       }
     }
 
-    // four level bytes -> two words of 16-bit offsets (level * 128)
+    if (!L16) {
+      // four level bytes -> two words of 16-bit offsets (level * 128)
 #pragma unroll
-    for (int j = 0; j < FS; ++j) {
+      for (int j = 0; j < FS; ++j) {
 #pragma unroll
-      for (int i = 0; i < PF_ROW; ++i) {
-        const int g = lane + 32 * i;
-        if (g < F4) {
-          const uint32_t v = pf[j * PF_ROW + i];
-          uint2 o;
-          o.x = ((v & 0xffu) << 7) | ((v & 0xff00u) << 15);
-          o.y = ((v >> 9) & 0x7f80u) | ((v >> 1) & 0x7f800000u);
-          *reinterpret_cast<uint2*>(sOff + (size_t)(warp * FS + j) * Fp2 + 2 * g) = o;
+        for (int i = 0; i < PF_ROW; ++i) {
+          const int g = lane + 32 * i;
+          if (g < F4) {
+            const uint32_t v = pf[j * PF_ROW + i];
+            uint2 o;
+            o.x = ((v & 0xffu) << 7) | ((v & 0xff00u) << 15);
+            o.y = ((v >> 9) & 0x7f80u) | ((v >> 1) & 0x7f800000u);
+            *reinterpret_cast<uint2*>(sOff + (size_t)(warp * FS + j) * Fp2 + 2 * g) = o;
+          }
         }
       }
+      __syncwarp();
+      if (u + 1 < u_end) prefetch(u + 1);
     }
-    __syncwarp();
-    if (u + 1 < u_end) prefetch(u + 1);
 
     uint32_t pl[FS][NP];
 #pragma unroll
@@ -502,57 +516,113 @@ __global__ void __launch_bounds__(FTHREADS, 1) levelid_fast_kernel(const LevelId
 #pragma unroll
       for (int i = 0; i < NP; ++i) pl[j][i] = ((init >> i) & 1u) ? 0xffffffffu : 0u;
 
-    const uint32_t* idp = sID + lane;
     const char* lvb = reinterpret_cast<const char*>(sLV);
     const uint32_t* myo = sOff + (size_t)(warp * FS) * Fp2;
 
-    // bound words of 16 features of sample j starting at feature f (f % 16 == 0)
+    // bound words of 16 features of sample j starting at (chunk-relative) feature f (f % 16 == 0)
     auto bind16 = [&](int f, int j, const uint32_t (&idw)[16], uint32_t (&x)[16]) {
       const uint4* op = reinterpret_cast<const uint4*>(myo + (size_t)j * Fp2 + (f >> 1));
       const uint4 oa = op[0], ob = op[1];
       const uint32_t o[8] = {oa.x, oa.y, oa.z, oa.w, ob.x, ob.y, ob.z, ob.w};
 #pragma unroll
       for (int i = 0; i < 8; ++i) {
-        // byte offset of the level row + lane word: 16-bit half of o times 1 plus lane4 as one dp2a
-        // (integer dot-product pipe, not the ALU pipe that the LOP3s saturate)
+        // byte offset of the level row + lane word: 16-bit half of o times 1 (times 128 for raw 16-bit indices)
+        // plus lane4 as one dp2a (integer dot-product pipe, not the ALU pipe that the LOP3s saturate)
         const uint32_t a_lo = __dp2a_lo(o[i], sel_lo, lane4);
         const uint32_t a_hi = __dp2a_lo(o[i], sel_hi, lane4);
         x[2 * i] = idw[2 * i] ^ *reinterpret_cast<const uint32_t*>(lvb + a_lo);
         x[2 * i + 1] = idw[2 * i + 1] ^ *reinterpret_cast<const uint32_t*>(lvb + a_hi);
       }
     };
-    int f = 0;
-    // 64 features: four 16-input trees, their weight-16 carries folded by three more CSAs, so the
-    // ripple into the upper planes runs once per 64 features
+    // 8-bit levels: the whole row is staged (one chunk).  16-bit levels: the rows are staged in chunks of
+    // p.chunk features (a multiple of 64) straight from global memory, so that 12 warps' rows fit beside an
+    // up-to-1024-level table slice; the other warps of the scheduler cover the load latency.
+    const int CH = L16 ? p.chunk : p.F;
 #pragma unroll 1
-    for (; f + 64 <= p.F; f += 64) {
-      uint32_t sxs[FS][3];
-#pragma unroll
-      for (int q4 = 0; q4 < 4; ++q4) {
-        uint32_t idw[16];
-#pragma unroll
-        for (int i = 0; i < 16; ++i) idw[i] = idp[(f + 16 * q4 + i) * SW];
+    for (int f0 = 0; f0 < p.F; f0 += CH) {
+      const int fc = p.F - f0 < CH ? p.F - f0 : CH;   // features of this chunk
+      if (L16) {
+        __syncwarp();  // the previous chunk's offsets have been read
+        const int64_t n0 = batch * FSB + warp * FS;
 #pragma unroll
         for (int j = 0; j < FS; ++j) {
-          uint32_t x[16];
-          bind16(f + 16 * q4, j, idw, x);
-          const uint32_t sx = tree16(pl[j], x);
-          if (q4 < 3) {
-            sxs[j][q4] = sx;
-          } else {
-            uint32_t ca, cb, c64;
-            HDC_CSA(ca, pl[j][4], pl[j][4], sxs[j][0], sxs[j][1]);
-            HDC_CSA(cb, pl[j][4], pl[j][4], sxs[j][2], sx);
-            HDC_CSA(c64, pl[j][5], pl[j][5], ca, cb);
-            ripple(pl[j], c64, 6);
+          const int64_t n = n0 + j;
+          const uint16_t* row = static_cast<const uint16_t*>(p.levels) + (n < p.N ? n : 0) * p.ldl + f0;
+          const bool word_ok = (reinterpret_cast<uintptr_t>(row) & 3u) == 0u;   // warp-uniform
+          for (int g = lane; g < Fp2; g += 32) {
+            uint32_t v = 0u;
+            if (n < p.N) {
+              if (word_ok && 2 * g + 1 < fc) {
+                v = __ldg(reinterpret_cast<const uint32_t*>(row) + g);
+              } else {
+                if (2 * g < fc) v = __ldg(row + 2 * g);
+                if (2 * g + 1 < fc) v |= (uint32_t)__ldg(row + 2 * g + 1) << 16;
+              }
+            }
+            sOff[(size_t)(warp * FS + j) * Fp2 + g] = v;
+          }
+        }
+        __syncwarp();
+      }
+      const uint32_t* idp = sID + (size_t)f0 * SW + lane;
+      int f = 0;
+      // 64 features: four 16-input trees, their weight-16 carries folded by three more CSAs, so the
+      // ripple into the upper planes runs once per 64 features
+#pragma unroll 1
+      for (; f + 64 <= fc; f += 64) {
+        uint32_t sxs[FS][3];
+#pragma unroll
+        for (int q4 = 0; q4 < 4; ++q4) {
+          uint32_t idw[16];
+#pragma unroll
+          for (int i = 0; i < 16; ++i) idw[i] = idp[(f + 16 * q4 + i) * SW];
+#pragma unroll
+          for (int j = 0; j < FS; ++j) {
+            uint32_t x[16];
+            bind16(f + 16 * q4, j, idw, x);
+            const uint32_t sx = tree16(pl[j], x);
+            if (q4 < 3) {
+              sxs[j][q4] = sx;
+            } else {
+              uint32_t ca, cb, c64;
+              HDC_CSA(ca, pl[j][4], pl[j][4], sxs[j][0], sxs[j][1]);
+              HDC_CSA(cb, pl[j][4], pl[j][4], sxs[j][2], sx);
+              HDC_CSA(c64, pl[j][5], pl[j][5], ca, cb);
+              ripple(pl[j], c64, 6);
+            }
           }
         }
       }
-    }
 #pragma unroll 1
-    for (; f + 32 <= p.F; f += 32) {
-      uint32_t sxa[FS];
-      {
+      for (; f + 32 <= fc; f += 32) {
+        uint32_t sxa[FS];
+        {
+          uint32_t idw[16];
+#pragma unroll
+          for (int i = 0; i < 16; ++i) idw[i] = idp[(f + i) * SW];
+#pragma unroll
+          for (int j = 0; j < FS; ++j) {
+            uint32_t x[16];
+            bind16(f, j, idw, x);
+            sxa[j] = tree16(pl[j], x);
+          }
+        }
+        {
+          uint32_t idw[16];
+#pragma unroll
+          for (int i = 0; i < 16; ++i) idw[i] = idp[(f + 16 + i) * SW];
+#pragma unroll
+          for (int j = 0; j < FS; ++j) {
+            uint32_t x[16];
+            bind16(f + 16, j, idw, x);
+            const uint32_t sxb = tree16(pl[j], x);
+            uint32_t c32;
+            HDC_CSA(c32, pl[j][4], pl[j][4], sxa[j], sxb);
+            ripple(pl[j], c32, 5);
+          }
+        }
+      }
+      if (f + 16 <= fc) {
         uint32_t idw[16];
 #pragma unroll
         for (int i = 0; i < 16; ++i) idw[i] = idp[(f + i) * SW];
@@ -560,43 +630,19 @@ __global__ void __launch_bounds__(FTHREADS, 1) levelid_fast_kernel(const LevelId
         for (int j = 0; j < FS; ++j) {
           uint32_t x[16];
           bind16(f, j, idw, x);
-          sxa[j] = tree16(pl[j], x);
+          ripple(pl[j], tree16(pl[j], x), 4);
         }
+        f += 16;
       }
-      {
-        uint32_t idw[16];
-#pragma unroll
-        for (int i = 0; i < 16; ++i) idw[i] = idp[(f + 16 + i) * SW];
+      for (; f < fc; ++f) {  // remainder features: plain ripple add
+        const uint32_t idw = idp[f * SW];
 #pragma unroll
         for (int j = 0; j < FS; ++j) {
-          uint32_t x[16];
-          bind16(f + 16, j, idw, x);
-          const uint32_t sxb = tree16(pl[j], x);
-          uint32_t c32;
-          HDC_CSA(c32, pl[j][4], pl[j][4], sxa[j], sxb);
-          ripple(pl[j], c32, 5);
+          const uint32_t o = myo[(size_t)j * Fp2 + (f >> 1)];
+          const uint32_t hv = ((f & 1) ? (o >> 16) : o) & 0xffffu;
+          const uint32_t a = L16 ? (hv * 128u + lane4) : (hv | lane4);
+          ripple(pl[j], idw ^ *reinterpret_cast<const uint32_t*>(lvb + a), 0);
         }
-      }
-    }
-    if (f + 16 <= p.F) {
-      uint32_t idw[16];
-#pragma unroll
-      for (int i = 0; i < 16; ++i) idw[i] = idp[(f + i) * SW];
-#pragma unroll
-      for (int j = 0; j < FS; ++j) {
-        uint32_t x[16];
-        bind16(f, j, idw, x);
-        ripple(pl[j], tree16(pl[j], x), 4);
-      }
-      f += 16;
-    }
-    for (; f < p.F; ++f) {  // remainder features: plain ripple add
-      const uint32_t idw = idp[f * SW];
-#pragma unroll
-      for (int j = 0; j < FS; ++j) {
-        const uint32_t o = myo[(size_t)j * Fp2 + (f >> 1)];
-        const uint32_t a = (((f & 1) ? (o >> 16) : o) & 0xffffu) | lane4;
-        ripple(pl[j], idw ^ *reinterpret_cast<const uint32_t*>(lvb + a), 0);
       }
     }
 
@@ -645,18 +691,51 @@ cudaError_t launch_levelid(const void* levels, int lvl16, int64_t N, int F, int6
       p.mul_hi16 = 0x0101u;
       p.mul128 = 0x8080u;
       p.rows_aligned = (F % 4 == 0 && (ldl & 3) == 0 && (reinterpret_cast<uintptr_t>(levels) & 3) == 0) ? 1 : 0;
+      p.chunk = F;
       const int64_t units = (int64_t)p.n_slices * p.n_batches;
       const int grid = (int)(units < sm_count ? units : sm_count);
-      cudaError_t e = cudaFuncSetAttribute(levelid_fast_kernel<11, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                           (int)smem_fast);
+      cudaError_t e = cudaFuncSetAttribute(levelid_fast_kernel<11, true, false, FWARPS>,
+                                           cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_fast);
       if (e == cudaSuccess)
-        e = cudaFuncSetAttribute(levelid_fast_kernel<11, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 (int)smem_fast);
+        e = cudaFuncSetAttribute(levelid_fast_kernel<11, false, false, FWARPS>,
+                                 cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_fast);
       if (e != cudaSuccess) return e;
       ++*nlaunch;
-      if (p.rows_aligned) levelid_fast_kernel<11, true><<<grid, FTHREADS, smem_fast, st>>>(p);
-      else levelid_fast_kernel<11, false><<<grid, FTHREADS, smem_fast, st>>>(p);
+      if (p.rows_aligned) levelid_fast_kernel<11, true, false, FWARPS><<<grid, FTHREADS, smem_fast, st>>>(p);
+      else levelid_fast_kernel<11, false, false, FWARPS><<<grid, FTHREADS, smem_fast, st>>>(p);
       return cudaGetLastError();
+    }
+    // 16-bit level indices: same kernel, dense path only, level rows staged in chunks of `chunk` features --
+    // the largest multiple of 64 (up to 320) whose 48 rows fit beside the table slices
+    if (lvl16 && F <= 1020 && Q <= 1024) {
+      const size_t tab = ((size_t)F + Q) * SW * 4 + (size_t)11 * SW * 4;
+      int chunk = 0;
+      for (int c = 320; c >= 64 && !chunk; c -= 64)
+        if (tab + (size_t)FSB * (c / 2) * 4 <= (size_t)smem_optin) chunk = c;
+      if (chunk) {
+        LevelIdParams p;
+        p.levels = levels; p.N = N; p.F = F; p.ldl = ldl;
+        p.ID = ID; p.ldid = ldid; p.LV = LV; p.Q = Q; p.ldlv = ldlv;
+        p.D_eff = D_eff; p.W = words_of(D_eff);
+        p.Hbits = Hbits; p.ldh = ldh;
+        p.n_slices = (p.W + SW - 1) / SW;
+        p.n_batches = (N + FSB - 1) / FSB;
+        p.Fpad = chunk / 2;   // words per staged row
+        p.chunk = chunk;
+        p.tables_in_smem = 1;
+        p.mul_hi16 = 0x0101u;
+        p.mul128 = 0x8080u;
+        p.rows_aligned = 0;
+        const size_t smem_16 = tab + (size_t)FSB * p.Fpad * 4;
+        const int64_t units = (int64_t)p.n_slices * p.n_batches;
+        const int grid = (int)(units < sm_count ? units : sm_count);
+        cudaError_t e = cudaFuncSetAttribute(levelid_fast_kernel<11, false, true, FWARPS>,
+                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_16);
+        if (e != cudaSuccess) return e;
+        ++*nlaunch;
+        levelid_fast_kernel<11, false, true, FWARPS><<<grid, FTHREADS, smem_16, st>>>(p);
+        return cudaGetLastError();
+      }
     }
   }
   LevelIdParams p;

@@ -541,6 +541,27 @@ def test_levelid_u16_indices_bit_exact(hd, h, N, F, Q, D, D_eff):
     assert np.array_equal(host_bits(H, D_eff), bits_or)
 
 
+@pytest.mark.parametrize("N,F,Q,ld,col0,D,D_eff", [(333, 617, 814, 617, 0, 1024, 1024), (129, 617, 814, 620, 1, 1100, 1055),
+                                                   (65, 640, 1024, 643, 3, 1024, 1000), (100, 63, 257, 63, 0, 4100, 4100),
+                                                   (37, 1, 300, 4, 2, 64, 33), (50, 1020, 300, 1020, 0, 96, 96),
+                                                   (40, 700, 1024, 700, 0, 512, 512)])
+def test_levelid_u16_fast_kernel_shapes_bit_exact(hd, h, N, F, Q, ld, col0, D, D_eff):
+    """16-bit level indices on the slice-resident fast kernel (Q <= 1024, tables + rows in shared memory): ragged
+    batches (N not a multiple of 32), odd F, rows that start at odd element offsets of a wider matrix, several
+    slices, partial last word; the last case exceeds the shared-memory budget and takes the general kernel."""
+    r = rng(16, N, F, Q, D_eff)
+    big = r.integers(0, Q, size=(N, ld)).astype(np.uint16)
+    big[0, col0:col0 + F] = Q - 1
+    big[r.random((N, ld)) < 0.2] = 0
+    lv = big[:, col0:col0 + F]
+    ID = r.integers(0, 2, size=(F, D), dtype=np.uint8)
+    LV = gen.level_table(9, Q, D)
+    bits_or = O.encode_levelid(lv, ID, LV, D_eff)
+    lvd = torch.from_numpy(big.view(np.int16)).cuda()[:, col0:col0 + F]
+    H = h.hdc_encode_levelid(lvd, dev_bits(ID), dev_bits(LV), D, hd.knobs(D_eff))
+    assert np.array_equal(host_bits(H, D_eff), bits_or)
+
+
 @pytest.mark.parametrize("F,ld,col0", [(617, 617, 0), (617, 620, 0), (616, 621, 1), (100, 107, 3), (1020, 1023, 3), (5, 9, 2)])
 def test_levelid_unaligned_rows_bit_exact(hd, h, F, ld, col0):
     """Level rows that start at any byte offset (a column slice of a wider uint8 matrix; F not a
