@@ -76,9 +76,9 @@ enum {
   HDC_FLAG_NONE = 0,
   HDC_FLAG_SIMT = 1, /* force the CUDA-core (FFMA / popcount) kernels where a tensor-core kernel
                         exists for the same operation (debugging, A/B measurement)              */
-  HDC_FLAG_TC_1CTA = 2, /* encode contraction: force the one-CTA-per-tile tcgen05 kernel        */
-  HDC_FLAG_TC_2CTA = 4, /* encode contraction: force the CTA-pair (cta_group::2) tcgen05 kernel;
-                           without either flag the library chooses by problem size              */
+  HDC_FLAG_TC_1CTA = 2, /* encode and similarity contractions: force the one-CTA-per-tile tcgen05 kernels */
+  HDC_FLAG_TC_2CTA = 4, /* ... force the CTA-pair (cta_group::2) tcgen05 kernels; without either flag the
+                           library chooses by problem size                                      */
   HDC_FLAG_F32_FAST = 8, /* precision HDC_F32 only, OFF by default: contract 2-way IEEE-half splits of
                            the row-scaled operands (22 of the 24 mantissa bits, three tensor-core
                            products instead of six; |error| <= 3 * 2^-22 * sum|x p|).  An extra point

@@ -438,7 +438,11 @@ int do_similarity(hdc_ctx* h, const uint32_t* Hbits, int64_t N, int64_t ldh, con
   // the popcount pipe would bound it (dist = (D_eff - dot)/2 is exact in int32)
   if (use_tc(h, k) && (k->sim != HDC_SIM_HAMMING || K >= 64)) {
     double* colscale = nullptr;
-    if (k->sim == HDC_SIM_COS) colscale = pm.take<double>((size_t)K);
+    float* colscale_f = nullptr;
+    if (k->sim == HDC_SIM_COS) {
+      colscale = pm.take<double>((size_t)K);
+      colscale_f = pm.take<float>((size_t)K);
+    }
     float* amax = pm.take<float>(1);
     void* cop = pm.take<uint8_t>(sim_tc_operand_bytes(K, k->hv_bits, D_eff));
     int8_t* Cq = nullptr;
@@ -452,18 +456,19 @@ int do_similarity(hdc_ctx* h, const uint32_t* Hbits, int64_t N, int64_t ldh, con
       if (k->hv_bits == 8) {
         ce = launch_quantize_tensor_i8(C_acc, K, D_eff, ldc, pf, Cq, ldq, amax, st, &h->launches);
         if (ce != cudaSuccess) return cuda_fail(h, ce, "quantize C");
-        ce = launch_col_scale(Operand{Cq, ldq, OPK_I8}, K, D_eff, 1, pf, colscale, st, &h->launches);
+        ce = launch_col_scale(Operand{Cq, ldq, OPK_I8}, K, D_eff, 1, pf, colscale, st, &h->launches, colscale_f);
       } else {
         const int ck = k->hv_bits == 32   ? OPK_F32
                        : k->hv_bits == 16 ? OPK_F32_RBF16
                        : k->hv_bits == HDC_HV_F16 ? OPK_F32_RF16
                                                   : OPK_BITS;
-        ce = launch_col_scale(Operand{C_acc, ldc, ck}, K, D_eff, 1, pf, colscale, st, &h->launches);
+        ce = launch_col_scale(Operand{C_acc, ldc, ck}, K, D_eff, 1, pf, colscale, st, &h->launches, colscale_f);
       }
       if (ce != cudaSuccess) return cuda_fail(h, ce, "col_scale");
     }
     Epilogue e{};
     e.colscale = colscale;
+    e.colscale_f = colscale_f;
     e.ham_D = k->sim == HDC_SIM_HAMMING ? n_vis : 0;
     if (labels) {
       e.kind = EPI_ARGMAX;
@@ -479,7 +484,7 @@ int do_similarity(hdc_ctx* h, const uint32_t* Hbits, int64_t N, int64_t ldh, con
     {
       Timed tm(h, HDC_K_SIM, st);
       ce = launch_sim_tc(h->tc, Hbits, N, ldh, C_acc, K, ldc, D_eff, k->hv_bits, cop, amax, e, pf, partial,
-                         !prep, prep_only(h), h->sm_count, st, &h->launches);
+                         !prep, prep_only(h), h->sm_count, tc_cta_group(k), st, &h->launches);
     }
     if (ce == cudaSuccess) return HDC_OK;
     if (ce != cudaErrorNotSupported) return cuda_fail(h, ce, "similarity tcgen05");
@@ -565,6 +570,7 @@ int do_similarity(hdc_ctx* h, const uint32_t* Hbits, int64_t N, int64_t ldh, con
 void similarity_model_ws(int K, const hdc_knobs_t* k, Bump& pm) {
   const int W = words_of(k->D_eff);
   pm.take<double>((size_t)K);
+  pm.take<float>((size_t)K);
   pm.take<float>(1);
   pm.take<int8_t>((size_t)K * round_up(k->D_eff, 16));
   pm.take<uint32_t>((size_t)K * W);
@@ -583,6 +589,7 @@ size_t similarity_ws(int64_t N, int K, const hdc_knobs_t* k) {
   }
   const int W = words_of(k->D_eff);
   b.take<double>((size_t)K);
+  b.take<float>((size_t)K);
   b.take<int8_t>((size_t)K * round_up(k->D_eff, 16));
   b.take<float>(1);
   b.take<uint32_t>((size_t)K * W);

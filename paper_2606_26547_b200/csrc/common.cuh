@@ -58,6 +58,7 @@ struct Epilogue {
   int64_t lds;
   int s_i32;
   const double* colscale;
+  const float* colscale_f;  // the same scales rounded to fp32 (sim_tc_kernel compares in fp32: FP64 is slow here)
   // EPI_ARGMAX: label = argmax_n acc*colscale[n], ties to lowest n; best/second nullable.
   // ham_D > 0: report best/second as Hamming distances (ham_D - dot)/2 (bits x bits).
   int32_t* labels;
@@ -109,7 +110,8 @@ size_t sim_tc_operand_bytes(int K, int hv_bits, int D_eff);
 cudaError_t launch_sim_tc(TcContext* tc, const uint32_t* Hbits, int64_t N, int64_t ldh, const float* C_acc,
                           int K, int64_t ldc, int D_eff, int hv_bits, void* cop, float* amax_scratch,
                           const Epilogue& e, Perf pf, double* partial, bool cop_ready, bool prep_only, int sm_count,
-                          cudaStream_t st, int64_t* nlaunch);
+                          int force_cg, cudaStream_t st, int64_t* nlaunch);
+// force_cg: 1 / 2 = one-CTA / CTA-pair kernel (knobs HDC_FLAG_TC_1CTA / _2CTA), else by problem size
 // cop_ready: cop already holds the staged class operand of the same (C_acc, knobs) -- skip its preparation
 // prep_only: stage the class operand into cop (and amax) and return without contracting
 // partial: workspace of sim_tc_partial_bytes() (0 bytes / NULL: no split of the reduction axis)
@@ -171,8 +173,9 @@ cudaError_t launch_sign_bits(const float* C, int K, int D_eff, int64_t ldc, uint
                              cudaStream_t st, int64_t* nlaunch);
 // colscale[k] = cos ? (nrm_k > 0 ? 1/(sqrt(n_visited)*nrm_k) : 0) : 1, nrm over the visited
 // dimensions of the operand as loaded
+// colscale_f (nullable): receives (float)colscale[k]
 cudaError_t launch_col_scale(const Operand& C, int K, int D_eff, int cos, Perf pf, double* colscale,
-                             cudaStream_t st, int64_t* nlaunch);
+                             cudaStream_t st, int64_t* nlaunch, float* colscale_f = nullptr);
 
 // packed XOR+popcount similarity with class bits in shared memory (hamming.cu)
 // mask (nullable): W words; distances count only the bits set in it (reduction perforation)

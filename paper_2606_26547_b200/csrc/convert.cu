@@ -265,7 +265,7 @@ __global__ void sign_bits_kernel(const float* __restrict__ C, int K, int D_eff, 
 // colscale[k] = cos ? (nrm > 0 ? 1 / (sqrt(D_eff) * nrm) : 0) : 1, nrm^2 = sum_d c[k,d]^2 in double
 // over the operand as the contraction loads it.  One block per class, fixed reduction order.
 __global__ void col_scale_kernel(Operand C, int K, int D_eff, int cos, Perf pf, int n_vis,
-                                 double* __restrict__ colscale) {
+                                 double* __restrict__ colscale, float* __restrict__ colscale_f) {
   const int k = blockIdx.x;
   __shared__ double part[32];
   double s = 0.0;
@@ -301,6 +301,7 @@ __global__ void col_scale_kernel(Operand C, int K, int D_eff, int cos, Perf pf, 
       const double nrm = sqrt(t);
       colscale[k] = nrm > 0.0 ? 1.0 / (sqrt((double)n_vis) * nrm) : 0.0;
     }
+    if (colscale_f) colscale_f[k] = (float)colscale[k];
   }
 }
 
@@ -524,8 +525,8 @@ cudaError_t launch_class_operand_f32(const float* C, int K, int D_eff, int64_t l
 }
 
 cudaError_t launch_col_scale(const Operand& C, int K, int D_eff, int cos, Perf pf, double* colscale,
-                             cudaStream_t st, int64_t* nlaunch) {
-  col_scale_kernel<<<K, 1024, 0, st>>>(C, K, D_eff, cos, pf, perf_count(pf, D_eff), colscale);
+                             cudaStream_t st, int64_t* nlaunch, float* colscale_f) {
+  col_scale_kernel<<<K, 1024, 0, st>>>(C, K, D_eff, cos, pf, perf_count(pf, D_eff), colscale, colscale_f);
   ++*nlaunch;
   return cudaGetLastError();
 }

@@ -13,6 +13,15 @@
 // group); for small N the reduction axis is split over several CTAs per m-tile (split_reduce_kernel
 // adds the partial sums in a fixed order).
 //
+// CG = 2 (large N, K >= 128): the two CTAs of a cluster share a 256-query x kc-class tile with
+// tcgen05.mma.cta_group::2.  Each CTA expands its own 128 queries and stages HALF of the class tile, so per
+// k-block an SM's shared memory takes 16 KB (expanders) + 16 KB (TMA) of writes and serves 32 KB of tensor-core
+// reads instead of 16 + 32 and 48: the one-CTA kernel is bound by exactly that traffic (profiles/r2_simtc.md:
+// tensor pipe 51 % active with the shared-memory data pipe saturated).  Barriers as in gemm_tc.cu: `full` lives in
+// the leader (even CTA) and collects the TMA bytes and the expander warps of BOTH CTAs (the peer's warps arrive
+// remotely after their proxy fence), `empty` / `tmem full` are signalled in both CTAs by multicast commits,
+// `tmem empty` lives in the leader.
+//
 // Reduction-axis permutation.  A sum over d is invariant under any permutation of d applied to both
 // operands, so the k-block position kappa <-> dimension map is chosen to make the expansion two or
 // three ALU ops per 32-bit shared-memory word (perm_bf16 / perm_i8 below); the class operand is
@@ -44,11 +53,12 @@ constexpr int NTHREADS = 192 + 32 * EXW;
 constexpr int TMEM_COLS = 512;
 constexpr int SMEM_LIMIT = 227 * 1024;
 constexpr int SMEM_EXTRA = 1024 /*alignment slack*/ + 256 /*barriers*/;
-constexpr int QW = 32;                       // packed words per row in one tile of the query ring
+// packed words per row in one tile of the query ring: 32 for the one-CTA kernel, 16 for CTA pairs (a 32 KB
+// stage: the 24 KB saved buy a sixth stage, i.e. three hand-off groups of two k-blocks)
+__host__ __device__ constexpr int qw_of(int cg) { return cg == 2 ? 16 : 32; }
 constexpr int Q_LD = BM + 1;                 // words between consecutive word-rows of a ring tile
-constexpr int Q_SLOT_WORDS = QW * Q_LD;
 constexpr int Q_SLOTS = 3;
-constexpr int QRING_BYTES = Q_SLOTS * Q_SLOT_WORDS * 4;
+__host__ __device__ constexpr int qring_bytes(int cg) { return Q_SLOTS * qw_of(cg) * Q_LD * 4; }
 
 // dimension offset (within a k-block) of shared-memory K position kappa
 __host__ __device__ __forceinline__ int perm_bf16(int kappa) {  // k-block = 64 dims = 2 words
@@ -80,12 +90,26 @@ struct SimParams {
   Epilogue e;
 };
 
-struct Top2 {
+struct Top2 {   // split_reduce_kernel (small N): double throughout
   double b1;
   int i1;
   double b2;
 };
 constexpr double NEG_BIG = -1.0e300;
+// Running arg-max of the main kernel.  FP64 arithmetic is ~50 cycles per warp instruction and SM on this part
+// (measured: with a double multiply, two double compares and a conversion per (query, class) the K = 1000
+// classify spent every cycle of its epilogue warps there and the tensor pipe idled at 51 %), so the scores are
+// compared in fp32 and the decision falls back to the exact double product only where two scores are within
+// 2e-6 relative of each other -- which keeps the integer paths' labels (and exact ties -> lowest index)
+// identical to an all-double comparison: an int32 / fp32 accumulator times the fp32-rounded scale is within
+// 2^-23 relative of the double product.  a1 / a2: the accumulators of the best and the runner-up, from
+// which their reported scores are recomputed in double once per row.
+struct Top2f {
+  float b1, b2;
+  float a1, a2;
+  int i1, i2;
+};
+constexpr float NEG_BIG_F = -3.0e38f;
 
 __device__ __forceinline__ uint32_t prmt_sign_bytes(uint32_t v) {
   uint32_t d;
@@ -93,7 +117,7 @@ __device__ __forceinline__ uint32_t prmt_sign_bytes(uint32_t v) {
   return d;
 }
 
-template <bool INT8, int EPI>
+template <bool INT8, int EPI, int CG>
 __global__ void __launch_bounds__(NTHREADS, 1)
 sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
   extern __shared__ uint8_t smem_raw[];
@@ -111,33 +135,36 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
   uint32_t* tmem_slot_ptr = reinterpret_cast<uint32_t*>(smem_raw + (tmem_slot - smem_u32(smem_raw)));
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int rank = CG == 2 ? (int)cluster_ctarank() : 0;   // 0 = leader: issues the MMAs, owns `full` / `tmem empty`
   constexpr int BK = INT8 ? 128 : 64;
-  const int nb_rows = p.nparts * p.kc;
+  const int nb_rows = p.nparts * p.kc;      // class rows of a tile (the MMA's N)
+  const int nb_half = nb_rows / CG;         // ... of which this CTA stages this many
 
   if (warp == 0 && lane == 0) {
     asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&tmB)) : "memory");
     for (int s = 0; s < NG; ++s) {
-      mbar_init(full_bar(s), 1 + EXW);  // producer (with the TMA byte count) + one arrival per expander warp
+      // leader's producer (with the TMA byte count of both CTAs) + one arrival per expander warp of each CTA
+      mbar_init(full_bar(s), 1 + EXW * CG);
       mbar_init(empty_bar(s), 1);
     }
     for (int s = 0; s < 2; ++s) {
       mbar_init(tfull_bar(s), 1);
-      mbar_init(tempty_bar(s), 4);
+      mbar_init(tempty_bar(s), 4 * CG);
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
-  if (warp == 1) tmem_alloc(tmem_slot, TMEM_COLS);
+  if (warp == 1) tmem_alloc<CG>(tmem_slot, TMEM_COLS);
   tc_fence_before();
-  __syncthreads();
+  if (CG == 2) cluster_sync_all(); else __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot_ptr;
 
-  // work item = (m-tile, split of the reduction axis); a CTA walks items blockIdx.x, +gridDim.x, ...
+  // work item = (m-tile of BM * CG queries, split of the reduction axis); a CTA (pair) walks items unit, +nunits, ...
+  const int64_t unit = blockIdx.x / CG, nunits = gridDim.x / CG;
   const int64_t n_items = (int64_t)p.m_tiles * p.splits;
-  const int64_t tiles_per_cta =
-      (n_items > (int64_t)blockIdx.x) ? ((n_items - 1 - (int64_t)blockIdx.x) / gridDim.x + 1) * p.n_tiles : 0;
+  const int64_t tiles_per_cta = (n_items > unit) ? ((n_items - 1 - unit) / nunits + 1) * p.n_tiles : 0;
   auto item_of = [&](int64_t i, int& mt, int& sp, int& kb_lo, int& kb_hi) {
-    const int64_t item = (int64_t)blockIdx.x + (i / p.n_tiles) * (int64_t)gridDim.x;
+    const int64_t item = unit + (i / p.n_tiles) * nunits;
     mt = (int)(item / p.splits);
     sp = (int)(item - (int64_t)mt * p.splits);
     kb_lo = sp * p.kbs;
@@ -155,10 +182,19 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
       for (int kb0 = kb_lo; kb0 < kb_hi; kb0 += G) {
         const int n = kb_hi - kb0 < G ? kb_hi - kb0 : G;
         mbar_wait(empty_bar(grp), phase ^ 1u);
-        mbar_arrive_expect_tx_elect(full_bar(grp), (uint32_t)(n * nb_rows) * KB_BYTES);
-        for (int u = 0; u < n; ++u)
-          tma_load_2d_elect(base + (grp * G + u) * STAGE_BYTES + A_BYTES, &tmB, full_bar(grp), (kb0 + u) * BK,
-                            nt * nb_rows);
+        if (CG == 2) {
+          // both CTAs' halves complete on the leader's barrier; only the leader arms it
+          if (rank == 0) mbar_arrive_expect_tx_elect(full_bar(grp), (uint32_t)(n * nb_rows) * KB_BYTES);
+          for (int u = 0; u < n; ++u)
+            tma_load_2d_2sm_elect(base + (grp * G + u) * STAGE_BYTES + A_BYTES, &tmB, full_bar(grp) & PEER_MASK,
+                                  (kb0 + u) * BK, nt * nb_rows + rank * nb_half);
+        } else {
+          mbar_arrive_expect_tx_elect(full_bar(grp), (uint32_t)(n * nb_rows) * KB_BYTES);
+          for (int u = 0; u < n; ++u)
+            tma_load_2d_elect(base + (grp * G + u) * STAGE_BYTES + A_BYTES, &tmB, full_bar(grp), (kb0 + u) * BK,
+                              nt * nb_rows);
+        }
+        __syncwarp();
         if (++grp == NG) {
           grp = 0;
           phase ^= 1u;
@@ -172,8 +208,8 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
     int acc = 0;
     uint32_t acc_phase = 0;
     // kind::f16 operand formats (bits 7..9 A, 10..12 B): 1 = bf16, 0 = IEEE half
-    const uint32_t idesc = instr_desc<INT8>(BM, nb_rows) & ((!INT8 && p.f16) ? ~((1u << 7) | (1u << 10)) : ~0u);
-    for (int64_t i = 0; i < tiles_per_cta; ++i) {
+    const uint32_t idesc = instr_desc<INT8>(BM * CG, nb_rows) & ((!INT8 && p.f16) ? ~((1u << 7) | (1u << 10)) : ~0u);
+    for (int64_t i = 0; rank == 0 && i < tiles_per_cta; ++i) {
       mbar_wait(tempty_bar(acc), acc_phase ^ 1u);
       tc_fence_after();
       const uint32_t d_tmem = tmem_base + (uint32_t)(acc * BN_MAX);
@@ -189,10 +225,11 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
           const uint64_t da = smem_desc(sa), db = smem_desc(sa + A_BYTES);
 #pragma unroll
           for (int k = 0; k < KB_BYTES / 32; ++k)
-            tc_mma_elect<INT8>(d_tmem, da + 2u * k, db + 2u * k, idesc, (kb0 + u != kb_lo || k != 0) ? 1u : 0u);
+            tc_mma_elect<INT8, CG>(d_tmem, da + 2u * k, db + 2u * k, idesc, (kb0 + u != kb_lo || k != 0) ? 1u : 0u);
         }
-        tc_commit_elect(empty_bar(grp));  // frees the group's slots when these MMAs retire
-        if (kb0 + n == kb_hi) tc_commit_elect(tfull_bar(acc));
+        tc_commit_elect<CG>(empty_bar(grp));  // frees the group's slots (in both CTAs) when these MMAs retire
+        if (kb0 + n == kb_hi) tc_commit_elect<CG>(tfull_bar(acc));
+        __syncwarp();
         if (++grp == NG) {
           grp = 0;
           phase ^= 1u;
@@ -208,12 +245,13 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
     const int q = warp & 3;
     int acc = 0;
     uint32_t acc_phase = 0;
-    Top2 run = Top2{NEG_BIG, INT_MAX, NEG_BIG};
+    Top2f run = Top2f{NEG_BIG_F, NEG_BIG_F, 0.0f, 0.0f, INT_MAX, INT_MAX};
+    const bool scaled = p.e.colscale != nullptr;
     for (int64_t i = 0; i < tiles_per_cta; ++i) {
       int mt, sp, kb_lo, kb_hi;
       item_of(i, mt, sp, kb_lo, kb_hi);
       const int nt = (int)(i % p.n_tiles);
-      const int64_t row = (int64_t)mt * BM + q * 32 + lane;
+      const int64_t row = (int64_t)(mt * CG + rank) * BM + q * 32 + lane;
       const bool row_ok = row < p.N;
       mbar_wait(tfull_bar(acc), acc_phase);
       tc_fence_after();
@@ -233,18 +271,27 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
         for (int j = 0; j < 16; ++j) {
           if (c0 + j < k_valid) {
             const int k = k_base + c0 + j;
-            double a;
+            // the accumulator as a float: exact for the integer paths below 2^24, one rounding for the sum of
+            // the three fp32-class parts
+            float a;
             if (INT8) {
-              a = (double)(int)v0[j];
+              a = (float)(int)v0[j];
             } else if (p.nparts == 3) {
-              a = ((double)__uint_as_float(v2[j]) + (double)__uint_as_float(v1[j])) + (double)__uint_as_float(v0[j]);
+              a = __fadd_rn(__fadd_rn(__uint_as_float(v2[j]), __uint_as_float(v1[j])), __uint_as_float(v0[j]));
             } else {
-              a = (double)__uint_as_float(v0[j]);
+              a = __uint_as_float(v0[j]);
             }
             if (p.splits > 1) {
               // partial sum of this split of the reduction axis; split_reduce_kernel adds the splits
               // in a fixed order and applies the epilogue
-              if (row_ok) p.partial[((int64_t)sp * p.N + row) * p.K + k] = a;
+              if (row_ok) {
+                double ad;
+                if (INT8) ad = (double)(int)v0[j];
+                else if (p.nparts == 3)
+                  ad = ((double)__uint_as_float(v2[j]) + (double)__uint_as_float(v1[j])) + (double)__uint_as_float(v0[j]);
+                else ad = (double)__uint_as_float(v0[j]);
+                p.partial[((int64_t)sp * p.N + row) * p.K + k] = ad;
+              }
             } else if (EPI == EPI_SCORE) {
               if (row_ok) {
                 if (p.e.s_i32) {
@@ -252,18 +299,25 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
                   if (p.e.ham_D > 0) iv = (p.e.ham_D - iv) >> 1;
                   reinterpret_cast<int32_t*>(p.e.S)[row * p.e.lds + k] = iv;
                 } else {
-                  const float s = p.e.colscale ? (float)(a * p.e.colscale[k]) : (float)a;
-                  reinterpret_cast<float*>(p.e.S)[row * p.e.lds + k] = s;
+                  reinterpret_cast<float*>(p.e.S)[row * p.e.lds + k] = scaled ? __fmul_rn(a, p.e.colscale_f[k]) : a;
                 }
               }
             } else {
-              const double s = p.e.colscale ? a * p.e.colscale[k] : a;
-              if (s > run.b1) {  // classes arrive in increasing order: strict > keeps the lowest index
-                run.b2 = run.b1;
-                run.b1 = s;
-                run.i1 = k;
-              } else if (s > run.b2) {
-                run.b2 = s;
+              // classes arrive in increasing order: strict > keeps the lowest index
+              const float sc = scaled ? __fmul_rn(a, p.e.colscale_f[k]) : a;
+              bool better = sc > run.b1;
+              if (scaled && fabsf(sc - run.b1) <= 2.0e-6f * fmaxf(fabsf(sc), fabsf(run.b1)) && run.i1 != INT_MAX) {
+                // too close for fp32: the exact products decide (rare)
+                const double ea = INT8 ? (double)(int)v0[j] : (double)a;
+                const double e1 = INT8 ? (double)__float_as_int(run.a1) : (double)run.a1;
+                better = ea * p.e.colscale[k] > e1 * p.e.colscale[run.i1];
+              }
+              const float araw = INT8 ? __uint_as_float(v0[j]) : a;   // integer accumulators are kept bit for bit
+              if (better) {
+                run.b2 = run.b1; run.a2 = run.a1; run.i2 = run.i1;
+                run.b1 = sc; run.a1 = araw; run.i1 = k;
+              } else if (sc > run.b2) {
+                run.b2 = sc; run.a2 = araw; run.i2 = k;
               }
             }
           }
@@ -271,15 +325,21 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
       }
       tc_fence_before();
       __syncwarp();
-      if (lane == 0) mbar_arrive(tempty_bar(acc));
+      if (lane == 0) {
+        if (CG == 2) mbar_arrive_cluster_relaxed(tempty_bar(acc) & PEER_MASK);  // the leader's barrier
+        else mbar_arrive(tempty_bar(acc));
+      }
       if (++acc == 2) {
         acc = 0;
         acc_phase ^= 1u;
       }
       if (EPI == EPI_ARGMAX && nt == p.n_tiles - 1 && p.splits == 1) {
         if (row_ok) {
-          double b1 = run.b1, b2 = run.b2;
-          if (b2 == NEG_BIG) b2 = b1;  // K == 1
+          // reported scores: the exact double products of the two winners (one conversion per row)
+          const double e1 = INT8 ? (double)__float_as_int(run.a1) : (double)run.a1;
+          const double e2 = INT8 ? (double)__float_as_int(run.a2) : (double)run.a2;
+          double b1 = scaled ? e1 * p.e.colscale[run.i1] : e1;
+          double b2 = run.i2 == INT_MAX ? b1 : (scaled ? e2 * p.e.colscale[run.i2] : e2);  // K == 1
           if (p.e.ham_D > 0) {
             b1 = 0.5 * ((double)p.e.ham_D - b1);
             b2 = 0.5 * ((double)p.e.ham_D - b2);
@@ -288,7 +348,7 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
           if (p.e.best) p.e.best[row] = (float)b1;
           if (p.e.second) p.e.second[row] = (float)b2;
         }
-        run = Top2{NEG_BIG, INT_MAX, NEG_BIG};
+        run = Top2f{NEG_BIG_F, NEG_BIG_F, 0.0f, 0.0f, INT_MAX, INT_MAX};
       }
     }
   } else {
@@ -303,6 +363,8 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
     constexpr int C_PER = 8 / (EXW / 4);
     static_assert(EXW == 8, "two expander threads per row");
     constexpr int WPK = INT8 ? 4 : 2;         // packed words per k-block
+    constexpr int QW = qw_of(CG);
+    constexpr int Q_SLOT_WORDS = QW * Q_LD;
     constexpr int KPC = QW / WPK;             // k-blocks per ring tile
     constexpr int WPP = WPK / 2;              // words of a k-block this thread's half needs
     const uint32_t sw = (uint32_t)(t & 7);
@@ -315,20 +377,22 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
       int mt, sp, kb_lo, kb_hi;
       item_of(is_i, mt, sp, kb_lo, kb_hi);
       const int nch = (kb_hi - kb_lo + KPC - 1) / KPC;
-      const int64_t m0 = (int64_t)mt * BM;
-      const int w = (kb_lo / KPC + is_c) * QW + lane;   // kbs is a multiple of KPC
+      const int64_t m0 = (int64_t)(mt * CG + rank) * BM;
+      constexpr int RPW = 32 / QW;                       // rows one warp instruction copies (QW words each)
+      const int wl = lane & (QW - 1), r0 = ew + EXW * (lane / QW);
+      const int w = (kb_lo / KPC + is_c) * QW + wl;      // kbs is a multiple of KPC
       const int64_t rows_left = p.N - m0;
       const int nrow = w < p.W ? (rows_left < BM ? (int)rows_left : BM) : 0;
-      const uint32_t* src = p.Hbits + (m0 + ew) * p.ldh + w;
-      uint32_t dst = q_smem + (uint32_t)(is_slot * Q_SLOT_WORDS + lane * Q_LD + ew) * 4u;
+      const uint32_t* src = p.Hbits + (m0 + r0) * p.ldh + w;
+      uint32_t dst = q_smem + (uint32_t)(is_slot * Q_SLOT_WORDS + wl * Q_LD + r0) * 4u;
 #pragma unroll 4
-      for (int rr = ew; rr < BM; rr += EXW) {
+      for (int rr = r0; rr < BM; rr += EXW * RPW) {
         const bool ok = rr < nrow;
         asm volatile("cp.async.ca.shared.global [%0], [%1], 4, %2;" ::"r"(dst), "l"(ok ? src : p.Hbits),
                      "r"(ok ? 4 : 0)
                      : "memory");
-        src += EXW * p.ldh;
-        dst += EXW * 4u;
+        src += EXW * RPW * p.ldh;
+        dst += EXW * RPW * 4u;
       }
       if (++is_slot == Q_SLOTS) is_slot = 0;
       if (++is_c == nch) {
@@ -401,7 +465,10 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
           // the group is published with one proxy fence and one arrival per warp
           fence_proxy_async_smem();
           __syncwarp();
-          if (lane == 0) mbar_arrive(full_bar(grp));
+          if (lane == 0) {
+            if (CG == 2) mbar_arrive_remote(full_bar(grp) & PEER_MASK);   // the leader's barrier, from either CTA
+            else mbar_arrive(full_bar(grp));
+          }
           if (++grp == NG) {
             grp = 0;
             phase ^= 1u;
@@ -415,10 +482,10 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
   }
 
   tc_fence_before();
-  __syncthreads();
+  if (CG == 2) cluster_sync_all(); else __syncthreads();
   if (warp == 1) {
     tc_fence_after();
-    tmem_dealloc(tmem_base, TMEM_COLS);
+    tmem_dealloc<CG>(tmem_base, TMEM_COLS);
   }
 }
 
@@ -520,15 +587,30 @@ __global__ void split_reduce_kernel(const double* __restrict__ partial, int spli
   }
 }
 
-template <bool INT8, int EPI>
-cudaError_t launch_one(const CUtensorMap& tmB, const SimParams& p, int grid, cudaStream_t st) {
+template <bool INT8, int EPI, int CG>
+cudaError_t launch_cg(const CUtensorMap& tmB, const SimParams& p, int grid, cudaStream_t st) {
   // per-device attribute of the function: set on every launch (handles on several devices of one process)
-  cudaError_t e = cudaFuncSetAttribute(sim_tc_kernel<INT8, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+  cudaError_t e = cudaFuncSetAttribute(sim_tc_kernel<INT8, EPI, CG>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                        SMEM_LIMIT);
   if (e != cudaSuccess) return e;
-  const int smem = p.stages * p.stage_bytes + SMEM_EXTRA + QRING_BYTES;
-  sim_tc_kernel<INT8, EPI><<<grid, NTHREADS, smem, st>>>(tmB, p);
-  return cudaGetLastError();
+  const int smem = p.stages * p.stage_bytes + SMEM_EXTRA + qring_bytes(CG);
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)grid);
+  cfg.blockDim = dim3(NTHREADS);
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeClusterDimension;
+  at[0].val.clusterDim.x = CG;
+  at[0].val.clusterDim.y = 1;
+  at[0].val.clusterDim.z = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, sim_tc_kernel<INT8, EPI, CG>, tmB, p);
+}
+template <bool INT8, int EPI>
+cudaError_t launch_one(const CUtensorMap& tmB, const SimParams& p, int cg, int grid, cudaStream_t st) {
+  return cg == 2 ? launch_cg<INT8, EPI, 2>(tmB, p, grid, st) : launch_cg<INT8, EPI, 1>(tmB, p, grid, st);
 }
 
 void sim_tc_shape(int K, int hv_bits, int D_eff, int& kc, int& nparts, int& n_tiles, int& num_kb, bool& int8) {
@@ -584,7 +666,7 @@ size_t sim_tc_partial_bytes(int64_t N, int K, int hv_bits, int D_eff, int sm_cou
 cudaError_t launch_sim_tc(TcContext* tc, const uint32_t* Hbits, int64_t N, int64_t ldh, const float* C_acc,
                           int K, int64_t ldc, int D_eff, int hv_bits, void* cop, float* amax_scratch,
                           const Epilogue& e, Perf pf, double* partial, bool cop_ready, bool prep_only, int sm_count,
-                          cudaStream_t st, int64_t* nlaunch) {
+                          int force_cg, cudaStream_t st, int64_t* nlaunch) {
   if (!tc) return cudaErrorNotSupported;
   if (N <= 0 && !prep_only) return cudaSuccess;
   if ((reinterpret_cast<uintptr_t>(cop) & 15) != 0) return cudaErrorNotSupported;
@@ -614,8 +696,12 @@ cudaError_t launch_sim_tc(TcContext* tc, const uint32_t* Hbits, int64_t N, int64
     if (ce != cudaSuccess) return ce;
   }
   if (prep_only) return cudaSuccess;
+  // CTA pairs once every pair has a 256-query tile of its own and the class tile is wide enough for the
+  // shared-memory traffic to be the limit (small K is bound by the expansion itself)
+  int cg = (sm_count >= 2 && K >= 128 && (N + 2 * BM - 1) / (2 * BM) >= sm_count / 2) ? 2 : 1;
+  if (force_cg == 1 || (force_cg == 2 && sm_count >= 2)) cg = force_cg;
   CUtensorMap tmB;
-  if (!tc_make_map(tc, &tmB, cop, int8, rows_total, ld, ld, nparts * kc)) return cudaErrorInvalidValue;
+  if (!tc_make_map(tc, &tmB, cop, int8, rows_total, ld, ld, nparts * kc / cg)) return cudaErrorInvalidValue;
   SimParams p;
   p.Hbits = Hbits;
   p.N = N;
@@ -624,36 +710,37 @@ cudaError_t launch_sim_tc(TcContext* tc, const uint32_t* Hbits, int64_t N, int64
   p.K = K;
   p.kc = kc;
   p.nparts = nparts;
-  p.m_tiles = (int)((N + BM - 1) / BM);
+  p.m_tiles = (int)((N + BM * cg - 1) / (BM * cg));
   p.n_tiles = n_tiles;
   p.num_kb = num_kb;
   p.f16 = hv_bits == HDC_HV_F16;
-  p.stage_bytes = A_BYTES + nparts * kc * KB_BYTES;
-  p.stages = (SMEM_LIMIT - SMEM_EXTRA - QRING_BYTES) / p.stage_bytes;
+  p.stage_bytes = A_BYTES + nparts * kc / cg * KB_BYTES;
+  p.stages = (SMEM_LIMIT - SMEM_EXTRA - qring_bytes(cg)) / p.stage_bytes;
   if (p.stages > MAX_STAGES) p.stages = MAX_STAGES;
   // k-blocks per pipeline group: every hand-off through the full / empty barriers costs several hundred
   // cycles whatever the k-block holds, so short k-blocks (few class rows) travel in groups
-  p.kps = p.stages >= 8 ? 4 : (p.stages >= 4 ? 2 : 1);
+  p.kps = p.stages >= 8 ? 4 : (p.stages >= 4 ? 2 : 1);   // (divides the k-blocks of a ring tile: 16 / 8 / 4)
   p.stages -= p.stages % p.kps;
   p.e = e;
-  p.splits = partial ? sim_tc_splits(N, K, hv_bits, D_eff, sm_count, &p.kbs) : 1;
+  p.splits = (partial && cg == 1) ? sim_tc_splits(N, K, hv_bits, D_eff, sm_count, &p.kbs) : 1;
   if (p.splits == 1) p.kbs = num_kb;
   p.partial = partial;
   const int64_t items = (int64_t)p.m_tiles * p.splits;
-  const int grid = (int)(items < sm_count ? items : sm_count);
+  const int max_units = sm_count / cg;
+  const int grid = (int)(items < max_units ? items : max_units) * cg;
   ++*nlaunch;
   if (p.splits > 1) {
-    ce = int8 ? launch_one<true, EPI_SCORE>(tmB, p, grid, st) : launch_one<false, EPI_SCORE>(tmB, p, grid, st);
+    ce = int8 ? launch_one<true, EPI_SCORE>(tmB, p, 1, grid, st) : launch_one<false, EPI_SCORE>(tmB, p, 1, grid, st);
     if (ce != cudaSuccess) return ce;
     split_reduce_kernel<<<(unsigned)((N + 127) / 128), 128, 0, st>>>(partial, p.splits, N, K, e);
     ++*nlaunch;
     return cudaGetLastError();
   }
   if (int8)
-    return e.kind == EPI_SCORE ? launch_one<true, EPI_SCORE>(tmB, p, grid, st)
-                               : launch_one<true, EPI_ARGMAX>(tmB, p, grid, st);
-  return e.kind == EPI_SCORE ? launch_one<false, EPI_SCORE>(tmB, p, grid, st)
-                             : launch_one<false, EPI_ARGMAX>(tmB, p, grid, st);
+    return e.kind == EPI_SCORE ? launch_one<true, EPI_SCORE>(tmB, p, cg, grid, st)
+                               : launch_one<true, EPI_ARGMAX>(tmB, p, cg, grid, st);
+  return e.kind == EPI_SCORE ? launch_one<false, EPI_SCORE>(tmB, p, cg, grid, st)
+                             : launch_one<false, EPI_ARGMAX>(tmB, p, cg, grid, st);
 }
 
 }  // namespace hdc

@@ -87,6 +87,13 @@ __device__ __forceinline__ void cluster_sync_all() {
 __device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_addr) {
   asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
 }
+// Arrival on a barrier of another CTA of the cluster with the default semantics (release at CTA scope): for a
+// hand-off whose data was written to THIS CTA's shared memory and made visible to the async proxy by
+// fence.proxy.async (the tensor core that reads it is this SM's own, driven by the pair's leader), so that no
+// cluster- or GPU-scope memory barrier is needed in front of the arrive.
+__device__ __forceinline__ void mbar_arrive_remote(uint32_t cluster_addr) {
+  asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
+}
 // Same without memory ordering.  For hand-offs that publish no generic-proxy memory: an epilogue warp
 // returning a TMEM accumulator has already waited for its tcgen05.ld (tcgen05.wait::ld) and fenced the
 // tensor proxy (tcgen05.fence::before_thread_sync).  The .release.cluster form compiles to MEMBAR.ALL.GPU +

@@ -171,14 +171,17 @@ def test_contraction_repeats_bit_for_bit(hd, h, prec, N, D_eff, flags):
     assert int(bad.item()) == 0
 
 
+@pytest.mark.parametrize("flags", [0, 4])
 @pytest.mark.parametrize("hv_bits,sim,N,K,D_eff", [(32, "COS", 300, 26, 10000), (16, "COS", 129, 1000, 4100),
-                                                   (1, "HAMMING", 777, 100, 10000), (8, "COS", 6238, 26, 10000)])
-def test_similarity_repeats_bit_for_bit(hd, h, hv_bits, sim, N, K, D_eff):
-    """sim_tc_kernel (bit expanders + TMA + tcgen05, with and without the split reduction axis) 200 times."""
+                                                   (1, "HAMMING", 777, 100, 10000), (8, "COS", 6238, 26, 10000),
+                                                   (16, "COS", 74 * 256 + 130, 300, 1100)])
+def test_similarity_repeats_bit_for_bit(hd, h, hv_bits, sim, N, K, D_eff, flags):
+    """sim_tc_kernel (bit expanders + TMA + tcgen05; one CTA with and without the split reduction axis, CTA pairs
+    with flags = HDC_FLAG_TC_2CTA or by size) 200 times."""
     r = np.random.default_rng([37, N, K])
     bits = r.integers(0, 2, size=(N, D_eff), dtype=np.uint8)
     C = (9 - 2 * r.binomial(9, 0.5, size=(K, D_eff))).astype(np.float32)
-    kn = hd.knobs(D_eff, hv_bits=hv_bits, sim=getattr(hd, "HDC_SIM_" + sim))
+    kn = hd.knobs(D_eff, hv_bits=hv_bits, sim=getattr(hd, "HDC_SIM_" + sim), flags=flags)
     Hd, Cd = dev_bits(bits), dev(C)
     m = h.hdc_model_prepare(None, Cd, kn)
     lab0, b0, s0 = h.hdc_classify_m(Hd, m, want_scores=True)

@@ -249,6 +249,53 @@ def test_dot_cos_similarity_and_classify(hd, h, sim, hv_bits, N, K, D, D_eff):
     assert np.allclose(sec.cpu().numpy()[same], sec_or[same], rtol=1e-3, atol=1e-5)
 
 
+@pytest.mark.parametrize("sim,hv_bits", [("COS", 32), ("DOT", 16), ("COS", 17), ("COS", 8), ("DOT", 8), ("DOT", 1), ("HAMMING", 1)])
+@pytest.mark.parametrize("N,K,D,D_eff,perf", [(300, 26, 2100, 2100, (0, 1)), (129, 1000, 520, 520, (0, 1)), (513, 200, 1300, 1000, (0, 1)),
+                                              (1, 70, 700, 33, (0, 1)), (257, 600, 1300, 1000, (3, 8)), (640, 6, 10000, 4099, (0, 1))])
+def test_similarity_on_cta_pairs(hd, h, sim, hv_bits, N, K, D, D_eff, perf):
+    """sim_tc_kernel on CTA pairs (cta_group::2, HDC_FLAG_TC_2CTA forces it at any size): odd numbers of 256-query
+    tiles, a pair whose peer has no valid row, class tiles of every width, perforation; scores and labels by the same
+    rules as the one-CTA kernel, which must also give the same labels."""
+    r = rng(55, N, K, D_eff, hv_bits)
+    hb = r.integers(0, 2, size=(N, D), dtype=np.uint8)
+    C = (r.standard_normal((K, D)) * 30).astype(np.float32)
+    C[r.random((K, D)) < 0.03] = 0.0
+    if K > 3:
+        C[3] = 0.0
+        C[2] = C[1]                                         # exact tie -> lowest index
+    simc = getattr(O, "SIM_" + sim)
+    S_or = O.similarity(hb, C, D_eff, simc, hv_bits, perf[0], perf[1])
+    lab_or, best_or, sec_or = O.classify(S_or, simc)
+    Hd, Cd = dev_bits(hb), dev(C)
+    out = {}
+    for flags in (hd.HDC_FLAG_TC_2CTA, hd.HDC_FLAG_TC_1CTA):
+        kn = hd.knobs(D_eff, hv_bits=hv_bits, sim=getattr(hd, "HDC_SIM_" + sim), flags=flags, perf_begin=perf[0],
+                      perf_stride=perf[1])
+        S = h.hdc_similarity(Hd, Cd, kn).cpu().numpy()
+        lab, best, sec = h.hdc_classify(Hd, Cd, kn, want_scores=True)
+        lab = lab.cpu().numpy()
+        if hv_bits in (8, 1):
+            if sim == "COS":
+                assert np.allclose(S, S_or, rtol=1e-6, atol=1e-9)
+            else:
+                assert np.array_equal(S.astype(np.float64), S_or)
+            assert np.array_equal(lab, lab_or)
+            assert np.allclose(best.cpu().numpy(), best_or, rtol=1e-6, atol=1e-9)
+            assert np.allclose(sec.cpu().numpy(), sec_or, rtol=1e-6, atol=1e-9)
+        else:
+            cop = O.class_operand(C[:, perf[0]:D_eff:perf[1]], len(range(perf[0], D_eff, perf[1])), hv_bits)
+            floor = 1e-6 * np.sqrt(cop.shape[1]) * np.sqrt((cop * cop).sum(axis=1))[None, :] if sim == "DOT" else 1e-6
+            check_scores(S, S_or, floor)
+            check_labels_float(lab, S_or, simc)
+        out[flags] = (S, lab)
+    if hv_bits in (8, 1):
+        if sim == "COS":   # (the split-reduction path of the one-CTA kernel scales in double, the others in fp32)
+            assert np.allclose(out[hd.HDC_FLAG_TC_2CTA][0], out[hd.HDC_FLAG_TC_1CTA][0], rtol=1e-6, atol=1e-9)
+        else:
+            assert np.array_equal(out[hd.HDC_FLAG_TC_2CTA][0], out[hd.HDC_FLAG_TC_1CTA][0])
+        assert np.array_equal(out[hd.HDC_FLAG_TC_2CTA][1], out[hd.HDC_FLAG_TC_1CTA][1])
+
+
 def test_classify_ties_go_to_lowest_index(hd, h):
     r = rng(6)
     N, K, D = 90, 9, 640
