@@ -697,8 +697,9 @@ cudaError_t launch_sim_tc(TcContext* tc, const uint32_t* Hbits, int64_t N, int64
   }
   if (prep_only) return cudaSuccess;
   // CTA pairs once every pair has a 256-query tile of its own and the class tile is wide enough for the
-  // shared-memory traffic to be the limit (small K is bound by the expansion itself)
-  int cg = (sm_count >= 2 && K >= 128 && (N + 2 * BM - 1) / (2 * BM) >= sm_count / 2) ? 2 : 1;
+  // shared-memory traffic to matter: K >= 128, or the three-part fp32 class operand (measured at K = 26: 0.338 ->
+  // 0.294 ms per 131072 queries; bf16 / int8 classes at small K are bound by the expansion itself and lose 5-15 %)
+  int cg = (sm_count >= 2 && (K >= 128 || nparts == 3) && (N + 2 * BM - 1) / (2 * BM) >= sm_count / 2) ? 2 : 1;
   if (force_cg == 1 || (force_cg == 2 && sm_count >= 2)) cg = force_cg;
   CUtensorMap tmB;
   if (!tc_make_map(tc, &tmB, cop, int8, rows_total, ld, ld, nparts * kc / cg)) return cudaErrorInvalidValue;
