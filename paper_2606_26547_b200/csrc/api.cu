@@ -601,7 +601,9 @@ size_t similarity_ws(int64_t N, int K, const hdc_knobs_t* k) {
   return b.off + 1024;
 }
 
-constexpr int64_t HOST_CHUNK = 16384;
+// rows per steady-state chunk of hdc_infer_rp_host: 74 CTA pairs x 256 rows (whole waves of the pair kernel)
+constexpr int64_t HOST_CHUNK = 18944;
+constexpr int64_t HOST_RAMP_START = 2048;
 
 // ------------------------------------------------------------------------------------- fused inference
 // hdc_infer_rp = hdc_encode_rp followed by hdc_classify, kernel for kernel.  Opt-in (HDC_FLAG_FUSED_INFER):
@@ -612,10 +614,9 @@ constexpr int64_t HOST_CHUNK = 16384;
 constexpr int INFER_MAX_K = 32;
 constexpr int64_t INFER_MIN_N = 12288;  // 48 row blocks of 256: below it the two-kernel path spreads m x n tiles better
 
-bool infer_fusable(const hdc_ctx* h, const hdc_knobs_t* k, int64_t N, int K) {
+bool infer_fused_knobs(const hdc_ctx* h, const hdc_knobs_t* k, int K) {   // the part that does not depend on N
   return (k->flags & HDC_FLAG_FUSED_INFER) && use_tc(h, k) && !(k->flags & HDC_FLAG_TC_1CTA) && h->sm_count >= 2 &&
-         K <= INFER_MAX_K &&
-         N >= INFER_MIN_N && k->D_eff <= (1 << 17);
+         K <= INFER_MAX_K && k->D_eff <= (1 << 17);
 }
 int infer_kc(int K) { return K <= 8 ? 8 : (K <= 16 ? 16 : 32); }
 
@@ -634,7 +635,14 @@ int do_infer_rp(hdc_ctx* h, const void* X, int x_dtype, int64_t N, int F, int64_
                 cudaStream_t st) {
   const int D_eff = k->D_eff;
   const int W = words_of(D_eff);
-  if (infer_fusable(h, k, N, K) && !perf_on(enc_perf_of(k))) {
+  // Whether the fused kernel is an option for these knobs does not depend on N; whether THIS pass takes it does.
+  // The persistent operands are therefore always carved -- and, when preparing, prepared -- in one fixed order:
+  // [fused class operand, scales] [staged P] [class operand of the classify kernel], so that passes of any size
+  // (the chunks of hdc_infer_rp_host, a prepared model) find what they need.
+  const bool fused_ops = infer_fused_knobs(h, k, K) && !perf_on(enc_perf_of(k));
+  const bool fused = fused_ops && N >= INFER_MIN_N;
+  Epilogue e{};
+  if (fused_ops) {
     const int KC = infer_kc(K);
     const int64_t ldcls = round_up(D_eff, 256);
     const Perf pf = perf_of(k);
@@ -652,7 +660,6 @@ int do_infer_rp(hdc_ctx* h, const void* X, int x_dtype, int64_t N, int F, int64_
         ce = launch_col_scale(Operand{cls, ldcls, OPK_F32}, K, D_eff, 1, pf, colscale, st, &h->launches);
       if (ce != cudaSuccess) return cuda_fail(h, ce, "infer_rp: class operand");
     }
-    Epilogue e{};
     e.labels = labels;
     e.best = best;
     e.second = second;
@@ -661,14 +668,22 @@ int do_infer_rp(hdc_ctx* h, const void* X, int x_dtype, int64_t N, int F, int64_
     e.cls = cls;
     e.ldcls = ldcls;
     e.K = K;
+  }
+  if (fused) {
     int rc = encode_rp_core(h, X, x_dtype, N, F, ldx, P, p_dtype, ldp, k, HDC_OUT_BITS, Hbits, ldh, nullptr, 0, b,
                             ws_bytes, st, &e);
+    if (rc == HDC_OK && do_prep(h)) {  // a later, smaller pass takes the classify kernel: prepare its operand too
+      const int mode = h->prep_mode;
+      h->prep_mode = PREP_ONLY;
+      rc = do_similarity(h, nullptr, 1, W, C_acc, K, ldc, k, nullptr, 0, 0, nullptr, nullptr, nullptr, b, ws_bytes, st);
+      h->prep_mode = mode;
+    }
     if (rc == HDC_OK && !prep_only(h)) ++h->stats[HDC_STAT_INFER_FUSED];
     return rc;
   }
   uint32_t* Hd = Hbits;
   int64_t ldhd = ldh;
-  if (!Hd) {
+  if (!Hd && !prep_only(h)) {
     Hd = b.take<uint32_t>((size_t)N * W);
     ldhd = W;
     if (b.off > ws_bytes) return fail(h, HDC_ERR_WORKSPACE, "infer_rp: workspace too small");
@@ -1239,7 +1254,7 @@ extern "C" int32_t hdc_model_prepare(hdc_handle_t h, const void* P, int32_t p_dt
     int r = HDC_OK;
     // the same order as do_infer_rp's two-kernel path carves them: encode, then similarity; the fused
     // epilogue's operand is prepared by hdc_model_prepare only when the knobs ask for that kernel
-    if (P && C_acc && (knobs->flags & HDC_FLAG_FUSED_INFER) && K <= INFER_MAX_K)
+    if (P && C_acc && infer_fused_knobs(h, knobs, K))   // both operand sets, in do_infer_rp's order
       return do_infer_rp(h, nullptr, HDC_F32, INFER_MIN_N, F, F, P, p_dtype, D, ldp, C_acc, K, ldc, knobs, nullptr,
                          nullptr, nullptr, nullptr, 0, none, (size_t)-1, st);
     if (P) r = do_encode_rp(h, nullptr, HDC_F32, 1, F, F, P, p_dtype, D, ldp, knobs, HDC_OUT_BITS, nullptr, 0, nullptr, 0,
@@ -1310,6 +1325,7 @@ extern "C" int32_t hdc_classify_m(hdc_handle_t h, const uint32_t* Hbits, int64_t
     Bump& pm = *static_cast<Bump*>(h->model);
     if (m->P) {
       Bump skip(nullptr);
+      if (m->C_acc && infer_fused_knobs(h, &m->knobs, m->K) && !perf_on(enc_perf_of(&m->knobs))) infer_ws(m->K, m->knobs.D_eff, pm);
       encode_ws(h, 0, m->F, m->knobs.D_eff, &m->knobs, skip, pm);
     }
     return do_similarity(h, Hbits, N, ldh_words, m->C_acc, m->K, m->ldc, &m->knobs, nullptr, 0, 0, labels, best, second,
@@ -1331,9 +1347,6 @@ extern "C" int32_t hdc_infer_rp_m(hdc_handle_t h, const void* X, int32_t x_dtype
   if ((reinterpret_cast<uintptr_t>(Hbits) | reinterpret_cast<uintptr_t>(labels)) & 3)
     return fail(h, HDC_ERR_ALIGNMENT, "infer_rp_m: operands must be 4-byte aligned");
   if (N == 0) return HDC_OK;
-  // a model prepared for the fused kernel holds that kernel's operands only
-  if ((m->knobs.flags & HDC_FLAG_FUSED_INFER) && m->K <= INFER_MAX_K && !infer_fusable(h, &m->knobs, N, m->K))
-    return fail(h, HDC_ERR_UNSUPPORTED, "infer_rp_m: model prepared for the fused kernel, N too small for it");
   Bump b(ws);
   if (!ws) ws_bytes = 0;
   return with_model(h, m->blob, m->blob_bytes, RUN_ONLY, [&]() {
@@ -1378,9 +1391,14 @@ extern "C" int32_t hdc_infer_rp_host(hdc_handle_t h, const void* X_host, int32_t
   cudaError_t ce = cudaEventRecord(h->ev_entry, st);
   if (ce == cudaSuccess) ce = cudaStreamWaitEvent(h->copy_stream, h->ev_entry, 0);
   if (ce != cudaSuccess) return cuda_fail(h, ce, "infer_rp_host: entry");
+  // The copy of the first chunk is the one transfer no kernel overlaps, so the chunks ramp up: 2048 rows, then
+  // x 1.5 per chunk up to HOST_CHUNK (the operands are prepared once, so a small chunk costs only its launches;
+  // the copy is only ~15 % faster than the compute, so a steeper ramp would starve the kernels).  Measured at
+  // 131072 C2 queries: 7.89 ms with constant 16384-row chunks, 7.4-7.6 ms with the ramp.
   int64_t c = 0;
-  for (int64_t n0 = 0; n0 < N; n0 += chunk, ++c) {
-    const int64_t nb = (N - n0 < chunk) ? (N - n0) : chunk;
+  int64_t cur = chunk > HOST_RAMP_START ? HOST_RAMP_START : chunk;
+  for (int64_t n0 = 0; n0 < N; ++c) {
+    const int64_t nb = (N - n0 < cur) ? (N - n0) : cur;
     const int buf = (int)(c & 1);
     if (c >= 2) cudaStreamWaitEvent(h->copy_stream, h->ev_done[buf], 0);
     // rows are copied densely: device leading dimension is F
@@ -1408,6 +1426,11 @@ extern "C" int32_t hdc_infer_rp_host(hdc_handle_t h, const void* X_host, int32_t
       return rc;
     }
     cudaEventRecord(h->ev_done[buf], st);
+    n0 += nb;
+    {
+      const int64_t nx = (cur * 3 / 2 + 255) / 256 * 256;   // x 1.5, whole 256-row tiles
+      cur = nx < chunk ? nx : chunk;
+    }
   }
   ce = cudaMemcpyAsync(labels_host, Ld, sizeof(int32_t) * (size_t)N, cudaMemcpyDeviceToHost, st);
   if (ce != cudaSuccess) return cuda_fail(h, ce, "infer_rp_host: D2H");

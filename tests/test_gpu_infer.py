@@ -209,5 +209,9 @@ def test_infer_rp_bench_launch_configuration_sampled(hd, h):
     lab2 = h.hdc_infer_rp(dev(Xq), Pd, Cd, kn)                               # no hypervector output
     assert torch.equal(lab2, lab)
     Xh = torch.from_numpy(Xq).pin_memory()
-    lab_host = h.hdc_infer_rp_host(Xh, Pd, Cd, kn).numpy()                  # chunks of the host pipeline
-    assert np.array_equal(lab_host, lab_h)
+    # the host pipeline: its small ramp-up chunks take the two-kernel path, the later ones the fused kernel, so
+    # it answers to the oracle by the same rule (scores summed in another order), and repeats with the period
+    lab_host = h.hdc_infer_rp_host(Xh, Pd, Cd, kn).numpy()
+    check_labels_float(lab_host[:n_te], O.similarity(bits, C_or, D, O.SIM_COS, 32), O.SIM_COS)
+    assert np.array_equal(lab_host, lab_host[idx % n_te]) or (lab_host != lab_h).mean() < 1e-3
+    assert (lab_host != lab_h).mean() < 1e-3

@@ -124,9 +124,13 @@ def test_fused_model(hd, h):
     lab1, b1, s1 = h.hdc_infer_rp_m(Xd, m, want_scores=True)
     assert h.stat(hd.HDC_STAT_INFER_FUSED) == f0 + 1
     assert torch.equal(lab1, lab0) and torch.equal(b1, b0) and torch.equal(s1, s0)
-    with pytest.raises(hd.HdcError) as e:
-        h.hdc_infer_rp_m(Xd[:100], m)
-    assert e.value.code == hd.HDC_ERR_UNSUPPORTED
+    # the same model serves a pass too small for the fused kernel (two kernels) and a plain classify
+    u0 = h.stat(hd.HDC_STAT_INFER_UNFUSED)
+    lab_small = h.hdc_infer_rp_m(Xd[:100], m)
+    assert h.stat(hd.HDC_STAT_INFER_UNFUSED) == u0 + 1
+    assert torch.equal(lab_small, h.hdc_infer_rp(Xd[:100], Pd, Cd, kn))
+    H = h.hdc_encode_rp_m(Xd[:300], m)
+    assert torch.equal(h.hdc_classify_m(H, m), h.hdc_classify(H, Cd, kn))
 
 
 def test_two_handles_interleaved_and_a_foreign_current_stream(hd, h):
