@@ -137,24 +137,28 @@ constexpr double NEG_BIG = -1.0e300;
 // time share B tiles and reuse A tiles from L2.
 // (CG = 2: the unit that walks the tiles is the cluster, and an m-tile is 256 rows.)
 template <int EPI, int CG>
-__device__ __forceinline__ bool tile_at(const TcParams& p, int64_t i, int& mt, int& nt) {
-  const int64_t unit = blockIdx.x / CG, nunits = gridDim.x / CG;
+__device__ __forceinline__ bool tile_at(const TcParams& p, int i, int& mt, int& nt) {
+  // 32-bit arithmetic (launch_gemm_tc bounds the tile count): every role calls this once per tile, and 64-bit
+  // divisions cost the producer warp several hundred cycles of a 2560-cycle int8 tile
+  const unsigned unit = blockIdx.x / CG, nunits = gridDim.x / CG;
   if (EPI == EPI_ARGMAX || EPI == EPI_INFER) {
-    const int64_t u = unit + (i / p.n_tiles) * nunits;
-    if (u >= p.m_tiles) return false;
+    const unsigned q = (unsigned)i / (unsigned)p.n_tiles;
+    const unsigned u = unit + q * nunits;
+    if (u >= (unsigned)p.m_tiles) return false;
     mt = (int)u;
-    nt = (int)(i % p.n_tiles);
+    nt = (int)((unsigned)i - q * (unsigned)p.n_tiles);
     return true;
   }
-  const int64_t t = unit + i * nunits;
-  if (t >= (int64_t)p.m_tiles * p.n_tiles) return false;
-  const int64_t gsz = (int64_t)p.group_m * p.n_tiles;
-  const int64_t g = t / gsz;
-  const int r = (int)(t - g * gsz);
-  int gm = p.m_tiles - (int)g * p.group_m;
-  if (gm > p.group_m) gm = p.group_m;
-  mt = (int)g * p.group_m + r % gm;
-  nt = r / gm;
+  const unsigned t = unit + (unsigned)i * nunits;
+  if (t >= (unsigned)p.m_tiles * (unsigned)p.n_tiles) return false;
+  const unsigned gsz = (unsigned)p.group_m * (unsigned)p.n_tiles;
+  const unsigned g = t / gsz;
+  const unsigned r = t - g * gsz;
+  unsigned gm = (unsigned)p.m_tiles - g * (unsigned)p.group_m;
+  if (gm > (unsigned)p.group_m) gm = (unsigned)p.group_m;
+  const unsigned rq = r / gm;
+  mt = (int)(g * (unsigned)p.group_m + (r - rq * gm));
+  nt = (int)rq;
   return true;
 }
 
@@ -215,7 +219,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     int stage = 0;
     uint32_t phase = 0;
     int mt, nt;
-    for (int64_t i = 0; tile_at<EPI, CG>(p, i, mt, nt); ++i) {
+    for (int i = 0; tile_at<EPI, CG>(p, i, mt, nt); ++i) {
       const int n0 = nt * BN;
       int nb = 0;
       if (CG == 2) {  // this CTA stages rows [rank * N/2, +N/2) of the tile's N (rounded to 16) columns
@@ -231,11 +235,11 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
         tma_load_2d_elect(cls0 + cs * CLS_BYTES, &tmC, cfull_bar(cs), n0, 0);
         __syncwarp();
       }
+      // k-blocks in segment order (no division in this loop: the producer shares its scheduler with two
+      // epilogue warps and has one k-block per 512 tensor cycles to issue)
+      int seg = 0, j = 0;
+      int acol = (int)(p.a_segs & 15u) * p.seg_stride, bcol = (int)(p.b_segs & 15u) * p.seg_stride;
       for (int kb = 0; kb < num_kb; ++kb) {
-        const int seg = kb / p.nkb_seg;
-        const int j = kb - seg * p.nkb_seg;
-        const int acol = (int)((p.a_segs >> (4 * seg)) & 15u) * p.seg_stride + j * BK;
-        const int bcol = (int)((p.b_segs >> (4 * seg)) & 15u) * p.seg_stride + j * BK;
         mbar_wait(empty_bar(stage), phase ^ 1u);
         {
           const uint32_t sa = base + stage * STAGE_BYTES;
@@ -255,6 +259,14 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
           stage = 0;
           phase ^= 1u;
         }
+        acol += BK;
+        bcol += BK;
+        if (++j == p.nkb_seg) {
+          j = 0;
+          ++seg;
+          acol = (int)((p.a_segs >> (4 * seg)) & 15u) * p.seg_stride;
+          bcol = (int)((p.b_segs >> (4 * seg)) & 15u) * p.seg_stride;
+        }
       }
     }
   } else if (warp == 1) {
@@ -264,7 +276,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     int acc = 0;
     uint32_t acc_phase = 0;
     int mt, nt;
-    for (int64_t i = 0; rank == 0 && tile_at<EPI, CG>(p, i, mt, nt); ++i) {
+    for (int i = 0; rank == 0 && tile_at<EPI, CG>(p, i, mt, nt); ++i) {
       int n_valid = p.Nc - nt * BN;
       if (n_valid > BN) n_valid = BN;
       // kind::f16 operand formats (bits 7..9 A, 10..12 B): 1 = bf16, 0 = IEEE half
@@ -315,7 +327,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
 #pragma unroll
     for (int k = 0; k < (KC > 0 ? KC : 1); ++k) irun[k] = 0.0f;
     int mt, nt;
-    for (int64_t i = 0; tile_at<EPI, CG>(p, i, mt, nt); ++i) {
+    for (int i = 0; tile_at<EPI, CG>(p, i, mt, nt); ++i) {
       const int n0 = nt * BN;
       int n_valid = p.Nc - n0;
       if (n_valid > BN) n_valid = BN;
@@ -636,6 +648,7 @@ cudaError_t launch_gemm_tc(TcContext* tc, const TcOperands& o, int64_t M, int Nc
     return cudaErrorNotSupported;
   if (M > (int64_t)INT_MAX - 2 * BM || o.cols_a > INT_MAX || o.cols_b > INT_MAX) return cudaErrorNotSupported;
   const int n_tiles = (Nc + BN - 1) / BN;
+  if ((M + BM - 1) / BM * (int64_t)n_tiles > (int64_t)INT_MAX / 2) return cudaErrorNotSupported;  // 32-bit tile indices
   const bool infer = e.kind == EPI_INFER;
   if (infer && (sm_count < 2 || e.K < 1 || e.K > 32 || Nc > (1 << 17) || !e.cls || (e.ldcls % BN) != 0 || e.ldcls < (int64_t)n_tiles * BN ||
                 (reinterpret_cast<uintptr_t>(e.cls) & 15) || !e.labels))
