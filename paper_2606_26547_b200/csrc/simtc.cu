@@ -8,7 +8,7 @@
 // layout TMA would have written), while the class operand arrives by TMA.  Roles (14 warps, one
 // persistent CTA per SM): warp 0 = TMA producer (class tiles), warp 1 = MMA issuer + TMEM
 // allocation, warps 2-5 = epilogue (thread = query row), warps 6-13 = expanders (thread = query row
-// x half of a k-block; the packed words reach them through a cp.async ring).  Producer, expanders and
+// x half of a k-block; the packed words reach each warp through a private cp.async ring).  Producer, expanders and
 // issuer hand k-blocks over in groups (one full / empty barrier pair, one proxy fence, one commit per
 // group); for small N the reduction axis is split over several CTAs per m-tile (split_reduce_kernel
 // adds the partial sums in a fixed order).
@@ -53,12 +53,17 @@ constexpr int NTHREADS = 192 + 32 * EXW;
 constexpr int TMEM_COLS = 512;
 constexpr int SMEM_LIMIT = 227 * 1024;
 constexpr int SMEM_EXTRA = 1024 /*alignment slack*/ + 256 /*barriers*/;
-// packed words per row in one tile of the query ring: 32 for the one-CTA kernel, 16 for CTA pairs (a 32 KB
-// stage: the 24 KB saved buy a sixth stage, i.e. three hand-off groups of two k-blocks)
-__host__ __device__ constexpr int qw_of(int cg) { return cg == 2 ? 16 : 32; }
-constexpr int Q_LD = BM + 1;                 // words between consecutive word-rows of a ring tile
+// Query ring: every expander warp keeps a private 3-slot ring of [32 rows][8 words (+1 pad)] tiles holding just the
+// packed words ITS threads expand (its 32 rows, its half of each k-block), filled by its own cp.async copies, so the
+// ring needs no barrier between warps: a cp.async.wait_group and a __syncwarp per chunk.  (The round-1 ring was one
+// [words][128 rows] tile shared by the eight warps behind a 256-thread named barrier per chunk: for int8 operands
+// -- 4 k-blocks per chunk -- the warps spent 44 % of their samples in that hand-shake, profiles/r2_simtc.md.)
+constexpr int CW = 8;                        // packed words per row and chunk in a warp's ring tile
+constexpr int RLD = CW + 1;                  // row stride (words): conflict-free reads, lane = row
+constexpr int WSLOT = 32 * RLD;              // words per slot and warp
 constexpr int Q_SLOTS = 3;
-__host__ __device__ constexpr int qring_bytes(int cg) { return Q_SLOTS * qw_of(cg) * Q_LD * 4; }
+constexpr int QRING_BYTES = 8 /*expander warps*/ * Q_SLOTS * WSLOT * 4;   // 27 648
+__host__ __device__ constexpr int qring_bytes(int) { return QRING_BYTES; }
 
 // dimension offset (within a k-block) of shared-memory K position kappa
 __host__ __device__ __forceinline__ int perm_bf16(int kappa) {  // k-block = 64 dims = 2 words
@@ -353,9 +358,8 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
     }
   } else {
     // ================================================================= expanders (warps 6..13)
-    // Query words reach the expanders through a 3-deep cp.async ring of [32 words][128 rows] tiles
-    // (transposed, row stride 129 words: conflict-free both ways): every copy instruction of a
-    // warp reads 128 contiguous bytes of one row whatever ldh is, and nothing is staged in registers.
+    // Query words reach each expander warp through its private 3-deep cp.async ring (see CW above): nothing is
+    // staged in registers, and a copy instruction covers 4 rows x 8 words whatever ldh is.
     const int et = (int)threadIdx.x - 192;    // 0..255
     const int t = et & (BM - 1);              // row of the tile
     const int part_id = et / BM;              // which half of a row's eight 16-byte chunks (warp-uniform)
@@ -363,41 +367,49 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
     constexpr int C_PER = 8 / (EXW / 4);
     static_assert(EXW == 8, "two expander threads per row");
     constexpr int WPK = INT8 ? 4 : 2;         // packed words per k-block
-    constexpr int QW = qw_of(CG);
-    constexpr int Q_SLOT_WORDS = QW * Q_LD;
-    constexpr int KPC = QW / WPK;             // k-blocks per ring tile
     constexpr int WPP = WPK / 2;              // words of a k-block this thread's half needs
+    constexpr int KPC = CW / WPP;             // k-blocks per ring chunk (8 / 4)
     const uint32_t sw = (uint32_t)(t & 7);
-    const uint32_t q_smem = bar0 + 256u;      // ring base (after the barriers)
+    const uint32_t q_smem = bar0 + 256u + (uint32_t)ew * (Q_SLOTS * WSLOT * 4);   // this warp's ring (after the barriers)
     const uint32_t* q_ptr = reinterpret_cast<const uint32_t*>(smem_raw + (q_smem - smem_u32(smem_raw)));
-    int64_t is_i = 0;   // producer cursor: tile, chunk of the tile's k-block range, ring slot
+    int64_t is_i = 0;   // copy cursor: tile, chunk of the tile's k-block range, ring slot
     int is_c = 0, is_slot = 0;
+    // geometry of the tile the cursor is in (item_of divides: once per tile, not once per chunk)
+    int is_kb_lo = 0, is_nch = 0, is_rows = 0;
+    const uint32_t* is_row0 = p.Hbits;
+    auto issue_tile = [&]() {
+      if (is_i >= tiles_per_cta) return;
+      int mt, sp, kb_hi;
+      item_of(is_i, mt, sp, is_kb_lo, kb_hi);
+      is_nch = (kb_hi - is_kb_lo + KPC - 1) / KPC;
+      const int64_t m0 = (int64_t)(mt * CG + rank) * BM + (t & ~31);   // first row of this warp
+      const int64_t rows_left = p.N - m0;
+      is_rows = rows_left < 32 ? (rows_left < 0 ? 0 : (int)rows_left) : 32;
+      is_row0 = p.Hbits + (is_rows > 0 ? m0 : 0) * p.ldh;
+    };
+    issue_tile();
     auto issue = [&]() {
       if (is_i >= tiles_per_cta) return;
-      int mt, sp, kb_lo, kb_hi;
-      item_of(is_i, mt, sp, kb_lo, kb_hi);
-      const int nch = (kb_hi - kb_lo + KPC - 1) / KPC;
-      const int64_t m0 = (int64_t)(mt * CG + rank) * BM;
-      constexpr int RPW = 32 / QW;                       // rows one warp instruction copies (QW words each)
-      const int wl = lane & (QW - 1), r0 = ew + EXW * (lane / QW);
-      const int w = (kb_lo / KPC + is_c) * QW + wl;      // kbs is a multiple of KPC
-      const int64_t rows_left = p.N - m0;
-      const int nrow = w < p.W ? (rows_left < BM ? (int)rows_left : BM) : 0;
-      const uint32_t* src = p.Hbits + (m0 + r0) * p.ldh + w;
-      uint32_t dst = q_smem + (uint32_t)(is_slot * Q_SLOT_WORDS + wl * Q_LD + r0) * 4u;
-#pragma unroll 4
-      for (int rr = r0; rr < BM; rr += EXW * RPW) {
+      const int lw = lane & (CW - 1), sub = lane >> 3;                  // word of the chunk, row within a group of 4
+      // word lw of the chunk = word (lw % WPP) of this half of k-block kb_lo + is_c * KPC + lw / WPP
+      const int w = (is_kb_lo + is_c * KPC + lw / WPP) * WPK + part_id * WPP + (lw % WPP);
+      const int nrow = w < p.W ? is_rows : 0;
+      const uint32_t* src = is_row0 + (int64_t)sub * p.ldh + w;
+      uint32_t dst = q_smem + (uint32_t)(is_slot * WSLOT + sub * RLD + lw) * 4u;
+#pragma unroll
+      for (int rr = sub; rr < 32; rr += 4) {
         const bool ok = rr < nrow;
         asm volatile("cp.async.ca.shared.global [%0], [%1], 4, %2;" ::"r"(dst), "l"(ok ? src : p.Hbits),
                      "r"(ok ? 4 : 0)
                      : "memory");
-        src += EXW * RPW * p.ldh;
-        dst += EXW * RPW * 4u;
+        src += 4 * p.ldh;
+        dst += 4 * RLD * 4u;
       }
       if (++is_slot == Q_SLOTS) is_slot = 0;
-      if (++is_c == nch) {
+      if (++is_c == is_nch) {
         is_c = 0;
         ++is_i;
+        issue_tile();
       }
     };
     for (int s0 = 0; s0 < Q_SLOTS - 1; ++s0) {
@@ -416,7 +428,7 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
       constexpr int C0 = PART * C_PER;
       uint32_t wq[WPP];
 #pragma unroll
-      for (int v = 0; v < WPP; ++v) wq[v] = qk[v * Q_LD];
+      for (int v = 0; v < WPP; ++v) wq[v] = qk[v];
 #pragma unroll
       for (int cc = 0; cc < C_PER; ++cc) {  // 16-byte chunk cidx of the row = 4 shared-memory words
         const int cidx = C0 + cc;
@@ -444,11 +456,11 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
       const int nch = (kb_hi - kb_lo + KPC - 1) / KPC;
       for (int c = 0; c < nch; ++c, ++step) {
         asm volatile("cp.async.wait_group %0;" ::"n"(Q_SLOTS - 2) : "memory");
-        asm volatile("bar.sync 1, %0;" ::"n"(32 * EXW) : "memory");  // tile visible; previous slot free
+        __syncwarp();   // this warp's tile is complete; its lanes are done with the slot about to be refilled
         issue();
         asm volatile("cp.async.commit_group;" ::: "memory");
         // this thread's words of the chunk's first k-block (groups never straddle a chunk: G | KPC)
-        const uint32_t* qk = q_ptr + slot * Q_SLOT_WORDS + t + part_id * (WPP * Q_LD);
+        const uint32_t* qk = q_ptr + slot * WSLOT + lane * RLD;
         int left = (kb_hi - kb_lo) - c * KPC;
         if (left > KPC) left = KPC;
         while (left > 0) {
@@ -459,7 +471,7 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
           for (int u = 0; u < n; ++u) {
             if (part_id == 0) expand(std::integral_constant<int, 0>{}, qk, a_row);
             else expand(std::integral_constant<int, 1>{}, qk, a_row);
-            qk += WPK * Q_LD;
+            qk += WPP;
             a_row += STAGE_BYTES;
           }
           // the group is published with one proxy fence and one arrival per warp
