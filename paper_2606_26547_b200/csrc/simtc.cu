@@ -87,7 +87,7 @@ struct SimParams {
   int num_kb;
   int splits;       // CTAs that share one m-tile, each reducing kbs k-blocks (split-D for small N)
   int kbs;          // k-blocks per split (multiple of 16)
-  double* partial;  // [splits][N][K] partial sums when splits > 1
+  float* partial;   // [splits][K][N] partial sums when splits > 1 (fp32: exact for the integer paths, see sim_tc_splits)
   int kps;          // k-blocks per pipeline group
   int stages;       // ring depth
   int stage_bytes;  // A_BYTES + nparts*kc*KB_BYTES
@@ -289,14 +289,7 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
             if (p.splits > 1) {
               // partial sum of this split of the reduction axis; split_reduce_kernel adds the splits
               // in a fixed order and applies the epilogue
-              if (row_ok) {
-                double ad;
-                if (INT8) ad = (double)(int)v0[j];
-                else if (p.nparts == 3)
-                  ad = ((double)__uint_as_float(v2[j]) + (double)__uint_as_float(v1[j])) + (double)__uint_as_float(v0[j]);
-                else ad = (double)__uint_as_float(v0[j]);
-                p.partial[((int64_t)sp * p.N + row) * p.K + k] = ad;
-              }
+              if (row_ok) p.partial[((int64_t)sp * p.K + k) * p.N + row] = a;   // [split][class][query]: coalesced
             } else if (EPI == EPI_SCORE) {
               if (row_ok) {
                 if (p.e.s_i32) {
@@ -559,36 +552,54 @@ __global__ void class_operand_kernel(const float* __restrict__ C, int K, int D_e
 }
 
 // Adds the split partial sums in split order (fixed: deterministic) and applies the epilogue of
-// sim_tc_kernel: scores (S) or arg-max with best / runner-up.  One thread per query row.
-__global__ void split_reduce_kernel(const double* __restrict__ partial, int splits, int64_t N, int K, Epilogue e) {
+// sim_tc_kernel: scores (S) or arg-max with best / runner-up, with the same fp32 comparison + exact double
+// tie-break.  One thread per query row; [split][class][query] layout: coalesced.  int_acc: the partial sums are
+// integers (exact in fp32 below 2^24, which sim_tc_splits guarantees).
+__global__ void split_reduce_kernel(const float* __restrict__ partial, int splits, int64_t N, int K, Epilogue e) {
   const int64_t n = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (n >= N) return;
-  Top2 run = Top2{NEG_BIG, INT_MAX, NEG_BIG};
-  for (int k = 0; k < K; ++k) {
-    double a = 0.0;
-    for (int sp = 0; sp < splits; ++sp) a += partial[((int64_t)sp * N + n) * K + k];
+  const bool scaled = e.colscale != nullptr;
+  Top2f run = Top2f{NEG_BIG_F, NEG_BIG_F, 0.0f, 0.0f, INT_MAX, INT_MAX};
+  constexpr int KU = 8;   // classes whose partial sums are fetched together (independent loads in flight)
+  for (int k0 = 0; k0 < K; k0 += KU) {
+    float av[KU];
+#pragma unroll
+    for (int j = 0; j < KU; ++j) av[j] = 0.0f;
+    for (int sp = 0; sp < splits; ++sp) {
+#pragma unroll
+      for (int j = 0; j < KU; ++j)
+        if (k0 + j < K) av[j] = __fadd_rn(av[j], __ldg(partial + ((int64_t)sp * K + k0 + j) * N + n));
+    }
+#pragma unroll
+    for (int j = 0; j < KU; ++j) {
+    const int k = k0 + j;
+    if (k >= K) break;
+    const float a = av[j];
     if (e.kind == EPI_SCORE) {
       if (e.s_i32) {
         int iv = (int)a;
         if (e.ham_D > 0) iv = (e.ham_D - iv) >> 1;
         reinterpret_cast<int32_t*>(e.S)[n * e.lds + k] = iv;
       } else {
-        reinterpret_cast<float*>(e.S)[n * e.lds + k] = e.colscale ? (float)(a * e.colscale[k]) : (float)a;
+        reinterpret_cast<float*>(e.S)[n * e.lds + k] = scaled ? __fmul_rn(a, e.colscale_f[k]) : a;
       }
     } else {
-      const double sc = e.colscale ? a * e.colscale[k] : a;
-      if (sc > run.b1) {
-        run.b2 = run.b1;
-        run.b1 = sc;
-        run.i1 = k;
+      const float sc = scaled ? __fmul_rn(a, e.colscale_f[k]) : a;
+      bool better = sc > run.b1;
+      if (scaled && fabsf(sc - run.b1) <= 2.0e-6f * fmaxf(fabsf(sc), fabsf(run.b1)) && run.i1 != INT_MAX)
+        better = (double)a * e.colscale[k] > (double)run.a1 * e.colscale[run.i1];
+      if (better) {
+        run.b2 = run.b1; run.a2 = run.a1; run.i2 = run.i1;
+        run.b1 = sc; run.a1 = a; run.i1 = k;
       } else if (sc > run.b2) {
-        run.b2 = sc;
+        run.b2 = sc; run.a2 = a; run.i2 = k;
       }
+    }
     }
   }
   if (e.kind == EPI_ARGMAX) {
-    double b1 = run.b1, b2 = run.b2;
-    if (b2 == NEG_BIG) b2 = b1;  // K == 1
+    double b1 = scaled ? (double)run.a1 * e.colscale[run.i1] : (double)run.a1;
+    double b2 = run.i2 == INT_MAX ? b1 : (scaled ? (double)run.a2 * e.colscale[run.i2] : (double)run.a2);  // K == 1
     if (e.ham_D > 0) {
       b1 = 0.5 * ((double)e.ham_D - b1);
       b2 = 0.5 * ((double)e.ham_D - b2);
@@ -647,14 +658,16 @@ size_t sim_tc_operand_bytes(int K, int hv_bits, int D_eff) {
 
 // Split-D for small N: with fewer m-tiles than half the SMs, `splits` CTAs share an m-tile, each
 // reducing kbs k-blocks (a multiple of 16, so that splits start on ring-chunk boundaries); their
-// partial sums go through a [splits][N][K] double buffer.  Returns 1 when not worth it.
+// partial sums go through a [splits][K][N] fp32 buffer (integer class operands: only while every score stays
+// below 2^24, i.e. exact in fp32).  Returns 1 when not worth it.
 int sim_tc_splits(int64_t N, int K, int hv_bits, int D_eff, int sm_count, int* kbs_out) {
   int kc, nparts, n_tiles, num_kb;
   bool int8;
   sim_tc_shape(K, hv_bits, D_eff, kc, nparts, n_tiles, num_kb, int8);
   const int64_t m_tiles = (N + BM - 1) / BM;
   int splits = 1, kbs = num_kb;
-  if (n_tiles == 1 && m_tiles * 2 <= sm_count && num_kb >= 32) {
+  const bool exact_ok = !int8 || (int64_t)D_eff * (hv_bits == 8 ? 127 : 1) < (1 << 24);
+  if (n_tiles == 1 && m_tiles * 2 <= sm_count && num_kb >= 32 && exact_ok) {
     int want = (int)(sm_count / m_tiles);
     if (want > 8) want = 8;
     if (want > num_kb / 16) want = num_kb / 16;
@@ -737,7 +750,7 @@ cudaError_t launch_sim_tc(TcContext* tc, const uint32_t* Hbits, int64_t N, int64
   p.e = e;
   p.splits = (partial && cg == 1) ? sim_tc_splits(N, K, hv_bits, D_eff, sm_count, &p.kbs) : 1;
   if (p.splits == 1) p.kbs = num_kb;
-  p.partial = partial;
+  p.partial = reinterpret_cast<float*>(partial);
   const int64_t items = (int64_t)p.m_tiles * p.splits;
   const int max_units = sm_count / cg;
   const int grid = (int)(items < max_units ? items : max_units) * cg;
@@ -745,7 +758,7 @@ cudaError_t launch_sim_tc(TcContext* tc, const uint32_t* Hbits, int64_t N, int64
   if (p.splits > 1) {
     ce = int8 ? launch_one<true, EPI_SCORE>(tmB, p, 1, grid, st) : launch_one<false, EPI_SCORE>(tmB, p, 1, grid, st);
     if (ce != cudaSuccess) return ce;
-    split_reduce_kernel<<<(unsigned)((N + 127) / 128), 128, 0, st>>>(partial, p.splits, N, K, e);
+    split_reduce_kernel<<<(unsigned)((N + 127) / 128), 128, 0, st>>>(p.partial, p.splits, N, K, e);
     ++*nlaunch;
     return cudaGetLastError();
   }
