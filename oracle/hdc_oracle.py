@@ -33,6 +33,7 @@ F32, BF16, I8, B1 = 0, 1, 2, 3
 F16 = 6         # encode operands as IEEE half ("floating-point types (FP16 or FP32)")
 SIM_DOT, SIM_COS, SIM_HAMMING = 0, 1, 2
 HV_F16 = 17      # hv_bits code (not a width): class operand as 16-bit IEEE half ("FP16")
+HV_I16 = 18      # hv_bits code (not a width): class operand as 16-bit integers ("integer data types (8, 16, ...")
 
 
 # ------------------------------------------------------------------------------------- S0
@@ -86,6 +87,18 @@ def quantize_int8_tensor(c: np.ndarray) -> np.ndarray:
     s = np.float32(127.0) / a if a > 0 else np.float32(1.0)
     q = np.rint((c * np.float32(s)).astype(np.float32))
     return np.clip(q, -127, 127).astype(np.int32)
+
+
+def quantize_int16_tensor(c: np.ndarray) -> np.ndarray:
+    """Per-tensor symmetric int16 over the given array (hypervectors "represented using
+    integer data types (8, 16, 32, or 64-bit)", inference "projecting class ... hypervectors onto
+    lower-precision integer types"; reading A7 carried to 16 bits, A21): s = fl32(32767/max|c|) (1 if the
+    array is all zero), q = clamp(rint(fl32(c*s)), -32767, 32767), rint = round half to even."""
+    c = np.ascontiguousarray(c, dtype=np.float32)
+    a = np.float32(np.max(np.abs(c))) if c.size else np.float32(0)
+    s = np.float32(32767.0) / a if a > 0 else np.float32(1.0)
+    q = np.rint((c * np.float32(s)).astype(np.float32))
+    return np.clip(q, -32767, 32767).astype(np.int32)
 
 
 def rp_operands(X: np.ndarray, P: np.ndarray, precision: int):
@@ -163,8 +176,8 @@ def class_operand(C_acc: np.ndarray, D_eff: int, hv_bits: int) -> np.ndarray:
     """Class operand derived from the fp32 accumulators at the hypervector element width
     (training in high precision, inference "projecting class ... hypervectors
     onto lower-precision integer types"; S5): 32 -> C_acc; 16 -> bf16 RNE; 8 -> per-tensor
-    symmetric int8 over k<K, d<D_eff; 1 -> bit [C_acc < 0]; HV_F16 -> IEEE half RNE.  Returned as float64 values
-    (bits as uint8)."""
+    symmetric int8 over k<K, d<D_eff; 1 -> bit [C_acc < 0]; HV_F16 -> IEEE half RNE; HV_I16 -> per-tensor
+    symmetric int16 over k<K, d<D_eff.  Returned as float64 values (bits as uint8)."""
     c = np.asarray(C_acc, dtype=np.float32)[:, :D_eff]
     if hv_bits == 32:
         return c.astype(np.float64)
@@ -176,6 +189,8 @@ def class_operand(C_acc: np.ndarray, D_eff: int, hv_bits: int) -> np.ndarray:
         return c.astype(np.float16).astype(np.float64)
     if hv_bits == 8:
         return quantize_int8_tensor(c).astype(np.float64)
+    if hv_bits == HV_I16:
+        return quantize_int16_tensor(c).astype(np.float64)
     if hv_bits == 1:
         return (c < 0).astype(np.uint8)
     raise ValueError("hv_bits")

@@ -961,3 +961,53 @@ def test_fp16_encode_operands_by_hand():
     Xi = r.integers(0, 256, size=(4, 9)).astype(np.float32)
     Pi = (1.0 - 2.0 * r.integers(0, 2, size=(6, 9))).astype(np.float32)
     assert np.array_equal(o.encode_rp(Xi, Pi, 6, o.F16)[1], o.encode_rp(Xi, Pi, 6, o.F32)[1])
+
+
+# ------------------------------------------------------------------ S5 per-tensor int16 (A21), by hand
+def test_int16_tensor_rounding_mode_and_scale_by_hand():
+    """quantize_int16_tensor ("integer data types (8, 16, 32, or 64-bit)"; reading A21 = A7 at
+    16 bits): ONE scale s = fl32(32767 / max|c|) for the array, q = rint-to-nearest-EVEN of fl32(c*s), codes in
+    [-32767, 32767].  Worked by hand so that truncation, half-up, half-away, a per-row scale and a 32768 full
+    scale each fail."""
+    # max|c| = 16383.5 -> s = 2 (exact): products are exact
+    #   16383.5*2 = 32767; 0.25*2 = 0.5 -> 0 (tie to even; half-up gives 1); 0.75*2 = 1.5 -> 2 (trunc gives 1)
+    #   1.25*2 = 2.5 -> 2 (tie to even; half-up / half-away give 3; a 32768 full scale gives 2.50004 -> 3)
+    #   -1.25*2 = -2.5 -> -2; 100.3*2 = 200.6 -> 201; -16383.5 -> -32767 (never -32768)
+    c = np.array([[16383.5, 0.25, 0.75, 1.25], [-1.25, 100.3, -16383.5, 0.0]], dtype=np.float32)
+    assert o.quantize_int16_tensor(c).tolist() == [[32767, 0, 2, 2], [-2, 201, -32767, 0]]
+    # max|c| = 2 -> s = 16383.5 (exact in fp32)
+    #   1.0*s = 16383.5 -> 16384 (tie, even); 0.5*s = 8191.75 -> 8192; -0.75*s = -12287.625 -> -12288
+    #   second row uses the SAME scale (per tensor): 0.25*s = 4095.875 -> 4096; a per-row scale would give 32767
+    c = np.array([[2.0, 1.0, 0.5, -0.75], [0.25, 0.0, 0.0, 0.0]], dtype=np.float32)
+    assert o.quantize_int16_tensor(c).tolist() == [[32767, 16384, 8192, -12288], [4096, 0, 0, 0]]
+    # the class operand takes the scale over d < D_eff only (S5)
+    C = np.array([[2.0, 1.0, 1000.0], [0.5, 0.25, -1000.0]], dtype=np.float32)
+    assert o.class_operand(C, 2, o.HV_I16).tolist() == [[32767.0, 16384.0], [8192.0, 4096.0]]
+    assert o.quantize_int16_tensor(np.zeros((2, 3), dtype=np.float32)).tolist() == [[0, 0, 0], [0, 0, 0]]
+
+
+def test_int16_similarity_brute_force_and_small_integer_identity():
+    """hv code HV_I16 through similarity(): DOT = python-integer sum of v*q over d < D_eff, COS = DOT /
+    (sqrt(D_eff) * |q|) with the norm of the CODES; integer accumulators whose max is 32767/2^j are held
+    exactly up to the power-of-two scale (labels and cosines of hv_bits = 32 are reproduced)."""
+    r = rng(210)
+    N, K, D, D_eff = 6, 4, 90, 77
+    hb = r.integers(0, 2, size=(N, D), dtype=np.uint8)
+    C = (r.standard_normal((K, D)) * 50).astype(np.float32)
+    amax = max(abs(float(C[k, d])) for k in range(K) for d in range(D_eff))
+    s = np.float32(32767.0) / np.float32(amax)
+    q = [[int(round(float(np.float32(C[k, d]) * s))) for d in range(D_eff)] for k in range(K)]   # python round: half-even
+    dot = o.similarity(hb, C, D_eff, o.SIM_DOT, o.HV_I16)
+    cos = o.similarity(hb, C, D_eff, o.SIM_COS, o.HV_I16)
+    for n in range(N):
+        for k in range(K):
+            acc = sum((1 - 2 * int(hb[n, d])) * q[k][d] for d in range(D_eff))
+            assert dot[n, k] == acc
+            nrm = sum(v * v for v in q[k]) ** 0.5
+            assert abs(cos[n, k] - acc / (D_eff ** 0.5 * nrm)) < 1e-12
+    # integer accumulators with max|c| = 32767: scale exactly 1 -> the int16 operand IS the accumulator
+    Ci = r.integers(-32767, 32768, size=(K, D)).astype(np.float32)
+    Ci[0, 0] = 32767.0
+    assert np.array_equal(o.similarity(hb, Ci, D, o.SIM_DOT, o.HV_I16), o.similarity(hb, Ci, D, o.SIM_DOT, 32))
+    assert np.allclose(o.similarity(hb, Ci, D, o.SIM_COS, o.HV_I16), o.similarity(hb, Ci, D, o.SIM_COS, 32),
+                       rtol=1e-14, atol=0)
