@@ -251,8 +251,8 @@ def row_classify(h, peaks, reps, N, K, D, hv_bits, sim_name):
         out["roofline"] = {"bound": "alu", "achieved": popc, "peak": peak, "unit": "Tpopc/s", "frac": popc / peak,
                            "peak_source": "148 SM x 16 POPC lanes x sm_max_mhz"}
     else:
-        parts = 3 if hv_bits == 32 else 1
-        mult = 2.0 if hv_bits in (8, 1) else 1.0
+        parts = 3 if hv_bits in (32, hd.HDC_HV_I16) else 1
+        mult = 2.0 if hv_bits in (hd.HDC_HV_I16, 8, 1) else 1.0
         kp = ((K + 15) // 16) * 16
         flops = 2.0 * N * D * kp * parts
         ach = flops / (k_ms * 1e-3) / 1e12
@@ -416,7 +416,9 @@ def row_c5_classify(h, peaks, reps, hv_bits, sim_name, B=65536, F=1024, D=16384,
     fn = lambda: h.hdc_classify(H, C, kn, labels=lab)  # noqa: E731
     call_ms = _time(fn, reps)
     k_ms, _ = _kernel(h, hd.HDC_K_SIM, fn, reps)
-    mult = 2.0 if hv_bits in (8, 1) else 1.0
+    # int16 class codes (hv code 18): algorithmic flops 2*B*D*K against the int8 tensor peak; the kernel executes
+    # three int8 digit columns per class, so a third of that peak is its ceiling
+    mult = 2.0 if hv_bits in (hd.HDC_HV_I16, 8, 1) else 1.0
     flops = 2.0 * B * D * (((K + 15) // 16) * 16)
     ach = flops / (k_ms * 1e-3) / 1e12
     peak = peaks["bf16_tflops"] * mult
@@ -588,6 +590,9 @@ ROWS = {
     "c5_encode_bf16": lambda h, p, r: row_encode(h, p, r, "c5", 65536, "bf16"),
     "c5_classify_bf16": lambda h, p, r: row_c5_classify(h, p, r, 16, "cos"),
     "c5_classify_1bit": lambda h, p, r: row_c5_classify(h, p, r, 1, "hamming"),
+    "c5_classify_i8": lambda h, p, r: row_c5_classify(h, p, r, 8, "cos"),
+    "c5_classify_i16": lambda h, p, r: row_c5_classify(h, p, r, hd.HDC_HV_I16, "cos"),
+    "c2_classify_cos_i16": lambda h, p, r: row_classify(h, p, r, 131072, 26, 10000, hd.HDC_HV_I16, "cos"),
     "c5_stream_bf16": lambda h, p, r: row_c5_stream(h, p, r, 16, "cos"),
     "c5_stream_1bit": lambda h, p, r: row_c5_stream(h, p, r, 1, "hamming"),
     "specpcm_adc_d1024": lambda h, p, r: row_adc(h, p, r, 131072, 26, 1024),

@@ -62,8 +62,9 @@ typedef enum {
 enum { HDC_F32 = 0, HDC_BF16 = 1, HDC_I8 = 2, HDC_B1 = 3, HDC_U8 = 4, HDC_I32 = 5, HDC_F16 = 6 };
 /* similarity kinds (L167 algorithmic choice) */
 enum { HDC_SIM_DOT = 0, HDC_SIM_COS = 1, HDC_SIM_HAMMING = 2 };
-/* knobs.hv_bits code (not a width) for a 16-bit IEEE half class operand (L165 "FP16") */
-enum { HDC_HV_F16 = 17 };
+/* knobs.hv_bits codes (not widths): 16-bit IEEE half class operand (L165 "FP16"); 16-bit integer class
+ * operand (L165 "integer data types (8, 16, 32, or 64-bit)") */
+enum { HDC_HV_F16 = 17, HDC_HV_I16 = 18 };
 /* hdc_train_epoch modes */
 enum { HDC_TRAIN_BUNDLE = 0, HDC_TRAIN_PERCEPTRON = 1, HDC_TRAIN_KMEANS = 2 };
 /* hdc_encode_rp outputs (bit-or) */
@@ -103,6 +104,8 @@ enum {
  *  hv_bits    element width of the CLASS hypervectors in similarity / classify / train (L165):
  *             32 fp32 | 16 bf16 (RNE of C_acc) | HDC_HV_F16 IEEE half (RNE of C_acc; |c| > 65504
  *             overflows, outside the contract) | 8 int8 (per-tensor symmetric over k<K, d<D_eff)
+ *             | HDC_HV_I16 int16 (per-tensor symmetric over k<K, d<D_eff: s = 32767/max|c|,
+ *             q = clamp(rint(c*s), +-32767); int32 accumulate, exact: D_eff*32767 < 2^31)
  *             | 1 sign bit [C_acc < 0].  Query hypervectors are always bipolar (packed bits).
  *  sim        HDC_SIM_*; HDC_SIM_HAMMING requires hv_bits == 1.
  *  flags      HDC_FLAG_*.
@@ -216,10 +219,10 @@ int32_t hdc_encode_levelid_u16(hdc_handle_t h, const uint16_t* levels, int64_t N
  * Hbits [N][ldh_words] packed queries; C_acc [K][ldc] fp32 class accumulators, from which the
  * class operand is derived at knobs->hv_bits.  Over d < D_eff:
  *   HAMMING  dist[n,k] = popcount(h[n] xor cbit[k])                       -> S int32 [N][lds]
- *   DOT      s[n,k]   = sum_d v[n,d]*c[k,d]                               -> S fp32 (int32 if hv_bits 8 or 1)
+ *   DOT      s[n,k]   = sum_d v[n,d]*c[k,d]                               -> S fp32 (int32 if hv_bits 8, HDC_HV_I16 or 1)
  *   COS      s[n,k]   = DOT / (sqrt(D_eff) * sqrt(sum_d c[k,d]^2)), 0 if the norm is 0   -> S fp32
  * s_dtype must be HDC_I32 for HAMMING, HDC_F32 for COS, HDC_F32 or HDC_I32 for DOT (HDC_I32 only
- * for hv_bits 8 or 1). */
+ * for hv_bits 8, HDC_HV_I16 or 1; fp32 scores of an int16 operand are the exact int32 sum rounded once). */
 int32_t hdc_similarity(hdc_handle_t h, const uint32_t* Hbits, int64_t N, int64_t ldh_words,
                        const float* C_acc, int32_t K, int64_t ldc, int32_t D,
                        const hdc_knobs_t* knobs, void* S, int32_t s_dtype, int64_t lds, void* ws,

@@ -25,6 +25,7 @@ HDC_OP_CLASSIFY, HDC_OP_TRAIN_EPOCH, HDC_OP_INFER_RP_HOST, HDC_OP_INFER_RP = 3, 
 HDC_FLAG_NONE, HDC_FLAG_SIMT, HDC_FLAG_TC_1CTA, HDC_FLAG_TC_2CTA, HDC_FLAG_F32_FAST = 0, 1, 2, 4, 8
 HDC_FLAG_FUSED_INFER = 16
 HDC_HV_F16 = 17
+HDC_HV_I16 = 18
 HDC_K_ENCODE_GEMM, HDC_K_SIM, HDC_K_LEVELID, HDC_K_CLASS_UPDATE = 0, 1, 2, 3
 HDC_STAT_TC_LAUNCHES, HDC_STAT_SIMT_FALLBACKS, HDC_STAT_INFER_FUSED, HDC_STAT_INFER_UNFUSED = 0, 1, 2, 3
 

@@ -109,8 +109,9 @@ int check_knobs(hdc_ctx* h, const hdc_knobs_t* k, int D) {
   return HDC_OK;
 }
 int check_sim_knobs(hdc_ctx* h, const hdc_knobs_t* k) {
-  if (k->hv_bits != 32 && k->hv_bits != 16 && k->hv_bits != HDC_HV_F16 && k->hv_bits != 8 && k->hv_bits != 1)
-    return fail(h, HDC_ERR_INVALID_ARG, "hv_bits must be 32, 16, HDC_HV_F16, 8 or 1");
+  if (k->hv_bits != 32 && k->hv_bits != 16 && k->hv_bits != HDC_HV_F16 && k->hv_bits != HDC_HV_I16 &&
+      k->hv_bits != 8 && k->hv_bits != 1)
+    return fail(h, HDC_ERR_INVALID_ARG, "hv_bits must be 32, 16, HDC_HV_F16, HDC_HV_I16, 8 or 1");
   if (k->sim != HDC_SIM_DOT && k->sim != HDC_SIM_COS && k->sim != HDC_SIM_HAMMING)
     return fail(h, HDC_ERR_INVALID_ARG, "bad sim");
   if (k->sim == HDC_SIM_HAMMING && k->hv_bits != 1)
@@ -448,6 +449,7 @@ int do_similarity(hdc_ctx* h, const uint32_t* Hbits, int64_t N, int64_t ldh, con
     int8_t* Cq = nullptr;
     const int64_t ldq = round_up(D_eff, 16);
     if (colscale && k->hv_bits == 8) Cq = pm.take<int8_t>((size_t)K * ldq);
+    if (colscale && k->hv_bits == HDC_HV_I16) Cq = pm.take<int8_t>((size_t)K * ldq * 2);   // int16 codes
     const size_t pbytes = sim_tc_partial_bytes(N, K, k->hv_bits, D_eff, h->sm_count);
     double* partial = pbytes ? b.take<double>(pbytes / sizeof(double)) : nullptr;
     if (!persistent_fits(h, b, ws_bytes)) return too_small();
@@ -457,6 +459,11 @@ int do_similarity(hdc_ctx* h, const uint32_t* Hbits, int64_t N, int64_t ldh, con
         ce = launch_quantize_tensor_i8(C_acc, K, D_eff, ldc, pf, Cq, ldq, amax, st, &h->launches);
         if (ce != cudaSuccess) return cuda_fail(h, ce, "quantize C");
         ce = launch_col_scale(Operand{Cq, ldq, OPK_I8}, K, D_eff, 1, pf, colscale, st, &h->launches, colscale_f);
+      } else if (k->hv_bits == HDC_HV_I16) {
+        int16_t* Cq16 = reinterpret_cast<int16_t*>(Cq);
+        ce = launch_quantize_tensor_i16(C_acc, K, D_eff, ldc, pf, Cq16, ldq, amax, st, &h->launches);
+        if (ce != cudaSuccess) return cuda_fail(h, ce, "quantize C");
+        ce = launch_col_scale(Operand{Cq16, ldq, OPK_I16}, K, D_eff, 1, pf, colscale, st, &h->launches, colscale_f);
       } else {
         const int ck = k->hv_bits == 32   ? OPK_F32
                        : k->hv_bits == 16 ? OPK_F32_RBF16
@@ -533,6 +540,17 @@ int do_similarity(hdc_ctx* h, const uint32_t* Hbits, int64_t N, int64_t ldh, con
     }
     B = Operand{Cq, ldq, OPK_I8};
     int_acc = true;
+  } else if (k->hv_bits == HDC_HV_I16) {
+    const int64_t ldq = round_up(D_eff, 16);
+    int16_t* Cq = reinterpret_cast<int16_t*>(pm.take<int8_t>((size_t)K * ldq * 2));
+    float* amax = pm.take<float>(1);
+    if (!persistent_fits(h, b, ws_bytes)) return too_small();
+    if (prep) {
+      ce = launch_quantize_tensor_i16(C_acc, K, D_eff, ldc, pf, Cq, ldq, amax, st, &h->launches);
+      if (ce != cudaSuccess) return cuda_fail(h, ce, "quantize C");
+    }
+    B = Operand{Cq, ldq, OPK_I16};
+    int_acc = true;
   } else {
     uint32_t* cbits = pm.take<uint32_t>((size_t)K * W);
     if (!persistent_fits(h, b, ws_bytes)) return too_small();
@@ -572,11 +590,11 @@ void similarity_model_ws(int K, const hdc_knobs_t* k, Bump& pm) {
   pm.take<double>((size_t)K);
   pm.take<float>((size_t)K);
   pm.take<float>(1);
-  pm.take<int8_t>((size_t)K * round_up(k->D_eff, 16));
+  pm.take<int8_t>((size_t)K * round_up(k->D_eff, 16) * 2);   // int8 or int16 codes
   pm.take<uint32_t>((size_t)K * W);
   pm.take<uint32_t>((size_t)W);  // perforation mask
   pm.take<uint8_t>(sim_tc_operand_bytes(K, k->hv_bits == 32 || k->hv_bits == 16 || k->hv_bits == HDC_HV_F16 ||
-                                               k->hv_bits == 8 ? k->hv_bits : 1,
+                                               k->hv_bits == HDC_HV_I16 || k->hv_bits == 8 ? k->hv_bits : 1,
                                         k->D_eff));
 }
 
@@ -590,13 +608,13 @@ size_t similarity_ws(int64_t N, int K, const hdc_knobs_t* k) {
   const int W = words_of(k->D_eff);
   b.take<double>((size_t)K);
   b.take<float>((size_t)K);
-  b.take<int8_t>((size_t)K * round_up(k->D_eff, 16));
+  b.take<int8_t>((size_t)K * round_up(k->D_eff, 16) * 2);   // int8 or int16 codes
   b.take<float>(1);
   b.take<uint32_t>((size_t)K * W);
   b.take<uint32_t>((size_t)W);  // perforation mask
   b.take<uint32_t>((size_t)((k->D_eff + 127) / 128) * 4 * K);  // [chunk][class] sign bits of hdc_similarity_adc
   b.take<uint8_t>(sim_tc_operand_bytes(K, k->hv_bits == 32 || k->hv_bits == 16 || k->hv_bits == HDC_HV_F16 ||
-                                               k->hv_bits == 8 ? k->hv_bits : 1,
+                                               k->hv_bits == HDC_HV_I16 || k->hv_bits == 8 ? k->hv_bits : 1,
                                        k->D_eff));
   return b.off + 1024;
 }
@@ -615,7 +633,8 @@ constexpr int INFER_MAX_K = 32;
 constexpr int64_t INFER_MIN_N = 12288;  // 48 row blocks of 256: below it the two-kernel path spreads m x n tiles better
 
 bool infer_fused_knobs(const hdc_ctx* h, const hdc_knobs_t* k, int K) {   // the part that does not depend on N
-  return (k->flags & HDC_FLAG_FUSED_INFER) && use_tc(h, k) && !(k->flags & HDC_FLAG_TC_1CTA) && h->sm_count >= 2 &&
+  // (int16 class codes: sums beyond 2^24, which the fp32 search of the fused epilogue does not hold exactly)
+  return (k->flags & HDC_FLAG_FUSED_INFER) && k->hv_bits != HDC_HV_I16 && use_tc(h, k) && !(k->flags & HDC_FLAG_TC_1CTA) && h->sm_count >= 2 &&
          K <= INFER_MAX_K && k->D_eff <= (1 << 17);
 }
 int infer_kc(int K) { return K <= 8 ? 8 : (K <= 16 ? 16 : 32); }
@@ -991,8 +1010,8 @@ extern "C" int32_t hdc_similarity(hdc_handle_t h, const uint32_t* Hbits, int64_t
   if (knobs->sim == HDC_SIM_COS && s_dtype != HDC_F32) return fail(h, HDC_ERR_INVALID_ARG, "similarity: COS writes fp32");
   if (knobs->sim == HDC_SIM_DOT) {
     if (s_dtype != HDC_F32 && s_dtype != HDC_I32) return fail(h, HDC_ERR_INVALID_ARG, "similarity: s_dtype");
-    if (s_dtype == HDC_I32 && knobs->hv_bits != 8 && knobs->hv_bits != 1)
-      return fail(h, HDC_ERR_INVALID_ARG, "similarity: int32 DOT needs hv_bits 8 or 1");
+    if (s_dtype == HDC_I32 && knobs->hv_bits != 8 && knobs->hv_bits != 1 && knobs->hv_bits != HDC_HV_I16)
+      return fail(h, HDC_ERR_INVALID_ARG, "similarity: int32 DOT needs hv_bits 8, HDC_HV_I16 or 1");
   }
   if (N == 0) return HDC_OK;
   Bump b(ws);

@@ -19,7 +19,8 @@ enum OperandKind : int {
   OPK_I8 = 4,         // int8
   OPK_F32_RF16 = 5,   // float rounded to nearest-even IEEE half on load (hv code HDC_HV_F16, precision HDC_F16)
   OPK_BF16_RF16 = 6,  // __nv_bfloat16 widened, then rounded to IEEE half (precision HDC_F16 on bf16 inputs)
-  OPK_F16 = 7         // __half (staged operands of the tcgen05 path)
+  OPK_F16 = 7,        // __half (staged operands of the tcgen05 path)
+  OPK_I16 = 8         // int16 (class codes of hv code HDC_HV_I16)
 };
 
 struct Operand {
@@ -162,6 +163,10 @@ cudaError_t launch_quantize_rows_i8(const void* src, int src_kind, int64_t rows,
 cudaError_t launch_quantize_tensor_i8(const float* C, int K, int D_eff, int64_t ldc, Perf pf, int8_t* dst,
                                       int64_t ld_dst, float* amax_scratch, cudaStream_t st,
                                       int64_t* nlaunch);
+// per-tensor symmetric int16 of C_acc[k<K][d<D_eff] (S5 at HDC_HV_I16, A21): scale 32767 / amax
+cudaError_t launch_quantize_tensor_i16(const float* C, int K, int D_eff, int64_t ldc, Perf pf, int16_t* dst,
+                                       int64_t ld_dst, float* amax_scratch, cudaStream_t st,
+                                       int64_t* nlaunch);
 // class operand of the fused inference epilogue (EPI_INFER): dst [KC][ld_dst] fp32, row k < K = the class
 // operand at hv_bits (32: C_acc; 16 / HDC_HV_F16: RNE to bf16 / half; 8: per-tensor int8 code, scale 127 / *amax;
 // 1: +-1 from the sign), zero for d >= D_eff, unvisited d and rows >= K

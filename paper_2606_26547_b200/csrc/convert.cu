@@ -208,6 +208,22 @@ __global__ void quantize_tensor_i8_kernel(const float* __restrict__ C, int K, in
   }
 }
 
+__global__ void quantize_tensor_i16_kernel(const float* __restrict__ C, int K, int D_eff, int64_t ldc,
+                                           int16_t* __restrict__ dst, int64_t ld_dst,
+                                           const float* __restrict__ amax) {
+  const float a = *amax;
+  const float s = a > 0.0f ? __fdiv_rn(32767.0f, a) : 1.0f;
+  const int64_t total = (int64_t)K * ld_dst;
+  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < total;
+       i += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t k = i / ld_dst;
+    const int d = (int)(i - k * ld_dst);
+    float q = 0.0f;
+    if (d < D_eff) q = fminf(fmaxf(rintf(__fmul_rn(__ldg(C + k * ldc + d), s)), -32767.0f), 32767.0f);
+    dst[i] = (int16_t)(int)q;
+  }
+}
+
 // ---------------------------------------------------------------------------------- fp32 class operand
 // Class operand of the fused inference epilogue (gemm_tc.cu, EPI_INFER), S5: the value the
 // similarity contracts at hv_bits, as a float (int8 codes and +-1 are exact in fp32).
@@ -283,6 +299,7 @@ __global__ void col_scale_kernel(Operand C, int K, int D_eff, int cos, Perf pf, 
           break;
         case OPK_F32_RF16: v = (double)__half2float(__float2half_rn(__ldg((const float*)C.p + idx))); break;
         case OPK_BITS: v = 1.0; break;
+        case OPK_I16: v = (double)((const int16_t*)C.p)[idx]; break;
         default: v = (double)((const int8_t*)C.p)[idx]; break;
       }
       s += v * v;
@@ -502,6 +519,17 @@ cudaError_t launch_quantize_tensor_i8(const float* C, int K, int D_eff, int64_t 
   cudaError_t e = launch_tensor_amax(C, K, D_eff, ldc, pf, amax_scratch, st, nlaunch);
   if (e != cudaSuccess) return e;
   quantize_tensor_i8_kernel<<<grid_for((int64_t)K * ld_dst, 256, 148 * 8), 256, 0, st>>>(
+      C, K, D_eff, ldc, dst, ld_dst, amax_scratch);
+  ++*nlaunch;
+  return cudaGetLastError();
+}
+
+cudaError_t launch_quantize_tensor_i16(const float* C, int K, int D_eff, int64_t ldc, Perf pf, int16_t* dst,
+                                       int64_t ld_dst, float* amax_scratch, cudaStream_t st,
+                                       int64_t* nlaunch) {
+  cudaError_t e = launch_tensor_amax(C, K, D_eff, ldc, pf, amax_scratch, st, nlaunch);
+  if (e != cudaSuccess) return e;
+  quantize_tensor_i16_kernel<<<grid_for((int64_t)K * ld_dst, 256, 148 * 8), 256, 0, st>>>(
       C, K, D_eff, ldc, dst, ld_dst, amax_scratch);
   ++*nlaunch;
   return cudaGetLastError();

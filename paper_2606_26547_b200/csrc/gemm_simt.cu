@@ -48,6 +48,8 @@ __device__ __forceinline__ T load_elem(const Operand& o, int64_t row, int k) {
       uint32_t w = __ldg((const uint32_t*)o.p + row * o.ld + (k >> 5));
       return (T)(1 - 2 * (int)((w >> (k & 31)) & 1u));
     }
+    case OPK_I16:
+      return (T)((const int16_t*)o.p)[row * o.ld + k];
     default:  // OPK_I8
       return (T)((const int8_t*)o.p)[row * o.ld + k];
   }
@@ -296,7 +298,7 @@ cudaError_t launch_tn(const GemmParams& p, cudaStream_t st) {
     b.M = p.M - roff;
     if (b.M > nt * BM) b.M = nt * BM;
     auto adv = [&](Operand o) {
-      size_t es = (o.kind == OPK_BF16 || o.kind == OPK_BF16_RF16) ? 2 : (o.kind == OPK_I8 ? 1 : 4);
+      size_t es = (o.kind == OPK_BF16 || o.kind == OPK_BF16_RF16 || o.kind == OPK_I16) ? 2 : (o.kind == OPK_I8 ? 1 : 4);
       o.p = (const char*)o.p + (size_t)roff * o.ld * es;
       return o;
     };

@@ -82,7 +82,7 @@ struct SimParams {
   int W;        // words holding d < D_eff
   int K;        // classes
   int kc;       // classes per n-tile (multiple of 16)
-  int nparts;   // 1, or 3 for the fp32 class operand
+  int nparts;   // 1, or 3: the fp32 class operand as three bf16 parts / the int16 one as three base-128 digits
   int m_tiles, n_tiles;
   int num_kb;
   int splits;       // CTAs that share one m-tile, each reducing kbs k-blocks (split-D for small N)
@@ -267,7 +267,7 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
       for (int c0 = 0; c0 < k_valid; c0 += 16) {
         uint32_t v0[16], v1[16], v2[16];
         tmem_ld16(taddr + (uint32_t)c0, v0);
-        if (!INT8 && p.nparts == 3) {
+        if (p.nparts == 3) {
           tmem_ld16(taddr + (uint32_t)(p.kc + c0), v1);
           tmem_ld16(taddr + (uint32_t)(2 * p.kc + c0), v2);
         }
@@ -279,8 +279,11 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
             // the accumulator as a float: exact for the integer paths below 2^24, one rounding for the sum of
             // the three fp32-class parts
             float a;
+            int iv = 0;
             if (INT8) {
-              a = (float)(int)v0[j];
+              // int16 class codes: three balanced base-128 digits, most significant first (exact in int32)
+              iv = p.nparts == 3 ? (int)v0[j] * 16384 + (int)v1[j] * 128 + (int)v2[j] : (int)v0[j];
+              a = (float)iv;
             } else if (p.nparts == 3) {
               a = __fadd_rn(__fadd_rn(__uint_as_float(v2[j]), __uint_as_float(v1[j])), __uint_as_float(v0[j]));
             } else {
@@ -293,7 +296,6 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
             } else if (EPI == EPI_SCORE) {
               if (row_ok) {
                 if (p.e.s_i32) {
-                  int iv = (int)v0[j];
                   if (p.e.ham_D > 0) iv = (p.e.ham_D - iv) >> 1;
                   reinterpret_cast<int32_t*>(p.e.S)[row * p.e.lds + k] = iv;
                 } else {
@@ -304,17 +306,23 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
               // classes arrive in increasing order: strict > keeps the lowest index
               const float sc = scaled ? __fmul_rn(a, p.e.colscale_f[k]) : a;
               bool better = sc > run.b1;
+              bool second = sc > run.b2;
               if (scaled && fabsf(sc - run.b1) <= 2.0e-6f * fmaxf(fabsf(sc), fabsf(run.b1)) && run.i1 != INT_MAX) {
                 // too close for fp32: the exact products decide (rare)
-                const double ea = INT8 ? (double)(int)v0[j] : (double)a;
+                const double ea = INT8 ? (double)iv : (double)a;
                 const double e1 = INT8 ? (double)__float_as_int(run.a1) : (double)run.a1;
                 better = ea * p.e.colscale[k] > e1 * p.e.colscale[run.i1];
               }
-              const float araw = INT8 ? __uint_as_float(v0[j]) : a;   // integer accumulators are kept bit for bit
+              if (INT8 && p.nparts == 3 && !scaled) {
+                // int16 codes: sums beyond 2^24 are not exact as floats, the integers decide
+                better = run.i1 == INT_MAX || iv > __float_as_int(run.a1);
+                second = run.i2 == INT_MAX || iv > __float_as_int(run.a2);
+              }
+              const float araw = INT8 ? __int_as_float(iv) : a;   // integer accumulators are kept bit for bit
               if (better) {
                 run.b2 = run.b1; run.a2 = run.a1; run.i2 = run.i1;
                 run.b1 = sc; run.a1 = araw; run.i1 = k;
-              } else if (sc > run.b2) {
+              } else if (second) {
                 run.b2 = sc; run.a2 = araw; run.i2 = k;
               }
             }
@@ -499,7 +507,9 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
 // k = tile*kc + (r % (nparts*kc)) % kc, part (r % (nparts*kc)) / kc of tile r / (nparts*kc); staged
 // column kb*BK + kappa holds dimension kb*BK + perm(kappa), zero for d >= D_eff or k >= K.
 // mode: 32 -> bf16 part j of the 3-way split; 16 -> bf16 RNE; HDC_HV_F16 -> IEEE half RNE; 8 -> int8
-// with scale 127/amax; 1 -> +-1 int8 from the sign.
+// with scale 127/amax; HDC_HV_I16 -> digit 2 - j (balanced, base 128, each in [-64, 63]; the top one in
+// [-2, 2]) of the int16 code with scale 32767/amax: q = 16384*part0 + 128*part1 + part2; 1 -> +-1 int8 from
+// the sign.
 __device__ __forceinline__ int quant_i8_c(float x, float s) {
   float q = rintf(__fmul_rn(x, s));
   q = fminf(fmaxf(q, -127.0f), 127.0f);
@@ -514,9 +524,9 @@ __global__ void class_operand_kernel(const float* __restrict__ C, int K, int D_e
   const int64_t ld = (int64_t)num_kb * BK;
   const int64_t total = (int64_t)rows_total * ld;
   float s = 1.0f;
-  if (mode == 8) {
+  if (mode == 8 || mode == HDC_HV_I16) {
     const float a = *amax;
-    s = a > 0.0f ? __fdiv_rn(127.0f, a) : 1.0f;
+    s = a > 0.0f ? __fdiv_rn(mode == 8 ? 127.0f : 32767.0f, a) : 1.0f;
   }
   for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < total;
        i += (int64_t)gridDim.x * blockDim.x) {
@@ -532,7 +542,19 @@ __global__ void class_operand_kernel(const float* __restrict__ C, int K, int D_e
     if (live) x = __ldg(C + (int64_t)k * ldc + d);
     if (INT8) {
       int qv = 0;
-      if (live) qv = (mode == 8) ? quant_i8_c(x, s) : (x < 0.0f ? -1 : 1);
+      if (live) {
+        if (mode == 8) {
+          qv = quant_i8_c(x, s);
+        } else if (mode == HDC_HV_I16) {
+          const int q = (int)fminf(fmaxf(rintf(__fmul_rn(x, s)), -32767.0f), 32767.0f);
+          const int d0 = ((q + 64) & 127) - 64;
+          const int r1 = (q - d0) >> 7;                  // exact: q - d0 is a multiple of 128
+          const int d1 = ((r1 + 64) & 127) - 64;
+          qv = part == 0 ? (r1 - d1) >> 7 : (part == 1 ? d1 : d0);
+        } else {
+          qv = x < 0.0f ? -1 : 1;
+        }
+      }
       reinterpret_cast<int8_t*>(dst)[i] = (int8_t)qv;
     } else if (mode == HDC_HV_F16) {
       reinterpret_cast<__half*>(dst)[i] = __float2half_rn(x);
@@ -637,8 +659,8 @@ cudaError_t launch_one(const CUtensorMap& tmB, const SimParams& p, int cg, int g
 }
 
 void sim_tc_shape(int K, int hv_bits, int D_eff, int& kc, int& nparts, int& n_tiles, int& num_kb, bool& int8) {
-  int8 = hv_bits == 8 || hv_bits == 1;
-  nparts = hv_bits == 32 ? 3 : 1;
+  int8 = hv_bits == 8 || hv_bits == 1 || hv_bits == HDC_HV_I16;
+  nparts = (hv_bits == 32 || hv_bits == HDC_HV_I16) ? 3 : 1;
   const int kc_max = nparts == 3 ? 80 : 256;
   kc = (K + 15) & ~15;
   if (kc > kc_max) kc = kc_max;
@@ -666,7 +688,7 @@ int sim_tc_splits(int64_t N, int K, int hv_bits, int D_eff, int sm_count, int* k
   sim_tc_shape(K, hv_bits, D_eff, kc, nparts, n_tiles, num_kb, int8);
   const int64_t m_tiles = (N + BM - 1) / BM;
   int splits = 1, kbs = num_kb;
-  const bool exact_ok = !int8 || (int64_t)D_eff * (hv_bits == 8 ? 127 : 1) < (1 << 24);
+  const bool exact_ok = !int8 || (int64_t)D_eff * (hv_bits == 8 ? 127 : (hv_bits == 1 ? 1 : 32767)) < (1 << 24);
   if (n_tiles == 1 && m_tiles * 2 <= sm_count && num_kb >= 32 && exact_ok) {
     int want = (int)(sm_count / m_tiles);
     if (want > 8) want = 8;
@@ -702,7 +724,7 @@ cudaError_t launch_sim_tc(TcContext* tc, const uint32_t* Hbits, int64_t N, int64
   const int BK = int8 ? 128 : 64;
   const int64_t ld = (int64_t)num_kb * BK;
   cudaError_t ce;
-  if (hv_bits == 8 && !cop_ready) {
+  if ((hv_bits == 8 || hv_bits == HDC_HV_I16) && !cop_ready) {
     ce = launch_tensor_amax(C_acc, K, D_eff, ldc, pf, amax_scratch, st, nlaunch);
     if (ce != cudaSuccess) return ce;
   }

@@ -250,3 +250,51 @@ def test_fp32_class_operand_carries_24_bit_integers_exactly(hd, h, K):
     absum = np.abs(Cd.astype(np.float64)).sum(axis=1)
     assert (np.abs(S - S_or) <= 2.0 ** -22 * absum[None, :]).all()
     check_labels_float(h.hdc_classify(Hd, dev(Cd), kn).cpu().numpy(), S_or, O.SIM_DOT)
+
+
+@pytest.mark.parametrize("K", [26, 1000])
+@pytest.mark.parametrize("flags_name", ["", "HDC_FLAG_TC_1CTA", "HDC_FLAG_SIMT"])
+def test_int16_class_operand_is_exact_in_int32(hd, h, K, flags_name):
+    """PAPER.md L165 "integer data types (8, 16, ...": hv code HDC_HV_I16 (reading A21).  Dense 16-bit accumulators with
+    max|c| = 32767 (scale exactly 1: the codes ARE the accumulators), D_eff = 10000, sums up to 3e8 -- far beyond what
+    fp32 holds exactly: the int32 DOT scores equal the oracle's integers, the fp32 scores are those integers rounded
+    once, labels (decided on the integers: adjacent integers above 2^24 collide as floats) and cosines agree; the
+    tensor path (three base-128 digits on kind::i8, CTA pairs and one CTA) and the CUDA-core path alike."""
+    N, D = 300, 10000
+    flags = getattr(hd, flags_name) if flags_name else 0
+    r = np.random.default_rng([44, K])
+    bits = r.integers(0, 2, size=(N, D), dtype=np.uint8)
+    C = r.integers(-32767, 32768, size=(K, D)).astype(np.float32)
+    C[0, 0] = 32767.0
+    # class 2 = class 1 except one +-2 change in one dimension: their scores differ by 2 or 4 around 1e6..3e8
+    C[2] = C[1]
+    C[2, 17] = C[1, 17] - 2.0 if C[1, 17] > 0 else C[1, 17] + 2.0
+    # queries 0..7 are (nearly) class 1's sign pattern: scores ~ sum|c| ~ 1.6e8 >> 2^24, winner decided by 2 units
+    bits[:8] = (C[1] < 0).astype(np.uint8)[None, :]
+    bits[:8, 17] = np.arange(8) % 2
+    Hd, Cd = dev_bits(bits), dev(C)
+    S_or = O.similarity(bits, C, D, O.SIM_DOT, O.HV_I16)
+    assert np.array_equal(S_or, O.similarity(bits, C, D, O.SIM_DOT, 32))        # scale 1: codes = accumulators
+    assert np.abs(S_or).max() > 2 ** 27
+    kn = hd.knobs(D, hv_bits=hd.HDC_HV_I16, sim=hd.HDC_SIM_DOT, flags=flags)
+    Si = h.hdc_similarity(Hd, Cd, kn, s_dtype=torch.int32).cpu().numpy()
+    assert np.array_equal(Si.astype(np.float64), S_or)
+    Sf = h.hdc_similarity(Hd, Cd, kn).cpu().numpy()
+    assert np.array_equal(Sf, S_or.astype(np.float32))
+    lab_or, best_or, sec_or = O.classify(S_or, O.SIM_DOT)
+    assert set(lab_or[:8].tolist()) <= {1, 2} and len(set(lab_or[:8].tolist())) == 2
+    lab, best, sec = h.hdc_classify(Hd, Cd, kn, want_scores=True)
+    assert np.array_equal(lab.cpu().numpy(), lab_or)
+    assert np.array_equal(best.cpu().numpy(), best_or.astype(np.float32))
+    assert np.array_equal(sec.cpu().numpy(), sec_or.astype(np.float32))
+    # cosine: codes' norms in double, labels exact
+    knc = hd.knobs(D, hv_bits=hd.HDC_HV_I16, sim=hd.HDC_SIM_COS, flags=flags)
+    Sc_or = O.similarity(bits, C, D, O.SIM_COS, O.HV_I16)
+    assert np.allclose(h.hdc_similarity(Hd, Cd, knc).cpu().numpy(), Sc_or, rtol=1e-6, atol=1e-9)
+    assert np.array_equal(h.hdc_classify(Hd, Cd, knc).cpu().numpy(), O.classify(Sc_or, O.SIM_COS)[0])
+    # a non-unit scale (max|c| not 32767) and a D_eff prefix
+    C2 = (r.standard_normal((K, D)) * 30).astype(np.float32)
+    kn2 = hd.knobs(4099, hv_bits=hd.HDC_HV_I16, sim=hd.HDC_SIM_DOT, flags=flags)
+    S2_or = O.similarity(bits, C2, 4099, O.SIM_DOT, O.HV_I16)
+    assert np.array_equal(h.hdc_similarity(Hd, dev(C2), kn2, s_dtype=torch.int32).cpu().numpy().astype(np.float64), S2_or)
+    assert np.array_equal(h.hdc_classify(Hd, dev(C2), kn2).cpu().numpy(), O.classify(S2_or, O.SIM_DOT)[0])

@@ -58,7 +58,7 @@ def _check_stage2(hd, lab, best, second, bits, C, D_eff, sim_name, hv_bits, begi
     sim = SIMS[sim_name]
     S_or = O.similarity(bits, C, D_eff, sim, hv_bits, begin, stride)
     lab_or, b_or, s_or = O.classify(S_or, sim)
-    if hv_bits in (8, 1):
+    if hv_bits in (18, 8, 1):
         assert np.array_equal(lab, lab_or)
         assert np.allclose(best, b_or, rtol=1e-6, atol=1e-6) and np.allclose(second, s_or, rtol=1e-6, atol=1e-6)
     else:
@@ -143,16 +143,17 @@ def test_infer_rp_fused_perforated_similarity(hd, h, sim_name, hv_bits, begin, s
                   stride)
 
 
-@pytest.mark.parametrize("N,K,flags", [(12288, 26, 0), (12288, 33, 16), (500, 26, 16), (12288, 26, 16 | 1),
-                                       (12288, 26, 16 | 2), (0, 26, 16)])
-def test_infer_rp_two_kernel_path_and_stats(hd, h, N, K, flags):
-    """The default (no HDC_FLAG_FUSED_INFER = 16), and with the flag: large K, small N, HDC_FLAG_SIMT and
-    HDC_FLAG_TC_1CTA, take hdc_encode_rp + hdc_classify; the result obeys the same rules and hdc_stat reports
-    which path ran."""
+@pytest.mark.parametrize("N,K,flags,hv_bits", [(12288, 26, 0, 8), (12288, 33, 16, 8), (500, 26, 16, 8),
+                                               (12288, 26, 16 | 1, 8), (12288, 26, 16 | 2, 8), (0, 26, 16, 8),
+                                               (12288, 26, 16, 18), (700, 26, 0, 18)])
+def test_infer_rp_two_kernel_path_and_stats(hd, h, N, K, flags, hv_bits):
+    """The default (no HDC_FLAG_FUSED_INFER = 16), and with the flag: large K, small N, HDC_FLAG_SIMT,
+    HDC_FLAG_TC_1CTA and int16 class codes (hv code 18: sums beyond what the fused fp32 search holds exactly),
+    take hdc_encode_rp + hdc_classify; the result obeys the same rules and hdc_stat reports which path ran."""
     F, D = 64, 600
     X, P, C = _int_inputs(max(N, 1), F, D, K, (4, N, K, flags))
     X = X[:N]
-    kn = hd.knobs(D, precision=hd.HDC_BF16, hv_bits=8, sim=hd.HDC_SIM_COS, flags=flags)
+    kn = hd.knobs(D, precision=hd.HDC_BF16, hv_bits=hv_bits, sim=hd.HDC_SIM_COS, flags=flags)
     u0, f0 = h.stat(hd.HDC_STAT_INFER_UNFUSED), h.stat(hd.HDC_STAT_INFER_FUSED)
     H = h.alloc_hbits(N, D)
     lab, best, second = h.hdc_infer_rp(dev(X) if N else torch.empty((0, F), device="cuda"), dev(P), dev(C), kn,
@@ -163,7 +164,7 @@ def test_infer_rp_two_kernel_path_and_stats(hd, h, N, K, flags):
     if N:
         bits = host_bits(H, D)
         assert np.array_equal(bits, O.encode_rp(X, P, D, O.BF16)[0])
-        _check_stage2(hd, lab.cpu().numpy(), best.cpu().numpy(), second.cpu().numpy(), bits, C, D, "COS", 8)
+        _check_stage2(hd, lab.cpu().numpy(), best.cpu().numpy(), second.cpu().numpy(), bits, C, D, "COS", hv_bits)
 
 
 def test_infer_rp_argument_errors(hd, h):

@@ -212,7 +212,7 @@ def test_encode_rp_bf16_inputs_in_place(hd, h):
 
 # ------------------------------------------------------------------------------------ dot / cos
 @pytest.mark.parametrize("sim", ["DOT", "COS"])
-@pytest.mark.parametrize("hv_bits", [32, 16, 17, 8, 1])   # 17 = HDC_HV_F16: IEEE half class operand
+@pytest.mark.parametrize("hv_bits", [32, 16, 17, 18, 8, 1])   # 17 = HDC_HV_F16 (IEEE half), 18 = HDC_HV_I16 (int16 codes)
 @pytest.mark.parametrize("N,K,D,D_eff", [(150, 26, 2100, 2100), (64, 6, 10000, 4099), (33, 1, 500, 500),
                                          (140, 70, 1300, 1000), (140, 600, 1300, 1000), (300, 200, 700, 640),
                                          (130, 1000, 520, 520)])
@@ -231,9 +231,11 @@ def test_dot_cos_similarity_and_classify(hd, h, sim, hv_bits, N, K, D, D_eff):
     lab, best, sec = h.hdc_classify(Hd, Cd, kn, want_scores=True)
     lab = lab.cpu().numpy()
     lab_or, best_or, sec_or = O.classify(S_or, simc)
-    if hv_bits in (8, 1):                                   # integer contraction: exact
+    if hv_bits in (18, 8, 1):                               # integer contraction: exact
         if sim == "DOT":
-            assert np.array_equal(S.astype(np.float64), S_or)
+            # fp32 scores: the exact int32 sum, rounded once where it exceeds 24 bits (int16 codes only)
+            assert np.array_equal(S, S_or.astype(np.float32))
+            assert hv_bits == 18 or np.array_equal(S.astype(np.float64), S_or)
             Si = h.hdc_similarity(Hd, Cd, kn, s_dtype=torch.int32).cpu().numpy()
             assert np.array_equal(Si.astype(np.float64), S_or)
         else:
@@ -249,7 +251,8 @@ def test_dot_cos_similarity_and_classify(hd, h, sim, hv_bits, N, K, D, D_eff):
     assert np.allclose(sec.cpu().numpy()[same], sec_or[same], rtol=1e-3, atol=1e-5)
 
 
-@pytest.mark.parametrize("sim,hv_bits", [("COS", 32), ("DOT", 16), ("COS", 17), ("COS", 8), ("DOT", 8), ("DOT", 1), ("HAMMING", 1)])
+@pytest.mark.parametrize("sim,hv_bits", [("COS", 32), ("DOT", 16), ("COS", 17), ("COS", 8), ("DOT", 8), ("DOT", 1), ("HAMMING", 1),
+                                         ("COS", 18), ("DOT", 18)])
 @pytest.mark.parametrize("N,K,D,D_eff,perf", [(300, 26, 2100, 2100, (0, 1)), (129, 1000, 520, 520, (0, 1)), (513, 200, 1300, 1000, (0, 1)),
                                               (1, 70, 700, 33, (0, 1)), (257, 600, 1300, 1000, (3, 8)), (640, 6, 10000, 4099, (0, 1))])
 def test_similarity_on_cta_pairs(hd, h, sim, hv_bits, N, K, D, D_eff, perf):
@@ -274,11 +277,11 @@ def test_similarity_on_cta_pairs(hd, h, sim, hv_bits, N, K, D, D_eff, perf):
         S = h.hdc_similarity(Hd, Cd, kn).cpu().numpy()
         lab, best, sec = h.hdc_classify(Hd, Cd, kn, want_scores=True)
         lab = lab.cpu().numpy()
-        if hv_bits in (8, 1):
+        if hv_bits in (18, 8, 1):
             if sim == "COS":
                 assert np.allclose(S, S_or, rtol=1e-6, atol=1e-9)
             else:
-                assert np.array_equal(S.astype(np.float64), S_or)
+                assert np.array_equal(S, S_or.astype(np.float32))
             assert np.array_equal(lab, lab_or)
             assert np.allclose(best.cpu().numpy(), best_or, rtol=1e-6, atol=1e-9)
             assert np.allclose(sec.cpu().numpy(), sec_or, rtol=1e-6, atol=1e-9)
@@ -288,7 +291,7 @@ def test_similarity_on_cta_pairs(hd, h, sim, hv_bits, N, K, D, D_eff, perf):
             check_scores(S, S_or, floor)
             check_labels_float(lab, S_or, simc)
         out[flags] = (S, lab)
-    if hv_bits in (8, 1):
+    if hv_bits in (18, 8, 1):
         if sim == "COS":   # (the split-reduction path of the one-CTA kernel scales in double, the others in fp32)
             assert np.allclose(out[hd.HDC_FLAG_TC_2CTA][0], out[hd.HDC_FLAG_TC_1CTA][0], rtol=1e-6, atol=1e-9)
         else:
@@ -328,7 +331,7 @@ def test_bundle_exact(hd, h, N, K, D, D_eff):
 
 
 @pytest.mark.parametrize("B", [0, 1, 7, 64])
-@pytest.mark.parametrize("hv_bits,sim", [(1, "HAMMING"), (8, "COS")])
+@pytest.mark.parametrize("hv_bits,sim", [(1, "HAMMING"), (8, "COS"), (18, "COS"), (18, "DOT")])
 def test_perceptron_epoch_integer_paths_exact(hd, h, B, hv_bits, sim):
     """Integer similarity => identical predictions => identical Delta => identical fp32 update."""
     w = gen.c1_tiny(D=512)
@@ -454,7 +457,7 @@ def test_kmeans_empty_cluster_keeps_accumulator(hd, h):
 # ------------------------------------------------------------------------------------ perforation
 @pytest.mark.parametrize("begin,stride", [(0, 8), (3, 8), (5, 2), (1, 3), (17, 1), (0, 64)])
 @pytest.mark.parametrize("sim,hv_bits", [("HAMMING", 1), ("DOT", 1), ("DOT", 8), ("COS", 8), ("COS", 32), ("COS", 16),
-                                         ("DOT", 32)])
+                                         ("DOT", 32), ("DOT", 18), ("COS", 18)])
 @pytest.mark.parametrize("N,K,D,D_eff", [(150, 10, 2100, 2100), (70, 70, 1300, 1000), (33, 3, 10000, 8400)])
 def test_perforated_similarity_and_classify(hd, h, begin, stride, sim, hv_bits, N, K, D, D_eff):
     """General reduction perforation of the similarity (reading A17): the kernels
@@ -472,11 +475,11 @@ def test_perforated_similarity_and_classify(hd, h, begin, stride, sim, hv_bits, 
     S = h.hdc_similarity(Hd, Cd, kn).cpu().numpy()
     lab = h.hdc_classify(Hd, Cd, kn).cpu().numpy()
     lab_or, _, _ = O.classify(S_or, simc)
-    if hv_bits in (8, 1):
+    if hv_bits in (18, 8, 1):
         if sim == "COS":
             assert np.allclose(S, S_or, rtol=1e-6, atol=1e-9)
         else:
-            assert np.array_equal(S.astype(np.float64), S_or.astype(np.float64))
+            assert np.array_equal(S, S_or.astype(np.float32))
         assert np.array_equal(lab, lab_or)
     else:
         idx = O.perforated_index(D_eff, begin, stride)
@@ -640,6 +643,8 @@ def test_similarity_classify_fuzz(hd, h, case):
                     ("DOT", 16)][int(r.integers(0, 8))]
     if hv_bits == 16 and case % 2:
         hv_bits = 17                                           # HDC_HV_F16
+    if hv_bits == 8 and case % 3 == 0:
+        hv_bits = 18                                           # HDC_HV_I16
     begin, stride = 0, 1
     if r.random() < 0.35:
         stride = int(r.choice([2, 3, 8, 32]))
@@ -654,11 +659,11 @@ def test_similarity_classify_fuzz(hd, h, case):
     S = h.hdc_similarity(Hd, Cd, kn).cpu().numpy()
     lab = h.hdc_classify(Hd, Cd, kn).cpu().numpy()
     lab_or, _, _ = O.classify(S_or, simc)
-    if hv_bits in (8, 1):
+    if hv_bits in (18, 8, 1):
         if sim == "COS":
             assert np.allclose(S, S_or, rtol=1e-6, atol=1e-9)
         else:
-            assert np.array_equal(S.astype(np.float64), S_or.astype(np.float64))
+            assert np.array_equal(S, S_or.astype(np.float32))
         assert np.array_equal(lab, lab_or)
     else:
         idx = O.perforated_index(D_eff, begin, stride)
