@@ -122,9 +122,21 @@ __device__ __forceinline__ uint32_t prmt_sign_bytes(uint32_t v) {
   return d;
 }
 
-template <bool INT8, int EPI, int CG>
+// TS: the expanded query tile lives in TENSOR memory instead of shared memory (tcgen05.mma with the A operand in
+// TMEM): expanders write their rows with tcgen05.st into a ring of 8 k-block slots (32 columns each) beside two
+// 128-column accumulators, the ring stages hold only the class tile.  For class tiles of <= 128 rows, where the
+// shared-memory traffic of the A tile (16 KB written + 16 KB read per k-block against 2..12 KB of class rows)
+// was the bound.  One CTA per tile.
+constexpr int TS_ACC_COLS = 128;
+constexpr int TS_A_COL0 = 2 * TS_ACC_COLS;
+constexpr int TS_STAGES = (TMEM_COLS - TS_A_COL0) / 32;   // 8
+
+template <bool INT8, int EPI, int CG, bool TS = false>
 __global__ void __launch_bounds__(NTHREADS, 1)
 sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
+  static_assert(!TS || CG == 1, "the tensor-memory A ring is a one-CTA layout");
+  constexpr uint32_t B_OFF = TS ? 0u : (uint32_t)A_BYTES;     // class tile within a ring stage
+  constexpr int ACC_STRIDE = TS ? TS_ACC_COLS : BN_MAX;       // TMEM columns between the two accumulators
   extern __shared__ uint8_t smem_raw[];
   const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
   const int STAGES = p.stages;  // k-block slots in the ring
@@ -191,12 +203,12 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
           // both CTAs' halves complete on the leader's barrier; only the leader arms it
           if (rank == 0) mbar_arrive_expect_tx_elect(full_bar(grp), (uint32_t)(n * nb_rows) * KB_BYTES);
           for (int u = 0; u < n; ++u)
-            tma_load_2d_2sm_elect(base + (grp * G + u) * STAGE_BYTES + A_BYTES, &tmB, full_bar(grp) & PEER_MASK,
+            tma_load_2d_2sm_elect(base + (grp * G + u) * STAGE_BYTES + B_OFF, &tmB, full_bar(grp) & PEER_MASK,
                                   (kb0 + u) * BK, nt * nb_rows + rank * nb_half);
         } else {
           mbar_arrive_expect_tx_elect(full_bar(grp), (uint32_t)(n * nb_rows) * KB_BYTES);
           for (int u = 0; u < n; ++u)
-            tma_load_2d_elect(base + (grp * G + u) * STAGE_BYTES + A_BYTES, &tmB, full_bar(grp), (kb0 + u) * BK,
+            tma_load_2d_elect(base + (grp * G + u) * STAGE_BYTES + B_OFF, &tmB, full_bar(grp), (kb0 + u) * BK,
                               nt * nb_rows);
         }
         __syncwarp();
@@ -217,7 +229,7 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
     for (int64_t i = 0; rank == 0 && i < tiles_per_cta; ++i) {
       mbar_wait(tempty_bar(acc), acc_phase ^ 1u);
       tc_fence_after();
-      const uint32_t d_tmem = tmem_base + (uint32_t)(acc * BN_MAX);
+      const uint32_t d_tmem = tmem_base + (uint32_t)(acc * ACC_STRIDE);
       int mt, sp, kb_lo, kb_hi;
       item_of(i, mt, sp, kb_lo, kb_hi);
       for (int kb0 = kb_lo; kb0 < kb_hi; kb0 += G) {
@@ -227,10 +239,18 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
         // whole warp, converged: each call issues once (tc_ptx.cuh, *_elect)
         for (int u = 0; u < n; ++u) {
           const uint32_t sa = base + (grp * G + u) * STAGE_BYTES;
-          const uint64_t da = smem_desc(sa), db = smem_desc(sa + A_BYTES);
+          if constexpr (TS) {
+            const uint64_t db = smem_desc(sa);
+            const uint32_t at = tmem_base + (uint32_t)(TS_A_COL0 + (grp * G + u) * 32);
 #pragma unroll
-          for (int k = 0; k < KB_BYTES / 32; ++k)
-            tc_mma_elect<INT8, CG>(d_tmem, da + 2u * k, db + 2u * k, idesc, (kb0 + u != kb_lo || k != 0) ? 1u : 0u);
+            for (int k = 0; k < KB_BYTES / 32; ++k)
+              tc_mma_ts_elect<INT8>(d_tmem, at + 8u * k, db + 2u * k, idesc, (kb0 + u != kb_lo || k != 0) ? 1u : 0u);
+          } else {
+            const uint64_t da = smem_desc(sa), db = smem_desc(sa + A_BYTES);
+#pragma unroll
+            for (int k = 0; k < KB_BYTES / 32; ++k)
+              tc_mma_elect<INT8, CG>(d_tmem, da + 2u * k, db + 2u * k, idesc, (kb0 + u != kb_lo || k != 0) ? 1u : 0u);
+          }
         }
         tc_commit_elect<CG>(empty_bar(grp));  // frees the group's slots (in both CTAs) when these MMAs retire
         if (kb0 + n == kb_hi) tc_commit_elect<CG>(tfull_bar(acc));
@@ -260,7 +280,7 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
       const bool row_ok = row < p.N;
       mbar_wait(tfull_bar(acc), acc_phase);
       tc_fence_after();
-      const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(acc * BN_MAX);
+      const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(acc * ACC_STRIDE);
       const int k_base = nt * p.kc;
       int k_valid = p.K - k_base;
       if (k_valid > p.kc) k_valid = p.kc;
@@ -362,7 +382,8 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
     // Query words reach each expander warp through its private 3-deep cp.async ring (see CW above): nothing is
     // staged in registers, and a copy instruction covers 4 rows x 8 words whatever ldh is.
     const int et = (int)threadIdx.x - 192;    // 0..255
-    const int t = et & (BM - 1);              // row of the tile
+    // row of the tile; TS: a warp reaches only the TMEM lanes of ITS quarter (warp index mod 4)
+    const int t = TS ? ((warp & 3) * 32 + lane) : (et & (BM - 1));
     const int part_id = et / BM;              // which half of a row's eight 16-byte chunks (warp-uniform)
     const int ew = et >> 5;                   // expander warp 0..7
     constexpr int C_PER = 8 / (EXW / 4);
@@ -430,26 +451,30 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
       uint32_t wq[WPP];
 #pragma unroll
       for (int v = 0; v < WPP; ++v) wq[v] = qk[v];
+      uint32_t o[4 * C_PER];
 #pragma unroll
-      for (int cc = 0; cc < C_PER; ++cc) {  // 16-byte chunk cidx of the row = 4 shared-memory words
+      for (int cc = 0; cc < C_PER; ++cc) {  // 16-byte chunk cidx of the row = 4 words
         const int cidx = C0 + cc;
-        uint32_t o[4];
 #pragma unroll
         for (int e = 0; e < 4; ++e) {
           const int iw = 4 * cidx + e;  // word index within the k-block's 32 output words
           if (INT8) {
             const uint32_t w = wq[(iw >> 3) - PART * WPP];
-            o[e] = prmt_sign_bytes(w << (7 - (iw & 7))) | 0x01010101u;
+            o[4 * cc + e] = prmt_sign_bytes(w << (7 - (iw & 7))) | 0x01010101u;
           } else {
             const uint32_t w = wq[(iw >> 4) - PART * WPP];
-            o[e] = ((w << (15 - (iw & 15))) & 0x80008000u) | one2;
+            o[4 * cc + e] = ((w << (15 - (iw & 15))) & 0x80008000u) | one2;
           }
         }
-        const uint32_t dst = a_row + ((((uint32_t)cidx) ^ sw) << 4);
-        asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(dst), "r"(o[0]), "r"(o[1]), "r"(o[2]),
-                     "r"(o[3])
-                     : "memory");
+        if constexpr (!TS) {
+          const uint32_t dst = a_row + ((((uint32_t)cidx) ^ sw) << 4);
+          asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(dst), "r"(o[4 * cc]), "r"(o[4 * cc + 1]),
+                       "r"(o[4 * cc + 2]), "r"(o[4 * cc + 3])
+                       : "memory");
+        }
       }
+      // TS: a_row is the k-block's TMEM slot (this warp's lane quarter); word iw of the row = column iw
+      if constexpr (TS) tmem_st16(a_row + (uint32_t)(4 * C0), o);
     };
     for (int64_t i = 0; i < tiles_per_cta; ++i) {
       int mt, sp, kb_lo, kb_hi;
@@ -467,16 +492,27 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
         while (left > 0) {
           const int n = left < G ? left : G;
           mbar_wait(empty_bar(grp), phase ^ 1u);
-          uint32_t a_row = base + (uint32_t)(grp * G) * STAGE_BYTES + (uint32_t)t * KB_BYTES;
+          uint32_t a_row;
+          if constexpr (TS) {
+            tc_fence_after();   // the MMAs that read these TMEM slots have retired (tcgen05.commit -> empty)
+            a_row = tmem_base + ((uint32_t)(t & ~31) << 16) + (uint32_t)(TS_A_COL0 + grp * G * 32);
+          } else {
+            a_row = base + (uint32_t)(grp * G) * STAGE_BYTES + (uint32_t)t * KB_BYTES;
+          }
 #pragma unroll 1
           for (int u = 0; u < n; ++u) {
             if (part_id == 0) expand(std::integral_constant<int, 0>{}, qk, a_row);
             else expand(std::integral_constant<int, 1>{}, qk, a_row);
             qk += WPP;
-            a_row += STAGE_BYTES;
+            a_row += TS ? 32u : STAGE_BYTES;
           }
-          // the group is published with one proxy fence and one arrival per warp
-          fence_proxy_async_smem();
+          // the group is published with one fence and one arrival per warp
+          if constexpr (TS) {
+            tmem_st_wait();
+            tc_fence_before();
+          } else {
+            fence_proxy_async_smem();
+          }
           __syncwarp();
           if (lane == 0) {
             if (CG == 2) mbar_arrive_remote(full_bar(grp) & PEER_MASK);   // the leader's barrier, from either CTA
@@ -632,10 +668,10 @@ __global__ void split_reduce_kernel(const float* __restrict__ partial, int split
   }
 }
 
-template <bool INT8, int EPI, int CG>
+template <bool INT8, int EPI, int CG, bool TS = false>
 cudaError_t launch_cg(const CUtensorMap& tmB, const SimParams& p, int grid, cudaStream_t st) {
   // per-device attribute of the function: set on every launch (handles on several devices of one process)
-  cudaError_t e = cudaFuncSetAttribute(sim_tc_kernel<INT8, EPI, CG>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+  cudaError_t e = cudaFuncSetAttribute(sim_tc_kernel<INT8, EPI, CG, TS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                        SMEM_LIMIT);
   if (e != cudaSuccess) return e;
   const int smem = p.stages * p.stage_bytes + SMEM_EXTRA + qring_bytes(CG);
@@ -651,10 +687,11 @@ cudaError_t launch_cg(const CUtensorMap& tmB, const SimParams& p, int grid, cuda
   at[0].val.clusterDim.z = 1;
   cfg.attrs = at;
   cfg.numAttrs = 1;
-  return cudaLaunchKernelEx(&cfg, sim_tc_kernel<INT8, EPI, CG>, tmB, p);
+  return cudaLaunchKernelEx(&cfg, sim_tc_kernel<INT8, EPI, CG, TS>, tmB, p);
 }
 template <bool INT8, int EPI>
-cudaError_t launch_one(const CUtensorMap& tmB, const SimParams& p, int cg, int grid, cudaStream_t st) {
+cudaError_t launch_one(const CUtensorMap& tmB, const SimParams& p, int cg, bool ts, int grid, cudaStream_t st) {
+  if (ts) return launch_cg<INT8, EPI, 1, true>(tmB, p, grid, st);
   return cg == 2 ? launch_cg<INT8, EPI, 2>(tmB, p, grid, st) : launch_cg<INT8, EPI, 1>(tmB, p, grid, st);
 }
 
@@ -748,6 +785,9 @@ cudaError_t launch_sim_tc(TcContext* tc, const uint32_t* Hbits, int64_t N, int64
   // 0.294 ms per 131072 queries; bf16 / int8 classes at small K are bound by the expansion itself and lose 5-15 %)
   int cg = (sm_count >= 2 && (K >= 128 || nparts == 3) && (N + 2 * BM - 1) / (2 * BM) >= sm_count / 2) ? 2 : 1;
   if (force_cg == 1 || (force_cg == 2 && sm_count >= 2)) cg = force_cg;
+  // class tiles of <= 128 rows: the one-CTA kernel with the query tile in tensor memory (unless pairs are forced)
+  const bool ts = nparts * kc <= TS_ACC_COLS && force_cg != 2;
+  if (ts) cg = 1;
   CUtensorMap tmB;
   if (!tc_make_map(tc, &tmB, cop, int8, rows_total, ld, ld, nparts * kc / cg)) return cudaErrorInvalidValue;
   SimParams p;
@@ -762,9 +802,10 @@ cudaError_t launch_sim_tc(TcContext* tc, const uint32_t* Hbits, int64_t N, int64
   p.n_tiles = n_tiles;
   p.num_kb = num_kb;
   p.f16 = hv_bits == HDC_HV_F16;
-  p.stage_bytes = A_BYTES + nparts * kc / cg * KB_BYTES;
+  p.stage_bytes = (ts ? 0 : A_BYTES) + nparts * kc / cg * KB_BYTES;
   p.stages = (SMEM_LIMIT - SMEM_EXTRA - qring_bytes(cg)) / p.stage_bytes;
   if (p.stages > MAX_STAGES) p.stages = MAX_STAGES;
+  if (ts && p.stages > TS_STAGES) p.stages = TS_STAGES;
   // k-blocks per pipeline group: every hand-off through the full / empty barriers costs several hundred
   // cycles whatever the k-block holds, so short k-blocks (few class rows) travel in groups
   p.kps = p.stages >= 8 ? 4 : (p.stages >= 4 ? 2 : 1);   // (divides the k-blocks of a ring tile: 16 / 8 / 4)
@@ -778,17 +819,18 @@ cudaError_t launch_sim_tc(TcContext* tc, const uint32_t* Hbits, int64_t N, int64
   const int grid = (int)(items < max_units ? items : max_units) * cg;
   ++*nlaunch;
   if (p.splits > 1) {
-    ce = int8 ? launch_one<true, EPI_SCORE>(tmB, p, 1, grid, st) : launch_one<false, EPI_SCORE>(tmB, p, 1, grid, st);
+    ce = int8 ? launch_one<true, EPI_SCORE>(tmB, p, 1, ts, grid, st)
+              : launch_one<false, EPI_SCORE>(tmB, p, 1, ts, grid, st);
     if (ce != cudaSuccess) return ce;
     split_reduce_kernel<<<(unsigned)((N + 127) / 128), 128, 0, st>>>(p.partial, p.splits, N, K, e);
     ++*nlaunch;
     return cudaGetLastError();
   }
   if (int8)
-    return e.kind == EPI_SCORE ? launch_one<true, EPI_SCORE>(tmB, p, cg, grid, st)
-                               : launch_one<true, EPI_ARGMAX>(tmB, p, cg, grid, st);
-  return e.kind == EPI_SCORE ? launch_one<false, EPI_SCORE>(tmB, p, cg, grid, st)
-                             : launch_one<false, EPI_ARGMAX>(tmB, p, cg, grid, st);
+    return e.kind == EPI_SCORE ? launch_one<true, EPI_SCORE>(tmB, p, cg, ts, grid, st)
+                               : launch_one<true, EPI_ARGMAX>(tmB, p, cg, ts, grid, st);
+  return e.kind == EPI_SCORE ? launch_one<false, EPI_SCORE>(tmB, p, cg, ts, grid, st)
+                             : launch_one<false, EPI_ARGMAX>(tmB, p, cg, ts, grid, st);
 }
 
 }  // namespace hdc

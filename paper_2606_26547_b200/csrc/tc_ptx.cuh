@@ -217,6 +217,31 @@ __device__ __forceinline__ void tc_mma_elect(uint32_t d_tmem, uint64_t adesc, ui
   }
 }
 #undef HDC_MMA_ELECT
+// A operand in tensor memory (lane = row of the 128-row tile, each 32-bit column = 32 bits of the row's K-major
+// elements; one MMA reads 8 columns), B from shared memory; one CTA
+#define HDC_MMA_TS_ELECT(KIND)                                                                       \
+  asm volatile(                                                                                      \
+      "{\n\t.reg .pred p, q;\n\telect.sync _|q, 0xffffffff;\n\tsetp.ne.b32 p, %4, 0;\n\t"            \
+      "@q tcgen05.mma.cta_group::1.kind::" KIND " [%0], [%1], %2, %3, p;\n\t}" ::"r"(d_tmem),           \
+      "r"(a_tmem), "l"(bdesc), "r"(idesc), "r"(accumulate)                                           \
+      : "memory")
+template <bool INT8>
+__device__ __forceinline__ void tc_mma_ts_elect(uint32_t d_tmem, uint32_t a_tmem, uint64_t bdesc, uint32_t idesc,
+                                                uint32_t accumulate) {
+  if (INT8) HDC_MMA_TS_ELECT("i8");
+  else HDC_MMA_TS_ELECT("f16");
+}
+#undef HDC_MMA_TS_ELECT
+// 32 lanes x 16 consecutive 32-bit columns, registers -> tensor memory: thread t of the warp writes lane (base + t)
+__device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t (&v)[16]) {
+  asm volatile(
+      "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], "
+      "{%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16};" ::"r"(taddr),
+      "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]), "r"(v[8]), "r"(v[9]),
+      "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15])
+      : "memory");
+}
+__device__ __forceinline__ void tmem_st_wait() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 
 // 32 lanes x 32 consecutive 32-bit columns: thread t of the warp gets lane (base + t), v[j] = column j
 __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
