@@ -353,6 +353,25 @@ int32_t hdc_infer_rp_m(hdc_handle_t h, const void* X, int32_t x_dtype, int64_t N
                        const hdc_model_t* m, int32_t* labels, float* best, float* second, uint32_t* Hbits,
                        int64_t ldh_words, void* ws, size_t ws_bytes, void* stream);
 
+/* ---- classify without any allocation or caller workspace ----------------------------------------
+ * = hdc_classify for knobs->sim == HDC_SIM_HAMMING, knobs->hv_bits == 1 (Hamming distance,
+ * arg-min, ties to the lowest k; perforation knobs honoured), same labels / best / second bit for bit, for callers
+ * that can neither allocate device memory nor hand over a workspace (under CUDA graph capture, tight serving
+ * loops).  The scratch the call needs -- the packed sign bits of the class accumulators, K * W words, and the
+ * perforation mask, W words, W = ceil(D_eff / 32) -- lives in a fixed array inside the library
+ * (HDC_STATIC_SCRATCH_BYTES of device memory on every GPU that loads the library, held until the process exits).
+ * Limits: (K + 1) * W * 4 <= HDC_STATIC_SCRATCH_BYTES and K <= 64; beyond them the call returns
+ * HDC_ERR_UNSUPPORTED (message in hdc_last_error) and launches nothing.  The call performs no cudaMalloc /
+ * cudaFree and calls no allocating library routine.
+ * The array is SHARED by every call on that GPU (all handles, all streams) and keeps the previous call's contents
+ * (each call rewrites every word it reads): two calls that may overlap on the GPU -- different streams without an
+ * event between them, or two host threads -- race on it; serialise them.  Other argument rules as hdc_classify. */
+#define HDC_STATIC_SCRATCH_BYTES (1u << 20)
+int32_t hdc_classify_hamming_static(hdc_handle_t h, const uint32_t* Hbits, int64_t N, int64_t ldh_words,
+                                    const float* C_acc, int32_t K, int64_t ldc, int32_t D,
+                                    const hdc_knobs_t* knobs, int32_t* labels, float* best, float* second,
+                                    void* stream);
+
 /* ---- end-to-end inference from host buffers ------------------------------------------------
  * encode_rp + classify for N queries whose features live in HOST memory (pinned for full speed):
  * copies X_host in chunks to the device (inside the call), runs hdc_infer_rp per chunk and copies the

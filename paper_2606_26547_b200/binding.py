@@ -34,7 +34,7 @@ EXPORTS = ("hdc_create", "hdc_destroy", "hdc_last_error", "hdc_version", "hdc_la
            "hdc_similarity", "hdc_similarity_adc",
            "hdc_classify", "hdc_train_epoch", "hdc_train_delta", "hdc_train_apply", "hdc_infer_rp_host",
            "hdc_kernel_timing", "hdc_kernel_time", "hdc_infer_rp", "hdc_stat", "hdc_model_bytes", "hdc_model_prepare",
-           "hdc_encode_rp_m", "hdc_classify_m", "hdc_infer_rp_m")
+           "hdc_encode_rp_m", "hdc_classify_m", "hdc_infer_rp_m", "hdc_classify_hamming_static")
 
 
 class hdc_knobs_t(C.Structure):
@@ -100,6 +100,8 @@ def lib() -> C.CDLL:
     L.hdc_similarity_adc.restype = i32
     L.hdc_classify.argtypes = [vp, vp, i64, i64, vp, i32, i64, i32, kp, vp, vp, vp, vp, sz, vp]
     L.hdc_classify.restype = i32
+    L.hdc_classify_hamming_static.argtypes = [vp, vp, i64, i64, vp, i32, i64, i32, kp, vp, vp, vp, vp]
+    L.hdc_classify_hamming_static.restype = i32
     L.hdc_train_epoch.argtypes = [vp, i32, vp, i64, i64, vp, vp, i32, i64, i32, kp, C.c_float, i64, vp, vp,
                                   vp, sz, vp]
     L.hdc_train_epoch.restype = i32
@@ -301,6 +303,24 @@ class Handle:
         rc = self._L.hdc_classify(self._h, _ptr(Hbits), N, _rowmajor(Hbits, "Hbits"), _ptr(C_acc), K,
                                   _rowmajor(C_acc, "C_acc"), D, C.byref(kn), _ptr(labels), _ptr(best),
                                   _ptr(second), ws, wsb, self._stream())
+        self._check(rc)
+        return (labels, best, second) if want_scores else labels
+
+    def hdc_classify_hamming_static(self, Hbits, C_acc, kn: hdc_knobs_t, want_scores: bool = False, labels=None,
+                                    best=None, second=None):
+        """hdc_classify (Hamming, 1-bit classes) with the library's fixed scratch array: no workspace argument, no
+        allocation inside the call (pass labels / best / second to allocate nothing on the torch side either)."""
+        N = Hbits.shape[0]
+        K, D = C_acc.shape
+        if labels is None:
+            labels = torch.empty(N, dtype=torch.int32, device=self.device)
+        if want_scores and best is None:
+            best = torch.empty(N, dtype=torch.float32, device=self.device)
+        if want_scores and second is None:
+            second = torch.empty(N, dtype=torch.float32, device=self.device)
+        rc = self._L.hdc_classify_hamming_static(self._h, _ptr(Hbits), N, _rowmajor(Hbits, "Hbits"), _ptr(C_acc), K,
+                                                 _rowmajor(C_acc, "C_acc"), D, C.byref(kn), _ptr(labels), _ptr(best),
+                                                 _ptr(second), self._stream())
         self._check(rc)
         return (labels, best, second) if want_scores else labels
 

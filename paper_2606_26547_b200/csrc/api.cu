@@ -31,6 +31,7 @@ struct hdc_ctx {
   std::vector<std::pair<cudaEvent_t, cudaEvent_t>> tev[HDC_K_COUNT];  // event pool per kernel id
   size_t tused[HDC_K_COUNT] = {0, 0, 0, 0};
   int64_t stats[HDC_STAT_COUNT] = {0, 0, 0, 0};
+  uint32_t* static_scratch = nullptr;  // device address of g_static_scratch on this handle's device (resolved once)
 };
 
 namespace hdc {
@@ -1456,4 +1457,51 @@ extern "C" int32_t hdc_infer_rp_host(hdc_handle_t h, const void* X_host, int32_t
   ce = cudaStreamSynchronize(st);
   if (ce != cudaSuccess) return cuda_fail(h, ce, "infer_rp_host: sync");
   return HDC_OK;
+}
+
+// =================================================================================== no-allocation classify
+// Scratch of hdc_classify_hamming_static: a fixed array in the library's device image (one copy per GPU that loads
+// the library).  In host code the NAME below is only a stand-in for the symbol: the device address comes from
+// cudaGetSymbolAddress, asked once per handle with the handle's device current, and that pointer is what the kernels
+// receive.
+static __device__ __align__(256) uint32_t g_static_scratch[HDC_STATIC_SCRATCH_BYTES / 4];
+
+extern "C" int32_t hdc_classify_hamming_static(hdc_handle_t h, const uint32_t* Hbits, int64_t N, int64_t ldh_words,
+                                               const float* C_acc, int32_t K, int64_t ldc, int32_t D,
+                                               const hdc_knobs_t* knobs, int32_t* labels, float* best,
+                                               float* second, void* stream) {
+  if (!h) return HDC_ERR_INVALID_ARG;
+  DeviceGuard device_guard(h->device);
+  int rc = check_sim_args(h, Hbits, N, ldh_words, C_acc, K, ldc, D, knobs);
+  if (rc) return rc;
+  if (knobs->sim != HDC_SIM_HAMMING || knobs->hv_bits != 1)
+    return fail(h, HDC_ERR_INVALID_ARG, "classify_hamming_static: needs sim = HDC_SIM_HAMMING, hv_bits = 1");
+  if (!labels && N > 0) return fail(h, HDC_ERR_INVALID_ARG, "classify_hamming_static: labels is NULL");
+  const int D_eff = knobs->D_eff;
+  const int W = words_of(D_eff);
+  if (K > 64 || ((size_t)K + 1) * (size_t)W * sizeof(uint32_t) > (size_t)HDC_STATIC_SCRATCH_BYTES)
+    return fail(h, HDC_ERR_UNSUPPORTED,
+                "classify_hamming_static: needs K <= 64 and (K + 1) * ceil(D_eff / 32) * 4 <= HDC_STATIC_SCRATCH_BYTES "
+                "(1 MiB); use hdc_classify with a workspace");
+  if (N == 0) return HDC_OK;
+  cudaError_t ce;
+  if (!h->static_scratch) {
+    void* ptr = nullptr;
+    ce = cudaGetSymbolAddress(&ptr, g_static_scratch);   // the current device is h->device (DeviceGuard)
+    if (ce != cudaSuccess || !ptr) return cuda_fail(h, ce, "classify_hamming_static: cudaGetSymbolAddress");
+    h->static_scratch = static_cast<uint32_t*>(ptr);
+  }
+  cudaStream_t st = (cudaStream_t)stream;
+  const Perf pf = perf_of(knobs);
+  uint32_t* cbits = h->static_scratch;                                         // [K][W], every word rewritten
+  uint32_t* pmask = perf_on(pf) ? h->static_scratch + (size_t)K * W : nullptr;  // [W], every word rewritten
+  ce = launch_sign_bits(C_acc, K, D_eff, ldc, cbits, W, st, &h->launches);
+  if (ce != cudaSuccess) return cuda_fail(h, ce, "classify_hamming_static: sign_bits");
+  if (pmask) {
+    ce = launch_perf_mask(pmask, W, D_eff, pf, st, &h->launches);
+    if (ce != cudaSuccess) return cuda_fail(h, ce, "classify_hamming_static: perforation mask");
+  }
+  ce = launch_hamming(Hbits, N, ldh_words, cbits, K, W, D_eff, pmask, nullptr, 0, labels, best, second, h->sm_count,
+                      h->smem_optin, st, &h->launches);
+  return ce == cudaSuccess ? HDC_OK : cuda_fail(h, ce, "classify_hamming_static: hamming");
 }
