@@ -232,8 +232,9 @@ __device__ __forceinline__ void ripple(uint32_t (&q)[NP], uint32_t c, int from) 
 // L16: 16-bit level indices (PAPER.md L245 / L255: up to 1024 levels; the Micro-HD comparison tunes 814).  The staged
 // offsets are then the raw indices, two per word, and the "* 128" of the table address moves into the dp2a
 // selector.  A 1024-bit slice of an 814-level table is 104 KB, so the level rows of the 12 warps are staged in
-// chunks of p.chunk features by plain loads (measured: the kernel's rate follows the number of warps, 8 warps
-// with or without the register prefetch gave 114 M samples/s); the sparse path is left out.
+// chunks of p.chunk features by plain loads behind an L1 prefetch of the next chunk issued one chunk earlier (a
+// register prefetch costs 40 registers for rows that are only 2-byte aligned -- two halves per word -- and spills);
+// the sparse path is left out.
 template <int NP, bool VEC, bool L16, int NW>
 __global__ void __launch_bounds__(NW * 32, 1) levelid_fast_kernel(const LevelIdParams p) {
   constexpr int FSB = NW * FS;      // samples per batch (shadows the 12-warp constant)
@@ -563,6 +564,24 @@ __global__ void __launch_bounds__(NW * 32, 1) levelid_fast_kernel(const LevelIdP
           }
         }
         __syncwarp();
+        // The next chunk of this warp's rows (of this unit or the next) is pulled into L1 / L2 while this one is
+        // computed: every warp of the CTA reaches its staging loads at the same time (equal work per batch), so the
+        // other warps do not cover their latency (ncu: a third of the stall samples sat behind those loads).
+        {
+          const bool same = f0 + CH < p.F;
+          if (same || u + 1 < u_end) {
+            const int64_t nb = same ? batch : (u + 1) % p.n_batches;
+            const int nf0 = same ? f0 + CH : 0;
+            const int nfc = p.F - nf0 < CH ? p.F - nf0 : CH;
+            const int j = lane >> 3, ln = lane & 7;                  // 8 lanes per row, one 128-byte line each
+            const int64_t n = nb * FSB + warp * FS + j;
+            if (j < FS && n < p.N && ln * 64 < nfc + 64) {   // (rows are not line-aligned: the last element's line too)
+              const int e = ln * 64 < nfc ? ln * 64 : nfc - 1;
+              const uint16_t* a = static_cast<const uint16_t*>(p.levels) + n * p.ldl + nf0 + e;
+              asm volatile("prefetch.global.L1 [%0];" ::"l"(a));
+            }
+          }
+        }
       }
       const uint32_t* idp = sID + (size_t)f0 * SW + lane;
       int f = 0;
