@@ -92,6 +92,7 @@ struct SimParams {
   int stages;       // ring depth
   int stage_bytes;  // A_BYTES + nparts*kc*KB_BYTES
   int f16;          // 16-bit operands are IEEE half instead of bf16 (hv code HDC_HV_F16)
+  const int32_t* rowsum;   // INT8: sum of every staged class row (see the expanders), behind the staged operand
   Epilogue e;
 };
 
@@ -301,8 +302,21 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
             float a;
             int iv = 0;
             if (INT8) {
+              // TS: the expanders write the query bit b as the byte -128 b (one AND per word) instead of v = 1 - 2 b, so
+              // the accumulator holds -128 sum_{b=1} c and  sum_d v c = sum_d c - 2 sum_{b=1} c = rowsum + (acc >> 6),
+              // exactly (acc is a multiple of 128).  A split of the reduction axis adds the row sum once (split 0).
+              int i0 = (int)v0[j], i1 = (int)v1[j], i2 = (int)v2[j];
+              if constexpr (TS) {   // (wide class tiles keep +-1 bytes: one more load per column costs their epilogue more)
+                const int32_t* rs = p.rowsum + (size_t)nt * p.nparts * p.kc + c0 + j;
+                const bool first = sp == 0;
+                i0 = (i0 >> 6) + (first ? __ldg(rs) : 0);
+                if (p.nparts == 3) {
+                  i1 = (i1 >> 6) + (first ? __ldg(rs + p.kc) : 0);
+                  i2 = (i2 >> 6) + (first ? __ldg(rs + 2 * p.kc) : 0);
+                }
+              }
               // int16 class codes: three balanced base-128 digits, most significant first (exact in int32)
-              iv = p.nparts == 3 ? (int)v0[j] * 16384 + (int)v1[j] * 128 + (int)v2[j] : (int)v0[j];
+              iv = p.nparts == 3 ? i0 * 16384 + i1 * 128 + i2 : i0;
               a = (float)iv;
             } else if (p.nparts == 3) {
               a = __fadd_rn(__fadd_rn(__uint_as_float(v2[j]), __uint_as_float(v1[j])), __uint_as_float(v0[j]));
@@ -460,7 +474,10 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
           const int iw = 4 * cidx + e;  // word index within the k-block's 32 output words
           if (INT8) {
             const uint32_t w = wq[(iw >> 3) - PART * WPP];
-            o[4 * cc + e] = prmt_sign_bytes(w << (7 - (iw & 7))) | 0x01010101u;
+            // TS: byte = -128 * bit, one ALU instruction per word (the epilogue adds the class row sum: the ALU pipe
+            // bounds the small-tile kernel); else byte = 1 - 2 * bit
+            o[4 * cc + e] = TS ? ((w << (7 - (iw & 7))) & 0x80808080u)
+                               : (prmt_sign_bytes(w << (7 - (iw & 7))) | 0x01010101u);
           } else {
             const uint32_t w = wq[(iw >> 4) - PART * WPP];
             o[4 * cc + e] = ((w << (15 - (iw & 15))) & 0x80008000u) | one2;
@@ -555,7 +572,8 @@ __device__ __forceinline__ int quant_i8_c(float x, float s) {
 template <bool INT8>
 __global__ void class_operand_kernel(const float* __restrict__ C, int K, int D_eff, int64_t ldc, int mode,
                                      int kc, int nparts, int rows_total, int num_kb,
-                                     const float* __restrict__ amax, Perf pf, void* __restrict__ dst) {
+                                     const float* __restrict__ amax, Perf pf, void* __restrict__ dst,
+                                     int32_t* __restrict__ rowsum) {
   constexpr int BK = INT8 ? 128 : 64;
   const int64_t ld = (int64_t)num_kb * BK;
   const int64_t total = (int64_t)rows_total * ld;
@@ -592,6 +610,12 @@ __global__ void class_operand_kernel(const float* __restrict__ C, int K, int D_e
         }
       }
       reinterpret_cast<int8_t*>(dst)[i] = (int8_t)qv;
+      // row sums (zeroed by the launcher): the 32 elements of a warp's step lie in one staged row (ld % 128 == 0,
+      // total % 32 == 0), integer atomics: deterministic
+      int sum = qv;
+#pragma unroll
+      for (int off = 16; off; off >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, off);
+      if ((threadIdx.x & 31) == 0 && sum != 0) atomicAdd(rowsum + r, sum);
     } else if (mode == HDC_HV_F16) {
       reinterpret_cast<__half*>(dst)[i] = __float2half_rn(x);
     } else {
@@ -712,7 +736,8 @@ size_t sim_tc_operand_bytes(int K, int hv_bits, int D_eff) {
   int kc, nparts, n_tiles, num_kb;
   bool int8;
   sim_tc_shape(K, hv_bits, D_eff, kc, nparts, n_tiles, num_kb, int8);
-  return (size_t)n_tiles * nparts * kc * num_kb * KB_BYTES;
+  // staged rows (a multiple of 128 bytes), then for the int8 kinds one int32 sum per staged row
+  return (size_t)n_tiles * nparts * kc * num_kb * KB_BYTES + (int8 ? (size_t)n_tiles * nparts * kc * 4 : 0);
 }
 
 // Split-D for small N: with fewer m-tiles than half the SMs, `splits` CTAs share an m-tile, each
@@ -725,7 +750,7 @@ int sim_tc_splits(int64_t N, int K, int hv_bits, int D_eff, int sm_count, int* k
   sim_tc_shape(K, hv_bits, D_eff, kc, nparts, n_tiles, num_kb, int8);
   const int64_t m_tiles = (N + BM - 1) / BM;
   int splits = 1, kbs = num_kb;
-  const bool exact_ok = !int8 || (int64_t)D_eff * (hv_bits == 8 ? 127 : (hv_bits == 1 ? 1 : 32767)) < (1 << 24);
+  const bool exact_ok = !int8 || (int64_t)D_eff * 3 * (hv_bits == 8 ? 127 : (hv_bits == 1 ? 1 : 32767)) < (1 << 24);   // (small tiles: row sum + 2 x the split's share)
   if (n_tiles == 1 && m_tiles * 2 <= sm_count && num_kb >= 32 && exact_ok) {
     int want = (int)(sm_count / m_tiles);
     if (want > 8) want = 8;
@@ -765,16 +790,20 @@ cudaError_t launch_sim_tc(TcContext* tc, const uint32_t* Hbits, int64_t N, int64
     ce = launch_tensor_amax(C_acc, K, D_eff, ldc, pf, amax_scratch, st, nlaunch);
     if (ce != cudaSuccess) return ce;
   }
+  int32_t* rowsum = int8 ? reinterpret_cast<int32_t*>(static_cast<char*>(cop) + (size_t)rows_total * ld) : nullptr;
   if (!cop_ready) {
     const int64_t total = (int64_t)rows_total * ld;
     int64_t g = (total + 255) / 256;
     if (g > (int64_t)sm_count * 16) g = (int64_t)sm_count * 16;
-    if (int8)
+    if (int8) {
+      ce = cudaMemsetAsync(rowsum, 0, (size_t)rows_total * 4, st);
+      if (ce != cudaSuccess) return ce;
       class_operand_kernel<true><<<(unsigned)g, 256, 0, st>>>(C_acc, K, D_eff, ldc, hv_bits, kc, nparts, rows_total,
-                                                             num_kb, amax_scratch, pf, cop);
-    else
+                                                             num_kb, amax_scratch, pf, cop, rowsum);
+    } else {
       class_operand_kernel<false><<<(unsigned)g, 256, 0, st>>>(C_acc, K, D_eff, ldc, hv_bits, kc, nparts,
-                                                              rows_total, num_kb, amax_scratch, pf, cop);
+                                                              rows_total, num_kb, amax_scratch, pf, cop, nullptr);
+    }
     ++*nlaunch;
     ce = cudaGetLastError();
     if (ce != cudaSuccess) return ce;
@@ -802,6 +831,7 @@ cudaError_t launch_sim_tc(TcContext* tc, const uint32_t* Hbits, int64_t N, int64
   p.n_tiles = n_tiles;
   p.num_kb = num_kb;
   p.f16 = hv_bits == HDC_HV_F16;
+  p.rowsum = rowsum;
   p.stage_bytes = (ts ? 0 : A_BYTES) + nparts * kc / cg * KB_BYTES;
   p.stages = (SMEM_LIMIT - SMEM_EXTRA - qring_bytes(cg)) / p.stage_bytes;
   if (p.stages > MAX_STAGES) p.stages = MAX_STAGES;
