@@ -299,6 +299,36 @@ def test_similarity_on_cta_pairs(hd, h, sim, hv_bits, N, K, D, D_eff, perf):
         assert np.array_equal(out[hd.HDC_FLAG_TC_2CTA][1], out[hd.HDC_FLAG_TC_1CTA][1])
 
 
+@pytest.mark.parametrize("hv_bits,K", [(16, 112), (16, 128), (16, 129), (8, 128), (8, 129), (1, 128), (1, 130), (32, 32),
+                                       (32, 33), (18, 32), (18, 33), (17, 127), (32, 16), (8, 17)])
+@pytest.mark.parametrize("N,D_eff", [(300, 4099), (2100, 1000), (129, 10000)])
+def test_similarity_class_tile_width_boundaries(hd, h, hv_bits, K, N, D_eff):
+    """Class tiles of exactly / just over 128 staged rows (96 / 144 for the three-part operands): the two sides of the
+    switch between the kernel with the query tile in tensor memory and the one through shared memory, with few
+    queries (split reduction axis) and many, rows 16-byte aligned; COS scores, labels, best / runner-up."""
+    r = rng(77, hv_bits, K, N, D_eff)
+    D = D_eff + 13
+    hb = r.integers(0, 2, size=(N, D), dtype=np.uint8)
+    C = (r.standard_normal((K, D)) * 30).astype(np.float32)
+    C[r.random((K, D)) < 0.03] = 0.0
+    C[K - 1] = C[K - 2]                                     # exact tie between the last two classes of the tile
+    S_or = O.similarity(hb, C, D_eff, O.SIM_COS, hv_bits)
+    lab_or, best_or, sec_or = O.classify(S_or, O.SIM_COS)
+    kn = hd.knobs(D_eff, hv_bits=hv_bits, sim=hd.HDC_SIM_COS)
+    Hd, Cd = dev_bits(hb, (D + 127) // 128 * 4), dev(C)
+    S = h.hdc_similarity(Hd, Cd, kn).cpu().numpy()
+    lab, best, sec = h.hdc_classify(Hd, Cd, kn, want_scores=True)
+    lab = lab.cpu().numpy()
+    if hv_bits in (18, 8, 1):
+        assert np.allclose(S, S_or, rtol=1e-6, atol=1e-9)
+        assert np.array_equal(lab, lab_or)
+        assert np.allclose(best.cpu().numpy(), best_or, rtol=1e-6, atol=1e-9)
+        assert np.allclose(sec.cpu().numpy(), sec_or, rtol=1e-6, atol=1e-9)
+    else:
+        check_scores(S, S_or, 1e-6)
+        check_labels_float(lab, S_or, O.SIM_COS)
+
+
 def test_classify_ties_go_to_lowest_index(hd, h):
     r = rng(6)
     N, K, D = 90, 9, 640
