@@ -251,7 +251,7 @@ int encode_rp_core(hdc_ctx* h, const void* X, int x_dtype, int64_t N, int F, int
       ce = launch_split2_f16(X, xk, N, F, ldx, (__half*)pl.Xs, pl.Fp, pl.ex, st, &h->launches);
       if (ce != cudaSuccess) return cuda_fail(h, ce, "split X");
       TcOperands o{pl.Xs, pl.Ps, OPK_F16, pl.ldxs, pl.ldps, pl.ldxs, pl.ldps, pl.Fp, 3,
-                   SPLIT2_A_SEGS, SPLIT2_B_SEGS, pl.Fp};
+                   SPLIT2_A_SEGS, SPLIT2_B_SEGS, pl.Fp, F};
       int rc = contract_tc(o, "encode_rp fp32 (2 x fp16) tcgen05");
       if (rc == HDC_OK && want_raw) {
         ce = launch_unscale_raw((float*)Hraw, N, D_eff, ldraw, pl.ex, pl.ep, st, &h->launches);
@@ -269,7 +269,7 @@ int encode_rp_core(hdc_ctx* h, const void* X, int x_dtype, int64_t N, int F, int
       ce = launch_split3_bf16(X, xk, N, F, ldx, (__nv_bfloat16*)pl.Xs, pl.Fp, st, &h->launches);
       if (ce != cudaSuccess) return cuda_fail(h, ce, "split X");
       TcOperands o{pl.Xs, pl.Ps, OPK_BF16, pl.ldxs, pl.ldps, pl.ldxs, pl.ldps, pl.Fp, 6,
-                   SPLIT_A_SEGS, SPLIT_B_SEGS, pl.Fp};
+                   SPLIT_A_SEGS, SPLIT_B_SEGS, pl.Fp, F};
       int rc = contract_tc(o, "encode_rp fp32 tcgen05");
       if (rc <= 0) return rc;
     }

@@ -99,6 +99,8 @@ struct TcOperands {
   int nseg;
   uint32_t a_segs, b_segs;
   int seg_stride;
+  int Kvalid;  // 0 = Kr; else: columns >= Kvalid of every segment are known to be zero (staged padding), so the MMAs
+               // of the last k-block that would only read them are not issued
 };
 // cta_group: 1 / 2 force the 1-CTA / CTA-pair kernel, anything else chooses by problem size
 cudaError_t launch_gemm_tc(TcContext* tc, const TcOperands& o, int64_t M, int Nc, const Epilogue& e,

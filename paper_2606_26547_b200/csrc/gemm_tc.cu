@@ -117,6 +117,7 @@ struct TcParams {
   int Nc;
   int m_tiles, n_tiles;
   int nseg, nkb_seg;            // number of reduction segments, k-blocks per segment
+  int nk_last;                  // MMAs (32 bytes of the reduction axis each) the last k-block of a segment needs: 1..4
   uint32_t a_segs, b_segs;      // 4 bits per segment: which operand segment it reads
   int seg_stride;               // elements between operand segments
   int group_m;                  // m-tiles per rasterisation group (EPI_SIGN / EPI_SCORE)
@@ -285,15 +286,29 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
       mbar_wait(tempty_bar(acc), acc_phase ^ 1u);
       tc_fence_after();
       const uint32_t d_tmem = tmem_base + (uint32_t)(acc * BN);
+      int jseg = 0;   // k-block within its segment
       for (int kb = 0; kb < num_kb; ++kb) {
         mbar_wait(full_bar(stage), phase);
         tc_fence_after();
         {  // whole warp, converged: each call issues once (tc_ptx.cuh, *_elect)
           const uint32_t sa = base + stage * STAGE_BYTES;
           const uint64_t da = smem_desc(sa), db = smem_desc(sa + A_BYTES);
+          // the last k-block of a segment: only the MMAs that reach valid columns (F = 617 bf16: 3 of 4, i.e. 39
+          // instead of 40 MMAs per segment)
+          int nk = KB_BYTES / 32;
+          if (++jseg == p.nkb_seg) {
+            jseg = 0;
+            nk = p.nk_last;
+          }
+          if (nk == KB_BYTES / 32) {
 #pragma unroll
-          for (int k = 0; k < KB_BYTES / 32; ++k)
-            tc_mma_elect<INT8, CG>(d_tmem, da + 2u * k, db + 2u * k, idesc, (kb | k) != 0 ? 1u : 0u);
+            for (int k = 0; k < KB_BYTES / 32; ++k)
+              tc_mma_elect<INT8, CG>(d_tmem, da + 2u * k, db + 2u * k, idesc, (kb | k) != 0 ? 1u : 0u);
+          } else {
+#pragma unroll 1
+            for (int k = 0; k < nk; ++k)
+              tc_mma_elect<INT8, CG>(d_tmem, da + 2u * k, db + 2u * k, idesc, (kb | k) != 0 ? 1u : 0u);
+          }
           tc_commit_elect<CG>(empty_bar(stage));            // frees the smem slot when these MMAs retire
           if (kb == num_kb - 1) tc_commit_elect<CG>(tfull_bar(acc));  // accumulator complete
         }
@@ -667,6 +682,13 @@ cudaError_t launch_gemm_tc(TcContext* tc, const TcOperands& o, int64_t M, int Nc
   p.n_tiles = n_tiles;
   p.nseg = o.nseg;
   p.nkb_seg = (o.Kr + BK - 1) / BK;
+  {
+    const int kv = (o.Kvalid > 0 && o.Kvalid < o.Kr) ? o.Kvalid : o.Kr;
+    const int last = kv - (p.nkb_seg - 1) * BK;                     // valid elements of a segment's last k-block
+    const int per = 32 / (int8 ? 1 : 2);                            // elements per MMA
+    p.nk_last = last <= 0 ? 1 : (last + per - 1) / per;
+    if (p.nk_last > KB_BYTES / 32) p.nk_last = KB_BYTES / 32;
+  }
   p.a_segs = o.a_segs;
   p.b_segs = o.b_segs;
   p.seg_stride = o.seg_stride;
