@@ -644,13 +644,21 @@ __global__ void split_reduce_kernel(const float* __restrict__ partial, int split
   Top2f run = Top2f{NEG_BIG_F, NEG_BIG_F, 0.0f, 0.0f, INT_MAX, INT_MAX};
   constexpr int KU = 8;   // classes whose partial sums are fetched together (independent loads in flight)
   for (int k0 = 0; k0 < K; k0 += KU) {
-    float av[KU];
+    // all splits of the KU classes are fetched before the first add (at most 8 splits: sim_tc_splits): one memory
+    // round trip per KU classes instead of one per (KU classes, split) -- the kernel is nothing but load latency
+    float t[8][KU];
 #pragma unroll
-    for (int j = 0; j < KU; ++j) av[j] = 0.0f;
-    for (int sp = 0; sp < splits; ++sp) {
+    for (int sp = 0; sp < 8; ++sp)
 #pragma unroll
       for (int j = 0; j < KU; ++j)
-        if (k0 + j < K) av[j] = __fadd_rn(av[j], __ldg(partial + ((int64_t)sp * K + k0 + j) * N + n));
+        t[sp][j] = (sp < splits && k0 + j < K) ? __ldg(partial + ((int64_t)sp * K + k0 + j) * N + n) : 0.0f;
+    float av[KU];
+#pragma unroll
+    for (int j = 0; j < KU; ++j) {
+      av[j] = t[0][j];
+#pragma unroll
+      for (int sp = 1; sp < 8; ++sp)
+        if (sp < splits) av[j] = __fadd_rn(av[j], t[sp][j]);   // split order: deterministic
     }
 #pragma unroll
     for (int j = 0; j < KU; ++j) {
@@ -852,7 +860,7 @@ cudaError_t launch_sim_tc(TcContext* tc, const uint32_t* Hbits, int64_t N, int64
     ce = int8 ? launch_one<true, EPI_SCORE>(tmB, p, 1, ts, grid, st)
               : launch_one<false, EPI_SCORE>(tmB, p, 1, ts, grid, st);
     if (ce != cudaSuccess) return ce;
-    split_reduce_kernel<<<(unsigned)((N + 127) / 128), 128, 0, st>>>(p.partial, p.splits, N, K, e);
+    split_reduce_kernel<<<(unsigned)((N + 63) / 64), 64, 0, st>>>(p.partial, p.splits, N, K, e);
     ++*nlaunch;
     return cudaGetLastError();
   }
