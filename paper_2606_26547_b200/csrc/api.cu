@@ -447,33 +447,11 @@ int do_similarity(hdc_ctx* h, const uint32_t* Hbits, int64_t N, int64_t ldh, con
     }
     float* amax = pm.take<float>(1);
     void* cop = pm.take<uint8_t>(sim_tc_operand_bytes(K, k->hv_bits, D_eff));
-    int8_t* Cq = nullptr;
-    const int64_t ldq = round_up(D_eff, 16);
-    if (colscale && k->hv_bits == 8) Cq = pm.take<int8_t>((size_t)K * ldq);
-    if (colscale && k->hv_bits == HDC_HV_I16) Cq = pm.take<int8_t>((size_t)K * ldq * 2);   // int16 codes
     const size_t pbytes = sim_tc_partial_bytes(N, K, k->hv_bits, D_eff, h->sm_count);
     double* partial = pbytes ? b.take<double>(pbytes / sizeof(double)) : nullptr;
     if (!persistent_fits(h, b, ws_bytes)) return too_small();
-    if (colscale && prep) {
-      // norms over the operand as the contraction sees it (permutation-invariant)
-      if (k->hv_bits == 8) {
-        ce = launch_quantize_tensor_i8(C_acc, K, D_eff, ldc, pf, Cq, ldq, amax, st, &h->launches);
-        if (ce != cudaSuccess) return cuda_fail(h, ce, "quantize C");
-        ce = launch_col_scale(Operand{Cq, ldq, OPK_I8}, K, D_eff, 1, pf, colscale, st, &h->launches, colscale_f);
-      } else if (k->hv_bits == HDC_HV_I16) {
-        int16_t* Cq16 = reinterpret_cast<int16_t*>(Cq);
-        ce = launch_quantize_tensor_i16(C_acc, K, D_eff, ldc, pf, Cq16, ldq, amax, st, &h->launches);
-        if (ce != cudaSuccess) return cuda_fail(h, ce, "quantize C");
-        ce = launch_col_scale(Operand{Cq16, ldq, OPK_I16}, K, D_eff, 1, pf, colscale, st, &h->launches, colscale_f);
-      } else {
-        const int ck = k->hv_bits == 32   ? OPK_F32
-                       : k->hv_bits == 16 ? OPK_F32_RBF16
-                       : k->hv_bits == HDC_HV_F16 ? OPK_F32_RF16
-                                                  : OPK_BITS;
-        ce = launch_col_scale(Operand{C_acc, ldc, ck}, K, D_eff, 1, pf, colscale, st, &h->launches, colscale_f);
-      }
-      if (ce != cudaSuccess) return cuda_fail(h, ce, "col_scale");
-    }
+    // (the cosine scales -- norms over the operand as the contraction sees it -- are written by the kernel that
+    // stages the class operand, inside launch_sim_tc)
     Epilogue e{};
     e.colscale = colscale;
     e.colscale_f = colscale_f;

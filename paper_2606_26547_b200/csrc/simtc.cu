@@ -25,7 +25,7 @@
 // Reduction-axis permutation.  A sum over d is invariant under any permutation of d applied to both
 // operands, so the k-block position kappa <-> dimension map is chosen to make the expansion two or
 // three ALU ops per 32-bit shared-memory word (perm_bf16 / perm_i8 below); the class operand is
-// staged once per call in the same order by class_operand_kernel (it is tiny: K x D_eff).
+// staged once per call in the same order by class_prepare_kernel (it is tiny: K x D_eff).
 //
 // Class operand precisions (S5): bf16 (hv_bits 16); fp32 (hv_bits 32) as three bf16 parts
 // c1+c2+c3 stacked along the class axis of one tile -- the three partial accumulators are summed in
@@ -569,66 +569,117 @@ __device__ __forceinline__ int quant_i8_c(float x, float s) {
   return (int)q;
 }
 
+// One block per (padded) class: writes the class's nparts staged rows and, in the same pass, what the epilogue
+// needs of it -- the cosine scale colscale[k] = 1 / (sqrt(n_vis) * |operand row|) (0 for a zero row; double, and
+// rounded to fp32 in colscale_f; both nullable = no cosine) and, for the int8 kinds, the integer sum of every staged
+// row (rowsum, see the expanders of sim_tc_kernel).  Fixed reduction order: thread-strided partial sums, then a
+// shuffle / shared-memory tree (deterministic).  The norm is taken over the operand as the contraction sees it:
+// the fp32 value (its three parts add up to it exactly), the rounded bf16 / half value, the integer code, +-1.
+// FP64 instructions retire at ~1 per 53 cycles and SM on this part, and a DFMA per element made this kernel (and
+// col_scale_kernel before it) 9 us of a 55 us retraining epoch: the per-thread partial sums are exact integers for
+// the integer kinds and fp32 for the float kinds (<= 40 terms per thread at D = 10^4: ~1e-7 relative, inside the
+// float paths' tolerance); the 1024 partials are added in double.
+constexpr int CP_THREADS = 1024;   // (the kernel is a chain of load latencies: many short chains)
 template <bool INT8>
-__global__ void class_operand_kernel(const float* __restrict__ C, int K, int D_eff, int64_t ldc, int mode,
-                                     int kc, int nparts, int rows_total, int num_kb,
-                                     const float* __restrict__ amax, Perf pf, void* __restrict__ dst,
-                                     int32_t* __restrict__ rowsum) {
+__global__ void __launch_bounds__(CP_THREADS)
+class_prepare_kernel(const float* __restrict__ C, int K, int D_eff, int64_t ldc, int mode, int kc, int nparts,
+                     int num_kb, const float* __restrict__ amax, Perf pf, int n_vis, void* __restrict__ dst,
+                     int32_t* __restrict__ rowsum, double* __restrict__ colscale, float* __restrict__ colscale_f) {
   constexpr int BK = INT8 ? 128 : 64;
-  const int64_t ld = (int64_t)num_kb * BK;
-  const int64_t total = (int64_t)rows_total * ld;
+  const int ld = num_kb * BK;
+  const int k = blockIdx.x;                                   // class (rows k >= K are zero padding)
+  const int64_t r0 = (int64_t)(k / kc) * (nparts * kc) + k % kc;   // staged row of part 0; part p: + p * kc
   float s = 1.0f;
   if (mode == 8 || mode == HDC_HV_I16) {
     const float a = *amax;
     s = a > 0.0f ? __fdiv_rn(mode == 8 ? 127.0f : 32767.0f, a) : 1.0f;
   }
-  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < total;
-       i += (int64_t)gridDim.x * blockDim.x) {
-    const int r = (int)(i / ld);
-    const int col = (int)(i - (int64_t)r * ld);
-    const int rem = r % (nparts * kc);
-    const int part = rem / kc;
-    const int k = (r / (nparts * kc)) * kc + rem % kc;
+  float nrm2f = 0.0f;                // float kinds
+  unsigned long long nrm2i = 0ull;   // integer kinds: exact
+  int sum0 = 0, sum1 = 0, sum2 = 0;
+#pragma unroll 4
+  for (int col = threadIdx.x; col < ld; col += CP_THREADS) {
     const int kb = col / BK, kappa = col % BK;
     const int d = kb * BK + (INT8 ? perm_i8(kappa) : perm_bf16(kappa));
-    float x = 0.0f;
     const bool live = k < K && d < D_eff && perf_visits(pf, d);  // unvisited dimensions contribute 0
-    if (live) x = __ldg(C + (int64_t)k * ldc + d);
+    const float x = live ? __ldg(C + (int64_t)k * ldc + d) : 0.0f;
     if (INT8) {
-      int qv = 0;
-      if (live) {
-        if (mode == 8) {
-          qv = quant_i8_c(x, s);
-        } else if (mode == HDC_HV_I16) {
-          const int q = (int)fminf(fmaxf(rintf(__fmul_rn(x, s)), -32767.0f), 32767.0f);
-          const int d0 = ((q + 64) & 127) - 64;
-          const int r1 = (q - d0) >> 7;                  // exact: q - d0 is a multiple of 128
-          const int d1 = ((r1 + 64) & 127) - 64;
-          qv = part == 0 ? (r1 - d1) >> 7 : (part == 1 ? d1 : d0);
-        } else {
-          qv = x < 0.0f ? -1 : 1;
-        }
+      int8_t* o = reinterpret_cast<int8_t*>(dst) + r0 * ld + col;
+      if (mode == HDC_HV_I16) {
+        const int q = live ? (int)fminf(fmaxf(rintf(__fmul_rn(x, s)), -32767.0f), 32767.0f) : 0;
+        const int d0 = ((q + 64) & 127) - 64;
+        const int r1 = (q - d0) >> 7;                  // exact: q - d0 is a multiple of 128
+        const int d1 = ((r1 + 64) & 127) - 64;
+        const int d2 = (r1 - d1) >> 7;
+        o[0] = (int8_t)d2;
+        o[(int64_t)kc * ld] = (int8_t)d1;
+        o[(int64_t)2 * kc * ld] = (int8_t)d0;
+        sum0 += d2; sum1 += d1; sum2 += d0;
+        nrm2i += (unsigned long long)(q * q);
+      } else {
+        const int qv = !live ? 0 : (mode == 8 ? quant_i8_c(x, s) : (x < 0.0f ? -1 : 1));
+        o[0] = (int8_t)qv;
+        sum0 += qv;
+        nrm2i += (unsigned long long)(qv * qv);
       }
-      reinterpret_cast<int8_t*>(dst)[i] = (int8_t)qv;
-      // row sums (zeroed by the launcher): the 32 elements of a warp's step lie in one staged row (ld % 128 == 0,
-      // total % 32 == 0), integer atomics: deterministic
-      int sum = qv;
-#pragma unroll
-      for (int off = 16; off; off >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, off);
-      if ((threadIdx.x & 31) == 0 && sum != 0) atomicAdd(rowsum + r, sum);
     } else if (mode == HDC_HV_F16) {
-      reinterpret_cast<__half*>(dst)[i] = __float2half_rn(x);
+      const __half hv = __float2half_rn(x);
+      reinterpret_cast<__half*>(dst)[r0 * ld + col] = hv;
+      const float v = __half2float(hv);
+      nrm2f = __fmaf_rn(v, v, nrm2f);
     } else {
-      __nv_bfloat16 b1 = __float2bfloat16_rn(x);
-      if (mode == 32 && part > 0) {
+      __nv_bfloat16* o = reinterpret_cast<__nv_bfloat16*>(dst) + r0 * ld + col;
+      const __nv_bfloat16 b1 = __float2bfloat16_rn(x);
+      o[0] = b1;
+      float v = __bfloat162float(b1);
+      if (mode == 32) {
         const float r1 = __fsub_rn(x, __bfloat162float(b1));
-        b1 = __float2bfloat16_rn(r1);
-        if (part > 1) {
-          const float r2 = __fsub_rn(r1, __bfloat162float(b1));
-          b1 = __float2bfloat16_rn(r2);
-        }
+        const __nv_bfloat16 b2 = __float2bfloat16_rn(r1);
+        const float r2 = __fsub_rn(r1, __bfloat162float(b2));
+        o[(int64_t)kc * ld] = b2;
+        o[(int64_t)2 * kc * ld] = __float2bfloat16_rn(r2);
+        v = x;
       }
-      reinterpret_cast<__nv_bfloat16*>(dst)[i] = b1;
+      nrm2f = __fmaf_rn(v, v, nrm2f);
+    }
+  }
+  double nrm2 = INT8 ? (double)nrm2i : (double)nrm2f;   // (integers below 2^53: exact)
+  __shared__ double sh_n[CP_THREADS / 32];
+  __shared__ int sh_s[3][CP_THREADS / 32];
+#pragma unroll
+  for (int off = 16; off; off >>= 1) {
+    nrm2 += __shfl_xor_sync(0xffffffffu, nrm2, off);
+    if (INT8) {
+      sum0 += __shfl_xor_sync(0xffffffffu, sum0, off);
+      sum1 += __shfl_xor_sync(0xffffffffu, sum1, off);
+      sum2 += __shfl_xor_sync(0xffffffffu, sum2, off);
+    }
+  }
+  const int warp = threadIdx.x >> 5;
+  if ((threadIdx.x & 31) == 0) {
+    sh_n[warp] = nrm2;
+    sh_s[0][warp] = sum0; sh_s[1][warp] = sum1; sh_s[2][warp] = sum2;
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double t = 0.0;
+    int t0 = 0, t1 = 0, t2 = 0;
+    for (int i = 0; i < CP_THREADS / 32; ++i) {
+      t += sh_n[i];
+      t0 += sh_s[0][i]; t1 += sh_s[1][i]; t2 += sh_s[2][i];
+    }
+    if (INT8) {
+      rowsum[r0] = t0;
+      if (nparts == 3) {
+        rowsum[r0 + kc] = t1;
+        rowsum[r0 + 2 * kc] = t2;
+      }
+    }
+    if (colscale && k < K) {
+      const double nrm = sqrt(t);
+      const double cs = nrm > 0.0 ? 1.0 / (sqrt((double)n_vis) * nrm) : 0.0;
+      colscale[k] = cs;
+      if (colscale_f) colscale_f[k] = (float)cs;
     }
   }
 }
@@ -637,18 +688,19 @@ __global__ void class_operand_kernel(const float* __restrict__ C, int K, int D_e
 // sim_tc_kernel: scores (S) or arg-max with best / runner-up, with the same fp32 comparison + exact double
 // tie-break.  One thread per query row; [split][class][query] layout: coalesced.  int_acc: the partial sums are
 // integers (exact in fp32 below 2^24, which sim_tc_splits guarantees).
+template <int SU>   // SU >= splits: 2, 4 or 8
 __global__ void split_reduce_kernel(const float* __restrict__ partial, int splits, int64_t N, int K, Epilogue e) {
   const int64_t n = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (n >= N) return;
   const bool scaled = e.colscale != nullptr;
   Top2f run = Top2f{NEG_BIG_F, NEG_BIG_F, 0.0f, 0.0f, INT_MAX, INT_MAX};
-  constexpr int KU = 8;   // classes whose partial sums are fetched together (independent loads in flight)
+  constexpr int KU = 64 / SU;   // classes whose partial sums are fetched together (64 independent loads in flight)
   for (int k0 = 0; k0 < K; k0 += KU) {
     // all splits of the KU classes are fetched before the first add (at most 8 splits: sim_tc_splits): one memory
     // round trip per KU classes instead of one per (KU classes, split) -- the kernel is nothing but load latency
-    float t[8][KU];
+    float t[SU][KU];
 #pragma unroll
-    for (int sp = 0; sp < 8; ++sp)
+    for (int sp = 0; sp < SU; ++sp)
 #pragma unroll
       for (int j = 0; j < KU; ++j)
         t[sp][j] = (sp < splits && k0 + j < K) ? __ldg(partial + ((int64_t)sp * K + k0 + j) * N + n) : 0.0f;
@@ -657,7 +709,7 @@ __global__ void split_reduce_kernel(const float* __restrict__ partial, int split
     for (int j = 0; j < KU; ++j) {
       av[j] = t[0][j];
 #pragma unroll
-      for (int sp = 1; sp < 8; ++sp)
+      for (int sp = 1; sp < SU; ++sp)
         if (sp < splits) av[j] = __fadd_rn(av[j], t[sp][j]);   // split order: deterministic
     }
 #pragma unroll
@@ -800,18 +852,17 @@ cudaError_t launch_sim_tc(TcContext* tc, const uint32_t* Hbits, int64_t N, int64
   }
   int32_t* rowsum = int8 ? reinterpret_cast<int32_t*>(static_cast<char*>(cop) + (size_t)rows_total * ld) : nullptr;
   if (!cop_ready) {
-    const int64_t total = (int64_t)rows_total * ld;
-    int64_t g = (total + 255) / 256;
-    if (g > (int64_t)sm_count * 16) g = (int64_t)sm_count * 16;
-    if (int8) {
-      ce = cudaMemsetAsync(rowsum, 0, (size_t)rows_total * 4, st);
-      if (ce != cudaSuccess) return ce;
-      class_operand_kernel<true><<<(unsigned)g, 256, 0, st>>>(C_acc, K, D_eff, ldc, hv_bits, kc, nparts, rows_total,
-                                                             num_kb, amax_scratch, pf, cop, rowsum);
-    } else {
-      class_operand_kernel<false><<<(unsigned)g, 256, 0, st>>>(C_acc, K, D_eff, ldc, hv_bits, kc, nparts,
-                                                              rows_total, num_kb, amax_scratch, pf, cop, nullptr);
-    }
+    const int n_vis = perf_count(pf, D_eff);
+    // (the scales are the caller's e.colscale / e.colscale_f: written here, read by the kernels below)
+    double* cs = const_cast<double*>(e.colscale);
+    float* csf = const_cast<float*>(e.colscale_f);
+    if (int8)
+      class_prepare_kernel<true><<<(unsigned)(n_tiles * kc), CP_THREADS, 0, st>>>(C_acc, K, D_eff, ldc, hv_bits, kc, nparts, num_kb,
+                                                                          amax_scratch, pf, n_vis, cop, rowsum, cs, csf);
+    else
+      class_prepare_kernel<false><<<(unsigned)(n_tiles * kc), CP_THREADS, 0, st>>>(C_acc, K, D_eff, ldc, hv_bits, kc, nparts,
+                                                                           num_kb, amax_scratch, pf, n_vis, cop, nullptr, cs,
+                                                                           csf);
     ++*nlaunch;
     ce = cudaGetLastError();
     if (ce != cudaSuccess) return ce;
@@ -860,7 +911,10 @@ cudaError_t launch_sim_tc(TcContext* tc, const uint32_t* Hbits, int64_t N, int64
     ce = int8 ? launch_one<true, EPI_SCORE>(tmB, p, 1, ts, grid, st)
               : launch_one<false, EPI_SCORE>(tmB, p, 1, ts, grid, st);
     if (ce != cudaSuccess) return ce;
-    split_reduce_kernel<<<(unsigned)((N + 63) / 64), 64, 0, st>>>(p.partial, p.splits, N, K, e);
+    const unsigned rg = (unsigned)((N + 63) / 64);
+    if (p.splits <= 2) split_reduce_kernel<2><<<rg, 64, 0, st>>>(p.partial, p.splits, N, K, e);
+    else if (p.splits <= 4) split_reduce_kernel<4><<<rg, 64, 0, st>>>(p.partial, p.splits, N, K, e);
+    else split_reduce_kernel<8><<<rg, 64, 0, st>>>(p.partial, p.splits, N, K, e);
     ++*nlaunch;
     return cudaGetLastError();
   }
