@@ -733,7 +733,7 @@ size_t infer_ws_bytes(const hdc_ctx* h, int64_t N, int F, int K, const hdc_knobs
 using namespace hdc;
 
 // =================================================================================== handle
-extern "C" int32_t hdc_version(void) { return 103; }  // 1.3: + hdc_infer_rp (fused inference), hdc_stat
+extern "C" int32_t hdc_version(void) { return 104; }  // 1.4: + HDC_HV_I16, hdc_classify_hamming_static
 
 extern "C" int32_t hdc_create(hdc_handle_t* out, int32_t device) {
   if (!out) return HDC_ERR_INVALID_ARG;
