@@ -34,7 +34,7 @@ __device__ __forceinline__ void csa(uint32_t& hi, uint32_t& lo, uint32_t a, uint
   hi = (a & b) | ((a ^ b) & c);
 }
 
-constexpr int NST = 3;                      // cp.async ring depth
+constexpr int NST = 2;                      // cp.async ring depth
 constexpr int HQ_WORDS = WC * (QT + 1);     // transposed query tile, stride QT+1: conflict-free
 __host__ __device__ constexpr int stage_words(int KC) { return HQ_WORDS + (KC + 1) * WC; }  // + mask row
 
