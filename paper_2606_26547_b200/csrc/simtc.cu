@@ -241,11 +241,11 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
         for (int u = 0; u < n; ++u) {
           const uint32_t sa = base + (grp * G + u) * STAGE_BYTES;
           if constexpr (TS) {
-            const uint64_t db = smem_desc(sa);
+            // (16..128-column MMAs take 8..64 tensor cycles: the issue sequence sets the pace, so the four MMAs of
+            // a k-block go out of one asm block with one election and 32-bit descriptor arithmetic)
+            const uint32_t b_lo = ((sa & 0x3FFFFu) >> 4) | (1u << 16);   // lower half of smem_desc(sa)
             const uint32_t at = tmem_base + (uint32_t)(TS_A_COL0 + (grp * G + u) * 32);
-#pragma unroll
-            for (int k = 0; k < KB_BYTES / 32; ++k)
-              tc_mma_ts_elect<INT8>(d_tmem, at + 8u * k, db + 2u * k, idesc, (kb0 + u != kb_lo || k != 0) ? 1u : 0u);
+            tc_mma_ts_kblock_elect<INT8>(d_tmem, at, b_lo, idesc, kb0 + u != kb_lo ? 1u : 0u);
           } else {
             const uint64_t da = smem_desc(sa), db = smem_desc(sa + A_BYTES);
 #pragma unroll

@@ -232,6 +232,31 @@ __device__ __forceinline__ void tc_mma_ts_elect(uint32_t d_tmem, uint32_t a_tmem
   else HDC_MMA_TS_ELECT("f16");
 }
 #undef HDC_MMA_TS_ELECT
+// The four MMAs of one k-block (4 x 32 bytes of the reduction axis) in one block: one election, the descriptors of
+// the class tile built from the 32-bit address field (the upper half of a 128-byte-swizzled K-major descriptor is the
+// constant 0x40004040: SBO 1024, version 1, SWIZZLE_128B), A advancing 8 TMEM columns per MMA.  b_lo = lower half of
+// smem_desc() of the k-block; first == 0: the first MMA overwrites the accumulator.
+#define HDC_MMA_TS_KB(KIND)                                                                             \
+  asm volatile(                                                                                         \
+      "{\n\t.reg .pred p, q;\n\t.reg .b64 d0, d1, d2, d3;\n\t.reg .b32 l1, l2, l3, a1, a2, a3;\n\t"        \
+      "elect.sync _|q, 0xffffffff;\n\tsetp.ne.b32 p, %4, 0;\n\t"                                         \
+      "add.u32 l1, %2, 2;\n\tadd.u32 l2, %2, 4;\n\tadd.u32 l3, %2, 6;\n\t"                              \
+      "add.u32 a1, %1, 8;\n\tadd.u32 a2, %1, 16;\n\tadd.u32 a3, %1, 24;\n\t"                            \
+      "mov.b64 d0, {%2, 0x40004040};\n\tmov.b64 d1, {l1, 0x40004040};\n\t"                              \
+      "mov.b64 d2, {l2, 0x40004040};\n\tmov.b64 d3, {l3, 0x40004040};\n\t"                              \
+      "@q tcgen05.mma.cta_group::1.kind::" KIND " [%0], [%1], d0, %3, p;\n\t"                            \
+      "@q tcgen05.mma.cta_group::1.kind::" KIND " [%0], [a1], d1, %3, 1;\n\t"                            \
+      "@q tcgen05.mma.cta_group::1.kind::" KIND " [%0], [a2], d2, %3, 1;\n\t"                            \
+      "@q tcgen05.mma.cta_group::1.kind::" KIND " [%0], [a3], d3, %3, 1;\n\t}" ::"r"(d_tmem),            \
+      "r"(a_tmem), "r"(b_lo), "r"(idesc), "r"(first)                                                   \
+      : "memory")
+template <bool INT8>
+__device__ __forceinline__ void tc_mma_ts_kblock_elect(uint32_t d_tmem, uint32_t a_tmem, uint32_t b_lo, uint32_t idesc,
+                                                       uint32_t first) {
+  if (INT8) HDC_MMA_TS_KB("i8");
+  else HDC_MMA_TS_KB("f16");
+}
+#undef HDC_MMA_TS_KB
 // 32 lanes x 16 consecutive 32-bit columns, registers -> tensor memory: thread t of the warp writes lane (base + t)
 __device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t (&v)[16]) {
   asm volatile(
