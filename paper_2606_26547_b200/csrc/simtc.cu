@@ -238,6 +238,12 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
         mbar_wait(full_bar(grp), phase);
         tc_fence_after();
         // whole warp, converged: each call issues once (tc_ptx.cuh, *_elect)
+        if (TS && n == 4 && G == 4) {
+          const uint32_t sa = base + (grp * G) * STAGE_BYTES;
+          tc_mma_ts_group_elect<INT8>(d_tmem, tmem_base + (uint32_t)(TS_A_COL0 + grp * G * 32),
+                                      ((sa & 0x3FFFFu) >> 4) | (1u << 16), (STAGE_BYTES >> 4) - 6u, idesc,
+                                      kb0 != kb_lo ? 1u : 0u);
+        } else
         for (int u = 0; u < n; ++u) {
           const uint32_t sa = base + (grp * G + u) * STAGE_BYTES;
           if constexpr (TS) {

@@ -257,6 +257,69 @@ __device__ __forceinline__ void tc_mma_ts_kblock_elect(uint32_t d_tmem, uint32_t
   else HDC_MMA_TS_KB("f16");
 }
 #undef HDC_MMA_TS_KB
+// A whole group of four k-blocks (16 MMAs) in one block.  b_step = (bytes between the class tiles of consecutive
+// k-blocks) / 16 - 6: what takes the descriptor address field from the last MMA of a k-block to the first of the next.
+#define HDC_MMA_TS_GROUP(KIND)                                                                          \
+  asm volatile(                                                                                         \
+      "{\n\t.reg .pred p, q;\n\t.reg .b64 d;\n\t.reg .b32 lo, a;\n\t" \
+      "elect.sync _|q, 0xffffffff;\n\tsetp.ne.b32 p, %5, 0;\n\t" \
+      "mov.b32 lo, %2;\n\tmov.b32 a, %1;\n\t" \
+      "mov.b64 d, {lo, 0x40004040};\n\t" \
+      "@q tcgen05.mma.cta_group::1.kind::" KIND " [%0], [a], d, %4, p;\n\t" \
+      "add.u32 lo, lo, 2;\n\tadd.u32 a, a, 8;\n\t" \
+      "mov.b64 d, {lo, 0x40004040};\n\t" \
+      "@q tcgen05.mma.cta_group::1.kind::" KIND " [%0], [a], d, %4, 1;\n\t" \
+      "add.u32 lo, lo, 2;\n\tadd.u32 a, a, 8;\n\t" \
+      "mov.b64 d, {lo, 0x40004040};\n\t" \
+      "@q tcgen05.mma.cta_group::1.kind::" KIND " [%0], [a], d, %4, 1;\n\t" \
+      "add.u32 lo, lo, 2;\n\tadd.u32 a, a, 8;\n\t" \
+      "mov.b64 d, {lo, 0x40004040};\n\t" \
+      "@q tcgen05.mma.cta_group::1.kind::" KIND " [%0], [a], d, %4, 1;\n\t" \
+      "add.u32 lo, lo, %3;\n\tadd.u32 a, a, 8;\n\t" \
+      "mov.b64 d, {lo, 0x40004040};\n\t" \
+      "@q tcgen05.mma.cta_group::1.kind::" KIND " [%0], [a], d, %4, 1;\n\t" \
+      "add.u32 lo, lo, 2;\n\tadd.u32 a, a, 8;\n\t" \
+      "mov.b64 d, {lo, 0x40004040};\n\t" \
+      "@q tcgen05.mma.cta_group::1.kind::" KIND " [%0], [a], d, %4, 1;\n\t" \
+      "add.u32 lo, lo, 2;\n\tadd.u32 a, a, 8;\n\t" \
+      "mov.b64 d, {lo, 0x40004040};\n\t" \
+      "@q tcgen05.mma.cta_group::1.kind::" KIND " [%0], [a], d, %4, 1;\n\t" \
+      "add.u32 lo, lo, 2;\n\tadd.u32 a, a, 8;\n\t" \
+      "mov.b64 d, {lo, 0x40004040};\n\t" \
+      "@q tcgen05.mma.cta_group::1.kind::" KIND " [%0], [a], d, %4, 1;\n\t" \
+      "add.u32 lo, lo, %3;\n\tadd.u32 a, a, 8;\n\t" \
+      "mov.b64 d, {lo, 0x40004040};\n\t" \
+      "@q tcgen05.mma.cta_group::1.kind::" KIND " [%0], [a], d, %4, 1;\n\t" \
+      "add.u32 lo, lo, 2;\n\tadd.u32 a, a, 8;\n\t" \
+      "mov.b64 d, {lo, 0x40004040};\n\t" \
+      "@q tcgen05.mma.cta_group::1.kind::" KIND " [%0], [a], d, %4, 1;\n\t" \
+      "add.u32 lo, lo, 2;\n\tadd.u32 a, a, 8;\n\t" \
+      "mov.b64 d, {lo, 0x40004040};\n\t" \
+      "@q tcgen05.mma.cta_group::1.kind::" KIND " [%0], [a], d, %4, 1;\n\t" \
+      "add.u32 lo, lo, 2;\n\tadd.u32 a, a, 8;\n\t" \
+      "mov.b64 d, {lo, 0x40004040};\n\t" \
+      "@q tcgen05.mma.cta_group::1.kind::" KIND " [%0], [a], d, %4, 1;\n\t" \
+      "add.u32 lo, lo, %3;\n\tadd.u32 a, a, 8;\n\t" \
+      "mov.b64 d, {lo, 0x40004040};\n\t" \
+      "@q tcgen05.mma.cta_group::1.kind::" KIND " [%0], [a], d, %4, 1;\n\t" \
+      "add.u32 lo, lo, 2;\n\tadd.u32 a, a, 8;\n\t" \
+      "mov.b64 d, {lo, 0x40004040};\n\t" \
+      "@q tcgen05.mma.cta_group::1.kind::" KIND " [%0], [a], d, %4, 1;\n\t" \
+      "add.u32 lo, lo, 2;\n\tadd.u32 a, a, 8;\n\t" \
+      "mov.b64 d, {lo, 0x40004040};\n\t" \
+      "@q tcgen05.mma.cta_group::1.kind::" KIND " [%0], [a], d, %4, 1;\n\t" \
+      "add.u32 lo, lo, 2;\n\tadd.u32 a, a, 8;\n\t" \
+      "mov.b64 d, {lo, 0x40004040};\n\t" \
+      "@q tcgen05.mma.cta_group::1.kind::" KIND " [%0], [a], d, %4, 1;\n\t" \
+      "}" ::"r"(d_tmem), "r"(a_tmem), "r"(b_lo), "r"(b_step), "r"(idesc), "r"(first)           \
+      : "memory")
+template <bool INT8>
+__device__ __forceinline__ void tc_mma_ts_group_elect(uint32_t d_tmem, uint32_t a_tmem, uint32_t b_lo, uint32_t b_step,
+                                                      uint32_t idesc, uint32_t first) {
+  if (INT8) HDC_MMA_TS_GROUP("i8");
+  else HDC_MMA_TS_GROUP("f16");
+}
+#undef HDC_MMA_TS_GROUP
 // 32 lanes x 16 consecutive 32-bit columns, registers -> tensor memory: thread t of the warp writes lane (base + t)
 __device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t (&v)[16]) {
   asm volatile(
