@@ -139,8 +139,12 @@ def _kernel(h, kid, fn, reps):
 
 
 def _rand_bits(n, w, name):
-    """[n][w] packed words of iid uniform bits from the seeded stream (0, name)."""
-    return _dev(gen.rng_for(0, name).integers(0, 2 ** 32, size=(n, w), dtype=np.uint32).view(np.int32))
+    """[n][w] packed words of iid uniform bits from the seeded stream (0, name), in rows of w rounded up to 4 words
+    (16-byte aligned rows: the layout Handle.alloc_hbits gives the hypervectors hdc_encode_* write)."""
+    ld = (w + 3) // 4 * 4
+    host = np.zeros((n, ld), dtype=np.uint32)
+    host[:, :w] = gen.rng_for(0, name).integers(0, 2 ** 32, size=(n, w), dtype=np.uint32)
+    return _dev(host.view(np.int32))[:, :w]
 
 
 def _class_acc(K, D, name, per_class=32):

@@ -75,6 +75,19 @@ bool tc_make_map(TcContext* tc, CUtensorMap* out, const void* ptr, bool int8, in
                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
 }
 
+// packed hypervector words [rows][cols] uint32, row stride ld words (ld % 4 == 0, 16-byte aligned base): boxes of
+// 32 words x 128 rows with the 128-byte swizzle (16-byte piece j of row r sits at piece j ^ (r & 7): lane = row
+// reads of one piece are conflict-free); out-of-range words and rows read as zero.
+bool tc_make_map_words(TcContext* tc, CUtensorMap* out, const void* ptr, int64_t rows, int64_t cols, int64_t ld) {
+  cuuint64_t dims[2] = {(cuuint64_t)cols, (cuuint64_t)rows};
+  cuuint64_t strides[1] = {(cuuint64_t)ld * 4};
+  cuuint32_t box[2] = {32, 128};
+  cuuint32_t estr[2] = {1, 1};
+  return CUDA_SUCCESS == tc->encode(out, CU_TENSOR_MAP_DATA_TYPE_UINT32, 2, const_cast<void*>(ptr), dims, strides,
+                                    box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                                    CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+}
+
 // fp32 [rows][cols] row-major, row stride ld elements: un-swizzled boxes of box_cols x box_rows
 static bool tc_make_map_f32(TcContext* tc, CUtensorMap* out, const void* ptr, int64_t rows, int64_t cols, int64_t ld,
                             int box_cols, int box_rows) {

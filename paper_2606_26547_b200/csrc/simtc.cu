@@ -32,6 +32,7 @@
 // the epilogue, so the queries are expanded once; int8 (hv_bits 8) and +-1 int8 (hv_bits 1) with
 // int32 accumulation (exact).
 #include <cuda_fp16.h>
+#include <cstdlib>
 #include <limits.h>
 
 #include <type_traits>
@@ -93,6 +94,9 @@ struct SimParams {
   int stage_bytes;  // A_BYTES + nparts*kc*KB_BYTES
   int f16;          // 16-bit operands are IEEE half instead of bf16 (hv code HDC_HV_F16)
   const int32_t* rowsum;   // INT8: sum of every staged class row (see the expanders), behind the staged operand
+  int acc_cols, acc_bufs;  // sim_ts_kernel: TMEM columns of one accumulator and how many there are
+  int ngroups;             // sim_ts_kernel: groups of 4 k-blocks in flight (class tiles in shared memory, expanded
+                           // queries in tensor memory)
   Epilogue e;
 };
 
@@ -121,6 +125,112 @@ __device__ __forceinline__ uint32_t prmt_sign_bytes(uint32_t v) {
   uint32_t d;
   asm("prmt.b32 %0, %1, %1, 0xBA98;" : "=r"(d) : "r"(v));  // byte b <- 0xFF if msb of byte b of v else 0
   return d;
+}
+
+// Epilogue of one accumulator tile for the query row of this thread (lane = TMEM lane of its warp's quarter): columns
+// [0, k_valid) of the tile at taddr are classes k_base + c of n-tile nt; with nparts == 3 the three parts of class c
+// sit kc columns apart.  sp: split of the reduction axis this CTA reduced (p.splits > 1: partial sums only).
+template <bool INT8, int EPI, bool TS>
+__device__ __forceinline__ void sim_epi_columns(const SimParams& p, uint32_t taddr, int nt, int k_base, int k_valid,
+                                                int64_t row, bool row_ok, int sp, bool scaled, Top2f& run) {
+  for (int c0 = 0; c0 < k_valid; c0 += 16) {
+    uint32_t v0[16], v1[16], v2[16];
+    tmem_ld16(taddr + (uint32_t)c0, v0);
+    if (p.nparts == 3) {
+      tmem_ld16(taddr + (uint32_t)(p.kc + c0), v1);
+      tmem_ld16(taddr + (uint32_t)(2 * p.kc + c0), v2);
+    }
+    tmem_ld_wait();
+#pragma unroll
+    for (int j = 0; j < 16; ++j) {
+      if (c0 + j < k_valid) {
+        const int k = k_base + c0 + j;
+        // the accumulator as a float: exact for the integer paths below 2^24, one rounding for the sum of
+        // the three fp32-class parts
+        float a;
+        int iv = 0;
+        if (INT8) {
+          // TS: the expanders write the query bit b as the byte -128 b (one AND per word) instead of v = 1 - 2 b, so
+          // the accumulator holds -128 sum_{b=1} c and  sum_d v c = sum_d c - 2 sum_{b=1} c = rowsum + (acc >> 6),
+          // exactly (acc is a multiple of 128).  A split of the reduction axis adds the row sum once (split 0).
+          int i0 = (int)v0[j], i1 = (int)v1[j], i2 = (int)v2[j];
+          if constexpr (TS) {   // (wide class tiles keep +-1 bytes: one more load per column costs their epilogue more)
+            const int32_t* rs = p.rowsum + (size_t)nt * p.nparts * p.kc + c0 + j;
+            const bool first = sp == 0;
+            i0 = (i0 >> 6) + (first ? __ldg(rs) : 0);
+            if (p.nparts == 3) {
+              i1 = (i1 >> 6) + (first ? __ldg(rs + p.kc) : 0);
+              i2 = (i2 >> 6) + (first ? __ldg(rs + 2 * p.kc) : 0);
+            }
+          }
+          // int16 class codes: three balanced base-128 digits, most significant first (exact in int32)
+          iv = p.nparts == 3 ? i0 * 16384 + i1 * 128 + i2 : i0;
+          a = (float)iv;
+        } else if (p.nparts == 3) {
+          a = __fadd_rn(__fadd_rn(__uint_as_float(v2[j]), __uint_as_float(v1[j])), __uint_as_float(v0[j]));
+        } else {
+          a = __uint_as_float(v0[j]);
+        }
+        if (p.splits > 1) {
+          // partial sum of this split of the reduction axis; split_reduce_kernel adds the splits
+          // in a fixed order and applies the epilogue
+          if (row_ok) p.partial[((int64_t)sp * p.K + k) * p.N + row] = a;   // [split][class][query]: coalesced
+        } else if (EPI == EPI_SCORE) {
+          if (row_ok) {
+            if (p.e.s_i32) {
+              if (p.e.ham_D > 0) iv = (p.e.ham_D - iv) >> 1;
+              reinterpret_cast<int32_t*>(p.e.S)[row * p.e.lds + k] = iv;
+            } else {
+              reinterpret_cast<float*>(p.e.S)[row * p.e.lds + k] = scaled ? __fmul_rn(a, p.e.colscale_f[k]) : a;
+            }
+          }
+        } else {
+          // classes arrive in increasing order: strict > keeps the lowest index
+          const float sc = scaled ? __fmul_rn(a, p.e.colscale_f[k]) : a;
+          bool better = sc > run.b1;
+          bool second = sc > run.b2;
+          if (scaled && fabsf(sc - run.b1) <= 2.0e-6f * fmaxf(fabsf(sc), fabsf(run.b1)) && run.i1 != INT_MAX) {
+            // too close for fp32: the exact products decide (rare)
+            const double ea = INT8 ? (double)iv : (double)a;
+            const double e1 = INT8 ? (double)__float_as_int(run.a1) : (double)run.a1;
+            better = ea * p.e.colscale[k] > e1 * p.e.colscale[run.i1];
+          }
+          if (INT8 && p.nparts == 3 && !scaled) {
+            // int16 codes: sums beyond 2^24 are not exact as floats, the integers decide
+            better = run.i1 == INT_MAX || iv > __float_as_int(run.a1);
+            second = run.i2 == INT_MAX || iv > __float_as_int(run.a2);
+          }
+          const float araw = INT8 ? __int_as_float(iv) : a;   // integer accumulators are kept bit for bit
+          if (better) {
+            run.b2 = run.b1; run.a2 = run.a1; run.i2 = run.i1;
+            run.b1 = sc; run.a1 = araw; run.i1 = k;
+          } else if (second) {
+            run.b2 = sc; run.a2 = araw; run.i2 = k;
+          }
+        }
+      }
+    }
+  }
+}
+
+// End of a query row's class sweep (EPI_ARGMAX): label, best and runner-up scores.
+template <bool INT8>
+__device__ __forceinline__ void sim_epi_finish(const SimParams& p, int64_t row, bool row_ok, bool scaled, Top2f& run) {
+  if (row_ok) {
+    // reported scores: the exact double products of the two winners (one conversion per row)
+    const double e1 = INT8 ? (double)__float_as_int(run.a1) : (double)run.a1;
+    const double e2 = INT8 ? (double)__float_as_int(run.a2) : (double)run.a2;
+    double b1 = scaled ? e1 * p.e.colscale[run.i1] : e1;
+    double b2 = run.i2 == INT_MAX ? b1 : (scaled ? e2 * p.e.colscale[run.i2] : e2);  // K == 1
+    if (p.e.ham_D > 0) {
+      b1 = 0.5 * ((double)p.e.ham_D - b1);
+      b2 = 0.5 * ((double)p.e.ham_D - b2);
+    }
+    p.e.labels[row] = run.i1;
+    if (p.e.best) p.e.best[row] = (float)b1;
+    if (p.e.second) p.e.second[row] = (float)b2;
+  }
+  run = Top2f{NEG_BIG_F, NEG_BIG_F, 0.0f, 0.0f, INT_MAX, INT_MAX};
 }
 
 // TS: the expanded query tile lives in TENSOR memory instead of shared memory (tcgen05.mma with the A operand in
@@ -291,84 +401,7 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
       const int k_base = nt * p.kc;
       int k_valid = p.K - k_base;
       if (k_valid > p.kc) k_valid = p.kc;
-      for (int c0 = 0; c0 < k_valid; c0 += 16) {
-        uint32_t v0[16], v1[16], v2[16];
-        tmem_ld16(taddr + (uint32_t)c0, v0);
-        if (p.nparts == 3) {
-          tmem_ld16(taddr + (uint32_t)(p.kc + c0), v1);
-          tmem_ld16(taddr + (uint32_t)(2 * p.kc + c0), v2);
-        }
-        tmem_ld_wait();
-#pragma unroll
-        for (int j = 0; j < 16; ++j) {
-          if (c0 + j < k_valid) {
-            const int k = k_base + c0 + j;
-            // the accumulator as a float: exact for the integer paths below 2^24, one rounding for the sum of
-            // the three fp32-class parts
-            float a;
-            int iv = 0;
-            if (INT8) {
-              // TS: the expanders write the query bit b as the byte -128 b (one AND per word) instead of v = 1 - 2 b, so
-              // the accumulator holds -128 sum_{b=1} c and  sum_d v c = sum_d c - 2 sum_{b=1} c = rowsum + (acc >> 6),
-              // exactly (acc is a multiple of 128).  A split of the reduction axis adds the row sum once (split 0).
-              int i0 = (int)v0[j], i1 = (int)v1[j], i2 = (int)v2[j];
-              if constexpr (TS) {   // (wide class tiles keep +-1 bytes: one more load per column costs their epilogue more)
-                const int32_t* rs = p.rowsum + (size_t)nt * p.nparts * p.kc + c0 + j;
-                const bool first = sp == 0;
-                i0 = (i0 >> 6) + (first ? __ldg(rs) : 0);
-                if (p.nparts == 3) {
-                  i1 = (i1 >> 6) + (first ? __ldg(rs + p.kc) : 0);
-                  i2 = (i2 >> 6) + (first ? __ldg(rs + 2 * p.kc) : 0);
-                }
-              }
-              // int16 class codes: three balanced base-128 digits, most significant first (exact in int32)
-              iv = p.nparts == 3 ? i0 * 16384 + i1 * 128 + i2 : i0;
-              a = (float)iv;
-            } else if (p.nparts == 3) {
-              a = __fadd_rn(__fadd_rn(__uint_as_float(v2[j]), __uint_as_float(v1[j])), __uint_as_float(v0[j]));
-            } else {
-              a = __uint_as_float(v0[j]);
-            }
-            if (p.splits > 1) {
-              // partial sum of this split of the reduction axis; split_reduce_kernel adds the splits
-              // in a fixed order and applies the epilogue
-              if (row_ok) p.partial[((int64_t)sp * p.K + k) * p.N + row] = a;   // [split][class][query]: coalesced
-            } else if (EPI == EPI_SCORE) {
-              if (row_ok) {
-                if (p.e.s_i32) {
-                  if (p.e.ham_D > 0) iv = (p.e.ham_D - iv) >> 1;
-                  reinterpret_cast<int32_t*>(p.e.S)[row * p.e.lds + k] = iv;
-                } else {
-                  reinterpret_cast<float*>(p.e.S)[row * p.e.lds + k] = scaled ? __fmul_rn(a, p.e.colscale_f[k]) : a;
-                }
-              }
-            } else {
-              // classes arrive in increasing order: strict > keeps the lowest index
-              const float sc = scaled ? __fmul_rn(a, p.e.colscale_f[k]) : a;
-              bool better = sc > run.b1;
-              bool second = sc > run.b2;
-              if (scaled && fabsf(sc - run.b1) <= 2.0e-6f * fmaxf(fabsf(sc), fabsf(run.b1)) && run.i1 != INT_MAX) {
-                // too close for fp32: the exact products decide (rare)
-                const double ea = INT8 ? (double)iv : (double)a;
-                const double e1 = INT8 ? (double)__float_as_int(run.a1) : (double)run.a1;
-                better = ea * p.e.colscale[k] > e1 * p.e.colscale[run.i1];
-              }
-              if (INT8 && p.nparts == 3 && !scaled) {
-                // int16 codes: sums beyond 2^24 are not exact as floats, the integers decide
-                better = run.i1 == INT_MAX || iv > __float_as_int(run.a1);
-                second = run.i2 == INT_MAX || iv > __float_as_int(run.a2);
-              }
-              const float araw = INT8 ? __int_as_float(iv) : a;   // integer accumulators are kept bit for bit
-              if (better) {
-                run.b2 = run.b1; run.a2 = run.a1; run.i2 = run.i1;
-                run.b1 = sc; run.a1 = araw; run.i1 = k;
-              } else if (second) {
-                run.b2 = sc; run.a2 = araw; run.i2 = k;
-              }
-            }
-          }
-        }
-      }
+      sim_epi_columns<INT8, EPI, TS>(p, taddr, nt, k_base, k_valid, row, row_ok, sp, scaled, run);
       tc_fence_before();
       __syncwarp();
       if (lane == 0) {
@@ -379,23 +412,7 @@ sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
         acc = 0;
         acc_phase ^= 1u;
       }
-      if (EPI == EPI_ARGMAX && nt == p.n_tiles - 1 && p.splits == 1) {
-        if (row_ok) {
-          // reported scores: the exact double products of the two winners (one conversion per row)
-          const double e1 = INT8 ? (double)__float_as_int(run.a1) : (double)run.a1;
-          const double e2 = INT8 ? (double)__float_as_int(run.a2) : (double)run.a2;
-          double b1 = scaled ? e1 * p.e.colscale[run.i1] : e1;
-          double b2 = run.i2 == INT_MAX ? b1 : (scaled ? e2 * p.e.colscale[run.i2] : e2);  // K == 1
-          if (p.e.ham_D > 0) {
-            b1 = 0.5 * ((double)p.e.ham_D - b1);
-            b2 = 0.5 * ((double)p.e.ham_D - b2);
-          }
-          p.e.labels[row] = run.i1;
-          if (p.e.best) p.e.best[row] = (float)b1;
-          if (p.e.second) p.e.second[row] = (float)b2;
-        }
-        run = Top2f{NEG_BIG_F, NEG_BIG_F, 0.0f, 0.0f, INT_MAX, INT_MAX};
-      }
+      if (EPI == EPI_ARGMAX && nt == p.n_tiles - 1 && p.splits == 1) sim_epi_finish<INT8>(p, row, row_ok, scaled, run);
     }
   } else {
     // ================================================================= expanders (warps 6..13)
@@ -758,6 +775,316 @@ __global__ void split_reduce_kernel(const float* __restrict__ partial, int split
   }
 }
 
+// ---------------------------------------------------------------------------------- small class tiles, TMA-fed
+// sim_ts_kernel: the small-tile kernel (query tile in tensor memory, see TS above) for query rows that are 16-byte
+// aligned (what Handle.alloc_hbits / hdc_encode_* give): the packed words arrive by TMA -- boxes of 128 rows x 32
+// words = 1024 dimensions, 128-byte swizzle, one elected lane of a producer warp per box -- instead of through the
+// expander warps' private cp.async rings, whose refill (8 four-byte copies per lane and chunk plus addresses) was a
+// quarter of an expander warp's time per group (profiles/r2_simtc.md 4.1).  Roles (16 warps, one persistent CTA per
+// SM): warp 0 = TMA producer of the class tiles, warp 1 = MMA issuer + TMEM allocation, warp 2 = TMA producer of the
+// query words, warps 4-7 = epilogue, warps 8-15 = expanders: warp w serves the TMEM lane quarter w % 4 (the only one
+// it can reach); the two warps of a quarter take alternate 16-byte pieces of every row = whole k-blocks (one int8
+// k-block of 128 dimensions or two 16-bit k-blocks of 64).  Groups and barriers as in the TS variant of
+// sim_tc_kernel; TMEM: acc_bufs accumulators of acc_cols columns, then ngroups x 4 k-block slots of 32 columns.
+constexpr int TSQ_THREADS = 512;
+constexpr int TSQ_SLOTS = 4;                       // query chunks in flight
+constexpr int TSQ_WORDS = 32;                      // packed words of a row per chunk
+constexpr int TSQ_BYTES = BM * TSQ_WORDS * 4;      // 16 KB
+constexpr int TSQ_G = 4;                           // k-blocks per group
+constexpr int TSQ_MAXG = 3;                        // groups in flight
+
+template <bool INT8, int EPI>
+__global__ void __launch_bounds__(TSQ_THREADS, 1)
+sim_ts_kernel(const __grid_constant__ CUtensorMap tmB, const __grid_constant__ CUtensorMap tmQ, const SimParams p) {
+  extern __shared__ uint8_t smem_raw[];
+  constexpr int BK = INT8 ? 128 : 64;
+  constexpr int WPK = INT8 ? 4 : 2;          // packed words per k-block
+  constexpr int KPC = TSQ_WORDS / WPK;       // k-blocks per query chunk (8 / 16)
+  constexpr int KPP = 4 / WPK;               // k-blocks per 16-byte piece of a row (1 / 2)
+  constexpr int G = TSQ_G, MG = TSQ_MAXG;
+  const int NG = p.ngroups;
+  const uint32_t base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  const int nb_rows = p.nparts * p.kc;
+  const uint32_t B_BYTES = (uint32_t)nb_rows * KB_BYTES;
+  const uint32_t q_base = base + (uint32_t)(NG * G) * B_BYTES;
+  const uint32_t bar0 = q_base + TSQ_SLOTS * TSQ_BYTES;
+  auto full_bar = [&](int s) { return bar0 + 8u * s; };
+  auto empty_bar = [&](int s) { return bar0 + 8u * (MG + s); };
+  auto qfull_bar = [&](int s) { return bar0 + 8u * (2 * MG + s); };
+  auto qempty_bar = [&](int s) { return bar0 + 8u * (2 * MG + TSQ_SLOTS + s); };
+  auto tfull_bar = [&](int s) { return bar0 + 8u * (2 * MG + 2 * TSQ_SLOTS + s); };
+  auto tempty_bar = [&](int s) { return bar0 + 8u * (2 * MG + 2 * TSQ_SLOTS + 2 + s); };
+  const uint32_t tmem_slot = bar0 + 8u * (2 * MG + 2 * TSQ_SLOTS + 4);
+  const int A_COL0 = p.acc_bufs * p.acc_cols;   // first TMEM column of the query slots
+  uint32_t* tmem_slot_ptr = reinterpret_cast<uint32_t*>(smem_raw + (tmem_slot - smem_u32(smem_raw)));
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  if (warp == 0 && lane == 0) {
+    asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&tmB)) : "memory");
+    asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(&tmQ)) : "memory");
+    for (int s = 0; s < NG; ++s) {
+      mbar_init(full_bar(s), 1 + EXW);   // class tiles (producer + bytes) and one arrival per expander warp
+      mbar_init(empty_bar(s), 1);
+    }
+    for (int s = 0; s < TSQ_SLOTS; ++s) {
+      mbar_init(qfull_bar(s), 1);
+      mbar_init(qempty_bar(s), EXW);
+    }
+    for (int s = 0; s < 2; ++s) {
+      mbar_init(tfull_bar(s), 1);
+      mbar_init(tempty_bar(s), 4);
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  if (warp == 1) tmem_alloc<1>(tmem_slot, TMEM_COLS);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = *tmem_slot_ptr;
+
+  // work item = (m-tile of 128 queries, split of the reduction axis); a CTA walks items blockIdx.x, +gridDim.x, ...
+  const int64_t n_items = (int64_t)p.m_tiles * p.splits;
+  auto item_of = [&](int64_t item, int& mt, int& sp, int& kb_lo, int& kb_hi) {
+    mt = (int)(item / p.splits);
+    sp = (int)(item - (int64_t)mt * p.splits);
+    kb_lo = sp * p.kbs;
+    kb_hi = kb_lo + p.kbs < p.num_kb ? kb_lo + p.kbs : p.num_kb;
+  };
+
+  if (warp == 0) {
+    // ================================================================= TMA producer: class tiles
+    int grp = 0;
+    uint32_t phase = 0;
+    for (int64_t item = blockIdx.x; item < n_items; item += gridDim.x) {
+      int mt, sp, kb_lo, kb_hi;
+      item_of(item, mt, sp, kb_lo, kb_hi);
+      for (int kb0 = kb_lo; kb0 < kb_hi; kb0 += G) {
+        const int n = kb_hi - kb0 < G ? kb_hi - kb0 : G;
+        mbar_wait(empty_bar(grp), phase ^ 1u);
+        mbar_arrive_expect_tx_elect(full_bar(grp), (uint32_t)n * B_BYTES);
+        for (int u = 0; u < n; ++u)
+          tma_load_2d_elect(base + (uint32_t)(grp * G + u) * B_BYTES, &tmB, full_bar(grp), (kb0 + u) * BK, 0);
+        __syncwarp();
+        if (++grp == NG) {
+          grp = 0;
+          phase ^= 1u;
+        }
+      }
+    }
+  } else if (warp == 2) {
+    // ================================================================= TMA producer: packed query words
+    int qs = 0;
+    uint32_t qphase = 0;
+    for (int64_t item = blockIdx.x; item < n_items; item += gridDim.x) {
+      int mt, sp, kb_lo, kb_hi;
+      item_of(item, mt, sp, kb_lo, kb_hi);
+      const int nch = (kb_hi - kb_lo + KPC - 1) / KPC;
+      for (int c = 0; c < nch; ++c) {
+        mbar_wait(qempty_bar(qs), qphase ^ 1u);
+        mbar_arrive_expect_tx_elect(qfull_bar(qs), TSQ_BYTES);
+        tma_load_2d_elect(q_base + (uint32_t)qs * TSQ_BYTES, &tmQ, qfull_bar(qs), kb_lo * WPK + c * TSQ_WORDS, mt * BM);
+        __syncwarp();
+        if (++qs == TSQ_SLOTS) {
+          qs = 0;
+          qphase ^= 1u;
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ================================================================= MMA issuer
+    int grp = 0;
+    uint32_t phase = 0;
+    int acc = 0;
+    uint32_t acc_phase = 0;
+    // kind::f16 operand formats (bits 7..9 A, 10..12 B): 1 = bf16, 0 = IEEE half
+    const uint32_t idesc = instr_desc<INT8>(BM, nb_rows) & ((!INT8 && p.f16) ? ~((1u << 7) | (1u << 10)) : ~0u);
+    for (int64_t item = blockIdx.x; item < n_items; item += gridDim.x) {
+      int mt, sp, kb_lo, kb_hi;
+      item_of(item, mt, sp, kb_lo, kb_hi);
+      mbar_wait(tempty_bar(acc), acc_phase ^ 1u);
+      tc_fence_after();
+      const uint32_t d_tmem = tmem_base + (uint32_t)(acc * p.acc_cols);
+      for (int kb0 = kb_lo; kb0 < kb_hi; kb0 += G) {
+        const int n = kb_hi - kb0 < G ? kb_hi - kb0 : G;
+        mbar_wait(full_bar(grp), phase);
+        tc_fence_after();
+        const uint32_t sa = base + (uint32_t)(grp * G) * B_BYTES;
+        const uint32_t b_lo = ((sa & 0x3FFFFu) >> 4) | (1u << 16);   // lower half of smem_desc(sa)
+        const uint32_t at = tmem_base + (uint32_t)(A_COL0 + grp * G * 32);
+        if (n == G) {
+          tc_mma_ts_group_elect<INT8>(d_tmem, at, b_lo, (B_BYTES >> 4) - 6u, idesc, kb0 != kb_lo ? 1u : 0u);
+        } else {
+          for (int u = 0; u < n; ++u)
+            tc_mma_ts_kblock_elect<INT8>(d_tmem, at + 32u * u, b_lo + (B_BYTES >> 4) * u, idesc,
+                                         kb0 + u != kb_lo ? 1u : 0u);
+        }
+        tc_commit_elect<1>(empty_bar(grp));  // frees the group's class tiles and TMEM slots when these MMAs retire
+        if (kb0 + n == kb_hi) tc_commit_elect<1>(tfull_bar(acc));
+        __syncwarp();
+        if (++grp == NG) {
+          grp = 0;
+          phase ^= 1u;
+        }
+      }
+      if (++acc == p.acc_bufs) {
+        acc = 0;
+        acc_phase ^= 1u;
+      }
+    }
+  } else if (warp >= 4 && warp < 8) {
+    // ================================================================= epilogue (warps 4..7)
+    const int q = warp & 3;
+    int acc = 0;
+    uint32_t acc_phase = 0;
+    Top2f run = Top2f{NEG_BIG_F, NEG_BIG_F, 0.0f, 0.0f, INT_MAX, INT_MAX};
+    const bool scaled = p.e.colscale != nullptr;
+    for (int64_t item = blockIdx.x; item < n_items; item += gridDim.x) {
+      int mt, sp, kb_lo, kb_hi;
+      item_of(item, mt, sp, kb_lo, kb_hi);
+      const int64_t row = (int64_t)mt * BM + q * 32 + lane;
+      const bool row_ok = row < p.N;
+      mbar_wait(tfull_bar(acc), acc_phase);
+      tc_fence_after();
+      const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(acc * p.acc_cols);
+      sim_epi_columns<INT8, EPI, true>(p, taddr, 0, 0, p.K, row, row_ok, sp, scaled, run);
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(tempty_bar(acc));
+      if (++acc == p.acc_bufs) {
+        acc = 0;
+        acc_phase ^= 1u;
+      }
+      if (EPI == EPI_ARGMAX && p.splits == 1) sim_epi_finish<INT8>(p, row, row_ok, scaled, run);
+    }
+  } else if (warp >= 8) {
+    // ================================================================= expanders (warps 8..15)
+    const int q = warp & 3;            // TMEM lane quarter of this warp
+    const int hsel = (warp - 8) >> 2;  // the two warps of a quarter take alternate 16-byte pieces of every row
+    const int t = q * 32 + lane;       // row of the tile
+    // row t of a query slot: 128 bytes, piece j at ((j ^ (t & 7)) << 4) (128-byte swizzle: conflict-free, lane = row)
+    const uint32_t q_row = (uint32_t)t * 128u;
+    const uint32_t sw = (uint32_t)(t & 7);
+    const uint32_t one2 = p.f16 ? 0x3C003C00u : 0x3F803F80u;  // two +1.0 in half / bf16; the sign bit makes -1.0
+    const uint32_t lane_base = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)A_COL0;
+    int grp = 0, qs = 0;
+    uint32_t phase = 0, qphase = 0;
+    // group hand-off of this warp: published with one fence and one arrival
+    auto publish = [&]() {
+      tmem_st_wait();
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(full_bar(grp));
+      if (++grp == NG) {
+        grp = 0;
+        phase ^= 1u;
+      }
+    };
+    auto acquire = [&]() {
+      mbar_wait(empty_bar(grp), phase ^ 1u);
+      tc_fence_after();   // the MMAs that read these TMEM slots have retired (tcgen05.commit -> empty)
+    };
+    for (int64_t item = blockIdx.x; item < n_items; item += gridDim.x) {
+      int mt, sp, kb_lo, kb_hi;
+      item_of(item, mt, sp, kb_lo, kb_hi);
+      const int nkb = kb_hi - kb_lo;
+      const int ngr = (nkb + G - 1) / G;
+      const int nch = (nkb + KPC - 1) / KPC;
+      int cur_g = 0;   // group (of this item) whose TMEM slots this warp is filling
+      acquire();
+      for (int c = 0; c < nch; ++c) {
+        mbar_wait(qfull_bar(qs), qphase);
+        const uint32_t q_slot = q_base + (uint32_t)qs * TSQ_BYTES + q_row;
+#pragma unroll
+        for (int jj = 0; jj < 4; ++jj) {
+          const int j = 2 * jj + hsel;               // piece of the chunk
+          const int kb = (c * 8 + j) * KPP;          // its first k-block (relative to kb_lo)
+          if (kb >= nkb) break;
+          const int g = kb / G;
+          while (cur_g < g) {                        // (a warp's pieces never skip a group: one step)
+            publish();
+            acquire();
+            ++cur_g;
+          }
+          uint32_t w[4];
+          asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];"
+                       : "=r"(w[0]), "=r"(w[1]), "=r"(w[2]), "=r"(w[3])
+                       : "r"(q_slot + ((((uint32_t)j) ^ sw) << 4))
+                       : "memory");
+          const uint32_t a_grp = lane_base + (uint32_t)(grp * G * 32);
+          if (INT8) {
+            // one k-block of 128 dimensions: 4 words -> 32 words of bytes -128 * bit (see sim_epi_columns)
+            const uint32_t dst = a_grp + (uint32_t)((kb - g * G) * 32);
+#pragma unroll
+            for (int hh = 0; hh < 2; ++hh) {
+              uint32_t o[16];
+#pragma unroll
+              for (int i = 0; i < 16; ++i) {
+                const int iw = 16 * hh + i;
+                o[i] = (w[iw >> 3] << (7 - (iw & 7))) & 0x80808080u;
+              }
+              tmem_st16(dst + 16u * hh, o);
+            }
+          } else {
+            // two k-blocks of 64 dimensions: 2 words -> 32 words of +-1.0 pairs, each
+#pragma unroll
+            for (int kk = 0; kk < 2; ++kk) {
+              if (kb + kk < nkb) {
+                const uint32_t dst = a_grp + (uint32_t)((kb + kk - g * G) * 32);
+#pragma unroll
+                for (int hh = 0; hh < 2; ++hh) {
+                  uint32_t o[16];
+#pragma unroll
+                  for (int i = 0; i < 16; ++i) o[i] = ((w[2 * kk + hh] << (15 - i)) & 0x80008000u) | one2;
+                  tmem_st16(dst + 16u * hh, o);
+                }
+              }
+            }
+          }
+        }
+        __syncwarp();   // every lane holds its words in registers: the slot may be refilled
+        if (lane == 0) mbar_arrive(qempty_bar(qs));
+        if (++qs == TSQ_SLOTS) {
+          qs = 0;
+          qphase ^= 1u;
+        }
+      }
+      // groups this warp has no piece in (the item's last k-blocks) still take its arrival
+      while (cur_g < ngr - 1) {
+        publish();
+        acquire();
+        ++cur_g;
+      }
+      publish();
+    }
+  }
+
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) {
+    tc_fence_after();
+    tmem_dealloc<1>(tmem_base, TMEM_COLS);
+  }
+}
+
+template <bool INT8, int EPI>
+cudaError_t launch_ts(const CUtensorMap& tmB, const CUtensorMap& tmQ, SimParams p, int grid, cudaStream_t st) {
+  // per-device attribute of the function: set on every launch (handles on several devices of one process)
+  cudaError_t e = cudaFuncSetAttribute(sim_ts_kernel<INT8, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                       SMEM_LIMIT);
+  if (e != cudaSuccess) return e;
+  const int nb_rows = p.nparts * p.kc;
+  const int group_bytes = TSQ_G * nb_rows * KB_BYTES;
+  // Two groups in flight beside two 128-column accumulators.  Measured alternatives: three groups with two
+  // accumulators of 32 columns (K = 6 int8: 0.105 against 0.104 ms per 131072 queries), three groups with ONE
+  // 128-column accumulator (K = 26 fp32: 0.234 against 0.218 ms; int16 0.171 against 0.130).
+  p.ngroups = 2;
+  p.acc_cols = TS_ACC_COLS;
+  p.acc_bufs = 2;
+  const int smem = p.ngroups * group_bytes + TSQ_SLOTS * TSQ_BYTES + SMEM_EXTRA;
+  sim_ts_kernel<INT8, EPI><<<grid, TSQ_THREADS, smem, st>>>(tmB, tmQ, p);
+  return cudaGetLastError();
+}
+
 template <bool INT8, int EPI, int CG, bool TS = false>
 cudaError_t launch_cg(const CUtensorMap& tmB, const SimParams& p, int grid, cudaStream_t st) {
   // per-device attribute of the function: set on every launch (handles on several devices of one process)
@@ -780,7 +1107,9 @@ cudaError_t launch_cg(const CUtensorMap& tmB, const SimParams& p, int grid, cuda
   return cudaLaunchKernelEx(&cfg, sim_tc_kernel<INT8, EPI, CG, TS>, tmB, p);
 }
 template <bool INT8, int EPI>
-cudaError_t launch_one(const CUtensorMap& tmB, const SimParams& p, int cg, bool ts, int grid, cudaStream_t st) {
+cudaError_t launch_one(const CUtensorMap& tmB, const CUtensorMap* tmQ, const SimParams& p, int cg, bool ts, int grid,
+                       cudaStream_t st) {
+  if (ts && tmQ) return launch_ts<INT8, EPI>(tmB, *tmQ, p, grid, st);
   if (ts) return launch_cg<INT8, EPI, 1, true>(tmB, p, grid, st);
   return cg == 2 ? launch_cg<INT8, EPI, 2>(tmB, p, grid, st) : launch_cg<INT8, EPI, 1>(tmB, p, grid, st);
 }
@@ -884,6 +1213,13 @@ cudaError_t launch_sim_tc(TcContext* tc, const uint32_t* Hbits, int64_t N, int64
   if (ts) cg = 1;
   CUtensorMap tmB;
   if (!tc_make_map(tc, &tmB, cop, int8, rows_total, ld, ld, nparts * kc / cg)) return cudaErrorInvalidValue;
+  // small tiles with 16-byte aligned query rows: the packed words by TMA (sim_ts_kernel)
+  CUtensorMap tmQ;
+  const CUtensorMap* tq = nullptr;
+  if (ts && (ldh & 3) == 0 && (reinterpret_cast<uintptr_t>(Hbits) & 15) == 0 && !getenv("HDC_NO_TSQ")) {
+    if (!tc_make_map_words(tc, &tmQ, Hbits, N, words_of(D_eff), ldh)) return cudaErrorInvalidValue;
+    tq = &tmQ;
+  }
   SimParams p;
   p.Hbits = Hbits;
   p.N = N;
@@ -914,8 +1250,8 @@ cudaError_t launch_sim_tc(TcContext* tc, const uint32_t* Hbits, int64_t N, int64
   const int grid = (int)(items < max_units ? items : max_units) * cg;
   ++*nlaunch;
   if (p.splits > 1) {
-    ce = int8 ? launch_one<true, EPI_SCORE>(tmB, p, 1, ts, grid, st)
-              : launch_one<false, EPI_SCORE>(tmB, p, 1, ts, grid, st);
+    ce = int8 ? launch_one<true, EPI_SCORE>(tmB, tq, p, 1, ts, grid, st)
+              : launch_one<false, EPI_SCORE>(tmB, tq, p, 1, ts, grid, st);
     if (ce != cudaSuccess) return ce;
     const unsigned rg = (unsigned)((N + 63) / 64);
     if (p.splits <= 2) split_reduce_kernel<2><<<rg, 64, 0, st>>>(p.partial, p.splits, N, K, e);
@@ -925,10 +1261,10 @@ cudaError_t launch_sim_tc(TcContext* tc, const uint32_t* Hbits, int64_t N, int64
     return cudaGetLastError();
   }
   if (int8)
-    return e.kind == EPI_SCORE ? launch_one<true, EPI_SCORE>(tmB, p, cg, ts, grid, st)
-                               : launch_one<true, EPI_ARGMAX>(tmB, p, cg, ts, grid, st);
-  return e.kind == EPI_SCORE ? launch_one<false, EPI_SCORE>(tmB, p, cg, ts, grid, st)
-                             : launch_one<false, EPI_ARGMAX>(tmB, p, cg, ts, grid, st);
+    return e.kind == EPI_SCORE ? launch_one<true, EPI_SCORE>(tmB, tq, p, cg, ts, grid, st)
+                               : launch_one<true, EPI_ARGMAX>(tmB, tq, p, cg, ts, grid, st);
+  return e.kind == EPI_SCORE ? launch_one<false, EPI_SCORE>(tmB, tq, p, cg, ts, grid, st)
+                             : launch_one<false, EPI_ARGMAX>(tmB, tq, p, cg, ts, grid, st);
 }
 
 }  // namespace hdc

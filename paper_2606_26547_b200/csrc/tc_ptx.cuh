@@ -415,5 +415,8 @@ __device__ __forceinline__ void tmem_dealloc(uint32_t taddr, uint32_t cols) {
 struct TcContext;
 bool tc_make_map(TcContext* tc, CUtensorMap* out, const void* ptr, bool int8, int64_t rows, int64_t cols,
                  int64_t ld, int box_rows);
+// host: packed hypervector words [rows][cols] uint32, row stride ld words (ld % 4 == 0, 16-byte aligned base): TMA
+// boxes of 32 words x 128 rows with the 128-byte swizzle; out-of-range words and rows read as zero.
+bool tc_make_map_words(TcContext* tc, CUtensorMap* out, const void* ptr, int64_t rows, int64_t cols, int64_t ld);
 
 }  // namespace hdc

@@ -216,7 +216,10 @@ def test_encode_rp_bf16_inputs_in_place(hd, h):
 @pytest.mark.parametrize("N,K,D,D_eff", [(150, 26, 2100, 2100), (64, 6, 10000, 4099), (33, 1, 500, 500),
                                          (140, 70, 1300, 1000), (140, 600, 1300, 1000), (300, 200, 700, 640),
                                          (130, 1000, 520, 520)])
-def test_dot_cos_similarity_and_classify(hd, h, sim, hv_bits, N, K, D, D_eff):
+@pytest.mark.parametrize("pad", [False, True])
+def test_dot_cos_similarity_and_classify(hd, h, sim, hv_bits, N, K, D, D_eff, pad):
+    """pad: query rows of W words rounded up to 4 (16-byte aligned rows, what Handle.alloc_hbits gives: class tiles of
+    <= 128 rows then take sim_ts_kernel, fed by TMA) or exactly W words (any alignment: the cp.async rings)."""
     r = rng(5, N, K, D_eff, hv_bits)
     hb = r.integers(0, 2, size=(N, D), dtype=np.uint8)
     C = (r.standard_normal((K, D)) * 30).astype(np.float32)
@@ -226,7 +229,7 @@ def test_dot_cos_similarity_and_classify(hd, h, sim, hv_bits, N, K, D, D_eff):
     simc = getattr(O, "SIM_" + sim)
     S_or = O.similarity(hb, C, D_eff, simc, hv_bits)
     kn = hd.knobs(D_eff, hv_bits=hv_bits, sim=getattr(hd, "HDC_SIM_" + sim))
-    Hd, Cd = dev_bits(hb), dev(C)
+    Hd, Cd = dev_bits(hb, (D + 127) // 128 * 4 if pad else None), dev(C)
     S = h.hdc_similarity(Hd, Cd, kn).cpu().numpy()
     lab, best, sec = h.hdc_classify(Hd, Cd, kn, want_scores=True)
     lab = lab.cpu().numpy()
@@ -269,7 +272,7 @@ def test_similarity_on_cta_pairs(hd, h, sim, hv_bits, N, K, D, D_eff, perf):
     simc = getattr(O, "SIM_" + sim)
     S_or = O.similarity(hb, C, D_eff, simc, hv_bits, perf[0], perf[1])
     lab_or, best_or, sec_or = O.classify(S_or, simc)
-    Hd, Cd = dev_bits(hb), dev(C)
+    Hd, Cd = dev_bits(hb, (D + 127) // 128 * 4 if N % 2 else None), dev(C)
     out = {}
     for flags in (hd.HDC_FLAG_TC_2CTA, hd.HDC_FLAG_TC_1CTA):
         kn = hd.knobs(D_eff, hv_bits=hv_bits, sim=getattr(hd, "HDC_SIM_" + sim), flags=flags, perf_begin=perf[0],
@@ -501,7 +504,7 @@ def test_perforated_similarity_and_classify(hd, h, begin, stride, sim, hv_bits, 
     simc = getattr(O, "SIM_" + sim)
     S_or = O.similarity(hb, C, D_eff, simc, hv_bits, begin, stride)
     kn = hd.knobs(D_eff, hv_bits=hv_bits, sim=getattr(hd, "HDC_SIM_" + sim), perf_begin=begin, perf_stride=stride)
-    Hd, Cd = dev_bits(hb), dev(C)
+    Hd, Cd = dev_bits(hb, (D + 127) // 128 * 4 if (begin + stride + N) % 2 else None), dev(C)
     S = h.hdc_similarity(Hd, Cd, kn).cpu().numpy()
     lab = h.hdc_classify(Hd, Cd, kn).cpu().numpy()
     lab_or, _, _ = O.classify(S_or, simc)
@@ -685,7 +688,7 @@ def test_similarity_classify_fuzz(hd, h, case):
     simc = getattr(O, "SIM_" + sim)
     S_or = O.similarity(hb, C, D_eff, simc, hv_bits, begin, stride)
     kn = hd.knobs(D_eff, hv_bits=hv_bits, sim=getattr(hd, "HDC_SIM_" + sim), perf_begin=begin, perf_stride=stride)
-    Hd, Cd = dev_bits(hb), dev(C)
+    Hd, Cd = dev_bits(hb, (D + 127) // 128 * 4 if case % 2 else None), dev(C)
     S = h.hdc_similarity(Hd, Cd, kn).cpu().numpy()
     lab = h.hdc_classify(Hd, Cd, kn).cpu().numpy()
     lab_or, _, _ = O.classify(S_or, simc)
