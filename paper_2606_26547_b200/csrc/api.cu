@@ -682,8 +682,10 @@ int do_infer_rp(hdc_ctx* h, const void* X, int x_dtype, int64_t N, int F, int64_
   uint32_t* Hd = Hbits;
   int64_t ldhd = ldh;
   if (!Hd && !prep_only(h)) {
-    Hd = b.take<uint32_t>((size_t)N * W);
-    ldhd = W;
+    // rows of W words rounded up to 4: 16-byte aligned rows let the encode epilogue write 16-byte stores and the
+    // small-tile similarity kernel fetch the words by TMA (as Handle.alloc_hbits does for caller-owned hypervectors)
+    ldhd = round_up(W, 4);
+    Hd = b.take<uint32_t>((size_t)N * (size_t)ldhd);
     if (b.off > ws_bytes) return fail(h, HDC_ERR_WORKSPACE, "infer_rp: workspace too small");
   }
   int rc = do_encode_rp(h, X, x_dtype, N, F, ldx, P, p_dtype, D, ldp, k, HDC_OUT_BITS, Hd, ldhd, nullptr, 0, b,
@@ -722,7 +724,7 @@ int with_model(hdc_ctx* h, void* blob, size_t cap, int mode, Fn fn) {
 size_t infer_ws_bytes(const hdc_ctx* h, int64_t N, int F, int K, const hdc_knobs_t* k) {
   Bump b(nullptr);
   infer_ws(K, k->D_eff, b);
-  b.take<uint32_t>((size_t)N * words_of(k->D_eff));
+  b.take<uint32_t>((size_t)N * (size_t)round_up(words_of(k->D_eff), 4));
   encode_ws(h, N, F, k->D_eff, k, b);
   return b.off + 1024 + similarity_ws(N, K, k);
 }
