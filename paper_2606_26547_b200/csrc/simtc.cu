@@ -32,7 +32,6 @@
 // the epilogue, so the queries are expanded once; int8 (hv_bits 8) and +-1 int8 (hv_bits 1) with
 // int32 accumulation (exact).
 #include <cuda_fp16.h>
-#include <cstdlib>
 #include <limits.h>
 
 #include <type_traits>
@@ -1216,7 +1215,7 @@ cudaError_t launch_sim_tc(TcContext* tc, const uint32_t* Hbits, int64_t N, int64
   // small tiles with 16-byte aligned query rows: the packed words by TMA (sim_ts_kernel)
   CUtensorMap tmQ;
   const CUtensorMap* tq = nullptr;
-  if (ts && (ldh & 3) == 0 && (reinterpret_cast<uintptr_t>(Hbits) & 15) == 0 && !getenv("HDC_NO_TSQ")) {
+  if (ts && (ldh & 3) == 0 && (reinterpret_cast<uintptr_t>(Hbits) & 15) == 0) {
     if (!tc_make_map_words(tc, &tmQ, Hbits, N, words_of(D_eff), ldh)) return cudaErrorInvalidValue;
     tq = &tmQ;
   }
