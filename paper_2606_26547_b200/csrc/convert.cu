@@ -181,17 +181,14 @@ __global__ void quantize_rows_i8_kernel(const void* __restrict__ src, int src_ki
 // max |C[k][d]| over k < K, d < D_eff; non-negative floats order as unsigned ints.
 __global__ void tensor_amax_kernel(const float* __restrict__ C, int K, int D_eff, int64_t ldc, Perf pf,
                                    float* __restrict__ amax) {
+  // blockIdx.y = class row, blockIdx.x = slice of its columns (no division per element)
+  const float* row = C + (int64_t)blockIdx.y * ldc;
   float a = 0.0f;
-  const int64_t total = (int64_t)K * D_eff;
-  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < total;
-       i += (int64_t)gridDim.x * blockDim.x) {
-    const int64_t k = i / D_eff;
-    const int d = (int)(i - k * D_eff);
-    if (perf_visits(pf, d)) a = fmaxf(a, fabsf(__ldg(C + k * ldc + d)));
-  }
+  for (int d = blockIdx.x * blockDim.x + threadIdx.x; d < D_eff; d += gridDim.x * blockDim.x)
+    if (perf_visits(pf, d)) a = fmaxf(a, fabsf(__ldg(row + d)));
 #pragma unroll
   for (int off = 16; off; off >>= 1) a = fmaxf(a, __shfl_xor_sync(0xffffffffu, a, off));
-  if ((threadIdx.x & 31) == 0) atomicMax(reinterpret_cast<unsigned int*>(amax), __float_as_uint(a));
+  if ((threadIdx.x & 31) == 0 && a > 0.0f) atomicMax(reinterpret_cast<unsigned int*>(amax), __float_as_uint(a));
 }
 
 __global__ void quantize_tensor_i8_kernel(const float* __restrict__ C, int K, int D_eff, int64_t ldc,
@@ -508,7 +505,9 @@ cudaError_t launch_tensor_amax(const float* C, int K, int D_eff, int64_t ldc, Pe
                                cudaStream_t st, int64_t* nlaunch) {
   cudaError_t e = cudaMemsetAsync(amax, 0, sizeof(float), st);
   if (e != cudaSuccess) return e;
-  tensor_amax_kernel<<<grid_for((int64_t)K * D_eff, 256, 148 * 4), 256, 0, st>>>(C, K, D_eff, ldc, pf, amax);
+  // K rows x slices of up to 2048 columns (8 per thread); K <= 65535 (checked at the API)
+  const int slices = (D_eff + 2047) / 2048;
+  tensor_amax_kernel<<<dim3((unsigned)slices, (unsigned)K), 256, 0, st>>>(C, K, D_eff, ldc, pf, amax);
   ++*nlaunch;
   return cudaGetLastError();
 }
