@@ -131,6 +131,36 @@ __device__ __forceinline__ uint32_t prmt_sign_bytes(uint32_t v) {
   return d;
 }
 
+// Running best / runner-up of a query row: class k arrives with its accumulator (iv: integer kinds, a: as a float) and
+// its fp32 score sc >= run.lim.  Classes arrive in increasing order: strict > keeps the lowest index.
+template <bool INT8>
+__device__ __forceinline__ void top2_update(const SimParams& p, Top2f& run, int k, int iv, float a, float sc,
+                                            bool scaled) {
+  bool better = sc > run.b1;
+  bool second = sc > run.b2;
+  if (scaled && fabsf(sc - run.b1) <= 2.0e-6f * fmaxf(fabsf(sc), fabsf(run.b1)) && run.i1 != INT_MAX) {
+    // too close for fp32: the exact products decide (rare)
+    const double ea = INT8 ? (double)iv : (double)a;
+    const double e1 = INT8 ? (double)__float_as_int(run.a1) : (double)run.a1;
+    better = ea * p.e.colscale[k] > e1 * p.e.colscale[run.i1];
+  }
+  if (INT8 && p.nparts == 3 && !scaled) {
+    // int16 codes: sums beyond 2^24 are not exact as floats, the integers decide
+    better = run.i1 == INT_MAX || iv > __float_as_int(run.a1);
+    second = run.i2 == INT_MAX || iv > __float_as_int(run.a2);
+  }
+  const float araw = INT8 ? __int_as_float(iv) : a;   // integer accumulators are kept bit for bit
+  if (better) {
+    run.b2 = run.b1; run.a2 = run.a1; run.i2 = run.i1;
+    run.b1 = sc; run.a1 = araw; run.i1 = k;
+  } else if (second) {
+    run.b2 = sc; run.a2 = araw; run.i2 = k;
+  }
+  // (superset of the ambiguity band |sc - b1| <= 2e-6 max(|sc|, |b1|) for sc < b1, and of sc > b2; the
+  // integer compares of the int16 codes are covered by float conversion being monotonic: >= not >)
+  run.lim = scaled ? fminf(run.b2, run.b1 - 2.1e-6f * fabsf(run.b1)) : run.b2;
+}
+
 // Epilogue of one accumulator tile for the query row of this thread (lane = TMEM lane of its warp's quarter): columns
 // [0, k_valid) of the tile at taddr are classes k_base + c of n-tile nt; with nparts == 3 the three parts of class c
 // sit kc columns apart.  sp: split of the reduction axis this CTA reduced (p.splits > 1: partial sums only).
@@ -145,6 +175,30 @@ __device__ __forceinline__ void sim_epi_columns(const SimParams& p, uint32_t tad
       tmem_ld16(taddr + (uint32_t)(2 * p.kc + c0), v2);
     }
     tmem_ld_wait();
+    if constexpr (INT8 && EPI == EPI_ARGMAX && !TS) {
+      // wide int8 tiles, sixteen valid classes: the sweep that paces the K = 1000 kernels -- scales by 16-byte loads,
+      // no per-column bounds test, convert + multiply + one compare per class in front of the update logic
+      if (p.nparts == 1 && p.splits == 1 && c0 + 16 <= k_valid) {
+        float cs[16];
+        if (scaled) {
+          const float4* cp = reinterpret_cast<const float4*>(p.e.colscale_f + k_base + c0);   // 64-byte aligned
+#pragma unroll
+          for (int q4 = 0; q4 < 4; ++q4) {
+            const float4 c4 = __ldg(cp + q4);
+            cs[4 * q4] = c4.x; cs[4 * q4 + 1] = c4.y; cs[4 * q4 + 2] = c4.z; cs[4 * q4 + 3] = c4.w;
+          }
+        }
+#pragma unroll
+        for (int j = 0; j < 16; ++j) {
+          const int iv = (int)v0[j];
+          const float a = (float)iv;
+          const float sc = scaled ? __fmul_rn(a, cs[j]) : a;
+          if (sc < run.lim) continue;
+          top2_update<INT8>(p, run, k_base + c0 + j, iv, a, sc, scaled);
+        }
+        continue;
+      }
+    }
 #pragma unroll
     for (int j = 0; j < 16; ++j) {
       if (c0 + j < k_valid) {
@@ -192,29 +246,7 @@ __device__ __forceinline__ void sim_epi_columns(const SimParams& p, uint32_t tad
           // classes arrive in increasing order: strict > keeps the lowest index
           const float sc = scaled ? __fmul_rn(a, p.e.colscale_f[k]) : a;
           if (sc < run.lim) continue;
-          bool better = sc > run.b1;
-          bool second = sc > run.b2;
-          if (scaled && fabsf(sc - run.b1) <= 2.0e-6f * fmaxf(fabsf(sc), fabsf(run.b1)) && run.i1 != INT_MAX) {
-            // too close for fp32: the exact products decide (rare)
-            const double ea = INT8 ? (double)iv : (double)a;
-            const double e1 = INT8 ? (double)__float_as_int(run.a1) : (double)run.a1;
-            better = ea * p.e.colscale[k] > e1 * p.e.colscale[run.i1];
-          }
-          if (INT8 && p.nparts == 3 && !scaled) {
-            // int16 codes: sums beyond 2^24 are not exact as floats, the integers decide
-            better = run.i1 == INT_MAX || iv > __float_as_int(run.a1);
-            second = run.i2 == INT_MAX || iv > __float_as_int(run.a2);
-          }
-          const float araw = INT8 ? __int_as_float(iv) : a;   // integer accumulators are kept bit for bit
-          if (better) {
-            run.b2 = run.b1; run.a2 = run.a1; run.i2 = run.i1;
-            run.b1 = sc; run.a1 = araw; run.i1 = k;
-          } else if (second) {
-            run.b2 = sc; run.a2 = araw; run.i2 = k;
-          }
-          // (superset of the ambiguity band |sc - b1| <= 2e-6 max(|sc|, |b1|) for sc < b1, and of sc > b2; the
-          // integer compares of the int16 codes are covered by float conversion being monotonic: >= not >)
-          run.lim = scaled ? fminf(run.b2, run.b1 - 2.1e-6f * fabsf(run.b1)) : run.b2;
+          top2_update<INT8>(p, run, k, iv, a, sc, scaled);
         }
       }
     }
