@@ -34,6 +34,8 @@ F16 = 6         # encode operands as IEEE half ("floating-point ty
 SIM_DOT, SIM_COS, SIM_HAMMING = 0, 1, 2
 HV_F16 = 17      # hv_bits code (not a width): class operand as 16-bit IEEE half ("FP16")
 HV_I16 = 18      # hv_bits code (not a width): class operand as 16-bit integers ("integer data types (8, 16, ...")
+HV_I32 = 19      # hv_bits codes: class operand as 32- / 64-bit integers ("... 32, or 64-bit)"; reading A22)
+HV_I64 = 20
 
 
 # ------------------------------------------------------------------------------------- S0
@@ -99,6 +101,25 @@ def quantize_int16_tensor(c: np.ndarray) -> np.ndarray:
     s = np.float32(32767.0) / a if a > 0 else np.float32(1.0)
     q = np.rint((c * np.float32(s)).astype(np.float32))
     return np.clip(q, -32767, 32767).astype(np.int32)
+
+
+def round_int_tensor(c: np.ndarray, width: int) -> np.ndarray:
+    """Class operand as 32- or 64-bit integers (hypervectors "represented using integer data
+    types (8, 16, 32, or 64-bit)"; L53 / L181: class hypervectors are sums of +-1 hypervectors, i.e. integers;
+    reading A22): the accumulators themselves, q = rint(c), round half to even, NO scale (an fp32 value has 24
+    significant bits: stretching it to 2^31 adds rounding and no information; for the integer accumulators
+    that training produces q = c), saturating symmetrically at +-(2^(width-1) - 1).  Returns int64."""
+    if width not in (32, 64):
+        raise ValueError("width")
+    c = np.ascontiguousarray(c, dtype=np.float32).astype(np.float64)     # every fp32 is a float64
+    q = np.rint(c)                                                        # half to even; integers in float64
+    lim = (1 << (width - 1)) - 1
+    edge = float(1 << (width - 1))                                        # 2^(width-1): first value out of range
+    inside = np.abs(q) < edge                                             # these convert exactly (fp32-valued)
+    out = np.where(inside, q, 0.0).astype(np.int64)
+    out[~inside & (q > 0)] = lim
+    out[~inside & (q < 0)] = -lim
+    return out
 
 
 def rp_operands(X: np.ndarray, P: np.ndarray, precision: int):
@@ -177,7 +198,8 @@ def class_operand(C_acc: np.ndarray, D_eff: int, hv_bits: int) -> np.ndarray:
     (training in high precision, inference "projecting class ... hypervectors
     onto lower-precision integer types"; S5): 32 -> C_acc; 16 -> bf16 RNE; 8 -> per-tensor
     symmetric int8 over k<K, d<D_eff; 1 -> bit [C_acc < 0]; HV_F16 -> IEEE half RNE; HV_I16 -> per-tensor
-    symmetric int16 over k<K, d<D_eff.  Returned as float64 values (bits as uint8)."""
+    symmetric int16 over k<K, d<D_eff; HV_I32 / HV_I64 -> rint(C_acc) as 32- / 64-bit integers (A22).
+    Returned as float64 values (bits as uint8, the 32- / 64-bit integer codes as int64)."""
     c = np.asarray(C_acc, dtype=np.float32)[:, :D_eff]
     if hv_bits == 32:
         return c.astype(np.float64)
@@ -191,6 +213,8 @@ def class_operand(C_acc: np.ndarray, D_eff: int, hv_bits: int) -> np.ndarray:
         return quantize_int8_tensor(c).astype(np.float64)
     if hv_bits == HV_I16:
         return quantize_int16_tensor(c).astype(np.float64)
+    if hv_bits in (HV_I32, HV_I64):
+        return round_int_tensor(c, 32 if hv_bits == HV_I32 else 64)
     if hv_bits == 1:
         return (c < 0).astype(np.uint8)
     raise ValueError("hv_bits")
@@ -230,6 +254,29 @@ def cosine(hbits: np.ndarray, cop: np.ndarray, D_eff: int) -> np.ndarray:
     return out
 
 
+def dot_int(hbits: np.ndarray, q: np.ndarray, D_eff: int) -> np.ndarray:
+    """s[n,k] = sum_{d<D_eff} v[n,d]*q[k,d] for integer codes q, in 64-bit integer arithmetic (exact while
+    sum_d |q[k,d]| < 2^63: the contract of the 32- / 64-bit integer class operands, A22).  int64 [N][K]."""
+    v = (1 - 2 * np.asarray(hbits, dtype=np.int64)[:, :D_eff])
+    q = np.asarray(q, dtype=np.int64)[:, :D_eff]
+    out = np.empty((v.shape[0], q.shape[0]), dtype=np.int64)
+    for k in range(q.shape[0]):
+        out[:, k] = (v * q[k][None, :]).sum(axis=1, dtype=np.int64)
+    return out
+
+
+def cosine_int(hbits: np.ndarray, q: np.ndarray, D_eff: int) -> np.ndarray:
+    """Cosine for integer codes: dot_int / (sqrt(D_eff) * |q[k]|), 0 where the class norm is 0 (A8); the
+    squared norm is summed in python integers (exact), the division done in float64."""
+    s = dot_int(hbits, q, D_eff)
+    out = np.zeros(s.shape, dtype=np.float64)
+    for k in range(s.shape[1]):
+        n2 = sum(int(x) * int(x) for x in np.asarray(q)[k, :D_eff])
+        if n2 > 0:
+            out[:, k] = s[:, k].astype(np.float64) / (np.sqrt(float(D_eff)) * np.sqrt(float(n2)))
+    return out
+
+
 def perforated_index(D_eff: int, begin: int = 0, stride: int = 1) -> np.ndarray:
     """Reduction perforation (the reduction-axis loop "skip[s] iterations at regular
     intervals, defined by a specified stride", annotation parameters "starting offset, ending offset,
@@ -257,6 +304,12 @@ def similarity(hbits: np.ndarray, C_acc: np.ndarray, D_eff: int, sim: int, hv_bi
         if hv_bits != 1:
             raise ValueError("Hamming needs hv_bits=1")
         return hamming(hbits, cop, D_eff)
+    if hv_bits in (HV_I32, HV_I64):
+        if sim == SIM_DOT:
+            return dot_int(hbits, cop, D_eff)
+        if sim == SIM_COS:
+            return cosine_int(hbits, cop, D_eff)
+        raise ValueError("sim")
     if hv_bits == 1:
         cop = bipolar(cop)
     if sim == SIM_DOT:

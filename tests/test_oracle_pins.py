@@ -1011,3 +1011,76 @@ def test_int16_similarity_brute_force_and_small_integer_identity():
     assert np.array_equal(o.similarity(hb, Ci, D, o.SIM_DOT, o.HV_I16), o.similarity(hb, Ci, D, o.SIM_DOT, 32))
     assert np.allclose(o.similarity(hb, Ci, D, o.SIM_COS, o.HV_I16), o.similarity(hb, Ci, D, o.SIM_COS, 32),
                        rtol=1e-14, atol=0)
+
+
+# ------------------------------------------------------------------ S5 32- / 64-bit integer class operand (A22)
+def test_int32_int64_codes_by_hand():
+    """round_int_tensor ("integer data types (8, 16, 32, or 64-bit)"; reading A22): the codes
+    ARE the accumulators, q = rint-to-nearest-EVEN(c), no scale, symmetric saturation at 2^(w-1) - 1.  By hand,
+    so that truncation (1.5 -> 1), half-up (0.5 -> 1, -1.5 -> -1), half-away (2.5 -> 3), any A7-style scale
+    (7 -> 7 * s), a clamp at -2^31 and a wrap of out-of-range values each fail."""
+    c = np.array([[0.5, 1.5, 2.5, 3.49, 7.0, 16777216.0],
+                  [-0.5, -1.5, -2.5, -3.51, 1e10, -3e9]], dtype=np.float32)
+    # 1e10 = 2^10 * 9765625 and 3e9 = 2^9 * 5859375 are fp32 values (odd parts < 2^24)
+    assert o.round_int_tensor(c, 32).tolist() == [[0, 2, 2, 3, 7, 16777216],
+                                                  [0, -2, -2, -4, 2147483647, -2147483647]]
+    assert o.round_int_tensor(c, 64).tolist() == [[0, 2, 2, 3, 7, 16777216],
+                                                  [0, -2, -2, -4, 10000000000, -3000000000]]
+    # the edges: 2^31 itself saturates to 2^31 - 1 (and -2^31 to -(2^31 - 1)); the largest fp32 below 2^31 does not
+    e = np.array([[2147483648.0, -2147483648.0, 2147483520.0, -2147483520.0]], dtype=np.float32)
+    assert o.round_int_tensor(e, 32).tolist() == [[2147483647, -2147483647, 2147483520, -2147483520]]
+    assert o.round_int_tensor(e, 64).tolist() == [[2147483648, -2147483648, 2147483520, -2147483520]]
+    e = np.array([[2.0 ** 63, -2.0 ** 63, 1e30, -1e30, 2.0 ** 62]], dtype=np.float32)
+    assert o.round_int_tensor(e, 64).tolist() == [[2 ** 63 - 1, -(2 ** 63 - 1), 2 ** 63 - 1, -(2 ** 63 - 1), 2 ** 62]]
+    # the class operand is the prefix d < D_eff, as int64
+    C = np.array([[2.5, -7.0, 1000.0], [0.5, 3.5, -1000.0]], dtype=np.float32)
+    for hv in (o.HV_I32, o.HV_I64):
+        got = o.class_operand(C, 2, hv)
+        assert got.dtype == np.int64 and got.tolist() == [[2, -7], [0, 4]]
+
+
+def test_int32_int64_similarity_brute_force_and_identities():
+    """hv codes HV_I32 / HV_I64 through similarity(): DOT = the python-integer sum of v*q over d < D_eff
+    (beyond 2^53 for the 64-bit codes: a float64 contraction would round there), COS = DOT / (sqrt(D_eff) |q|);
+    for integer accumulators the scores of hv_bits = 32 are reproduced exactly, and the two widths agree
+    wherever the 32-bit codes do not saturate."""
+    r = rng(220)
+    N, K, D, D_eff = 6, 4, 90, 77
+    hb = r.integers(0, 2, size=(N, D), dtype=np.uint8)
+    for hv, mag in ((o.HV_I32, 1.2e9), (o.HV_I64, 2.0 ** 52)):
+        C = (r.standard_normal((K, D)) * mag).astype(np.float32)
+        C[1, 3] = 0.5                                    # a tie (-> 0) and a non-integer (-> rint) among them
+        C[2, 5] = -1234.5
+        w = 32 if hv == o.HV_I32 else 64
+        lim = 2 ** (w - 1) - 1
+        q = [[max(-lim, min(lim, int(round(float(C[k, d]))))) for d in range(D_eff)] for k in range(K)]  # python round: half-even, exact ints
+        assert hv == o.HV_I64 or any(abs(v) == lim for row in q for v in row)   # the 32-bit case does saturate
+        dot = o.similarity(hb, C, D_eff, o.SIM_DOT, hv)
+        cos = o.similarity(hb, C, D_eff, o.SIM_COS, hv)
+        assert dot.dtype == np.int64
+        big = 0
+        for n in range(N):
+            for k in range(K):
+                acc = sum((1 - 2 * int(hb[n, d])) * q[k][d] for d in range(D_eff))
+                assert int(dot[n, k]) == acc
+                big = max(big, abs(acc))
+                nrm = float(sum(v * v for v in q[k])) ** 0.5
+                assert abs(cos[n, k] - acc / (D_eff ** 0.5 * nrm)) <= 1e-12 * abs(cos[n, k]) + 1e-300
+        assert hv == o.HV_I32 or big > 2 ** 53
+    # integer accumulators as training leaves them: the integer operand IS the accumulator
+    Ci = r.integers(-5000, 5001, size=(K, D)).astype(np.float32)
+    want = o.similarity(hb, Ci, D_eff, o.SIM_DOT, 32)
+    for hv in (o.HV_I32, o.HV_I64):
+        assert np.array_equal(o.similarity(hb, Ci, D_eff, o.SIM_DOT, hv).astype(np.float64), want)
+        assert np.allclose(o.similarity(hb, Ci, D_eff, o.SIM_COS, hv), o.similarity(hb, Ci, D_eff, o.SIM_COS, 32),
+                           rtol=1e-14, atol=0)
+        lab, best, second = o.classify(o.similarity(hb, Ci, D_eff, o.SIM_DOT, hv), o.SIM_DOT)
+        lab32, best32, second32 = o.classify(want, o.SIM_DOT)
+        assert np.array_equal(lab, lab32) and np.array_equal(best, best32) and np.array_equal(second, second32)
+    # a zero class row has cosine 0 (A8), perforation gathers the visited dimensions (A17)
+    Cz = Ci.copy()
+    Cz[2] = 0.0
+    assert np.all(o.similarity(hb, Cz, D_eff, o.SIM_COS, o.HV_I32)[:, 2] == 0.0)
+    idx = np.arange(3, D_eff, 4)
+    assert np.array_equal(o.similarity(hb, Ci, D_eff, o.SIM_DOT, o.HV_I64, 3, 4),
+                          o.similarity(hb[:, idx], Ci[:, idx], len(idx), o.SIM_DOT, o.HV_I64))
