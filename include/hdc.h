@@ -59,12 +59,12 @@ typedef enum {
 } hdc_status;
 
 /* element types of buffers */
-enum { HDC_F32 = 0, HDC_BF16 = 1, HDC_I8 = 2, HDC_B1 = 3, HDC_U8 = 4, HDC_I32 = 5, HDC_F16 = 6 };
+enum { HDC_F32 = 0, HDC_BF16 = 1, HDC_I8 = 2, HDC_B1 = 3, HDC_U8 = 4, HDC_I32 = 5, HDC_F16 = 6, HDC_I64 = 7 };
 /* similarity kinds (L167 algorithmic choice) */
 enum { HDC_SIM_DOT = 0, HDC_SIM_COS = 1, HDC_SIM_HAMMING = 2 };
-/* knobs.hv_bits codes (not widths): 16-bit IEEE half class operand (L165 "FP16"); 16-bit integer class
- * operand (L165 "integer data types (8, 16, 32, or 64-bit)") */
-enum { HDC_HV_F16 = 17, HDC_HV_I16 = 18 };
+/* knobs.hv_bits codes (not widths): 16-bit IEEE half class operand (L165 "FP16"); 16-, 32- and 64-bit
+ * integer class operands (L165 "integer data types (8, 16, 32, or 64-bit)") */
+enum { HDC_HV_F16 = 17, HDC_HV_I16 = 18, HDC_HV_I32 = 19, HDC_HV_I64 = 20 };
 /* hdc_train_epoch modes */
 enum { HDC_TRAIN_BUNDLE = 0, HDC_TRAIN_PERCEPTRON = 1, HDC_TRAIN_KMEANS = 2 };
 /* hdc_encode_rp outputs (bit-or) */
@@ -106,6 +106,11 @@ enum {
  *             overflows, outside the contract) | 8 int8 (per-tensor symmetric over k<K, d<D_eff)
  *             | HDC_HV_I16 int16 (per-tensor symmetric over k<K, d<D_eff: s = 32767/max|c|,
  *             q = clamp(rint(c*s), +-32767); int32 accumulate, exact: D_eff*32767 < 2^31)
+ *             | HDC_HV_I32 / HDC_HV_I64 32- / 64-bit integers: the accumulators themselves,
+ *             q = rint(c) (half to even), NO scale, saturating at +-(2^31 - 1) / +-(2^63 - 1); scores
+ *             are exact integers accumulated in 64 bits (contract: sum_d |q[k,d]| < 2^63, beyond it the
+ *             sums wrap), DOT / COS only; contracted on the integer dot-product units (dp4a over the
+ *             byte planes of the codes), not on the tensor cores
  *             | 1 sign bit [C_acc < 0].  Query hypervectors are always bipolar (packed bits).
  *  sim        HDC_SIM_*; HDC_SIM_HAMMING requires hv_bits == 1.
  *  flags      HDC_FLAG_*.
@@ -222,7 +227,9 @@ int32_t hdc_encode_levelid_u16(hdc_handle_t h, const uint16_t* levels, int64_t N
  *   DOT      s[n,k]   = sum_d v[n,d]*c[k,d]                               -> S fp32 (int32 if hv_bits 8, HDC_HV_I16 or 1)
  *   COS      s[n,k]   = DOT / (sqrt(D_eff) * sqrt(sum_d c[k,d]^2)), 0 if the norm is 0   -> S fp32
  * s_dtype must be HDC_I32 for HAMMING, HDC_F32 for COS, HDC_F32 or HDC_I32 for DOT (HDC_I32 only
- * for hv_bits 8, HDC_HV_I16 or 1; fp32 scores of an int16 operand are the exact int32 sum rounded once). */
+ * for hv_bits 8, HDC_HV_I16 or 1; fp32 scores of an int16 operand are the exact int32 sum rounded once).
+ * hv_bits HDC_HV_I32 / HDC_HV_I64: DOT writes HDC_F32 (the exact 64-bit sum rounded once) or HDC_I64
+ * (S int64 [N][lds], 8-byte aligned), COS writes HDC_F32. */
 int32_t hdc_similarity(hdc_handle_t h, const uint32_t* Hbits, int64_t N, int64_t ldh_words,
                        const float* C_acc, int32_t K, int64_t ldc, int32_t D,
                        const hdc_knobs_t* knobs, void* S, int32_t s_dtype, int64_t lds, void* ws,

@@ -16,7 +16,7 @@ _LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "lib", "lib
 HDC_OK = 0
 HDC_ERR_INVALID_ARG, HDC_ERR_UNSUPPORTED, HDC_ERR_ALIGNMENT = -1, -2, -3
 HDC_ERR_WORKSPACE, HDC_ERR_CUDA, HDC_ERR_ARCH = -4, -5, -6
-HDC_F32, HDC_BF16, HDC_I8, HDC_B1, HDC_U8, HDC_I32, HDC_F16 = 0, 1, 2, 3, 4, 5, 6
+HDC_F32, HDC_BF16, HDC_I8, HDC_B1, HDC_U8, HDC_I32, HDC_F16, HDC_I64 = 0, 1, 2, 3, 4, 5, 6, 7
 HDC_SIM_DOT, HDC_SIM_COS, HDC_SIM_HAMMING = 0, 1, 2
 HDC_TRAIN_BUNDLE, HDC_TRAIN_PERCEPTRON, HDC_TRAIN_KMEANS = 0, 1, 2
 HDC_OUT_BITS, HDC_OUT_RAW = 1, 4
@@ -26,6 +26,7 @@ HDC_FLAG_NONE, HDC_FLAG_SIMT, HDC_FLAG_TC_1CTA, HDC_FLAG_TC_2CTA, HDC_FLAG_F32_F
 HDC_FLAG_FUSED_INFER = 16
 HDC_HV_F16 = 17
 HDC_HV_I16 = 18
+HDC_HV_I32, HDC_HV_I64 = 19, 20
 HDC_K_ENCODE_GEMM, HDC_K_SIM, HDC_K_LEVELID, HDC_K_CLASS_UPDATE = 0, 1, 2, 3
 HDC_STAT_TC_LAUNCHES, HDC_STAT_SIMT_FALLBACKS, HDC_STAT_INFER_FUSED, HDC_STAT_INFER_UNFUSED = 0, 1, 2, 3
 
@@ -144,7 +145,7 @@ def knobs(D_eff: int, precision: int = HDC_F32, hv_bits: int = 32, sim: int = HD
 
 
 _DT = {torch.float32: HDC_F32, torch.bfloat16: HDC_BF16, torch.int8: HDC_I8, torch.uint8: HDC_U8,
-       torch.int32: HDC_I32}
+       torch.int32: HDC_I32, torch.int64: HDC_I64}
 
 
 def _ptr(t):

@@ -15,7 +15,7 @@ ROOT = os.path.dirname(PKG)
 CSRC = os.path.join(PKG, "csrc")
 OBJ = os.path.join(ROOT, "build", "obj")
 LIB = os.path.join(PKG, "lib", "libhdc.so")
-SOURCES = ["adc.cu", "api.cu", "convert.cu", "gemm_simt.cu", "gemm_tc.cu", "hamming.cu", "levelid.cu", "simtc.cu", "train.cu"]
+SOURCES = ["adc.cu", "api.cu", "convert.cu", "gemm_simt.cu", "gemm_tc.cu", "hamming.cu", "levelid.cu", "simtc.cu", "train.cu", "widedot.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-I" + os.path.join(ROOT, "include"), "-I" + CSRC]
 

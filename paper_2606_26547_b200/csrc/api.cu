@@ -111,8 +111,8 @@ int check_knobs(hdc_ctx* h, const hdc_knobs_t* k, int D) {
 }
 int check_sim_knobs(hdc_ctx* h, const hdc_knobs_t* k) {
   if (k->hv_bits != 32 && k->hv_bits != 16 && k->hv_bits != HDC_HV_F16 && k->hv_bits != HDC_HV_I16 &&
-      k->hv_bits != 8 && k->hv_bits != 1)
-    return fail(h, HDC_ERR_INVALID_ARG, "hv_bits must be 32, 16, HDC_HV_F16, HDC_HV_I16, 8 or 1");
+      k->hv_bits != HDC_HV_I32 && k->hv_bits != HDC_HV_I64 && k->hv_bits != 8 && k->hv_bits != 1)
+    return fail(h, HDC_ERR_INVALID_ARG, "hv_bits must be 32, 16, HDC_HV_F16, HDC_HV_I16, HDC_HV_I32, HDC_HV_I64, 8 or 1");
   if (k->sim != HDC_SIM_DOT && k->sim != HDC_SIM_COS && k->sim != HDC_SIM_HAMMING)
     return fail(h, HDC_ERR_INVALID_ARG, "bad sim");
   if (k->sim == HDC_SIM_HAMMING && k->hv_bits != 1)
@@ -121,6 +121,7 @@ int check_sim_knobs(hdc_ctx* h, const hdc_knobs_t* k) {
     return fail(h, HDC_ERR_INVALID_ARG, "perforation: need perf_stride >= 0 and 0 <= perf_begin < D_eff");
   return HDC_OK;
 }
+bool wide_int(const hdc_knobs_t* k) { return k->hv_bits == HDC_HV_I32 || k->hv_bits == HDC_HV_I64; }
 Perf perf_of(const hdc_knobs_t* k) { return Perf{k->perf_begin, k->perf_stride <= 1 ? 1 : k->perf_stride}; }
 Perf enc_perf_of(const hdc_knobs_t* k) {
   return Perf{k->enc_perf_begin, k->enc_perf_stride <= 1 ? 1 : k->enc_perf_stride};
@@ -436,6 +437,35 @@ int do_similarity(hdc_ctx* h, const uint32_t* Hbits, int64_t N, int64_t ldh, con
   Bump& pm = persistent(h, b);   // class operand, scales, masks: per-call-invariant (prepared-model modes)
   bool prep = do_prep(h);
   auto too_small = [&]() { return fail(h, HDC_ERR_WORKSPACE, "similarity: workspace too small"); };
+  if (wide_int(k)) {
+    // 32- / 64-bit integer class codes (A22): byte planes + dp4a contraction with exact 64-bit sums (widedot.cu)
+    uint32_t* planes = pm.take<uint32_t>(wide_operand_bytes(K, k->hv_bits, D_eff) / sizeof(uint32_t));
+    double* colscale = pm.take<double>((size_t)K);
+    if (!persistent_fits(h, b, ws_bytes)) return too_small();
+    const int cos = k->sim == HDC_SIM_COS;
+    if (prep) {
+      ce = launch_wide_prepare(C_acc, K, ldc, D_eff, k->hv_bits, pf, cos, planes, colscale, st, &h->launches);
+      if (ce != cudaSuccess) return cuda_fail(h, ce, "wide-integer class operand");
+    }
+    if (prep_only(h)) return HDC_OK;
+    Epilogue e{};
+    if (labels) {
+      e.kind = EPI_ARGMAX;
+      e.labels = labels;
+      e.best = best;
+      e.second = second;
+    } else {
+      e.kind = EPI_SCORE;
+      e.S = S;
+      e.lds = lds;
+      e.s_i32 = s_i32;
+    }
+    {
+      Timed tm(h, HDC_K_SIM, st);
+      ce = launch_wide_dot(Hbits, N, ldh, K, D_eff, k->hv_bits, cos, planes, colscale, e, st, &h->launches);
+    }
+    return ce == cudaSuccess ? HDC_OK : cuda_fail(h, ce, "wide-integer similarity");
+  }
   // tensor-core path from packed queries: DOT / COS at any K; Hamming once K is large enough that
   // the popcount pipe would bound it (dist = (D_eff - dot)/2 is exact in int32)
   if (use_tc(h, k) && (k->sim != HDC_SIM_HAMMING || K >= 64)) {
@@ -572,6 +602,7 @@ void similarity_model_ws(int K, const hdc_knobs_t* k, Bump& pm) {
   pm.take<int8_t>((size_t)K * round_up(k->D_eff, 16) * 2);   // int8 or int16 codes
   pm.take<uint32_t>((size_t)K * W);
   pm.take<uint32_t>((size_t)W);  // perforation mask
+  pm.take<uint8_t>(wide_operand_bytes(K, k->hv_bits, k->D_eff));  // byte planes of 32- / 64-bit integer codes
   pm.take<uint8_t>(sim_tc_operand_bytes(K, k->hv_bits == 32 || k->hv_bits == 16 || k->hv_bits == HDC_HV_F16 ||
                                                k->hv_bits == HDC_HV_I16 || k->hv_bits == 8 ? k->hv_bits : 1,
                                         k->D_eff));
@@ -592,6 +623,7 @@ size_t similarity_ws(int64_t N, int K, const hdc_knobs_t* k) {
   b.take<uint32_t>((size_t)K * W);
   b.take<uint32_t>((size_t)W);  // perforation mask
   b.take<uint32_t>((size_t)((k->D_eff + 127) / 128) * 4 * K);  // [chunk][class] sign bits of hdc_similarity_adc
+  b.take<uint8_t>(wide_operand_bytes(K, k->hv_bits, k->D_eff));  // byte planes of 32- / 64-bit integer codes
   b.take<uint8_t>(sim_tc_operand_bytes(K, k->hv_bits == 32 || k->hv_bits == 16 || k->hv_bits == HDC_HV_F16 ||
                                                k->hv_bits == HDC_HV_I16 || k->hv_bits == 8 ? k->hv_bits : 1,
                                        k->D_eff));
@@ -613,7 +645,7 @@ constexpr int64_t INFER_MIN_N = 12288;  // 48 row blocks of 256: below it the tw
 
 bool infer_fused_knobs(const hdc_ctx* h, const hdc_knobs_t* k, int K) {   // the part that does not depend on N
   // (int16 class codes: sums beyond 2^24, which the fp32 search of the fused epilogue does not hold exactly)
-  return (k->flags & HDC_FLAG_FUSED_INFER) && k->hv_bits != HDC_HV_I16 && use_tc(h, k) && !(k->flags & HDC_FLAG_TC_1CTA) && h->sm_count >= 2 &&
+  return (k->flags & HDC_FLAG_FUSED_INFER) && k->hv_bits != HDC_HV_I16 && !wide_int(k) && use_tc(h, k) && !(k->flags & HDC_FLAG_TC_1CTA) && h->sm_count >= 2 &&
          K <= INFER_MAX_K && k->D_eff <= (1 << 17);
 }
 int infer_kc(int K) { return K <= 8 ? 8 : (K <= 16 ? 16 : 32); }
@@ -735,7 +767,7 @@ size_t infer_ws_bytes(const hdc_ctx* h, int64_t N, int F, int K, const hdc_knobs
 using namespace hdc;
 
 // =================================================================================== handle
-extern "C" int32_t hdc_version(void) { return 104; }  // 1.4: + HDC_HV_I16, hdc_classify_hamming_static
+extern "C" int32_t hdc_version(void) { return 105; }  // 1.5: + HDC_HV_I32 / HDC_HV_I64, HDC_I64 scores
 
 extern "C" int32_t hdc_create(hdc_handle_t* out, int32_t device) {
   if (!out) return HDC_ERR_INVALID_ARG;
@@ -989,7 +1021,12 @@ extern "C" int32_t hdc_similarity(hdc_handle_t h, const uint32_t* Hbits, int64_t
   if (knobs->sim == HDC_SIM_HAMMING && s_dtype != HDC_I32)
     return fail(h, HDC_ERR_INVALID_ARG, "similarity: HAMMING writes int32");
   if (knobs->sim == HDC_SIM_COS && s_dtype != HDC_F32) return fail(h, HDC_ERR_INVALID_ARG, "similarity: COS writes fp32");
-  if (knobs->sim == HDC_SIM_DOT) {
+  if (wide_int(knobs)) {
+    if (s_dtype != HDC_F32 && !(s_dtype == HDC_I64 && knobs->sim == HDC_SIM_DOT))
+      return fail(h, HDC_ERR_INVALID_ARG, "similarity: 32- / 64-bit integer classes write fp32, or int64 for DOT");
+    if (s_dtype == HDC_I64 && (reinterpret_cast<uintptr_t>(S) & 7))
+      return fail(h, HDC_ERR_ALIGNMENT, "similarity: int64 scores must be 8-byte aligned");
+  } else if (knobs->sim == HDC_SIM_DOT) {
     if (s_dtype != HDC_F32 && s_dtype != HDC_I32) return fail(h, HDC_ERR_INVALID_ARG, "similarity: s_dtype");
     if (s_dtype == HDC_I32 && knobs->hv_bits != 8 && knobs->hv_bits != 1 && knobs->hv_bits != HDC_HV_I16)
       return fail(h, HDC_ERR_INVALID_ARG, "similarity: int32 DOT needs hv_bits 8, HDC_HV_I16 or 1");
@@ -997,7 +1034,7 @@ extern "C" int32_t hdc_similarity(hdc_handle_t h, const uint32_t* Hbits, int64_t
   if (N == 0) return HDC_OK;
   Bump b(ws);
   if (!ws) ws_bytes = 0;
-  return do_similarity(h, Hbits, N, ldh_words, C_acc, K, ldc, knobs, S, s_dtype == HDC_I32, lds, nullptr,
+  return do_similarity(h, Hbits, N, ldh_words, C_acc, K, ldc, knobs, S, s_dtype == HDC_I32 ? 1 : (s_dtype == HDC_I64 ? 2 : 0), lds, nullptr,
                        nullptr, nullptr, b, ws_bytes, (cudaStream_t)stream);
 }
 

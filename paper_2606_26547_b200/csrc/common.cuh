@@ -54,7 +54,7 @@ struct Epilogue {
   int64_t ldbits;
   void* raw;  // float* (float accumulate) or int32_t* (integer accumulate), nullable
   int64_t ldraw;
-  // EPI_SCORE: S[m,n] = acc * colscale[n] (colscale nullable => 1); s_i32 => store as int32
+  // EPI_SCORE: S[m,n] = acc * colscale[n] (colscale nullable => 1); s_i32 = 1 => store as int32 (2: int64, widedot.cu only)
   void* S;
   int64_t lds;
   int s_i32;
@@ -183,6 +183,17 @@ cudaError_t launch_sign_bits(const float* C, int K, int D_eff, int64_t ldc, uint
 // colscale_f (nullable): receives (float)colscale[k]
 cudaError_t launch_col_scale(const Operand& C, int K, int D_eff, int cos, Perf pf, double* colscale,
                              cudaStream_t st, int64_t* nlaunch, float* colscale_f = nullptr);
+
+// 32- / 64-bit integer class operands (widedot.cu; hv codes HDC_HV_I32 / HDC_HV_I64, reading A22): the codes
+// rint(C_acc) staged as byte planes (wide_operand_bytes; 0 for any other hv_bits) with the cosine scales, and
+// the dp4a contraction of packed queries against them (e.kind EPI_ARGMAX, or EPI_SCORE with e.s_i32 = 0 for
+// fp32 scores, 2 for int64 scores)
+size_t wide_operand_bytes(int K, int hv_bits, int D_eff);
+cudaError_t launch_wide_prepare(const float* C_acc, int K, int64_t ldc, int D_eff, int hv_bits, Perf pf, int cos,
+                                uint32_t* planes, double* colscale, cudaStream_t st, int64_t* nlaunch);
+cudaError_t launch_wide_dot(const uint32_t* Hbits, int64_t N, int64_t ldh, int K, int D_eff, int hv_bits, int cos,
+                            const uint32_t* planes, const double* colscale, const Epilogue& e, cudaStream_t st,
+                            int64_t* nlaunch);
 
 // packed XOR+popcount similarity with class bits in shared memory (hamming.cu)
 // mask (nullable): W words; distances count only the bits set in it (reduction perforation)

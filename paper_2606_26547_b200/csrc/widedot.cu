@@ -1,0 +1,276 @@
+// widedot.cu -- DOT / COS similarity and arg-max of packed queries against class operands held as 32- or
+// 64-bit integers (hv codes HDC_HV_I32 / HDC_HV_I64; "integer data types (8, 16, 32, or
+// 64-bit)"; reading A22: q = rint(C_acc), no scale, symmetric saturation).
+//
+//   s[n,k] = sum_{d visited, d < D_eff} (1 - 2 b[n,d]) * q[k,d]        exact, in 64-bit integers
+//
+// The contraction runs on the integer dot-product instruction: the two's-complement bytes of the codes are
+// staged once per model as BYTE PLANES -- for every group of four dimensions ("quad") P = 4 or 8 words, word p
+// holding byte p of the four codes -- so that one dp4a multiplies four +-1 query bytes with four code bytes
+// (unsigned for the lower planes, signed for the top one) into an int32 per-plane sum (|.| <= 255 * D_eff),
+// and the sums of the planes are recombined as sum_p acc_p << 8p in 64 bits when a class is finished.
+// Unvisited (perforated) dimensions and the padding beyond D_eff are staged as zero codes: no masks in the loop.
+//
+// Thread = query; a CTA of 128 queries walks the reduction axis in chunks of 512 dimensions (16 query words
+// per row through a padded shared-memory tile, 128 quads of KC classes as broadcast 16-byte reads) with KC x P
+// accumulators in registers; classes beyond KC take further passes over the query rows (L2-resident).
+// Bound: the dp4a issue rate -- N * K * D_eff * P / 4 instructions per call.
+#include <limits.h>
+
+#include "common.cuh"
+
+namespace hdc {
+namespace {
+
+constexpr int WQ = 128;        // queries per CTA
+constexpr int CHUNK_W = 16;    // query words per chunk (512 dimensions = 128 quads)
+constexpr int CHUNK_Q = CHUNK_W * 8;
+
+__device__ __forceinline__ int dp4a_su(uint32_t a, uint32_t b, int c) {   // signed a bytes x unsigned b bytes
+  int d;
+  asm("dp4a.s32.u32 %0, %1, %2, %3;" : "=r"(d) : "r"(a), "r"(b), "r"(c));
+  return d;
+}
+__device__ __forceinline__ int dp4a_ss(uint32_t a, uint32_t b, int c) {
+  int d;
+  asm("dp4a.s32.s32 %0, %1, %2, %3;" : "=r"(d) : "r"(a), "r"(b), "r"(c));
+  return d;
+}
+
+// ---------------------------------------------------------------------------------- preparation
+// One block per class: codes -> byte planes [K][quads_ld][P] words, and the cosine scale
+// 1 / (sqrt(n_vis) * |q|) (0 for a zero row; 1 for DOT), norm summed in double in a fixed order.
+__global__ void wide_prepare_kernel(const float* __restrict__ C, int D_eff, int64_t ldc, Perf pf, int P,
+                                    uint32_t* __restrict__ planes, int quads_ld, int cos, int n_vis,
+                                    double* __restrict__ colscale) {
+  const int k = blockIdx.x;
+  const long long lim = P == 4 ? 2147483647LL : 9223372036854775807LL;
+  __shared__ double part[32];
+  double ss = 0.0;
+  for (int qd = threadIdx.x; qd < quads_ld; qd += blockDim.x) {
+    unsigned long long code[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const int d = qd * 4 + i;
+      long long q = 0;
+      if (d < D_eff && perf_visits(pf, d)) {
+        q = __float2ll_rn(__ldg(C + (int64_t)k * ldc + d));   // round half to even, saturates at the int64 range
+        q = q > lim ? lim : (q < -lim ? -lim : q);
+      }
+      code[i] = (unsigned long long)q;
+      const double v = (double)q;
+      ss += v * v;
+    }
+    uint32_t* dst = planes + ((int64_t)k * quads_ld + qd) * P;
+    for (int p = 0; p < P; ++p) {
+      const int sh = 8 * p;
+      dst[p] = (uint32_t)((code[0] >> sh) & 0xFFu) | (uint32_t)((code[1] >> sh) & 0xFFu) << 8 |
+               (uint32_t)((code[2] >> sh) & 0xFFu) << 16 | (uint32_t)((code[3] >> sh) & 0xFFu) << 24;
+    }
+  }
+#pragma unroll
+  for (int off = 16; off; off >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, off);
+  if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = ss;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double t = 0.0;
+    for (int i = 0; i < (int)(blockDim.x >> 5); ++i) t += part[i];
+    const double nrm = sqrt(t);
+    colscale[k] = !cos ? 1.0 : (nrm > 0.0 ? 1.0 / (sqrt((double)n_vis) * nrm) : 0.0);
+  }
+}
+
+// ---------------------------------------------------------------------------------- contraction
+struct WideParams {
+  const uint32_t* H;
+  int64_t N, ldh;
+  int W;                      // query words per row that carry visited dimensions
+  const uint32_t* planes;
+  int quads_ld;
+  int K;
+  const double* colscale;     // [K]; all ones for DOT
+  int cos;
+  // arg-max outputs (labels != NULL) or scores
+  int32_t* labels;
+  float* best;
+  float* second;
+  void* S;
+  int64_t lds;
+  int s_mode;                 // 0 fp32, 2 int64
+};
+
+template <int P>
+__device__ __forceinline__ long long recombine(const int (&a)[P]) {
+  unsigned long long s = 0;
+#pragma unroll
+  for (int p = 0; p < P; ++p) s += (unsigned long long)(long long)a[p] << (8 * p);
+  return (long long)s;
+}
+
+template <int P, int KC>
+__global__ void __launch_bounds__(WQ) wide_dot_kernel(const WideParams p) {
+  constexpr int V = P / 4;                                  // 16-byte vectors per quad
+  __shared__ uint32_t sq[WQ][CHUNK_W + 1];
+  __shared__ uint4 sc[KC][CHUNK_Q][V];
+  const int t = threadIdx.x;
+  const int64_t n0 = (int64_t)blockIdx.x * WQ;
+  const int64_t n = n0 + t;
+
+  // running arg-max state of this thread's query: exact integers for DOT, doubles for COS
+  long long bi1 = LLONG_MIN, bi2 = LLONG_MIN;
+  double bd1 = -1.0e300, bd2 = -1.0e300;
+  int lab = 0;
+
+  for (int kg = 0; kg < p.K; kg += KC) {
+    int acc[KC][P];
+#pragma unroll
+    for (int k = 0; k < KC; ++k)
+#pragma unroll
+      for (int j = 0; j < P; ++j) acc[k][j] = 0;
+
+    for (int c0 = 0; c0 < p.W; c0 += CHUNK_W) {
+      __syncthreads();   // the previous chunk's readers are done
+#pragma unroll
+      for (int j = 0; j < CHUNK_W; ++j) {
+        const int i = t + WQ * j;
+        const int r = i / CHUNK_W, w = i % CHUNK_W;
+        int64_t row = n0 + r;
+        if (row >= p.N) row = p.N - 1;
+        sq[r][w] = (c0 + w < p.W) ? __ldg(p.H + row * p.ldh + c0 + w) : 0u;
+      }
+      for (int i = t; i < KC * CHUNK_Q * V; i += WQ) {
+        const int k = i / (CHUNK_Q * V), rem = i % (CHUNK_Q * V);
+        uint4 v = make_uint4(0u, 0u, 0u, 0u);
+        if (kg + k < p.K)
+          v = __ldg(reinterpret_cast<const uint4*>(p.planes + ((int64_t)(kg + k) * p.quads_ld + (int64_t)c0 * 8) * P) + rem);
+        (&sc[k][0][0])[rem] = v;
+      }
+      __syncthreads();
+#pragma unroll 1
+      for (int w = 0; w < CHUNK_W; ++w) {
+        const uint32_t qw = sq[t][w];
+#pragma unroll
+        for (int nib = 0; nib < 8; ++nib) {
+          // bit i of the nibble -> byte i: 0x01 (bit 0: +1) or 0xFF (bit 1: -1)
+          const uint32_t spread = (((qw >> (4 * nib)) & 0xFu) * 0x00204081u) & 0x01010101u;
+          const uint32_t a = spread * 0xFEu + 0x01010101u;
+#pragma unroll
+          for (int k = 0; k < KC; ++k) {
+#pragma unroll
+            for (int v = 0; v < V; ++v) {
+              const uint4 c = sc[k][w * 8 + nib][v];
+              const bool top = v == V - 1;
+              acc[k][4 * v + 0] = dp4a_su(a, c.x, acc[k][4 * v + 0]);
+              acc[k][4 * v + 1] = dp4a_su(a, c.y, acc[k][4 * v + 1]);
+              acc[k][4 * v + 2] = dp4a_su(a, c.z, acc[k][4 * v + 2]);
+              acc[k][4 * v + 3] = top ? dp4a_ss(a, c.w, acc[k][4 * v + 3]) : dp4a_su(a, c.w, acc[k][4 * v + 3]);
+            }
+          }
+        }
+      }
+    }
+
+#pragma unroll
+    for (int k = 0; k < KC; ++k) {
+      const int cls = kg + k;
+      if (cls >= p.K) break;
+      const long long s = recombine<P>(acc[k]);
+      if (p.labels) {
+        if (p.cos) {
+          const double v = (double)s * p.colscale[cls];
+          if (v > bd1) {
+            bd2 = bd1;
+            bd1 = v;
+            lab = cls;
+          } else if (v > bd2) {
+            bd2 = v;
+          }
+        } else {
+          if (s > bi1) {      // ties keep the lower index: classes arrive in ascending order
+            bi2 = bi1;
+            bi1 = s;
+            lab = cls;
+          } else if (s > bi2) {
+            bi2 = s;
+          }
+        }
+      } else if (n < p.N) {
+        if (p.s_mode == 2)
+          reinterpret_cast<long long*>(p.S)[n * p.lds + cls] = s;
+        else
+          reinterpret_cast<float*>(p.S)[n * p.lds + cls] = p.cos ? (float)((double)s * p.colscale[cls]) : (float)s;
+      }
+    }
+  }
+
+  if (p.labels && n < p.N) {
+    p.labels[n] = lab;
+    float b1, b2;
+    if (p.cos) {
+      b1 = (float)bd1;
+      b2 = p.K > 1 ? (float)bd2 : b1;
+    } else {
+      b1 = (float)bi1;
+      b2 = p.K > 1 ? (float)bi2 : b1;
+    }
+    if (p.best) p.best[n] = b1;
+    if (p.second) p.second[n] = b2;
+  }
+}
+
+}  // namespace
+
+static inline int wide_planes(int hv_bits) { return hv_bits == HDC_HV_I32 ? 4 : (hv_bits == HDC_HV_I64 ? 8 : 0); }
+static inline int wide_quads_ld(int D_eff) { return (int)round_up((D_eff + 3) / 4, CHUNK_Q); }
+
+size_t wide_operand_bytes(int K, int hv_bits, int D_eff) {
+  const int P = wide_planes(hv_bits);
+  return P ? (size_t)K * (size_t)wide_quads_ld(D_eff) * P * sizeof(uint32_t) : 0;
+}
+
+cudaError_t launch_wide_prepare(const float* C_acc, int K, int64_t ldc, int D_eff, int hv_bits, Perf pf, int cos,
+                                uint32_t* planes, double* colscale, cudaStream_t st, int64_t* nlaunch) {
+  const int P = wide_planes(hv_bits);
+  if (!P) return cudaErrorInvalidValue;
+  wide_prepare_kernel<<<K, 256, 0, st>>>(C_acc, D_eff, ldc, pf, P, planes, wide_quads_ld(D_eff), cos,
+                                         perf_count(pf, D_eff), colscale);
+  *nlaunch += 1;
+  return cudaGetLastError();
+}
+
+cudaError_t launch_wide_dot(const uint32_t* Hbits, int64_t N, int64_t ldh, int K, int D_eff, int hv_bits, int cos,
+                            const uint32_t* planes, const double* colscale, const Epilogue& e, cudaStream_t st,
+                            int64_t* nlaunch) {
+  const int P = wide_planes(hv_bits);
+  if (!P) return cudaErrorInvalidValue;
+  if (N <= 0) return cudaSuccess;
+  WideParams p{};
+  p.H = Hbits;
+  p.N = N;
+  p.ldh = ldh;
+  p.W = words_of(D_eff);
+  p.planes = planes;
+  p.quads_ld = wide_quads_ld(D_eff);
+  p.K = K;
+  p.colscale = colscale;
+  p.cos = cos;
+  if (e.kind == EPI_ARGMAX) {
+    p.labels = e.labels;
+    p.best = e.best;
+    p.second = e.second;
+  } else {
+    p.S = e.S;
+    p.lds = e.lds;
+    p.s_mode = e.s_i32;
+  }
+  const int64_t blocks = (N + WQ - 1) / WQ;
+  if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
+  if (P == 4)
+    wide_dot_kernel<4, 8><<<(unsigned)blocks, WQ, 0, st>>>(p);
+  else
+    wide_dot_kernel<8, 4><<<(unsigned)blocks, WQ, 0, st>>>(p);
+  *nlaunch += 1;
+  return cudaGetLastError();
+}
+
+}  // namespace hdc

@@ -364,7 +364,8 @@ def test_bundle_exact(hd, h, N, K, D, D_eff):
 
 
 @pytest.mark.parametrize("B", [0, 1, 7, 64])
-@pytest.mark.parametrize("hv_bits,sim", [(1, "HAMMING"), (8, "COS"), (18, "COS"), (18, "DOT")])
+@pytest.mark.parametrize("hv_bits,sim", [(1, "HAMMING"), (8, "COS"), (18, "COS"), (18, "DOT"),
+                                         (19, "COS"), (19, "DOT"), (20, "DOT")])   # 19 / 20 = HDC_HV_I32 / HDC_HV_I64
 def test_perceptron_epoch_integer_paths_exact(hd, h, B, hv_bits, sim):
     """Integer similarity => identical predictions => identical Delta => identical fp32 update."""
     w = gen.c1_tiny(D=512)

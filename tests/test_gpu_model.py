@@ -51,6 +51,7 @@ CASES = [  # precision, flags, hv_bits, sim, K, perf (begin, stride), enc_perf (
     ("I8", 0, 1, "DOT", 200, (0, 1), (0, 1)), ("BF16", 1, 1, "DOT", 5, (0, 1), (0, 1)),
     ("BF16", 0, 18, "COS", 26, (0, 1), (0, 1)), ("I8", 0, 18, "DOT", 200, (2, 3), (0, 1)),   # 18 = HDC_HV_I16
     ("I8", 1, 18, "COS", 6, (0, 1), (0, 1)),
+    ("BF16", 0, 19, "COS", 26, (0, 1), (0, 1)), ("I8", 0, 20, "DOT", 200, (2, 3), (0, 1)),   # 19 / 20 = HDC_HV_I32 / _I64
 ]
 
 
@@ -90,7 +91,7 @@ def test_prepared_model_equals_plain_calls_and_the_oracle(hd, h, prec, flags, hv
     margin = np.abs(np.sort(S_or, axis=1)[:, -1] - np.sort(S_or, axis=1)[:, -2]) if K > 1 else np.ones(N)
     if sim == "HAMMING":
         margin = np.abs(np.sort(S_or, axis=1)[:, 0] - np.sort(S_or, axis=1)[:, min(1, K - 1)]) if K > 1 else np.ones(N)
-    clear = margin > 1e-3 * np.maximum(np.abs(best_or), 1e-30) if hv_bits not in (18, 8, 1) else np.ones(N, dtype=bool)
+    clear = margin > 1e-3 * np.maximum(np.abs(best_or), 1e-30) if hv_bits not in (20, 19, 18, 8, 1) else np.ones(N, dtype=bool)
     assert np.array_equal(lab1.cpu().numpy()[clear], lab_or[clear])
 
 
