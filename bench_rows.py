@@ -235,12 +235,12 @@ def row_point(h, peaks, reps, cfg, N, prec_name):
 
 
 # ------------------------------------------------------------------------------------ similarity rows
-def row_classify(h, peaks, reps, N, K, D, hv_bits, sim_name):
+def row_classify(h, peaks, reps, N, K, D, hv_bits, sim_name, flags=0):
     sim = {"cos": hd.HDC_SIM_COS, "dot": hd.HDC_SIM_DOT, "hamming": hd.HDC_SIM_HAMMING}[sim_name]
     W = (D + 31) // 32
     H = _rand_bits(N, W, "rows_query_bits")
     C = _class_acc(K, D, "rows_class_acc")
-    kn = hd.knobs(D, hv_bits=hv_bits, sim=sim)
+    kn = hd.knobs(D, hv_bits=hv_bits, sim=sim, flags=flags)
     lab = torch.empty(N, dtype=torch.int32, device="cuda")
     fn = lambda: h.hdc_classify(H, C, kn, labels=lab)  # noqa: E731
     call_ms = _time(fn, reps)
@@ -254,9 +254,19 @@ def row_classify(h, peaks, reps, N, K, D, hv_bits, sim_name):
         peak = 148 * 16 * peaks["sm_max_mhz"] * 1e6 / 1e12
         out["roofline"] = {"bound": "alu", "achieved": popc, "peak": peak, "unit": "Tpopc/s", "frac": popc / peak,
                            "peak_source": "148 SM x 16 POPC lanes x sm_max_mhz"}
+    elif hv_bits in (hd.HDC_HV_I32, hd.HDC_HV_I64) and (flags & hd.HDC_FLAG_SIMT):
+        # widedot.cu: one dp4a per (query, class, 4 dimensions, byte plane of the codes); the integer dot-product
+        # instruction issues at 64 lanes per clock and SM (measured: DESIGN.md section 6)
+        planes = 4 if hv_bits == hd.HDC_HV_I32 else 8
+        dp4a = float(N) * K * ((D + 3) // 4) * planes / (k_ms * 1e-3) / 1e12
+        peak = 148 * 64 * peaks["sm_max_mhz"] * 1e6 / 1e12
+        out["roofline"] = {"bound": "alu", "achieved": dp4a, "peak": peak, "unit": "Tdp4a/s", "frac": dp4a / peak,
+                           "peak_source": "148 SM x 64 dp4a lanes x sm_max_mhz"}
     else:
-        parts = 3 if hv_bits in (32, hd.HDC_HV_I16) else 1
-        mult = 2.0 if hv_bits in (hd.HDC_HV_I16, 8, 1) else 1.0
+        # (32- / 64-bit integer codes: two / four 16-bit pieces, each three base-128 digits on kind::i8; kernel_ms
+        # spans the pieces' contractions and the 64-bit recombination)
+        parts = {32: 3, hd.HDC_HV_I16: 3, hd.HDC_HV_I32: 6, hd.HDC_HV_I64: 12}.get(hv_bits, 1)
+        mult = 2.0 if hv_bits in (hd.HDC_HV_I16, hd.HDC_HV_I32, hd.HDC_HV_I64, 8, 1) else 1.0
         kp = ((K + 15) // 16) * 16
         flops = 2.0 * N * D * kp * parts
         ach = flops / (k_ms * 1e-3) / 1e12
@@ -422,7 +432,8 @@ def row_c5_classify(h, peaks, reps, hv_bits, sim_name, B=65536, F=1024, D=16384,
     k_ms, _ = _kernel(h, hd.HDC_K_SIM, fn, reps)
     # int16 class codes (hv code 18): algorithmic flops 2*B*D*K against the int8 tensor peak; the kernel executes
     # three int8 digit columns per class, so a third of that peak is its ceiling
-    mult = 2.0 if hv_bits in (hd.HDC_HV_I16, 8, 1) else 1.0
+    # (32-bit integer codes, hv code 19: two 16-bit pieces = six digit columns per class, a sixth of that peak)
+    mult = 2.0 if hv_bits in (hd.HDC_HV_I16, hd.HDC_HV_I32, hd.HDC_HV_I64, 8, 1) else 1.0
     flops = 2.0 * B * D * (((K + 15) // 16) * 16)
     ach = flops / (k_ms * 1e-3) / 1e12
     peak = peaks["bf16_tflops"] * mult
@@ -597,6 +608,11 @@ ROWS = {
     "c5_classify_i8": lambda h, p, r: row_c5_classify(h, p, r, 8, "cos"),
     "c5_classify_i16": lambda h, p, r: row_c5_classify(h, p, r, hd.HDC_HV_I16, "cos"),
     "c2_classify_cos_i16": lambda h, p, r: row_classify(h, p, r, 131072, 26, 10000, hd.HDC_HV_I16, "cos"),
+    "c2_classify_cos_i32": lambda h, p, r: row_classify(h, p, r, 131072, 26, 10000, hd.HDC_HV_I32, "cos"),
+    "c2_classify_dot_i64": lambda h, p, r: row_classify(h, p, r, 131072, 26, 10000, hd.HDC_HV_I64, "dot"),
+    "c2_classify_cos_i32_dp4a": lambda h, p, r: row_classify(h, p, r, 131072, 26, 10000, hd.HDC_HV_I32, "cos", hd.HDC_FLAG_SIMT),
+    "c2_classify_dot_i64_dp4a": lambda h, p, r: row_classify(h, p, r, 131072, 26, 10000, hd.HDC_HV_I64, "dot", hd.HDC_FLAG_SIMT),
+    "c5_classify_i32": lambda h, p, r: row_c5_classify(h, p, r, hd.HDC_HV_I32, "cos"),
     "c5_stream_bf16": lambda h, p, r: row_c5_stream(h, p, r, 16, "cos"),
     "c5_stream_1bit": lambda h, p, r: row_c5_stream(h, p, r, 1, "hamming"),
     "specpcm_adc_d1024": lambda h, p, r: row_adc(h, p, r, 131072, 26, 1024),

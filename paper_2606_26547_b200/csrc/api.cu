@@ -122,6 +122,23 @@ int check_sim_knobs(hdc_ctx* h, const hdc_knobs_t* k) {
   return HDC_OK;
 }
 bool wide_int(const hdc_knobs_t* k) { return k->hv_bits == HDC_HV_I32 || k->hv_bits == HDC_HV_I64; }
+// Rows per pass of the tensor-core route of the 32- / 64-bit integer class operands: the int32 scores of one 16-bit
+// piece of a pass ([rows][K]) stay around 32 MB (L2-resident between sim_tc_kernel and the combine kernel), but a
+// pass is never smaller than one wave of 128-row tiles on 148 SMs
+int64_t wide_chunk_rows(int64_t N, int K) {
+  int64_t rows = ((int64_t)8 << 20) / (K > 0 ? K : 1);
+  rows -= rows % 256;
+  if (rows < 18944) rows = 18944;
+  return N < rows ? (N > 0 ? N : 1) : rows;
+}
+// workspace of that route: persistent class pieces (pm) and per-pass piece scores (b)
+void wide_tc_ws(int64_t N, int K, const hdc_knobs_t* k, Bump* pm, Bump* b) {
+  if (!wide_int(k)) return;
+  const int pieces = k->hv_bits == HDC_HV_I32 ? 2 : 4;
+  if (pm)
+    for (int j = 0; j < pieces; ++j) pm->take<uint8_t>(sim_tc_operand_bytes(K, HDC_HV_I16, k->D_eff));
+  if (b) b->take<int32_t>((size_t)pieces * (size_t)wide_chunk_rows(N, K) * (size_t)K);
+}
 Perf perf_of(const hdc_knobs_t* k) { return Perf{k->perf_begin, k->perf_stride <= 1 ? 1 : k->perf_stride}; }
 Perf enc_perf_of(const hdc_knobs_t* k) {
   return Perf{k->enc_perf_begin, k->enc_perf_stride <= 1 ? 1 : k->enc_perf_stride};
@@ -438,16 +455,9 @@ int do_similarity(hdc_ctx* h, const uint32_t* Hbits, int64_t N, int64_t ldh, con
   bool prep = do_prep(h);
   auto too_small = [&]() { return fail(h, HDC_ERR_WORKSPACE, "similarity: workspace too small"); };
   if (wide_int(k)) {
-    // 32- / 64-bit integer class codes (A22): byte planes + dp4a contraction with exact 64-bit sums (widedot.cu)
-    uint32_t* planes = pm.take<uint32_t>(wide_operand_bytes(K, k->hv_bits, D_eff) / sizeof(uint32_t));
-    double* colscale = pm.take<double>((size_t)K);
-    if (!persistent_fits(h, b, ws_bytes)) return too_small();
+    // 32- / 64-bit integer class codes (A22), exact 64-bit sums.
     const int cos = k->sim == HDC_SIM_COS;
-    if (prep) {
-      ce = launch_wide_prepare(C_acc, K, ldc, D_eff, k->hv_bits, pf, cos, planes, colscale, st, &h->launches);
-      if (ce != cudaSuccess) return cuda_fail(h, ce, "wide-integer class operand");
-    }
-    if (prep_only(h)) return HDC_OK;
+    const int width = k->hv_bits == HDC_HV_I32 ? 32 : 64;
     Epilogue e{};
     if (labels) {
       e.kind = EPI_ARGMAX;
@@ -460,6 +470,69 @@ int do_similarity(hdc_ctx* h, const uint32_t* Hbits, int64_t N, int64_t ldh, con
       e.lds = lds;
       e.s_i32 = s_i32;
     }
+    double* colscale = pm.take<double>((size_t)K);
+    // Tensor-core route: the codes as balanced base-65536 pieces, each staged like an int16 operand (three base-128
+    // digits on tcgen05 kind::i8, exact int32 scores per piece: D_eff * 32768 < 2^31) and contracted by sim_tc_kernel
+    // over row chunks; the pieces' scores are recombined in 64 bits by wide_combine_kernel.
+    if (use_tc(h, k) && D_eff <= 65535) {
+      const int pieces = width / 16;
+      const size_t cop_bytes = sim_tc_operand_bytes(K, HDC_HV_I16, D_eff);
+      void* cop[4];
+      for (int j = 0; j < pieces; ++j) cop[j] = pm.take<uint8_t>(cop_bytes);
+      const int64_t rows_max = wide_chunk_rows(N, K);
+      int32_t* Sp = b.take<int32_t>((size_t)pieces * (size_t)rows_max * (size_t)K);
+      if (!persistent_fits(h, b, ws_bytes)) return too_small();
+      bool ok = true;
+      if (prep) {
+        ce = launch_wide_prepare(C_acc, K, ldc, D_eff, k->hv_bits, pf, cos, nullptr, colscale, st, &h->launches);
+        if (ce != cudaSuccess) return cuda_fail(h, ce, "wide-integer cosine scales");
+        Epilogue none{};
+        none.kind = EPI_SCORE;
+        for (int j = 0; j < pieces && ok; ++j) {
+          ce = launch_sim_tc(h->tc, Hbits, 0, ldh, C_acc, K, ldc, D_eff, HDC_HV_I16, cop[j], nullptr, none, pf, nullptr,
+                             false, true, h->sm_count, tc_cta_group(k), st, &h->launches, j + 1, width);
+          if (ce == cudaErrorNotSupported) ok = false;
+          else if (ce != cudaSuccess) return cuda_fail(h, ce, "wide-integer class pieces");
+        }
+      }
+      if (ok && prep_only(h)) return HDC_OK;
+      if (ok) {
+        Timed tm(h, HDC_K_SIM, st);
+        for (int64_t r0 = 0; r0 < N && ok; r0 += rows_max) {
+          const int64_t rows = N - r0 < rows_max ? N - r0 : rows_max;
+          for (int j = 0; j < pieces && ok; ++j) {
+            Epilogue es{};
+            es.kind = EPI_SCORE;
+            es.S = Sp + (size_t)j * (size_t)rows * (size_t)K;
+            es.lds = K;
+            es.s_i32 = 1;
+            ce = launch_sim_tc(h->tc, Hbits + r0 * ldh, rows, ldh, C_acc, K, ldc, D_eff, HDC_HV_I16, cop[j], nullptr, es,
+                               pf, nullptr, true, false, h->sm_count, tc_cta_group(k), st, &h->launches, j + 1, width);
+            if (ce == cudaErrorNotSupported && r0 == 0 && j == 0) ok = false;
+            else if (ce != cudaSuccess) return cuda_fail(h, ce, "wide-integer similarity (tcgen05)");
+          }
+          if (!ok) break;
+          Epilogue er = e;
+          if (er.labels) er.labels += r0;
+          if (er.best) er.best += r0;
+          if (er.second) er.second += r0;
+          if (er.S) er.S = static_cast<char*>(er.S) + (size_t)r0 * (size_t)lds * (s_i32 == 2 ? 8 : 4);
+          ce = launch_wide_combine(Sp, pieces, rows, K, cos, colscale, er, st, &h->launches);
+          if (ce != cudaSuccess) return cuda_fail(h, ce, "wide-integer combine");
+        }
+        if (ok) return HDC_OK;
+      }
+      ++h->stats[HDC_STAT_SIMT_FALLBACKS];
+      h->err = "wide-integer similarity: tensor-core kernel refused the operands, dp4a kernel used";
+    }
+    // CUDA-core route: byte planes + dp4a contraction (widedot.cu)
+    uint32_t* planes = pm.take<uint32_t>(wide_operand_bytes(K, k->hv_bits, D_eff) / sizeof(uint32_t));
+    if (!persistent_fits(h, b, ws_bytes)) return too_small();
+    if (prep) {
+      ce = launch_wide_prepare(C_acc, K, ldc, D_eff, k->hv_bits, pf, cos, planes, colscale, st, &h->launches);
+      if (ce != cudaSuccess) return cuda_fail(h, ce, "wide-integer class operand");
+    }
+    if (prep_only(h)) return HDC_OK;
     {
       Timed tm(h, HDC_K_SIM, st);
       ce = launch_wide_dot(Hbits, N, ldh, K, D_eff, k->hv_bits, cos, planes, colscale, e, st, &h->launches);
@@ -603,6 +676,7 @@ void similarity_model_ws(int K, const hdc_knobs_t* k, Bump& pm) {
   pm.take<uint32_t>((size_t)K * W);
   pm.take<uint32_t>((size_t)W);  // perforation mask
   pm.take<uint8_t>(wide_operand_bytes(K, k->hv_bits, k->D_eff));  // byte planes of 32- / 64-bit integer codes
+  wide_tc_ws(0, K, k, &pm, nullptr);                              // ... and their 16-bit pieces (tensor-core route)
   pm.take<uint8_t>(sim_tc_operand_bytes(K, k->hv_bits == 32 || k->hv_bits == 16 || k->hv_bits == HDC_HV_F16 ||
                                                k->hv_bits == HDC_HV_I16 || k->hv_bits == 8 ? k->hv_bits : 1,
                                         k->D_eff));
@@ -624,6 +698,7 @@ size_t similarity_ws(int64_t N, int K, const hdc_knobs_t* k) {
   b.take<uint32_t>((size_t)W);  // perforation mask
   b.take<uint32_t>((size_t)((k->D_eff + 127) / 128) * 4 * K);  // [chunk][class] sign bits of hdc_similarity_adc
   b.take<uint8_t>(wide_operand_bytes(K, k->hv_bits, k->D_eff));  // byte planes of 32- / 64-bit integer codes
+  wide_tc_ws(N, K, k, &b, &b);                                   // their 16-bit pieces and per-pass piece scores
   b.take<uint8_t>(sim_tc_operand_bytes(K, k->hv_bits == 32 || k->hv_bits == 16 || k->hv_bits == HDC_HV_F16 ||
                                                k->hv_bits == HDC_HV_I16 || k->hv_bits == 8 ? k->hv_bits : 1,
                                        k->D_eff));

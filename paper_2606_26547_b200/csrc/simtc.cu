@@ -647,13 +647,14 @@ template <bool INT8>
 __global__ void __launch_bounds__(CP_THREADS)
 class_prepare_kernel(const float* __restrict__ C, int K, int D_eff, int64_t ldc, int mode, int kc, int nparts,
                      int num_kb, const float* __restrict__ amax, Perf pf, int n_vis, void* __restrict__ dst,
-                     int32_t* __restrict__ rowsum, double* __restrict__ colscale, float* __restrict__ colscale_f) {
+                     int32_t* __restrict__ rowsum, double* __restrict__ colscale, float* __restrict__ colscale_f,
+                     int piece, int width) {
   constexpr int BK = INT8 ? 128 : 64;
   const int ld = num_kb * BK;
   const int k = blockIdx.x;                                   // class (rows k >= K are zero padding)
   const int64_t r0 = (int64_t)(k / kc) * (nparts * kc) + k % kc;   // staged row of part 0; part p: + p * kc
   float s = 1.0f;
-  if (mode == 8 || mode == HDC_HV_I16) {
+  if (mode == 8 || (mode == HDC_HV_I16 && piece == 0)) {
     const float a = *amax;
     s = a > 0.0f ? __fdiv_rn(mode == 8 ? 127.0f : 32767.0f, a) : 1.0f;
   }
@@ -669,7 +670,27 @@ class_prepare_kernel(const float* __restrict__ C, int K, int D_eff, int64_t ldc,
     if (INT8) {
       int8_t* o = reinterpret_cast<int8_t*>(dst) + r0 * ld + col;
       if (mode == HDC_HV_I16) {
-        const int q = live ? (int)fminf(fmaxf(rintf(__fmul_rn(x, s)), -32767.0f), 32767.0f) : 0;
+        int q;
+        if (piece > 0) {
+          // 32- / 64-bit integer codes (HDC_HV_I32 / _I64, reading A22): w = rint(x) saturated to `width` bits,
+          // written as balanced base-65536 pieces w = sum_j p_j 65536^j (p_j in [-32768, 32767], the top one in
+          // [-32768, 32768]); this call stages piece `piece - 1` like an int16 code
+          long long w = live ? __float2ll_rn(x) : 0ll;
+          const long long lim = width == 32 ? 2147483647ll : 9223372036854775807ll;
+          w = w > lim ? lim : (w < -lim ? -lim : w);
+          q = 0;
+          for (int j = 1; j <= piece; ++j) {
+            if (j * 16 == width) {
+              q = (int)w;
+            } else {
+              const int low = (int)(w & 0xFFFFll);
+              q = low >= 32768 ? low - 65536 : low;
+              w = (w >> 16) + (low >= 32768 ? 1 : 0);
+            }
+          }
+        } else {
+          q = live ? (int)fminf(fmaxf(rintf(__fmul_rn(x, s)), -32767.0f), 32767.0f) : 0;
+        }
         const int d0 = ((q + 64) & 127) - 64;
         const int r1 = (q - d0) >> 7;                  // exact: q - d0 is a multiple of 128
         const int d1 = ((r1 + 64) & 127) - 64;
@@ -1210,7 +1231,7 @@ size_t sim_tc_partial_bytes(int64_t N, int K, int hv_bits, int D_eff, int sm_cou
 cudaError_t launch_sim_tc(TcContext* tc, const uint32_t* Hbits, int64_t N, int64_t ldh, const float* C_acc,
                           int K, int64_t ldc, int D_eff, int hv_bits, void* cop, float* amax_scratch,
                           const Epilogue& e, Perf pf, double* partial, bool cop_ready, bool prep_only, int sm_count,
-                          int force_cg, cudaStream_t st, int64_t* nlaunch) {
+                          int force_cg, cudaStream_t st, int64_t* nlaunch, int piece, int width) {
   if (!tc) return cudaErrorNotSupported;
   if (N <= 0 && !prep_only) return cudaSuccess;
   if ((reinterpret_cast<uintptr_t>(cop) & 15) != 0) return cudaErrorNotSupported;
@@ -1221,7 +1242,7 @@ cudaError_t launch_sim_tc(TcContext* tc, const uint32_t* Hbits, int64_t N, int64
   const int BK = int8 ? 128 : 64;
   const int64_t ld = (int64_t)num_kb * BK;
   cudaError_t ce;
-  if ((hv_bits == 8 || hv_bits == HDC_HV_I16) && !cop_ready) {
+  if ((hv_bits == 8 || (hv_bits == HDC_HV_I16 && piece == 0)) && !cop_ready) {
     ce = launch_tensor_amax(C_acc, K, D_eff, ldc, pf, amax_scratch, st, nlaunch);
     if (ce != cudaSuccess) return ce;
   }
@@ -1233,11 +1254,11 @@ cudaError_t launch_sim_tc(TcContext* tc, const uint32_t* Hbits, int64_t N, int64
     float* csf = const_cast<float*>(e.colscale_f);
     if (int8)
       class_prepare_kernel<true><<<(unsigned)(n_tiles * kc), CP_THREADS, 0, st>>>(C_acc, K, D_eff, ldc, hv_bits, kc, nparts, num_kb,
-                                                                          amax_scratch, pf, n_vis, cop, rowsum, cs, csf);
+                                                                          amax_scratch, pf, n_vis, cop, rowsum, cs, csf, piece, width);
     else
       class_prepare_kernel<false><<<(unsigned)(n_tiles * kc), CP_THREADS, 0, st>>>(C_acc, K, D_eff, ldc, hv_bits, kc, nparts,
                                                                            num_kb, amax_scratch, pf, n_vis, cop, nullptr, cs,
-                                                                           csf);
+                                                                           csf, 0, 0);
     ++*nlaunch;
     ce = cudaGetLastError();
     if (ce != cudaSuccess) return ce;

@@ -61,6 +61,7 @@ __global__ void wide_prepare_kernel(const float* __restrict__ C, int D_eff, int6
       const double v = (double)q;
       ss += v * v;
     }
+    if (!planes) continue;   // tensor-core route: only the cosine scales are wanted
     uint32_t* dst = planes + ((int64_t)k * quads_ld + qd) * P;
     for (int p = 0; p < P; ++p) {
       const int sh = 8 * p;
@@ -80,6 +81,58 @@ __global__ void wide_prepare_kernel(const float* __restrict__ C, int D_eff, int6
   }
 }
 
+// Epilogue shared by the dp4a kernel and the tensor-core route's combine kernel: exact integer arg-max for DOT
+// (ties keep the lower index: classes arrive in ascending order), the cosine compared in double; or scores.
+struct WideOut {
+  const double* colscale;
+  int cos;
+  int32_t* labels;
+  float* best;
+  float* second;
+  void* S;
+  int64_t lds;
+  int s_mode;   // 0 fp32, 2 int64
+};
+struct WideTop2 {
+  long long bi1 = LLONG_MIN, bi2 = LLONG_MIN;
+  double bd1 = -1.0e300, bd2 = -1.0e300;
+  int lab = 0;
+};
+__device__ __forceinline__ void wide_push(const WideOut& o, WideTop2& t, int64_t n, int cls, long long s) {
+  if (o.labels) {
+    if (o.cos) {
+      const double v = (double)s * o.colscale[cls];
+      if (v > t.bd1) {
+        t.bd2 = t.bd1;
+        t.bd1 = v;
+        t.lab = cls;
+      } else if (v > t.bd2) {
+        t.bd2 = v;
+      }
+    } else {
+      if (s > t.bi1) {
+        t.bi2 = t.bi1;
+        t.bi1 = s;
+        t.lab = cls;
+      } else if (s > t.bi2) {
+        t.bi2 = s;
+      }
+    }
+  } else if (o.s_mode == 2) {
+    reinterpret_cast<long long*>(o.S)[n * o.lds + cls] = s;
+  } else {
+    reinterpret_cast<float*>(o.S)[n * o.lds + cls] = o.cos ? (float)((double)s * o.colscale[cls]) : (float)s;
+  }
+}
+__device__ __forceinline__ void wide_finish(const WideOut& o, const WideTop2& t, int64_t n, int K) {
+  if (!o.labels) return;
+  o.labels[n] = t.lab;
+  const float b1 = o.cos ? (float)t.bd1 : (float)t.bi1;
+  const float b2 = K > 1 ? (o.cos ? (float)t.bd2 : (float)t.bi2) : b1;
+  if (o.best) o.best[n] = b1;
+  if (o.second) o.second[n] = b2;
+}
+
 // ---------------------------------------------------------------------------------- contraction
 struct WideParams {
   const uint32_t* H;
@@ -88,15 +141,7 @@ struct WideParams {
   const uint32_t* planes;
   int quads_ld;
   int K;
-  const double* colscale;     // [K]; all ones for DOT
-  int cos;
-  // arg-max outputs (labels != NULL) or scores
-  int32_t* labels;
-  float* best;
-  float* second;
-  void* S;
-  int64_t lds;
-  int s_mode;                 // 0 fp32, 2 int64
+  WideOut o;                  // arg-max outputs (labels != NULL) or scores
 };
 
 template <int P>
@@ -116,10 +161,7 @@ __global__ void __launch_bounds__(WQ) wide_dot_kernel(const WideParams p) {
   const int64_t n0 = (int64_t)blockIdx.x * WQ;
   const int64_t n = n0 + t;
 
-  // running arg-max state of this thread's query: exact integers for DOT, doubles for COS
-  long long bi1 = LLONG_MIN, bi2 = LLONG_MIN;
-  double bd1 = -1.0e300, bd2 = -1.0e300;
-  int lab = 0;
+  WideTop2 top;   // running arg-max state of this thread's query
 
   for (int kg = 0; kg < p.K; kg += KC) {
     int acc[KC][P];
@@ -159,11 +201,11 @@ __global__ void __launch_bounds__(WQ) wide_dot_kernel(const WideParams p) {
 #pragma unroll
             for (int v = 0; v < V; ++v) {
               const uint4 c = sc[k][w * 8 + nib][v];
-              const bool top = v == V - 1;
+              const bool last = v == V - 1;
               acc[k][4 * v + 0] = dp4a_su(a, c.x, acc[k][4 * v + 0]);
               acc[k][4 * v + 1] = dp4a_su(a, c.y, acc[k][4 * v + 1]);
               acc[k][4 * v + 2] = dp4a_su(a, c.z, acc[k][4 * v + 2]);
-              acc[k][4 * v + 3] = top ? dp4a_ss(a, c.w, acc[k][4 * v + 3]) : dp4a_su(a, c.w, acc[k][4 * v + 3]);
+              acc[k][4 * v + 3] = last ? dp4a_ss(a, c.w, acc[k][4 * v + 3]) : dp4a_su(a, c.w, acc[k][4 * v + 3]);
             }
           }
         }
@@ -173,49 +215,25 @@ __global__ void __launch_bounds__(WQ) wide_dot_kernel(const WideParams p) {
 #pragma unroll
     for (int k = 0; k < KC; ++k) {
       const int cls = kg + k;
-      if (cls >= p.K) break;
-      const long long s = recombine<P>(acc[k]);
-      if (p.labels) {
-        if (p.cos) {
-          const double v = (double)s * p.colscale[cls];
-          if (v > bd1) {
-            bd2 = bd1;
-            bd1 = v;
-            lab = cls;
-          } else if (v > bd2) {
-            bd2 = v;
-          }
-        } else {
-          if (s > bi1) {      // ties keep the lower index: classes arrive in ascending order
-            bi2 = bi1;
-            bi1 = s;
-            lab = cls;
-          } else if (s > bi2) {
-            bi2 = s;
-          }
-        }
-      } else if (n < p.N) {
-        if (p.s_mode == 2)
-          reinterpret_cast<long long*>(p.S)[n * p.lds + cls] = s;
-        else
-          reinterpret_cast<float*>(p.S)[n * p.lds + cls] = p.cos ? (float)((double)s * p.colscale[cls]) : (float)s;
-      }
+      if (cls < p.K && n < p.N) wide_push(p.o, top, n, cls, recombine<P>(acc[k]));
     }
   }
+  if (n < p.N) wide_finish(p.o, top, n, p.K);
+}
 
-  if (p.labels && n < p.N) {
-    p.labels[n] = lab;
-    float b1, b2;
-    if (p.cos) {
-      b1 = (float)bd1;
-      b2 = p.K > 1 ? (float)bd2 : b1;
-    } else {
-      b1 = (float)bi1;
-      b2 = p.K > 1 ? (float)bi2 : b1;
-    }
-    if (p.best) p.best[n] = b1;
-    if (p.second) p.second[n] = b2;
+// Tensor-core route: recombines the int32 scores of the 16-bit pieces, S_j [rows][K] at Sp + j * rows * K.
+// One thread per query row.
+__global__ void wide_combine_kernel(const int32_t* __restrict__ Sp, int pieces, int64_t rows, int K, WideOut o) {
+  const int64_t n = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (n >= rows) return;
+  WideTop2 top;
+  for (int k = 0; k < K; ++k) {
+    unsigned long long s = 0;
+    for (int j = 0; j < pieces; ++j)
+      s += (unsigned long long)(long long)__ldg(Sp + ((int64_t)j * rows + n) * K + k) << (16 * j);
+    wide_push(o, top, n, k, (long long)s);
   }
+  wide_finish(o, top, n, K);
 }
 
 }  // namespace
@@ -226,6 +244,30 @@ static inline int wide_quads_ld(int D_eff) { return (int)round_up((D_eff + 3) / 
 size_t wide_operand_bytes(int K, int hv_bits, int D_eff) {
   const int P = wide_planes(hv_bits);
   return P ? (size_t)K * (size_t)wide_quads_ld(D_eff) * P * sizeof(uint32_t) : 0;
+}
+
+static WideOut wide_out(const Epilogue& e, int cos, const double* colscale) {
+  WideOut o{};
+  o.colscale = colscale;
+  o.cos = cos;
+  if (e.kind == EPI_ARGMAX) {
+    o.labels = e.labels;
+    o.best = e.best;
+    o.second = e.second;
+  } else {
+    o.S = e.S;
+    o.lds = e.lds;
+    o.s_mode = e.s_i32;
+  }
+  return o;
+}
+
+cudaError_t launch_wide_combine(const int32_t* Sp, int pieces, int64_t rows, int K, int cos, const double* colscale,
+                                const Epilogue& e, cudaStream_t st, int64_t* nlaunch) {
+  if (rows <= 0) return cudaSuccess;
+  wide_combine_kernel<<<(unsigned)((rows + 127) / 128), 128, 0, st>>>(Sp, pieces, rows, K, wide_out(e, cos, colscale));
+  *nlaunch += 1;
+  return cudaGetLastError();
 }
 
 cudaError_t launch_wide_prepare(const float* C_acc, int K, int64_t ldc, int D_eff, int hv_bits, Perf pf, int cos,
@@ -252,17 +294,7 @@ cudaError_t launch_wide_dot(const uint32_t* Hbits, int64_t N, int64_t ldh, int K
   p.planes = planes;
   p.quads_ld = wide_quads_ld(D_eff);
   p.K = K;
-  p.colscale = colscale;
-  p.cos = cos;
-  if (e.kind == EPI_ARGMAX) {
-    p.labels = e.labels;
-    p.best = e.best;
-    p.second = e.second;
-  } else {
-    p.S = e.S;
-    p.lds = e.lds;
-    p.s_mode = e.s_i32;
-  }
+  p.o = wide_out(e, cos, colscale);
   const int64_t blocks = (N + WQ - 1) / WQ;
   if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
   if (P == 4)

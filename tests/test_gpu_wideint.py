@@ -1,7 +1,8 @@
 """32- and 64-bit integer class operands ("integer data types (8, 16, 32, or 64-bit)"; hv codes
 HDC_HV_I32 / HDC_HV_I64, reading A22: q = rint(C_acc), no scale, symmetric saturation) through the C ABI:
-widedot.cu stages the byte planes of the codes and contracts them against the packed queries with dp4a; the 64-bit
-integer sums must equal the oracle's python / int64 integers bit for bit at every shape (ragged query tiles, class
+the tensor-core route contracts the balanced 16-bit pieces of the codes on tcgen05 kind::i8 (sim_tc_kernel) and recombines
+the pieces' int32 scores in 64 bits; widedot.cu's dp4a kernel over the byte planes of the codes is the CUDA-core route
+(HDC_FLAG_SIMT).  On both the 64-bit integer sums must equal the oracle's python / int64 integers bit for bit at every shape (ragged query tiles, class
 counts around the register tile, D_eff not a multiple of 4 / 32 / 512), saturating 32-bit codes, sums beyond 2^53,
 perforation, ties, a zero class, padded query rows with dirty bits beyond D_eff."""
 from __future__ import annotations
@@ -42,7 +43,11 @@ def test_codes_match_header(hd):
                                               (129, 8, 513, 513, (0, 1)), (128, 4, 512, 512, (0, 1)),
                                               (200, 13, 1300, 1000, (3, 4)), (64, 5, 700, 640, (1, 7))])
 @pytest.mark.parametrize("pad", [False, True])
-def test_wide_integer_similarity_and_classify(hd, h, width, N, K, D, D_eff, perf, pad):
+@pytest.mark.parametrize("flags_name", ["", "HDC_FLAG_SIMT", "HDC_FLAG_TC_2CTA"])
+def test_wide_integer_similarity_and_classify(hd, h, width, N, K, D, D_eff, perf, pad, flags_name):
+    """flags: default = the tensor-core route (16-bit pieces of the codes on sim_tc_kernel, recombined in 64 bits),
+    HDC_FLAG_SIMT = the dp4a kernel over byte planes, HDC_FLAG_TC_2CTA = the pieces on CTA pairs."""
+    flags = getattr(hd, flags_name) if flags_name else 0
     code, ocode, mag = HV[width]
     r = np.random.default_rng([71, code, N, K, D_eff])
     hb = r.integers(0, 2, size=(N, D), dtype=np.uint8)       # bits beyond D_eff are random: they must not count
@@ -57,7 +62,7 @@ def test_wide_integer_similarity_and_classify(hd, h, width, N, K, D, D_eff, perf
     if width == "I64" and D_eff >= 1000 and perf[1] == 1:
         assert np.abs(S_or).max() > 2 ** 53                  # a float64 contraction would round here
     Hd, Cd = dev_bits(hb, (D + 127) // 128 * 4 if pad else None), dev(C)
-    kn = hd.knobs(D_eff, hv_bits=code, sim=hd.HDC_SIM_DOT, perf_begin=perf[0], perf_stride=perf[1])
+    kn = hd.knobs(D_eff, hv_bits=code, sim=hd.HDC_SIM_DOT, flags=flags, perf_begin=perf[0], perf_stride=perf[1])
     Si = h.hdc_similarity(Hd, Cd, kn, s_dtype=torch.int64).cpu().numpy()
     assert np.array_equal(Si, S_or)
     Sf = h.hdc_similarity(Hd, Cd, kn).cpu().numpy()
@@ -69,7 +74,7 @@ def test_wide_integer_similarity_and_classify(hd, h, width, N, K, D, D_eff, perf
     assert np.array_equal(best.cpu().numpy(), best_or.astype(np.float32))
     assert np.array_equal(sec.cpu().numpy(), sec_or.astype(np.float32))
     # cosine over the integer codes
-    knc = hd.knobs(D_eff, hv_bits=code, sim=hd.HDC_SIM_COS, perf_begin=perf[0], perf_stride=perf[1])
+    knc = hd.knobs(D_eff, hv_bits=code, sim=hd.HDC_SIM_COS, flags=flags, perf_begin=perf[0], perf_stride=perf[1])
     Sc_or = O.similarity(hb, C, D_eff, O.SIM_COS, ocode, perf[0], perf[1])
     Sc = h.hdc_similarity(Hd, Cd, knc).cpu().numpy()
     assert np.allclose(Sc, Sc_or, rtol=1e-6, atol=1e-12)
@@ -82,7 +87,8 @@ def test_wide_integer_similarity_and_classify(hd, h, width, N, K, D, D_eff, perf
 
 
 @pytest.mark.parametrize("width", ["I32", "I64"])
-def test_wide_integer_operand_is_the_trained_accumulator(hd, h, width):
+@pytest.mark.parametrize("flags_name", ["", "HDC_FLAG_SIMT"])
+def test_wide_integer_operand_is_the_trained_accumulator(hd, h, width, flags_name):
     """Integer accumulators as bundling leaves them (L53 / L181): the 32- / 64-bit operand IS the accumulator -- DOT scores
     equal those of hv_bits = 32 computed by the oracle in float64, winners decided by 2 units at sums ~ 1e9 (far beyond
     what an fp32 accumulate holds); K = 1000 covers 125 / 250 class passes per CTA."""
@@ -99,11 +105,35 @@ def test_wide_integer_operand_is_the_trained_accumulator(hd, h, width):
     assert np.array_equal(S_or.astype(np.float64), O.similarity(hb, C, D, O.SIM_DOT, 32))
     assert np.abs(S_or).max() > 2 ** 29
     Hd, Cd = dev_bits(hb), dev(C)
-    kn = hd.knobs(D, hv_bits=code, sim=hd.HDC_SIM_DOT)
+    kn = hd.knobs(D, hv_bits=code, sim=hd.HDC_SIM_DOT, flags=getattr(hd, flags_name) if flags_name else 0)
     assert np.array_equal(h.hdc_similarity(Hd, Cd, kn, s_dtype=torch.int64).cpu().numpy(), S_or)
     lab_or = O.classify(S_or, O.SIM_DOT)[0]
     assert set(lab_or[:8].tolist()) == {1, 2}
     assert np.array_equal(h.hdc_classify(Hd, Cd, kn).cpu().numpy(), lab_or)
+
+
+@pytest.mark.parametrize("width", ["I32", "I64"])
+def test_wide_integer_row_passes_of_the_tensor_core_route(hd, h, width):
+    """More queries than one pass of the tensor-core route holds (18944 rows at this K): two passes, the second one
+    ragged; scores, labels and best / runner-up land in the right rows."""
+    code, ocode, mag = HV[width]
+    N, K, D = 19100, 450, 96
+    r = np.random.default_rng([73, code])
+    hb = r.integers(0, 2, size=(N, D), dtype=np.uint8)
+    C = (r.standard_normal((K, D)) * mag).astype(np.float32)
+    S_or = O.similarity(hb, C, D, O.SIM_DOT, ocode)
+    Hd, Cd = dev_bits(hb), dev(C)
+    kn = hd.knobs(D, hv_bits=code, sim=hd.HDC_SIM_DOT)
+    assert np.array_equal(h.hdc_similarity(Hd, Cd, kn, s_dtype=torch.int64).cpu().numpy(), S_or)
+    lab_or, best_or, sec_or = O.classify(S_or, O.SIM_DOT)
+    lab, best, sec = h.hdc_classify(Hd, Cd, kn, want_scores=True)
+    assert np.array_equal(lab.cpu().numpy(), lab_or)
+    assert np.array_equal(best.cpu().numpy(), best_or.astype(np.float32))
+    assert np.array_equal(sec.cpu().numpy(), sec_or.astype(np.float32))
+    knc = hd.knobs(D, hv_bits=code, sim=hd.HDC_SIM_COS)
+    Sc_or = O.similarity(hb, C, D, O.SIM_COS, ocode)
+    assert np.allclose(h.hdc_similarity(Hd, Cd, knc).cpu().numpy(), Sc_or, rtol=1e-6, atol=1e-12)
+    assert np.array_equal(h.hdc_classify(Hd, Cd, knc).cpu().numpy(), O.classify(Sc_or, O.SIM_COS)[0])
 
 
 def test_wide_integer_argument_errors(hd, h):
