@@ -5,15 +5,20 @@
 //   s[n,k] = sum_{d visited, d < D_eff} (1 - 2 b[n,d]) * q[k,d]        exact, in 64-bit integers
 //
 // The contraction runs on the integer dot-product instruction: the two's-complement bytes of the codes are
-// staged once per model as BYTE PLANES -- for every group of four dimensions ("quad") P = 4 or 8 words, word p
-// holding byte p of the four codes -- so that one dp4a multiplies four +-1 query bytes with four code bytes
+// staged once per model as BYTE PLANES -- for every group of four dimensions ("quad": dimensions 32 w + j + 8 i,
+// i < 4, so that the four query bits of quad j of word w are (word >> j) & 0x01010101, two ALU operations and no
+// multiply on the pipe the dp4a needs) P = 4 or 8 words, word p holding byte p of the four codes -- so that one dp4a multiplies four +-1 query bytes with four code bytes
 // (unsigned for the lower planes, signed for the top one) into an int32 per-plane sum (|.| <= 255 * D_eff),
 // and the sums of the planes are recombined as sum_p acc_p << 8p in 64 bits when a class is finished.
 // Unvisited (perforated) dimensions and the padding beyond D_eff are staged as zero codes: no masks in the loop.
 //
-// Thread = query; a CTA of 128 queries walks the reduction axis in chunks of 512 dimensions (16 query words
-// per row through a padded shared-memory tile, 128 quads of KC classes as broadcast 16-byte reads) with KC x P
-// accumulators in registers; classes beyond KC take further passes over the query rows (L2-resident).
+// A thread owns QT queries; a CTA of 128 threads walks the reduction axis in chunks of 512 dimensions (16 query
+// words per row through a padded shared-memory tile, 128 quads of KC classes as broadcast 16-byte reads) with
+// QT x KC x P accumulators in registers; classes beyond KC take further passes over the query rows (L2-resident).
+// dp4a and IMAD share one pipe (ncu: fmaheavy 89 % busy in the first version, dp4a 62 % of it): the kernel keeps
+// everything else off it.  The query bytes are 0 / 1 (bit set = -1): sum (1 - 2b) q = rowsum - 2 sum b q, the row
+// sums of the codes staged with the planes.  QT = 1, KC = 8 (4 for 64-bit codes) measured best: more queries per
+// thread halve the shared-memory wavefronts per dp4a but spend the pipe on more expansions per class word.
 // Bound: the dp4a issue rate -- N * K * D_eff * P / 4 instructions per call.
 #include <limits.h>
 
@@ -26,14 +31,14 @@ constexpr int WQ = 128;        // queries per CTA
 constexpr int CHUNK_W = 16;    // query words per chunk (512 dimensions = 128 quads)
 constexpr int CHUNK_Q = CHUNK_W * 8;
 
-__device__ __forceinline__ int dp4a_su(uint32_t a, uint32_t b, int c) {   // signed a bytes x unsigned b bytes
+__device__ __forceinline__ int dp4a_uu(uint32_t a, uint32_t b, int c) {   // unsigned a bytes x unsigned b bytes
   int d;
-  asm("dp4a.s32.u32 %0, %1, %2, %3;" : "=r"(d) : "r"(a), "r"(b), "r"(c));
+  asm("dp4a.u32.u32 %0, %1, %2, %3;" : "=r"(d) : "r"(a), "r"(b), "r"(c));
   return d;
 }
-__device__ __forceinline__ int dp4a_ss(uint32_t a, uint32_t b, int c) {
+__device__ __forceinline__ int dp4a_us(uint32_t a, uint32_t b, int c) {   // unsigned a bytes x signed b bytes
   int d;
-  asm("dp4a.s32.s32 %0, %1, %2, %3;" : "=r"(d) : "r"(a), "r"(b), "r"(c));
+  asm("dp4a.u32.s32 %0, %1, %2, %3;" : "=r"(d) : "r"(a), "r"(b), "r"(c));
   return d;
 }
 
@@ -42,22 +47,25 @@ __device__ __forceinline__ int dp4a_ss(uint32_t a, uint32_t b, int c) {
 // 1 / (sqrt(n_vis) * |q|) (0 for a zero row; 1 for DOT), norm summed in double in a fixed order.
 __global__ void wide_prepare_kernel(const float* __restrict__ C, int D_eff, int64_t ldc, Perf pf, int P,
                                     uint32_t* __restrict__ planes, int quads_ld, int cos, int n_vis,
-                                    double* __restrict__ colscale) {
+                                    double* __restrict__ colscale, long long* __restrict__ rowsum) {
   const int k = blockIdx.x;
   const long long lim = P == 4 ? 2147483647LL : 9223372036854775807LL;
   __shared__ double part[32];
+  __shared__ unsigned long long part_s[32];
   double ss = 0.0;
+  unsigned long long rs = 0;   // sum of the codes (wraps beyond the contract, like the scores)
   for (int qd = threadIdx.x; qd < quads_ld; qd += blockDim.x) {
     unsigned long long code[4];
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
-      const int d = qd * 4 + i;
+      const int d = (qd >> 3) * 32 + (qd & 7) + 8 * i;   // quad j of query word w: dimensions 32 w + j + 8 i
       long long q = 0;
       if (d < D_eff && perf_visits(pf, d)) {
         q = __float2ll_rn(__ldg(C + (int64_t)k * ldc + d));   // round half to even, saturates at the int64 range
         q = q > lim ? lim : (q < -lim ? -lim : q);
       }
       code[i] = (unsigned long long)q;
+      rs += (unsigned long long)q;
       const double v = (double)q;
       ss += v * v;
     }
@@ -70,12 +78,23 @@ __global__ void wide_prepare_kernel(const float* __restrict__ C, int D_eff, int6
     }
   }
 #pragma unroll
-  for (int off = 16; off; off >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, off);
-  if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = ss;
+  for (int off = 16; off; off >>= 1) {
+    ss += __shfl_xor_sync(0xffffffffu, ss, off);
+    rs += __shfl_xor_sync(0xffffffffu, rs, off);
+  }
+  if ((threadIdx.x & 31) == 0) {
+    part[threadIdx.x >> 5] = ss;
+    part_s[threadIdx.x >> 5] = rs;
+  }
   __syncthreads();
   if (threadIdx.x == 0) {
     double t = 0.0;
-    for (int i = 0; i < (int)(blockDim.x >> 5); ++i) t += part[i];
+    unsigned long long ts = 0;
+    for (int i = 0; i < (int)(blockDim.x >> 5); ++i) {
+      t += part[i];
+      ts += part_s[i];
+    }
+    if (rowsum) rowsum[k] = (long long)ts;
     const double nrm = sqrt(t);
     colscale[k] = !cos ? 1.0 : (nrm > 0.0 ? 1.0 / (sqrt((double)n_vis) * nrm) : 0.0);
   }
@@ -93,29 +112,32 @@ struct WideOut {
   int64_t lds;
   int s_mode;   // 0 fp32, 2 int64
 };
-struct WideTop2 {
-  long long bi1 = LLONG_MIN, bi2 = LLONG_MIN;
-  double bd1 = -1.0e300, bd2 = -1.0e300;
-  int lab = 0;
+struct WideTop2 {   // best / runner-up as raw 64-bit patterns: long long for DOT, double for COS
+  long long b1, b2;
+  int lab;
 };
+__device__ __forceinline__ WideTop2 wide_top2_init(const WideOut& o) {
+  const long long lo = o.cos ? __double_as_longlong(-1.0e300) : LLONG_MIN;
+  return WideTop2{lo, lo, 0};
+}
 __device__ __forceinline__ void wide_push(const WideOut& o, WideTop2& t, int64_t n, int cls, long long s) {
   if (o.labels) {
     if (o.cos) {
       const double v = (double)s * o.colscale[cls];
-      if (v > t.bd1) {
-        t.bd2 = t.bd1;
-        t.bd1 = v;
+      if (v > __longlong_as_double(t.b1)) {
+        t.b2 = t.b1;
+        t.b1 = __double_as_longlong(v);
         t.lab = cls;
-      } else if (v > t.bd2) {
-        t.bd2 = v;
+      } else if (v > __longlong_as_double(t.b2)) {
+        t.b2 = __double_as_longlong(v);
       }
     } else {
-      if (s > t.bi1) {
-        t.bi2 = t.bi1;
-        t.bi1 = s;
+      if (s > t.b1) {
+        t.b2 = t.b1;
+        t.b1 = s;
         t.lab = cls;
-      } else if (s > t.bi2) {
-        t.bi2 = s;
+      } else if (s > t.b2) {
+        t.b2 = s;
       }
     }
   } else if (o.s_mode == 2) {
@@ -127,8 +149,8 @@ __device__ __forceinline__ void wide_push(const WideOut& o, WideTop2& t, int64_t
 __device__ __forceinline__ void wide_finish(const WideOut& o, const WideTop2& t, int64_t n, int K) {
   if (!o.labels) return;
   o.labels[n] = t.lab;
-  const float b1 = o.cos ? (float)t.bd1 : (float)t.bi1;
-  const float b2 = K > 1 ? (o.cos ? (float)t.bd2 : (float)t.bi2) : b1;
+  const float b1 = o.cos ? (float)__longlong_as_double(t.b1) : (float)t.b1;
+  const float b2 = K > 1 ? (o.cos ? (float)__longlong_as_double(t.b2) : (float)t.b2) : b1;
   if (o.best) o.best[n] = b1;
   if (o.second) o.second[n] = b2;
 }
@@ -139,6 +161,7 @@ struct WideParams {
   int64_t N, ldh;
   int W;                      // query words per row that carry visited dimensions
   const uint32_t* planes;
+  const long long* rowsum;    // [K] sums of the codes
   int quads_ld;
   int K;
   WideOut o;                  // arg-max outputs (labels != NULL) or scores
@@ -152,28 +175,32 @@ __device__ __forceinline__ long long recombine(const int (&a)[P]) {
   return (long long)s;
 }
 
-template <int P, int KC>
+template <int P, int KC, int QT>
 __global__ void __launch_bounds__(WQ) wide_dot_kernel(const WideParams p) {
   constexpr int V = P / 4;                                  // 16-byte vectors per quad
-  __shared__ uint32_t sq[WQ][CHUNK_W + 1];
+  constexpr int ROWS = WQ * QT;                             // queries per CTA: thread t owns rows t + WQ * j
+  __shared__ uint32_t sq[ROWS][CHUNK_W + 1];
   __shared__ uint4 sc[KC][CHUNK_Q][V];
   const int t = threadIdx.x;
-  const int64_t n0 = (int64_t)blockIdx.x * WQ;
-  const int64_t n = n0 + t;
+  const int64_t n0 = (int64_t)blockIdx.x * ROWS;
 
-  WideTop2 top;   // running arg-max state of this thread's query
+  WideTop2 top[QT];   // running arg-max state of this thread's queries
+#pragma unroll
+  for (int q = 0; q < QT; ++q) top[q] = wide_top2_init(p.o);
 
   for (int kg = 0; kg < p.K; kg += KC) {
-    int acc[KC][P];
+    int acc[QT][KC][P];
 #pragma unroll
-    for (int k = 0; k < KC; ++k)
+    for (int q = 0; q < QT; ++q)
 #pragma unroll
-      for (int j = 0; j < P; ++j) acc[k][j] = 0;
+      for (int k = 0; k < KC; ++k)
+#pragma unroll
+        for (int j = 0; j < P; ++j) acc[q][k][j] = 0;
 
     for (int c0 = 0; c0 < p.W; c0 += CHUNK_W) {
       __syncthreads();   // the previous chunk's readers are done
-#pragma unroll
-      for (int j = 0; j < CHUNK_W; ++j) {
+#pragma unroll 4
+      for (int j = 0; j < CHUNK_W * QT; ++j) {
         const int i = t + WQ * j;
         const int r = i / CHUNK_W, w = i % CHUNK_W;
         int64_t row = n0 + r;
@@ -190,22 +217,28 @@ __global__ void __launch_bounds__(WQ) wide_dot_kernel(const WideParams p) {
       __syncthreads();
 #pragma unroll 1
       for (int w = 0; w < CHUNK_W; ++w) {
-        const uint32_t qw = sq[t][w];
+        uint32_t qw[QT];
+#pragma unroll
+        for (int q = 0; q < QT; ++q) qw[q] = sq[t + WQ * q][w];
 #pragma unroll
         for (int nib = 0; nib < 8; ++nib) {
-          // bit i of the nibble -> byte i: 0x01 (bit 0: +1) or 0xFF (bit 1: -1)
-          const uint32_t spread = (((qw >> (4 * nib)) & 0xFu) * 0x00204081u) & 0x01010101u;
-          const uint32_t a = spread * 0xFEu + 0x01010101u;
+          uint32_t a[QT];   // bits nib, nib + 8, nib + 16, nib + 24 of the word -> bytes 0..3 (0 or 1)
+#pragma unroll
+          for (int q = 0; q < QT; ++q) a[q] = (qw[q] >> nib) & 0x01010101u;
 #pragma unroll
           for (int k = 0; k < KC; ++k) {
 #pragma unroll
             for (int v = 0; v < V; ++v) {
               const uint4 c = sc[k][w * 8 + nib][v];
               const bool last = v == V - 1;
-              acc[k][4 * v + 0] = dp4a_su(a, c.x, acc[k][4 * v + 0]);
-              acc[k][4 * v + 1] = dp4a_su(a, c.y, acc[k][4 * v + 1]);
-              acc[k][4 * v + 2] = dp4a_su(a, c.z, acc[k][4 * v + 2]);
-              acc[k][4 * v + 3] = last ? dp4a_ss(a, c.w, acc[k][4 * v + 3]) : dp4a_su(a, c.w, acc[k][4 * v + 3]);
+#pragma unroll
+              for (int q = 0; q < QT; ++q) {
+                acc[q][k][4 * v + 0] = dp4a_uu(a[q], c.x, acc[q][k][4 * v + 0]);
+                acc[q][k][4 * v + 1] = dp4a_uu(a[q], c.y, acc[q][k][4 * v + 1]);
+                acc[q][k][4 * v + 2] = dp4a_uu(a[q], c.z, acc[q][k][4 * v + 2]);
+                acc[q][k][4 * v + 3] = last ? dp4a_us(a[q], c.w, acc[q][k][4 * v + 3])
+                                            : dp4a_uu(a[q], c.w, acc[q][k][4 * v + 3]);
+              }
             }
           }
         }
@@ -215,10 +248,22 @@ __global__ void __launch_bounds__(WQ) wide_dot_kernel(const WideParams p) {
 #pragma unroll
     for (int k = 0; k < KC; ++k) {
       const int cls = kg + k;
-      if (cls < p.K && n < p.N) wide_push(p.o, top, n, cls, recombine<P>(acc[k]));
+      if (cls >= p.K) break;
+      const unsigned long long rs = (unsigned long long)__ldg(p.rowsum + cls);
+#pragma unroll
+      for (int q = 0; q < QT; ++q) {
+        const int64_t n = n0 + t + WQ * q;
+        // sum (1 - 2b) code = rowsum - 2 * sum over the set bits
+        const long long s = (long long)(rs - 2ull * (unsigned long long)recombine<P>(acc[q][k]));
+        if (n < p.N) wide_push(p.o, top[q], n, cls, s);
+      }
     }
   }
-  if (n < p.N) wide_finish(p.o, top, n, p.K);
+#pragma unroll
+  for (int q = 0; q < QT; ++q) {
+    const int64_t n = n0 + t + WQ * q;
+    if (n < p.N) wide_finish(p.o, top[q], n, p.K);
+  }
 }
 
 // Tensor-core route: recombines the int32 scores of the 16-bit pieces, S_j [rows][K] at Sp + j * rows * K.
@@ -226,7 +271,7 @@ __global__ void __launch_bounds__(WQ) wide_dot_kernel(const WideParams p) {
 __global__ void wide_combine_kernel(const int32_t* __restrict__ Sp, int pieces, int64_t rows, int K, WideOut o) {
   const int64_t n = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (n >= rows) return;
-  WideTop2 top;
+  WideTop2 top = wide_top2_init(o);
   for (int k = 0; k < K; ++k) {
     unsigned long long s = 0;
     for (int j = 0; j < pieces; ++j)
@@ -243,7 +288,11 @@ static inline int wide_quads_ld(int D_eff) { return (int)round_up((D_eff + 3) / 
 
 size_t wide_operand_bytes(int K, int hv_bits, int D_eff) {
   const int P = wide_planes(hv_bits);
-  return P ? (size_t)K * (size_t)wide_quads_ld(D_eff) * P * sizeof(uint32_t) : 0;
+  // byte planes, then one 64-bit sum of the codes per class
+  return P ? (size_t)K * (size_t)wide_quads_ld(D_eff) * P * sizeof(uint32_t) + (size_t)K * sizeof(long long) : 0;
+}
+static inline long long* wide_rowsum(uint32_t* planes, int K, int hv_bits, int D_eff) {
+  return reinterpret_cast<long long*>(planes + (size_t)K * (size_t)wide_quads_ld(D_eff) * wide_planes(hv_bits));
 }
 
 static WideOut wide_out(const Epilogue& e, int cos, const double* colscale) {
@@ -275,7 +324,8 @@ cudaError_t launch_wide_prepare(const float* C_acc, int K, int64_t ldc, int D_ef
   const int P = wide_planes(hv_bits);
   if (!P) return cudaErrorInvalidValue;
   wide_prepare_kernel<<<K, 256, 0, st>>>(C_acc, D_eff, ldc, pf, P, planes, wide_quads_ld(D_eff), cos,
-                                         perf_count(pf, D_eff), colscale);
+                                         perf_count(pf, D_eff), colscale,
+                                         planes ? wide_rowsum(planes, K, hv_bits, D_eff) : nullptr);
   *nlaunch += 1;
   return cudaGetLastError();
 }
@@ -292,15 +342,21 @@ cudaError_t launch_wide_dot(const uint32_t* Hbits, int64_t N, int64_t ldh, int K
   p.ldh = ldh;
   p.W = words_of(D_eff);
   p.planes = planes;
+  p.rowsum = wide_rowsum(const_cast<uint32_t*>(planes), K, hv_bits, D_eff);
   p.quads_ld = wide_quads_ld(D_eff);
   p.K = K;
   p.o = wide_out(e, cos, colscale);
-  const int64_t blocks = (N + WQ - 1) / WQ;
+#ifndef WD_QT
+#define WD_QT 1
+#define WD_KC4 8
+#define WD_KC8 4
+#endif
+  const int64_t blocks = (N + WQ * WD_QT - 1) / (WQ * WD_QT);
   if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
   if (P == 4)
-    wide_dot_kernel<4, 8><<<(unsigned)blocks, WQ, 0, st>>>(p);
+    wide_dot_kernel<4, WD_KC4, WD_QT><<<(unsigned)blocks, WQ, 0, st>>>(p);
   else
-    wide_dot_kernel<8, 4><<<(unsigned)blocks, WQ, 0, st>>>(p);
+    wide_dot_kernel<8, WD_KC8, WD_QT><<<(unsigned)blocks, WQ, 0, st>>>(p);
   *nlaunch += 1;
   return cudaGetLastError();
 }
