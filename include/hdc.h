@@ -109,8 +109,9 @@ enum {
  *             | HDC_HV_I32 / HDC_HV_I64 32- / 64-bit integers: the accumulators themselves,
  *             q = rint(c) (half to even), NO scale, saturating at +-(2^31 - 1) / +-(2^63 - 1); scores
  *             are exact integers accumulated in 64 bits (contract: sum_d |q[k,d]| < 2^63, beyond it the
- *             sums wrap), DOT / COS only; contracted on the integer dot-product units (dp4a over the
- *             byte planes of the codes), not on the tensor cores
+ *             sums wrap), DOT / COS only; contracted on the tensor cores as balanced 16-bit pieces of the
+ *             codes (each an int16-style operand, exact int32 scores, recombined in 64 bits), or with
+ *             HDC_FLAG_SIMT by dp4a over the byte planes of the codes
  *             | 1 sign bit [C_acc < 0].  Query hypervectors are always bipolar (packed bits).
  *  sim        HDC_SIM_*; HDC_SIM_HAMMING requires hv_bits == 1.
  *  flags      HDC_FLAG_*.
