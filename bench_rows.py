@@ -624,7 +624,8 @@ ROWS = {
 # the rows bench.py folds into its default JSON line (every run; about a minute on one B200)
 DEFAULT_ROWS = ("c2_encode_bf16", "c2_encode_i8", "c4_point_bf16", "c4_point_i8", "c2_classify_cos32",
                 "c3_levelid", "c3_levelid_dense_input", "microhd_levelid_q814", "c3_hamming_k10", "c3_pipeline",
-                "c5_classify_bf16", "c5_classify_1bit", "c5_stream_bf16", "c5_stream_1bit", "c2_train_epoch")
+                "c5_classify_bf16", "c5_classify_1bit", "c5_stream_bf16", "c5_stream_1bit", "c2_train_epoch",
+                "c2_classify_cos_i32")
 
 
 def run(h, peaks, reps=5, only=None, cool_s=0.5):
