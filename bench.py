@@ -294,9 +294,12 @@ def run_gpu(args):
     h.kernel_timing(True)
     torch.cuda.synchronize()
     with ClockSampler(local) as cs_k:
+        ev[0].record()
         for _ in range(args.steps):
             step()
+        ev[1].record()
         torch.cuda.synchronize()
+    pass2_step_ms = ev[0].elapsed_time(ev[1]) / args.steps   # the step as timed in THIS pass (its own clocks)
     enc_ms_tot, enc_n = h.kernel_time(hd.HDC_K_ENCODE_GEMM)
     sim_ms_tot, sim_n = h.kernel_time(hd.HDC_K_SIM)
     enc_ms = enc_ms_tot / max(1, enc_n)
@@ -349,7 +352,9 @@ def run_gpu(args):
                                 "the library's per-kernel events on, encode_call_ms and `alone` from a third pass of "
                                 "encode calls only; each ran after the timed region, at the clocks the part had then, "
                                 "so they need not add up to ms_per_step",
-                "share_of_step": enc_ms / (ms / args.steps),
+                "share_of_step": enc_ms / pass2_step_ms, "step_ms_in_kernel_pass": pass2_step_ms,
+                "share_of_step_how": "contraction ms per launch / ms per step, both from the second pass (same clocks); "
+                                     "compare with the ncu launch list profiles/r2_launches.md",
                 "fp32_alu_peak_tflops": SM_COUNT * FP32_LANES * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12,
                 "traffic": NCU_TRAFFIC_BYTES, "traffic_source": NCU_TRAFFIC_SOURCE,
                 "algorithmic_bytes_per_launch": float(NQ) * 3 * Fp * 2 + float(D) * 3 * Fp * 2 + float(NQ) * W * 4}
