@@ -12,8 +12,8 @@ Pins (tests/test_oracle_*.py, `-m "not gpu"`): brute-force python loops on tiny 
 bipolar identity dot = D_eff - 2*Hamming, near-orthogonality |cos| <~ 3/sqrt(D), the
 angle/Hamming closed form for Gaussian projections, majority-bundling recovery probability
 1/2 + C(F-1,(F-1)/2)/2^F, D_eff slice-equivalence and Listing 1's "first 1024 of 2048",
-bf16 RNE against ml_dtypes, per-row and per-tensor int8 codes worked by hand (non-unit scales, ties of
-both parities), perceptron invariants (sum_k Delta = 0; B=1 == textbook online perceptron; 1 < B < N with
+bf16 RNE against ml_dtypes, per-row and per-tensor int8 / int16 codes worked by hand (non-unit scales, ties of
+both parities), the 32- / 64-bit integer class codes (A22) by hand and against python-integer sums beyond 2^53, perceptron invariants (sum_k Delta = 0; B=1 == textbook online perceptron; 1 < B < N with
 a ragged last batch == a python-loop restatement that re-derives the operand per mini-batch); the ADC-quantised chunked dot (S12) against hand loops, the transparent-window case
 (= D_eff - 2*Hamming) and a hand-worked clipped example -- its transfer function itself is a
 reading (A19), the paper prints no formula: "parity unpinned" for the ADC formula.  Unpinned: accuracy parity with the paper's ISOLET numbers (datasets absent) --

@@ -524,6 +524,7 @@ int do_similarity(hdc_ctx* h, const uint32_t* Hbits, int64_t N, int64_t ldh, con
       }
       ++h->stats[HDC_STAT_SIMT_FALLBACKS];
       h->err = "wide-integer similarity: tensor-core kernel refused the operands, dp4a kernel used";
+      prep = true;   // the dp4a kernel takes another operand form (byte planes): stage it here
     }
     // CUDA-core route: byte planes + dp4a contraction (widedot.cu)
     uint32_t* planes = pm.take<uint32_t>(wide_operand_bytes(K, k->hv_bits, D_eff) / sizeof(uint32_t));
