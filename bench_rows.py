@@ -235,17 +235,23 @@ def row_point(h, peaks, reps, cfg, N, prec_name):
 
 
 # ------------------------------------------------------------------------------------ similarity rows
-def row_classify(h, peaks, reps, N, K, D, hv_bits, sim_name, flags=0):
+def row_classify(h, peaks, reps, N, K, D, hv_bits, sim_name, flags=0, acc_scale=None):
+    """acc_scale: multiplies the bundle-shaped accumulators (|c| <= 32) -- 32- / 64-bit integer classes whose every
+    16-bit piece holds nonzero codes (without it only the lowest piece does and the others are skipped)."""
     sim = {"cos": hd.HDC_SIM_COS, "dot": hd.HDC_SIM_DOT, "hamming": hd.HDC_SIM_HAMMING}[sim_name]
     W = (D + 31) // 32
     H = _rand_bits(N, W, "rows_query_bits")
     C = _class_acc(K, D, "rows_class_acc")
+    if acc_scale is not None:
+        C = C * float(acc_scale)
     kn = hd.knobs(D, hv_bits=hv_bits, sim=sim, flags=flags)
     lab = torch.empty(N, dtype=torch.int32, device="cuda")
     fn = lambda: h.hdc_classify(H, C, kn, labels=lab)  # noqa: E731
     call_ms = _time(fn, reps)
     k_ms, _ = _kernel(h, hd.HDC_K_SIM, fn, reps)
-    out = {"what": f"hdc_classify N={N} K={K} D={D} hv_bits={hv_bits} sim={sim_name}", "call_ms": call_ms,
+    out = {"what": f"hdc_classify N={N} K={K} D={D} hv_bits={hv_bits} sim={sim_name}"
+                   + (f" accumulators x {acc_scale:g} (every 16-bit piece live)" if acc_scale is not None else ""),
+           "call_ms": call_ms,
            "kernel_ms": k_ms, "queries_per_s": N / (call_ms * 1e-3)}
     hbm = N * W * 4 / (k_ms * 1e-3) / 1e9
     out["hbm_GBps_query_bits"] = hbm
@@ -610,6 +616,8 @@ ROWS = {
     "c2_classify_cos_i16": lambda h, p, r: row_classify(h, p, r, 131072, 26, 10000, hd.HDC_HV_I16, "cos"),
     "c2_classify_cos_i32": lambda h, p, r: row_classify(h, p, r, 131072, 26, 10000, hd.HDC_HV_I32, "cos"),
     "c2_classify_dot_i64": lambda h, p, r: row_classify(h, p, r, 131072, 26, 10000, hd.HDC_HV_I64, "dot"),
+    "c2_classify_cos_i32_full": lambda h, p, r: row_classify(h, p, r, 131072, 26, 10000, hd.HDC_HV_I32, "cos", acc_scale=6.0e7),
+    "c2_classify_dot_i64_full": lambda h, p, r: row_classify(h, p, r, 131072, 26, 10000, hd.HDC_HV_I64, "dot", acc_scale=2.0 ** 44),
     "c2_classify_cos_i32_dp4a": lambda h, p, r: row_classify(h, p, r, 131072, 26, 10000, hd.HDC_HV_I32, "cos", hd.HDC_FLAG_SIMT),
     "c2_classify_dot_i64_dp4a": lambda h, p, r: row_classify(h, p, r, 131072, 26, 10000, hd.HDC_HV_I64, "dot", hd.HDC_FLAG_SIMT),
     "c5_classify_i32": lambda h, p, r: row_c5_classify(h, p, r, hd.HDC_HV_I32, "cos"),

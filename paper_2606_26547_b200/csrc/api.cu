@@ -135,8 +135,10 @@ int64_t wide_chunk_rows(int64_t N, int K) {
 void wide_tc_ws(int64_t N, int K, const hdc_knobs_t* k, Bump* pm, Bump* b) {
   if (!wide_int(k)) return;
   const int pieces = k->hv_bits == HDC_HV_I32 ? 2 : 4;
-  if (pm)
+  if (pm) {
     for (int j = 0; j < pieces; ++j) pm->take<uint8_t>(sim_tc_operand_bytes(K, HDC_HV_I16, k->D_eff));
+    pm->take<int>(4);   // live flags of the pieces
+  }
   if (b) b->take<int32_t>((size_t)pieces * (size_t)wide_chunk_rows(N, K) * (size_t)K);
 }
 Perf perf_of(const hdc_knobs_t* k) { return Perf{k->perf_begin, k->perf_stride <= 1 ? 1 : k->perf_stride}; }
@@ -479,18 +481,21 @@ int do_similarity(hdc_ctx* h, const uint32_t* Hbits, int64_t N, int64_t ldh, con
       const size_t cop_bytes = sim_tc_operand_bytes(K, HDC_HV_I16, D_eff);
       void* cop[4];
       for (int j = 0; j < pieces; ++j) cop[j] = pm.take<uint8_t>(cop_bytes);
+      // live[j] = piece j holds a nonzero code.  Accumulators as training leaves them are small integers whose upper
+      // pieces are all zero: their contractions return at once and the combine kernel skips them
+      int* live = pm.take<int>(4);
       const int64_t rows_max = wide_chunk_rows(N, K);
       int32_t* Sp = b.take<int32_t>((size_t)pieces * (size_t)rows_max * (size_t)K);
       if (!persistent_fits(h, b, ws_bytes)) return too_small();
       bool ok = true;
       if (prep) {
-        ce = launch_wide_prepare(C_acc, K, ldc, D_eff, k->hv_bits, pf, cos, nullptr, colscale, st, &h->launches);
+        ce = launch_wide_prepare(C_acc, K, ldc, D_eff, k->hv_bits, pf, cos, nullptr, colscale, st, &h->launches, live);
         if (ce != cudaSuccess) return cuda_fail(h, ce, "wide-integer cosine scales");
         Epilogue none{};
         none.kind = EPI_SCORE;
         for (int j = 0; j < pieces && ok; ++j) {
           ce = launch_sim_tc(h->tc, Hbits, 0, ldh, C_acc, K, ldc, D_eff, HDC_HV_I16, cop[j], nullptr, none, pf, nullptr,
-                             false, true, h->sm_count, tc_cta_group(k), st, &h->launches, j + 1, width);
+                             false, true, h->sm_count, tc_cta_group(k), st, &h->launches, j + 1, width, live + j);
           if (ce == cudaErrorNotSupported) ok = false;
           else if (ce != cudaSuccess) return cuda_fail(h, ce, "wide-integer class pieces");
         }
@@ -507,7 +512,8 @@ int do_similarity(hdc_ctx* h, const uint32_t* Hbits, int64_t N, int64_t ldh, con
             es.lds = K;
             es.s_i32 = 1;
             ce = launch_sim_tc(h->tc, Hbits + r0 * ldh, rows, ldh, C_acc, K, ldc, D_eff, HDC_HV_I16, cop[j], nullptr, es,
-                               pf, nullptr, true, false, h->sm_count, tc_cta_group(k), st, &h->launches, j + 1, width);
+                               pf, nullptr, true, false, h->sm_count, tc_cta_group(k), st, &h->launches, j + 1, width,
+                               live + j);
             if (ce == cudaErrorNotSupported && r0 == 0 && j == 0) ok = false;
             else if (ce != cudaSuccess) return cuda_fail(h, ce, "wide-integer similarity (tcgen05)");
           }
@@ -517,7 +523,7 @@ int do_similarity(hdc_ctx* h, const uint32_t* Hbits, int64_t N, int64_t ldh, con
           if (er.best) er.best += r0;
           if (er.second) er.second += r0;
           if (er.S) er.S = static_cast<char*>(er.S) + (size_t)r0 * (size_t)lds * (s_i32 == 2 ? 8 : 4);
-          ce = launch_wide_combine(Sp, pieces, rows, K, cos, colscale, er, st, &h->launches);
+          ce = launch_wide_combine(Sp, pieces, rows, K, cos, colscale, live, er, st, &h->launches);
           if (ce != cudaSuccess) return cuda_fail(h, ce, "wide-integer combine");
         }
         if (ok) return HDC_OK;

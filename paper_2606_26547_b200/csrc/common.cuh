@@ -113,9 +113,12 @@ size_t sim_tc_operand_bytes(int K, int hv_bits, int D_eff);
 cudaError_t launch_sim_tc(TcContext* tc, const uint32_t* Hbits, int64_t N, int64_t ldh, const float* C_acc,
                           int K, int64_t ldc, int D_eff, int hv_bits, void* cop, float* amax_scratch,
                           const Epilogue& e, Perf pf, double* partial, bool cop_ready, bool prep_only, int sm_count,
-                          int force_cg, cudaStream_t st, int64_t* nlaunch, int piece = 0, int width = 0);
+                          int force_cg, cudaStream_t st, int64_t* nlaunch, int piece = 0, int width = 0,
+                          int* live = nullptr);
 // piece > 0 (with hv_bits = HDC_HV_I16): the staged operand is the balanced base-65536 piece `piece - 1` of the
 // `width`-bit integer code rint(C_acc) (HDC_HV_I32 / HDC_HV_I64, reading A22) instead of the scaled int16 code
+// live (piece mode, nullable): one int, set to 1 by the preparation when the piece holds a nonzero code (the caller
+// zeroes it first: launch_wide_prepare); the contraction returns at once while it is 0
 // force_cg: 1 / 2 = one-CTA / CTA-pair kernel (knobs HDC_FLAG_TC_1CTA / _2CTA), else by problem size
 // cop_ready: cop already holds the staged class operand of the same (C_acc, knobs) -- skip its preparation
 // prep_only: stage the class operand into cop (and amax) and return without contracting
@@ -195,9 +198,11 @@ size_t wide_operand_bytes(int K, int hv_bits, int D_eff);
 // S_j [rows][K], j < pieces, piece j at Sp + j * rows * K) and recombined here as sum_j S_j << 16j in 64 bits
 // before the same epilogue (arg-max / fp32 / int64 scores); e's row pointers are those of the first row
 cudaError_t launch_wide_combine(const int32_t* Sp, int pieces, int64_t rows, int K, int cos, const double* colscale,
-                                const Epilogue& e, cudaStream_t st, int64_t* nlaunch);
+                                const int* live, const Epilogue& e, cudaStream_t st, int64_t* nlaunch);
+// live: `pieces` ints, piece j is read only where live[j] != 0 (its scores were not written otherwise)
 cudaError_t launch_wide_prepare(const float* C_acc, int K, int64_t ldc, int D_eff, int hv_bits, Perf pf, int cos,
-                                uint32_t* planes, double* colscale, cudaStream_t st, int64_t* nlaunch);
+                                uint32_t* planes, double* colscale, cudaStream_t st, int64_t* nlaunch,
+                                int* live = nullptr);   // live (nullable): four ints, zeroed here
 cudaError_t launch_wide_dot(const uint32_t* Hbits, int64_t N, int64_t ldh, int K, int D_eff, int hv_bits, int cos,
                             const uint32_t* planes, const double* colscale, const Epilogue& e, cudaStream_t st,
                             int64_t* nlaunch);

@@ -93,6 +93,8 @@ struct SimParams {
   int stage_bytes;  // A_BYTES + nparts*kc*KB_BYTES
   int f16;          // 16-bit operands are IEEE half instead of bf16 (hv code HDC_HV_F16)
   const int32_t* rowsum;   // INT8: sum of every staged class row (see the expanders), behind the staged operand
+  const int* live;         // nullable: *live == 0 -> the staged class operand is all zero and nobody reads the scores
+                           // (an all-zero 16-bit piece of 32- / 64-bit integer codes): the kernel returns at once
   int acc_cols, acc_bufs;  // sim_ts_kernel: TMEM columns of one accumulator and how many there are
   int ngroups;             // sim_ts_kernel: groups of 4 k-blocks in flight (class tiles in shared memory, expanded
                            // queries in tensor memory)
@@ -286,6 +288,7 @@ template <bool INT8, int EPI, int CG, bool TS = false>
 __global__ void __launch_bounds__(NTHREADS, 1)
 sim_tc_kernel(const __grid_constant__ CUtensorMap tmB, const SimParams p) {
   static_assert(!TS || CG == 1, "the tensor-memory A ring is a one-CTA layout");
+  if (p.live && *p.live == 0) return;   // (uniform over the grid: every CTA of a cluster leaves)
   constexpr uint32_t B_OFF = TS ? 0u : (uint32_t)A_BYTES;     // class tile within a ring stage
   constexpr int ACC_STRIDE = TS ? TS_ACC_COLS : BN_MAX;       // TMEM columns between the two accumulators
   extern __shared__ uint8_t smem_raw[];
@@ -648,7 +651,7 @@ __global__ void __launch_bounds__(CP_THREADS)
 class_prepare_kernel(const float* __restrict__ C, int K, int D_eff, int64_t ldc, int mode, int kc, int nparts,
                      int num_kb, const float* __restrict__ amax, Perf pf, int n_vis, void* __restrict__ dst,
                      int32_t* __restrict__ rowsum, double* __restrict__ colscale, float* __restrict__ colscale_f,
-                     int piece, int width) {
+                     int piece, int width, int* __restrict__ live) {
   constexpr int BK = INT8 ? 128 : 64;
   const int ld = num_kb * BK;
   const int k = blockIdx.x;                                   // class (rows k >= K are zero padding)
@@ -726,6 +729,9 @@ class_prepare_kernel(const float* __restrict__ C, int K, int D_eff, int64_t ldc,
       }
       nrm2f = __fmaf_rn(v, v, nrm2f);
     }
+  }
+  if (INT8 && live) {   // piece mode: does this piece hold any nonzero code?  (live[] zeroed by wide_prepare_kernel)
+    if (__syncthreads_or(nrm2i != 0ull) && threadIdx.x == 0) atomicOr(live, 1);
   }
   double nrm2 = INT8 ? (double)nrm2i : (double)nrm2f;   // (integers below 2^53: exact)
   __shared__ double sh_n[CP_THREADS / 32];
@@ -857,6 +863,7 @@ constexpr int TSQ_MAXG = 3;                        // groups in flight
 template <bool INT8, int EPI>
 __global__ void __launch_bounds__(TSQ_THREADS, 1)
 sim_ts_kernel(const __grid_constant__ CUtensorMap tmB, const __grid_constant__ CUtensorMap tmQ, const SimParams p) {
+  if (p.live && *p.live == 0) return;
   extern __shared__ uint8_t smem_raw[];
   constexpr int BK = INT8 ? 128 : 64;
   constexpr int WPK = INT8 ? 4 : 2;          // packed words per k-block
@@ -1231,7 +1238,7 @@ size_t sim_tc_partial_bytes(int64_t N, int K, int hv_bits, int D_eff, int sm_cou
 cudaError_t launch_sim_tc(TcContext* tc, const uint32_t* Hbits, int64_t N, int64_t ldh, const float* C_acc,
                           int K, int64_t ldc, int D_eff, int hv_bits, void* cop, float* amax_scratch,
                           const Epilogue& e, Perf pf, double* partial, bool cop_ready, bool prep_only, int sm_count,
-                          int force_cg, cudaStream_t st, int64_t* nlaunch, int piece, int width) {
+                          int force_cg, cudaStream_t st, int64_t* nlaunch, int piece, int width, int* live) {
   if (!tc) return cudaErrorNotSupported;
   if (N <= 0 && !prep_only) return cudaSuccess;
   if ((reinterpret_cast<uintptr_t>(cop) & 15) != 0) return cudaErrorNotSupported;
@@ -1254,11 +1261,11 @@ cudaError_t launch_sim_tc(TcContext* tc, const uint32_t* Hbits, int64_t N, int64
     float* csf = const_cast<float*>(e.colscale_f);
     if (int8)
       class_prepare_kernel<true><<<(unsigned)(n_tiles * kc), CP_THREADS, 0, st>>>(C_acc, K, D_eff, ldc, hv_bits, kc, nparts, num_kb,
-                                                                          amax_scratch, pf, n_vis, cop, rowsum, cs, csf, piece, width);
+                                                                          amax_scratch, pf, n_vis, cop, rowsum, cs, csf, piece, width, live);
     else
       class_prepare_kernel<false><<<(unsigned)(n_tiles * kc), CP_THREADS, 0, st>>>(C_acc, K, D_eff, ldc, hv_bits, kc, nparts,
                                                                            num_kb, amax_scratch, pf, n_vis, cop, nullptr, cs,
-                                                                           csf, 0, 0);
+                                                                           csf, 0, 0, nullptr);
     ++*nlaunch;
     ce = cudaGetLastError();
     if (ce != cudaSuccess) return ce;
@@ -1294,6 +1301,7 @@ cudaError_t launch_sim_tc(TcContext* tc, const uint32_t* Hbits, int64_t N, int64
   p.num_kb = num_kb;
   p.f16 = hv_bits == HDC_HV_F16;
   p.rowsum = rowsum;
+  p.live = live;
   p.stage_bytes = (ts ? 0 : A_BYTES) + nparts * kc / cg * KB_BYTES;
   p.stages = (SMEM_LIMIT - SMEM_EXTRA - qring_bytes(cg)) / p.stage_bytes;
   if (p.stages > MAX_STAGES) p.stages = MAX_STAGES;

@@ -47,8 +47,10 @@ __device__ __forceinline__ int dp4a_us(uint32_t a, uint32_t b, int c) {   // uns
 // 1 / (sqrt(n_vis) * |q|) (0 for a zero row; 1 for DOT), norm summed in double in a fixed order.
 __global__ void wide_prepare_kernel(const float* __restrict__ C, int D_eff, int64_t ldc, Perf pf, int P,
                                     uint32_t* __restrict__ planes, int quads_ld, int cos, int n_vis,
-                                    double* __restrict__ colscale, long long* __restrict__ rowsum) {
+                                    double* __restrict__ colscale, long long* __restrict__ rowsum,
+                                    int* __restrict__ live) {
   const int k = blockIdx.x;
+  if (live && k == 0 && threadIdx.x < 4) live[threadIdx.x] = 0;   // the pieces' preparation (next launches) sets them
   const long long lim = P == 4 ? 2147483647LL : 9223372036854775807LL;
   __shared__ double part[32];
   __shared__ unsigned long long part_s[32];
@@ -276,8 +278,11 @@ __device__ __forceinline__ long long wide_max(int cos, long long a, long long b)
 
 constexpr int WC_WARPS = 8;
 __global__ void __launch_bounds__(WC_WARPS * 32)
-wide_combine_kernel(const int32_t* __restrict__ Sp, int pieces, int64_t rows, int K, WideOut o) {
+wide_combine_kernel(const int32_t* __restrict__ Sp, int pieces, int64_t rows, int K, const int* __restrict__ live,
+                    WideOut o) {
   const int lane = threadIdx.x & 31;
+  int on = 0;   // pieces that hold a nonzero code (the others' scores are zero and were never written)
+  for (int j = 0; j < pieces; ++j) on |= (__ldg(live + j) != 0) << j;
   const int64_t warp0 = (int64_t)blockIdx.x * WC_WARPS + (threadIdx.x >> 5);
   for (int64_t n = warp0; n < rows; n += (int64_t)gridDim.x * WC_WARPS) {
     WideTop2 top = wide_top2_init(o);
@@ -285,7 +290,7 @@ wide_combine_kernel(const int32_t* __restrict__ Sp, int pieces, int64_t rows, in
     for (int k = lane; k < K; k += 32) {
       unsigned long long s = 0;
       for (int j = 0; j < pieces; ++j)
-        s += (unsigned long long)(long long)__ldg(Sp + ((int64_t)j * rows + n) * K + k) << (16 * j);
+        if (on >> j & 1) s += (unsigned long long)(long long)__ldg(Sp + ((int64_t)j * rows + n) * K + k) << (16 * j);
       wide_push(o, top, n, k, (long long)s);
     }
     if (!o.labels) continue;
@@ -310,14 +315,17 @@ wide_combine_kernel(const int32_t* __restrict__ Sp, int pieces, int64_t rows, in
 
 // Few classes: one thread per query row (a warp per row leaves lanes idle and pays the butterfly per row; measured
 // at K = 26: 24 us against 58 us per 131072 rows; at K = 1000 the strided reads of this form cost 0.5 ms per pass).
-__global__ void wide_combine_rows_kernel(const int32_t* __restrict__ Sp, int pieces, int64_t rows, int K, WideOut o) {
+__global__ void wide_combine_rows_kernel(const int32_t* __restrict__ Sp, int pieces, int64_t rows, int K,
+                                         const int* __restrict__ live, WideOut o) {
   const int64_t n = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (n >= rows) return;
+  int on = 0;
+  for (int j = 0; j < pieces; ++j) on |= (__ldg(live + j) != 0) << j;
   WideTop2 top = wide_top2_init(o);
   for (int k = 0; k < K; ++k) {
     unsigned long long s = 0;
     for (int j = 0; j < pieces; ++j)
-      s += (unsigned long long)(long long)__ldg(Sp + ((int64_t)j * rows + n) * K + k) << (16 * j);
+      if (on >> j & 1) s += (unsigned long long)(long long)__ldg(Sp + ((int64_t)j * rows + n) * K + k) << (16 * j);
     wide_push(o, top, n, k, (long long)s);
   }
   wide_finish(o, top, n, K);
@@ -354,27 +362,27 @@ static WideOut wide_out(const Epilogue& e, int cos, const double* colscale) {
 }
 
 cudaError_t launch_wide_combine(const int32_t* Sp, int pieces, int64_t rows, int K, int cos, const double* colscale,
-                                const Epilogue& e, cudaStream_t st, int64_t* nlaunch) {
+                                const int* live, const Epilogue& e, cudaStream_t st, int64_t* nlaunch) {
   if (rows <= 0) return cudaSuccess;
   if (K < 64) {
-    wide_combine_rows_kernel<<<(unsigned)((rows + 127) / 128), 128, 0, st>>>(Sp, pieces, rows, K, wide_out(e, cos, colscale));
+    wide_combine_rows_kernel<<<(unsigned)((rows + 127) / 128), 128, 0, st>>>(Sp, pieces, rows, K, live, wide_out(e, cos, colscale));
     *nlaunch += 1;
     return cudaGetLastError();
   }
   int64_t grid = (rows + WC_WARPS - 1) / WC_WARPS;
   if (grid > 148 * 16) grid = 148 * 16;
-  wide_combine_kernel<<<(unsigned)grid, WC_WARPS * 32, 0, st>>>(Sp, pieces, rows, K, wide_out(e, cos, colscale));
+  wide_combine_kernel<<<(unsigned)grid, WC_WARPS * 32, 0, st>>>(Sp, pieces, rows, K, live, wide_out(e, cos, colscale));
   *nlaunch += 1;
   return cudaGetLastError();
 }
 
 cudaError_t launch_wide_prepare(const float* C_acc, int K, int64_t ldc, int D_eff, int hv_bits, Perf pf, int cos,
-                                uint32_t* planes, double* colscale, cudaStream_t st, int64_t* nlaunch) {
+                                uint32_t* planes, double* colscale, cudaStream_t st, int64_t* nlaunch, int* live) {
   const int P = wide_planes(hv_bits);
   if (!P) return cudaErrorInvalidValue;
   wide_prepare_kernel<<<K, 256, 0, st>>>(C_acc, D_eff, ldc, pf, P, planes, wide_quads_ld(D_eff), cos,
                                          perf_count(pf, D_eff), colscale,
-                                         planes ? wide_rowsum(planes, K, hv_bits, D_eff) : nullptr);
+                                         planes ? wide_rowsum(planes, K, hv_bits, D_eff) : nullptr, live);
   *nlaunch += 1;
   return cudaGetLastError();
 }

@@ -136,6 +136,36 @@ def test_wide_integer_row_passes_of_the_tensor_core_route(hd, h, width):
     assert np.array_equal(h.hdc_classify(Hd, Cd, knc).cpu().numpy(), O.classify(Sc_or, O.SIM_COS)[0])
 
 
+@pytest.mark.parametrize("width", ["I32", "I64"])
+def test_wide_integer_all_zero_pieces_are_skipped_exactly(hd, h, width):
+    """The tensor-core route does not contract a 16-bit piece of the codes that is zero everywhere (small accumulators:
+    the upper pieces) and the recombination skips its never-written scores: alternating models with and without live
+    upper pieces on one handle (same workspace, stale piece scores in it) must each give the oracle's integers."""
+    code, ocode, mag = HV[width]
+    N, K, D = 700, 26, 1500
+    r = np.random.default_rng([74, code])
+    hb = r.integers(0, 2, size=(N, D), dtype=np.uint8)
+    Hd = dev_bits(hb)
+    models = [(r.standard_normal((K, D)) * mag).astype(np.float32),                    # every piece live
+              r.integers(-40, 41, size=(K, D)).astype(np.float32),                     # piece 0 only
+              np.zeros((K, D), dtype=np.float32),                                      # no piece at all
+              (r.integers(-3, 4, size=(K, D)) * 65536.0).astype(np.float32),           # piece 1 only
+              (r.standard_normal((K, D)) * mag).astype(np.float32)]
+    kn = hd.knobs(D, hv_bits=code, sim=hd.HDC_SIM_DOT)
+    knc = hd.knobs(D, hv_bits=code, sim=hd.HDC_SIM_COS)
+    for C in models:
+        Cd = dev(C)
+        S_or = O.similarity(hb, C, D, O.SIM_DOT, ocode)
+        assert np.array_equal(h.hdc_similarity(Hd, Cd, kn, s_dtype=torch.int64).cpu().numpy(), S_or)
+        lab, best, sec = h.hdc_classify(Hd, Cd, kn, want_scores=True)
+        lab_or, best_or, sec_or = O.classify(S_or, O.SIM_DOT)
+        assert np.array_equal(lab.cpu().numpy(), lab_or)
+        assert np.array_equal(best.cpu().numpy(), best_or.astype(np.float32))
+        assert np.array_equal(sec.cpu().numpy(), sec_or.astype(np.float32))
+        Sc_or = O.similarity(hb, C, D, O.SIM_COS, ocode)
+        assert np.allclose(h.hdc_similarity(Hd, Cd, knc).cpu().numpy(), Sc_or, rtol=1e-6, atol=1e-12)
+
+
 def test_wide_integer_argument_errors(hd, h):
     hb = np.zeros((4, 64), dtype=np.uint8)
     C = np.ones((2, 64), dtype=np.float32)
