@@ -242,7 +242,10 @@ def row_classify(h, peaks, reps, N, K, D, hv_bits, sim_name, flags=0, acc_scale=
     W = (D + 31) // 32
     H = _rand_bits(N, W, "rows_query_bits")
     C = _class_acc(K, D, "rows_class_acc")
-    if acc_scale is not None:
+    if isinstance(acc_scale, (list, tuple)):   # one scale per class, cycling (an fp32 value spans at most 24 bits)
+        sc = torch.tensor([float(acc_scale[k % len(acc_scale)]) for k in range(K)], device=C.device)
+        C = C * sc[:, None]
+    elif acc_scale is not None:
         C = C * float(acc_scale)
     kn = hd.knobs(D, hv_bits=hv_bits, sim=sim, flags=flags)
     lab = torch.empty(N, dtype=torch.int32, device="cuda")
@@ -250,7 +253,7 @@ def row_classify(h, peaks, reps, N, K, D, hv_bits, sim_name, flags=0, acc_scale=
     call_ms = _time(fn, reps)
     k_ms, _ = _kernel(h, hd.HDC_K_SIM, fn, reps)
     out = {"what": f"hdc_classify N={N} K={K} D={D} hv_bits={hv_bits} sim={sim_name}"
-                   + (f" accumulators x {acc_scale:g} (every 16-bit piece live)" if acc_scale is not None else ""),
+                   + (f" accumulators x {acc_scale} (every 16-bit piece live)" if acc_scale is not None else ""),
            "call_ms": call_ms,
            "kernel_ms": k_ms, "queries_per_s": N / (call_ms * 1e-3)}
     hbm = N * W * 4 / (k_ms * 1e-3) / 1e9
@@ -617,7 +620,8 @@ ROWS = {
     "c2_classify_cos_i32": lambda h, p, r: row_classify(h, p, r, 131072, 26, 10000, hd.HDC_HV_I32, "cos"),
     "c2_classify_dot_i64": lambda h, p, r: row_classify(h, p, r, 131072, 26, 10000, hd.HDC_HV_I64, "dot"),
     "c2_classify_cos_i32_full": lambda h, p, r: row_classify(h, p, r, 131072, 26, 10000, hd.HDC_HV_I32, "cos", acc_scale=6.0e7),
-    "c2_classify_dot_i64_full": lambda h, p, r: row_classify(h, p, r, 131072, 26, 10000, hd.HDC_HV_I64, "dot", acc_scale=2.0 ** 44),
+    "c2_classify_dot_i64_full": lambda h, p, r: row_classify(h, p, r, 131072, 26, 10000, hd.HDC_HV_I64, "dot",
+                                                                 acc_scale=(1.0, 2.0 ** 16, 2.0 ** 32, 2.0 ** 44)),
     "c2_classify_cos_i32_dp4a": lambda h, p, r: row_classify(h, p, r, 131072, 26, 10000, hd.HDC_HV_I32, "cos", hd.HDC_FLAG_SIMT),
     "c2_classify_dot_i64_dp4a": lambda h, p, r: row_classify(h, p, r, 131072, 26, 10000, hd.HDC_HV_I64, "dot", hd.HDC_FLAG_SIMT),
     "c5_classify_i32": lambda h, p, r: row_c5_classify(h, p, r, hd.HDC_HV_I32, "cos"),

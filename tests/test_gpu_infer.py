@@ -58,7 +58,7 @@ def _check_stage2(hd, lab, best, second, bits, C, D_eff, sim_name, hv_bits, begi
     sim = SIMS[sim_name]
     S_or = O.similarity(bits, C, D_eff, sim, hv_bits, begin, stride)
     lab_or, b_or, s_or = O.classify(S_or, sim)
-    if hv_bits in (18, 8, 1):
+    if hv_bits in (20, 19, 18, 8, 1):
         assert np.array_equal(lab, lab_or)
         assert np.allclose(best, b_or, rtol=1e-6, atol=1e-6) and np.allclose(second, s_or, rtol=1e-6, atol=1e-6)
     else:
@@ -145,7 +145,8 @@ def test_infer_rp_fused_perforated_similarity(hd, h, sim_name, hv_bits, begin, s
 
 @pytest.mark.parametrize("N,K,flags,hv_bits", [(12288, 26, 0, 8), (12288, 33, 16, 8), (500, 26, 16, 8),
                                                (12288, 26, 16 | 1, 8), (12288, 26, 16 | 2, 8), (0, 26, 16, 8),
-                                               (12288, 26, 16, 18), (700, 26, 0, 18)])
+                                               (12288, 26, 16, 18), (700, 26, 0, 18),
+                                               (12288, 26, 16, 19), (700, 26, 0, 20)])   # 19 / 20 = HDC_HV_I32 / _I64
 def test_infer_rp_two_kernel_path_and_stats(hd, h, N, K, flags, hv_bits):
     """The default (no HDC_FLAG_FUSED_INFER = 16), and with the flag: large K, small N, HDC_FLAG_SIMT,
     HDC_FLAG_TC_1CTA and int16 class codes (hv code 18: sums beyond what the fused fp32 search holds exactly),

@@ -166,6 +166,25 @@ def test_wide_integer_all_zero_pieces_are_skipped_exactly(hd, h, width):
         assert np.allclose(h.hdc_similarity(Hd, Cd, knc).cpu().numpy(), Sc_or, rtol=1e-6, atol=1e-12)
 
 
+@pytest.mark.parametrize("width", ["I32", "I64"])
+def test_wide_integer_classes_through_the_host_pipeline(hd, h, width):
+    """hdc_infer_rp_host (chunks of 2048, 3072, ... rows; the first one prepares the class pieces, the later ones reuse
+    them) and hdc_infer_rp on the same inputs: labels identical, and equal to the oracle's on exact-arithmetic inputs."""
+    code, ocode, mag = HV[width]
+    N, F, D, K = 30000, 48, 640, 11
+    r = np.random.default_rng([75, code])
+    X = r.integers(0, 256, size=(N, F)).astype(np.float32)
+    P = (1.0 - 2.0 * r.integers(0, 2, size=(D, F))).astype(np.float32)
+    C = (r.standard_normal((K, D)) * mag).astype(np.float32)
+    kn = hd.knobs(D, precision=hd.HDC_BF16, hv_bits=code, sim=hd.HDC_SIM_DOT)
+    Pd, Cd = dev(P), dev(C)
+    lab = h.hdc_infer_rp(dev(X), Pd, Cd, kn).cpu().numpy()
+    lab_host = h.hdc_infer_rp_host(torch.from_numpy(X).pin_memory(), Pd, Cd, kn).numpy()
+    assert np.array_equal(lab_host, lab)
+    bits = O.encode_rp(X, P, D, O.BF16)[0]
+    assert np.array_equal(lab, O.classify(O.similarity(bits, C, D, O.SIM_DOT, ocode), O.SIM_DOT)[0])
+
+
 def test_wide_integer_argument_errors(hd, h):
     hb = np.zeros((4, 64), dtype=np.uint8)
     C = np.ones((2, 64), dtype=np.float32)
