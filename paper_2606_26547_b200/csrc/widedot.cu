@@ -287,11 +287,31 @@ wide_combine_kernel(const int32_t* __restrict__ Sp, int pieces, int64_t rows, in
   for (int64_t n = warp0; n < rows; n += (int64_t)gridDim.x * WC_WARPS) {
     WideTop2 top = wide_top2_init(o);
     top.lab = INT_MAX;   // lanes without a class never win a tie
-    for (int k = lane; k < K; k += 32) {
-      unsigned long long s = 0;
-      for (int j = 0; j < pieces; ++j)
-        if (on >> j & 1) s += (unsigned long long)(long long)__ldg(Sp + ((int64_t)j * rows + n) * K + k) << (16 * j);
-      wide_push(o, top, n, k, (long long)s);
+    if ((K & 3) == 0) {
+      // four classes per lane and load: a row is a chain of load latencies, 16-byte loads put 4x the bytes in flight
+      // (rows of K int32 are 16-byte aligned when K is a multiple of 4)
+      for (int k = 4 * lane; k < K; k += 128) {
+        unsigned long long s0 = 0, s1 = 0, s2 = 0, s3 = 0;
+        for (int j = 0; j < pieces; ++j) {
+          if (!(on >> j & 1)) continue;
+          const int4 v = __ldg(reinterpret_cast<const int4*>(Sp + ((int64_t)j * rows + n) * K + k));
+          s0 += (unsigned long long)(long long)v.x << (16 * j);
+          s1 += (unsigned long long)(long long)v.y << (16 * j);
+          s2 += (unsigned long long)(long long)v.z << (16 * j);
+          s3 += (unsigned long long)(long long)v.w << (16 * j);
+        }
+        wide_push(o, top, n, k, (long long)s0);
+        wide_push(o, top, n, k + 1, (long long)s1);
+        wide_push(o, top, n, k + 2, (long long)s2);
+        wide_push(o, top, n, k + 3, (long long)s3);
+      }
+    } else {
+      for (int k = lane; k < K; k += 32) {
+        unsigned long long s = 0;
+        for (int j = 0; j < pieces; ++j)
+          if (on >> j & 1) s += (unsigned long long)(long long)__ldg(Sp + ((int64_t)j * rows + n) * K + k) << (16 * j);
+        wide_push(o, top, n, k, (long long)s);
+      }
     }
     if (!o.labels) continue;
 #pragma unroll
