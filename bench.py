@@ -511,6 +511,13 @@ def rows_cpu_baseline(w):
     _, dt = timed(lambda: O.train_epoch(btr, w["ytr"][:n_tr], C, w["D"], 32, O.SIM_COS, w["lr"], 0))
     out["c2_train_epoch"] = {"value": n_tr / dt, "unit": "samples/s", "cores": cores, "kind": "oracle",
                              "sample": f"one retraining epoch (B=N) over the {n_tr} C2 training samples (pre-encoded), {dt:.2f} s"}
+    # classify against the class accumulators held as 32-bit integers (exact 64-bit sums), C2 shape
+    nq = 2048
+    _, dt = timed(lambda: O.infer(btr[:nq], C, w["D"], O.SIM_COS, O.HV_I32))
+    out["c2_classify_cos_i32"] = {"value": nq / dt, "unit": "queries/s", "cores": cores, "kind": "oracle",
+                                  "sample": f"{nq} encoded C2 queries against K={w['K']} classes as 32-bit integers "
+                                            f"(cosine + argmax), {dt:.2f} s; the integer sums are numpy loops over "
+                                            "the classes: one core"}
     # level-ID encode, C3
     c3 = gen.c3_mnist_shaped(n_tr=16, n_te=256)
     hb3, dt = timed(lambda: O.encode_levelid(c3["Lte"], c3["ID"], c3["LV"], c3["D"]))
