@@ -421,7 +421,8 @@ def run_gpu(args):
     # ---- end to end through the host entry point (pinned host buffers, H2D + D2H inside)
     Xh = torch.from_numpy(Xq).pin_memory()
     Lh = torch.empty(NQ, dtype=torch.int32).pin_memory()
-    h.hdc_infer_rp_host(Xh, Pd, C, kn, labels_host=Lh)
+    for _ in range(max(3, args.warmup)):      # the same number of warm-up steps as the device-resident loop
+        h.hdc_infer_rp_host(Xh, Pd, C, kn, labels_host=Lh)
     torch.cuda.synchronize()
     if world > 1:
         dist.barrier()
